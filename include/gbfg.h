@@ -1,0 +1,199 @@
+/* gbfg.h — C ABI of libgbfg, the B200 (sm_100a) galactic-binary foreground simulator.
+ *
+ * What the library computes: catalog of galactic binaries (A, f, fdot per source) ->
+ * confusion-noise power spectral density S_n(f) by the iterative subtraction algorithm of
+ * arxiv 2602.18560, Appendix D (steps 1-10 at :521-530), in the power-domain
+ * form of BASELINE.json:configs[0].  DESIGN.md §3 (R0-R6) states every reading of the paper that
+ * the arithmetic below follows; DESIGN.md §4 specifies the elementary functions of stage (i).
+ *
+ * Conventions
+ *  - "dev" pointers are DEVICE pointers owned by the caller (e.g. torch tensors); "host" pointers
+ *    are ordinary host memory.  The library never frees or retains a caller pointer past the
+ *    call, except that asynchronous calls use them until the work queued on `stream` has run.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *  - Catalogs are structure-of-arrays binary64: A[N], f[N], fdot[N].  A batch of n_cat catalogs is
+ *    the concatenation of its catalogs; `offsets` (HOST, n_cat+1 entries, offsets[0] = 0) gives the
+ *    first source of each.  Per-bin arrays of a batch are [n_cat][n_bins], row-major.
+ *  - The spectrum is int64 fixed point: one unit = 2^scale_log2 strain^2 (configs: -140).
+ *  - Every function returns GBFG_OK (0) or a negative gbfg_status.  Nothing throws, aborts or
+ *    prints.  The four stage calls and the helpers are asynchronous on `stream`;
+ *    gbfg_subtract_until_converged and gbfg_simulate* synchronise `stream` (one 8-byte scalar per
+ *    iteration) and fill HOST results.
+ *  - The library runs on compute capability 10.x devices only (GBFG_ERR_ARCH otherwise).  There is
+ *    no CPU fallback and no other backend.
+ */
+#ifndef GBFG_H
+#define GBFG_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum gbfg_status {
+    GBFG_OK = 0,
+    GBFG_ERR_INVALID_ARG = -1, /* null pointer, even / non-positive window, n_bins < h+1, f_min >= f_max, bad struct_size, n_cat out of range */
+    GBFG_ERR_WORKSPACE = -2,   /* workspace NULL or smaller than gbfg_workspace_bytes() */
+    GBFG_ERR_CUDA = -3,        /* a CUDA runtime call failed: see gbfg_last_cuda_error() */
+    GBFG_ERR_ARCH = -4,        /* current device is not compute capability 10.x */
+    GBFG_ERR_UNSUPPORTED = -5  /* window wider than GBFG_MAX_WINDOW, or n_cat > GBFG_MAX_CAT */
+} gbfg_status;
+
+#define GBFG_MAX_CAT 256        /* catalogs per batched call */
+#define GBFG_MAX_WINDOW 4097    /* widest running-median window of this build (odd) */
+#define GBFG_MAX_ITER_TRACE 64  /* per-iteration counts kept in gbfg_iter_result */
+
+/* Frequency grid: bins of width 1/t_obs covering [f_min, f_max); bin k = [f_min + k/T, f_min + (k+1)/T).
+ * n_bins = ceil((f_max - f_min) * t_obs)  (R2).  Fill with gbfg_grid_init. */
+typedef struct gbfg_grid {
+    uint32_t struct_size;   /* = sizeof(gbfg_grid) */
+    int32_t scale_log2;     /* spectrum unit = 2^scale_log2 */
+    double f_min, f_max;    /* Hz */
+    double t_obs;           /* s */
+    int64_t n_bins;
+} gbfg_grid;
+
+/* Population parameters Lambda of BASELINE.json's generator (configs[0], configs[4]):
+ *   p(f) ∝ f^-slope on [f_min, f_max);  log10 A ~ N(logA_offset + (2/3) log10(f / 1 mHz), logA_sigma);
+ *   fdot = (96/5) pi^(8/3) (G Mc / c^3)^(5/3) f^(11/3)  (eq. 4),
+ *   log10(Mc / Msun) ~ N(logMc_mean, logMc_sigma). */
+typedef struct gbfg_pop {
+    uint32_t struct_size;   /* = sizeof(gbfg_pop) */
+    uint32_t reserved;
+    double slope, logA_offset, logA_sigma, logMc_mean, logMc_sigma;
+    int64_t n_src;
+} gbfg_pop;
+
+/* Parameters of the subtraction loop (R3, R4, R6). */
+typedef struct gbfg_iter_params {
+    uint32_t struct_size;   /* = sizeof(gbfg_iter_params) */
+    int32_t window;         /* odd running-median window W = 2h+1 (paper: ~2000) */
+    double median_norm;     /* C of eq. (D3); paper value exactly 729/512 */
+    double rho_th;          /* SNR threshold, 7 in the paper */
+    int32_t max_iter;       /* iteration cap (BASELINE: 30) */
+    uint32_t flags;         /* GBFG_FLAG_* */
+} gbfg_iter_params;
+
+#define GBFG_FLAG_NO_PRESELECT 1u   /* test every unresolved source every iteration (no R5 candidate cut) */
+#define GBFG_FLAG_NO_INCREMENTAL 2u /* recompute every median tile every iteration (no dirty-tile skipping) */
+
+/* Per-catalog outcome of the loop (HOST). */
+typedef struct gbfg_iter_result {
+    int32_t n_iter;             /* iterations run; = max_iter when the cap was hit */
+    int32_t converged;          /* 1: an iteration resolved no new source; 0: cap hit */
+    int64_t n_resolved;         /* sources resolved by this call */
+    int64_t n_near_threshold;   /* tests with |rho^2 / rho_th^2 - 1| <= 2e-9, summed over iterations */
+    int64_t n_candidates;       /* sources that passed the pre-selection (= tested sources if disabled) */
+    int64_t n_new_per_iter[GBFG_MAX_ITER_TRACE];
+} gbfg_iter_result;
+
+int gbfg_version(void);                    /* 10000*major + 100*minor + patch */
+const char *gbfg_strerror(int status);     /* static string */
+const char *gbfg_last_cuda_error(void);    /* thread-local; text of the CUDA error behind the last GBFG_ERR_CUDA */
+
+/* Fills *out, computing n_bins = ceil((f_max - f_min) * t_obs).  INVALID_ARG unless
+ * 0 < f_min < f_max, t_obs > 0 and 1 <= n_bins < 2^31. */
+int gbfg_grid_init(double f_min, double f_max, double t_obs, int32_t scale_log2, gbfg_grid *out);
+
+/* Helper: Robson, Cornish & Liu 2019 sky-averaged LISA noise (paper ref [70]) with
+ * BASELINE.json:configs[0]'s constants, evaluated at bin centres f_min + (k + 1/2)/T (R3).
+ * dev_s_instr: [n_bins] binary64, written. */
+int gbfg_instrument_noise(const gbfg_grid *grid, double *dev_s_instr, void *stream);
+
+/* Stage (i) — step 1 of the algorithm: draw every catalog of the batch from its
+ * population with Philox4x32-10 (R1, §4).  pops: HOST [n_cat]; offsets: HOST [n_cat+1]
+ * with offsets[c+1]-offsets[c] = pops[c].n_src.  Catalog c uses Philox counter word 3 =
+ * first_cat_id + c, so a batch can be drawn in pieces.  dev_A / dev_f / dev_fdot: [offsets[n_cat]],
+ * written (16-byte aligned). */
+int gbfg_sample_catalog(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets,
+                        int32_t n_cat, uint32_t first_cat_id, uint64_t seed,
+                        double *dev_A, double *dev_f, double *dev_fdot, void *stream);
+
+/* Stage (ii)/(v) — deposit (sign = +1) or subtract (sign = -1) source power (R2;
+ * subtraction is eq. (D4)): for every addressed source
+ *     spectrum[c][k] += sign * q_i   for k in [k0_i, k0_i + w_eff_i).
+ * dev_sel_idx == NULL: all sources.  Otherwise dev_sel_idx holds GLOBAL source indices and
+ * dev_sel_count points to one int64 on the device = number of entries (read on the device).
+ * dev_spectrum: [n_cat][n_bins] int64, accumulated into (zero it first for a fresh deposit).
+ * dev_err_count: one int64, incremented by the number of rejected sources (NaN, A<0, fdot<0, f
+ * outside the band: DOMAIN; width or quantised power beyond 2^62: RANGE); may be NULL.
+ * workspace: >= gbfg_workspace_bytes(...); holds the difference array of the range-update form. */
+int gbfg_deposit(const gbfg_grid *grid, const double *dev_A, const double *dev_f, const double *dev_fdot,
+                 const int64_t *offsets, int32_t n_cat,
+                 const int64_t *dev_sel_idx, const int64_t *dev_sel_count, int32_t sign,
+                 int64_t *dev_spectrum, int64_t *dev_err_count,
+                 void *workspace, size_t workspace_bytes, void *stream);
+
+/* Stage (iii) — exact running median of eq. (D2), PAPER.md:542 (R3): for each row,
+ * median_out[k] = the h-th smallest of x[k-h .. k+h], W = 2h+1 odd, ends reflected
+ * (x[-j] = x[j-1], x[n-1+j] = x[n-j]).  Requires n_bins >= h+1 and W <= GBFG_MAX_WINDOW.
+ * dev_spectrum, dev_median_out: [n_cat][n_bins] int64 (must not alias). */
+int gbfg_running_median(const int64_t *dev_spectrum, int64_t n_bins, int32_t n_cat, int32_t window,
+                        int64_t *dev_median_out, void *stream);
+
+/* psd[c][k] = s_instr[k] + median_norm * (median[c][k] * 2^scale_log2): eqs. (10), (D2), (D3)
+ * (PAPER.md:142-145, 542-549).  dev_s_instr: [n_bins], shared by the batch. */
+int gbfg_psd(const int64_t *dev_median, const double *dev_s_instr, int64_t n_bins, int32_t n_cat,
+             double median_norm, int32_t scale_log2, double *dev_psd, void *stream);
+
+/* Stage (iv) — SNR of every unresolved source against the current PSD and selection
+ * (eqs. 11-12; R4): rho2_i = sum_{k in bins(i)} 4 p_i / psd[c][k];
+ * newly resolved iff rho2_i > rho_th^2 (strict).  For those, dev_resolved[i] is set to 1 and i is
+ * appended to dev_sel_idx (set semantics: order unspecified).
+ *  dev_resolved:  [N] uint8 in/out; sources with a non-zero flag are not tested.
+ *  dev_rho2_out:  [N] or NULL; rho2 of every tested source (NaN for rejected sources); untested
+ *                 entries are left untouched.
+ *  dev_sel_idx:   [N] capacity, written.   dev_sel_count: [1 + n_cat] int64, written: total, then
+ *                 the number selected in each catalog.
+ *  dev_near_count: one int64 or NULL, incremented by the number of tests within 1e-9 (relative, in
+ *                 rho) of the threshold. */
+int gbfg_snr_select(const gbfg_grid *grid, const double *dev_A, const double *dev_f, const double *dev_fdot,
+                    const int64_t *offsets, int32_t n_cat, const double *dev_psd, double rho_th,
+                    uint8_t *dev_resolved, double *dev_rho2_out,
+                    int64_t *dev_sel_idx, int64_t *dev_sel_count, int64_t *dev_near_count,
+                    void *workspace, size_t workspace_bytes, void *stream);
+
+/* Stage (v) — the loop, steps 4-10 (R6), device resident with one
+ * 8-byte scalar read back per iteration.  Catalogs of a batch iterate independently; a catalog
+ * that resolved nothing is frozen.
+ *  dev_spectrum: [n_cat][n_bins] in: total deposited spectrum, out: residual.
+ *  dev_median, dev_psd: [n_cat][n_bins] out, always those of the returned residual.
+ *  dev_resolved: [N] uint8 in/out (zero it for a fresh run).
+ *  host_results: HOST [n_cat]. */
+int gbfg_subtract_until_converged(const gbfg_grid *grid, const double *dev_A, const double *dev_f,
+                                  const double *dev_fdot, const int64_t *offsets, int32_t n_cat,
+                                  const double *dev_s_instr, const gbfg_iter_params *params,
+                                  int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
+                                  uint8_t *dev_resolved, gbfg_iter_result *host_results,
+                                  void *workspace, size_t workspace_bytes, void *stream);
+
+/* The whole hot path on device buffers: sample (i) -> deposit (ii) -> loop (iii)-(v).
+ * Outputs as above plus the catalog itself and the total spectrum (dev_total may be NULL).
+ * dev_err_count: one int64 or NULL. */
+int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
+                  uint64_t seed, const double *dev_s_instr, const gbfg_iter_params *params,
+                  double *dev_A, double *dev_f, double *dev_fdot,
+                  int64_t *dev_total, int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
+                  uint8_t *dev_resolved, int64_t *dev_err_count, gbfg_iter_result *host_results,
+                  void *workspace, size_t workspace_bytes, void *stream);
+
+/* The same path with HOST buffers: the library allocates device memory, copies host_s_instr in,
+ * runs gbfg_simulate on its own stream, and copies the PSD ([n_cat][n_bins] binary64) and the
+ * resolved flags ([N] uint8, may be NULL) back.  Host pointers should be pinned for full speed.
+ * Synchronous. */
+int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
+                       uint64_t seed, const double *host_s_instr, const gbfg_iter_params *params,
+                       double *host_psd, uint8_t *host_resolved, gbfg_iter_result *host_results);
+
+/* Bytes of device workspace sufficient for any call above on this grid / batch. */
+size_t gbfg_workspace_bytes(const gbfg_grid *grid, int64_t n_src_total, int32_t n_cat);
+
+/* Number of kernels the calling thread's library calls have launched so far (for bench.py). */
+int64_t gbfg_kernel_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GBFG_H */

@@ -1,0 +1,222 @@
+"""ctypes binding of libgbfg (include/gbfg.h): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels; torch supplies device memory and
+the stream.  There is no CPU fallback: `load()` raises if the library is missing, and every call
+raises `GbfgError` on a non-zero status.  Function names and argument order follow gbfg.h.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libgbfg.so")
+
+MAX_CAT = 256
+MAX_WINDOW = 4097
+MAX_ITER_TRACE = 64
+FLAG_NO_PRESELECT = 1
+FLAG_NO_INCREMENTAL = 2
+
+EXPORTS = [
+    "gbfg_version", "gbfg_strerror", "gbfg_last_cuda_error", "gbfg_grid_init", "gbfg_instrument_noise",
+    "gbfg_sample_catalog", "gbfg_deposit", "gbfg_running_median", "gbfg_psd", "gbfg_snr_select",
+    "gbfg_subtract_until_converged", "gbfg_simulate", "gbfg_simulate_host", "gbfg_workspace_bytes",
+    "gbfg_kernel_launch_count",
+]
+
+
+class GbfgError(RuntimeError):
+    def __init__(self, status: int, what: str):
+        self.status = status
+        super().__init__(what)
+
+
+class Grid(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("scale_log2", C.c_int32), ("f_min", C.c_double),
+                ("f_max", C.c_double), ("t_obs", C.c_double), ("n_bins", C.c_int64)]
+
+
+class Pop(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("reserved", C.c_uint32), ("slope", C.c_double),
+                ("logA_offset", C.c_double), ("logA_sigma", C.c_double), ("logMc_mean", C.c_double),
+                ("logMc_sigma", C.c_double), ("n_src", C.c_int64)]
+
+
+class IterParams(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("window", C.c_int32), ("median_norm", C.c_double),
+                ("rho_th", C.c_double), ("max_iter", C.c_int32), ("flags", C.c_uint32)]
+
+
+class IterResult(C.Structure):
+    _fields_ = [("n_iter", C.c_int32), ("converged", C.c_int32), ("n_resolved", C.c_int64),
+                ("n_near_threshold", C.c_int64), ("n_candidates", C.c_int64),
+                ("n_new_per_iter", C.c_int64 * MAX_ITER_TRACE)]
+
+
+_lib = None
+
+
+def load():
+    """Loads libgbfg.so (built in-tree by paper_2602_18560_b200.build).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise GbfgError(-100, f"{LIB_PATH} is missing: run `python -m paper_2602_18560_b200.build` "
+                              "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, i32, i64, u32, u64, dbl, sz = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_uint64, C.c_double, C.c_size_t
+    gp, pp, ip, rp = C.POINTER(Grid), C.POINTER(Pop), C.POINTER(IterParams), C.POINTER(IterResult)
+    op = C.POINTER(C.c_int64)
+    L.gbfg_version.restype = C.c_int
+    L.gbfg_strerror.restype = C.c_char_p
+    L.gbfg_strerror.argtypes = [C.c_int]
+    L.gbfg_last_cuda_error.restype = C.c_char_p
+    L.gbfg_kernel_launch_count.restype = i64
+    L.gbfg_grid_init.argtypes = [dbl, dbl, dbl, i32, gp]
+    L.gbfg_instrument_noise.argtypes = [gp, vp, vp]
+    L.gbfg_sample_catalog.argtypes = [gp, pp, op, i32, u32, u64, vp, vp, vp, vp]
+    L.gbfg_deposit.argtypes = [gp, vp, vp, vp, op, i32, vp, vp, i32, vp, vp, vp, sz, vp]
+    L.gbfg_running_median.argtypes = [vp, i64, i32, i32, vp, vp]
+    L.gbfg_psd.argtypes = [vp, vp, i64, i32, dbl, i32, vp, vp]
+    L.gbfg_snr_select.argtypes = [gp, vp, vp, vp, op, i32, vp, dbl, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.gbfg_subtract_until_converged.argtypes = [gp, vp, vp, vp, op, i32, vp, ip, vp, vp, vp, vp, rp, vp, sz, vp]
+    L.gbfg_simulate.argtypes = [gp, pp, op, i32, u64, vp, ip, vp, vp, vp, vp, vp, vp, vp, vp, vp, rp, vp, sz, vp]
+    L.gbfg_simulate_host.argtypes = [gp, pp, op, i32, u64, vp, ip, vp, vp, rp]
+    L.gbfg_workspace_bytes.restype = sz
+    L.gbfg_workspace_bytes.argtypes = [gp, i64, i32]
+    _lib = L
+    return L
+
+
+def _check(status: int):
+    if status != 0:
+        L = load()
+        msg = L.gbfg_strerror(status).decode()
+        if status == -3:
+            msg += ": " + L.gbfg_last_cuda_error().decode()
+        raise GbfgError(status, msg)
+
+
+def _ptr(t) -> Optional[int]:
+    """Device (or host) address of a torch tensor / numpy array / int / None."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        return t.data_ptr()
+    return t.ctypes.data
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return stream if isinstance(stream, int) else stream.cuda_stream
+
+
+def _offsets(offsets: Sequence[int]):
+    return (C.c_int64 * len(offsets))(*[int(o) for o in offsets])
+
+
+def _pops(pops):
+    arr = (Pop * len(pops))()
+    for i, p in enumerate(pops):
+        arr[i] = p if isinstance(p, Pop) else make_pop(p)
+    return arr
+
+
+def make_pop(p) -> Pop:
+    """From any object with the fields of gbfg_pop (e.g. gbfg_workloads.Population)."""
+    return Pop(C.sizeof(Pop), 0, p.slope, p.logA_offset, p.logA_sigma, p.logMc_mean, p.logMc_sigma, p.n_src)
+
+
+def make_iter_params(window: int, median_norm: float, rho_th: float, max_iter: int, flags: int = 0) -> IterParams:
+    return IterParams(C.sizeof(IterParams), window, median_norm, rho_th, max_iter, flags)
+
+
+def version() -> int:
+    return load().gbfg_version()
+
+
+def kernel_launch_count() -> int:
+    return load().gbfg_kernel_launch_count()
+
+
+def grid_init(f_min: float, f_max: float, t_obs: float, scale_log2: int = -140) -> Grid:
+    g = Grid()
+    _check(load().gbfg_grid_init(f_min, f_max, t_obs, scale_log2, C.byref(g)))
+    return g
+
+
+def workspace_bytes(grid: Grid, n_src_total: int, n_cat: int = 1) -> int:
+    return load().gbfg_workspace_bytes(C.byref(grid), n_src_total, n_cat)
+
+
+def instrument_noise(grid: Grid, dev_s_instr, stream=None):
+    _check(load().gbfg_instrument_noise(C.byref(grid), _ptr(dev_s_instr), _stream(stream)))
+
+
+def sample_catalog(grid: Grid, pops, offsets, seed: int, dev_A, dev_f, dev_fdot, first_cat_id: int = 0, stream=None):
+    _check(load().gbfg_sample_catalog(C.byref(grid), _pops(pops), _offsets(offsets), len(pops), first_cat_id, seed,
+                                      _ptr(dev_A), _ptr(dev_f), _ptr(dev_fdot), _stream(stream)))
+
+
+def deposit(grid: Grid, dev_A, dev_f, dev_fdot, offsets, dev_spectrum, workspace, sign: int = 1,
+            dev_sel_idx=None, dev_sel_count=None, dev_err_count=None, stream=None):
+    _check(load().gbfg_deposit(C.byref(grid), _ptr(dev_A), _ptr(dev_f), _ptr(dev_fdot), _offsets(offsets),
+                               len(offsets) - 1, _ptr(dev_sel_idx), _ptr(dev_sel_count), sign, _ptr(dev_spectrum),
+                               _ptr(dev_err_count), _ptr(workspace), workspace.numel() * workspace.element_size(),
+                               _stream(stream)))
+
+
+def running_median(dev_spectrum, n_bins: int, n_cat: int, window: int, dev_median_out, stream=None):
+    _check(load().gbfg_running_median(_ptr(dev_spectrum), n_bins, n_cat, window, _ptr(dev_median_out), _stream(stream)))
+
+
+def psd(dev_median, dev_s_instr, n_bins: int, n_cat: int, median_norm: float, scale_log2: int, dev_psd, stream=None):
+    _check(load().gbfg_psd(_ptr(dev_median), _ptr(dev_s_instr), n_bins, n_cat, median_norm, scale_log2,
+                           _ptr(dev_psd), _stream(stream)))
+
+
+def snr_select(grid: Grid, dev_A, dev_f, dev_fdot, offsets, dev_psd, rho_th: float, dev_resolved, dev_sel_idx,
+               dev_sel_count, workspace, dev_rho2_out=None, dev_near_count=None, stream=None):
+    _check(load().gbfg_snr_select(C.byref(grid), _ptr(dev_A), _ptr(dev_f), _ptr(dev_fdot), _offsets(offsets),
+                                  len(offsets) - 1, _ptr(dev_psd), rho_th, _ptr(dev_resolved), _ptr(dev_rho2_out),
+                                  _ptr(dev_sel_idx), _ptr(dev_sel_count), _ptr(dev_near_count), _ptr(workspace),
+                                  workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+def subtract_until_converged(grid: Grid, dev_A, dev_f, dev_fdot, offsets, dev_s_instr, params: IterParams,
+                             dev_spectrum, dev_median, dev_psd, dev_resolved, workspace, stream=None):
+    n_cat = len(offsets) - 1
+    res = (IterResult * n_cat)()
+    _check(load().gbfg_subtract_until_converged(
+        C.byref(grid), _ptr(dev_A), _ptr(dev_f), _ptr(dev_fdot), _offsets(offsets), n_cat, _ptr(dev_s_instr),
+        C.byref(params), _ptr(dev_spectrum), _ptr(dev_median), _ptr(dev_psd), _ptr(dev_resolved), res,
+        _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)))
+    return list(res)
+
+
+def simulate(grid: Grid, pops, offsets, seed: int, dev_s_instr, params: IterParams, dev_A, dev_f, dev_fdot,
+             dev_total, dev_spectrum, dev_median, dev_psd, dev_resolved, workspace, dev_err_count=None, stream=None):
+    n_cat = len(offsets) - 1
+    res = (IterResult * n_cat)()
+    _check(load().gbfg_simulate(
+        C.byref(grid), _pops(pops), _offsets(offsets), n_cat, seed, _ptr(dev_s_instr), C.byref(params),
+        _ptr(dev_A), _ptr(dev_f), _ptr(dev_fdot), _ptr(dev_total), _ptr(dev_spectrum), _ptr(dev_median),
+        _ptr(dev_psd), _ptr(dev_resolved), _ptr(dev_err_count), res, _ptr(workspace),
+        workspace.numel() * workspace.element_size(), _stream(stream)))
+    return list(res)
+
+
+def simulate_host(grid: Grid, pops, offsets, seed: int, host_s_instr, params: IterParams, host_psd,
+                  host_resolved=None):
+    n_cat = len(offsets) - 1
+    res = (IterResult * n_cat)()
+    _check(load().gbfg_simulate_host(C.byref(grid), _pops(pops), _offsets(offsets), n_cat, seed, _ptr(host_s_instr),
+                                     C.byref(params), _ptr(host_psd), _ptr(host_resolved), res))
+    return list(res)

@@ -1,0 +1,90 @@
+// api.cu — host-side plumbing of libgbfg: status strings, device check, grid, launch counter.
+#include <stdio.h>
+#include <string.h>
+
+#include "gbfg_common.cuh"
+
+namespace gbfg {
+
+static thread_local char g_cuda_error[512] = "";
+static thread_local int64_t g_launches = 0;
+
+int set_cuda_error(cudaError_t e, const char *where)
+{
+    snprintf(g_cuda_error, sizeof(g_cuda_error), "%s: %s (%s)", where, cudaGetErrorString(e), cudaGetErrorName(e));
+    (void)cudaGetLastError();   // clear the sticky-less error state
+    return GBFG_ERR_CUDA;
+}
+
+void count_launch(int n) { g_launches += n; }
+
+struct DevInfo { int ok; int status; int sms; };
+static DevInfo g_dev[64];
+
+static int probe_device(int *sms)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return set_cuda_error(e, "cudaGetDevice");
+    if (dev < 0 || dev >= 64) return GBFG_ERR_ARCH;
+    if (!g_dev[dev].ok) {
+        int major = 0, n = 0;
+        e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev);
+        if (e != cudaSuccess) return set_cuda_error(e, "cudaDeviceGetAttribute");
+        e = cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return set_cuda_error(e, "cudaDeviceGetAttribute");
+        g_dev[dev].status = (major == 10) ? GBFG_OK : GBFG_ERR_ARCH;
+        g_dev[dev].sms = n;
+        g_dev[dev].ok = 1;
+    }
+    if (sms) *sms = g_dev[dev].sms;
+    return g_dev[dev].status;
+}
+
+int check_device() { return probe_device(nullptr); }
+
+int sm_count()
+{
+    int n = 148;
+    probe_device(&n);
+    return n > 0 ? n : 148;
+}
+
+}  // namespace gbfg
+
+using namespace gbfg;
+
+extern "C" int gbfg_version(void) { return 100; /* 0.1.0 */ }
+
+extern "C" const char *gbfg_strerror(int status)
+{
+    switch (status) {
+    case GBFG_OK: return "ok";
+    case GBFG_ERR_INVALID_ARG: return "invalid argument";
+    case GBFG_ERR_WORKSPACE: return "workspace missing or too small";
+    case GBFG_ERR_CUDA: return "CUDA runtime error (see gbfg_last_cuda_error)";
+    case GBFG_ERR_ARCH: return "device is not compute capability 10.x (sm_100)";
+    case GBFG_ERR_UNSUPPORTED: return "unsupported size (window > GBFG_MAX_WINDOW or n_cat > GBFG_MAX_CAT)";
+    default: return "unknown status";
+    }
+}
+
+extern "C" const char *gbfg_last_cuda_error(void) { return g_cuda_error; }
+
+extern "C" int64_t gbfg_kernel_launch_count(void) { return g_launches; }
+
+extern "C" int gbfg_grid_init(double f_min, double f_max, double t_obs, int32_t scale_log2, gbfg_grid *out)
+{
+    if (!out) return GBFG_ERR_INVALID_ARG;
+    if (!(f_min > 0.0) || !(f_max > f_min) || !(t_obs > 0.0)) return GBFG_ERR_INVALID_ARG;
+    if (!(f_max < 1e300) || !(t_obs < 1e300)) return GBFG_ERR_INVALID_ARG;
+    if (scale_log2 < -1000 || scale_log2 > 0) return GBFG_ERR_INVALID_ARG;
+    double nb = ceil((f_max - f_min) * t_obs);          // DESIGN.md R2
+    if (!(nb >= 1.0) || !(nb < 2147483648.0)) return GBFG_ERR_INVALID_ARG;
+    memset(out, 0, sizeof(*out));
+    out->struct_size = (uint32_t)sizeof(gbfg_grid);
+    out->scale_log2 = scale_log2;
+    out->f_min = f_min; out->f_max = f_max; out->t_obs = t_obs;
+    out->n_bins = (int64_t)nb;
+    return GBFG_OK;
+}

@@ -1,0 +1,179 @@
+// deposit.cu — stages (ii) and (v): spectrum[k] += sign * q_i over the bins a source's chirp covers.
+//
+// DESIGN.md R2 fixes the arithmetic.  The accumulator is int64, so any order and any regrouping of
+// the additions gives the same bits.  That is used twice:
+//   * narrow sources (w_eff <= NARROW) add q straight into the spectrum with 64-bit L2 atomics;
+//   * wide sources use the range-update form: +q at k0 and -q at k0+w_eff in a difference array,
+//     followed by one inclusive scan that is added into the spectrum (2 updates per source instead
+//     of w; chirps reach 7e4 bins at 4 yr).  sum_k spectrum[k] is identical bit for bit.
+// The scan is the three-phase tile scan (tile sums -> scan of tile sums -> rescan + add); the
+// difference array is zeroed again on the way so the workspace is reusable.
+#include "gbfg_common.cuh"
+
+namespace gbfg {
+
+constexpr int NARROW = 4;            // <= NARROW bins: direct atomics
+constexpr int SCAN_THREADS = 256;
+constexpr int SCAN_ITEMS = 8;        // int64 per thread
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
+
+// One thread per addressed source.  `wide_flag` is set if any source used the difference array.
+__global__ void __launch_bounds__(256)
+deposit_kernel(GridDev g, CatTable ct, const double *__restrict__ A, const double *__restrict__ f,
+               const double *__restrict__ fdot, const int64_t *__restrict__ sel_idx,
+               const int64_t *__restrict__ sel_count, int64_t n_all, int32_t sign,
+               int64_t *__restrict__ spectrum, int64_t *__restrict__ diff,
+               int64_t *__restrict__ err_count, int *__restrict__ wide_flag)
+{
+    const int64_t n = sel_idx ? *sel_count : n_all;
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    int rejected = 0;
+    for (; t < n; t += stride) {
+        const int64_t i = sel_idx ? sel_idx[t] : t;
+        SrcBins s = source_bins(g, A[i], f[i], fdot[i]);
+        if (s.status) { ++rejected; continue; }
+        const int64_t row = (int64_t)cat_of(ct, i) * g.n_bins;
+        const int64_t v = sign >= 0 ? s.q : -s.q;
+        if (v == 0) continue;
+        if (s.w_eff <= NARROW) {
+            for (int64_t k = s.k0; k < s.k0 + s.w_eff; ++k) atomic_add_i64(spectrum + row + k, v);
+        } else {
+            atomic_add_i64(diff + row + s.k0, v);
+            if (s.k0 + s.w_eff < g.n_bins) atomic_add_i64(diff + row + s.k0 + s.w_eff, -v);
+            *wide_flag = 1;
+        }
+    }
+    if (err_count) {
+        // warp-aggregate the reject count
+        for (int o = 16; o; o >>= 1) rejected += __shfl_down_sync(0xffffffffu, rejected, o);
+        if ((threadIdx.x & 31) == 0 && rejected) atomic_add_i64(err_count, rejected);
+    }
+}
+
+// phase 1: tile sums of the difference array.  grid = (tiles_per_row, n_cat)
+__global__ void __launch_bounds__(SCAN_THREADS)
+scan_tile_sums_kernel(const int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
+                      int64_t *__restrict__ tile_sums, const int *__restrict__ wide_flag)
+{
+    if (*wide_flag == 0) return;
+    __shared__ int64_t warp_sum[SCAN_THREADS / 32];
+    const int64_t row = (int64_t)blockIdx.y * n_bins;
+    const int64_t base = (int64_t)blockIdx.x * SCAN_TILE;
+    int64_t acc = 0;
+#pragma unroll
+    for (int j = 0; j < SCAN_ITEMS; ++j) {
+        int64_t k = base + (int64_t)j * SCAN_THREADS + threadIdx.x;
+        if (k < n_bins) acc += diff[row + k];
+    }
+    for (int o = 16; o; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+    if ((threadIdx.x & 31) == 0) warp_sum[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int64_t s = 0;
+        for (int w = 0; w < SCAN_THREADS / 32; ++w) s += warp_sum[w];
+        tile_sums[(int64_t)blockIdx.y * tiles_per_row + blockIdx.x] = s;
+    }
+}
+
+// phase 2: exclusive scan of each row's tile sums, one CTA per row (tiles_per_row is a few thousand)
+__global__ void __launch_bounds__(1024)
+scan_tile_offsets_kernel(int64_t *__restrict__ tile_sums, int tiles_per_row, const int *__restrict__ wide_flag)
+{
+    if (*wide_flag == 0) return;
+    __shared__ int64_t warp_tot[32];
+    __shared__ int64_t carry_s;
+    int64_t *row = tile_sums + (int64_t)blockIdx.x * tiles_per_row;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (int base = 0; base < tiles_per_row; base += 1024) {
+        int idx = base + threadIdx.x;
+        int64_t v = idx < tiles_per_row ? row[idx] : 0;
+        int64_t incl = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            int64_t up = __shfl_up_sync(0xffffffffu, incl, o);
+            if ((threadIdx.x & 31) >= o) incl += up;
+        }
+        if ((threadIdx.x & 31) == 31) warp_tot[threadIdx.x >> 5] = incl;
+        __syncthreads();
+        int64_t before = carry_s;
+        for (int w = 0; w < (threadIdx.x >> 5); ++w) before += warp_tot[w];
+        if (idx < tiles_per_row) row[idx] = before + incl - v;
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = before + incl;
+        __syncthreads();
+    }
+}
+
+// phase 3: rescan each tile, add the running value into the spectrum, zero the difference array
+__global__ void __launch_bounds__(SCAN_THREADS)
+scan_add_kernel(int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
+                const int64_t *__restrict__ tile_offsets, int64_t *__restrict__ spectrum,
+                const int *__restrict__ wide_flag)
+{
+    if (*wide_flag == 0) return;
+    __shared__ int64_t warp_tot[SCAN_THREADS / 32];
+    const int64_t row = (int64_t)blockIdx.y * n_bins;
+    const int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+    int64_t v[SCAN_ITEMS];
+    int64_t tsum = 0;
+#pragma unroll
+    for (int j = 0; j < SCAN_ITEMS; ++j) {
+        int64_t k = base + j;
+        v[j] = k < n_bins ? diff[row + k] : 0;
+        tsum += v[j];
+    }
+    int64_t incl = tsum;
+    for (int o = 1; o < 32; o <<= 1) {
+        int64_t up = __shfl_up_sync(0xffffffffu, incl, o);
+        if ((threadIdx.x & 31) >= o) incl += up;
+    }
+    if ((threadIdx.x & 31) == 31) warp_tot[threadIdx.x >> 5] = incl;
+    __syncthreads();
+    int64_t run = tile_offsets[(int64_t)blockIdx.y * tiles_per_row + blockIdx.x] + incl - tsum;
+    for (int w = 0; w < (threadIdx.x >> 5); ++w) run += warp_tot[w];
+#pragma unroll
+    for (int j = 0; j < SCAN_ITEMS; ++j) {
+        int64_t k = base + j;
+        run += v[j];
+        if (k < n_bins) {
+            if (run != 0) spectrum[row + k] += run;
+            if (v[j] != 0) diff[row + k] = 0;
+        }
+    }
+}
+
+__global__ void clear_flag_kernel(int *flag) { *flag = 0; }
+
+// ---------------------------------------------------------------------------------------------
+// internal entry used by the stage call and by the loop.  diff: [n_cat*n_bins] zero on entry and
+// on exit; tile_sums: [n_cat*tiles_per_row]; wide_flag: one int (zero on entry and exit).
+// ---------------------------------------------------------------------------------------------
+int scan_tiles_per_row(int64_t n_bins) { return (int)((n_bins + SCAN_TILE - 1) / SCAN_TILE); }
+
+int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
+                   const int64_t *sel_idx, const int64_t *sel_count, int64_t n_launch, int32_t sign,
+                   int64_t *spectrum, int64_t *err_count, int64_t *diff, int64_t *tile_sums, int *wide_flag,
+                   cudaStream_t st)
+{
+    if (n_launch <= 0) return GBFG_OK;
+    int64_t blocks = (n_launch + 255) / 256;
+    int64_t cap = (int64_t)sm_count() * 16;
+    if (blocks > cap) blocks = cap;
+    deposit_kernel<<<(int)blocks, 256, 0, st>>>(g, ct, A, f, fdot, sel_idx, sel_count, ct.offsets[ct.n_cat], sign,
+                                                spectrum, diff, err_count, wide_flag);
+    GBFG_LAUNCH_CHECK("deposit_kernel");
+    const int tiles = scan_tiles_per_row(g.n_bins);
+    dim3 grid(tiles, ct.n_cat);
+    scan_tile_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, wide_flag);
+    GBFG_LAUNCH_CHECK("scan_tile_sums_kernel");
+    scan_tile_offsets_kernel<<<ct.n_cat, 1024, 0, st>>>(tile_sums, tiles, wide_flag);
+    GBFG_LAUNCH_CHECK("scan_tile_offsets_kernel");
+    scan_add_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, spectrum, wide_flag);
+    GBFG_LAUNCH_CHECK("scan_add_kernel");
+    clear_flag_kernel<<<1, 1, 0, st>>>(wide_flag);
+    GBFG_LAUNCH_CHECK("clear_flag_kernel");
+    return GBFG_OK;
+}
+
+}  // namespace gbfg

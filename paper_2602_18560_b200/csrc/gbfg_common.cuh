@@ -1,0 +1,113 @@
+// gbfg_common.cuh — shared declarations of the CUDA side of libgbfg (sm_100a).
+//
+// Nothing in this directory is shared with oracle/: constants and algorithms are typed here
+// independently from DESIGN.md §3-§4.  The translation units are compiled with -fmad=false so
+// that every binary64 operation is singly rounded; fma() appears only where DESIGN.md §4 says so.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include "../../include/gbfg.h"
+
+namespace gbfg {
+
+// ---------------------------------------------------------------------------------------------
+// host-side plumbing
+// ---------------------------------------------------------------------------------------------
+int set_cuda_error(cudaError_t e, const char *where);   // records text, returns GBFG_ERR_CUDA
+int check_device();                                     // GBFG_OK or GBFG_ERR_ARCH / GBFG_ERR_CUDA
+void count_launch(int n = 1);
+int sm_count();
+
+#define GBFG_CUDA(call)                                                        \
+    do {                                                                       \
+        cudaError_t e__ = (call);                                              \
+        if (e__ != cudaSuccess) return gbfg::set_cuda_error(e__, #call);       \
+    } while (0)
+
+#define GBFG_LAUNCH_CHECK(name)                                                \
+    do {                                                                       \
+        gbfg::count_launch();                                                  \
+        cudaError_t e__ = cudaGetLastError();                                  \
+        if (e__ != cudaSuccess) return gbfg::set_cuda_error(e__, name);        \
+    } while (0)
+
+// Per-batch catalog table passed by value to kernels (<= GBFG_MAX_CAT catalogs).
+struct CatTable {
+    int32_t n_cat;
+    int64_t offsets[GBFG_MAX_CAT + 1];
+};
+
+// Grid constants precomputed on the host (each a single IEEE operation, R2).
+struct GridDev {
+    double f_min, f_max, T, T2, halfT;
+    int64_t n_bins;
+    int32_t scale_log2;
+};
+
+inline GridDev make_grid_dev(const gbfg_grid *g)
+{
+    GridDev d;
+    d.f_min = g->f_min; d.f_max = g->f_max; d.T = g->t_obs;
+    d.T2 = g->t_obs * g->t_obs;
+    d.halfT = 0.5 * g->t_obs;
+    d.n_bins = g->n_bins; d.scale_log2 = g->scale_log2;
+    return d;
+}
+
+// ---------------------------------------------------------------------------------------------
+// device helpers
+// ---------------------------------------------------------------------------------------------
+
+// catalog of global source index i (n_cat is small: linear scan for <= 4, else binary search)
+__device__ __forceinline__ int cat_of(const CatTable &ct, int64_t i)
+{
+    if (ct.n_cat == 1) return 0;
+    int lo = 0, hi = ct.n_cat;          // invariant: offsets[lo] <= i < offsets[hi]
+    while (hi - lo > 1) {
+        int mid = (lo + hi) >> 1;
+        if (ct.offsets[mid] <= i) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+// The integer triple and per-bin power of one source (R2).
+struct SrcBins {
+    int64_t k0, w_eff, q;
+    double p;
+    int status;     // 0 deposits, 1 DOMAIN, 2 RANGE
+};
+
+__device__ __forceinline__ SrcBins source_bins(const GridDev &g, double A, double f, double fdot)
+{
+    SrcBins s;
+    s.k0 = 0; s.w_eff = 0; s.q = 0; s.p = 0.0; s.status = 1;
+    if (!(A >= 0.0) || !(fdot >= 0.0) || !(f >= g.f_min) || !(f < g.f_max)) return s;
+    double kk = floor((f - g.f_min) * g.T);
+    if (!(kk < (double)g.n_bins)) return s;
+    s.status = 2;
+    double ww = ceil(fdot * g.T2);
+    if (!(ww < 0x1p62)) return s;
+    if (ww < 1.0) ww = 1.0;
+    double P = (A * A) * g.halfT;
+    double pp = P / ww;
+    double qd = ldexp(pp, -g.scale_log2);
+    if (!(qd < 0x1p62)) return s;
+    s.k0 = (int64_t)kk;
+    int64_t w = (int64_t)ww;
+    int64_t room = g.n_bins - s.k0;
+    s.w_eff = w < room ? w : room;
+    s.p = pp;
+    s.q = __double2ll_rn(qd);           // round half to even, as llrint
+    s.status = 0;
+    return s;
+}
+
+__device__ __forceinline__ void atomic_add_i64(int64_t *addr, int64_t v)
+{
+    atomicAdd(reinterpret_cast<unsigned long long *>(addr), (unsigned long long)v);
+}
+
+}  // namespace gbfg

@@ -1,0 +1,308 @@
+// loop.cu — the C-ABI stage calls that need workspace, and stage (v): the subtraction loop of
+// Appendix D steps 4-10 (R6), device resident, one small scalar
+// read back per iteration.
+#include <string.h>
+
+#include "gbfg_common.cuh"
+
+namespace gbfg {
+
+// from the other translation units
+int scan_tiles_per_row(int64_t n_bins);
+int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
+                   const int64_t *sel_idx, const int64_t *sel_count, int64_t n_launch, int32_t sign,
+                   int64_t *spectrum, int64_t *err_count, int64_t *diff, int64_t *tile_sums, int *wide_flag,
+                   cudaStream_t st);
+int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *med,
+                  const double *s_instr, double *psd, double norm, int scale_log2,
+                  const uint8_t *tile_dirty, cudaStream_t st);
+int snr_inv_blocks_per_row(int64_t n_bins);
+int launch_snr_select(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
+                      const double *psd, double rho_th, uint8_t *resolved, double *rho2_out,
+                      const int64_t *cand_idx, const int64_t *cand_count, int64_t n_launch,
+                      int64_t *sel_idx, int64_t *sel_count, int64_t *near_count, int near_per_cat,
+                      double *inv_blocks, cudaStream_t st);
+
+// ------------------------------------------------------------------------------- workspace
+struct Workspace {
+    int64_t *diff;        // [n_cat * n_bins]   difference array of the range-update deposit
+    int64_t *tile_sums;   // [n_cat * scan_tiles]
+    double *inv_blocks;   // [n_cat * inv_blocks_per_row]
+    int64_t *sel_idx;     // [n_src_total]
+    int64_t *counters;    // [COUNTERS]: sel_count[1 + n_cat], near[n_cat], spare
+    int *wide_flag;
+    size_t bytes;
+};
+
+constexpr int WS_COUNTERS = 2 * GBFG_MAX_CAT + 8;
+
+static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
+
+static Workspace carve(void *base, int64_t n_bins, int64_t n_src_total, int n_cat)
+{
+    Workspace w;
+    size_t off = 0;
+    char *b = (char *)base;
+    w.diff = (int64_t *)(b + off);       off += align_up(sizeof(int64_t) * (size_t)n_cat * (size_t)n_bins);
+    w.tile_sums = (int64_t *)(b + off);  off += align_up(sizeof(int64_t) * (size_t)n_cat * (size_t)scan_tiles_per_row(n_bins));
+    w.inv_blocks = (double *)(b + off);  off += align_up(sizeof(double) * (size_t)n_cat * (size_t)snr_inv_blocks_per_row(n_bins));
+    w.sel_idx = (int64_t *)(b + off);    off += align_up(sizeof(int64_t) * (size_t)(n_src_total > 0 ? n_src_total : 1));
+    w.counters = (int64_t *)(b + off);   off += align_up(sizeof(int64_t) * WS_COUNTERS);
+    w.wide_flag = (int *)(b + off);      off += align_up(sizeof(int));
+    w.bytes = off;
+    return w;
+}
+
+static int make_cat_table(const int64_t *offsets, int n_cat, CatTable *ct)
+{
+    if (!offsets || n_cat < 1) return GBFG_ERR_INVALID_ARG;
+    if (n_cat > GBFG_MAX_CAT) return GBFG_ERR_UNSUPPORTED;
+    if (offsets[0] != 0) return GBFG_ERR_INVALID_ARG;
+    ct->n_cat = n_cat;
+    for (int c = 0; c <= n_cat; ++c) {
+        if (c && offsets[c] < offsets[c - 1]) return GBFG_ERR_INVALID_ARG;
+        ct->offsets[c] = offsets[c];
+    }
+    for (int c = n_cat + 1; c <= GBFG_MAX_CAT; ++c) ct->offsets[c] = offsets[n_cat];
+    return GBFG_OK;
+}
+
+static int valid_grid(const gbfg_grid *g)
+{
+    return g && g->struct_size == sizeof(gbfg_grid) && g->n_bins >= 1 && g->n_bins < 2147483648ll &&
+           g->f_min > 0.0 && g->f_max > g->f_min && g->t_obs > 0.0 && g->scale_log2 >= -1000 && g->scale_log2 <= 0;
+}
+
+// pinned host scratch for the per-iteration readback (one per host thread)
+static int64_t *host_scratch()
+{
+    static thread_local int64_t *p = nullptr;
+    if (!p) {
+        if (cudaHostAlloc((void **)&p, sizeof(int64_t) * WS_COUNTERS, cudaHostAllocDefault) != cudaSuccess) {
+            (void)cudaGetLastError();
+            p = nullptr;
+        }
+    }
+    return p;
+}
+
+}  // namespace gbfg
+
+using namespace gbfg;
+
+extern "C" size_t gbfg_workspace_bytes(const gbfg_grid *grid, int64_t n_src_total, int32_t n_cat)
+{
+    if (!valid_grid(grid) || n_cat < 1 || n_cat > GBFG_MAX_CAT || n_src_total < 0) return 0;
+    return carve(nullptr, grid->n_bins, n_src_total, n_cat).bytes;
+}
+
+extern "C" int gbfg_deposit(const gbfg_grid *grid, const double *dev_A, const double *dev_f, const double *dev_fdot,
+                            const int64_t *offsets, int32_t n_cat,
+                            const int64_t *dev_sel_idx, const int64_t *dev_sel_count, int32_t sign,
+                            int64_t *dev_spectrum, int64_t *dev_err_count,
+                            void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (!valid_grid(grid) || !dev_spectrum || (sign != 1 && sign != -1)) return GBFG_ERR_INVALID_ARG;
+    if ((dev_sel_idx == nullptr) != (dev_sel_count == nullptr)) return GBFG_ERR_INVALID_ARG;
+    CatTable ct;
+    int rc = make_cat_table(offsets, n_cat, &ct);
+    if (rc) return rc;
+    const int64_t n = ct.offsets[n_cat];
+    if (n > 0 && (!dev_A || !dev_f || !dev_fdot)) return GBFG_ERR_INVALID_ARG;
+    if (!workspace) return GBFG_ERR_WORKSPACE;
+    Workspace w = carve(workspace, grid->n_bins, n, n_cat);
+    if (workspace_bytes < w.bytes) return GBFG_ERR_WORKSPACE;
+    rc = check_device();
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    GBFG_CUDA(cudaMemsetAsync(w.diff, 0, sizeof(int64_t) * (size_t)n_cat * (size_t)grid->n_bins, st));
+    GBFG_CUDA(cudaMemsetAsync(w.wide_flag, 0, sizeof(int), st));
+    return launch_deposit(make_grid_dev(grid), ct, dev_A, dev_f, dev_fdot, dev_sel_idx, dev_sel_count, n, sign,
+                          dev_spectrum, dev_err_count, w.diff, w.tile_sums, w.wide_flag, st);
+}
+
+extern "C" int gbfg_snr_select(const gbfg_grid *grid, const double *dev_A, const double *dev_f, const double *dev_fdot,
+                               const int64_t *offsets, int32_t n_cat, const double *dev_psd, double rho_th,
+                               uint8_t *dev_resolved, double *dev_rho2_out,
+                               int64_t *dev_sel_idx, int64_t *dev_sel_count, int64_t *dev_near_count,
+                               void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (!valid_grid(grid) || !dev_psd || !dev_resolved || !dev_sel_idx || !dev_sel_count) return GBFG_ERR_INVALID_ARG;
+    if (!(rho_th >= 0.0)) return GBFG_ERR_INVALID_ARG;
+    CatTable ct;
+    int rc = make_cat_table(offsets, n_cat, &ct);
+    if (rc) return rc;
+    const int64_t n = ct.offsets[n_cat];
+    if (n > 0 && (!dev_A || !dev_f || !dev_fdot)) return GBFG_ERR_INVALID_ARG;
+    if (!workspace) return GBFG_ERR_WORKSPACE;
+    Workspace w = carve(workspace, grid->n_bins, n, n_cat);
+    if (workspace_bytes < w.bytes) return GBFG_ERR_WORKSPACE;
+    rc = check_device();
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    GBFG_CUDA(cudaMemsetAsync(dev_sel_count, 0, sizeof(int64_t) * (size_t)(1 + n_cat), st));
+    return launch_snr_select(make_grid_dev(grid), ct, dev_A, dev_f, dev_fdot, dev_psd, rho_th, dev_resolved,
+                             dev_rho2_out, nullptr, nullptr, n, dev_sel_idx, dev_sel_count, dev_near_count, 0,
+                             w.inv_blocks, st);
+}
+
+extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double *dev_A, const double *dev_f,
+                                             const double *dev_fdot, const int64_t *offsets, int32_t n_cat,
+                                             const double *dev_s_instr, const gbfg_iter_params *params,
+                                             int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
+                                             uint8_t *dev_resolved, gbfg_iter_result *host_results,
+                                             void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (!valid_grid(grid) || !params || params->struct_size != sizeof(gbfg_iter_params)) return GBFG_ERR_INVALID_ARG;
+    if (!dev_s_instr || !dev_spectrum || !dev_median || !dev_psd || !dev_resolved || !host_results) return GBFG_ERR_INVALID_ARG;
+    const int W = params->window;
+    if (W < 1 || (W & 1) == 0 || params->max_iter < 1 || !(params->rho_th >= 0.0) || !(params->median_norm > 0.0))
+        return GBFG_ERR_INVALID_ARG;
+    if (W > GBFG_MAX_WINDOW) return GBFG_ERR_UNSUPPORTED;
+    if (grid->n_bins < W / 2 + 1) return GBFG_ERR_INVALID_ARG;
+    CatTable ct;
+    int rc = make_cat_table(offsets, n_cat, &ct);
+    if (rc) return rc;
+    const int64_t n = ct.offsets[n_cat];
+    if (n > 0 && (!dev_A || !dev_f || !dev_fdot)) return GBFG_ERR_INVALID_ARG;
+    if (!workspace) return GBFG_ERR_WORKSPACE;
+    Workspace w = carve(workspace, grid->n_bins, n, n_cat);
+    if (workspace_bytes < w.bytes) return GBFG_ERR_WORKSPACE;
+    rc = check_device();
+    if (rc) return rc;
+    int64_t *host = host_scratch();
+    if (!host) return set_cuda_error(cudaErrorMemoryAllocation, "cudaHostAlloc");
+    cudaStream_t st = (cudaStream_t)stream;
+    const GridDev g = make_grid_dev(grid);
+    const size_t row_bytes = sizeof(int64_t) * (size_t)n_cat * (size_t)grid->n_bins;
+
+    int64_t *sel_count = w.counters;                // [1 + n_cat]
+    int64_t *near = w.counters + 1 + n_cat;         // [n_cat]
+    const size_t n_counters = (size_t)(1 + 2 * n_cat);
+    const size_t n_read = n_cat == 1 ? 1 : n_counters;
+
+    GBFG_CUDA(cudaMemsetAsync(w.diff, 0, row_bytes, st));
+    GBFG_CUDA(cudaMemsetAsync(w.wide_flag, 0, sizeof(int), st));
+    GBFG_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(int64_t) * WS_COUNTERS, st));
+
+    bool done[GBFG_MAX_CAT];
+    for (int c = 0; c < n_cat; ++c) {
+        memset(&host_results[c], 0, sizeof(gbfg_iter_result));
+        host_results[c].n_candidates = ct.offsets[c + 1] - ct.offsets[c];
+        done[c] = false;
+    }
+    int n_done = 0;
+    for (int it = 0; it < params->max_iter && n_done < n_cat; ++it) {
+        rc = launch_median(dev_spectrum, grid->n_bins, n_cat, W, dev_median, dev_s_instr, dev_psd,
+                           params->median_norm, grid->scale_log2, nullptr, st);
+        if (rc) return rc;
+        if (n_cat == 1) GBFG_CUDA(cudaMemsetAsync(sel_count, 0, sizeof(int64_t) * 2, st));
+        else GBFG_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(int64_t) * n_counters, st));
+        rc = launch_snr_select(g, ct, dev_A, dev_f, dev_fdot, dev_psd, params->rho_th, dev_resolved, nullptr,
+                               nullptr, nullptr, n, w.sel_idx, sel_count, near, 1, w.inv_blocks, st);
+        if (rc) return rc;
+        GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read, cudaMemcpyDeviceToHost, st));
+        GBFG_CUDA(cudaStreamSynchronize(st));
+        const int64_t total = host[0];
+        for (int c = 0; c < n_cat; ++c) {
+            if (done[c]) continue;
+            const int64_t n_new = n_cat == 1 ? total : host[1 + c];
+            gbfg_iter_result &r = host_results[c];
+            if (it < GBFG_MAX_ITER_TRACE) r.n_new_per_iter[it] = n_new;
+            r.n_resolved += n_new;
+            if (n_cat > 1) r.n_near_threshold += host[1 + n_cat + c];
+            if (n_new == 0) { done[c] = true; ++n_done; r.n_iter = it + 1; r.converged = 1; }
+        }
+        if (total == 0) break;
+        rc = launch_deposit(g, ct, dev_A, dev_f, dev_fdot, w.sel_idx, sel_count, n, -1, dev_spectrum, nullptr,
+                            w.diff, w.tile_sums, w.wide_flag, st);
+        if (rc) return rc;
+    }
+    if (n_done < n_cat) {
+        // cap hit: the PSD must match the returned residual (rows of converged catalogs are unchanged)
+        for (int c = 0; c < n_cat; ++c)
+            if (!done[c]) { host_results[c].n_iter = params->max_iter; host_results[c].converged = 0; }
+        rc = launch_median(dev_spectrum, grid->n_bins, n_cat, W, dev_median, dev_s_instr, dev_psd,
+                           params->median_norm, grid->scale_log2, nullptr, st);
+        if (rc) return rc;
+    }
+    if (n_cat == 1) {
+        GBFG_CUDA(cudaMemcpyAsync(host, near, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
+        GBFG_CUDA(cudaStreamSynchronize(st));
+        host_results[0].n_near_threshold = host[0];
+    } else {
+        GBFG_CUDA(cudaStreamSynchronize(st));
+    }
+    return GBFG_OK;
+}
+
+extern "C" int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
+                             uint64_t seed, const double *dev_s_instr, const gbfg_iter_params *params,
+                             double *dev_A, double *dev_f, double *dev_fdot,
+                             int64_t *dev_total, int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
+                             uint8_t *dev_resolved, int64_t *dev_err_count, gbfg_iter_result *host_results,
+                             void *workspace, size_t workspace_bytes, void *stream)
+{
+    if (!valid_grid(grid) || !offsets || n_cat < 1 || !dev_spectrum || !dev_resolved) return GBFG_ERR_INVALID_ARG;
+    if (n_cat > GBFG_MAX_CAT) return GBFG_ERR_UNSUPPORTED;
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = gbfg_sample_catalog(grid, pops, offsets, n_cat, 0u, seed, dev_A, dev_f, dev_fdot, stream);
+    if (rc) return rc;
+    const int64_t n = offsets[n_cat];
+    const size_t row_bytes = sizeof(int64_t) * (size_t)n_cat * (size_t)grid->n_bins;
+    GBFG_CUDA(cudaMemsetAsync(dev_spectrum, 0, row_bytes, st));
+    if (n > 0) GBFG_CUDA(cudaMemsetAsync(dev_resolved, 0, (size_t)n, st));
+    rc = gbfg_deposit(grid, dev_A, dev_f, dev_fdot, offsets, n_cat, nullptr, nullptr, +1, dev_spectrum, dev_err_count,
+                      workspace, workspace_bytes, stream);
+    if (rc) return rc;
+    if (dev_total) GBFG_CUDA(cudaMemcpyAsync(dev_total, dev_spectrum, row_bytes, cudaMemcpyDeviceToDevice, st));
+    return gbfg_subtract_until_converged(grid, dev_A, dev_f, dev_fdot, offsets, n_cat, dev_s_instr, params,
+                                         dev_spectrum, dev_median, dev_psd, dev_resolved, host_results,
+                                         workspace, workspace_bytes, stream);
+}
+
+extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
+                                  uint64_t seed, const double *host_s_instr, const gbfg_iter_params *params,
+                                  double *host_psd, uint8_t *host_resolved, gbfg_iter_result *host_results)
+{
+    if (!valid_grid(grid) || !pops || !offsets || n_cat < 1 || !host_s_instr || !host_psd || !host_results)
+        return GBFG_ERR_INVALID_ARG;
+    if (n_cat > GBFG_MAX_CAT) return GBFG_ERR_UNSUPPORTED;
+    int rc = check_device();
+    if (rc) return rc;
+    const int64_t n = offsets[n_cat];
+    const size_t nb = (size_t)grid->n_bins, rows = (size_t)n_cat * nb;
+    const size_t ws_bytes = gbfg_workspace_bytes(grid, n, n_cat);
+    if (!ws_bytes) return GBFG_ERR_INVALID_ARG;
+    // one allocation, carved
+    size_t off = 0;
+    auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
+    const size_t nn = (size_t)(n > 0 ? n : 1);
+    const size_t oA = take(8 * nn), oF = take(8 * nn), oD = take(8 * nn);
+    const size_t oS = take(8 * rows), oM = take(8 * rows), oP = take(8 * rows), oI = take(8 * nb);
+    const size_t oR = take(nn), oW = take(ws_bytes);
+    char *base = nullptr;
+    cudaStream_t st = nullptr;
+    GBFG_CUDA(cudaMalloc((void **)&base, off));
+    cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
+    if (e != cudaSuccess) { cudaFree(base); return set_cuda_error(e, "cudaStreamCreate"); }
+    rc = GBFG_OK;
+    e = cudaMemcpyAsync(base + oI, host_s_instr, 8 * nb, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) rc = set_cuda_error(e, "cudaMemcpyAsync(s_instr)");
+    if (!rc)
+        rc = gbfg_simulate(grid, pops, offsets, n_cat, seed, (const double *)(base + oI), params,
+                           (double *)(base + oA), (double *)(base + oF), (double *)(base + oD), nullptr,
+                           (int64_t *)(base + oS), (int64_t *)(base + oM), (double *)(base + oP),
+                           (uint8_t *)(base + oR), nullptr, host_results, base + oW, ws_bytes, st);
+    if (!rc) {
+        e = cudaMemcpyAsync(host_psd, base + oP, 8 * rows, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && host_resolved && n > 0)
+            e = cudaMemcpyAsync(host_resolved, base + oR, (size_t)n, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) rc = set_cuda_error(e, "copy back");
+    }
+    cudaStreamSynchronize(st);
+    cudaStreamDestroy(st);
+    cudaFree(base);
+    return rc;
+}

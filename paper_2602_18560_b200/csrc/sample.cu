@@ -1,0 +1,326 @@
+// sample.cu — stage (i): Philox4x32-10 catalog sampling, and the instrument-noise helper.
+//
+// Follows DESIGN.md R1 (counter layout, draws) and §4 (elementary functions, operation by
+// operation).  The kernel is ALU-bound (two Philox blocks + 2 log + 3 exp10 + sincos + sqrt per
+// source against 24 bytes written); two sources per thread so that every store is 128 bits wide.
+#include "gbfg_common.cuh"
+
+namespace gbfg {
+
+// ------------------------------------------------------------------------------ DESIGN.md §4
+#define GB_SQRT_HALF 0.7071067811865476
+#define GB_LN2_HI 0.6931471803691238
+#define GB_LN2_LO 1.9082149292705877e-10
+#define GB_LOG10_E 0.4342944819032518
+#define GB_LN10 2.302585092994046
+#define GB_LOG2_10 3.321928094887362
+#define GB_LOG10_2_HI 0.3010299955494702
+#define GB_LOG10_2_LO 1.1451100898021838e-10
+#define GB_PIO2 1.5707963267948966
+#define GB_PIO2_HI 1.5707963267341256
+#define GB_PIO2_LO 6.077100506506192e-11
+#define GB_TWO_OVER_PI 0.6366197723675814
+#define GB_TWO_PI 6.283185307179586
+#define GB_LOG10_K 2.6090342225545732      /* log10((96/5) pi^(8/3)), eq. (4) */
+#define GB_LOG10_TSUN -5.3075504747653498  /* log10(G Msun / c^3 / 1 s) */
+
+__host__ __device__ inline double det_log(double x)
+{
+    int e;
+    double m = frexp(x, &e);
+    if (m < GB_SQRT_HALF) { m = 2.0 * m; e -= 1; }
+    double s = (m - 1.0) / (m + 1.0);
+    double z = s * s;
+    double q = 1.0 / 23.0;
+    q = fma(q, z, 1.0 / 21.0);
+    q = fma(q, z, 1.0 / 19.0);
+    q = fma(q, z, 1.0 / 17.0);
+    q = fma(q, z, 1.0 / 15.0);
+    q = fma(q, z, 1.0 / 13.0);
+    q = fma(q, z, 1.0 / 11.0);
+    q = fma(q, z, 1.0 / 9.0);
+    q = fma(q, z, 1.0 / 7.0);
+    q = fma(q, z, 1.0 / 5.0);
+    q = fma(q, z, 1.0 / 3.0);
+    double t = 2.0 * s;
+    double lm = fma(t * z, q, t);
+    double de = (double)e;
+    return de * GB_LN2_HI + fma(de, GB_LN2_LO, lm);
+}
+
+__host__ __device__ inline double det_exp_small(double t)
+{
+    double p = 1.0 / 87178291200.0;
+    p = fma(p, t, 1.0 / 6227020800.0);
+    p = fma(p, t, 1.0 / 479001600.0);
+    p = fma(p, t, 1.0 / 39916800.0);
+    p = fma(p, t, 1.0 / 3628800.0);
+    p = fma(p, t, 1.0 / 362880.0);
+    p = fma(p, t, 1.0 / 40320.0);
+    p = fma(p, t, 1.0 / 5040.0);
+    p = fma(p, t, 1.0 / 720.0);
+    p = fma(p, t, 1.0 / 120.0);
+    p = fma(p, t, 1.0 / 24.0);
+    p = fma(p, t, 1.0 / 6.0);
+    p = fma(p, t, 0.5);
+    return 1.0 + fma(t * t, p, t);
+}
+
+__host__ __device__ inline double det_exp10(double y)
+{
+    double k = rint(y * GB_LOG2_10);
+    double r = fma(-k, GB_LOG10_2_HI, y);
+    r = fma(-k, GB_LOG10_2_LO, r);
+    double t = r * GB_LN10;
+    return ldexp(det_exp_small(t), (int)k);
+}
+
+__host__ __device__ inline void det_sincos_small(double phi, double &sn, double &cs)
+{
+    double z = phi * phi;
+    double p = -1.0 / 121645100408832000.0;
+    p = fma(p, z, 1.0 / 355687428096000.0);
+    p = fma(p, z, -1.0 / 1307674368000.0);
+    p = fma(p, z, 1.0 / 6227020800.0);
+    p = fma(p, z, -1.0 / 39916800.0);
+    p = fma(p, z, 1.0 / 362880.0);
+    p = fma(p, z, -1.0 / 5040.0);
+    p = fma(p, z, 1.0 / 120.0);
+    p = fma(p, z, -1.0 / 6.0);
+    sn = fma(phi * z, p, phi);
+    double q = -1.0 / 6402373705728000.0;
+    q = fma(q, z, 1.0 / 20922789888000.0);
+    q = fma(q, z, -1.0 / 87178291200.0);
+    q = fma(q, z, 1.0 / 479001600.0);
+    q = fma(q, z, -1.0 / 3628800.0);
+    q = fma(q, z, 1.0 / 40320.0);
+    q = fma(q, z, -1.0 / 720.0);
+    q = fma(q, z, 1.0 / 24.0);
+    q = fma(q, z, -0.5);
+    cs = fma(z, q, 1.0);
+}
+
+__host__ __device__ inline void det_quadrant(int quad, double sn, double cs, double &s_out, double &c_out)
+{
+    switch (quad & 3) {
+    case 0: s_out = sn;  c_out = cs;  break;
+    case 1: s_out = cs;  c_out = -sn; break;
+    case 2: s_out = -sn; c_out = -cs; break;
+    default: s_out = -cs; c_out = sn; break;
+    }
+}
+
+__host__ __device__ inline void det_sincos2pi(double u, double &s_out, double &c_out)
+{
+    double t = 4.0 * u;
+    double n = rint(t);
+    double d = t - n;
+    double sn, cs;
+    det_sincos_small(d * GB_PIO2, sn, cs);
+    det_quadrant((int)n, sn, cs, s_out, c_out);
+}
+
+__host__ __device__ inline void det_sincos(double x, double &s_out, double &c_out)
+{
+    double n = rint(x * GB_TWO_OVER_PI);
+    double r = fma(-n, GB_PIO2_HI, x);
+    r = fma(-n, GB_PIO2_LO, r);
+    double sn, cs;
+    det_sincos_small(r, sn, cs);
+    det_quadrant((int)((long long)n & 3), sn, cs, s_out, c_out);
+}
+
+// ------------------------------------------------------------------------------ Philox4x32-10
+struct U4 { uint32_t x, y, z, w; };
+
+__device__ __forceinline__ U4 philox4x32_10(U4 c, uint32_t k0, uint32_t k1)
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        uint32_t hi0 = __umulhi(0xD2511F53u, c.x), lo0 = 0xD2511F53u * c.x;
+        uint32_t hi1 = __umulhi(0xCD9E8D57u, c.z), lo1 = 0xCD9E8D57u * c.z;
+        U4 n;
+        n.x = hi1 ^ c.y ^ k0;
+        n.y = lo1;
+        n.z = hi0 ^ c.w ^ k1;
+        n.w = lo0;
+        c = n;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    return c;
+}
+
+__device__ __forceinline__ double u01(uint32_t lo, uint32_t hi)
+{
+    uint64_t x = (((uint64_t)hi << 32) | (uint64_t)lo) >> 12;
+    return ((double)x + 0.5) * 0x1p-52;
+}
+
+// Per-catalog constants (host-computed with the same det_* functions, R1).
+struct PopDev {
+    double c0, c1, c2;          // frequency draw
+    int flat_in_log;
+    double logA_offset, logA_sigma, logMc_mean, logMc_sigma;
+    double f_min, f_max, f_top; // clamp
+    int64_t n_src;
+    uint32_t cat_id, key0, key1;
+};
+
+__device__ __forceinline__ void draw_source(const PopDev &P, int64_t i, double &A, double &f, double &fdot)
+{
+    U4 ctr;
+    ctr.x = (uint32_t)i; ctr.y = (uint32_t)((uint64_t)i >> 32); ctr.z = 0u; ctr.w = P.cat_id;
+    U4 b0 = philox4x32_10(ctr, P.key0, P.key1);
+    ctr.z = 1u;
+    U4 b1 = philox4x32_10(ctr, P.key0, P.key1);
+    double u_f = u01(b0.x, b0.y);
+    double u_1 = u01(b0.z, b0.w);
+    double u_2 = u01(b1.x, b1.y);
+    double lf;
+    if (P.flat_in_log) {
+        lf = P.c0 + u_f * P.c1;
+    } else {
+        double x = P.c0 + u_f * P.c1;
+        lf = (det_log(x) * GB_LOG10_E) * P.c2;
+    }
+    double fi = det_exp10(lf);
+    if (fi < P.f_min) fi = P.f_min;
+    if (fi >= P.f_max) fi = P.f_top;
+    double r = sqrt(-2.0 * det_log(u_1));
+    double sn, cs;
+    det_sincos2pi(u_2, sn, cs);
+    double z_A = r * cs;
+    double z_M = r * sn;
+    double t1 = lf + 3.0;
+    double t2 = (2.0 / 3.0) * t1;
+    double t3 = P.logA_offset + t2;
+    double t4 = P.logA_sigma * z_A;
+    A = det_exp10(t3 + t4);
+    double lmc = P.logMc_mean + P.logMc_sigma * z_M;
+    double m1 = (5.0 / 3.0) * (GB_LOG10_TSUN + lmc);
+    double m2 = (11.0 / 3.0) * lf;
+    fdot = det_exp10((GB_LOG10_K + m1) + m2);
+    f = fi;
+}
+
+// Two sources per thread, 128-bit stores.  Arrays are offset to the catalog's first source; the
+// pair (2t, 2t+1) is aligned when that offset is even, else a scalar path handles the ends.
+__global__ void __launch_bounds__(256)
+sample_kernel(PopDev P, double *__restrict__ A, double *__restrict__ f, double *__restrict__ fdot, int head)
+{
+    // sources [0, head) (0 or 1 of them) are done by thread 0 scalar so that the pairs are 16-byte aligned
+    int64_t n_pairs = (P.n_src - head) / 2;
+    int64_t tail = head + 2 * n_pairs;
+    int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t pr = t; pr < n_pairs; pr += stride) {
+        int64_t i = head + 2 * pr;
+        double a0, f0, d0, a1, f1, d1;
+        draw_source(P, i, a0, f0, d0);
+        draw_source(P, i + 1, a1, f1, d1);
+        *reinterpret_cast<double2 *>(A + i) = make_double2(a0, a1);
+        *reinterpret_cast<double2 *>(f + i) = make_double2(f0, f1);
+        *reinterpret_cast<double2 *>(fdot + i) = make_double2(d0, d1);
+    }
+    if (t == 0) {
+        for (int64_t i = 0; i < head; ++i) draw_source(P, i, A[i], f[i], fdot[i]);
+        for (int64_t i = tail; i < P.n_src; ++i) draw_source(P, i, A[i], f[i], fdot[i]);
+    }
+}
+
+// Robson et al. 2019 curve at bin centres (R3)
+__device__ __forceinline__ double robson_sn(double fq)
+{
+    const double L = 2.5e9, fstar = 19.09e-3;
+    double r2 = 2.0e-3 / fq;  r2 = r2 * r2;
+    double p_oms = (1.5e-11 * 1.5e-11) * (1.0 + r2 * r2);
+    double r4 = 0.4e-3 / fq;
+    double r8 = fq / 8.0e-3;  r8 = r8 * r8;
+    double p_acc = (3.0e-15 * 3.0e-15) * (1.0 + r4 * r4) * (1.0 + r8 * r8);
+    double x = fq / fstar;
+    double sn, cs;
+    det_sincos(x, sn, cs);
+    double y = GB_TWO_PI * fq;  y = y * y;  y = y * y;
+    double acc = 2.0 * (1.0 + cs * cs) * p_acc / y;
+    return (10.0 / (3.0 * L * L)) * (p_oms + acc) * (1.0 + 0.6 * (x * x));
+}
+
+__global__ void __launch_bounds__(256)
+instrument_noise_kernel(double f_min, double T, int64_t n_bins, double *__restrict__ s_instr)
+{
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (; k < n_bins; k += stride) {
+        double fk = f_min + ((double)k + 0.5) / T;
+        s_instr[k] = robson_sn(fk);
+    }
+}
+
+}  // namespace gbfg
+
+using namespace gbfg;
+
+extern "C" int gbfg_instrument_noise(const gbfg_grid *grid, double *dev_s_instr, void *stream)
+{
+    if (!grid || grid->struct_size != sizeof(gbfg_grid) || !dev_s_instr) return GBFG_ERR_INVALID_ARG;
+    int rc = check_device();
+    if (rc) return rc;
+    int blocks = (int)((grid->n_bins + 255) / 256);
+    int cap = sm_count() * 8;
+    if (blocks > cap) blocks = cap;
+    instrument_noise_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(grid->f_min, grid->t_obs, grid->n_bins, dev_s_instr);
+    GBFG_LAUNCH_CHECK("instrument_noise_kernel");
+    return GBFG_OK;
+}
+
+extern "C" int gbfg_sample_catalog(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets,
+                                   int32_t n_cat, uint32_t first_cat_id, uint64_t seed,
+                                   double *dev_A, double *dev_f, double *dev_fdot, void *stream)
+{
+    if (!grid || grid->struct_size != sizeof(gbfg_grid) || !pops || !offsets) return GBFG_ERR_INVALID_ARG;
+    if (n_cat < 1) return GBFG_ERR_INVALID_ARG;
+    if (n_cat > GBFG_MAX_CAT) return GBFG_ERR_UNSUPPORTED;
+    if (offsets[0] != 0) return GBFG_ERR_INVALID_ARG;
+    for (int c = 0; c < n_cat; ++c) {
+        if (pops[c].struct_size != sizeof(gbfg_pop) || pops[c].n_src < 0) return GBFG_ERR_INVALID_ARG;
+        if (offsets[c + 1] - offsets[c] != pops[c].n_src) return GBFG_ERR_INVALID_ARG;
+    }
+    if (offsets[n_cat] > 0 && (!dev_A || !dev_f || !dev_fdot)) return GBFG_ERR_INVALID_ARG;
+    if (((uintptr_t)dev_A | (uintptr_t)dev_f | (uintptr_t)dev_fdot) & 15) return GBFG_ERR_INVALID_ARG;
+    int rc = check_device();
+    if (rc) return rc;
+    const double lfmin = det_log(grid->f_min) * GB_LOG10_E;
+    const double lfmax = det_log(grid->f_max) * GB_LOG10_E;
+    for (int c = 0; c < n_cat; ++c) {
+        const gbfg_pop &p = pops[c];
+        if (p.n_src == 0) continue;
+        PopDev P;
+        double oms = 1.0 - p.slope;
+        P.flat_in_log = fabs(oms) < 1e-12;
+        if (P.flat_in_log) {
+            P.c0 = lfmin; P.c1 = lfmax - lfmin; P.c2 = 1.0;
+        } else {
+            double a = det_exp10(oms * lfmin);
+            double b = det_exp10(oms * lfmax);
+            P.c0 = a; P.c1 = b - a; P.c2 = 1.0 / oms;
+        }
+        P.logA_offset = p.logA_offset; P.logA_sigma = p.logA_sigma;
+        P.logMc_mean = p.logMc_mean; P.logMc_sigma = p.logMc_sigma;
+        P.f_min = grid->f_min; P.f_max = grid->f_max; P.f_top = nextafter(grid->f_max, 0.0);
+        P.n_src = p.n_src;
+        P.cat_id = first_cat_id + (uint32_t)c;
+        P.key0 = (uint32_t)seed; P.key1 = (uint32_t)(seed >> 32);
+        int head = (int)(offsets[c] & 1);                 // keep the pairs 16-byte aligned
+        if (head > p.n_src) head = (int)p.n_src;
+        int64_t n_pairs = (p.n_src - head) / 2;
+        int64_t blocks = (n_pairs + 255) / 256;
+        if (blocks < 1) blocks = 1;
+        int64_t cap = (int64_t)sm_count() * 16;
+        if (blocks > cap) blocks = cap;
+        sample_kernel<<<(int)blocks, 256, 0, (cudaStream_t)stream>>>(
+            P, dev_A + offsets[c], dev_f + offsets[c], dev_fdot + offsets[c], head);
+        GBFG_LAUNCH_CHECK("sample_kernel");
+    }
+    return GBFG_OK;
+}

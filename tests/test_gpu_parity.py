@@ -1,0 +1,367 @@
+"""Parity of the CUDA path (through the C ABI) with the oracle, stage by stage and for the whole loop.
+
+Bars (BASELINE.json:north_star): catalogs, spectra, medians, PSDs bit-exact; resolved sets identical
+(sources within 1e-9 of the threshold counted); fp64 SNR relative error <= 1e-12.
+All inputs are seeded and synthetic (gbfg_workloads).
+"""
+import numpy as np
+import pytest
+
+import gbfg_workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+RHO2_RTOL = 1e-12          # north_star: "fp64 SNR values: relative error <= 1e-12"
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch as t
+    return t
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def bits(a):
+    return np.ascontiguousarray(a).view(np.int64)
+
+
+def gpu_grid(gb, w):
+    return gb.grid_init(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+
+
+def workspace(torch, gb, g, n, n_cat=1):
+    return torch.empty(gb.workspace_bytes(g, n, n_cat), dtype=torch.uint8, device="cuda")
+
+
+# ------------------------------------------------------------------------------------- stage (i)
+@pytest.mark.parametrize("case", ["cfg0", "cfg1", "odd_offset_batch", "slopes"])
+def test_sample_catalog_bit_exact(gb, orc, torch, case):
+    if case == "cfg0":
+        w = wl.config(0)
+    elif case == "cfg1":
+        w = wl.config(1)
+    elif case == "odd_offset_batch":      # odd catalog sizes: unaligned pair path, several catalogs
+        w = wl.scaled(wl.config(4), n_cat=5)
+        w = wl.replace(w, pops=[wl.replace(p, n_src=1001 + 2 * i + (i % 2)) for i, p in enumerate(w.pops)])
+    else:                                 # slope == 1 (log-uniform branch) and slopes near it
+        w = wl.config(2)
+        w = wl.replace(w, pops=[wl.replace(w.pops[0], slope=s, n_src=5000) for s in (1.0, 1.0 + 1e-13, 1.2, 2.0)])
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    assert g.n_bins == og.n_bins
+    off = w.offsets()
+    n = int(off[-1])
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    gb.sample_catalog(g, w.pops, off, w.seed, A, f, fd)
+    A, f, fd = A.cpu().numpy(), f.cpu().numpy(), fd.cpu().numpy()
+    for c, p in enumerate(w.pops):
+        oA, of, ofd = orc.sample_catalog(og, p, c, w.seed)
+        s = slice(int(off[c]), int(off[c + 1]))
+        assert np.array_equal(bits(A[s]), bits(oA))
+        assert np.array_equal(bits(f[s]), bits(of))
+        assert np.array_equal(bits(fd[s]), bits(ofd))
+
+
+def test_sample_catalog_pieces(gb, orc, torch):
+    """first_cat_id lets a batch be drawn in pieces: catalog 3 alone == catalog 3 of the batch."""
+    w = wl.scaled(wl.config(4), n_cat=4, n_src=777)
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    A, f, fd = (torch.empty(777, dtype=torch.float64, device="cuda") for _ in range(3))
+    gb.sample_catalog(g, [w.pops[3]], [0, 777], w.seed, A, f, fd, first_cat_id=3)
+    oA, of, ofd = orc.sample_catalog(og, w.pops[3], 3, w.seed)
+    assert np.array_equal(bits(A.cpu().numpy()), bits(oA))
+    assert np.array_equal(bits(fd.cpu().numpy()), bits(ofd))
+
+
+@pytest.mark.parametrize("cfg", [0, 2])
+def test_instrument_noise_bit_exact(gb, orc, torch, cfg):
+    w = wl.config(cfg)
+    g = gpu_grid(gb, w)
+    s = torch.empty(g.n_bins, dtype=torch.float64, device="cuda")
+    gb.instrument_noise(g, s)
+    ref = orc.instrument_noise(orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2))
+    assert np.array_equal(bits(s.cpu().numpy()), bits(ref))
+
+
+# ------------------------------------------------------------------------------------ stage (ii)
+def _deposit_both(gb, orc, torch, w, A, f, fd, sel=None, sign=1, start=None):
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    n = A.size
+    spec0 = np.zeros(og.n_bins, dtype=np.int64) if start is None else start.copy()
+    ref = spec0.copy()
+    rej_ref = orc.deposit(og, A, f, fd, ref, sel=sel, sign=sign)
+    d_spec = dev(torch, spec0)
+    err = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ws = workspace(torch, gb, g, n)
+    kw = {}
+    if sel is not None:
+        kw = dict(dev_sel_idx=dev(torch, np.append(np.asarray(sel, dtype=np.int64), 0)),   # capacity >= 1
+                  dev_sel_count=dev(torch, np.array([len(sel)], dtype=np.int64)))
+    gb.deposit(g, dev(torch, A), dev(torch, f), dev(torch, fd), [0, n], d_spec, ws, sign=sign, dev_err_count=err, **kw)
+    return d_spec.cpu().numpy(), ref, int(err.item()), rej_ref
+
+
+@pytest.mark.parametrize("kind", ["narrow", "wide", "bad", "edges", "dupes"])
+@pytest.mark.parametrize("cfg", [0, 2])
+def test_deposit_handmade_bit_exact(gb, orc, torch, kind, cfg):
+    w = wl.config(cfg)
+    A, f, fd = wl.handmade_catalog(kind, w, n=3000, seed=7 + cfg)
+    got, ref, err, rej = _deposit_both(gb, orc, torch, w, A, f, fd)
+    assert np.array_equal(got, ref)
+    assert err == rej
+    if kind == "bad":
+        assert rej > 0
+
+
+@pytest.mark.parametrize("cfg,n", [(0, None), (1, None), (2, 200_000)])
+def test_deposit_catalog_and_subtract(gb, orc, torch, cfg, n):
+    w = wl.config(cfg)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    pop = w.pops[0] if n is None else wl.replace(w.pops[0], n_src=n)
+    A, f, fd = orc.sample_catalog(og, pop, 0, w.seed)
+    got, ref, err, rej = _deposit_both(gb, orc, torch, w, A, f, fd)
+    assert np.array_equal(got, ref) and err == rej == 0
+    # subtract a subset (stage v form: index list + device count), incl. duplicates of wide sources
+    rng = np.random.default_rng(5)
+    sel = rng.choice(A.size, size=A.size // 7, replace=False).astype(np.int64)
+    got2, ref2, _, _ = _deposit_both(gb, orc, torch, w, A, f, fd, sel=sel, sign=-1, start=ref)
+    assert np.array_equal(got2, ref2)
+    # empty selection leaves the spectrum untouched
+    got3, ref3, _, _ = _deposit_both(gb, orc, torch, w, A, f, fd, sel=np.zeros(0, dtype=np.int64), sign=-1, start=ref)
+    assert np.array_equal(got3, ref)
+    # +1 then -1 of everything is exactly zero
+    got4, _, _, _ = _deposit_both(gb, orc, torch, w, A, f, fd, sign=-1, start=ref)
+    assert not got4.any()
+
+
+def test_deposit_empty_catalog(gb, torch):
+    w = wl.config(0)
+    g = gpu_grid(gb, w)
+    spec = torch.zeros(g.n_bins, dtype=torch.int64, device="cuda")
+    e = torch.empty(0, dtype=torch.float64, device="cuda")
+    gb.deposit(g, e, e, e, [0, 0], spec, workspace(torch, gb, g, 0))
+    assert not spec.any().item()
+
+
+# ----------------------------------------------------------------------------------- stage (iii)
+@pytest.mark.parametrize("kind", ["lognormal", "dupes", "zeros", "full64", "ramp", "const"])
+@pytest.mark.parametrize("n,window", [(20011, 1001), (30000, 2001), (9000, 4097), (7000, 3), (6193, 2001),
+                                      (6192, 2001), (1001, 2001), (501, 1001), (12500, 101), (8190, 1), (40000, 33)])
+def test_running_median_bit_exact(gb, orc, torch, kind, n, window):
+    x = wl.random_spectrum(n, seed=n + window, kind=kind)
+    ref = orc.running_median(x, window)
+    out = torch.empty(n, dtype=torch.int64, device="cuda")
+    gb.running_median(dev(torch, x), n, 1, window, out)
+    assert np.array_equal(out.cpu().numpy(), ref)
+
+
+def test_running_median_batch_rows(gb, orc, torch):
+    n, window = 15000, 1001
+    rows = [wl.random_spectrum(n, seed=100 + r, kind=k) for r, k in enumerate(["lognormal", "zeros", "full64"])]
+    x = np.stack(rows)
+    out = torch.empty((3, n), dtype=torch.int64, device="cuda")
+    gb.running_median(dev(torch, x), n, 3, window, out)
+    got = out.cpu().numpy()
+    for r in range(3):
+        assert np.array_equal(got[r], orc.running_median(rows[r], window))
+
+
+def test_psd_bit_exact(gb, orc, torch):
+    w = wl.config(0)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    s_instr = orc.instrument_noise(og)
+    med = wl.random_spectrum(og.n_bins, seed=3, kind="zeros")
+    for norm in (1.0, wl.MEDIAN_NORM_PAPER):
+        ref = orc.psd_from_median(med, s_instr, norm, w.scale_log2)
+        out = torch.empty(og.n_bins, dtype=torch.float64, device="cuda")
+        gb.psd(dev(torch, med), dev(torch, s_instr), og.n_bins, 1, norm, w.scale_log2, out)
+        assert np.array_equal(bits(out.cpu().numpy()), bits(ref))
+
+
+# ------------------------------------------------------------------------------------ stage (iv)
+def _snr_case(gb, orc, torch, w, A, f, fd, rho_th, resolved0=None):
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    n = A.size
+    s_instr = orc.instrument_noise(og)
+    spec = np.zeros(og.n_bins, dtype=np.int64)
+    orc.deposit(og, A, f, fd, spec)
+    psd = orc.psd_from_median(orc.running_median(spec, w.window), s_instr, w.median_norm, w.scale_log2)
+    res_ref = np.zeros(n, dtype=np.uint8) if resolved0 is None else resolved0.copy()
+    res_gpu = dev(torch, res_ref)
+    sel_ref, r2_ref, near_ref = orc.snr_select(og, A, f, fd, psd, rho_th, res_ref)
+    r2 = torch.full((n,), -1.0, dtype=torch.float64, device="cuda")
+    sel = torch.empty(max(n, 1), dtype=torch.int64, device="cuda")
+    cnt = torch.empty(2, dtype=torch.int64, device="cuda")
+    near = torch.zeros(1, dtype=torch.int64, device="cuda")
+    gb.snr_select(g, dev(torch, A), dev(torch, f), dev(torch, fd), [0, n], dev(torch, psd), rho_th, res_gpu, sel, cnt,
+                  workspace(torch, gb, g, n), dev_rho2_out=r2, dev_near_count=near)
+    cnt = cnt.cpu().numpy()
+    got_sel = np.sort(sel.cpu().numpy()[: cnt[0]])
+    r2 = r2.cpu().numpy()
+    tested = (np.zeros(n, dtype=np.uint8) if resolved0 is None else resolved0) == 0
+    # untested entries untouched, rejected sources NaN on both sides
+    assert np.all(r2[~tested] == -1.0)
+    assert np.array_equal(np.isnan(r2[tested]), np.isnan(r2_ref[tested]))
+    okm = tested & ~np.isnan(r2_ref)
+    rel = np.abs(r2[okm] - r2_ref[okm]) / np.maximum(np.abs(r2_ref[okm]), 1e-300)
+    assert rel.size == 0 or rel.max() <= RHO2_RTOL, rel.max()
+    assert cnt[0] == cnt[1] == sel_ref.size
+    assert np.array_equal(got_sel, sel_ref)                    # identical resolved set
+    assert np.array_equal(res_gpu.cpu().numpy(), res_ref)
+    assert int(near.item()) == near_ref
+    return rel.max() if rel.size else 0.0, near_ref
+
+
+@pytest.mark.parametrize("cfg,n", [(0, None), (1, None), (2, 300_000)])
+def test_snr_select_catalog(gb, orc, torch, cfg, n):
+    w = wl.config(cfg)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    pop = w.pops[0] if n is None else wl.replace(w.pops[0], n_src=n)
+    A, f, fd = orc.sample_catalog(og, pop, 0, w.seed)
+    rng = np.random.default_rng(9)
+    resolved0 = (rng.random(A.size) < 0.1).astype(np.uint8)
+    _snr_case(gb, orc, torch, w, A, f, fd, w.rho_th)
+    _snr_case(gb, orc, torch, w, A, f, fd, w.rho_th, resolved0=resolved0)
+    _snr_case(gb, orc, torch, w, A, f, fd, float("inf"))
+    _snr_case(gb, orc, torch, w, A, f, fd, 1e-30)
+
+
+@pytest.mark.parametrize("kind", ["narrow", "wide", "bad", "edges", "dupes"])
+def test_snr_select_handmade(gb, orc, torch, kind):
+    w = wl.config(2)
+    A, f, fd = wl.handmade_catalog(kind, w, n=2000, seed=21)
+    _snr_case(gb, orc, torch, w, A, f, fd, w.rho_th)
+
+
+def test_snr_threshold_decisions_on_the_definition(gb, orc, torch):
+    """Wide sources whose rho^2 sits within rounding of the threshold: the decision is the oracle's."""
+    w = wl.config(2)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    A, f, fd = wl.handmade_catalog("wide", w, n=400, seed=33)
+    s_instr = orc.instrument_noise(og)
+    spec = np.zeros(og.n_bins, dtype=np.int64)
+    orc.deposit(og, A, f, fd, spec)
+    psd = orc.psd_from_median(orc.running_median(spec, w.window), s_instr, w.median_norm, w.scale_log2)
+    # rescale every amplitude so that its own rho^2 lands within a few ulp of 49
+    r2 = np.array([orc.rho2(og, A[i], f[i], fd[i], psd) for i in range(A.size)])
+    ok = ~np.isnan(r2) & (r2 > 0)
+    A2 = A.copy()
+    A2[ok] = A[ok] * np.sqrt(49.0 / r2[ok]) * (1.0 + np.random.default_rng(1).integers(-3, 4, ok.sum()) * 1.1e-16)
+    _, near = _snr_case(gb, orc, torch, w, A2, f, fd, 7.0)
+    assert near >= ok.sum() // 2
+
+
+# ------------------------------------------------------------------------------- the whole loop
+def _loop_case(gb, orc, torch, w, max_iter=None, rho_th=None, check_host=False):
+    max_iter = w.max_iter if max_iter is None else max_iter
+    rho_th = w.rho_th if rho_th is None else rho_th
+    w = wl.replace(w, max_iter=max_iter, rho_th=rho_th)
+    ref = orc.simulate(w)
+    g = gpu_grid(gb, w)
+    n, nb = w.n_src_total, g.n_bins
+    s_instr = dev(torch, ref["s_instr"])
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    total, spec, med = (torch.empty(nb, dtype=torch.int64, device="cuda") for _ in range(3))
+    psd = torch.empty(nb, dtype=torch.float64, device="cuda")
+    resolved = torch.empty(n, dtype=torch.uint8, device="cuda")
+    err = torch.zeros(1, dtype=torch.int64, device="cuda")
+    params = gb.make_iter_params(w.window, w.median_norm, rho_th, max_iter)
+    res = gb.simulate(g, w.pops, w.offsets(), w.seed, s_instr, params, A, f, fd, total, spec, med, psd, resolved,
+                      workspace(torch, gb, g, n), dev_err_count=err)[0]
+    assert np.array_equal(bits(A.cpu().numpy()), bits(ref["A"]))
+    assert np.array_equal(total.cpu().numpy(), ref["total"])              # deposited spectrum: bit-exact
+    assert np.array_equal(spec.cpu().numpy(), ref["residual"])            # residual: bit-exact
+    assert np.array_equal(med.cpu().numpy(), ref["median"])               # median: bit-exact
+    assert np.array_equal(bits(psd.cpu().numpy()), bits(ref["psd"]))      # final PSD: bit-exact
+    assert np.array_equal(resolved.cpu().numpy(), ref["resolved"])        # resolved set: identical
+    assert (res.n_iter, res.converged, res.n_resolved) == (ref["n_iter"], ref["converged"], ref["n_resolved"])
+    assert res.n_near_threshold == ref["n_near_threshold"]
+    k = min(ref["n_iter"], gb.MAX_ITER_TRACE)
+    assert list(res.n_new_per_iter[:k]) == list(ref["n_new_per_iter"][:k])
+    assert int(err.item()) == ref["rejected"]
+    if check_host:
+        hp = np.empty(nb, dtype=np.float64)
+        hr = np.empty(n, dtype=np.uint8)
+        res2 = gb.simulate_host(g, w.pops, w.offsets(), w.seed, ref["s_instr"], params, hp, hr)[0]
+        assert np.array_equal(bits(hp), bits(ref["psd"])) and np.array_equal(hr, ref["resolved"])
+        assert res2.n_iter == ref["n_iter"]
+    return ref
+
+
+def test_loop_config0(gb, orc, torch):
+    _loop_case(gb, orc, torch, wl.config(0), check_host=True)
+
+
+def test_loop_config1(gb, orc, torch):
+    _loop_case(gb, orc, torch, wl.config(1))
+
+
+def test_loop_dense_short(gb, orc, torch):
+    ref = _loop_case(gb, orc, torch, wl.dense_case("short"))
+    assert ref["n_iter"] >= 4
+
+
+def test_loop_dense_long(gb, orc, torch):
+    ref = _loop_case(gb, orc, torch, wl.dense_case("long"))
+    assert ref["n_iter"] >= 10
+
+
+def test_loop_degenerate_thresholds_and_cap(gb, orc, torch):
+    w = wl.config(0)
+    ref = _loop_case(gb, orc, torch, w, rho_th=float("inf"))
+    assert ref["n_iter"] == 1 and ref["n_resolved"] == 0
+    ref = _loop_case(gb, orc, torch, w, rho_th=1e-30)
+    assert not ref["residual"].any()
+    ref = _loop_case(gb, orc, torch, wl.dense_case("short"), max_iter=1)       # cap branch
+    assert ref["converged"] == 0
+    ref = _loop_case(gb, orc, torch, wl.dense_case("short"), max_iter=3)
+    assert ref["converged"] == 0 and ref["n_iter"] == 3
+
+
+@pytest.mark.slow
+def test_loop_config2_full(gb, orc, torch):
+    ref = _loop_case(gb, orc, torch, wl.config(2))
+    assert ref["n_iter"] > 10
+
+
+@pytest.mark.slow
+def test_loop_config3_full(gb, orc, torch):
+    """The headline workload, in the launch configuration bench.py times."""
+    _loop_case(gb, orc, torch, wl.config(3))
+
+
+def test_loop_batch_matches_per_catalog_oracle(gb, orc, torch):
+    """configs[4] in miniature: ragged catalogs with different Lambda iterate independently."""
+    w = wl.scaled(wl.config(4), n_cat=4)
+    w = wl.replace(w, pops=[wl.replace(p, n_src=n) for p, n in zip(w.pops, (60_000, 25_001, 90_000, 40_003))])
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    n, nb, nc = w.n_src_total, g.n_bins, w.n_cat
+    s_instr_h = orc.instrument_noise(og)
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    total, spec, med = (torch.empty((nc, nb), dtype=torch.int64, device="cuda") for _ in range(3))
+    psd = torch.empty((nc, nb), dtype=torch.float64, device="cuda")
+    resolved = torch.empty(n, dtype=torch.uint8, device="cuda")
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter)
+    res = gb.simulate(g, w.pops, w.offsets(), w.seed, dev(torch, s_instr_h), params, A, f, fd, total, spec, med, psd,
+                      resolved, workspace(torch, gb, g, n, nc))
+    off = w.offsets()
+    iters = set()
+    for c in range(nc):
+        ref = orc.simulate(w, cat=c)
+        s = slice(int(off[c]), int(off[c + 1]))
+        assert np.array_equal(total[c].cpu().numpy(), ref["total"])
+        assert np.array_equal(spec[c].cpu().numpy(), ref["residual"])
+        assert np.array_equal(med[c].cpu().numpy(), ref["median"])
+        assert np.array_equal(bits(psd[c].cpu().numpy()), bits(ref["psd"]))
+        assert np.array_equal(resolved[s].cpu().numpy(), ref["resolved"])
+        assert (res[c].n_iter, res[c].converged, res[c].n_resolved) == (ref["n_iter"], ref["converged"], ref["n_resolved"])
+        assert res[c].n_near_threshold == ref["n_near_threshold"]
+        iters.add(ref["n_iter"])
+    assert len(iters) > 1          # the catalogs really stop at different iterations
