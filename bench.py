@@ -1,0 +1,335 @@
+#!/usr/bin/env python
+"""bench.py — catalog -> converged foreground on B200 (BASELINE.json:metric, configs[3]).
+
+One "step" = one pass of the whole hot path (sample -> deposit -> [median+PSD ->
+SNR+select -> subtract] until converged or capped) over one 1e7-source, 4-yr synthetic catalog,
+through the C ABI (gbfg_simulate).  Prints ONE JSON line (see the task contract):
+  value      sources/s with every buffer resident in HBM (the catalog is drawn on the device by stage i)
+  e2e        the same through gbfg_simulate_host: host buffers, H2D/D2H inside the timed region
+  roofline   the dominant kernel's algorithmic bytes / CUDA-event time against MEASURED_PEAKS.json
+  kernels    the same for every kernel class (events recorded on the launching stream, live)
+  cpu_baseline  the oracle, as it stands, on the host cores, on a bounded sample
+
+`--impl reference` times the oracle alone (rank 0 only) and prints its own line.
+N > 1 (torchrun): every rank runs its own independent catalog (seed + rank); no data-path
+collective; value = all ranks' sources / max-over-ranks time; scaling "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+import gbfg_workloads as wl
+
+METRIC = "catalog_to_foreground_throughput"
+UNIT = "sources/s"
+CPU_SAMPLE_SOURCES = 1_000_000      # bounded oracle sample: the first 1e6 sources of the config-3 catalog
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+# ------------------------------------------------------------------------------------ clocks
+class ClockSampler:
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0])); mx.append(float(parts[1])); pw.append(float(parts[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, parts[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------- reference arm
+def oracle_sample_run(w: wl.Workload, n_src: int):
+    """The oracle, as it stands, on the first n_src sources of workload w's catalog, whole path."""
+    import oracle
+    oracle.build()
+    oracle.lib()
+    t0 = time.perf_counter()
+    out = oracle.simulate(w, cat=0, n_src=n_src)
+    dt = time.perf_counter() - t0
+    return dt, out
+
+
+def run_reference(args, w: wl.Workload):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    n_s = min(CPU_SAMPLE_SOURCES, w.n_src_total)
+    sample = (f"{w.name}: first {n_s} of {w.n_src_total} sources of the seeded catalog on the full grid "
+              f"(window {w.window}, cap {w.max_iter}), whole path sample->deposit->loop, 1 thread")
+    for _ in range(args.warmup):
+        pass        # the oracle has no warm-up state; warm-up steps are not run (minutes each)
+    times, iters = [], None
+    for _ in range(args.steps):
+        dt, out = oracle_sample_run(w, n_s)
+        times.append(dt)
+        iters = int(out["n_iter"])
+    t = float(np.mean(times))
+    val = n_s / t
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64+i64", "data": "synthetic",
+        "config": {"workload": w.name, "sample": sample, "n_iter": iters},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------ GPU arm
+def algorithmic_bytes(w: wl.Workload, n_bins: int, res, prof) -> dict:
+    """Algorithmic bytes of ONE step per kernel class: what the method itself
+    must move, not what the implementation happens to move."""
+    n = w.n_src_total
+    n_iter = res.n_iter
+    trace = [int(res.n_new_per_iter[i]) for i in range(min(n_iter, 64))]
+    n_sub = sum(trace)
+    n_med = prof["median"][0]
+    n_snr = prof["snr"][0]
+    n_dep = prof["deposit"][0]
+    n_scan = prof["scan"][0]
+    return {
+        "sample": 24 * n,                                   # 24 B written per source
+        "deposit": 24 * n + 32 * n_sub,                     # catalog read once; 8 B index + 24 B per subtracted source
+        "scan": 16 * n_bins * n_scan,                       # spectrum read + written per range-update pass
+        "median": 32 * n_bins * n_med,                      # spectrum in, median out, s_instr in, PSD out
+        "inv_blocks": 8 * n_bins * prof["inv_blocks"][0],   # PSD read once per pass
+        "snr": 25 * res.n_candidates * max(n_snr - 1, 0) + 25 * n,   # 24 B + flag per tested source
+        "_counts": {"n_iter": n_iter, "n_sub": n_sub, "n_dep": n_dep},
+    }
+
+
+def run_gpu(args, w: wl.Workload):
+    import torch
+    import paper_2602_18560_b200 as gb
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: libgbfg has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    gb.load()
+    dev = torch.device("cuda", local)
+    w = wl.replace(w, seed=w.seed + 1000 * rank)           # independent catalogs, one per rank
+    g = gb.grid_init(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    n, nb, nc = w.n_src_total, g.n_bins, w.n_cat
+    off = w.offsets()
+
+    s_instr = torch.empty(nb, dtype=torch.float64, device=dev)
+    gb.instrument_noise(g, s_instr)
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device=dev) for _ in range(3))
+    spec, med = (torch.empty((nc, nb), dtype=torch.int64, device=dev) for _ in range(2))
+    psd = torch.empty((nc, nb), dtype=torch.float64, device=dev)
+    resolved = torch.empty(n, dtype=torch.uint8, device=dev)
+    ws = torch.empty(gb.workspace_bytes(g, n, nc), dtype=torch.uint8, device=dev)
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter, args.flags)
+
+    def step():
+        return gb.simulate(g, w.pops, off, w.seed, s_instr, params, A, f, fd, None, spec, med, psd, resolved, ws)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 0)):
+        step()
+    barrier()
+
+    # ---- device-resident timing (value), per-kernel events live in the same region
+    clocks = ClockSampler(local)
+    clocks.start()
+    gb.profile_enable(True)
+    launches0 = gb.kernel_launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        res = step()
+    e1.record()
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    launches = gb.kernel_launch_count() - launches0
+    prof = gb.profile_read()
+    gb.profile_enable(False)
+    clk = clocks.stop()
+    if dist is not None:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * n / (ms_step * 1e-3)
+
+    # ---- the same region without the per-kernel events (cross-check that the events cost nothing)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    ms_step_noprof = e0.elapsed_time(e1) / args.steps
+
+    # ---- end to end through the host-buffer entry point
+    h_s = s_instr.cpu().pin_memory()
+    h_psd = torch.empty((nc, nb), dtype=torch.float64).pin_memory()
+    h_res = torch.empty(n, dtype=torch.uint8).pin_memory()
+    e2e_steps = max(1, min(args.steps, args.e2e_steps))
+    gb.simulate_host(g, w.pops, off, w.seed, h_s.numpy(), params, h_psd.numpy(), h_res.numpy())
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        gb.simulate_host(g, w.pops, off, w.seed, h_s.numpy(), params, h_psd.numpy(), h_res.numpy())
+    torch.cuda.synchronize()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    if dist is not None:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    same_psd = bool(torch.equal(h_psd.view(torch.int64), psd.cpu().view(torch.int64)))
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- roofline of every kernel class, and of the dominant one
+    peak, peak_src = measured_peaks()
+    r0 = res[0]
+    ab = algorithmic_bytes(w, nb, r0, {k: (v[0] // args.steps, v[1], v[2]) for k, v in prof.items()})
+    kernels = {}
+    for k, (cnt, tot, mx) in prof.items():
+        if cnt == 0:
+            continue
+        per_step_ms = tot / args.steps
+        gbs = ab.get(k, 0) / (per_step_ms * 1e-3) / 1e9 if per_step_ms > 0 else 0.0
+        kernels[k] = {"launches_per_step": cnt / args.steps, "ms_per_step": per_step_ms, "avg_launch_ms": tot / cnt,
+                      "max_launch_ms": mx, "algorithmic_bytes_per_step": ab.get(k, 0), "achieved_gbs": gbs,
+                      "frac_of_hbm": gbs / peak, "share_of_step": per_step_ms / ms_step}
+    dom = max(kernels, key=lambda k: kernels[k]["ms_per_step"])
+    kd = kernels[dom]
+    bytes_per_launch = kd["algorithmic_bytes_per_step"] / kd["launches_per_step"]
+    roofline = {"kernel": dom, "bound": "hbm", "achieved": bytes_per_launch / (kd["avg_launch_ms"] * 1e-3) / 1e9,
+                "peak": peak, "peak_source": peak_src, "unit": "GB/s",
+                "frac": bytes_per_launch / (kd["avg_launch_ms"] * 1e-3) / 1e9 / peak,
+                "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_ms": kd["avg_launch_ms"],
+                "traffic": args.traffic}
+
+    # ---- the oracle on the host cores, bounded sample
+    cpu = None
+    if not args.no_cpu_baseline:
+        n_s = min(CPU_SAMPLE_SOURCES, n)
+        dt, out = oracle_sample_run(wl.replace(w, seed=w.seed), n_s)
+        cpu = {"value": n_s / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
+               "sample": f"first {n_s} of {n} sources of the same seeded catalog on the full grid, whole path "
+                         f"(sample->deposit->loop, {int(out['n_iter'])} iterations), 1 thread of "
+                         f"{os.cpu_count()} host cores"}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64+i64", "data": "synthetic",
+        "config": {"workload": w.name, "n_src": n, "n_cat": nc, "n_bins": nb, "window": w.window, "rho_th": w.rho_th,
+                   "max_iter": w.max_iter, "t_obs_s": w.t_obs, "band_hz": [w.f_min, w.f_max], "seed": w.seed,
+                   "n_iter": r0.n_iter, "converged": r0.converged, "n_resolved": r0.n_resolved,
+                   "n_near_threshold": r0.n_near_threshold, "flags": args.flags,
+                   "l2": "inputs larger than L2: every step redraws and re-reads the 240 MB catalog (126 MB L2)",
+                   "wall_time_s": ms_step * 1e-3},
+        "ms_per_step_without_kernel_events": ms_step_noprof,
+        "e2e": {"value": world * n / e2e_s, "unit": UNIT, "ms_per_step": 1e3 * e2e_s, "steps": e2e_steps,
+                "h2d_bytes_per_step": 8 * nb, "d2h_bytes_per_step": 8 * nc * nb + n, "psd_equal_to_device_run": same_psd},
+        "gpu_launches": int(launches),
+        "clocks": clk,
+        "roofline": roofline,
+        "kernels": kernels,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="gbfg", choices=["gbfg", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (default 3: the headline 1e7-source run)")
+    ap.add_argument("--n-src", type=int, default=None, help="override the number of sources (parity/debug only)")
+    ap.add_argument("--flags", type=int, default=0, help="gbfg_iter_params.flags")
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per launch of the dominant kernel from the committed ncu --set full capture")
+    args = ap.parse_args()
+    w = wl.config(args.config)
+    if args.n_src is not None:
+        w = wl.scaled(w, n_src=args.n_src, name=f"{w.name}_n{args.n_src}")
+    if args.impl == "reference":
+        return run_reference(args, w)
+    return run_gpu(args, w)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

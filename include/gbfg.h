@@ -193,6 +193,32 @@ size_t gbfg_workspace_bytes(const gbfg_grid *grid, int64_t n_src_total, int32_t 
 /* Number of kernels the calling thread's library calls have launched so far (for bench.py). */
 int64_t gbfg_kernel_launch_count(void);
 
+/* Measurement helper (bench.py's roofline leg).  While enabled for the calling
+ * thread, every kernel the library launches is bracketed by a pair of CUDA events recorded on the
+ * stream the kernel is launched on.  gbfg_profile_read waits for those events, fills
+ * out[GBFG_K_*] (HOST, n_out >= GBFG_K_COUNT) with the number of timed launches of each kernel
+ * class and their summed / largest device time in milliseconds, and clears the record.
+ * Costs two event records per launch; off by default. */
+enum {
+    GBFG_K_SAMPLE = 0,      /* sample_kernel                      stage (i)   */
+    GBFG_K_NOISE,           /* instrument_noise_kernel            helper      */
+    GBFG_K_DEPOSIT,         /* deposit kernels                    stage (ii)/(v) */
+    GBFG_K_SCAN,            /* difference-array scan kernels      stage (ii)/(v) */
+    GBFG_K_MEDIAN,          /* running median (+ fused PSD)       stage (iii) */
+    GBFG_K_PSD,             /* psd_kernel                         stage (iii) */
+    GBFG_K_INV_BLOCKS,      /* block sums of 1/psd                stage (iv)  */
+    GBFG_K_SNR,             /* SNR + select kernels               stage (iv)  */
+    GBFG_K_AUX,             /* small bookkeeping kernels                      */
+    GBFG_K_COUNT
+};
+typedef struct gbfg_kernel_time {
+    int64_t launches;
+    double total_ms;
+    double max_ms;
+} gbfg_kernel_time;
+int gbfg_profile_enable(int on);
+int gbfg_profile_read(gbfg_kernel_time *out, int32_t n_out);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,8 +23,10 @@ EXPORTS = [
     "gbfg_version", "gbfg_strerror", "gbfg_last_cuda_error", "gbfg_grid_init", "gbfg_instrument_noise",
     "gbfg_sample_catalog", "gbfg_deposit", "gbfg_running_median", "gbfg_psd", "gbfg_snr_select",
     "gbfg_subtract_until_converged", "gbfg_simulate", "gbfg_simulate_host", "gbfg_workspace_bytes",
-    "gbfg_kernel_launch_count",
+    "gbfg_kernel_launch_count", "gbfg_profile_enable", "gbfg_profile_read",
 ]
+
+KERNEL_CLASSES = ["sample", "noise", "deposit", "scan", "median", "psd", "inv_blocks", "snr", "aux"]
 
 
 class GbfgError(RuntimeError):
@@ -53,6 +55,10 @@ class IterResult(C.Structure):
     _fields_ = [("n_iter", C.c_int32), ("converged", C.c_int32), ("n_resolved", C.c_int64),
                 ("n_near_threshold", C.c_int64), ("n_candidates", C.c_int64),
                 ("n_new_per_iter", C.c_int64 * MAX_ITER_TRACE)]
+
+
+class KernelTime(C.Structure):
+    _fields_ = [("launches", C.c_int64), ("total_ms", C.c_double), ("max_ms", C.c_double)]
 
 
 _lib = None
@@ -85,6 +91,8 @@ def load():
     L.gbfg_subtract_until_converged.argtypes = [gp, vp, vp, vp, op, i32, vp, ip, vp, vp, vp, vp, rp, vp, sz, vp]
     L.gbfg_simulate.argtypes = [gp, pp, op, i32, u64, vp, ip, vp, vp, vp, vp, vp, vp, vp, vp, vp, rp, vp, sz, vp]
     L.gbfg_simulate_host.argtypes = [gp, pp, op, i32, u64, vp, ip, vp, vp, rp]
+    L.gbfg_profile_enable.argtypes = [C.c_int]
+    L.gbfg_profile_read.argtypes = [C.POINTER(KernelTime), i32]
     L.gbfg_workspace_bytes.restype = sz
     L.gbfg_workspace_bytes.argtypes = [gp, i64, i32]
     _lib = L
@@ -144,6 +152,17 @@ def version() -> int:
 
 def kernel_launch_count() -> int:
     return load().gbfg_kernel_launch_count()
+
+
+def profile_enable(on: bool):
+    _check(load().gbfg_profile_enable(1 if on else 0))
+
+
+def profile_read() -> dict:
+    """{kernel class: (launches, total_ms, max_ms)} of the launches timed since the last read."""
+    arr = (KernelTime * len(KERNEL_CLASSES))()
+    _check(load().gbfg_profile_read(arr, len(KERNEL_CLASSES)))
+    return {k: (int(arr[i].launches), float(arr[i].total_ms), float(arr[i].max_ms)) for i, k in enumerate(KERNEL_CLASSES)}
 
 
 def grid_init(f_min: float, f_max: float, t_obs: float, scale_log2: int = -140) -> Grid:

@@ -2,6 +2,8 @@
 #include <stdio.h>
 #include <string.h>
 
+#include <vector>
+
 #include "gbfg_common.cuh"
 
 namespace gbfg {
@@ -17,6 +19,31 @@ int set_cuda_error(cudaError_t e, const char *where)
 }
 
 void count_launch(int n) { g_launches += n; }
+
+// ---- per-kernel timing helper (measurement only; off by default)
+struct TimedLaunch { cudaEvent_t a, b; int kid; };
+static thread_local bool g_prof_on = false;
+static thread_local std::vector<TimedLaunch> *g_prof = nullptr;   // event pairs, reused across reads
+static thread_local size_t g_prof_used = 0;
+
+LaunchTimer::LaunchTimer(int kernel_id, cudaStream_t stream) : slot(-1), st(stream)
+{
+    if (!g_prof_on) return;
+    if (!g_prof) g_prof = new std::vector<TimedLaunch>();
+    if (g_prof_used == g_prof->size()) {
+        TimedLaunch t;
+        if (cudaEventCreate(&t.a) != cudaSuccess || cudaEventCreate(&t.b) != cudaSuccess) { (void)cudaGetLastError(); return; }
+        g_prof->push_back(t);
+    }
+    slot = (int)g_prof_used++;
+    (*g_prof)[slot].kid = kernel_id;
+    cudaEventRecord((*g_prof)[slot].a, st);
+}
+
+LaunchTimer::~LaunchTimer()
+{
+    if (slot >= 0) cudaEventRecord((*g_prof)[slot].b, st);
+}
 
 struct DevInfo { int ok; int status; int sms; };
 static DevInfo g_dev[64];
@@ -72,6 +99,30 @@ extern "C" const char *gbfg_strerror(int status)
 extern "C" const char *gbfg_last_cuda_error(void) { return g_cuda_error; }
 
 extern "C" int64_t gbfg_kernel_launch_count(void) { return g_launches; }
+
+extern "C" int gbfg_profile_enable(int on)
+{
+    g_prof_on = on != 0;
+    g_prof_used = 0;
+    return GBFG_OK;
+}
+
+extern "C" int gbfg_profile_read(gbfg_kernel_time *out, int32_t n_out)
+{
+    if (!out || n_out < GBFG_K_COUNT) return GBFG_ERR_INVALID_ARG;
+    for (int k = 0; k < GBFG_K_COUNT; ++k) { out[k].launches = 0; out[k].total_ms = 0.0; out[k].max_ms = 0.0; }
+    for (size_t i = 0; i < g_prof_used; ++i) {
+        TimedLaunch &t = (*g_prof)[i];
+        GBFG_CUDA(cudaEventSynchronize(t.b));
+        float ms = 0.f;
+        GBFG_CUDA(cudaEventElapsedTime(&ms, t.a, t.b));
+        out[t.kid].launches += 1;
+        out[t.kid].total_ms += (double)ms;
+        if ((double)ms > out[t.kid].max_ms) out[t.kid].max_ms = (double)ms;
+    }
+    g_prof_used = 0;
+    return GBFG_OK;
+}
 
 extern "C" int gbfg_grid_init(double f_min, double f_max, double t_obs, int32_t scale_log2, gbfg_grid *out)
 {

@@ -160,11 +160,15 @@ int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const 
     int64_t blocks = (n_launch + 255) / 256;
     int64_t cap = (int64_t)sm_count() * 16;
     if (blocks > cap) blocks = cap;
-    deposit_kernel<<<(int)blocks, 256, 0, st>>>(g, ct, A, f, fdot, sel_idx, sel_count, ct.offsets[ct.n_cat], sign,
-                                                spectrum, diff, err_count, wide_flag);
+    {
+        LaunchTimer lt(K_DEPOSIT, st);
+        deposit_kernel<<<(int)blocks, 256, 0, st>>>(g, ct, A, f, fdot, sel_idx, sel_count, ct.offsets[ct.n_cat], sign,
+                                                    spectrum, diff, err_count, wide_flag);
+    }
     GBFG_LAUNCH_CHECK("deposit_kernel");
     const int tiles = scan_tiles_per_row(g.n_bins);
     dim3 grid(tiles, ct.n_cat);
+    LaunchTimer lt_scan(K_SCAN, st);     // the three scan kernels and the flag reset, as one
     scan_tile_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, wide_flag);
     GBFG_LAUNCH_CHECK("scan_tile_sums_kernel");
     scan_tile_offsets_kernel<<<ct.n_cat, 1024, 0, st>>>(tile_sums, tiles, wide_flag);

@@ -21,6 +21,18 @@ int check_device();                                     // GBFG_OK or GBFG_ERR_A
 void count_launch(int n = 1);
 int sm_count();
 
+// Kernel classes of the per-kernel timing helper (gbfg_profile_*; order = GBFG_K_* in gbfg.h).
+enum KernelId { K_SAMPLE = 0, K_NOISE, K_DEPOSIT, K_SCAN, K_MEDIAN, K_PSD, K_INV_BLOCKS, K_SNR, K_AUX, K_COUNT };
+
+// Brackets the launches issued during its lifetime with a pair of CUDA events on `st` when the
+// calling thread has enabled profiling (gbfg_profile_enable); otherwise does nothing.
+struct LaunchTimer {
+    int slot;
+    cudaStream_t st;
+    LaunchTimer(int kernel_id, cudaStream_t stream);
+    ~LaunchTimer();
+};
+
 #define GBFG_CUDA(call)                                                        \
     do {                                                                       \
         cudaError_t e__ = (call);                                              \

@@ -254,7 +254,10 @@ int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64
         attr_dev = dev;
     }
     dim3 grid(a.tiles, n_cat);
-    running_median_kernel<<<grid, MED_THREADS, MED_SMEM, st>>>(a);
+    {
+        LaunchTimer lt(K_MEDIAN, st);
+        running_median_kernel<<<grid, MED_THREADS, MED_SMEM, st>>>(a);
+    }
     GBFG_LAUNCH_CHECK("running_median_kernel");
     return GBFG_OK;
 }
@@ -287,8 +290,11 @@ extern "C" int gbfg_psd(const int64_t *dev_median, const double *dev_s_instr, in
     int bx = (int)((n_bins + 255) / 256);
     int cap = sm_count() * 8;
     if (bx > cap) bx = cap;
-    psd_kernel<<<dim3(bx, n_cat), 256, 0, (cudaStream_t)stream>>>(dev_median, dev_s_instr, n_bins, median_norm,
-                                                                   ldexp(1.0, scale_log2), dev_psd);
+    {
+        LaunchTimer lt(K_PSD, (cudaStream_t)stream);
+        psd_kernel<<<dim3(bx, n_cat), 256, 0, (cudaStream_t)stream>>>(dev_median, dev_s_instr, n_bins, median_norm,
+                                                                       ldexp(1.0, scale_log2), dev_psd);
+    }
     GBFG_LAUNCH_CHECK("psd_kernel");
     return GBFG_OK;
 }

@@ -269,7 +269,10 @@ extern "C" int gbfg_instrument_noise(const gbfg_grid *grid, double *dev_s_instr,
     int blocks = (int)((grid->n_bins + 255) / 256);
     int cap = sm_count() * 8;
     if (blocks > cap) blocks = cap;
-    instrument_noise_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(grid->f_min, grid->t_obs, grid->n_bins, dev_s_instr);
+    {
+        LaunchTimer lt(K_NOISE, (cudaStream_t)stream);
+        instrument_noise_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(grid->f_min, grid->t_obs, grid->n_bins, dev_s_instr);
+    }
     GBFG_LAUNCH_CHECK("instrument_noise_kernel");
     return GBFG_OK;
 }
@@ -318,8 +321,11 @@ extern "C" int gbfg_sample_catalog(const gbfg_grid *grid, const gbfg_pop *pops, 
         if (blocks < 1) blocks = 1;
         int64_t cap = (int64_t)sm_count() * 16;
         if (blocks > cap) blocks = cap;
-        sample_kernel<<<(int)blocks, 256, 0, (cudaStream_t)stream>>>(
-            P, dev_A + offsets[c], dev_f + offsets[c], dev_fdot + offsets[c], head);
+        {
+            LaunchTimer lt(K_SAMPLE, (cudaStream_t)stream);
+            sample_kernel<<<(int)blocks, 256, 0, (cudaStream_t)stream>>>(
+                P, dev_A + offsets[c], dev_f + offsets[c], dev_fdot + offsets[c], head);
+        }
         GBFG_LAUNCH_CHECK("sample_kernel");
     }
     return GBFG_OK;

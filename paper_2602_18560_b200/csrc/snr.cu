@@ -163,7 +163,10 @@ int launch_snr_select(const GridDev &g, const CatTable &ct, const double *A, con
     const int bpr = snr_inv_blocks_per_row(g.n_bins);
     if (inv_blocks) {
         int bx = bpr < sm_count() * 8 ? bpr : sm_count() * 8;
-        inv_block_sums_kernel<<<dim3(bx, ct.n_cat), 256, 0, st>>>(psd, g.n_bins, bpr, inv_blocks);
+        {
+            LaunchTimer lt(K_INV_BLOCKS, st);
+            inv_block_sums_kernel<<<dim3(bx, ct.n_cat), 256, 0, st>>>(psd, g.n_bins, bpr, inv_blocks);
+        }
         GBFG_LAUNCH_CHECK("inv_block_sums_kernel");
     }
     if (n_launch <= 0) return GBFG_OK;
@@ -176,7 +179,10 @@ int launch_snr_select(const GridDev &g, const CatTable &ct, const double *A, con
     int64_t blocks = (n_launch + 255) / 256;
     int64_t cap = (int64_t)sm_count() * 16;
     if (blocks > cap) blocks = cap;
-    snr_select_kernel<<<(int)blocks, 256, 0, st>>>(g, ct, a);
+    {
+        LaunchTimer lt(K_SNR, st);
+        snr_select_kernel<<<(int)blocks, 256, 0, st>>>(g, ct, a);
+    }
     GBFG_LAUNCH_CHECK("snr_select_kernel");
     return GBFG_OK;
 }

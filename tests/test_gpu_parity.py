@@ -184,14 +184,15 @@ def test_psd_bit_exact(gb, orc, torch):
 
 
 # ------------------------------------------------------------------------------------ stage (iv)
-def _snr_case(gb, orc, torch, w, A, f, fd, rho_th, resolved0=None):
+def _snr_case(gb, orc, torch, w, A, f, fd, rho_th, resolved0=None, psd=None):
     g = gpu_grid(gb, w)
     og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
     n = A.size
-    s_instr = orc.instrument_noise(og)
-    spec = np.zeros(og.n_bins, dtype=np.int64)
-    orc.deposit(og, A, f, fd, spec)
-    psd = orc.psd_from_median(orc.running_median(spec, w.window), s_instr, w.median_norm, w.scale_log2)
+    if psd is None:
+        s_instr = orc.instrument_noise(og)
+        spec = np.zeros(og.n_bins, dtype=np.int64)
+        orc.deposit(og, A, f, fd, spec)
+        psd = orc.psd_from_median(orc.running_median(spec, w.window), s_instr, w.median_norm, w.scale_log2)
     res_ref = np.zeros(n, dtype=np.uint8) if resolved0 is None else resolved0.copy()
     res_gpu = dev(torch, res_ref)
     sel_ref, r2_ref, near_ref = orc.snr_select(og, A, f, fd, psd, rho_th, res_ref)
@@ -253,7 +254,7 @@ def test_snr_threshold_decisions_on_the_definition(gb, orc, torch):
     ok = ~np.isnan(r2) & (r2 > 0)
     A2 = A.copy()
     A2[ok] = A[ok] * np.sqrt(49.0 / r2[ok]) * (1.0 + np.random.default_rng(1).integers(-3, 4, ok.sum()) * 1.1e-16)
-    _, near = _snr_case(gb, orc, torch, w, A2, f, fd, 7.0)
+    _, near = _snr_case(gb, orc, torch, w, A2, f, fd, 7.0, psd=psd)      # same PSD: rho^2 scales exactly as A^2
     assert near >= ok.sum() // 2
 
 
