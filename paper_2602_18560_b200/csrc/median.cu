@@ -4,13 +4,17 @@
 // of the 2h+1 int64 values.  Only integer comparisons decide the result, so it is exact.
 //
 // One CTA per tile of S = LT - 2h outputs.  The tile and its two h-bin halos (LT positions) are
-// staged in shared memory and sorted ONCE by (value, position).  With the sorted order in hand a
-// window is a position interval, and its median is found without ever sorting a window:
-//   * a (rank-bucket x position-block) table of counts locates, by bisection, the h-th smallest
-//     element of a block-aligned position interval (start of a chunk of 32 outputs);
-//   * from there one thread walks its chunk: sliding the window by one bin removes one position
-//     and adds one, which moves the median by at most one place in the sorted order; the
-//     neighbouring in-window element is found by stepping through the sorted positions
+// staged in shared memory and sorted ONCE by (value, position): an LSD radix sort, 8 bits per pass,
+// that skips the passes whose digit is the same for the whole tile (spectrum values rarely need
+// more than four).  With the sorted order in hand a window is a position interval, and its median
+// is found without ever sorting a window:
+//   * a (rank-bucket x position-block) table of counts locates the h-th smallest element of a
+//     block-aligned position interval; one warp does this for the start of every chunk of 32
+//     outputs (coarse states);
+//   * every thread then takes 8 outputs: it jumps from the coarse state to its first output by
+//     counting the ranks that left and entered, and walks: sliding the window by one bin removes
+//     one position and adds one, which moves the median by at most one place in the sorted order;
+//     the neighbouring in-window element is found by stepping through the sorted positions
 //     (on average LT/W steps).
 // The per-output rank is kept in shared memory and written out coalesced, fused with
 //     psd[k] = s_instr[k] + C * (med[k] * 2^scale_log2)        (eqs. 10, D2, D3).
@@ -20,18 +24,25 @@ namespace gbfg {
 
 constexpr int MED_LT = 8192;                  // positions per tile, halos included (power of two)
 constexpr int MED_THREADS = 1024;
-constexpr int MED_PB = 32;                    // position block = outputs per chunk
+constexpr int MED_WARPS = MED_THREADS / 32;
+constexpr int MED_ITEMS = MED_LT / MED_THREADS;   // 8 keys per thread in the sort
+constexpr int MED_PB = 32;                    // position block = outputs per coarse chunk
+constexpr int MED_FINE = 8;                   // outputs per walking thread
 constexpr int MED_RB = 128;                   // sorted ranks per bucket
 constexpr int MED_NPB = MED_LT / MED_PB;      // 256
 constexpr int MED_NRB = MED_LT / MED_RB;      // 64
 constexpr int MED_TROW = MED_NPB + 2;         // table row stride in u16 (even: rows stay 4-byte aligned)
+constexpr int MED_CROW = 256 + 2;             // radix counter row stride in u16 (one row per warp)
 constexpr uint64_t SIGN64 = 0x8000000000000000ull;
 
+constexpr size_t MED_AUX_U16 = (MED_NRB * MED_TROW > MED_WARPS * MED_CROW) ? MED_NRB * MED_TROW : MED_WARPS * MED_CROW;
 constexpr size_t MED_SMEM = sizeof(uint64_t) * MED_LT      // skey
                           + sizeof(uint16_t) * MED_LT      // spos
                           + sizeof(uint16_t) * MED_LT      // rop
                           + sizeof(uint16_t) * MED_LT      // orank
-                          + sizeof(uint16_t) * MED_NRB * MED_TROW;
+                          + sizeof(uint16_t) * MED_AUX_U16 // radix counters, then the count table
+                          + sizeof(uint16_t) * MED_NPB     // coarse medians
+                          + sizeof(uint32_t) * 40;         // scan partials, varying-bit mask
 
 struct MedianArgs {
     const int64_t *x;        // [n_cat][n]
@@ -46,6 +57,13 @@ struct MedianArgs {
     double norm, scale;      // C and 2^scale_log2
 };
 
+// n-th (1-based) set bit of a non-zero mask that has at least n bits set
+__device__ __forceinline__ int nth_set_bit(unsigned m, int n)
+{
+    for (int i = 1; i < n; ++i) m &= m - 1;
+    return __ffs(m) - 1;
+}
+
 __global__ void __launch_bounds__(MED_THREADS, 1)
 running_median_kernel(MedianArgs a)
 {
@@ -54,10 +72,16 @@ running_median_kernel(MedianArgs a)
     uint16_t *spos = reinterpret_cast<uint16_t *>(skey + MED_LT);
     uint16_t *rop = spos + MED_LT;
     uint16_t *orank = rop + MED_LT;
-    uint16_t *tab = orank + MED_LT;
-    uint32_t *tab32 = reinterpret_cast<uint32_t *>(tab);
+    uint16_t *aux = orank + MED_LT;                       // radix counters, later the count table
+    uint16_t *cm = aux + MED_AUX_U16;                     // coarse medians
+    uint32_t *misc = reinterpret_cast<uint32_t *>(cm + MED_NPB);
+    uint16_t *tab = aux;
+    uint32_t *aux32 = reinterpret_cast<uint32_t *>(aux);
 
     const int tid = threadIdx.x;
+    const int warp = tid >> 5, lane = tid & 31;
+    const unsigned FULL = 0xffffffffu;
+    const unsigned lt_mask = (1u << lane) - 1u;
     const int tile = blockIdx.x;
     if (a.tile_dirty && a.tile_dirty[(int64_t)blockIdx.y * a.tiles + tile] == 0) return;
     const int64_t row = (int64_t)blockIdx.y * a.n;
@@ -66,50 +90,111 @@ running_median_kernel(MedianArgs a)
     const int n_out = (int)((a.n - o0 < a.S) ? (a.n - o0) : a.S);
     const int Lt = n_out + 2 * h;                        // positions really used
 
-    // ---- stage the tile: position p <-> global bin o0 - h + p, reflected at both ends
-    for (int p = tid; p < MED_LT; p += MED_THREADS) {
-        uint64_t key = ~0ull;
-        if (p < Lt) {
-            int64_t g = o0 - h + p;
-            if (g < 0) g = -g - 1;
-            if (g >= a.n) g = 2 * a.n - 1 - g;
-            key = (uint64_t)a.x[row + g] ^ SIGN64;
-        }
-        skey[p] = key;
-        spos[p] = (uint16_t)p;
-    }
-    for (int e = tid; e < MED_NRB * MED_TROW / 2; e += MED_THREADS) tab32[e] = 0u;
+    // ---- stage the tile: position p <-> global bin o0 - h + p, reflected at both ends.
+    // Unused positions (last tile only) repeat position 0: they are never inside a window.
+    if (tid < 2) misc[32 + tid] = 0u;
     __syncthreads();
-
-    // ---- bitonic sort by (key, position)
-    for (int k = 2; k <= MED_LT; k <<= 1) {
-        for (int j = k >> 1; j > 0; j >>= 1) {
-            for (int t = tid; t < MED_LT / 2; t += MED_THREADS) {
-                int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
-                int l = i | j;
-                bool up = (i & k) == 0;
-                uint64_t ka = skey[i], kb = skey[l];
-                uint16_t pa = spos[i], pb = spos[l];
-                bool gt = (ka > kb) || (ka == kb && pa > pb);
-                if (gt == up) { skey[i] = kb; skey[l] = ka; spos[i] = pb; spos[l] = pa; }
+    {
+        int64_t g0 = o0 - h;
+        if (g0 < 0) g0 = -g0 - 1;
+        if (g0 >= a.n) g0 = 2 * a.n - 1 - g0;
+        const uint64_t key_ref = (uint64_t)a.x[row + g0] ^ SIGN64;
+        uint64_t vary = 0;
+        for (int p = tid; p < MED_LT; p += MED_THREADS) {
+            uint64_t key = key_ref;
+            if (p < Lt) {
+                int64_t g = o0 - h + p;
+                if (g < 0) g = -g - 1;
+                if (g >= a.n) g = 2 * a.n - 1 - g;
+                key = (uint64_t)a.x[row + g] ^ SIGN64;
             }
-            __syncthreads();
+            vary |= key ^ key_ref;
+            skey[p] = key;
+            spos[p] = (uint16_t)p;
         }
+        const unsigned vlo = __reduce_or_sync(FULL, (unsigned)vary);
+        const unsigned vhi = __reduce_or_sync(FULL, (unsigned)(vary >> 32));
+        if (lane == 0) {
+            if (vlo) atomicOr(&misc[32], vlo);
+            if (vhi) atomicOr(&misc[33], vhi);
+        }
+    }
+    __syncthreads();
+    const uint64_t vary_all = ((uint64_t)misc[33] << 32) | misc[32];
+    const int n_pass = vary_all ? (64 - __clzll((long long)vary_all) + 7) / 8 : 0;
+
+    // ---- LSD radix sort by key, stable, so that equal keys stay in position order.
+    // Warp w owns elements [256 w, 256 w + 256) of the current order, 32 consecutive ones per round.
+    for (int pass = 0; pass < n_pass; ++pass) {
+        const int shift = 8 * pass;
+        for (int e = tid; e < MED_WARPS * MED_CROW / 2; e += MED_THREADS) aux32[e] = 0u;
+        __syncthreads();
+        uint16_t *cw = aux + warp * MED_CROW;
+        uint64_t k[MED_ITEMS];
+        uint32_t pp[MED_ITEMS], off[MED_ITEMS];
+#pragma unroll
+        for (int r = 0; r < MED_ITEMS; ++r) {
+            const int e = warp * (32 * MED_ITEMS) + r * 32 + lane;
+            k[r] = skey[e];
+            pp[r] = spos[e];
+            const unsigned d = (unsigned)(k[r] >> shift) & 255u;
+            const unsigned peers = __match_any_sync(FULL, d);
+            const unsigned base = cw[d];
+            __syncwarp();
+            const unsigned rank = __popc(peers & lt_mask);
+            if (rank == 0) cw[d] = (uint16_t)(base + __popc(peers));
+            __syncwarp();
+            off[r] = (d << 16) | (base + rank);
+        }
+        __syncthreads();
+        {   // exclusive scan of the counters in (digit, warp) order: thread t owns digit t/4, warps 8(t%4)..+8
+            const int d = tid >> 2, wg = (tid & 3) * 8;
+            unsigned v[8], s = 0;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) { v[i] = aux[(wg + i) * MED_CROW + d]; s += v[i]; }
+            unsigned incl = s;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                unsigned up = __shfl_up_sync(FULL, incl, o);
+                if (lane >= o) incl += up;
+            }
+            if (lane == 31) misc[warp] = incl;
+            __syncthreads();
+            unsigned wt = misc[lane], wincl = wt;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                unsigned up = __shfl_up_sync(FULL, wincl, o);
+                if (lane >= o) wincl += up;
+            }
+            const unsigned wprev = __shfl_sync(FULL, wincl - wt, warp);
+            unsigned run = wprev + incl - s;
+#pragma unroll
+            for (int i = 0; i < 8; ++i) { aux[(wg + i) * MED_CROW + d] = (uint16_t)run; run += v[i]; }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int r = 0; r < MED_ITEMS; ++r) {
+            const unsigned dst = (unsigned)cw[off[r] >> 16] + (off[r] & 0xffffu);
+            skey[dst] = k[r];
+            spos[dst] = (uint16_t)pp[r];
+        }
+        __syncthreads();
     }
 
     // ---- inverse permutation and the count table
+    for (int e = tid; e < MED_NRB * MED_TROW / 2; e += MED_THREADS) aux32[e] = 0u;
+    __syncthreads();
     for (int r = tid; r < MED_LT; r += MED_THREADS) {
         int p = spos[r];
         rop[p] = (uint16_t)r;
         int e = (r / MED_RB) * MED_TROW + (p / MED_PB) + 1;
-        atomicAdd(&tab32[e >> 1], (e & 1) ? 0x10000u : 1u);
+        atomicAdd(&aux32[e >> 1], (e & 1) ? 0x10000u : 1u);
     }
     __syncthreads();
     // prefix along the position blocks: tab[rb][pb] = #{r in bucket rb : pos < pb*PB}
     {
-        const int warp = tid >> 5, lane = tid & 31;
         constexpr int PER = (MED_NPB + 1 + 31) / 32;     // 9 entries per lane
-        for (int rb = warp; rb < MED_NRB; rb += MED_THREADS / 32) {
+        for (int rb = warp; rb < MED_NRB; rb += MED_WARPS) {
             uint16_t *rowp = tab + rb * MED_TROW;
             int v[PER], s = 0;
 #pragma unroll
@@ -120,7 +205,7 @@ running_median_kernel(MedianArgs a)
             }
             int incl = s;
             for (int o = 1; o < 32; o <<= 1) {
-                int up = __shfl_up_sync(0xffffffffu, incl, o);
+                int up = __shfl_up_sync(FULL, incl, o);
                 if (lane >= o) incl += up;
             }
             int run = incl - s;
@@ -144,64 +229,113 @@ running_median_kernel(MedianArgs a)
     }
     __syncthreads();
 
-    // ---- one thread per chunk of PB outputs
-    const int n_chunks = (n_out + MED_PB - 1) / MED_PB;
-    if (tid < n_chunks) {
-        const int j0 = tid * MED_PB;
-        const int j1 = (j0 + MED_PB < n_out) ? j0 + MED_PB : n_out;
-        const int b0 = tid, b1 = (j0 + W) / MED_PB;
-        const int na = b1 * MED_PB - j0;
-        int plo = j0, phi, m, below;
+    // ---- coarse states: one warp finds the median rank of the window of output 32 c
+    const int n_coarse = (n_out + MED_PB - 1) / MED_PB;
+    for (int c = warp; c < n_coarse; c += MED_WARPS) {
+        const int j0 = c * MED_PB;
+        const int b0 = c, b1 = (j0 + W) / MED_PB;
+        const int na = b1 * MED_PB - j0;                 // block-aligned part of the window
+        int m = MED_LT, below = 0, phi = j0 - 1;
         if (na > 0) {
             const int t = (h < na - 1) ? h : na - 1;
-            int lo = 0, hi = MED_NRB;
-            while (hi - lo > 1) {
-                int mid = (lo + hi) >> 1;
-                int cnt = (int)tab[mid * MED_TROW + b1] - (int)tab[mid * MED_TROW + b0];
-                if (cnt <= t) lo = mid; else hi = mid;
-            }
-            int need = t - ((int)tab[lo * MED_TROW + b1] - (int)tab[lo * MED_TROW + b0]);
-            const unsigned span = (unsigned)(na - 1);
-            m = lo * MED_RB;
-            for (;; ++m) {
-                if ((unsigned)((int)spos[m] - j0) <= span) {
-                    if (need == 0) break;
-                    --need;
-                }
+            // largest bucket lo with #{rank < 128 lo, position in the aligned part} <= t
+            const int c0 = (int)tab[lane * MED_TROW + b1] - (int)tab[lane * MED_TROW + b0];
+            const int c1 = (int)tab[(lane + 32) * MED_TROW + b1] - (int)tab[(lane + 32) * MED_TROW + b0];
+            const unsigned m0 = __ballot_sync(FULL, c0 <= t), m1 = __ballot_sync(FULL, c1 <= t);
+            const int lo = m1 ? 63 - __clz(m1) : 31 - __clz(m0);
+            const int cl = lo < 32 ? __shfl_sync(FULL, c0, lo & 31) : __shfl_sync(FULL, c1, lo & 31);
+            int need = t - cl;
+            int base = lo * MED_RB;
+            for (;;) {                                   // ends inside bucket lo by construction
+                const int r = base + lane;
+                const bool in = r < MED_LT && (unsigned)((int)spos[r < MED_LT ? r : 0] - j0) < (unsigned)na;
+                const unsigned bal = __ballot_sync(FULL, in);
+                const int cn = __popc(bal);
+                if (need < cn) { m = base + nth_set_bit(bal, need + 1); break; }
+                need -= cn;
+                base += 32;
+                if (base >= MED_LT) break;               // not reachable for a consistent table
             }
             below = t;
             phi = b1 * MED_PB - 1;
-        } else {
-            m = MED_LT; below = 0; phi = j0 - 1;
         }
+        {   // complete the window with the (at most 31, or W when W < 32) remaining positions
+            for (int pbase = phi + 1; pbase < j0 + W; pbase += 32) {
+                const int p = pbase + lane;
+                const bool add = p < j0 + W && (int)rop[p < j0 + W ? p : 0] < m;
+                below += __popc(__ballot_sync(FULL, add));
+            }
+        }
+        if (below > h) {                                 // down to the (below - h)-th window element under m
+            int need = below - h, base = m - 1;
+            for (;;) {
+                const int r = base - lane;
+                const bool in = r >= 0 && (unsigned)((int)spos[r >= 0 ? r : 0] - j0) < (unsigned)W;
+                const unsigned bal = __ballot_sync(FULL, in);
+                const int cn = __popc(bal);
+                if (need <= cn) { m = base - nth_set_bit(bal, need); break; }
+                need -= cn;
+                base -= 32;
+                if (base < 0) break;
+            }
+        } else {                                         // up to the (h - below + 1)-th window element at or above m
+            int need = h - below + 1, base = m;
+            for (;;) {
+                const int r = base + lane;
+                const bool in = r < MED_LT && (unsigned)((int)spos[r < MED_LT ? r : 0] - j0) < (unsigned)W;
+                const unsigned bal = __ballot_sync(FULL, in);
+                const int cn = __popc(bal);
+                if (need <= cn) { m = base + nth_set_bit(bal, need); break; }
+                need -= cn;
+                base += 32;
+                if (base >= MED_LT) break;
+            }
+        }
+        if (lane == 0) cm[c] = (uint16_t)m;
+    }
+    __syncthreads();
+
+    // ---- every thread walks MED_FINE outputs, starting from the coarse state of its chunk
+    {
+        const int s = tid / n_coarse, c = tid - s * n_coarse;
+        const int j_first = c * MED_PB + s * MED_FINE;
+        if (s < MED_PB / MED_FINE && j_first < n_out) {
+            const int j_end = (j_first + MED_FINE < n_out) ? j_first + MED_FINE : n_out;
+            int m = cm[c], below = h;
+            int plo = c * MED_PB, phi = plo + W - 1;
+            // jump: count the ranks under m that left and entered
+            const int jump = s * MED_FINE;
+            for (int i = 0; i < jump; ++i) {
+                below += ((int)rop[phi + 1 + i] < m) - ((int)rop[plo + i] < m);
+            }
+            plo += jump;
+            phi += jump;
 #define IN_SET(r) ((unsigned)((int)spos[r] - plo) <= (unsigned)(phi - plo))
 #define REBALANCE()                                                                  \
-        do {                                                                         \
-            while (below > h) { do { --m; } while (!IN_SET(m)); --below; }           \
-            while (below < h && m < MED_LT) {                                        \
-                do { ++m; } while (m < MED_LT && !IN_SET(m));                        \
-                ++below;                                                             \
-            }                                                                        \
-        } while (0)
-        for (int p = phi + 1; p < j0 + W; ++p) {         // complete the first window
-            phi = p;
-            if ((int)rop[p] < m) ++below;
-        }
-        REBALANCE();
-        orank[j0] = (uint16_t)m;
-        for (int j = j0 + 1; j < j1; ++j) {
-            int gone = rop[plo];                          // position j-1 leaves
-            ++plo;
-            int come = rop[phi + 1];                      // position j+2h enters
-            ++phi;
-            if (gone < m) --below;
-            else if (gone == m) { do { ++m; } while (m < MED_LT && !IN_SET(m)); }
-            if (come < m) ++below;
+            do {                                                                     \
+                while (below > h) { do { --m; } while (!IN_SET(m)); --below; }       \
+                while (below < h && m < MED_LT) {                                    \
+                    do { ++m; } while (m < MED_LT && !IN_SET(m));                    \
+                    ++below;                                                         \
+                }                                                                    \
+            } while (0)
+            if (below <= h) { while (m < MED_LT && !IN_SET(m)) ++m; }
             REBALANCE();
-            orank[j] = (uint16_t)m;
-        }
+            orank[j_first] = (uint16_t)m;
+            for (int j = j_first + 1; j < j_end; ++j) {
+                int gone = rop[plo];                      // position j-1 leaves
+                ++plo;
+                int come = rop[phi + 1];                  // position j+2h enters
+                ++phi;
+                if (gone < m) --below;
+                else if (gone == m) { do { ++m; } while (m < MED_LT && !IN_SET(m)); }
+                if (come < m) ++below;
+                REBALANCE();
+                orank[j] = (uint16_t)m;
+            }
 #undef IN_SET
 #undef REBALANCE
+        }
     }
     __syncthreads();
 
