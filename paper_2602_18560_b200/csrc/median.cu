@@ -131,18 +131,22 @@ running_median_kernel(MedianArgs a)
         __syncthreads();
         uint16_t *cw = aux + warp * MED_CROW;
         uint64_t k[MED_ITEMS];
-        uint32_t pp[MED_ITEMS], off[MED_ITEMS];
+        uint32_t pp[MED_ITEMS], off[MED_ITEMS], peers[MED_ITEMS];
 #pragma unroll
-        for (int r = 0; r < MED_ITEMS; ++r) {
+        for (int r = 0; r < MED_ITEMS; ++r) {            // the eight matches are independent: issue them together
             const int e = warp * (32 * MED_ITEMS) + r * 32 + lane;
             k[r] = skey[e];
             pp[r] = spos[e];
-            const unsigned d = (unsigned)(k[r] >> shift) & 255u;
-            const unsigned peers = __match_any_sync(FULL, d);
+            off[r] = (unsigned)(k[r] >> shift) & 255u;
+            peers[r] = __match_any_sync(FULL, off[r]);
+        }
+#pragma unroll
+        for (int r = 0; r < MED_ITEMS; ++r) {            // counter updates, round after round
+            const unsigned d = off[r];
             const unsigned base = cw[d];
             __syncwarp();
-            const unsigned rank = __popc(peers & lt_mask);
-            if (rank == 0) cw[d] = (uint16_t)(base + __popc(peers));
+            const unsigned rank = __popc(peers[r] & lt_mask);
+            if (rank == 0) cw[d] = (uint16_t)(base + __popc(peers[r]));
             __syncwarp();
             off[r] = (d << 16) | (base + rank);
         }
@@ -311,30 +315,30 @@ running_median_kernel(MedianArgs a)
             plo += jump;
             phi += jump;
 #define IN_SET(r) ((unsigned)((int)spos[r] - plo) <= (unsigned)(phi - plo))
-#define REBALANCE()                                                                  \
-            do {                                                                     \
-                while (below > h) { do { --m; } while (!IN_SET(m)); --below; }       \
-                while (below < h && m < MED_LT) {                                    \
-                    do { ++m; } while (m < MED_LT && !IN_SET(m));                    \
-                    ++below;                                                         \
-                }                                                                    \
-            } while (0)
-            if (below <= h) { while (m < MED_LT && !IN_SET(m)) ++m; }
-            REBALANCE();
+            // One rule for every move: with `below` = #{window elements of rank < m}, the median is
+            // the (below - h)-th window element under m, or the (h - below)-th above it, counting m
+            // itself first when it is still in the window.
+            {
+                int dir, need;
+                if (below > h) { dir = -1; need = below - h; }
+                else { dir = 1; need = h - below + (IN_SET(m) ? 0 : 1); }
+                while (need) { m += dir; if (IN_SET(m)) --need; }
+                below = h;
+            }
             orank[j_first] = (uint16_t)m;
             for (int j = j_first + 1; j < j_end; ++j) {
-                int gone = rop[plo];                      // position j-1 leaves
+                const int gone = rop[plo];                // position j-1 leaves
                 ++plo;
-                int come = rop[phi + 1];                  // position j+2h enters
+                const int come = rop[phi + 1];            // position j+2h enters
                 ++phi;
-                if (gone < m) --below;
-                else if (gone == m) { do { ++m; } while (m < MED_LT && !IN_SET(m)); }
-                if (come < m) ++below;
-                REBALANCE();
+                below += (come < m) - (gone < m);         // below is now h-1, h or h+1
+                const int dir = below > h ? -1 : 1;
+                bool move = below != h || gone == m;
+                while (move) { m += dir; move = !IN_SET(m); }
+                below = h;
                 orank[j] = (uint16_t)m;
             }
 #undef IN_SET
-#undef REBALANCE
         }
     }
     __syncthreads();
