@@ -7,7 +7,10 @@
 //     followed by one inclusive scan that is added into the spectrum (2 updates per source instead
 //     of w; chirps reach 7e4 bins at 4 yr).  sum_k spectrum[k] is identical bit for bit.
 // The scan is the three-phase tile scan (tile sums -> scan of tile sums -> rescan + add); the
-// difference array is zeroed again on the way so the workspace is reusable.
+// difference array is zeroed again on the way so the workspace is reusable.  Scan tiles that hold
+// no update and start from a zero running value are skipped (stamps written by the deposit kernel).
+// A subtraction also stamps the running-median tiles whose windows see a changed bin, so that
+// stage (iii) recomputes only those (DepositMarks).
 #include "gbfg_common.cuh"
 
 namespace gbfg {
@@ -23,7 +26,7 @@ deposit_kernel(GridDev g, CatTable ct, const double *__restrict__ A, const doubl
                const double *__restrict__ fdot, const int64_t *__restrict__ sel_idx,
                const int64_t *__restrict__ sel_count, int64_t n_all, int32_t sign,
                int64_t *__restrict__ spectrum, int64_t *__restrict__ diff,
-               int64_t *__restrict__ err_count, int *__restrict__ wide_flag)
+               int64_t *__restrict__ err_count, int *__restrict__ wide_flag, DepositMarks mk)
 {
     const int64_t n = sel_idx ? *sel_count : n_all;
     int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -33,15 +36,27 @@ deposit_kernel(GridDev g, CatTable ct, const double *__restrict__ A, const doubl
         const int64_t i = sel_idx ? sel_idx[t] : t;
         SrcBins s = source_bins(g, A[i], f[i], fdot[i]);
         if (s.status) { ++rejected; continue; }
-        const int64_t row = (int64_t)cat_of(ct, i) * g.n_bins;
+        const int cat = cat_of(ct, i);
+        const int64_t row = (int64_t)cat * g.n_bins;
         const int64_t v = sign >= 0 ? s.q : -s.q;
         if (v == 0) continue;
         if (s.w_eff <= NARROW) {
             for (int64_t k = s.k0; k < s.k0 + s.w_eff; ++k) atomic_add_i64(spectrum + row + k, v);
         } else {
             atomic_add_i64(diff + row + s.k0, v);
-            if (s.k0 + s.w_eff < g.n_bins) atomic_add_i64(diff + row + s.k0 + s.w_eff, -v);
+            mk.scan_stamp[(int64_t)cat * mk.scan_tiles + s.k0 / SCAN_TILE] = mk.stamp;
+            if (s.k0 + s.w_eff < g.n_bins) {
+                atomic_add_i64(diff + row + s.k0 + s.w_eff, -v);
+                mk.scan_stamp[(int64_t)cat * mk.scan_tiles + (s.k0 + s.w_eff) / SCAN_TILE] = mk.stamp;
+            }
             *wide_flag = 1;
+        }
+        if (mk.med_stamp) {
+            // outputs k with |k - b| <= h see bin b (reflected ends included)
+            int64_t lo = s.k0 - mk.med_h, hi = s.k0 + s.w_eff - 1 + mk.med_h;
+            if (lo < 0) lo = 0;
+            if (hi > g.n_bins - 1) hi = g.n_bins - 1;
+            for (int64_t t = lo / mk.med_S; t <= hi / mk.med_S; ++t) mk.med_stamp[(int64_t)cat * mk.med_tiles + t] = mk.stamp;
         }
     }
     if (err_count) {
@@ -54,10 +69,15 @@ deposit_kernel(GridDev g, CatTable ct, const double *__restrict__ A, const doubl
 // phase 1: tile sums of the difference array.  grid = (tiles_per_row, n_cat)
 __global__ void __launch_bounds__(SCAN_THREADS)
 scan_tile_sums_kernel(const int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
-                      int64_t *__restrict__ tile_sums, const int *__restrict__ wide_flag)
+                      int64_t *__restrict__ tile_sums, const int *__restrict__ wide_flag,
+                      const int *__restrict__ scan_stamp, int stamp)
 {
     if (*wide_flag == 0) return;
     __shared__ int64_t warp_sum[SCAN_THREADS / 32];
+    if (scan_stamp[(int64_t)blockIdx.y * tiles_per_row + blockIdx.x] != stamp) {      // untouched tile: sum 0
+        if (threadIdx.x == 0) tile_sums[(int64_t)blockIdx.y * tiles_per_row + blockIdx.x] = 0;
+        return;
+    }
     const int64_t row = (int64_t)blockIdx.y * n_bins;
     const int64_t base = (int64_t)blockIdx.x * SCAN_TILE;
     int64_t acc = 0;
@@ -109,10 +129,14 @@ scan_tile_offsets_kernel(int64_t *__restrict__ tile_sums, int tiles_per_row, con
 __global__ void __launch_bounds__(SCAN_THREADS)
 scan_add_kernel(int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
                 const int64_t *__restrict__ tile_offsets, int64_t *__restrict__ spectrum,
-                const int *__restrict__ wide_flag)
+                const int *__restrict__ wide_flag, const int *__restrict__ scan_stamp, int stamp)
 {
     if (*wide_flag == 0) return;
     __shared__ int64_t warp_tot[SCAN_THREADS / 32];
+    {   // nothing to add in a tile without updates that starts from a zero running value
+        const int64_t ti = (int64_t)blockIdx.y * tiles_per_row + blockIdx.x;
+        if (scan_stamp[ti] != stamp && tile_offsets[ti] == 0) return;
+    }
     const int64_t row = (int64_t)blockIdx.y * n_bins;
     const int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
     int64_t v[SCAN_ITEMS];
@@ -148,13 +172,14 @@ __global__ void clear_flag_kernel(int *flag) { *flag = 0; }
 // ---------------------------------------------------------------------------------------------
 // internal entry used by the stage call and by the loop.  diff: [n_cat*n_bins] zero on entry and
 // on exit; tile_sums: [n_cat*tiles_per_row]; wide_flag: one int (zero on entry and exit).
+// mk.scan_stamp: [n_cat*tiles_per_row] ints, none equal to mk.stamp on entry.
 // ---------------------------------------------------------------------------------------------
 int scan_tiles_per_row(int64_t n_bins) { return (int)((n_bins + SCAN_TILE - 1) / SCAN_TILE); }
 
 int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
                    const int64_t *sel_idx, const int64_t *sel_count, int64_t n_launch, int32_t sign,
                    int64_t *spectrum, int64_t *err_count, int64_t *diff, int64_t *tile_sums, int *wide_flag,
-                   cudaStream_t st)
+                   const DepositMarks &mk, cudaStream_t st)
 {
     if (n_launch <= 0) return GBFG_OK;
     int64_t blocks = (n_launch + 255) / 256;
@@ -163,17 +188,17 @@ int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const 
     {
         LaunchTimer lt(K_DEPOSIT, st);
         deposit_kernel<<<(int)blocks, 256, 0, st>>>(g, ct, A, f, fdot, sel_idx, sel_count, ct.offsets[ct.n_cat], sign,
-                                                    spectrum, diff, err_count, wide_flag);
+                                                    spectrum, diff, err_count, wide_flag, mk);
     }
     GBFG_LAUNCH_CHECK("deposit_kernel");
     const int tiles = scan_tiles_per_row(g.n_bins);
     dim3 grid(tiles, ct.n_cat);
     LaunchTimer lt_scan(K_SCAN, st);     // the three scan kernels and the flag reset, as one
-    scan_tile_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, wide_flag);
+    scan_tile_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, wide_flag, mk.scan_stamp, mk.stamp);
     GBFG_LAUNCH_CHECK("scan_tile_sums_kernel");
     scan_tile_offsets_kernel<<<ct.n_cat, 1024, 0, st>>>(tile_sums, tiles, wide_flag);
     GBFG_LAUNCH_CHECK("scan_tile_offsets_kernel");
-    scan_add_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, spectrum, wide_flag);
+    scan_add_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, spectrum, wide_flag, mk.scan_stamp, mk.stamp);
     GBFG_LAUNCH_CHECK("scan_add_kernel");
     clear_flag_kernel<<<1, 1, 0, st>>>(wide_flag);
     GBFG_LAUNCH_CHECK("clear_flag_kernel");

@@ -69,6 +69,30 @@ inline GridDev make_grid_dev(const gbfg_grid *g)
     return d;
 }
 
+// Stamps written by a deposit / subtraction (deposit.cu): which scan tiles hold range updates, and
+// which running-median tiles see a changed bin (med_stamp NULL: not tracked).
+struct DepositMarks {
+    int *scan_stamp;    // [n_cat][scan_tiles]
+    int scan_tiles;
+    int *med_stamp;     // [n_cat][med_tiles] or NULL
+    int med_tiles;
+    int med_S;          // outputs per median tile
+    int med_h;          // half window
+    int stamp;          // value written
+};
+
+// Workspace of stage (iv) (snr.cu): the 128-bit fixed-point prefix of 1/psd and the candidate records.
+struct SnrWork {
+    void *pref;         // [n_cat][n_bins] 16-byte local prefixes
+    void *tile_off;     // [n_cat][pfx_tiles_per_row] 16-byte tile offsets
+    void *hdr;          // scale of the fixed point
+    int64_t *cand_gk0;  // [n_src_total] first bin (index into [n_cat][n_bins])
+    int32_t *cand_w;    // [n_src_total] width, 0 once resolved
+    double *cand_4p;    // [n_src_total]
+    int64_t *cand_src;  // [n_src_total] global source index
+    int64_t *cand_count;// [1 + n_cat]: number of records, per catalog
+};
+
 // ---------------------------------------------------------------------------------------------
 // device helpers
 // ---------------------------------------------------------------------------------------------

@@ -1,6 +1,12 @@
 // loop.cu — the C-ABI stage calls that need workspace, and stage (v): the subtraction loop of
 // Appendix D steps 4-10 (R6), device resident, one small scalar
 // read back per iteration.
+//
+// Shape of one gbfg_subtract_until_converged call:
+//   prefix of 1/S_instr -> candidate records (pre-selection, R5)           once
+//   per iteration:  running median + PSD of the tiles the last subtraction touched
+//                   prefix of 1/S_n -> SNR test of the candidates -> counters to the host
+//                   subtraction of the newly resolved (stamps the tiles it touches)
 #include <string.h>
 
 #include "gbfg_common.cuh"
@@ -12,29 +18,45 @@ int scan_tiles_per_row(int64_t n_bins);
 int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
                    const int64_t *sel_idx, const int64_t *sel_count, int64_t n_launch, int32_t sign,
                    int64_t *spectrum, int64_t *err_count, int64_t *diff, int64_t *tile_sums, int *wide_flag,
-                   cudaStream_t st);
+                   const DepositMarks &mk, cudaStream_t st);
+int median_tile_outputs(int window);
+int median_tiles(int64_t n_bins, int window);
+int median_max_tiles(int64_t n_bins);
 int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *med,
                   const double *s_instr, double *psd, double norm, int scale_log2,
-                  const uint8_t *tile_dirty, cudaStream_t st);
-int snr_inv_blocks_per_row(int64_t n_bins);
-int launch_snr_select(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
-                      const double *psd, double rho_th, uint8_t *resolved, double *rho2_out,
-                      const int64_t *cand_idx, const int64_t *cand_count, int64_t n_launch,
-                      int64_t *sel_idx, int64_t *sel_count, int64_t *near_count, int near_per_cat,
-                      double *inv_blocks, cudaStream_t st);
+                  const int *tile_stamp, int stamp, int *neg_flag, cudaStream_t st);
+int pfx_tiles_per_row(int64_t n_bins);
+size_t snr_pref_bytes(int64_t n_bins, int n_cat);
+size_t snr_tile_off_bytes(int64_t n_bins, int n_cat);
+size_t snr_hdr_bytes();
+int launch_prefix_header(const double *arr, int64_t n, int64_t n_bins_row, const SnrWork &sw, cudaStream_t st);
+int launch_inv_prefix(const double *psd, int64_t n_bins, int n_cat, const SnrWork &sw, cudaStream_t st);
+int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
+                      const uint8_t *resolved, const double *s_instr, double rho_th, double *rho2_out,
+                      const SnrWork &sw, cudaStream_t st);
+int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th, uint8_t *resolved, double *rho2_out,
+                    int64_t n_launch, int64_t *sel_idx, int64_t *sel_count, int64_t *near_count, int near_per_cat,
+                    const int *abort_flag, bool use_prefix, const SnrWork &sw, cudaStream_t st);
 
 // ------------------------------------------------------------------------------- workspace
+constexpr int WS_COUNTERS = 4 * GBFG_MAX_CAT + 16;
+
+// layout of `counters` (int64): what the host reads back each iteration comes first
+//   [0 .. n_cat]            sel_count: total, per catalog
+//   [1+n_cat .. 1+2 n_cat)  near-threshold counts per catalog
+//   [1+2 n_cat]             flags word: bit 0 = a median was negative
+//   [2+2 n_cat .. 3+3 n_cat) cand_count: total, per catalog
 struct Workspace {
     int64_t *diff;        // [n_cat * n_bins]   difference array of the range-update deposit
     int64_t *tile_sums;   // [n_cat * scan_tiles]
-    double *inv_blocks;   // [n_cat * inv_blocks_per_row]
+    int *scan_stamp;      // [n_cat * scan_tiles]
+    int *med_stamp;       // [n_cat * median_max_tiles]
     int64_t *sel_idx;     // [n_src_total]
-    int64_t *counters;    // [COUNTERS]: sel_count[1 + n_cat], near[n_cat], spare
+    int64_t *counters;    // [WS_COUNTERS]
     int *wide_flag;
+    SnrWork sw;
     size_t bytes;
 };
-
-constexpr int WS_COUNTERS = 2 * GBFG_MAX_CAT + 8;
 
 static size_t align_up(size_t v) { return (v + 255) & ~(size_t)255; }
 
@@ -43,12 +65,24 @@ static Workspace carve(void *base, int64_t n_bins, int64_t n_src_total, int n_ca
     Workspace w;
     size_t off = 0;
     char *b = (char *)base;
-    w.diff = (int64_t *)(b + off);       off += align_up(sizeof(int64_t) * (size_t)n_cat * (size_t)n_bins);
-    w.tile_sums = (int64_t *)(b + off);  off += align_up(sizeof(int64_t) * (size_t)n_cat * (size_t)scan_tiles_per_row(n_bins));
-    w.inv_blocks = (double *)(b + off);  off += align_up(sizeof(double) * (size_t)n_cat * (size_t)snr_inv_blocks_per_row(n_bins));
-    w.sel_idx = (int64_t *)(b + off);    off += align_up(sizeof(int64_t) * (size_t)(n_src_total > 0 ? n_src_total : 1));
-    w.counters = (int64_t *)(b + off);   off += align_up(sizeof(int64_t) * WS_COUNTERS);
-    w.wide_flag = (int *)(b + off);      off += align_up(sizeof(int));
+    const size_t nsrc = (size_t)(n_src_total > 0 ? n_src_total : 1);
+    const size_t rows = (size_t)n_cat * (size_t)n_bins;
+    auto take = [&](size_t bytes) { char *p = b + off; off += align_up(bytes); return p; };
+    w.diff = (int64_t *)take(sizeof(int64_t) * rows);
+    w.tile_sums = (int64_t *)take(sizeof(int64_t) * (size_t)n_cat * (size_t)scan_tiles_per_row(n_bins));
+    w.scan_stamp = (int *)take(sizeof(int) * (size_t)n_cat * (size_t)scan_tiles_per_row(n_bins));
+    w.med_stamp = (int *)take(sizeof(int) * (size_t)n_cat * (size_t)median_max_tiles(n_bins));
+    w.sel_idx = (int64_t *)take(sizeof(int64_t) * nsrc);
+    w.counters = (int64_t *)take(sizeof(int64_t) * WS_COUNTERS);
+    w.wide_flag = (int *)take(sizeof(int));
+    w.sw.pref = take(snr_pref_bytes(n_bins, n_cat));
+    w.sw.tile_off = take(snr_tile_off_bytes(n_bins, n_cat));
+    w.sw.hdr = take(snr_hdr_bytes());
+    w.sw.cand_gk0 = (int64_t *)take(sizeof(int64_t) * nsrc);
+    w.sw.cand_w = (int32_t *)take(sizeof(int32_t) * nsrc);
+    w.sw.cand_4p = (double *)take(sizeof(double) * nsrc);
+    w.sw.cand_src = (int64_t *)take(sizeof(int64_t) * nsrc);
+    w.sw.cand_count = w.counters + 2 + 2 * n_cat;
     w.bytes = off;
     return w;
 }
@@ -86,6 +120,15 @@ static int64_t *host_scratch()
     return p;
 }
 
+static DepositMarks plain_marks(const Workspace &w, int64_t n_bins, int stamp)
+{
+    DepositMarks mk;
+    mk.scan_stamp = w.scan_stamp; mk.scan_tiles = scan_tiles_per_row(n_bins);
+    mk.med_stamp = nullptr; mk.med_tiles = 0; mk.med_S = 1; mk.med_h = 0;
+    mk.stamp = stamp;
+    return mk;
+}
+
 }  // namespace gbfg
 
 using namespace gbfg;
@@ -117,8 +160,10 @@ extern "C" int gbfg_deposit(const gbfg_grid *grid, const double *dev_A, const do
     cudaStream_t st = (cudaStream_t)stream;
     GBFG_CUDA(cudaMemsetAsync(w.diff, 0, sizeof(int64_t) * (size_t)n_cat * (size_t)grid->n_bins, st));
     GBFG_CUDA(cudaMemsetAsync(w.wide_flag, 0, sizeof(int), st));
+    GBFG_CUDA(cudaMemsetAsync(w.scan_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)scan_tiles_per_row(grid->n_bins), st));
     return launch_deposit(make_grid_dev(grid), ct, dev_A, dev_f, dev_fdot, dev_sel_idx, dev_sel_count, n, sign,
-                          dev_spectrum, dev_err_count, w.diff, w.tile_sums, w.wide_flag, st);
+                          dev_spectrum, dev_err_count, w.diff, w.tile_sums, w.wide_flag,
+                          plain_marks(w, grid->n_bins, 1), st);
 }
 
 extern "C" int gbfg_snr_select(const gbfg_grid *grid, const double *dev_A, const double *dev_f, const double *dev_fdot,
@@ -140,10 +185,19 @@ extern "C" int gbfg_snr_select(const gbfg_grid *grid, const double *dev_A, const
     rc = check_device();
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
+    const GridDev g = make_grid_dev(grid);
     GBFG_CUDA(cudaMemsetAsync(dev_sel_count, 0, sizeof(int64_t) * (size_t)(1 + n_cat), st));
-    return launch_snr_select(make_grid_dev(grid), ct, dev_A, dev_f, dev_fdot, dev_psd, rho_th, dev_resolved,
-                             dev_rho2_out, nullptr, nullptr, n, dev_sel_idx, dev_sel_count, dev_near_count, 0,
-                             w.inv_blocks, st);
+    GBFG_CUDA(cudaMemsetAsync(w.sw.cand_count, 0, sizeof(int64_t) * (size_t)(1 + n_cat), st));
+    if (n <= 0) return GBFG_OK;
+    // every unresolved valid source is a candidate (no pre-selection: the PSD is the caller's)
+    rc = launch_prefix_header(dev_psd, (int64_t)n_cat * grid->n_bins, grid->n_bins, w.sw, st);
+    if (rc) return rc;
+    rc = launch_inv_prefix(dev_psd, grid->n_bins, n_cat, w.sw, st);
+    if (rc) return rc;
+    rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, nullptr, rho_th, dev_rho2_out, w.sw, st);
+    if (rc) return rc;
+    return launch_snr_cand(grid->n_bins, n_cat, dev_psd, rho_th, dev_resolved, dev_rho2_out, n, dev_sel_idx,
+                           dev_sel_count, dev_near_count, 0, nullptr, true, w.sw, st);
 }
 
 extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double *dev_A, const double *dev_f,
@@ -174,65 +228,99 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     if (!host) return set_cuda_error(cudaErrorMemoryAllocation, "cudaHostAlloc");
     cudaStream_t st = (cudaStream_t)stream;
     const GridDev g = make_grid_dev(grid);
-    const size_t row_bytes = sizeof(int64_t) * (size_t)n_cat * (size_t)grid->n_bins;
+    const int64_t nb = grid->n_bins;
+    const size_t row_bytes = sizeof(int64_t) * (size_t)n_cat * (size_t)nb;
+    const int scan_tiles = scan_tiles_per_row(nb);
+    const int med_tiles = median_tiles(nb, W);
 
-    int64_t *sel_count = w.counters;                // [1 + n_cat]
-    int64_t *near = w.counters + 1 + n_cat;         // [n_cat]
-    const size_t n_counters = (size_t)(1 + 2 * n_cat);
-    const size_t n_read = n_cat == 1 ? 1 : n_counters;
+    int64_t *sel_count = w.counters;                    // [1 + n_cat]
+    int64_t *near = w.counters + 1 + n_cat;             // [n_cat]
+    int *neg_flag = (int *)(w.counters + 1 + 2 * n_cat);
+    const size_t n_iter_counters = (size_t)(1 + 2 * n_cat);      // zeroed every iteration
+    const size_t n_read_all = (size_t)(3 + 3 * n_cat);           // ... + flags + cand_count
+    const int i_flags = 1 + 2 * n_cat, i_cand = 2 + 2 * n_cat;
+    bool preselect = (params->flags & GBFG_FLAG_NO_PRESELECT) == 0;
+    const bool incremental = (params->flags & GBFG_FLAG_NO_INCREMENTAL) == 0;
 
     GBFG_CUDA(cudaMemsetAsync(w.diff, 0, row_bytes, st));
     GBFG_CUDA(cudaMemsetAsync(w.wide_flag, 0, sizeof(int), st));
     GBFG_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(int64_t) * WS_COUNTERS, st));
+    GBFG_CUDA(cudaMemsetAsync(w.scan_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)scan_tiles, st));
+    GBFG_CUDA(cudaMemsetAsync(w.med_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)med_tiles, st));
+
+    // candidate records: with pre-selection, only sources whose rho^2 against S_instr reaches the threshold
+    rc = launch_prefix_header(dev_s_instr, nb, nb, w.sw, st);
+    if (rc) return rc;
+    if (preselect) {
+        rc = launch_inv_prefix(dev_s_instr, nb, 1, w.sw, st);
+        if (rc) return rc;
+    }
+    rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, preselect ? dev_s_instr : nullptr,
+                           params->rho_th, nullptr, w.sw, st);
+    if (rc) return rc;
 
     bool done[GBFG_MAX_CAT];
     for (int c = 0; c < n_cat; ++c) {
         memset(&host_results[c], 0, sizeof(gbfg_iter_result));
-        host_results[c].n_candidates = ct.offsets[c + 1] - ct.offsets[c];
         done[c] = false;
     }
+    int64_t n_cand = n;                                 // upper bound until the first readback
     int n_done = 0;
     for (int it = 0; it < params->max_iter && n_done < n_cat; ++it) {
-        rc = launch_median(dev_spectrum, grid->n_bins, n_cat, W, dev_median, dev_s_instr, dev_psd,
-                           params->median_norm, grid->scale_log2, nullptr, st);
+        rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
+                           grid->scale_log2, (it > 0 && incremental) ? w.med_stamp : nullptr, it, neg_flag, st);
         if (rc) return rc;
-        if (n_cat == 1) GBFG_CUDA(cudaMemsetAsync(sel_count, 0, sizeof(int64_t) * 2, st));
-        else GBFG_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(int64_t) * n_counters, st));
-        rc = launch_snr_select(g, ct, dev_A, dev_f, dev_fdot, dev_psd, params->rho_th, dev_resolved, nullptr,
-                               nullptr, nullptr, n, w.sel_idx, sel_count, near, 1, w.inv_blocks, st);
+        GBFG_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(int64_t) * n_iter_counters, st));
+        rc = launch_inv_prefix(dev_psd, nb, n_cat, w.sw, st);
         if (rc) return rc;
-        GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read, cudaMemcpyDeviceToHost, st));
+        rc = launch_snr_cand(nb, n_cat, dev_psd, params->rho_th, dev_resolved, nullptr, n_cand, w.sel_idx, sel_count,
+                             near, 1, preselect ? neg_flag : nullptr, true, w.sw, st);
+        if (rc) return rc;
+        GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
         GBFG_CUDA(cudaStreamSynchronize(st));
+        if (preselect && host[i_flags] != 0) {
+            // A negative median: S_n >= S_instr no longer holds, so the pre-selection is not valid
+            // (the caller's spectrum does not contain the catalog).  Every unresolved source becomes
+            // a candidate, and this iteration's test, which did nothing, is run on them.
+            preselect = false;
+            GBFG_CUDA(cudaMemsetAsync(w.sw.cand_count, 0, sizeof(int64_t) * (size_t)(1 + n_cat), st));
+            rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, nullptr, params->rho_th, nullptr, w.sw, st);
+            if (rc) return rc;
+            rc = launch_snr_cand(nb, n_cat, dev_psd, params->rho_th, dev_resolved, nullptr, n, w.sel_idx, sel_count,
+                                 near, 1, nullptr, true, w.sw, st);
+            if (rc) return rc;
+            GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
+            GBFG_CUDA(cudaStreamSynchronize(st));
+            for (int c = 0; c < n_cat; ++c) host_results[c].n_candidates = 0;
+        }
+        n_cand = host[i_cand];
         const int64_t total = host[0];
         for (int c = 0; c < n_cat; ++c) {
-            if (done[c]) continue;
-            const int64_t n_new = n_cat == 1 ? total : host[1 + c];
             gbfg_iter_result &r = host_results[c];
+            if (r.n_candidates == 0) r.n_candidates = n_cat == 1 ? host[i_cand] : host[i_cand + 1 + c];
+            if (done[c]) continue;
+            const int64_t n_new = host[1 + c];
             if (it < GBFG_MAX_ITER_TRACE) r.n_new_per_iter[it] = n_new;
             r.n_resolved += n_new;
-            if (n_cat > 1) r.n_near_threshold += host[1 + n_cat + c];
+            r.n_near_threshold += host[1 + n_cat + c];
             if (n_new == 0) { done[c] = true; ++n_done; r.n_iter = it + 1; r.converged = 1; }
         }
         if (total == 0) break;
-        rc = launch_deposit(g, ct, dev_A, dev_f, dev_fdot, w.sel_idx, sel_count, n, -1, dev_spectrum, nullptr,
-                            w.diff, w.tile_sums, w.wide_flag, st);
+        DepositMarks mk = plain_marks(w, nb, it + 1);
+        if (incremental) { mk.med_stamp = w.med_stamp; mk.med_tiles = med_tiles; mk.med_S = median_tile_outputs(W); mk.med_h = W / 2; }
+        rc = launch_deposit(g, ct, dev_A, dev_f, dev_fdot, w.sel_idx, sel_count, total, -1, dev_spectrum, nullptr,
+                            w.diff, w.tile_sums, w.wide_flag, mk, st);
         if (rc) return rc;
     }
     if (n_done < n_cat) {
         // cap hit: the PSD must match the returned residual (rows of converged catalogs are unchanged)
         for (int c = 0; c < n_cat; ++c)
             if (!done[c]) { host_results[c].n_iter = params->max_iter; host_results[c].converged = 0; }
-        rc = launch_median(dev_spectrum, grid->n_bins, n_cat, W, dev_median, dev_s_instr, dev_psd,
-                           params->median_norm, grid->scale_log2, nullptr, st);
+        rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
+                           grid->scale_log2, incremental ? w.med_stamp : nullptr, params->max_iter, nullptr, st);
         if (rc) return rc;
     }
-    if (n_cat == 1) {
-        GBFG_CUDA(cudaMemcpyAsync(host, near, sizeof(int64_t), cudaMemcpyDeviceToHost, st));
-        GBFG_CUDA(cudaStreamSynchronize(st));
-        host_results[0].n_near_threshold = host[0];
-    } else {
-        GBFG_CUDA(cudaStreamSynchronize(st));
-    }
+    GBFG_CUDA(cudaStreamSynchronize(st));
     return GBFG_OK;
 }
 

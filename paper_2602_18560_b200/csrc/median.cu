@@ -49,7 +49,9 @@ struct MedianArgs {
     int64_t *med;            // [n_cat][n]
     const double *s_instr;   // [n] or NULL (no PSD)
     double *psd;             // [n_cat][n] or NULL
-    const uint8_t *tile_dirty; // [n_cat][tiles] or NULL: skip tiles whose flag is 0
+    const int *tile_stamp;   // [n_cat][tiles] or NULL: only tiles whose stamp equals `stamp` are recomputed
+    int stamp;
+    int *neg_flag;           // nullable: set to 1 when a median is negative
     int64_t n;
     int h;
     int S;                   // outputs per tile = MED_LT - 2h
@@ -83,7 +85,7 @@ running_median_kernel(MedianArgs a)
     const unsigned FULL = 0xffffffffu;
     const unsigned lt_mask = (1u << lane) - 1u;
     const int tile = blockIdx.x;
-    if (a.tile_dirty && a.tile_dirty[(int64_t)blockIdx.y * a.tiles + tile] == 0) return;
+    if (a.tile_stamp && a.tile_stamp[(int64_t)blockIdx.y * a.tiles + tile] != a.stamp) return;
     const int64_t row = (int64_t)blockIdx.y * a.n;
     const int64_t o0 = (int64_t)tile * a.S;
     const int h = a.h, W = 2 * a.h + 1;
@@ -344,15 +346,18 @@ running_median_kernel(MedianArgs a)
     __syncthreads();
 
     // ---- coalesced epilogue: median and PSD
+    bool neg = false;
     for (int j = tid; j < n_out; j += MED_THREADS) {
         int64_t v = (int64_t)(skey[orank[j]] ^ SIGN64);
         int64_t g = o0 + j;
         a.med[row + g] = v;
+        neg |= v < 0;
         if (a.psd) {
             double e = (double)v * a.scale;
             a.psd[row + g] = a.s_instr[g] + a.norm * e;
         }
     }
+    if (a.neg_flag && neg) *a.neg_flag = 1;
 }
 
 __global__ void __launch_bounds__(256)
@@ -368,19 +373,22 @@ psd_kernel(const int64_t *__restrict__ med, const double *__restrict__ s_instr, 
     }
 }
 
+int median_tile_outputs(int window) { return MED_LT - (window - 1); }
+
 int median_tiles(int64_t n_bins, int window)
 {
     int S = MED_LT - (window - 1);
     return (int)((n_bins + S - 1) / S);
 }
 
-// internal entry: median (+ PSD when psd != NULL) of every row; tile_dirty nullable
+// internal entry: median (+ PSD when psd != NULL) of every row.  tile_stamp nullable: recompute only
+// the tiles whose stamp equals `stamp`.  neg_flag nullable: raised when a median is negative.
 int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *med,
                   const double *s_instr, double *psd, double norm, int scale_log2,
-                  const uint8_t *tile_dirty, cudaStream_t st)
+                  const int *tile_stamp, int stamp, int *neg_flag, cudaStream_t st)
 {
     MedianArgs a;
-    a.x = x; a.med = med; a.s_instr = s_instr; a.psd = psd; a.tile_dirty = tile_dirty;
+    a.x = x; a.med = med; a.s_instr = s_instr; a.psd = psd; a.tile_stamp = tile_stamp; a.stamp = stamp; a.neg_flag = neg_flag;
     a.n = n_bins; a.h = window / 2; a.S = MED_LT - 2 * a.h;
     a.tiles = median_tiles(n_bins, window);
     a.norm = norm; a.scale = ldexp(1.0, scale_log2);
@@ -413,7 +421,7 @@ extern "C" int gbfg_running_median(const int64_t *dev_spectrum, int64_t n_bins, 
     if (n_bins < window / 2 + 1) return GBFG_ERR_INVALID_ARG;
     int rc = check_device();
     if (rc) return rc;
-    return launch_median(dev_spectrum, n_bins, n_cat, window, dev_median_out, nullptr, nullptr, 1.0, 0, nullptr,
+    return launch_median(dev_spectrum, n_bins, n_cat, window, dev_median_out, nullptr, nullptr, 1.0, 0, nullptr, 0, nullptr,
                          (cudaStream_t)stream);
 }
 
@@ -436,3 +444,12 @@ extern "C" int gbfg_psd(const int64_t *dev_median, const double *dev_s_instr, in
     GBFG_LAUNCH_CHECK("psd_kernel");
     return GBFG_OK;
 }
+
+namespace gbfg {
+// upper bound of median_tiles over every supported window (workspace sizing)
+int median_max_tiles(int64_t n_bins)
+{
+    const int s_min = MED_LT - (GBFG_MAX_WINDOW - 1);
+    return (int)((n_bins + s_min - 1) / s_min);
+}
+}  // namespace gbfg

@@ -1,74 +1,309 @@
 // snr.cu — stage (iv): rho^2 of every unresolved source against the current PSD, threshold test
-// and compaction of the newly resolved (eqs. 11-12; R4).
+// and compaction of the newly resolved (eqs. 11-12; R4, R5).
 //
 //   rho2_i = sum_{k = k0 .. k0 + w_eff - 1} (4 p_i) / psd[k]
 //
-// Narrow sources (w_eff <= SNR_NARROW, ~90 % of a catalog) are summed by their own thread in
-// ascending k with one division per bin: bit-identical to the definition.  Wider chirps (up to
-// 7e4 bins at 4 yr) are summed by the whole warp over 1/psd, using per-256-bin block sums of
-// 1/psd for the interior, then multiplied by 4p: relative difference from the ascending sum is a few 1e-16
-// per term, far inside the 1e-12 contract.  A source whose rho2 lands within 1e-9 (relative) of
-// the threshold is re-summed in ascending order with the definition's arithmetic, so the
-// resolved/unresolved decision is always taken on the definition's value.
-// Selection: warp ballot + one atomic per warp reserves slots in the index list.
+// Three pieces:
+//  * candidate records (cand_build_kernel).  One pass over the catalog keeps, for every source that
+//    can still be resolved, its first bin, width, 4p and index.  With pre-selection (R5;
+//    steps 2-3 of the algorithm) a source is kept only if its rho^2 against the
+//    instrument noise alone reaches the threshold: S_n >= S_instr, so nothing else ever can.
+//  * an exact prefix of 1/psd (inv_prefix kernels).  1/psd[k] is rounded once (IEEE division) and
+//    accumulated as a 128-bit fixed-point integer, so sum_{k0 <= k < k1} 1/psd[k] is a difference of
+//    two prefixes, exact and independent of the order of accumulation.  (A binary64 prefix is not
+//    accurate enough: its differences are off by up to 2e-10.)
+//  * the test (snr_cand_kernel), one thread per candidate.  Narrow sources (w_eff <= SNR_NARROW) are
+//    summed in ascending k with one division per bin: bit-identical to the definition.  Wider chirps
+//    (up to 7e4 bins at 4 yr) take 4p * (prefix difference): relative difference from the ascending
+//    sum is a few 1e-16 per term, far inside the 1e-12 contract.  A source whose rho2 lands within
+//    4e-9 (relative) of the threshold is re-summed in ascending order with the definition's
+//    arithmetic, so the resolved/unresolved decision is always taken on the definition's value.
+//    Selection: warp ballot + one atomic per warp reserves slots in the index list.
 #include "gbfg_common.cuh"
 
 namespace gbfg {
 
 constexpr int SNR_NARROW = 8;
-constexpr int SNR_IB = 256;          // bins per block sum of 1/psd
+constexpr int PFX_THREADS = 512;
+constexpr int PFX_ITEMS = 8;
+constexpr int PFX_TILE = PFX_THREADS * PFX_ITEMS;     // 4096 bins per prefix tile
 
-// inv_blocks[c][j] = sum_{k in [256 j, 256 j + 256)} 1 / psd[c][k]   (fixed tree order)
-__global__ void __launch_bounds__(256)
-inv_block_sums_kernel(const double *__restrict__ psd, int64_t n_bins, int blocks_per_row,
-                      double *__restrict__ inv_blocks)
+// ------------------------------------------------------------------------- 128-bit fixed point
+struct U128 { uint64_t lo, hi; };
+
+__device__ __forceinline__ U128 u128_add(U128 a, U128 b)
 {
-    __shared__ double wsum[8];
-    const int64_t row = (int64_t)blockIdx.y * n_bins;
-    for (int jb = blockIdx.x; jb < blocks_per_row; jb += gridDim.x) {
-        int64_t k = (int64_t)jb * SNR_IB + threadIdx.x;
-        double v = k < n_bins ? 1.0 / psd[row + k] : 0.0;
-        for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = v;
-        __syncthreads();
-        if (threadIdx.x == 0) {
-            double s = ((wsum[0] + wsum[1]) + (wsum[2] + wsum[3])) + ((wsum[4] + wsum[5]) + (wsum[6] + wsum[7]));
-            inv_blocks[(int64_t)blockIdx.y * blocks_per_row + jb] = s;
-        }
-        __syncthreads();
-    }
+    U128 r;
+    r.lo = a.lo + b.lo;
+    r.hi = a.hi + b.hi + (r.lo < a.lo ? 1ull : 0ull);
+    return r;
+}
+__device__ __forceinline__ U128 u128_sub(U128 a, U128 b)
+{
+    U128 r;
+    r.lo = a.lo - b.lo;
+    r.hi = a.hi - b.hi - (a.lo < b.lo ? 1ull : 0ull);
+    return r;
+}
+__device__ __forceinline__ U128 u128_shfl_up(U128 v, int o)
+{
+    U128 r;
+    r.lo = __shfl_up_sync(0xffffffffu, v.lo, o);
+    r.hi = __shfl_up_sync(0xffffffffu, v.hi, o);
+    return r;
 }
 
-__device__ __forceinline__ double warp_sum(double v)
+// Header of the prefix: unit_exp = exponent U of one fixed-point unit (value = integer * 2^U),
+// e_top = bound on the terms (every term < 2^e_top), bad = some term was not representable.
+struct PrefixHeader { int unit_exp; int e_top; int bad; int pad; };
+
+// x = 1/psd as fixed point with unit 2^U, truncated.  ok = 0 when x is negative, not finite or >= 2^e_top.
+__device__ __forceinline__ U128 inv_to_fixed(double psd, int U, int e_top, int *ok)
 {
-    for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const double x = 1.0 / psd;
+    const long long bits = __double_as_longlong(x);
+    const int e = (int)((bits >> 52) & 0x7ff);
+    U128 v; v.lo = 0; v.hi = 0;
+    if (bits < 0 || e == 0x7ff || e - 1022 > e_top) { *ok = 0; return v; }
+    if (e == 0) return v;                                   // zero / subnormal: below one unit anyway
+    const uint64_t mant = ((uint64_t)bits & 0x000fffffffffffffull) | 0x0010000000000000ull;
+    const int sh = (e - 1075) - U;                          // x = mant * 2^(e - 1075)
+    if (sh >= 0) {
+        if (sh >= 64) { v.hi = mant << (sh - 64); }
+        else { v.lo = mant << sh; v.hi = sh ? (mant >> (64 - sh)) : 0ull; }
+    } else if (sh > -64) {
+        v.lo = mant >> (-sh);
+    }
     return v;
 }
 
-// sum over [k0, k1) of 1/psd, all 32 lanes cooperate (arguments warp-uniform)
-__device__ __forceinline__ double warp_inv_sum(const double *__restrict__ psd_row, const double *__restrict__ ib_row,
-                                               int64_t k0, int64_t k1, int lane)
+// integer * 2^U -> binary64, round to nearest
+__device__ __forceinline__ double fixed_to_double(U128 d, int U)
+{
+    if (d.hi == 0) return ldexp(__ull2double_rn(d.lo), U);
+    const int lz = __clzll((long long)d.hi);
+    uint64_t top = lz ? ((d.hi << lz) | (d.lo >> (64 - lz))) : d.hi;
+    const uint64_t rest = lz ? (d.lo << lz) : d.lo;
+    if (rest) top |= 1ull;                                  // sticky bit
+    return ldexp(__ull2double_rn(top), U + 64 - lz);
+}
+
+// e_top from the largest 1/arr[k] of the grid (arr = s_instr in the loop, psd in the stage call)
+__global__ void __launch_bounds__(1024)
+prefix_header_kernel(const double *__restrict__ arr, int64_t n, int64_t n_bins_row, PrefixHeader *hdr)
+{
+    __shared__ int wmax[32];
+    int emax = -100000;
+    int bad = 0;
+    for (int64_t k = threadIdx.x; k < n; k += blockDim.x) {
+        const double x = 1.0 / arr[k];
+        const long long bits = __double_as_longlong(x);
+        const int e = (int)((bits >> 52) & 0x7ff);
+        if (bits < 0 || e == 0x7ff) bad = 1;
+        else if (e - 1022 > emax) emax = e - 1022;
+    }
+    for (int o = 16; o; o >>= 1) {
+        emax = max(emax, __shfl_xor_sync(0xffffffffu, emax, o));
+        bad |= __shfl_xor_sync(0xffffffffu, bad, o);
+    }
+    if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = bad ? 100000 : emax;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int e = -100000;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) e = max(e, wmax[w]);
+        int L = 0;
+        while (((int64_t)1 << L) < n_bins_row) ++L;
+        PrefixHeader h;
+        h.bad = (e == 100000 || e == -100000) ? 1 : 0;
+        h.e_top = h.bad ? 0 : e;
+        h.unit_exp = h.e_top + L - 127;
+        h.pad = 0;
+        *hdr = h;
+    }
+}
+
+// phase A: local inclusive prefix of every tile of PFX_TILE bins + the tile totals
+__global__ void __launch_bounds__(PFX_THREADS)
+inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tiles_per_row,
+                        U128 *__restrict__ pref, U128 *__restrict__ tile_tot, PrefixHeader *hdr)
+{
+    __shared__ U128 wtot[PFX_THREADS / 32];
+    const int U = hdr->unit_exp, e_top = hdr->e_top;
+    const int64_t row = (int64_t)blockIdx.y * n_bins;
+    const int64_t base = (int64_t)blockIdx.x * PFX_TILE + (int64_t)threadIdx.x * PFX_ITEMS;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    U128 v[PFX_ITEMS];
+    U128 run; run.lo = 0; run.hi = 0;
+    int ok = 1;
+#pragma unroll
+    for (int j = 0; j < PFX_ITEMS; ++j) {
+        const int64_t k = base + j;
+        U128 t; t.lo = 0; t.hi = 0;
+        if (k < n_bins) t = inv_to_fixed(psd[row + k], U, e_top, &ok);
+        run = u128_add(run, t);
+        v[j] = run;
+    }
+    U128 incl = run;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        U128 up = u128_shfl_up(incl, o);
+        if (lane >= o) incl = u128_add(incl, up);
+    }
+    if (lane == 31) wtot[warp] = incl;
+    __syncthreads();
+    U128 before = u128_sub(incl, run);
+    for (int w = 0; w < warp; ++w) before = u128_add(before, wtot[w]);
+#pragma unroll
+    for (int j = 0; j < PFX_ITEMS; ++j) {
+        const int64_t k = base + j;
+        if (k < n_bins) pref[row + k] = u128_add(before, v[j]);
+    }
+    if (threadIdx.x == PFX_THREADS - 1) tile_tot[(int64_t)blockIdx.y * tiles_per_row + blockIdx.x] = u128_add(before, run);
+    if (!ok) hdr->bad = 1;
+}
+
+// phase B: exclusive scan of each row's tile totals (one CTA per row)
+__global__ void __launch_bounds__(1024)
+inv_prefix_tiles_kernel(U128 *__restrict__ tile_tot, int tiles_per_row)
+{
+    __shared__ U128 wtot[32];
+    __shared__ U128 carry_s;
+    U128 *rowp = tile_tot + (int64_t)blockIdx.x * tiles_per_row;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) { carry_s.lo = 0; carry_s.hi = 0; }
+    __syncthreads();
+    for (int b = 0; b < tiles_per_row; b += 1024) {
+        const int idx = b + threadIdx.x;
+        U128 v; v.lo = 0; v.hi = 0;
+        if (idx < tiles_per_row) v = rowp[idx];
+        U128 incl = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            U128 up = u128_shfl_up(incl, o);
+            if (lane >= o) incl = u128_add(incl, up);
+        }
+        if (lane == 31) wtot[warp] = incl;
+        __syncthreads();
+        U128 before = carry_s;
+        for (int w = 0; w < warp; ++w) before = u128_add(before, wtot[w]);
+        if (idx < tiles_per_row) rowp[idx] = u128_add(before, u128_sub(incl, v));
+        __syncthreads();
+        if (threadIdx.x == 1023) carry_s = u128_add(before, incl);
+        __syncthreads();
+    }
+}
+
+// inclusive prefix through bin k of row `row_tile0` (k >= 0)
+__device__ __forceinline__ U128 prefix_at(const U128 *__restrict__ pref, const U128 *__restrict__ tile_off,
+                                          int64_t row_bin0, int64_t row_tile0, int64_t k)
+{
+    const U128 a = pref[row_bin0 + k];
+    const U128 b = tile_off[row_tile0 + k / PFX_TILE];
+    return u128_add(a, b);
+}
+
+// What the test needs of the prefix (all NULL / 0: direct sums only)
+struct PrefixView {
+    const U128 *pref;           // [rows][n_bins] local inclusive prefixes
+    const U128 *tile_off;       // [rows][tiles_per_row] exclusive tile offsets
+    const PrefixHeader *hdr;
+    int tiles_per_row;
+};
+
+// sum over [gk0, gk0 + w) of four_p / psd (psd, pref indexed by global bin; row = its catalog row)
+__device__ __forceinline__ double rho2_direct(const double *__restrict__ psd, int64_t gk0, int64_t w, double four_p)
 {
     double acc = 0.0;
-    int64_t jb0 = (k0 + SNR_IB - 1) / SNR_IB, jb1 = k1 / SNR_IB;
-    if (ib_row && jb1 > jb0) {
-        for (int64_t k = k0 + lane; k < jb0 * SNR_IB; k += 32) acc += 1.0 / psd_row[k];
-        for (int64_t j = jb0 + lane; j < jb1; j += 32) acc += ib_row[j];
-        for (int64_t k = jb1 * SNR_IB + lane; k < k1; k += 32) acc += 1.0 / psd_row[k];
-    } else {
-        for (int64_t k = k0 + lane; k < k1; k += 32) acc += 1.0 / psd_row[k];
+    for (int64_t k = gk0; k < gk0 + w; ++k) acc = acc + four_p / psd[k];
+    return acc;
+}
+
+__device__ __forceinline__ double rho2_of(const double *__restrict__ psd, const PrefixView &pv, bool pref_ok, int unit_exp,
+                                          int64_t gk0, int64_t w, int64_t n_bins, int row, double four_p, bool *exact)
+{
+    *exact = true;
+    if (w <= SNR_NARROW || !pref_ok) return rho2_direct(psd, gk0, w, four_p);
+    const int64_t row_bin0 = (int64_t)row * n_bins, row_tile0 = (int64_t)row * pv.tiles_per_row;
+    const int64_t k0 = gk0 - row_bin0;
+    U128 hi = prefix_at(pv.pref, pv.tile_off, row_bin0, row_tile0, k0 + w - 1);
+    if (k0 > 0) hi = u128_sub(hi, prefix_at(pv.pref, pv.tile_off, row_bin0, row_tile0, k0 - 1));
+    // every term was truncated by less than one unit: keep the relative error under 2^-46
+    if (hi.hi == 0 && hi.lo < ((uint64_t)w << 46)) return rho2_direct(psd, gk0, w, four_p);
+    *exact = false;
+    return four_p * fixed_to_double(hi, unit_exp);
+}
+
+struct CandArrays {
+    int64_t *gk0;       // first bin, as index into the [n_cat][n_bins] arrays
+    int32_t *w;         // w_eff; set to 0 once the source is resolved
+    double *four_p;
+    int64_t *src;       // global source index
+};
+
+struct BuildArgs {
+    const double *A, *f, *fdot;
+    const uint8_t *resolved;
+    const double *s_instr;      // [n_bins], NULL: keep every valid unresolved source (no pre-selection)
+    PrefixView pv;              // prefix of 1/s_instr (one row)
+    double thr_pre;             // rho_th^2 (1 - 4e-9)
+    double *rho2_out;           // nullable: NaN is written for rejected sources
+    CandArrays cand;
+    int64_t *cand_count;        // [1 + n_cat]: total, per catalog
+    int64_t n_all;
+};
+
+__global__ void __launch_bounds__(256)
+cand_build_kernel(GridDev g, CatTable ct, BuildArgs a)
+{
+    const int lane = threadIdx.x & 31;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    const int64_t n_round = (a.n_all + 31) & ~(int64_t)31;
+    bool pref_ok = false;
+    int unit_exp = 0;
+    if (a.s_instr && a.pv.pref) { pref_ok = a.pv.hdr->bad == 0; unit_exp = a.pv.hdr->unit_exp; }
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += stride) {
+        bool keep = false;
+        SrcBins s; s.status = 1; s.k0 = 0; s.w_eff = 0; s.p = 0.0; s.q = 0;
+        int cat = 0;
+        if (i < a.n_all && a.resolved[i] == 0) {
+            s = source_bins(g, a.A[i], a.f[i], a.fdot[i]);
+            if (s.status == 0) {
+                keep = true;
+                if (ct.n_cat > 1) cat = cat_of(ct, i);
+                if (a.s_instr) {
+                    bool exact;
+                    const double r2 = rho2_of(a.s_instr, a.pv, pref_ok, unit_exp, s.k0, s.w_eff, g.n_bins, 0, 4.0 * s.p, &exact);
+                    keep = r2 > a.thr_pre;
+                }
+            } else if (a.rho2_out) {
+                a.rho2_out[i] = __longlong_as_double(0x7ff8000000000000ll);
+            }
+        }
+        const unsigned mask = __ballot_sync(0xffffffffu, keep);
+        if (mask) {
+            int64_t base = 0;
+            if (lane == 0) base = (int64_t)atomicAdd((unsigned long long *)a.cand_count, (unsigned long long)__popc(mask));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (keep) {
+                const int64_t t = base + __popc(mask & ((1u << lane) - 1u));
+                a.cand.gk0[t] = (int64_t)cat * g.n_bins + s.k0;
+                a.cand.w[t] = (int32_t)s.w_eff;
+                a.cand.four_p[t] = 4.0 * s.p;
+                a.cand.src[t] = i;
+                if (ct.n_cat > 1) atomicAdd((unsigned long long *)(a.cand_count + 1 + cat), 1ull);
+            }
+        }
     }
-    return warp_sum(acc);
 }
 
 struct SnrArgs {
-    const double *A, *f, *fdot;
     const double *psd;          // [n_cat][n_bins]
-    const double *inv_blocks;   // [n_cat][blocks_per_row] or NULL
-    int blocks_per_row;
-    const int64_t *cand_idx;    // NULL = every source; else a list of global indices ...
-    const int64_t *cand_count;  // ... with its length on the device
-    int64_t n_all;
+    PrefixView pv;              // prefix of 1/psd
+    CandArrays cand;
+    const int64_t *cand_count;
+    const int *abort_flag;      // nullable: when *abort_flag != 0 the kernel does nothing (loop.cu)
+    int64_t n_bins;
+    int n_cat;
     double thr;                 // rho_th^2
     uint8_t *resolved;
     double *rho2_out;           // nullable
@@ -79,58 +314,33 @@ struct SnrArgs {
 };
 
 __global__ void __launch_bounds__(256)
-snr_select_kernel(GridDev g, CatTable ct, SnrArgs a)
+snr_cand_kernel(SnrArgs a)
 {
+    if (a.abort_flag && *a.abort_flag) return;
     const int lane = threadIdx.x & 31;
-    const int64_t n = a.cand_idx ? *a.cand_count : a.n_all;
+    const int64_t n = *a.cand_count;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    // whole warps iterate together (the loop bound is rounded up to a warp)
     const int64_t n_round = (n + 31) & ~(int64_t)31;
+    const bool pref_ok = a.pv.pref && a.pv.hdr->bad == 0;
+    const int unit_exp = a.pv.pref ? a.pv.hdr->unit_exp : 0;
     for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n_round; t += stride) {
-        int64_t i = -1;
-        bool test = false;
-        if (t < n) {
-            i = a.cand_idx ? a.cand_idx[t] : t;
-            test = a.resolved[i] == 0;
-        }
-        SrcBins s; s.status = 1; s.k0 = 0; s.w_eff = 0; s.p = 0.0; s.q = 0;
-        int cat = 0;
-        if (test) {
-            s = source_bins(g, a.A[i], a.f[i], a.fdot[i]);
-            cat = cat_of(ct, i);
-        }
-        const bool ok = test && s.status == 0;
-        const double four_p = 4.0 * s.p;
-        const double *psd_row = a.psd + (int64_t)cat * g.n_bins;
-        double r2 = 0.0;
-        if (ok && s.w_eff <= SNR_NARROW) {
-            for (int64_t k = s.k0; k < s.k0 + s.w_eff; ++k) r2 = r2 + four_p / psd_row[k];
-        }
-        // wide sources: one at a time, the whole warp sums
-        unsigned wide = __ballot_sync(0xffffffffu, ok && s.w_eff > SNR_NARROW);
-        while (wide) {
-            const int src = __ffs(wide) - 1;
-            wide &= wide - 1;
-            const int64_t k0 = __shfl_sync(0xffffffffu, s.k0, src);
-            const int64_t we = __shfl_sync(0xffffffffu, s.w_eff, src);
-            const int c = __shfl_sync(0xffffffffu, cat, src);
-            const double *pr = a.psd + (int64_t)c * g.n_bins;
-            const double *ir = a.inv_blocks ? a.inv_blocks + (int64_t)c * a.blocks_per_row : nullptr;
-            double tot = warp_inv_sum(pr, ir, k0, k0 + we, lane);
-            if (lane == src) r2 = four_p * tot;
-        }
+        int32_t w = 0;
+        if (t < n) w = a.cand.w[t];
         bool sel = false, near = false;
-        if (ok) {
-            if (fabs(r2 / a.thr - 1.0) <= 4e-9 && s.w_eff > SNR_NARROW) {
-                // decision on the definition's ascending sum
-                double acc = 0.0;
-                for (int64_t k = s.k0; k < s.k0 + s.w_eff; ++k) acc = acc + four_p / psd_row[k];
-                r2 = acc;
-            }
+        int cat = 0;
+        int64_t src = -1;
+        if (w > 0) {
+            const int64_t gk0 = a.cand.gk0[t];
+            const double four_p = a.cand.four_p[t];
+            if (a.n_cat > 1) cat = (int)(gk0 / a.n_bins);
+            bool exact;
+            double r2 = rho2_of(a.psd, a.pv, pref_ok, unit_exp, gk0, w, a.n_bins, cat, four_p, &exact);
+            if (!exact && fabs(r2 / a.thr - 1.0) <= 4e-9) r2 = rho2_direct(a.psd, gk0, w, four_p);   // decide on the definition's sum
             near = fabs(r2 / a.thr - 1.0) <= 2e-9;
             sel = r2 > a.thr;
+            if (a.rho2_out || sel) src = a.cand.src[t];
+            if (a.rho2_out) a.rho2_out[src] = r2;
         }
-        if (test && a.rho2_out) a.rho2_out[i] = ok ? r2 : __longlong_as_double(0x7ff8000000000000ll);
         const unsigned sel_mask = __ballot_sync(0xffffffffu, sel);
         const unsigned near_mask = __ballot_sync(0xffffffffu, near);
         if (sel_mask) {
@@ -138,8 +348,9 @@ snr_select_kernel(GridDev g, CatTable ct, SnrArgs a)
             if (lane == 0) base = (int64_t)atomicAdd((unsigned long long *)a.sel_count, (unsigned long long)__popc(sel_mask));
             base = __shfl_sync(0xffffffffu, base, 0);
             if (sel) {
-                a.sel_idx[base + __popc(sel_mask & ((1u << lane) - 1u))] = i;
-                a.resolved[i] = 1;
+                a.sel_idx[base + __popc(sel_mask & ((1u << lane) - 1u))] = src;
+                a.resolved[src] = 1;
+                a.cand.w[t] = 0;
                 atomicAdd((unsigned long long *)(a.sel_count + 1 + cat), 1ull);
             }
         }
@@ -150,41 +361,98 @@ snr_select_kernel(GridDev g, CatTable ct, SnrArgs a)
     }
 }
 
-int snr_inv_blocks_per_row(int64_t n_bins) { return (int)((n_bins + SNR_IB - 1) / SNR_IB); }
+// ---------------------------------------------------------------------------------------------
+// internal entries (used by the stage call and by the loop, loop.cu)
+// ---------------------------------------------------------------------------------------------
+int pfx_tiles_per_row(int64_t n_bins) { return (int)((n_bins + PFX_TILE - 1) / PFX_TILE); }
 
-// internal entry.  inv_blocks: scratch [n_cat * blocks_per_row] doubles (or NULL: direct sums only).
-// sel_count[0 .. n_cat] must be zero on entry.
-int launch_snr_select(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
-                      const double *psd, double rho_th, uint8_t *resolved, double *rho2_out,
-                      const int64_t *cand_idx, const int64_t *cand_count, int64_t n_launch,
-                      int64_t *sel_idx, int64_t *sel_count, int64_t *near_count, int near_per_cat,
-                      double *inv_blocks, cudaStream_t st)
+static PrefixView make_view(const SnrWork &sw, int64_t n_bins)
 {
-    const int bpr = snr_inv_blocks_per_row(g.n_bins);
-    if (inv_blocks) {
-        int bx = bpr < sm_count() * 8 ? bpr : sm_count() * 8;
-        {
-            LaunchTimer lt(K_INV_BLOCKS, st);
-            inv_block_sums_kernel<<<dim3(bx, ct.n_cat), 256, 0, st>>>(psd, g.n_bins, bpr, inv_blocks);
-        }
-        GBFG_LAUNCH_CHECK("inv_block_sums_kernel");
-    }
+    PrefixView pv;
+    pv.pref = (const U128 *)sw.pref;
+    pv.tile_off = (const U128 *)sw.tile_off;
+    pv.hdr = (const PrefixHeader *)sw.hdr;
+    pv.tiles_per_row = pfx_tiles_per_row(n_bins);
+    return pv;
+}
+
+// hdr <- scale of the fixed-point prefix, from the largest 1/arr[k]; arr: [n], rows of n_bins_row
+int launch_prefix_header(const double *arr, int64_t n, int64_t n_bins_row, const SnrWork &sw, cudaStream_t st)
+{
+    LaunchTimer lt(K_INV_BLOCKS, st);
+    prefix_header_kernel<<<1, 1024, 0, st>>>(arr, n, n_bins_row, (PrefixHeader *)sw.hdr);
+    GBFG_LAUNCH_CHECK("prefix_header_kernel");
+    return GBFG_OK;
+}
+
+// prefix of 1/psd for every row
+int launch_inv_prefix(const double *psd, int64_t n_bins, int n_cat, const SnrWork &sw, cudaStream_t st)
+{
+    const int tiles = pfx_tiles_per_row(n_bins);
+    LaunchTimer lt(K_INV_BLOCKS, st);
+    inv_prefix_local_kernel<<<dim3(tiles, n_cat), PFX_THREADS, 0, st>>>(psd, n_bins, tiles, (U128 *)sw.pref,
+                                                                        (U128 *)sw.tile_off, (PrefixHeader *)sw.hdr);
+    GBFG_LAUNCH_CHECK("inv_prefix_local_kernel");
+    inv_prefix_tiles_kernel<<<n_cat, 1024, 0, st>>>((U128 *)sw.tile_off, tiles);
+    GBFG_LAUNCH_CHECK("inv_prefix_tiles_kernel");
+    return GBFG_OK;
+}
+
+// candidate records of every unresolved valid source; s_instr != NULL: pre-selection against the
+// instrument noise (the prefix in sw must then be that of 1/s_instr, one row).
+// sw.cand_count[0 .. n_cat] must be zero on entry.
+int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
+                      const uint8_t *resolved, const double *s_instr, double rho_th, double *rho2_out,
+                      const SnrWork &sw, cudaStream_t st)
+{
+    const int64_t n = ct.offsets[ct.n_cat];
+    if (n <= 0) return GBFG_OK;
+    BuildArgs a;
+    a.A = A; a.f = f; a.fdot = fdot; a.resolved = resolved; a.s_instr = s_instr;
+    a.pv = make_view(sw, g.n_bins);
+    a.thr_pre = (rho_th * rho_th) * (1.0 - 4e-9);    // keeps every source the near-threshold count (2e-9) can see
+    a.rho2_out = rho2_out;
+    a.cand.gk0 = sw.cand_gk0; a.cand.w = sw.cand_w; a.cand.four_p = sw.cand_4p; a.cand.src = sw.cand_src;
+    a.cand_count = sw.cand_count;
+    a.n_all = n;
+    int64_t blocks = (n + 255) / 256;
+    const int64_t cap = (int64_t)sm_count() * 16;
+    if (blocks > cap) blocks = cap;
+    LaunchTimer lt(K_SNR, st);
+    cand_build_kernel<<<(int)blocks, 256, 0, st>>>(g, ct, a);
+    GBFG_LAUNCH_CHECK("cand_build_kernel");
+    return GBFG_OK;
+}
+
+// the test over the candidate records; n_launch = upper bound of the candidate count (grid sizing).
+// sel_count[0 .. n_cat] is accumulated into (zero it for a fresh selection).
+int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th, uint8_t *resolved, double *rho2_out,
+                    int64_t n_launch, int64_t *sel_idx, int64_t *sel_count, int64_t *near_count, int near_per_cat,
+                    const int *abort_flag, bool use_prefix, const SnrWork &sw, cudaStream_t st)
+{
     if (n_launch <= 0) return GBFG_OK;
     SnrArgs a;
-    a.A = A; a.f = f; a.fdot = fdot; a.psd = psd; a.inv_blocks = inv_blocks; a.blocks_per_row = bpr;
-    a.cand_idx = cand_idx; a.cand_count = cand_count; a.n_all = ct.offsets[ct.n_cat];
+    a.psd = psd;
+    a.pv = make_view(sw, n_bins);
+    if (!use_prefix) { a.pv.pref = nullptr; a.pv.tile_off = nullptr; }
+    a.cand.gk0 = sw.cand_gk0; a.cand.w = sw.cand_w; a.cand.four_p = sw.cand_4p; a.cand.src = sw.cand_src;
+    a.cand_count = sw.cand_count;
+    a.abort_flag = abort_flag;
+    a.n_bins = n_bins; a.n_cat = n_cat;
     a.thr = rho_th * rho_th;
     a.resolved = resolved; a.rho2_out = rho2_out; a.sel_idx = sel_idx; a.sel_count = sel_count;
     a.near_count = near_count; a.near_per_cat = near_per_cat;
     int64_t blocks = (n_launch + 255) / 256;
-    int64_t cap = (int64_t)sm_count() * 16;
+    const int64_t cap = (int64_t)sm_count() * 16;
     if (blocks > cap) blocks = cap;
-    {
-        LaunchTimer lt(K_SNR, st);
-        snr_select_kernel<<<(int)blocks, 256, 0, st>>>(g, ct, a);
-    }
-    GBFG_LAUNCH_CHECK("snr_select_kernel");
+    LaunchTimer lt(K_SNR, st);
+    snr_cand_kernel<<<(int)blocks, 256, 0, st>>>(a);
+    GBFG_LAUNCH_CHECK("snr_cand_kernel");
     return GBFG_OK;
 }
+
+size_t snr_pref_bytes(int64_t n_bins, int n_cat) { return sizeof(U128) * (size_t)n_cat * (size_t)n_bins; }
+size_t snr_tile_off_bytes(int64_t n_bins, int n_cat) { return sizeof(U128) * (size_t)n_cat * (size_t)pfx_tiles_per_row(n_bins); }
+size_t snr_hdr_bytes() { return sizeof(PrefixHeader); }
 
 }  // namespace gbfg
