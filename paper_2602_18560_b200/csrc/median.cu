@@ -28,6 +28,7 @@ constexpr int MED_WARPS = MED_THREADS / 32;
 constexpr int MED_ITEMS = MED_LT / MED_THREADS;   // 8 keys per thread in the sort
 constexpr int MED_PB = 32;                    // position block = outputs per coarse chunk
 constexpr int MED_FINE = 8;                   // outputs per walking thread
+constexpr int MED_STEP_CAP = 12;               // places a thread steps alone before the warp takes over
 constexpr int MED_RB = 128;                   // sorted ranks per bucket
 constexpr int MED_NPB = MED_LT / MED_PB;      // 256
 constexpr int MED_NRB = MED_LT / MED_RB;      // 64
@@ -62,8 +63,7 @@ struct MedianArgs {
 // n-th (1-based) set bit of a non-zero mask that has at least n bits set
 __device__ __forceinline__ int nth_set_bit(unsigned m, int n)
 {
-    for (int i = 1; i < n; ++i) m &= m - 1;
-    return __ffs(m) - 1;
+    return (int)__fns(m, 0u, n);
 }
 
 __global__ void __launch_bounds__(MED_THREADS, 1)
@@ -301,14 +301,47 @@ running_median_kernel(MedianArgs a)
     }
     __syncthreads();
 
-    // ---- every thread walks MED_FINE outputs, starting from the coarse state of its chunk
+    // ---- every thread walks MED_FINE outputs, starting from the coarse state of its chunk.
+    // `below` = #{window elements of rank < m}.  One rule for every move: the median is the
+    // (below - h)-th window element under m, or the (h - below)-th above it, counting m itself first
+    // when it is still in the window.  A thread steps along the sorted order on its own for at most
+    // MED_STEP_CAP places; spectra with plateaus (wide chirps put the same power in consecutive bins)
+    // and level-correlated neighbourhoods have stretches of hundreds of out-of-window elements, and
+    // those searches are finished by the whole warp, 32 places per step (warp_finish).
     {
         const int s = tid / n_coarse, c = tid - s * n_coarse;
         const int j_first = c * MED_PB + s * MED_FINE;
-        if (s < MED_PB / MED_FINE && j_first < n_out) {
-            const int j_end = (j_first + MED_FINE < n_out) ? j_first + MED_FINE : n_out;
-            int m = cm[c], below = h;
-            int plo = c * MED_PB, phi = plo + W - 1;
+        const bool alive = s < MED_PB / MED_FINE && j_first < n_out;
+        const int j_end = alive ? ((j_first + MED_FINE < n_out) ? j_first + MED_FINE : n_out) : j_first;
+        int m = 0, plo = 0, phi = -1, dir = 1, need = 0;
+#define IN_SET(r) ((unsigned)((int)spos[r] - plo) <= (unsigned)(phi - plo))
+        // the warp completes the searches its lanes left unfinished: lane `src` still needs `need`
+        // window elements from rank m (exclusive) in direction dir
+#define WARP_FINISH()                                                                              \
+        for (unsigned pend = __ballot_sync(FULL, need > 0); pend; pend &= pend - 1) {              \
+            const int src = __ffs(pend) - 1;                                                       \
+            int wm = __shfl_sync(FULL, m, src);                                                    \
+            const int wdir = __shfl_sync(FULL, dir, src);                                          \
+            int wneed = __shfl_sync(FULL, need, src);                                              \
+            const int wplo = __shfl_sync(FULL, plo, src), wphi = __shfl_sync(FULL, phi, src);      \
+            for (;;) {                                                                             \
+                const int r = wm + wdir * (1 + lane);                                              \
+                const bool ok = (unsigned)r < (unsigned)MED_LT;                                    \
+                const bool in = ok && (unsigned)((int)spos[ok ? r : 0] - wplo) <= (unsigned)(wphi - wplo); \
+                const unsigned bal = __ballot_sync(FULL, in);                                      \
+                const int cn = __popc(bal);                                                        \
+                if (wneed <= cn) { wm += wdir * (1 + nth_set_bit(bal, wneed)); break; }            \
+                wneed -= cn;                                                                       \
+                wm += 32 * wdir;                                                                   \
+                if ((unsigned)wm >= (unsigned)MED_LT) break;   /* not reachable: the window holds the element */ \
+            }                                                                                      \
+            if (lane == src) { m = wm; need = 0; }                                                 \
+        }
+        if (alive) {
+            int below = h;
+            m = cm[c];
+            plo = c * MED_PB;
+            phi = plo + W - 1;
             // jump: count the ranks under m that left and entered
             const int jump = s * MED_FINE;
             for (int i = 0; i < jump; ++i) {
@@ -316,32 +349,31 @@ running_median_kernel(MedianArgs a)
             }
             plo += jump;
             phi += jump;
-#define IN_SET(r) ((unsigned)((int)spos[r] - plo) <= (unsigned)(phi - plo))
-            // One rule for every move: with `below` = #{window elements of rank < m}, the median is
-            // the (below - h)-th window element under m, or the (h - below)-th above it, counting m
-            // itself first when it is still in the window.
-            {
-                int dir, need;
-                if (below > h) { dir = -1; need = below - h; }
-                else { dir = 1; need = h - below + (IN_SET(m) ? 0 : 1); }
-                while (need) { m += dir; if (IN_SET(m)) --need; }
-                below = h;
-            }
-            orank[j_first] = (uint16_t)m;
-            for (int j = j_first + 1; j < j_end; ++j) {
-                const int gone = rop[plo];                // position j-1 leaves
-                ++plo;
-                const int come = rop[phi + 1];            // position j+2h enters
-                ++phi;
-                below += (come < m) - (gone < m);         // below is now h-1, h or h+1
-                const int dir = below > h ? -1 : 1;
-                bool move = below != h || gone == m;
-                while (move) { m += dir; move = !IN_SET(m); }
-                below = h;
-                orank[j] = (uint16_t)m;
-            }
-#undef IN_SET
+            if (below > h) { dir = -1; need = below - h; }
+            else { dir = 1; need = h - below + (IN_SET(m) ? 0 : 1); }
+            for (int t = 0; need && t < 3 * MED_STEP_CAP; ++t) { m += dir; if (IN_SET(m)) --need; }
         }
+        WARP_FINISH();
+        if (alive) orank[j_first] = (uint16_t)m;
+#pragma unroll 1
+        for (int jj = 1; jj < MED_FINE; ++jj) {
+            const int j = j_first + jj;
+            const bool on = j < j_end;
+            if (on) {
+                const int gone = rop[plo];                    // position j-1 leaves
+                ++plo;
+                const int come = rop[phi + 1];                // position j+2h enters
+                ++phi;
+                const int b = h + (come < m) - (gone < m);    // h-1, h or h+1
+                dir = b > h ? -1 : 1;
+                need = (b != h || gone == m) ? 1 : 0;
+                for (int t = 0; need && t < MED_STEP_CAP; ++t) { m += dir; if (IN_SET(m)) need = 0; }
+            }
+            WARP_FINISH();
+            if (on) orank[j] = (uint16_t)m;
+        }
+#undef WARP_FINISH
+#undef IN_SET
     }
     __syncthreads();
 

@@ -28,6 +28,8 @@ constexpr int PFX_THREADS = 512;
 constexpr int PFX_ITEMS = 8;
 constexpr int PFX_TILE = PFX_THREADS * PFX_ITEMS;     // 4096 bins per prefix tile
 
+size_t snr_hdr_bytes();
+
 // ------------------------------------------------------------------------- 128-bit fixed point
 struct U128 { uint64_t lo, hi; };
 
@@ -88,14 +90,20 @@ __device__ __forceinline__ double fixed_to_double(U128 d, int U)
     return ldexp(__ull2double_rn(top), U + 64 - lz);
 }
 
-// e_top from the largest 1/arr[k] of the grid (arr = s_instr in the loop, psd in the stage call)
-__global__ void __launch_bounds__(1024)
+// e_top from the largest 1/arr[k] of the grid (arr = s_instr in the loop, psd in the stage call).
+// Grid-wide: every CTA folds its maximum into the scratch words behind the header (zero on entry);
+// the last CTA to finish writes the header and clears the scratch.
+struct PrefixScratch { int emax_biased; int bad; unsigned ticket; int pad; };   // emax_biased = e + 200000, 0 = none
+
+__global__ void __launch_bounds__(256)
 prefix_header_kernel(const double *__restrict__ arr, int64_t n, int64_t n_bins_row, PrefixHeader *hdr)
 {
-    __shared__ int wmax[32];
+    __shared__ int wmax[8], wbad[8];
+    PrefixScratch *sc = reinterpret_cast<PrefixScratch *>(hdr + 1);
     int emax = -100000;
     int bad = 0;
-    for (int64_t k = threadIdx.x; k < n; k += blockDim.x) {
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += stride) {
         const double x = 1.0 / arr[k];
         const long long bits = __double_as_longlong(x);
         const int e = (int)((bits >> 52) & 0x7ff);
@@ -106,19 +114,27 @@ prefix_header_kernel(const double *__restrict__ arr, int64_t n, int64_t n_bins_r
         emax = max(emax, __shfl_xor_sync(0xffffffffu, emax, o));
         bad |= __shfl_xor_sync(0xffffffffu, bad, o);
     }
-    if ((threadIdx.x & 31) == 0) wmax[threadIdx.x >> 5] = bad ? 100000 : emax;
+    if ((threadIdx.x & 31) == 0) { wmax[threadIdx.x >> 5] = emax; wbad[threadIdx.x >> 5] = bad; }
     __syncthreads();
     if (threadIdx.x == 0) {
-        int e = -100000;
-        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) e = max(e, wmax[w]);
-        int L = 0;
-        while (((int64_t)1 << L) < n_bins_row) ++L;
-        PrefixHeader h;
-        h.bad = (e == 100000 || e == -100000) ? 1 : 0;
-        h.e_top = h.bad ? 0 : e;
-        h.unit_exp = h.e_top + L - 127;
-        h.pad = 0;
-        *hdr = h;
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) { emax = max(emax, wmax[w]); bad |= wbad[w]; }
+        if (emax > -100000) atomicMax(&sc->emax_biased, emax + 200000);
+        if (bad) atomicOr(&sc->bad, 1);
+        __threadfence();
+        if (atomicAdd(&sc->ticket, 1u) == gridDim.x - 1) {
+            __threadfence();
+            const int eb = atomicAdd(&sc->emax_biased, 0);
+            const int anybad = atomicAdd(&sc->bad, 0);
+            int L = 0;
+            while (((int64_t)1 << L) < n_bins_row) ++L;
+            PrefixHeader h;
+            h.bad = (anybad || eb == 0) ? 1 : 0;
+            h.e_top = h.bad ? 0 : eb - 200000;
+            h.unit_exp = h.e_top + L - 127;
+            h.pad = 0;
+            *hdr = h;
+            sc->emax_biased = 0; sc->bad = 0; sc->ticket = 0u;
+        }
     }
 }
 
@@ -379,8 +395,13 @@ static PrefixView make_view(const SnrWork &sw, int64_t n_bins)
 // hdr <- scale of the fixed-point prefix, from the largest 1/arr[k]; arr: [n], rows of n_bins_row
 int launch_prefix_header(const double *arr, int64_t n, int64_t n_bins_row, const SnrWork &sw, cudaStream_t st)
 {
+    GBFG_CUDA(cudaMemsetAsync(sw.hdr, 0, snr_hdr_bytes(), st));
+    int64_t blocks = (n + 255) / 256;
+    const int64_t cap = (int64_t)sm_count() * 8;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
     LaunchTimer lt(K_INV_BLOCKS, st);
-    prefix_header_kernel<<<1, 1024, 0, st>>>(arr, n, n_bins_row, (PrefixHeader *)sw.hdr);
+    prefix_header_kernel<<<(int)blocks, 256, 0, st>>>(arr, n, n_bins_row, (PrefixHeader *)sw.hdr);
     GBFG_LAUNCH_CHECK("prefix_header_kernel");
     return GBFG_OK;
 }
@@ -453,6 +474,6 @@ int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th,
 
 size_t snr_pref_bytes(int64_t n_bins, int n_cat) { return sizeof(U128) * (size_t)n_cat * (size_t)n_bins; }
 size_t snr_tile_off_bytes(int64_t n_bins, int n_cat) { return sizeof(U128) * (size_t)n_cat * (size_t)pfx_tiles_per_row(n_bins); }
-size_t snr_hdr_bytes() { return sizeof(PrefixHeader); }
+size_t snr_hdr_bytes() { return sizeof(PrefixHeader) + sizeof(PrefixScratch); }
 
 }  // namespace gbfg
