@@ -9,8 +9,8 @@
 // The scan is the three-phase tile scan (tile sums -> scan of tile sums -> rescan + add); the
 // difference array is zeroed again on the way so the workspace is reusable.  Scan tiles that hold
 // no update and start from a zero running value are skipped (stamps written by the deposit kernel).
-// A subtraction also stamps the running-median tiles whose windows see a changed bin, so that
-// stage (iii) recomputes only those (DepositMarks).
+// A subtraction also stamps the dirty blocks (gbfg_common.cuh) whose running-median outputs see a
+// changed bin, so that stages (iii) and (iv) redo only those (DepositMarks).
 #include "gbfg_common.cuh"
 
 namespace gbfg {
@@ -51,12 +51,13 @@ deposit_kernel(GridDev g, CatTable ct, const double *__restrict__ A, const doubl
             }
             *wide_flag = 1;
         }
-        if (mk.med_stamp) {
+        if (mk.blk_stamp) {
             // outputs k with |k - b| <= h see bin b (reflected ends included)
             int64_t lo = s.k0 - mk.med_h, hi = s.k0 + s.w_eff - 1 + mk.med_h;
             if (lo < 0) lo = 0;
             if (hi > g.n_bins - 1) hi = g.n_bins - 1;
-            for (int64_t t = lo / mk.med_S; t <= hi / mk.med_S; ++t) mk.med_stamp[(int64_t)cat * mk.med_tiles + t] = mk.stamp;
+            int *bs = mk.blk_stamp + (int64_t)cat * mk.n_dblk;
+            for (int64_t b = lo >> mk.dblk_log2; b <= (hi >> mk.dblk_log2); ++b) bs[b] = mk.stamp;
         }
     }
     if (err_count) {

@@ -69,25 +69,61 @@ inline GridDev make_grid_dev(const gbfg_grid *g)
     return d;
 }
 
+// Dirty blocks.  The bins of a row are grouped in blocks of 2^dblk_log2 bins (>= 256, at most
+// DIRTY_MAX_BLOCKS per row).  A subtraction stamps the blocks whose running-median OUTPUT can
+// change: those within h bins of a bin it touched.  plan_kernel (median.cu) turns the stamps of
+// one iteration into (a) the work list of the running median, (b) cum[c][b] = number of dirty
+// blocks before block b, which lets the prefix of 1/S_n and the SNR test skip what did not change.
+constexpr int DIRTY_MAX_BLOCKS = 32768;
+
+inline int dirty_block_log2(int64_t n_bins)
+{
+    int L = 8;
+    while (((n_bins + ((int64_t)1 << L) - 1) >> L) > DIRTY_MAX_BLOCKS) ++L;
+    return L;
+}
+inline int dirty_blocks_per_row(int64_t n_bins)
+{
+    const int L = dirty_block_log2(n_bins);
+    return (int)((n_bins + ((int64_t)1 << L) - 1) >> L);
+}
+
+struct DirtyView {
+    const int *cum;     // [n_cat][n_dblk + 1], NULL: everything is dirty
+    int n_dblk;
+    int dblk_log2;
+};
+
 // Stamps written by a deposit / subtraction (deposit.cu): which scan tiles hold range updates, and
-// which running-median tiles see a changed bin (med_stamp NULL: not tracked).
+// which dirty blocks see a changed bin within h (blk_stamp NULL: not tracked).
 struct DepositMarks {
     int *scan_stamp;    // [n_cat][scan_tiles]
     int scan_tiles;
-    int *med_stamp;     // [n_cat][med_tiles] or NULL
-    int med_tiles;
-    int med_S;          // outputs per median tile
+    int *blk_stamp;     // [n_cat][n_dblk] or NULL
+    int n_dblk;
+    int dblk_log2;
     int med_h;          // half window
     int stamp;          // value written
+};
+
+// Work list of the running median (median.cu): items[i] = (row, first output, outputs, 0).
+struct MedianPlan {
+    int4 *items;
+    int *ctr;           // [0] number of items, [1] next item to take (both zero before plan_kernel)
+    int *cum;           // [n_cat][n_dblk + 1]
+    int n_dblk;
+    int dblk_log2;
+    int max_items;
 };
 
 // Workspace of stage (iv) (snr.cu): the 128-bit fixed-point prefix of 1/psd and the candidate records.
 struct SnrWork {
     void *pref;         // [n_cat][n_bins] 16-byte local prefixes
-    void *tile_off;     // [n_cat][pfx_tiles_per_row] 16-byte tile offsets
+    void *tile_off;     // [n_cat][pfx_tiles_per_row] 16-byte tile offsets (exclusive scan of tile_tot)
+    void *tile_tot;     // [n_cat][pfx_tiles_per_row] 16-byte tile totals
     void *hdr;          // scale of the fixed point
     int64_t *cand_gk0;  // [n_src_total] first bin (index into [n_cat][n_bins])
-    int32_t *cand_w;    // [n_src_total] width, 0 once resolved
+    int32_t *cand_w;    // [n_src_total] width; 0 once resolved; negated once a test was near the threshold
     double *cand_4p;    // [n_src_total]
     int64_t *cand_src;  // [n_src_total] global source index
     int64_t *cand_count;// [1 + n_cat]: number of records, per catalog

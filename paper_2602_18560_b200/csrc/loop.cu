@@ -19,24 +19,24 @@ int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const 
                    const int64_t *sel_idx, const int64_t *sel_count, int64_t n_launch, int32_t sign,
                    int64_t *spectrum, int64_t *err_count, int64_t *diff, int64_t *tile_sums, int *wide_flag,
                    const DepositMarks &mk, cudaStream_t st);
-int median_tile_outputs(int window);
-int median_tiles(int64_t n_bins, int window);
-int median_max_tiles(int64_t n_bins);
+int median_max_items(int64_t n_bins);
+int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins, int n_cat, int window,
+                const MedianPlan &pl, cudaStream_t st);
 int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *med,
                   const double *s_instr, double *psd, double norm, int scale_log2,
-                  const int *tile_stamp, int stamp, int *neg_flag, cudaStream_t st);
+                  const MedianPlan *plan, int *neg_flag, cudaStream_t st);
 int pfx_tiles_per_row(int64_t n_bins);
 size_t snr_pref_bytes(int64_t n_bins, int n_cat);
 size_t snr_tile_off_bytes(int64_t n_bins, int n_cat);
 size_t snr_hdr_bytes();
 int launch_prefix_header(const double *arr, int64_t n, int64_t n_bins_row, const SnrWork &sw, cudaStream_t st);
-int launch_inv_prefix(const double *psd, int64_t n_bins, int n_cat, const SnrWork &sw, cudaStream_t st);
+int launch_inv_prefix(const double *psd, int64_t n_bins, int n_cat, const SnrWork &sw, const DirtyView &dv, cudaStream_t st);
 int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
                       const uint8_t *resolved, const double *s_instr, double rho_th, double *rho2_out,
                       const SnrWork &sw, cudaStream_t st);
 int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th, uint8_t *resolved, double *rho2_out,
                     int64_t n_launch, int64_t *sel_idx, int64_t *sel_count, int64_t *near_count, int near_per_cat,
-                    const int *abort_flag, bool use_prefix, const SnrWork &sw, cudaStream_t st);
+                    const int *abort_flag, bool use_prefix, const SnrWork &sw, const DirtyView &dv, cudaStream_t st);
 
 // ------------------------------------------------------------------------------- workspace
 constexpr int WS_COUNTERS = 4 * GBFG_MAX_CAT + 16;
@@ -50,7 +50,8 @@ struct Workspace {
     int64_t *diff;        // [n_cat * n_bins]   difference array of the range-update deposit
     int64_t *tile_sums;   // [n_cat * scan_tiles]
     int *scan_stamp;      // [n_cat * scan_tiles]
-    int *med_stamp;       // [n_cat * median_max_tiles]
+    int *blk_stamp;       // [n_cat * n_dblk]        dirty-block stamps
+    MedianPlan plan;      // work list of the running median, cum of the dirty blocks
     int64_t *sel_idx;     // [n_src_total]
     int64_t *counters;    // [WS_COUNTERS]
     int *wide_flag;
@@ -71,12 +72,20 @@ static Workspace carve(void *base, int64_t n_bins, int64_t n_src_total, int n_ca
     w.diff = (int64_t *)take(sizeof(int64_t) * rows);
     w.tile_sums = (int64_t *)take(sizeof(int64_t) * (size_t)n_cat * (size_t)scan_tiles_per_row(n_bins));
     w.scan_stamp = (int *)take(sizeof(int) * (size_t)n_cat * (size_t)scan_tiles_per_row(n_bins));
-    w.med_stamp = (int *)take(sizeof(int) * (size_t)n_cat * (size_t)median_max_tiles(n_bins));
+    const int n_dblk = dirty_blocks_per_row(n_bins);
+    w.blk_stamp = (int *)take(sizeof(int) * (size_t)n_cat * (size_t)n_dblk);
+    w.plan.n_dblk = n_dblk;
+    w.plan.dblk_log2 = dirty_block_log2(n_bins);
+    w.plan.max_items = n_cat * median_max_items(n_bins);
+    w.plan.cum = (int *)take(sizeof(int) * (size_t)n_cat * (size_t)(n_dblk + 1));
+    w.plan.items = (int4 *)take(sizeof(int4) * (size_t)w.plan.max_items);
+    w.plan.ctr = (int *)take(sizeof(int) * 4);
     w.sel_idx = (int64_t *)take(sizeof(int64_t) * nsrc);
     w.counters = (int64_t *)take(sizeof(int64_t) * WS_COUNTERS);
     w.wide_flag = (int *)take(sizeof(int));
     w.sw.pref = take(snr_pref_bytes(n_bins, n_cat));
     w.sw.tile_off = take(snr_tile_off_bytes(n_bins, n_cat));
+    w.sw.tile_tot = take(snr_tile_off_bytes(n_bins, n_cat));
     w.sw.hdr = take(snr_hdr_bytes());
     w.sw.cand_gk0 = (int64_t *)take(sizeof(int64_t) * nsrc);
     w.sw.cand_w = (int32_t *)take(sizeof(int32_t) * nsrc);
@@ -124,7 +133,7 @@ static DepositMarks plain_marks(const Workspace &w, int64_t n_bins, int stamp)
 {
     DepositMarks mk;
     mk.scan_stamp = w.scan_stamp; mk.scan_tiles = scan_tiles_per_row(n_bins);
-    mk.med_stamp = nullptr; mk.med_tiles = 0; mk.med_S = 1; mk.med_h = 0;
+    mk.blk_stamp = nullptr; mk.n_dblk = 0; mk.dblk_log2 = 0; mk.med_h = 0;
     mk.stamp = stamp;
     return mk;
 }
@@ -192,12 +201,13 @@ extern "C" int gbfg_snr_select(const gbfg_grid *grid, const double *dev_A, const
     // every unresolved valid source is a candidate (no pre-selection: the PSD is the caller's)
     rc = launch_prefix_header(dev_psd, (int64_t)n_cat * grid->n_bins, grid->n_bins, w.sw, st);
     if (rc) return rc;
-    rc = launch_inv_prefix(dev_psd, grid->n_bins, n_cat, w.sw, st);
+    const DirtyView all_dirty = {nullptr, 0, 0};
+    rc = launch_inv_prefix(dev_psd, grid->n_bins, n_cat, w.sw, all_dirty, st);
     if (rc) return rc;
     rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, nullptr, rho_th, dev_rho2_out, w.sw, st);
     if (rc) return rc;
     return launch_snr_cand(grid->n_bins, n_cat, dev_psd, rho_th, dev_resolved, dev_rho2_out, n, dev_sel_idx,
-                           dev_sel_count, dev_near_count, 0, nullptr, true, w.sw, st);
+                           dev_sel_count, dev_near_count, 0, nullptr, true, w.sw, all_dirty, st);
 }
 
 extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double *dev_A, const double *dev_f,
@@ -231,7 +241,6 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     const int64_t nb = grid->n_bins;
     const size_t row_bytes = sizeof(int64_t) * (size_t)n_cat * (size_t)nb;
     const int scan_tiles = scan_tiles_per_row(nb);
-    const int med_tiles = median_tiles(nb, W);
 
     int64_t *sel_count = w.counters;                    // [1 + n_cat]
     int64_t *near = w.counters + 1 + n_cat;             // [n_cat]
@@ -246,13 +255,15 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     GBFG_CUDA(cudaMemsetAsync(w.wide_flag, 0, sizeof(int), st));
     GBFG_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(int64_t) * WS_COUNTERS, st));
     GBFG_CUDA(cudaMemsetAsync(w.scan_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)scan_tiles, st));
-    GBFG_CUDA(cudaMemsetAsync(w.med_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)med_tiles, st));
+    GBFG_CUDA(cudaMemsetAsync(w.blk_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)w.plan.n_dblk, st));
+    const DirtyView all_dirty = {nullptr, 0, 0};
+    const DirtyView dirty = {w.plan.cum, w.plan.n_dblk, w.plan.dblk_log2};
 
     // candidate records: with pre-selection, only sources whose rho^2 against S_instr reaches the threshold
     rc = launch_prefix_header(dev_s_instr, nb, nb, w.sw, st);
     if (rc) return rc;
     if (preselect) {
-        rc = launch_inv_prefix(dev_s_instr, nb, 1, w.sw, st);
+        rc = launch_inv_prefix(dev_s_instr, nb, 1, w.sw, all_dirty, st);
         if (rc) return rc;
     }
     rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, preselect ? dev_s_instr : nullptr,
@@ -267,14 +278,17 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     int64_t n_cand = n;                                 // upper bound until the first readback
     int n_done = 0;
     for (int it = 0; it < params->max_iter && n_done < n_cat; ++it) {
+        // what the last subtraction made dirty (everything, the first time): work list + cum
+        rc = launch_plan(w.blk_stamp, it, it == 0 || !incremental, nb, n_cat, W, w.plan, st);
+        if (rc) return rc;
         rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
-                           grid->scale_log2, (it > 0 && incremental) ? w.med_stamp : nullptr, it, neg_flag, st);
+                           grid->scale_log2, &w.plan, neg_flag, st);
         if (rc) return rc;
         GBFG_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(int64_t) * n_iter_counters, st));
-        rc = launch_inv_prefix(dev_psd, nb, n_cat, w.sw, st);
+        rc = launch_inv_prefix(dev_psd, nb, n_cat, w.sw, dirty, st);
         if (rc) return rc;
         rc = launch_snr_cand(nb, n_cat, dev_psd, params->rho_th, dev_resolved, nullptr, n_cand, w.sel_idx, sel_count,
-                             near, 1, preselect ? neg_flag : nullptr, true, w.sw, st);
+                             near, 1, preselect ? neg_flag : nullptr, true, w.sw, dirty, st);
         if (rc) return rc;
         GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
         GBFG_CUDA(cudaStreamSynchronize(st));
@@ -287,7 +301,7 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
             rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, nullptr, params->rho_th, nullptr, w.sw, st);
             if (rc) return rc;
             rc = launch_snr_cand(nb, n_cat, dev_psd, params->rho_th, dev_resolved, nullptr, n, w.sel_idx, sel_count,
-                                 near, 1, nullptr, true, w.sw, st);
+                                 near, 1, nullptr, true, w.sw, all_dirty, st);
             if (rc) return rc;
             GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
             GBFG_CUDA(cudaStreamSynchronize(st));
@@ -307,7 +321,7 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
         }
         if (total == 0) break;
         DepositMarks mk = plain_marks(w, nb, it + 1);
-        if (incremental) { mk.med_stamp = w.med_stamp; mk.med_tiles = med_tiles; mk.med_S = median_tile_outputs(W); mk.med_h = W / 2; }
+        mk.blk_stamp = w.blk_stamp; mk.n_dblk = w.plan.n_dblk; mk.dblk_log2 = w.plan.dblk_log2; mk.med_h = W / 2;
         rc = launch_deposit(g, ct, dev_A, dev_f, dev_fdot, w.sel_idx, sel_count, total, -1, dev_spectrum, nullptr,
                             w.diff, w.tile_sums, w.wide_flag, mk, st);
         if (rc) return rc;
@@ -316,8 +330,10 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
         // cap hit: the PSD must match the returned residual (rows of converged catalogs are unchanged)
         for (int c = 0; c < n_cat; ++c)
             if (!done[c]) { host_results[c].n_iter = params->max_iter; host_results[c].converged = 0; }
+        rc = launch_plan(w.blk_stamp, params->max_iter, !incremental, nb, n_cat, W, w.plan, st);
+        if (rc) return rc;
         rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
-                           grid->scale_log2, incremental ? w.med_stamp : nullptr, params->max_iter, nullptr, st);
+                           grid->scale_log2, &w.plan, nullptr, st);
         if (rc) return rc;
     }
     GBFG_CUDA(cudaStreamSynchronize(st));

@@ -3,7 +3,10 @@
 // DESIGN.md R3: odd window W = 2h+1 centred on k, ends reflected, statistic = the h-th smallest
 // of the 2h+1 int64 values.  Only integer comparisons decide the result, so it is exact.
 //
-// One CTA per tile of S = LT - 2h outputs.  The tile and its two h-bin halos (LT positions) are
+// Persistent CTAs, one per SM, take tiles of at most S = LT - 2h consecutive outputs — from the work
+// list plan_kernel derives from the blocks the last subtraction made dirty, or (stage call) from a
+// static tiling of every row.  The tile and its two h-bin halos (Lt = outputs + 2h <= LT positions,
+// rounded up to a multiple of 1024) are
 // staged in shared memory and sorted ONCE by (value, position): an LSD radix sort, 8 bits per pass,
 // that skips the passes whose digit is the same for the whole tile (spectrum values rarely need
 // more than four).  With the sorted order in hand a window is a position interval, and its median
@@ -50,8 +53,9 @@ struct MedianArgs {
     int64_t *med;            // [n_cat][n]
     const double *s_instr;   // [n] or NULL (no PSD)
     double *psd;             // [n_cat][n] or NULL
-    const int *tile_stamp;   // [n_cat][tiles] or NULL: only tiles whose stamp equals `stamp` are recomputed
-    int stamp;
+    const int4 *items;       // work list (row, first output, outputs, -) or NULL: static tiling of every row
+    int *ctr;                // [0] number of items, [1] next item
+    int n_cat;
     int *neg_flag;           // nullable: set to 1 when a median is negative
     int64_t n;
     int h;
@@ -84,16 +88,36 @@ running_median_kernel(MedianArgs a)
     const int warp = tid >> 5, lane = tid & 31;
     const unsigned FULL = 0xffffffffu;
     const unsigned lt_mask = (1u << lane) - 1u;
-    const int tile = blockIdx.x;
-    if (a.tile_stamp && a.tile_stamp[(int64_t)blockIdx.y * a.tiles + tile] != a.stamp) return;
-    const int64_t row = (int64_t)blockIdx.y * a.n;
-    const int64_t o0 = (int64_t)tile * a.S;
     const int h = a.h, W = 2 * a.h + 1;
-    const int n_out = (int)((a.n - o0 < a.S) ? (a.n - o0) : a.S);
+    __shared__ int s_item;
+    bool neg = false;
+
+  for (int64_t turn = blockIdx.x;; turn += gridDim.x) {
+    int64_t row, o0;
+    int n_out;
+    __syncthreads();                                     // the previous tile's epilogue is done with shared memory
+    if (a.items) {
+        if (tid == 0) s_item = atomicAdd(&a.ctr[1], 1);
+        __syncthreads();
+        const int item = s_item;
+        if (item >= a.ctr[0]) break;
+        const int4 v = a.items[item];
+        row = (int64_t)v.x * a.n;
+        o0 = v.y;
+        n_out = v.z;
+    } else {
+        if (turn >= (int64_t)a.tiles * a.n_cat) break;
+        const int64_t r = turn / a.tiles, tile = turn - r * a.tiles;
+        row = r * a.n;
+        o0 = tile * a.S;
+        n_out = (int)((a.n - o0 < a.S) ? (a.n - o0) : a.S);
+    }
     const int Lt = n_out + 2 * h;                        // positions really used
+    const int rounds = (Lt + MED_THREADS - 1) / MED_THREADS;   // keys per thread in the sort (<= MED_ITEMS)
+    const int LTe = rounds * MED_THREADS;                // positions sorted
 
     // ---- stage the tile: position p <-> global bin o0 - h + p, reflected at both ends.
-    // Unused positions (last tile only) repeat position 0: they are never inside a window.
+    // Unused positions (Lt <= p < LTe) repeat position 0: they are never inside a window.
     if (tid < 2) misc[32 + tid] = 0u;
     __syncthreads();
     {
@@ -102,7 +126,7 @@ running_median_kernel(MedianArgs a)
         if (g0 >= a.n) g0 = 2 * a.n - 1 - g0;
         const uint64_t key_ref = (uint64_t)a.x[row + g0] ^ SIGN64;
         uint64_t vary = 0;
-        for (int p = tid; p < MED_LT; p += MED_THREADS) {
+        for (int p = tid; p < LTe; p += MED_THREADS) {
             uint64_t key = key_ref;
             if (p < Lt) {
                 int64_t g = o0 - h + p;
@@ -126,7 +150,7 @@ running_median_kernel(MedianArgs a)
     const int n_pass = vary_all ? (64 - __clzll((long long)vary_all) + 7) / 8 : 0;
 
     // ---- LSD radix sort by key, stable, so that equal keys stay in position order.
-    // Warp w owns elements [256 w, 256 w + 256) of the current order, 32 consecutive ones per round.
+    // Warp w owns elements [32 rounds w, 32 rounds (w + 1)) of the current order, 32 consecutive ones per round.
     for (int pass = 0; pass < n_pass; ++pass) {
         const int shift = 8 * pass;
         for (int e = tid; e < MED_WARPS * MED_CROW / 2; e += MED_THREADS) aux32[e] = 0u;
@@ -135,22 +159,26 @@ running_median_kernel(MedianArgs a)
         uint64_t k[MED_ITEMS];
         uint32_t pp[MED_ITEMS], off[MED_ITEMS], peers[MED_ITEMS];
 #pragma unroll
-        for (int r = 0; r < MED_ITEMS; ++r) {            // the eight matches are independent: issue them together
-            const int e = warp * (32 * MED_ITEMS) + r * 32 + lane;
-            k[r] = skey[e];
-            pp[r] = spos[e];
-            off[r] = (unsigned)(k[r] >> shift) & 255u;
-            peers[r] = __match_any_sync(FULL, off[r]);
+        for (int r = 0; r < MED_ITEMS; ++r) {            // the matches are independent: issue them together
+            if (r < rounds) {
+                const int e = warp * (32 * rounds) + r * 32 + lane;
+                k[r] = skey[e];
+                pp[r] = spos[e];
+                off[r] = (unsigned)(k[r] >> shift) & 255u;
+                peers[r] = __match_any_sync(FULL, off[r]);
+            }
         }
 #pragma unroll
         for (int r = 0; r < MED_ITEMS; ++r) {            // counter updates, round after round
-            const unsigned d = off[r];
-            const unsigned base = cw[d];
-            __syncwarp();
-            const unsigned rank = __popc(peers[r] & lt_mask);
-            if (rank == 0) cw[d] = (uint16_t)(base + __popc(peers[r]));
-            __syncwarp();
-            off[r] = (d << 16) | (base + rank);
+            if (r < rounds) {
+                const unsigned d = off[r];
+                const unsigned base = cw[d];
+                __syncwarp();
+                const unsigned rank = __popc(peers[r] & lt_mask);
+                if (rank == 0) cw[d] = (uint16_t)(base + __popc(peers[r]));
+                __syncwarp();
+                off[r] = (d << 16) | (base + rank);
+            }
         }
         __syncthreads();
         {   // exclusive scan of the counters in (digit, warp) order: thread t owns digit t/4, warps 8(t%4)..+8
@@ -180,9 +208,11 @@ running_median_kernel(MedianArgs a)
         __syncthreads();
 #pragma unroll
         for (int r = 0; r < MED_ITEMS; ++r) {
-            const unsigned dst = (unsigned)cw[off[r] >> 16] + (off[r] & 0xffffu);
-            skey[dst] = k[r];
-            spos[dst] = (uint16_t)pp[r];
+            if (r < rounds) {
+                const unsigned dst = (unsigned)cw[off[r] >> 16] + (off[r] & 0xffffu);
+                skey[dst] = k[r];
+                spos[dst] = (uint16_t)pp[r];
+            }
         }
         __syncthreads();
     }
@@ -190,7 +220,7 @@ running_median_kernel(MedianArgs a)
     // ---- inverse permutation and the count table
     for (int e = tid; e < MED_NRB * MED_TROW / 2; e += MED_THREADS) aux32[e] = 0u;
     __syncthreads();
-    for (int r = tid; r < MED_LT; r += MED_THREADS) {
+    for (int r = tid; r < LTe; r += MED_THREADS) {
         int p = spos[r];
         rop[p] = (uint16_t)r;
         int e = (r / MED_RB) * MED_TROW + (p / MED_PB) + 1;
@@ -241,7 +271,7 @@ running_median_kernel(MedianArgs a)
         const int j0 = c * MED_PB;
         const int b0 = c, b1 = (j0 + W) / MED_PB;
         const int na = b1 * MED_PB - j0;                 // block-aligned part of the window
-        int m = MED_LT, below = 0, phi = j0 - 1;
+        int m = LTe, below = 0, phi = j0 - 1;
         if (na > 0) {
             const int t = (h < na - 1) ? h : na - 1;
             // largest bucket lo with #{rank < 128 lo, position in the aligned part} <= t
@@ -254,13 +284,13 @@ running_median_kernel(MedianArgs a)
             int base = lo * MED_RB;
             for (;;) {                                   // ends inside bucket lo by construction
                 const int r = base + lane;
-                const bool in = r < MED_LT && (unsigned)((int)spos[r < MED_LT ? r : 0] - j0) < (unsigned)na;
+                const bool in = r < LTe && (unsigned)((int)spos[r < LTe ? r : 0] - j0) < (unsigned)na;
                 const unsigned bal = __ballot_sync(FULL, in);
                 const int cn = __popc(bal);
                 if (need < cn) { m = base + nth_set_bit(bal, need + 1); break; }
                 need -= cn;
                 base += 32;
-                if (base >= MED_LT) break;               // not reachable for a consistent table
+                if (base >= LTe) break;                  // not reachable for a consistent table
             }
             below = t;
             phi = b1 * MED_PB - 1;
@@ -288,13 +318,13 @@ running_median_kernel(MedianArgs a)
             int need = h - below + 1, base = m;
             for (;;) {
                 const int r = base + lane;
-                const bool in = r < MED_LT && (unsigned)((int)spos[r < MED_LT ? r : 0] - j0) < (unsigned)W;
+                const bool in = r < LTe && (unsigned)((int)spos[r < LTe ? r : 0] - j0) < (unsigned)W;
                 const unsigned bal = __ballot_sync(FULL, in);
                 const int cn = __popc(bal);
                 if (need <= cn) { m = base + nth_set_bit(bal, need); break; }
                 need -= cn;
                 base += 32;
-                if (base >= MED_LT) break;
+                if (base >= LTe) break;
             }
         }
         if (lane == 0) cm[c] = (uint16_t)m;
@@ -326,14 +356,14 @@ running_median_kernel(MedianArgs a)
             const int wplo = __shfl_sync(FULL, plo, src), wphi = __shfl_sync(FULL, phi, src);      \
             for (;;) {                                                                             \
                 const int r = wm + wdir * (1 + lane);                                              \
-                const bool ok = (unsigned)r < (unsigned)MED_LT;                                    \
+                const bool ok = (unsigned)r < (unsigned)LTe;                                       \
                 const bool in = ok && (unsigned)((int)spos[ok ? r : 0] - wplo) <= (unsigned)(wphi - wplo); \
                 const unsigned bal = __ballot_sync(FULL, in);                                      \
                 const int cn = __popc(bal);                                                        \
                 if (wneed <= cn) { wm += wdir * (1 + nth_set_bit(bal, wneed)); break; }            \
                 wneed -= cn;                                                                       \
                 wm += 32 * wdir;                                                                   \
-                if ((unsigned)wm >= (unsigned)MED_LT) break;   /* not reachable: the window holds the element */ \
+                if ((unsigned)wm >= (unsigned)LTe) break;      /* not reachable: the window holds the element */ \
             }                                                                                      \
             if (lane == src) { m = wm; need = 0; }                                                 \
         }
@@ -378,7 +408,6 @@ running_median_kernel(MedianArgs a)
     __syncthreads();
 
     // ---- coalesced epilogue: median and PSD
-    bool neg = false;
     for (int j = tid; j < n_out; j += MED_THREADS) {
         int64_t v = (int64_t)(skey[orank[j]] ^ SIGN64);
         int64_t g = o0 + j;
@@ -389,6 +418,7 @@ running_median_kernel(MedianArgs a)
             a.psd[row + g] = a.s_instr[g] + a.norm * e;
         }
     }
+  }   // tiles
     if (a.neg_flag && neg) *a.neg_flag = 1;
 }
 
@@ -405,6 +435,118 @@ psd_kernel(const int64_t *__restrict__ med, const double *__restrict__ s_instr, 
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// plan_kernel: one CTA per row.  Turns the dirty-block stamps of the last subtraction into
+//   cum[row][b]  = number of dirty blocks before block b (b = 0 .. n_dblk), and
+//   the work list of the running median: every maximal run of dirty blocks is cut into pieces of at
+//   most S outputs (runs longer than one wave of CTAs are cut into a multiple of `wave` pieces).
+// all_dirty != 0: every block counts as dirty (first iteration, cap branch without tracking).
+// ctr[0] must be zero on entry; ctr[1] (the consumers' ticket) likewise.
+// ---------------------------------------------------------------------------------------------
+constexpr int PLAN_THREADS = 1024;
+constexpr int PLAN_BIG = 64;
+
+struct PlanArgs {
+    const int *blk_stamp;   // [n_cat][n_dblk]
+    int stamp;
+    int all_dirty;
+    int n_dblk, dblk_log2;
+    int64_t n_bins;
+    int S;                  // outputs per tile at most
+    int wave;               // CTAs of one wave of the median kernel
+    int *cum;               // [n_cat][n_dblk + 1]
+    int4 *items;
+    int *ctr;
+    int max_items;
+};
+
+__device__ __forceinline__ void plan_pieces(int64_t len, int S, int wave, int *pieces, int *piece_len)
+{
+    int64_t np = (len + S - 1) / S;
+    if (np > wave) np = (np + wave - 1) / wave * wave;
+    const int64_t pl = (len + np - 1) / np;
+    *piece_len = (int)pl;
+    *pieces = (int)((len + pl - 1) / pl);
+}
+
+__global__ void __launch_bounds__(PLAN_THREADS)
+plan_kernel(PlanArgs a)
+{
+    extern __shared__ int s_cum[];                      // [n_dblk + 1]
+    __shared__ int wtot[32];
+    __shared__ int big_n;
+    __shared__ int big_b0[PLAN_BIG], big_b1[PLAN_BIG], big_base[PLAN_BIG];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int row = blockIdx.x;
+    const int nb = a.n_dblk;
+    const int *st = a.blk_stamp ? a.blk_stamp + (int64_t)row * nb : nullptr;
+    int *cum = a.cum + (int64_t)row * (nb + 1);
+    const int per = (nb + PLAN_THREADS - 1) / PLAN_THREADS;
+    const int b_lo = min(tid * per, nb), b_hi = min(b_lo + per, nb);
+    if (tid == 0) big_n = 0;
+    int cnt = 0;
+    for (int b = b_lo; b < b_hi; ++b) cnt += (a.all_dirty || st[b] == a.stamp) ? 1 : 0;
+    int incl = cnt;
+    for (int o = 1; o < 32; o <<= 1) {
+        const int up = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += up;
+    }
+    if (lane == 31) wtot[warp] = incl;
+    __syncthreads();
+    int run = incl - cnt;
+    for (int w = 0; w < warp; ++w) run += wtot[w];
+    for (int b = b_lo; b < b_hi; ++b) {
+        s_cum[b] = run;
+        cum[b] = run;
+        run += (a.all_dirty || st[b] == a.stamp) ? 1 : 0;
+    }
+    if (b_hi == nb && b_lo < nb) { s_cum[nb] = run; cum[nb] = run; }
+    if (nb == 0 && tid == 0) { s_cum[0] = 0; cum[0] = 0; }
+    __syncthreads();
+    // runs: a dirty block whose predecessor is clean starts one; its end by bisection on cum
+    for (int b = b_lo; b < b_hi; ++b) {
+        const bool dirty = s_cum[b + 1] != s_cum[b];
+        if (!dirty || (b > 0 && s_cum[b] != s_cum[b - 1])) continue;
+        int lo = b + 1, hi = nb;                        // largest e in [b+1, nb] with cum[e] - cum[b] == e - b
+        while (lo < hi) {
+            const int mid = (lo + hi + 1) >> 1;
+            if (s_cum[mid] - s_cum[b] == mid - b) lo = mid; else hi = mid - 1;
+        }
+        const int e = lo;
+        const int64_t first = (int64_t)b << a.dblk_log2;
+        int64_t last = (int64_t)e << a.dblk_log2;
+        if (last > a.n_bins) last = a.n_bins;
+        int pieces, piece_len;
+        plan_pieces(last - first, a.S, a.wave, &pieces, &piece_len);
+        const int base = atomicAdd(&a.ctr[0], pieces);
+        int slot = PLAN_BIG;
+        if (pieces > 8) slot = atomicAdd(&big_n, 1);
+        if (slot < PLAN_BIG) { big_b0[slot] = b; big_b1[slot] = e; big_base[slot] = base; }
+        else {
+            for (int i = 0; i < pieces; ++i) {
+                const int64_t o = first + (int64_t)i * piece_len;
+                const int64_t n_out = (last - o < piece_len) ? last - o : piece_len;
+                if (base + i < a.max_items) a.items[base + i] = make_int4(row, (int)o, (int)n_out, 0);
+            }
+        }
+    }
+    __syncthreads();
+    const int nbig = min(big_n, PLAN_BIG);
+    for (int sgm = 0; sgm < nbig; ++sgm) {
+        const int64_t first = (int64_t)big_b0[sgm] << a.dblk_log2;
+        int64_t last = (int64_t)big_b1[sgm] << a.dblk_log2;
+        if (last > a.n_bins) last = a.n_bins;
+        int pieces, piece_len;
+        plan_pieces(last - first, a.S, a.wave, &pieces, &piece_len);
+        const int base = big_base[sgm];
+        for (int i = tid; i < pieces; i += PLAN_THREADS) {
+            const int64_t o = first + (int64_t)i * piece_len;
+            const int64_t n_out = (last - o < piece_len) ? last - o : piece_len;
+            if (base + i < a.max_items) a.items[base + i] = make_int4(row, (int)o, (int)n_out, 0);
+        }
+    }
+}
+
 int median_tile_outputs(int window) { return MED_LT - (window - 1); }
 
 int median_tiles(int64_t n_bins, int window)
@@ -413,16 +555,59 @@ int median_tiles(int64_t n_bins, int window)
     return (int)((n_bins + S - 1) / S);
 }
 
-// internal entry: median (+ PSD when psd != NULL) of every row.  tile_stamp nullable: recompute only
-// the tiles whose stamp equals `stamp`.  neg_flag nullable: raised when a median is negative.
+// upper bound of the number of work items plan_kernel can emit for one row
+int median_max_items(int64_t n_bins)
+{
+    const int s_min = MED_LT - (GBFG_MAX_WINDOW - 1);
+    return dirty_blocks_per_row(n_bins) + 2 * (int)((n_bins + s_min - 1) / s_min) + 16;
+}
+
+// work list + cum from the stamps (blk_stamp NULL or all_dirty: everything)
+int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins, int n_cat, int window,
+                const MedianPlan &pl, cudaStream_t st)
+{
+    PlanArgs a;
+    a.blk_stamp = blk_stamp; a.stamp = stamp; a.all_dirty = (all_dirty || !blk_stamp) ? 1 : 0;
+    a.n_dblk = pl.n_dblk; a.dblk_log2 = pl.dblk_log2; a.n_bins = n_bins;
+    a.S = MED_LT - (window - 1);
+    a.wave = sm_count();
+    a.cum = pl.cum; a.items = pl.items; a.ctr = pl.ctr; a.max_items = pl.max_items;
+    const size_t smem = sizeof(int) * (size_t)(pl.n_dblk + 1);
+    static thread_local int attr_dev = -1;
+    int dev = 0;
+    GBFG_CUDA(cudaGetDevice(&dev));
+    if (attr_dev != dev) {
+        GBFG_CUDA(cudaFuncSetAttribute(plan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)(sizeof(int) * (DIRTY_MAX_BLOCKS + 1))));
+        attr_dev = dev;
+    }
+    GBFG_CUDA(cudaMemsetAsync(pl.ctr, 0, 2 * sizeof(int), st));
+    {
+        LaunchTimer lt(K_AUX, st);
+        plan_kernel<<<n_cat, PLAN_THREADS, smem, st>>>(a);
+    }
+    GBFG_LAUNCH_CHECK("plan_kernel");
+    return GBFG_OK;
+}
+
+// internal entry: median (+ PSD when psd != NULL).  plan != NULL: the tiles of its work list (made by
+// launch_plan on the same stream); NULL: every row, statically tiled.  neg_flag nullable: raised when
+// a median is negative.
 int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *med,
                   const double *s_instr, double *psd, double norm, int scale_log2,
-                  const int *tile_stamp, int stamp, int *neg_flag, cudaStream_t st)
+                  const MedianPlan *plan, int *neg_flag, cudaStream_t st)
 {
     MedianArgs a;
-    a.x = x; a.med = med; a.s_instr = s_instr; a.psd = psd; a.tile_stamp = tile_stamp; a.stamp = stamp; a.neg_flag = neg_flag;
-    a.n = n_bins; a.h = window / 2; a.S = MED_LT - 2 * a.h;
-    a.tiles = median_tiles(n_bins, window);
+    a.x = x; a.med = med; a.s_instr = s_instr; a.psd = psd; a.neg_flag = neg_flag;
+    a.items = plan ? plan->items : nullptr; a.ctr = plan ? plan->ctr : nullptr; a.n_cat = n_cat;
+    a.n = n_bins; a.h = window / 2;
+    const int s_max = MED_LT - 2 * a.h;
+    const int sms = sm_count();
+    // static tiling: whole waves of CTAs when a row needs more than one
+    int64_t tiles = (n_bins + s_max - 1) / s_max;
+    if (tiles * n_cat > sms && n_cat == 1) tiles = (tiles + sms - 1) / sms * sms;
+    a.S = (int)((n_bins + tiles - 1) / tiles);
+    a.tiles = (int)((n_bins + a.S - 1) / a.S);
     a.norm = norm; a.scale = ldexp(1.0, scale_log2);
     static thread_local int attr_dev = -1;
     int dev = 0;
@@ -431,10 +616,11 @@ int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64
         GBFG_CUDA(cudaFuncSetAttribute(running_median_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MED_SMEM));
         attr_dev = dev;
     }
-    dim3 grid(a.tiles, n_cat);
+    int64_t grid = plan ? sms : (int64_t)a.tiles * n_cat;
+    if (grid > sms) grid = sms;
     {
         LaunchTimer lt(K_MEDIAN, st);
-        running_median_kernel<<<grid, MED_THREADS, MED_SMEM, st>>>(a);
+        running_median_kernel<<<(int)grid, MED_THREADS, MED_SMEM, st>>>(a);
     }
     GBFG_LAUNCH_CHECK("running_median_kernel");
     return GBFG_OK;
@@ -453,7 +639,7 @@ extern "C" int gbfg_running_median(const int64_t *dev_spectrum, int64_t n_bins, 
     if (n_bins < window / 2 + 1) return GBFG_ERR_INVALID_ARG;
     int rc = check_device();
     if (rc) return rc;
-    return launch_median(dev_spectrum, n_bins, n_cat, window, dev_median_out, nullptr, nullptr, 1.0, 0, nullptr, 0, nullptr,
+    return launch_median(dev_spectrum, n_bins, n_cat, window, dev_median_out, nullptr, nullptr, 1.0, 0, nullptr, nullptr,
                          (cudaStream_t)stream);
 }
 
@@ -477,11 +663,3 @@ extern "C" int gbfg_psd(const int64_t *dev_median, const double *dev_s_instr, in
     return GBFG_OK;
 }
 
-namespace gbfg {
-// upper bound of median_tiles over every supported window (workspace sizing)
-int median_max_tiles(int64_t n_bins)
-{
-    const int s_min = MED_LT - (GBFG_MAX_WINDOW - 1);
-    return (int)((n_bins + s_min - 1) / s_min);
-}
-}  // namespace gbfg

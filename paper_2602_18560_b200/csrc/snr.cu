@@ -141,9 +141,16 @@ prefix_header_kernel(const double *__restrict__ arr, int64_t n, int64_t n_bins_r
 // phase A: local inclusive prefix of every tile of PFX_TILE bins + the tile totals
 __global__ void __launch_bounds__(PFX_THREADS)
 inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tiles_per_row,
-                        U128 *__restrict__ pref, U128 *__restrict__ tile_tot, PrefixHeader *hdr)
+                        U128 *__restrict__ pref, U128 *__restrict__ tile_tot, PrefixHeader *hdr, DirtyView dv)
 {
     __shared__ U128 wtot[PFX_THREADS / 32];
+    if (dv.cum) {                                           // psd of this tile unchanged: its prefix stands
+        const int64_t k_first = (int64_t)blockIdx.x * PFX_TILE;
+        int64_t k_last = k_first + PFX_TILE - 1;
+        if (k_last > n_bins - 1) k_last = n_bins - 1;
+        const int *cum = dv.cum + (int64_t)blockIdx.y * (dv.n_dblk + 1);
+        if (cum[(k_last >> dv.dblk_log2) + 1] == cum[k_first >> dv.dblk_log2]) return;
+    }
     const int U = hdr->unit_exp, e_top = hdr->e_top;
     const int64_t row = (int64_t)blockIdx.y * n_bins;
     const int64_t base = (int64_t)blockIdx.x * PFX_TILE + (int64_t)threadIdx.x * PFX_ITEMS;
@@ -180,11 +187,12 @@ inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tile
 
 // phase B: exclusive scan of each row's tile totals (one CTA per row)
 __global__ void __launch_bounds__(1024)
-inv_prefix_tiles_kernel(U128 *__restrict__ tile_tot, int tiles_per_row)
+inv_prefix_tiles_kernel(const U128 *__restrict__ tile_tot, U128 *__restrict__ tile_off, int tiles_per_row)
 {
     __shared__ U128 wtot[32];
     __shared__ U128 carry_s;
-    U128 *rowp = tile_tot + (int64_t)blockIdx.x * tiles_per_row;
+    const U128 *rowp = tile_tot + (int64_t)blockIdx.x * tiles_per_row;
+    U128 *outp = tile_off + (int64_t)blockIdx.x * tiles_per_row;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (threadIdx.x == 0) { carry_s.lo = 0; carry_s.hi = 0; }
     __syncthreads();
@@ -202,7 +210,7 @@ inv_prefix_tiles_kernel(U128 *__restrict__ tile_tot, int tiles_per_row)
         __syncthreads();
         U128 before = carry_s;
         for (int w = 0; w < warp; ++w) before = u128_add(before, wtot[w]);
-        if (idx < tiles_per_row) rowp[idx] = u128_add(before, u128_sub(incl, v));
+        if (idx < tiles_per_row) outp[idx] = u128_add(before, u128_sub(incl, v));
         __syncthreads();
         if (threadIdx.x == 1023) carry_s = u128_add(before, incl);
         __syncthreads();
@@ -318,6 +326,7 @@ struct SnrArgs {
     CandArrays cand;
     const int64_t *cand_count;
     const int *abort_flag;      // nullable: when *abort_flag != 0 the kernel does nothing (loop.cu)
+    DirtyView dv;               // cum != NULL: a candidate whose bins lie in clean blocks is not re-tested
     int64_t n_bins;
     int n_cat;
     double thr;                 // rho_th^2
@@ -344,11 +353,21 @@ snr_cand_kernel(SnrArgs a)
         if (t < n) w = a.cand.w[t];
         bool sel = false, near = false;
         int cat = 0;
-        int64_t src = -1;
+        int64_t src = -1, gk0 = 0;
+        const bool always = w < 0;                          // was near the threshold: counted every iteration
+        if (always) w = -w;
         if (w > 0) {
-            const int64_t gk0 = a.cand.gk0[t];
-            const double four_p = a.cand.four_p[t];
+            gk0 = a.cand.gk0[t];
             if (a.n_cat > 1) cat = (int)(gk0 / a.n_bins);
+            if (a.dv.cum && !always) {
+                // the PSD under this source is what it was at its last test: same rho2, same answer
+                const int64_t k0 = gk0 - (int64_t)cat * a.n_bins;
+                const int *cum = a.dv.cum + (int64_t)cat * (a.dv.n_dblk + 1);
+                if (cum[((k0 + w - 1) >> a.dv.dblk_log2) + 1] == cum[k0 >> a.dv.dblk_log2]) w = 0;
+            }
+        }
+        if (w > 0) {
+            const double four_p = a.cand.four_p[t];
             bool exact;
             double r2 = rho2_of(a.psd, a.pv, pref_ok, unit_exp, gk0, w, a.n_bins, cat, four_p, &exact);
             if (!exact && fabs(r2 / a.thr - 1.0) <= 4e-9) r2 = rho2_direct(a.psd, gk0, w, four_p);   // decide on the definition's sum
@@ -370,6 +389,7 @@ snr_cand_kernel(SnrArgs a)
                 atomicAdd((unsigned long long *)(a.sel_count + 1 + cat), 1ull);
             }
         }
+        if (near && !sel && !always) a.cand.w[t] = -w;
         if (near_mask && a.near_count) {
             if (a.near_per_cat) { if (near) atomicAdd((unsigned long long *)(a.near_count + cat), 1ull); }
             else if (lane == 0) atomicAdd((unsigned long long *)a.near_count, (unsigned long long)__popc(near_mask));
@@ -406,15 +426,16 @@ int launch_prefix_header(const double *arr, int64_t n, int64_t n_bins_row, const
     return GBFG_OK;
 }
 
-// prefix of 1/psd for every row
-int launch_inv_prefix(const double *psd, int64_t n_bins, int n_cat, const SnrWork &sw, cudaStream_t st)
+// prefix of 1/psd for every row; dv.cum != NULL: only the tiles that hold a dirty block are redone
+// (the others must hold the prefix of an earlier call on the same psd values)
+int launch_inv_prefix(const double *psd, int64_t n_bins, int n_cat, const SnrWork &sw, const DirtyView &dv, cudaStream_t st)
 {
     const int tiles = pfx_tiles_per_row(n_bins);
     LaunchTimer lt(K_INV_BLOCKS, st);
     inv_prefix_local_kernel<<<dim3(tiles, n_cat), PFX_THREADS, 0, st>>>(psd, n_bins, tiles, (U128 *)sw.pref,
-                                                                        (U128 *)sw.tile_off, (PrefixHeader *)sw.hdr);
+                                                                        (U128 *)sw.tile_tot, (PrefixHeader *)sw.hdr, dv);
     GBFG_LAUNCH_CHECK("inv_prefix_local_kernel");
-    inv_prefix_tiles_kernel<<<n_cat, 1024, 0, st>>>((U128 *)sw.tile_off, tiles);
+    inv_prefix_tiles_kernel<<<n_cat, 1024, 0, st>>>((const U128 *)sw.tile_tot, (U128 *)sw.tile_off, tiles);
     GBFG_LAUNCH_CHECK("inv_prefix_tiles_kernel");
     return GBFG_OK;
 }
@@ -449,10 +470,11 @@ int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, con
 // sel_count[0 .. n_cat] is accumulated into (zero it for a fresh selection).
 int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th, uint8_t *resolved, double *rho2_out,
                     int64_t n_launch, int64_t *sel_idx, int64_t *sel_count, int64_t *near_count, int near_per_cat,
-                    const int *abort_flag, bool use_prefix, const SnrWork &sw, cudaStream_t st)
+                    const int *abort_flag, bool use_prefix, const SnrWork &sw, const DirtyView &dv, cudaStream_t st)
 {
     if (n_launch <= 0) return GBFG_OK;
     SnrArgs a;
+    a.dv = dv;
     a.psd = psd;
     a.pv = make_view(sw, n_bins);
     if (!use_prefix) { a.pv.pref = nullptr; a.pv.tile_off = nullptr; }
