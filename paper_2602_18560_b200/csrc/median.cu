@@ -67,7 +67,26 @@ struct MedianArgs {
 // n-th (1-based) set bit of a non-zero mask that has at least n bits set
 __device__ __forceinline__ int nth_set_bit(unsigned m, int n)
 {
-    return (int)__fns(m, 0u, n);
+    int pos = 0, c;
+    c = __popc(m & 0xffffu); if (n > c) { n -= c; m >>= 16; pos += 16; }
+    c = __popc(m & 0xffu);   if (n > c) { n -= c; m >>= 8;  pos += 8; }
+    c = __popc(m & 0xfu);    if (n > c) { n -= c; m >>= 4;  pos += 4; }
+    c = __popc(m & 0x3u);    if (n > c) { n -= c; m >>= 2;  pos += 2; }
+    if (n > (int)(m & 1u)) pos += 1;
+    return pos;
+}
+
+// lanes of the warp whose 8-bit digit equals this lane's (what match.any computes, from 8 ballots)
+__device__ __forceinline__ unsigned same_digit_lanes(unsigned d)
+{
+    unsigned peers = 0xffffffffu;
+#pragma unroll
+    for (int b = 0; b < 8; ++b) {
+        const bool bit = (d >> b) & 1u;
+        const unsigned bal = __ballot_sync(0xffffffffu, bit);
+        peers &= bit ? bal : ~bal;
+    }
+    return peers;
 }
 
 __global__ void __launch_bounds__(MED_THREADS, 1)
@@ -165,7 +184,7 @@ running_median_kernel(MedianArgs a)
                 k[r] = skey[e];
                 pp[r] = spos[e];
                 off[r] = (unsigned)(k[r] >> shift) & 255u;
-                peers[r] = __match_any_sync(FULL, off[r]);
+                peers[r] = same_digit_lanes(off[r]);
             }
         }
 #pragma unroll
@@ -484,8 +503,10 @@ plan_kernel(PlanArgs a)
     const int per = (nb + PLAN_THREADS - 1) / PLAN_THREADS;
     const int b_lo = min(tid * per, nb), b_hi = min(b_lo + per, nb);
     if (tid == 0) big_n = 0;
+    for (int b = tid; b < nb; b += PLAN_THREADS) s_cum[b + 1] = (a.all_dirty || st[b] == a.stamp) ? 1 : 0;   // coalesced
+    __syncthreads();
     int cnt = 0;
-    for (int b = b_lo; b < b_hi; ++b) cnt += (a.all_dirty || st[b] == a.stamp) ? 1 : 0;
+    for (int b = b_lo; b < b_hi; ++b) cnt += s_cum[b + 1];
     int incl = cnt;
     for (int o = 1; o < 32; o <<= 1) {
         const int up = __shfl_up_sync(0xffffffffu, incl, o);
@@ -495,13 +516,13 @@ plan_kernel(PlanArgs a)
     __syncthreads();
     int run = incl - cnt;
     for (int w = 0; w < warp; ++w) run += wtot[w];
-    for (int b = b_lo; b < b_hi; ++b) {
-        s_cum[b] = run;
-        cum[b] = run;
-        run += (a.all_dirty || st[b] == a.stamp) ? 1 : 0;
+    if (tid == 0) s_cum[0] = 0;
+    for (int b = b_lo; b < b_hi; ++b) {                 // s_cum[b + 1] = flag of block b -> inclusive count
+        run += s_cum[b + 1];
+        s_cum[b + 1] = run;
     }
-    if (b_hi == nb && b_lo < nb) { s_cum[nb] = run; cum[nb] = run; }
-    if (nb == 0 && tid == 0) { s_cum[0] = 0; cum[0] = 0; }
+    __syncthreads();
+    for (int b = tid; b <= nb; b += PLAN_THREADS) cum[b] = s_cum[b];
     __syncthreads();
     // runs: a dirty block whose predecessor is clean starts one; its end by bisection on cum
     for (int b = b_lo; b < b_hi; ++b) {
