@@ -74,7 +74,7 @@ inline GridDev make_grid_dev(const gbfg_grid *g)
 // change: those within h bins of a bin it touched.  plan_kernel (median.cu) turns the stamps of
 // one iteration into (a) the work list of the running median, (b) cum[c][b] = number of dirty
 // blocks before block b, which lets the prefix of 1/S_n and the SNR test skip what did not change.
-constexpr int DIRTY_MAX_BLOCKS = 32768;
+constexpr int DIRTY_MAX_BLOCKS = 16384;
 
 inline int dirty_block_log2(int64_t n_bins)
 {

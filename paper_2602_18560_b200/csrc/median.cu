@@ -463,7 +463,7 @@ psd_kernel(const int64_t *__restrict__ med, const double *__restrict__ s_instr, 
 // ctr[0] must be zero on entry; ctr[1] (the consumers' ticket) likewise.
 // ---------------------------------------------------------------------------------------------
 constexpr int PLAN_THREADS = 1024;
-constexpr int PLAN_BIG = 64;
+constexpr int PLAN_MIN_OUT = 512;              // outputs of the smallest tile the plan cuts
 
 struct PlanArgs {
     const int *blk_stamp;   // [n_cat][n_dblk]
@@ -479,22 +479,25 @@ struct PlanArgs {
     int max_items;
 };
 
-__device__ __forceinline__ void plan_pieces(int64_t len, int S, int wave, int *pieces, int *piece_len)
+// len < 2^31 (n_bins is): 32-bit divisions, the 64-bit ones are long instruction sequences
+static size_t plan_smem_bytes(int n_dblk) { return sizeof(int) * (size_t)((n_dblk + 1) + 3 * (n_dblk / 2 + 1)); }
+
+__device__ __forceinline__ void plan_pieces(int64_t len64, int S, int wave, int *pieces, int *piece_len)
 {
-    int64_t np = (len + S - 1) / S;
-    if (np > wave) np = (np + wave - 1) / wave * wave;
-    const int64_t pl = (len + np - 1) / np;
+    const unsigned len = (unsigned)len64;
+    unsigned np = (len + (unsigned)S - 1u) / (unsigned)S;
+    if (np > (unsigned)wave) np = (np + (unsigned)wave - 1u) / (unsigned)wave * (unsigned)wave;
+    const unsigned pl = (len + np - 1u) / np;
     *piece_len = (int)pl;
-    *pieces = (int)((len + pl - 1) / pl);
+    *pieces = (int)((len + pl - 1u) / pl);
 }
 
 __global__ void __launch_bounds__(PLAN_THREADS)
 plan_kernel(PlanArgs a)
 {
-    extern __shared__ int s_cum[];                      // [n_dblk + 1]
+    extern __shared__ int s_cum[];                      // [n_dblk + 1], then the runs: 3 ints each, [n_dblk / 2 + 1]
     __shared__ int wtot[32];
-    __shared__ int big_n;
-    __shared__ int big_b0[PLAN_BIG], big_b1[PLAN_BIG], big_base[PLAN_BIG];
+    __shared__ int n_runs, row_pieces, row_base;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int row = blockIdx.x;
     const int nb = a.n_dblk;
@@ -502,8 +505,21 @@ plan_kernel(PlanArgs a)
     int *cum = a.cum + (int64_t)row * (nb + 1);
     const int per = (nb + PLAN_THREADS - 1) / PLAN_THREADS;
     const int b_lo = min(tid * per, nb), b_hi = min(b_lo + per, nb);
-    if (tid == 0) big_n = 0;
-    for (int b = tid; b < nb; b += PLAN_THREADS) s_cum[b + 1] = (a.all_dirty || st[b] == a.stamp) ? 1 : 0;   // coalesced
+    int *s_run = s_cum + nb + 1;
+    if (tid == 0) { n_runs = 0; row_pieces = 0; }
+    for (int b0 = tid; b0 < nb; b0 += 8 * PLAN_THREADS) {   // coalesced, eight loads in flight per thread
+        int v[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int b = b0 + u * PLAN_THREADS;
+            v[u] = (!a.all_dirty && b < nb) ? st[b] : a.stamp;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const int b = b0 + u * PLAN_THREADS;
+            if (b < nb) s_cum[b + 1] = (v[u] == a.stamp) ? 1 : 0;
+        }
+    }
     __syncthreads();
     int cnt = 0;
     for (int b = b_lo; b < b_hi; ++b) cnt += s_cum[b + 1];
@@ -524,7 +540,20 @@ plan_kernel(PlanArgs a)
     __syncthreads();
     for (int b = tid; b <= nb; b += PLAN_THREADS) cum[b] = s_cum[b];
     __syncthreads();
-    // runs: a dirty block whose predecessor is clean starts one; its end by bisection on cum
+    // Tile size of this row: S outputs at most, less when the dirty part of the row would not fill
+    // the row's share of one wave of CTAs (the latency of a short tile is what the tail iterations pay).
+    int S = a.S;
+    {
+        const unsigned dirty_out = (unsigned)s_cum[nb] << a.dblk_log2;      // <= n_bins + one block
+        int share = a.wave / (int)gridDim.x;
+        if (share < 1) share = 1;
+        unsigned s_fit = (dirty_out + (unsigned)share - 1u) / (unsigned)share;
+        if (s_fit < (unsigned)PLAN_MIN_OUT) s_fit = PLAN_MIN_OUT;
+        if (s_fit < (unsigned)S) S = (int)s_fit;
+    }
+    // runs: a dirty block whose predecessor is clean starts one; its end by bisection on cum.
+    // Every run is recorded in shared memory with the place of its pieces in the row's part of the
+    // list; then the warps write the items, one run per warp at a time.
     for (int b = b_lo; b < b_hi; ++b) {
         const bool dirty = s_cum[b + 1] != s_cum[b];
         if (!dirty || (b > 0 && s_cum[b] != s_cum[b - 1])) continue;
@@ -538,29 +567,27 @@ plan_kernel(PlanArgs a)
         int64_t last = (int64_t)e << a.dblk_log2;
         if (last > a.n_bins) last = a.n_bins;
         int pieces, piece_len;
-        plan_pieces(last - first, a.S, a.wave, &pieces, &piece_len);
-        const int base = atomicAdd(&a.ctr[0], pieces);
-        int slot = PLAN_BIG;
-        if (pieces > 8) slot = atomicAdd(&big_n, 1);
-        if (slot < PLAN_BIG) { big_b0[slot] = b; big_b1[slot] = e; big_base[slot] = base; }
-        else {
-            for (int i = 0; i < pieces; ++i) {
-                const int64_t o = first + (int64_t)i * piece_len;
-                const int64_t n_out = (last - o < piece_len) ? last - o : piece_len;
-                if (base + i < a.max_items) a.items[base + i] = make_int4(row, (int)o, (int)n_out, 0);
-            }
-        }
+        plan_pieces(last - first, S, a.wave, &pieces, &piece_len);
+        const int slot = atomicAdd(&n_runs, 1);
+        s_run[3 * slot] = b;
+        s_run[3 * slot + 1] = e;
+        s_run[3 * slot + 2] = atomicAdd(&row_pieces, pieces);
     }
     __syncthreads();
-    const int nbig = min(big_n, PLAN_BIG);
-    for (int sgm = 0; sgm < nbig; ++sgm) {
-        const int64_t first = (int64_t)big_b0[sgm] << a.dblk_log2;
-        int64_t last = (int64_t)big_b1[sgm] << a.dblk_log2;
+    if (tid == 0) {
+        if (gridDim.x == 1) { row_base = 0; a.ctr[0] = row_pieces; }
+        else row_base = atomicAdd(&a.ctr[0], row_pieces);
+    }
+    __syncthreads();
+    const int nr = n_runs, rb0 = row_base;
+    for (int r = warp; r < nr; r += PLAN_THREADS / 32) {
+        const int64_t first = (int64_t)s_run[3 * r] << a.dblk_log2;
+        int64_t last = (int64_t)s_run[3 * r + 1] << a.dblk_log2;
         if (last > a.n_bins) last = a.n_bins;
         int pieces, piece_len;
-        plan_pieces(last - first, a.S, a.wave, &pieces, &piece_len);
-        const int base = big_base[sgm];
-        for (int i = tid; i < pieces; i += PLAN_THREADS) {
+        plan_pieces(last - first, S, a.wave, &pieces, &piece_len);
+        const int base = rb0 + s_run[3 * r + 2];
+        for (int i = lane; i < pieces; i += 32) {
             const int64_t o = first + (int64_t)i * piece_len;
             const int64_t n_out = (last - o < piece_len) ? last - o : piece_len;
             if (base + i < a.max_items) a.items[base + i] = make_int4(row, (int)o, (int)n_out, 0);
@@ -580,7 +607,8 @@ int median_tiles(int64_t n_bins, int window)
 int median_max_items(int64_t n_bins)
 {
     const int s_min = MED_LT - (GBFG_MAX_WINDOW - 1);
-    return dirty_blocks_per_row(n_bins) + 2 * (int)((n_bins + s_min - 1) / s_min) + 16;
+    const int s_small = s_min < PLAN_MIN_OUT ? s_min : PLAN_MIN_OUT;
+    return dirty_blocks_per_row(n_bins) + 2 * (int)((n_bins + s_small - 1) / s_small) + 16;
 }
 
 // work list + cum from the stamps (blk_stamp NULL or all_dirty: everything)
@@ -593,13 +621,13 @@ int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins,
     a.S = MED_LT - (window - 1);
     a.wave = sm_count();
     a.cum = pl.cum; a.items = pl.items; a.ctr = pl.ctr; a.max_items = pl.max_items;
-    const size_t smem = sizeof(int) * (size_t)(pl.n_dblk + 1);
+    const size_t smem = plan_smem_bytes(pl.n_dblk);
     static thread_local int attr_dev = -1;
     int dev = 0;
     GBFG_CUDA(cudaGetDevice(&dev));
     if (attr_dev != dev) {
         GBFG_CUDA(cudaFuncSetAttribute(plan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)(sizeof(int) * (DIRTY_MAX_BLOCKS + 1))));
+                                       (int)plan_smem_bytes(DIRTY_MAX_BLOCKS)));
         attr_dev = dev;
     }
     GBFG_CUDA(cudaMemsetAsync(pl.ctr, 0, 2 * sizeof(int), st));
