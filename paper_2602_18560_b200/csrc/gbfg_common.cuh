@@ -90,6 +90,7 @@ inline int dirty_blocks_per_row(int64_t n_bins)
 
 struct DirtyView {
     const int *cum;     // [n_cat][n_dblk + 1], NULL: everything is dirty
+    const int *range;   // [n_cat][2] first and last dirty block of each row (first > last: none)
     int n_dblk;
     int dblk_log2;
 };
@@ -111,6 +112,7 @@ struct MedianPlan {
     int4 *items;
     int *ctr;           // [0] number of items, [1] next item to take (both zero before plan_kernel)
     int *cum;           // [n_cat][n_dblk + 1]
+    int *range;         // [n_cat][2] first and last dirty block
     int n_dblk;
     int dblk_log2;
     int max_items;
@@ -127,6 +129,18 @@ struct SnrWork {
     double *cand_4p;    // [n_src_total]
     int64_t *cand_src;  // [n_src_total] global source index
     int64_t *cand_count;// [1 + n_cat]: number of records, per catalog
+    // the records as first compacted (any order); the arrays above hold them ordered by (row, dirty
+    // block of the first bin), which makes the gathers of the test coherent and lets it skip the
+    // part of the list that lies outside the dirty range
+    int64_t *tmp_gk0;   // [n_src_total]
+    int32_t *tmp_w;
+    double *tmp_4p;
+    int64_t *tmp_src;
+    int *bkt_count;     // [n_cat][n_dblk]      records per bucket, then the scatter cursor
+    int *bkt_ext;       // [n_cat][n_dblk]      last block any record of the bucket reaches, then its prefix maximum
+    int *bkt_reach;     // [n_cat][n_dblk]      first bucket with a record that reaches block b (n_dblk: none)
+    int64_t *bkt_off;   // [n_cat][n_dblk + 1]  first record of each bucket (global record index)
+    int *any_near;      // one int: a record was flagged near-threshold (the whole list is tested from then on)
 };
 
 // ---------------------------------------------------------------------------------------------

@@ -78,6 +78,7 @@ static Workspace carve(void *base, int64_t n_bins, int64_t n_src_total, int n_ca
     w.plan.dblk_log2 = dirty_block_log2(n_bins);
     w.plan.max_items = n_cat * median_max_items(n_bins);
     w.plan.cum = (int *)take(sizeof(int) * (size_t)n_cat * (size_t)(n_dblk + 1));
+    w.plan.range = (int *)take(sizeof(int) * 2 * (size_t)n_cat);
     w.plan.items = (int4 *)take(sizeof(int4) * (size_t)w.plan.max_items);
     w.plan.ctr = (int *)take(sizeof(int) * 4);
     w.sel_idx = (int64_t *)take(sizeof(int64_t) * nsrc);
@@ -92,6 +93,15 @@ static Workspace carve(void *base, int64_t n_bins, int64_t n_src_total, int n_ca
     w.sw.cand_4p = (double *)take(sizeof(double) * nsrc);
     w.sw.cand_src = (int64_t *)take(sizeof(int64_t) * nsrc);
     w.sw.cand_count = w.counters + 2 + 2 * n_cat;
+    w.sw.tmp_gk0 = (int64_t *)take(sizeof(int64_t) * nsrc);
+    w.sw.tmp_w = (int32_t *)take(sizeof(int32_t) * nsrc);
+    w.sw.tmp_4p = (double *)take(sizeof(double) * nsrc);
+    w.sw.tmp_src = (int64_t *)take(sizeof(int64_t) * nsrc);
+    w.sw.bkt_count = (int *)take(sizeof(int) * (size_t)n_cat * (size_t)n_dblk);
+    w.sw.bkt_ext = (int *)take(sizeof(int) * (size_t)n_cat * (size_t)n_dblk);
+    w.sw.bkt_reach = (int *)take(sizeof(int) * (size_t)n_cat * (size_t)n_dblk);
+    w.sw.bkt_off = (int64_t *)take(sizeof(int64_t) * (size_t)n_cat * (size_t)(n_dblk + 1));
+    w.sw.any_near = (int *)take(sizeof(int));
     w.bytes = off;
     return w;
 }
@@ -201,7 +211,7 @@ extern "C" int gbfg_snr_select(const gbfg_grid *grid, const double *dev_A, const
     // every unresolved valid source is a candidate (no pre-selection: the PSD is the caller's)
     rc = launch_prefix_header(dev_psd, (int64_t)n_cat * grid->n_bins, grid->n_bins, w.sw, st);
     if (rc) return rc;
-    const DirtyView all_dirty = {nullptr, 0, 0};
+    const DirtyView all_dirty = {nullptr, nullptr, 0, 0};
     rc = launch_inv_prefix(dev_psd, grid->n_bins, n_cat, w.sw, all_dirty, st);
     if (rc) return rc;
     rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, nullptr, rho_th, dev_rho2_out, w.sw, st);
@@ -256,8 +266,8 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     GBFG_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(int64_t) * WS_COUNTERS, st));
     GBFG_CUDA(cudaMemsetAsync(w.scan_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)scan_tiles, st));
     GBFG_CUDA(cudaMemsetAsync(w.blk_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)w.plan.n_dblk, st));
-    const DirtyView all_dirty = {nullptr, 0, 0};
-    const DirtyView dirty = {w.plan.cum, w.plan.n_dblk, w.plan.dblk_log2};
+    const DirtyView all_dirty = {nullptr, nullptr, 0, 0};
+    const DirtyView dirty = {w.plan.cum, w.plan.range, w.plan.n_dblk, w.plan.dblk_log2};
 
     // candidate records: with pre-selection, only sources whose rho^2 against S_instr reaches the threshold
     rc = launch_prefix_header(dev_s_instr, nb, nb, w.sw, st);

@@ -474,6 +474,7 @@ struct PlanArgs {
     int S;                  // outputs per tile at most
     int wave;               // CTAs of one wave of the median kernel
     int *cum;               // [n_cat][n_dblk + 1]
+    int *range;             // [n_cat][2]
     int4 *items;
     int *ctr;
     int max_items;
@@ -538,7 +539,14 @@ plan_kernel(PlanArgs a)
         s_cum[b + 1] = run;
     }
     __syncthreads();
-    for (int b = tid; b <= nb; b += PLAN_THREADS) cum[b] = s_cum[b];
+    for (int b = tid; b <= nb; b += PLAN_THREADS) {
+        cum[b] = s_cum[b];
+        if (b < nb && s_cum[b + 1] != s_cum[b]) {          // first / last dirty block of the row
+            if (s_cum[b] == 0) a.range[2 * row] = b;
+            if (s_cum[b + 1] == s_cum[nb]) a.range[2 * row + 1] = b;
+        }
+    }
+    if (tid == 0 && s_cum[nb] == 0) { a.range[2 * row] = 1; a.range[2 * row + 1] = 0; }
     __syncthreads();
     // Tile size of this row: S outputs at most, less when the dirty part of the row would not fill
     // the row's share of one wave of CTAs (the latency of a short tile is what the tail iterations pay).
@@ -620,7 +628,7 @@ int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins,
     a.n_dblk = pl.n_dblk; a.dblk_log2 = pl.dblk_log2; a.n_bins = n_bins;
     a.S = MED_LT - (window - 1);
     a.wave = sm_count();
-    a.cum = pl.cum; a.items = pl.items; a.ctr = pl.ctr; a.max_items = pl.max_items;
+    a.cum = pl.cum; a.range = pl.range; a.items = pl.items; a.ctr = pl.ctr; a.max_items = pl.max_items;
     const size_t smem = plan_smem_bytes(pl.n_dblk);
     static thread_local int attr_dev = -1;
     int dev = 0;

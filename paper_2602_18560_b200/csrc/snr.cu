@@ -274,6 +274,8 @@ struct BuildArgs {
     CandArrays cand;
     int64_t *cand_count;        // [1 + n_cat]: total, per catalog
     int64_t n_all;
+    int *bkt_count, *bkt_ext;   // [n_cat][n_dblk]: zero on entry
+    int n_dblk, dblk_log2;
 };
 
 __global__ void __launch_bounds__(256)
@@ -315,8 +317,86 @@ cand_build_kernel(GridDev g, CatTable ct, BuildArgs a)
                 a.cand.four_p[t] = 4.0 * s.p;
                 a.cand.src[t] = i;
                 if (ct.n_cat > 1) atomicAdd((unsigned long long *)(a.cand_count + 1 + cat), 1ull);
+                const int64_t gb = (int64_t)cat * a.n_dblk + (s.k0 >> a.dblk_log2);
+                atomicAdd(a.bkt_count + gb, 1);
+                atomicMax(a.bkt_ext + gb, (int)((s.k0 + s.w_eff - 1) >> a.dblk_log2));
             }
         }
+    }
+}
+
+// Buckets = (row, dirty block of the first bin).  One CTA per row: first record of every bucket
+// (exclusive scan of the counts, on top of the records of the rows before), the scatter cursors,
+// and the prefix maximum of the last block reached.
+constexpr int BKT_THREADS = 1024;
+
+__global__ void __launch_bounds__(BKT_THREADS)
+cand_bucket_scan_kernel(int *__restrict__ bkt_count, int *__restrict__ bkt_ext, int64_t *__restrict__ bkt_off,
+                        const int64_t *__restrict__ cand_count, int n_dblk)
+{
+    __shared__ int wsum[32], wmax[32];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int row = blockIdx.x;
+    int64_t base = 0;
+    if (gridDim.x > 1) for (int c = 0; c < row; ++c) base += cand_count[1 + c];
+    int *cnt = bkt_count + (int64_t)row * n_dblk;
+    int *ext = bkt_ext + (int64_t)row * n_dblk;
+    int64_t *off = bkt_off + (int64_t)row * (n_dblk + 1);
+    const int per = (n_dblk + BKT_THREADS - 1) / BKT_THREADS;
+    const int b_lo = min(tid * per, n_dblk), b_hi = min(b_lo + per, n_dblk);
+    int s = 0, m = -1;
+    for (int b = b_lo; b < b_hi; ++b) { s += cnt[b]; m = max(m, cnt[b] ? ext[b] : -1); }
+    int incl = s, imax = m;
+    for (int o = 1; o < 32; o <<= 1) {
+        const int us = __shfl_up_sync(0xffffffffu, incl, o), um = __shfl_up_sync(0xffffffffu, imax, o);
+        if (lane >= o) { incl += us; imax = max(imax, um); }
+    }
+    if (lane == 31) { wsum[warp] = incl; wmax[warp] = imax; }
+    __syncthreads();
+    int run = incl - s;
+    int pm = __shfl_up_sync(0xffffffffu, imax, 1);
+    if (lane == 0) pm = -1;
+    for (int w = 0; w < warp; ++w) { run += wsum[w]; pm = max(pm, wmax[w]); }
+    for (int b = b_lo; b < b_hi; ++b) {
+        const int c = cnt[b];
+        off[b] = base + run;
+        cnt[b] = 0;                                    // becomes the scatter cursor (relative to off[b])
+        if (c) pm = max(pm, ext[b]);
+        ext[b] = pm;
+        run += c;
+    }
+    if (tid == BKT_THREADS - 1) off[n_dblk] = base + run;
+}
+
+// reach[b] = first bucket whose records reach block b = first index with prefix maximum >= b (n_dblk: none)
+__global__ void __launch_bounds__(256)
+cand_bucket_reach_kernel(const int *__restrict__ bkt_pm, int *__restrict__ bkt_reach, int n_dblk)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= n_dblk) return;
+    const int *pm = bkt_pm + (int64_t)blockIdx.y * n_dblk;
+    int lo = 0, hi = n_dblk;
+    while (lo < hi) { const int mid = (lo + hi) >> 1; if (pm[mid] >= b) hi = mid; else lo = mid + 1; }
+    bkt_reach[(int64_t)blockIdx.y * n_dblk + b] = lo;
+}
+
+struct CandArraysConst { const int64_t *gk0; const int32_t *w; const double *four_p; const int64_t *src; };
+
+__global__ void __launch_bounds__(256)
+cand_scatter_kernel(CandArraysConst in, CandArrays out, const int64_t *__restrict__ cand_count, int *__restrict__ bkt_cur,
+                    const int64_t *__restrict__ bkt_off, int64_t n_bins, int n_dblk, int dblk_log2)
+{
+    const int64_t n = *cand_count;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += stride) {
+        const int64_t gk0 = in.gk0[t];
+        const int64_t row = gk0 / n_bins;
+        const int64_t b = (gk0 - row * n_bins) >> dblk_log2;
+        const int64_t dst = bkt_off[row * (n_dblk + 1) + b] + atomicAdd(bkt_cur + row * n_dblk + b, 1);
+        out.gk0[dst] = gk0;
+        out.w[dst] = in.w[t];
+        out.four_p[dst] = in.four_p[t];
+        out.src[dst] = in.src[t];
     }
 }
 
@@ -327,6 +407,10 @@ struct SnrArgs {
     const int64_t *cand_count;
     const int *abort_flag;      // nullable: when *abort_flag != 0 the kernel does nothing (loop.cu)
     DirtyView dv;               // cum != NULL: a candidate whose bins lie in clean blocks is not re-tested
+    const int64_t *bkt_off;     // [n_cat][n_dblk + 1] first record of each bucket
+    const int *bkt_reach;       // [n_cat][n_dblk] first bucket with a record that reaches block b
+    int *any_near;
+    int n_dblk;
     int64_t n_bins;
     int n_cat;
     double thr;                 // rho_th^2
@@ -343,12 +427,23 @@ snr_cand_kernel(SnrArgs a)
 {
     if (a.abort_flag && *a.abort_flag) return;
     const int lane = threadIdx.x & 31;
-    const int64_t n = *a.cand_count;
+    // records of row blockIdx.y, narrowed to the buckets that can reach a dirty block
+    const int rowc = blockIdx.y;
+    const int64_t *off = a.bkt_off + (int64_t)rowc * (a.n_dblk + 1);
+    int64_t t_first = off[0], n = off[a.n_dblk];
+    if (a.dv.cum && *a.any_near == 0) {
+        const int b_min = a.dv.range[2 * rowc], b_max = a.dv.range[2 * rowc + 1];
+        if (b_min > b_max) return;                          // nothing dirty in this row
+        const int first_bucket = a.bkt_reach[(int64_t)rowc * a.n_dblk + b_min];
+        if (first_bucket >= a.n_dblk) return;
+        t_first = off[first_bucket];
+        n = off[b_max + 1];
+    }
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    const int64_t n_round = (n + 31) & ~(int64_t)31;
+    const int64_t n_round = t_first + ((n - t_first + 31) & ~(int64_t)31);
     const bool pref_ok = a.pv.pref && a.pv.hdr->bad == 0;
     const int unit_exp = a.pv.pref ? a.pv.hdr->unit_exp : 0;
-    for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n_round; t += stride) {
+    for (int64_t t = t_first + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n_round; t += stride) {
         int32_t w = 0;
         if (t < n) w = a.cand.w[t];
         bool sel = false, near = false;
@@ -389,7 +484,7 @@ snr_cand_kernel(SnrArgs a)
                 atomicAdd((unsigned long long *)(a.sel_count + 1 + cat), 1ull);
             }
         }
-        if (near && !sel && !always) a.cand.w[t] = -w;
+        if (near && !sel && !always) { a.cand.w[t] = -w; *a.any_near = 1; }
         if (near_mask && a.near_count) {
             if (a.near_per_cat) { if (near) atomicAdd((unsigned long long *)(a.near_count + cat), 1ull); }
             else if (lane == 0) atomicAdd((unsigned long long *)a.near_count, (unsigned long long)__popc(near_mask));
@@ -454,15 +549,29 @@ int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, con
     a.pv = make_view(sw, g.n_bins);
     a.thr_pre = (rho_th * rho_th) * (1.0 - 4e-9);    // keeps every source the near-threshold count (2e-9) can see
     a.rho2_out = rho2_out;
-    a.cand.gk0 = sw.cand_gk0; a.cand.w = sw.cand_w; a.cand.four_p = sw.cand_4p; a.cand.src = sw.cand_src;
+    a.cand.gk0 = sw.tmp_gk0; a.cand.w = sw.tmp_w; a.cand.four_p = sw.tmp_4p; a.cand.src = sw.tmp_src;
     a.cand_count = sw.cand_count;
     a.n_all = n;
+    const int n_dblk = dirty_blocks_per_row(g.n_bins), dblk_log2 = dirty_block_log2(g.n_bins);
+    a.bkt_count = sw.bkt_count; a.bkt_ext = sw.bkt_ext; a.n_dblk = n_dblk; a.dblk_log2 = dblk_log2;
+    GBFG_CUDA(cudaMemsetAsync(sw.bkt_count, 0, sizeof(int) * (size_t)ct.n_cat * (size_t)n_dblk, st));
+    GBFG_CUDA(cudaMemsetAsync(sw.bkt_ext, 0, sizeof(int) * (size_t)ct.n_cat * (size_t)n_dblk, st));
+    GBFG_CUDA(cudaMemsetAsync(sw.any_near, 0, sizeof(int), st));
     int64_t blocks = (n + 255) / 256;
     const int64_t cap = (int64_t)sm_count() * 16;
     if (blocks > cap) blocks = cap;
     LaunchTimer lt(K_SNR, st);
     cand_build_kernel<<<(int)blocks, 256, 0, st>>>(g, ct, a);
     GBFG_LAUNCH_CHECK("cand_build_kernel");
+    // order the records by (row, dirty block of the first bin)
+    cand_bucket_scan_kernel<<<ct.n_cat, BKT_THREADS, 0, st>>>(sw.bkt_count, sw.bkt_ext, sw.bkt_off, sw.cand_count, n_dblk);
+    GBFG_LAUNCH_CHECK("cand_bucket_scan_kernel");
+    cand_bucket_reach_kernel<<<dim3((n_dblk + 255) / 256, ct.n_cat), 256, 0, st>>>(sw.bkt_ext, sw.bkt_reach, n_dblk);
+    GBFG_LAUNCH_CHECK("cand_bucket_reach_kernel");
+    CandArraysConst in = {sw.tmp_gk0, sw.tmp_w, sw.tmp_4p, sw.tmp_src};
+    CandArrays out = {sw.cand_gk0, sw.cand_w, sw.cand_4p, sw.cand_src};
+    cand_scatter_kernel<<<(int)blocks, 256, 0, st>>>(in, out, sw.cand_count, sw.bkt_count, sw.bkt_off, g.n_bins, n_dblk, dblk_log2);
+    GBFG_LAUNCH_CHECK("cand_scatter_kernel");
     return GBFG_OK;
 }
 
@@ -485,11 +594,13 @@ int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th,
     a.thr = rho_th * rho_th;
     a.resolved = resolved; a.rho2_out = rho2_out; a.sel_idx = sel_idx; a.sel_count = sel_count;
     a.near_count = near_count; a.near_per_cat = near_per_cat;
-    int64_t blocks = (n_launch + 255) / 256;
-    const int64_t cap = (int64_t)sm_count() * 16;
+    a.bkt_off = sw.bkt_off; a.bkt_reach = sw.bkt_reach; a.any_near = sw.any_near; a.n_dblk = dirty_blocks_per_row(n_bins);
+    int64_t blocks = (n_launch / n_cat + 255) / 256 + 1;   // per row; the rows share the records unevenly: grid-stride
+    int64_t cap = (int64_t)sm_count() * 16 / n_cat;
+    if (cap < 4) cap = 4;
     if (blocks > cap) blocks = cap;
     LaunchTimer lt(K_SNR, st);
-    snr_cand_kernel<<<(int)blocks, 256, 0, st>>>(a);
+    snr_cand_kernel<<<dim3((unsigned)blocks, (unsigned)n_cat), 256, 0, st>>>(a);
     GBFG_LAUNCH_CHECK("snr_cand_kernel");
     return GBFG_OK;
 }
