@@ -49,7 +49,7 @@ deposit_kernel(GridDev g, CatTable ct, const double *__restrict__ A, const doubl
                 atomic_add_i64(diff + row + s.k0 + s.w_eff, -v);
                 mk.scan_stamp[(int64_t)cat * mk.scan_tiles + (s.k0 + s.w_eff) / SCAN_TILE] = mk.stamp;
             }
-            *wide_flag = 1;
+            *wide_flag = mk.stamp;
         }
         if (mk.blk_stamp) {
             // outputs k with |k - b| <= h see bin b (reflected ends included)
@@ -67,61 +67,61 @@ deposit_kernel(GridDev g, CatTable ct, const double *__restrict__ A, const doubl
     }
 }
 
-// phase 1: tile sums of the difference array.  grid = (tiles_per_row, n_cat)
+// phase 1: tile sums of the difference array, grid = (tiles_per_row, n_cat); the last CTA of a row
+// to finish (ticket) turns the row's tile sums into exclusive offsets (phase 2).
 __global__ void __launch_bounds__(SCAN_THREADS)
 scan_tile_sums_kernel(const int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
                       int64_t *__restrict__ tile_sums, const int *__restrict__ wide_flag,
-                      const int *__restrict__ scan_stamp, int stamp)
+                      const int *__restrict__ scan_stamp, int stamp, unsigned *__restrict__ ticket)
 {
-    if (*wide_flag == 0) return;
+    if (*wide_flag != stamp) return;
     __shared__ int64_t warp_sum[SCAN_THREADS / 32];
-    if (scan_stamp[(int64_t)blockIdx.y * tiles_per_row + blockIdx.x] != stamp) {      // untouched tile: sum 0
-        if (threadIdx.x == 0) tile_sums[(int64_t)blockIdx.y * tiles_per_row + blockIdx.x] = 0;
-        return;
-    }
-    const int64_t row = (int64_t)blockIdx.y * n_bins;
-    const int64_t base = (int64_t)blockIdx.x * SCAN_TILE;
+    __shared__ int64_t carry_s;
+    __shared__ int is_last;
+    const int64_t ti = (int64_t)blockIdx.y * tiles_per_row + blockIdx.x;
     int64_t acc = 0;
+    if (scan_stamp[ti] == stamp) {                      // untouched tile: sum 0
+        const int64_t row = (int64_t)blockIdx.y * n_bins;
+        const int64_t base = (int64_t)blockIdx.x * SCAN_TILE;
 #pragma unroll
-    for (int j = 0; j < SCAN_ITEMS; ++j) {
-        int64_t k = base + (int64_t)j * SCAN_THREADS + threadIdx.x;
-        if (k < n_bins) acc += diff[row + k];
+        for (int j = 0; j < SCAN_ITEMS; ++j) {
+            int64_t k = base + (int64_t)j * SCAN_THREADS + threadIdx.x;
+            if (k < n_bins) acc += diff[row + k];
+        }
     }
     for (int o = 16; o; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
     if ((threadIdx.x & 31) == 0) warp_sum[threadIdx.x >> 5] = acc;
     __syncthreads();
     if (threadIdx.x == 0) {
-        int64_t s = 0;
-        for (int w = 0; w < SCAN_THREADS / 32; ++w) s += warp_sum[w];
-        tile_sums[(int64_t)blockIdx.y * tiles_per_row + blockIdx.x] = s;
+        int64_t t = 0;
+        for (int w = 0; w < SCAN_THREADS / 32; ++w) t += warp_sum[w];
+        tile_sums[ti] = t;
+        __threadfence();
+        is_last = atomicAdd(ticket + blockIdx.y, 1u) == (unsigned)tiles_per_row - 1u;
+        carry_s = 0;
     }
-}
-
-// phase 2: exclusive scan of each row's tile sums, one CTA per row (tiles_per_row is a few thousand)
-__global__ void __launch_bounds__(1024)
-scan_tile_offsets_kernel(int64_t *__restrict__ tile_sums, int tiles_per_row, const int *__restrict__ wide_flag)
-{
-    if (*wide_flag == 0) return;
-    __shared__ int64_t warp_tot[32];
-    __shared__ int64_t carry_s;
-    int64_t *row = tile_sums + (int64_t)blockIdx.x * tiles_per_row;
-    if (threadIdx.x == 0) carry_s = 0;
     __syncthreads();
-    for (int base = 0; base < tiles_per_row; base += 1024) {
-        int idx = base + threadIdx.x;
-        int64_t v = idx < tiles_per_row ? row[idx] : 0;
+    if (!is_last) return;
+    __threadfence();
+    if (threadIdx.x == 0) ticket[blockIdx.y] = 0u;      // ready for the next call
+    // phase 2: exclusive scan of the row's tile sums
+    volatile int64_t *rowp = tile_sums + (int64_t)blockIdx.y * tiles_per_row;
+    for (int base = 0; base < tiles_per_row; base += SCAN_THREADS) {
+        const int idx = base + threadIdx.x;
+        const int64_t v = idx < tiles_per_row ? rowp[idx] : 0;
         int64_t incl = v;
         for (int o = 1; o < 32; o <<= 1) {
             int64_t up = __shfl_up_sync(0xffffffffu, incl, o);
             if ((threadIdx.x & 31) >= o) incl += up;
         }
-        if ((threadIdx.x & 31) == 31) warp_tot[threadIdx.x >> 5] = incl;
+        __syncthreads();
+        if ((threadIdx.x & 31) == 31) warp_sum[threadIdx.x >> 5] = incl;
         __syncthreads();
         int64_t before = carry_s;
-        for (int w = 0; w < (threadIdx.x >> 5); ++w) before += warp_tot[w];
-        if (idx < tiles_per_row) row[idx] = before + incl - v;
+        for (int w = 0; w < (threadIdx.x >> 5); ++w) before += warp_sum[w];
+        if (idx < tiles_per_row) rowp[idx] = before + incl - v;
         __syncthreads();
-        if (threadIdx.x == 1023) carry_s = before + incl;
+        if (threadIdx.x == SCAN_THREADS - 1) carry_s = before + incl;
         __syncthreads();
     }
 }
@@ -132,7 +132,7 @@ scan_add_kernel(int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
                 const int64_t *__restrict__ tile_offsets, int64_t *__restrict__ spectrum,
                 const int *__restrict__ wide_flag, const int *__restrict__ scan_stamp, int stamp)
 {
-    if (*wide_flag == 0) return;
+    if (*wide_flag != stamp) return;
     __shared__ int64_t warp_tot[SCAN_THREADS / 32];
     {   // nothing to add in a tile without updates that starts from a zero running value
         const int64_t ti = (int64_t)blockIdx.y * tiles_per_row + blockIdx.x;
@@ -168,11 +168,11 @@ scan_add_kernel(int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
     }
 }
 
-__global__ void clear_flag_kernel(int *flag) { *flag = 0; }
-
 // ---------------------------------------------------------------------------------------------
 // internal entry used by the stage call and by the loop.  diff: [n_cat*n_bins] zero on entry and
-// on exit; tile_sums: [n_cat*tiles_per_row]; wide_flag: one int (zero on entry and exit).
+// on exit; tile_sums: [n_cat*tiles_per_row]; wide_flag: one int followed by n_cat ticket words: the
+// flag must differ from mk.stamp on entry (it is left equal to it when a wide source was seen), the
+// tickets are zero on entry and on exit.
 // mk.scan_stamp: [n_cat*tiles_per_row] ints, none equal to mk.stamp on entry.
 // ---------------------------------------------------------------------------------------------
 int scan_tiles_per_row(int64_t n_bins) { return (int)((n_bins + SCAN_TILE - 1) / SCAN_TILE); }
@@ -194,15 +194,12 @@ int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const 
     GBFG_LAUNCH_CHECK("deposit_kernel");
     const int tiles = scan_tiles_per_row(g.n_bins);
     dim3 grid(tiles, ct.n_cat);
-    LaunchTimer lt_scan(K_SCAN, st);     // the three scan kernels and the flag reset, as one
-    scan_tile_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, wide_flag, mk.scan_stamp, mk.stamp);
+    LaunchTimer lt_scan(K_SCAN, st);     // the two scan kernels, as one
+    scan_tile_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, wide_flag, mk.scan_stamp, mk.stamp,
+                                                         (unsigned *)(wide_flag + 1));
     GBFG_LAUNCH_CHECK("scan_tile_sums_kernel");
-    scan_tile_offsets_kernel<<<ct.n_cat, 1024, 0, st>>>(tile_sums, tiles, wide_flag);
-    GBFG_LAUNCH_CHECK("scan_tile_offsets_kernel");
     scan_add_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, spectrum, wide_flag, mk.scan_stamp, mk.stamp);
     GBFG_LAUNCH_CHECK("scan_add_kernel");
-    clear_flag_kernel<<<1, 1, 0, st>>>(wide_flag);
-    GBFG_LAUNCH_CHECK("clear_flag_kernel");
     return GBFG_OK;
 }
 

@@ -21,7 +21,7 @@ int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const 
                    const DepositMarks &mk, cudaStream_t st);
 int median_max_items(int64_t n_bins);
 int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins, int n_cat, int window,
-                const MedianPlan &pl, cudaStream_t st);
+                const MedianPlan &pl, int64_t *zero_ptr, int zero_n, cudaStream_t st);
 int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *med,
                   const double *s_instr, double *psd, double norm, int scale_log2,
                   const MedianPlan *plan, int *neg_flag, cudaStream_t st);
@@ -83,7 +83,7 @@ static Workspace carve(void *base, int64_t n_bins, int64_t n_src_total, int n_ca
     w.plan.ctr = (int *)take(sizeof(int) * 4);
     w.sel_idx = (int64_t *)take(sizeof(int64_t) * nsrc);
     w.counters = (int64_t *)take(sizeof(int64_t) * WS_COUNTERS);
-    w.wide_flag = (int *)take(sizeof(int));
+    w.wide_flag = (int *)take(sizeof(int) * (size_t)(1 + n_cat));   // flag, then one scan ticket per row
     w.sw.pref = take(snr_pref_bytes(n_bins, n_cat));
     w.sw.tile_off = take(snr_tile_off_bytes(n_bins, n_cat));
     w.sw.tile_tot = take(snr_tile_off_bytes(n_bins, n_cat));
@@ -178,7 +178,7 @@ extern "C" int gbfg_deposit(const gbfg_grid *grid, const double *dev_A, const do
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     GBFG_CUDA(cudaMemsetAsync(w.diff, 0, sizeof(int64_t) * (size_t)n_cat * (size_t)grid->n_bins, st));
-    GBFG_CUDA(cudaMemsetAsync(w.wide_flag, 0, sizeof(int), st));
+    GBFG_CUDA(cudaMemsetAsync(w.wide_flag, 0, sizeof(int) * (size_t)(1 + n_cat), st));
     GBFG_CUDA(cudaMemsetAsync(w.scan_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)scan_tiles_per_row(grid->n_bins), st));
     return launch_deposit(make_grid_dev(grid), ct, dev_A, dev_f, dev_fdot, dev_sel_idx, dev_sel_count, n, sign,
                           dev_spectrum, dev_err_count, w.diff, w.tile_sums, w.wide_flag,
@@ -262,7 +262,7 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     const bool incremental = (params->flags & GBFG_FLAG_NO_INCREMENTAL) == 0;
 
     GBFG_CUDA(cudaMemsetAsync(w.diff, 0, row_bytes, st));
-    GBFG_CUDA(cudaMemsetAsync(w.wide_flag, 0, sizeof(int), st));
+    GBFG_CUDA(cudaMemsetAsync(w.wide_flag, 0, sizeof(int) * (size_t)(1 + n_cat), st));
     GBFG_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(int64_t) * WS_COUNTERS, st));
     GBFG_CUDA(cudaMemsetAsync(w.scan_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)scan_tiles, st));
     GBFG_CUDA(cudaMemsetAsync(w.blk_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)w.plan.n_dblk, st));
@@ -289,12 +289,11 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     int n_done = 0;
     for (int it = 0; it < params->max_iter && n_done < n_cat; ++it) {
         // what the last subtraction made dirty (everything, the first time): work list + cum
-        rc = launch_plan(w.blk_stamp, it, it == 0 || !incremental, nb, n_cat, W, w.plan, st);
+        rc = launch_plan(w.blk_stamp, it, it == 0 || !incremental, nb, n_cat, W, w.plan, w.counters, (int)n_iter_counters, st);
         if (rc) return rc;
         rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
                            grid->scale_log2, &w.plan, neg_flag, st);
         if (rc) return rc;
-        GBFG_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(int64_t) * n_iter_counters, st));
         rc = launch_inv_prefix(dev_psd, nb, n_cat, w.sw, dirty, st);
         if (rc) return rc;
         rc = launch_snr_cand(nb, n_cat, dev_psd, params->rho_th, dev_resolved, nullptr, n_cand, w.sel_idx, sel_count,
@@ -340,7 +339,7 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
         // cap hit: the PSD must match the returned residual (rows of converged catalogs are unchanged)
         for (int c = 0; c < n_cat; ++c)
             if (!done[c]) { host_results[c].n_iter = params->max_iter; host_results[c].converged = 0; }
-        rc = launch_plan(w.blk_stamp, params->max_iter, !incremental, nb, n_cat, W, w.plan, st);
+        rc = launch_plan(w.blk_stamp, params->max_iter, !incremental, nb, n_cat, W, w.plan, nullptr, 0, st);
         if (rc) return rc;
         rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
                            grid->scale_log2, &w.plan, nullptr, st);

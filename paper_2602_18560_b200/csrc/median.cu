@@ -478,6 +478,8 @@ struct PlanArgs {
     int4 *items;
     int *ctr;
     int max_items;
+    int64_t *zero_ptr;      // per-iteration counters of the loop, cleared here (nullable)
+    int zero_n;
 };
 
 // len < 2^31 (n_bins is): 32-bit divisions, the 64-bit ones are long instruction sequences
@@ -508,6 +510,7 @@ plan_kernel(PlanArgs a)
     const int b_lo = min(tid * per, nb), b_hi = min(b_lo + per, nb);
     int *s_run = s_cum + nb + 1;
     if (tid == 0) { n_runs = 0; row_pieces = 0; }
+    if (row == 0 && a.zero_ptr) for (int i = tid; i < a.zero_n; i += PLAN_THREADS) a.zero_ptr[i] = 0;
     for (int b0 = tid; b0 < nb; b0 += 8 * PLAN_THREADS) {   // coalesced, eight loads in flight per thread
         int v[8];
 #pragma unroll
@@ -583,7 +586,7 @@ plan_kernel(PlanArgs a)
     }
     __syncthreads();
     if (tid == 0) {
-        if (gridDim.x == 1) { row_base = 0; a.ctr[0] = row_pieces; }
+        if (gridDim.x == 1) { row_base = 0; a.ctr[0] = row_pieces; a.ctr[1] = 0; }
         else row_base = atomicAdd(&a.ctr[0], row_pieces);
     }
     __syncthreads();
@@ -621,9 +624,10 @@ int median_max_items(int64_t n_bins)
 
 // work list + cum from the stamps (blk_stamp NULL or all_dirty: everything)
 int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins, int n_cat, int window,
-                const MedianPlan &pl, cudaStream_t st)
+                const MedianPlan &pl, int64_t *zero_ptr, int zero_n, cudaStream_t st)
 {
     PlanArgs a;
+    a.zero_ptr = zero_ptr; a.zero_n = zero_n;
     a.blk_stamp = blk_stamp; a.stamp = stamp; a.all_dirty = (all_dirty || !blk_stamp) ? 1 : 0;
     a.n_dblk = pl.n_dblk; a.dblk_log2 = pl.dblk_log2; a.n_bins = n_bins;
     a.S = MED_LT - (window - 1);
@@ -638,7 +642,7 @@ int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins,
                                        (int)plan_smem_bytes(DIRTY_MAX_BLOCKS)));
         attr_dev = dev;
     }
-    GBFG_CUDA(cudaMemsetAsync(pl.ctr, 0, 2 * sizeof(int), st));
+    if (n_cat > 1) GBFG_CUDA(cudaMemsetAsync(pl.ctr, 0, 2 * sizeof(int), st));   // one row: the kernel sets both words
     {
         LaunchTimer lt(K_AUX, st);
         plan_kernel<<<n_cat, PLAN_THREADS, smem, st>>>(a);

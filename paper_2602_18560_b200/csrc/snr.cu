@@ -24,6 +24,7 @@
 namespace gbfg {
 
 constexpr int SNR_NARROW = 8;
+constexpr int SNR_SEL_CAP = 1024;              // selected indices a CTA holds before it appends them to the list
 constexpr int PFX_THREADS = 512;
 constexpr int PFX_ITEMS = 8;
 constexpr int PFX_TILE = PFX_THREADS * PFX_ITEMS;     // 4096 bins per prefix tile
@@ -138,69 +139,41 @@ prefix_header_kernel(const double *__restrict__ arr, int64_t n, int64_t n_bins_r
     }
 }
 
-// phase A: local inclusive prefix of every tile of PFX_TILE bins + the tile totals
+// phase A: local inclusive prefix of every tile of PFX_TILE bins + the tile totals (skipped for
+// tiles without a dirty block: their prefix stands)
 __global__ void __launch_bounds__(PFX_THREADS)
 inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tiles_per_row,
-                        U128 *__restrict__ pref, U128 *__restrict__ tile_tot, PrefixHeader *hdr, DirtyView dv)
+                        U128 *__restrict__ pref, U128 *__restrict__ tile_tot, U128 *__restrict__ tile_off,
+                        PrefixHeader *hdr, DirtyView dv, unsigned *__restrict__ ticket)
 {
     __shared__ U128 wtot[PFX_THREADS / 32];
+    __shared__ U128 carry_s;
+    __shared__ int is_last;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    bool clean = false;
     if (dv.cum) {                                           // psd of this tile unchanged: its prefix stands
         const int64_t k_first = (int64_t)blockIdx.x * PFX_TILE;
         int64_t k_last = k_first + PFX_TILE - 1;
         if (k_last > n_bins - 1) k_last = n_bins - 1;
         const int *cum = dv.cum + (int64_t)blockIdx.y * (dv.n_dblk + 1);
-        if (cum[(k_last >> dv.dblk_log2) + 1] == cum[k_first >> dv.dblk_log2]) return;
+        clean = cum[(k_last >> dv.dblk_log2) + 1] == cum[k_first >> dv.dblk_log2];
     }
-    const int U = hdr->unit_exp, e_top = hdr->e_top;
-    const int64_t row = (int64_t)blockIdx.y * n_bins;
-    const int64_t base = (int64_t)blockIdx.x * PFX_TILE + (int64_t)threadIdx.x * PFX_ITEMS;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    U128 v[PFX_ITEMS];
-    U128 run; run.lo = 0; run.hi = 0;
-    int ok = 1;
+    if (!clean) {
+        const int U = hdr->unit_exp, e_top = hdr->e_top;
+        const int64_t row = (int64_t)blockIdx.y * n_bins;
+        const int64_t base = (int64_t)blockIdx.x * PFX_TILE + (int64_t)threadIdx.x * PFX_ITEMS;
+        U128 v[PFX_ITEMS];
+        U128 run; run.lo = 0; run.hi = 0;
+        int ok = 1;
 #pragma unroll
-    for (int j = 0; j < PFX_ITEMS; ++j) {
-        const int64_t k = base + j;
-        U128 t; t.lo = 0; t.hi = 0;
-        if (k < n_bins) t = inv_to_fixed(psd[row + k], U, e_top, &ok);
-        run = u128_add(run, t);
-        v[j] = run;
-    }
-    U128 incl = run;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        U128 up = u128_shfl_up(incl, o);
-        if (lane >= o) incl = u128_add(incl, up);
-    }
-    if (lane == 31) wtot[warp] = incl;
-    __syncthreads();
-    U128 before = u128_sub(incl, run);
-    for (int w = 0; w < warp; ++w) before = u128_add(before, wtot[w]);
-#pragma unroll
-    for (int j = 0; j < PFX_ITEMS; ++j) {
-        const int64_t k = base + j;
-        if (k < n_bins) pref[row + k] = u128_add(before, v[j]);
-    }
-    if (threadIdx.x == PFX_THREADS - 1) tile_tot[(int64_t)blockIdx.y * tiles_per_row + blockIdx.x] = u128_add(before, run);
-    if (!ok) hdr->bad = 1;
-}
-
-// phase B: exclusive scan of each row's tile totals (one CTA per row)
-__global__ void __launch_bounds__(1024)
-inv_prefix_tiles_kernel(const U128 *__restrict__ tile_tot, U128 *__restrict__ tile_off, int tiles_per_row)
-{
-    __shared__ U128 wtot[32];
-    __shared__ U128 carry_s;
-    const U128 *rowp = tile_tot + (int64_t)blockIdx.x * tiles_per_row;
-    U128 *outp = tile_off + (int64_t)blockIdx.x * tiles_per_row;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) { carry_s.lo = 0; carry_s.hi = 0; }
-    __syncthreads();
-    for (int b = 0; b < tiles_per_row; b += 1024) {
-        const int idx = b + threadIdx.x;
-        U128 v; v.lo = 0; v.hi = 0;
-        if (idx < tiles_per_row) v = rowp[idx];
-        U128 incl = v;
+        for (int j = 0; j < PFX_ITEMS; ++j) {
+            const int64_t k = base + j;
+            U128 t; t.lo = 0; t.hi = 0;
+            if (k < n_bins) t = inv_to_fixed(psd[row + k], U, e_top, &ok);
+            run = u128_add(run, t);
+            v[j] = run;
+        }
+        U128 incl = run;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             U128 up = u128_shfl_up(incl, o);
@@ -208,11 +181,49 @@ inv_prefix_tiles_kernel(const U128 *__restrict__ tile_tot, U128 *__restrict__ ti
         }
         if (lane == 31) wtot[warp] = incl;
         __syncthreads();
+        U128 before = u128_sub(incl, run);
+        for (int w = 0; w < warp; ++w) before = u128_add(before, wtot[w]);
+#pragma unroll
+        for (int j = 0; j < PFX_ITEMS; ++j) {
+            const int64_t k = base + j;
+            if (k < n_bins) pref[row + k] = u128_add(before, v[j]);
+        }
+        if (threadIdx.x == PFX_THREADS - 1) {
+            tile_tot[(int64_t)blockIdx.y * tiles_per_row + blockIdx.x] = u128_add(before, run);
+            __threadfence();
+        }
+        if (!ok) hdr->bad = 1;
+    }
+    // phase B by the last CTA of the row to finish: exclusive scan of the row's tile totals
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        is_last = atomicAdd(ticket + blockIdx.y, 1u) == (unsigned)tiles_per_row - 1u;
+        carry_s.lo = 0; carry_s.hi = 0;
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    if (threadIdx.x == 0) ticket[blockIdx.y] = 0u;
+    const volatile uint64_t *totp = reinterpret_cast<const volatile uint64_t *>(tile_tot + (int64_t)blockIdx.y * tiles_per_row);
+    U128 *outp = tile_off + (int64_t)blockIdx.y * tiles_per_row;
+    for (int b = 0; b < tiles_per_row; b += PFX_THREADS) {
+        const int idx = b + threadIdx.x;
+        U128 v; v.lo = 0; v.hi = 0;
+        if (idx < tiles_per_row) { v.lo = totp[2 * idx]; v.hi = totp[2 * idx + 1]; }
+        U128 incl = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            U128 up = u128_shfl_up(incl, o);
+            if (lane >= o) incl = u128_add(incl, up);
+        }
+        __syncthreads();
+        if (lane == 31) wtot[warp] = incl;
+        __syncthreads();
         U128 before = carry_s;
         for (int w = 0; w < warp; ++w) before = u128_add(before, wtot[w]);
         if (idx < tiles_per_row) outp[idx] = u128_add(before, u128_sub(incl, v));
         __syncthreads();
-        if (threadIdx.x == 1023) carry_s = u128_add(before, incl);
+        if (threadIdx.x == PFX_THREADS - 1) carry_s = u128_add(before, incl);
         __syncthreads();
     }
 }
@@ -440,20 +451,27 @@ snr_cand_kernel(SnrArgs a)
         n = off[b_max + 1];
     }
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    const int64_t n_round = t_first + ((n - t_first + 31) & ~(int64_t)31);
     const bool pref_ok = a.pv.pref && a.pv.hdr->bad == 0;
     const int unit_exp = a.pv.pref ? a.pv.hdr->unit_exp : 0;
-    for (int64_t t = t_first + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < n_round; t += stride) {
+    // The selected indices of the CTA are collected in shared memory and appended to the list with
+    // one global atomic per flush (tens of thousands of sources pass in the first iterations: one
+    // atomic per warp on a single address is what the kernel then waits for).
+    __shared__ int64_t s_sel[SNR_SEL_CAP + 256];
+    __shared__ int s_n, s_near;
+    __shared__ long long s_base;
+    if (threadIdx.x == 0) { s_n = 0; s_near = 0; }
+    __syncthreads();
+    for (int64_t t0 = t_first + (int64_t)blockIdx.x * blockDim.x; t0 < n; t0 += stride) {
+        const int64_t t = t0 + threadIdx.x;
         int32_t w = 0;
         if (t < n) w = a.cand.w[t];
         bool sel = false, near = false;
-        int cat = 0;
+        const int cat = rowc;
         int64_t src = -1, gk0 = 0;
         const bool always = w < 0;                          // was near the threshold: counted every iteration
         if (always) w = -w;
         if (w > 0) {
             gk0 = a.cand.gk0[t];
-            if (a.n_cat > 1) cat = (int)(gk0 / a.n_bins);
             if (a.dv.cum && !always) {
                 // the PSD under this source is what it was at its last test: same rho2, same answer
                 const int64_t k0 = gk0 - (int64_t)cat * a.n_bins;
@@ -474,22 +492,34 @@ snr_cand_kernel(SnrArgs a)
         const unsigned sel_mask = __ballot_sync(0xffffffffu, sel);
         const unsigned near_mask = __ballot_sync(0xffffffffu, near);
         if (sel_mask) {
-            int64_t base = 0;
-            if (lane == 0) base = (int64_t)atomicAdd((unsigned long long *)a.sel_count, (unsigned long long)__popc(sel_mask));
+            int base = 0;
+            if (lane == 0) base = atomicAdd(&s_n, __popc(sel_mask));
             base = __shfl_sync(0xffffffffu, base, 0);
             if (sel) {
-                a.sel_idx[base + __popc(sel_mask & ((1u << lane) - 1u))] = src;
+                s_sel[base + __popc(sel_mask & ((1u << lane) - 1u))] = src;
                 a.resolved[src] = 1;
                 a.cand.w[t] = 0;
-                atomicAdd((unsigned long long *)(a.sel_count + 1 + cat), 1ull);
             }
         }
         if (near && !sel && !always) { a.cand.w[t] = -w; *a.any_near = 1; }
-        if (near_mask && a.near_count) {
-            if (a.near_per_cat) { if (near) atomicAdd((unsigned long long *)(a.near_count + cat), 1ull); }
-            else if (lane == 0) atomicAdd((unsigned long long *)a.near_count, (unsigned long long)__popc(near_mask));
+        if (near_mask && lane == 0) atomicAdd(&s_near, __popc(near_mask));
+        __syncthreads();
+        const bool last = t0 + stride >= n;
+        if (s_n > SNR_SEL_CAP || (last && s_n > 0)) {       // uniform over the CTA
+            const int cnt = s_n;
+            if (threadIdx.x == 0) {
+                s_base = (long long)atomicAdd((unsigned long long *)a.sel_count, (unsigned long long)cnt);
+                atomicAdd((unsigned long long *)(a.sel_count + 1 + rowc), (unsigned long long)cnt);
+            }
+            __syncthreads();
+            for (int i = threadIdx.x; i < cnt; i += blockDim.x) a.sel_idx[s_base + i] = s_sel[i];
+            __syncthreads();
+            if (threadIdx.x == 0) s_n = 0;
+            __syncthreads();
         }
     }
+    if (threadIdx.x == 0 && s_near && a.near_count)
+        atomicAdd((unsigned long long *)(a.near_count + (a.near_per_cat ? rowc : 0)), (unsigned long long)s_near);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -527,11 +557,10 @@ int launch_inv_prefix(const double *psd, int64_t n_bins, int n_cat, const SnrWor
 {
     const int tiles = pfx_tiles_per_row(n_bins);
     LaunchTimer lt(K_INV_BLOCKS, st);
-    inv_prefix_local_kernel<<<dim3(tiles, n_cat), PFX_THREADS, 0, st>>>(psd, n_bins, tiles, (U128 *)sw.pref,
-                                                                        (U128 *)sw.tile_tot, (PrefixHeader *)sw.hdr, dv);
+    unsigned *ticket = reinterpret_cast<unsigned *>((char *)sw.hdr + sizeof(PrefixHeader) + sizeof(PrefixScratch));
+    inv_prefix_local_kernel<<<dim3(tiles, n_cat), PFX_THREADS, 0, st>>>(psd, n_bins, tiles, (U128 *)sw.pref, (U128 *)sw.tile_tot,
+                                                                        (U128 *)sw.tile_off, (PrefixHeader *)sw.hdr, dv, ticket);
     GBFG_LAUNCH_CHECK("inv_prefix_local_kernel");
-    inv_prefix_tiles_kernel<<<n_cat, 1024, 0, st>>>((const U128 *)sw.tile_tot, (U128 *)sw.tile_off, tiles);
-    GBFG_LAUNCH_CHECK("inv_prefix_tiles_kernel");
     return GBFG_OK;
 }
 
@@ -607,6 +636,6 @@ int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th,
 
 size_t snr_pref_bytes(int64_t n_bins, int n_cat) { return sizeof(U128) * (size_t)n_cat * (size_t)n_bins; }
 size_t snr_tile_off_bytes(int64_t n_bins, int n_cat) { return sizeof(U128) * (size_t)n_cat * (size_t)pfx_tiles_per_row(n_bins); }
-size_t snr_hdr_bytes() { return sizeof(PrefixHeader) + sizeof(PrefixScratch); }
+size_t snr_hdr_bytes() { return sizeof(PrefixHeader) + sizeof(PrefixScratch) + sizeof(unsigned) * GBFG_MAX_CAT; }   // header, scratch, one ticket per row
 
 }  // namespace gbfg
