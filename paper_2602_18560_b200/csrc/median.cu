@@ -284,69 +284,78 @@ running_median_kernel(MedianArgs a)
     }
     __syncthreads();
 
-    // ---- coarse states: one warp finds the median rank of the window of output 32 c
+    // ---- coarse states.  Warp w owns the chunks [w cpw, (w+1) cpw) of 32 outputs.  The median rank of
+    // the window of its first chunk comes from the count table; the following ones by sliding the
+    // window 32 bins at a time: two ballots count the ranks under m that left and entered, and the
+    // warp moves m by that many window elements, 32 places of the sorted order per step.
     const int n_coarse = (n_out + MED_PB - 1) / MED_PB;
-    for (int c = warp; c < n_coarse; c += MED_WARPS) {
-        const int j0 = c * MED_PB;
-        const int b0 = c, b1 = (j0 + W) / MED_PB;
-        const int na = b1 * MED_PB - j0;                 // block-aligned part of the window
-        int m = LTe, below = 0, phi = j0 - 1;
-        if (na > 0) {
-            const int t = (h < na - 1) ? h : na - 1;
-            // largest bucket lo with #{rank < 128 lo, position in the aligned part} <= t
-            const int c0 = (int)tab[lane * MED_TROW + b1] - (int)tab[lane * MED_TROW + b0];
-            const int c1 = (int)tab[(lane + 32) * MED_TROW + b1] - (int)tab[(lane + 32) * MED_TROW + b0];
-            const unsigned m0 = __ballot_sync(FULL, c0 <= t), m1 = __ballot_sync(FULL, c1 <= t);
-            const int lo = m1 ? 63 - __clz(m1) : 31 - __clz(m0);
-            const int cl = lo < 32 ? __shfl_sync(FULL, c0, lo & 31) : __shfl_sync(FULL, c1, lo & 31);
-            int need = t - cl;
-            int base = lo * MED_RB;
-            for (;;) {                                   // ends inside bucket lo by construction
-                const int r = base + lane;
-                const bool in = r < LTe && (unsigned)((int)spos[r < LTe ? r : 0] - j0) < (unsigned)na;
-                const unsigned bal = __ballot_sync(FULL, in);
-                const int cn = __popc(bal);
-                if (need < cn) { m = base + nth_set_bit(bal, need + 1); break; }
-                need -= cn;
-                base += 32;
-                if (base >= LTe) break;                  // not reachable for a consistent table
-            }
-            below = t;
-            phi = b1 * MED_PB - 1;
+    const int cpw = (n_coarse + MED_WARPS - 1) / MED_WARPS;
+    const int c_first = warp * cpw;
+    // warp-cooperative search: from rank wm (exclusive) in direction wdir to the wneed-th element whose
+    // position lies in [wplo, wphi]; all arguments warp-uniform; wm is updated
+#define WARP_SEEK(wm, wdir, wneed, wplo, wphi)                                                     \
+        for (;;) {                                                                                 \
+            const int r_ = (wm) + (wdir) * (1 + lane);                                             \
+            const bool ok_ = (unsigned)r_ < (unsigned)LTe;                                         \
+            const bool in_ = ok_ && (unsigned)((int)spos[ok_ ? r_ : 0] - (wplo)) <= (unsigned)((wphi) - (wplo)); \
+            const unsigned bal_ = __ballot_sync(FULL, in_);                                        \
+            const int cn_ = __popc(bal_);                                                          \
+            if ((wneed) <= cn_) { (wm) += (wdir) * (1 + nth_set_bit(bal_, (wneed))); break; }      \
+            (wneed) -= cn_;                                                                        \
+            (wm) += 32 * (wdir);                                                                   \
+            if ((unsigned)(wm) >= (unsigned)LTe) break;    /* not reachable: the window holds the element */ \
         }
-        {   // complete the window with the (at most 31, or W when W < 32) remaining positions
+    if (c_first < n_coarse) {
+        int m = LTe;
+        {
+            const int c = c_first;
+            const int j0 = c * MED_PB;
+            const int b0 = c, b1 = (j0 + W) / MED_PB;
+            const int na = b1 * MED_PB - j0;                 // block-aligned part of the window
+            int below = 0, phi = j0 - 1;
+            if (na > 0) {
+                const int t = (h < na - 1) ? h : na - 1;
+                // largest bucket lo with #{rank < 128 lo, position in the aligned part} <= t
+                const int c0 = (int)tab[lane * MED_TROW + b1] - (int)tab[lane * MED_TROW + b0];
+                const int c1 = (int)tab[(lane + 32) * MED_TROW + b1] - (int)tab[(lane + 32) * MED_TROW + b0];
+                const unsigned m0 = __ballot_sync(FULL, c0 <= t), m1 = __ballot_sync(FULL, c1 <= t);
+                const int lo = m1 ? 63 - __clz(m1) : 31 - __clz(m0);
+                const int cl = lo < 32 ? __shfl_sync(FULL, c0, lo & 31) : __shfl_sync(FULL, c1, lo & 31);
+                int need = t - cl + 1;                       // the (t - cl + 1)-th aligned element from rank 128 lo on
+                m = lo * MED_RB - 1;
+                WARP_SEEK(m, 1, need, j0, j0 + na - 1);
+                below = t;
+                phi = b1 * MED_PB - 1;
+            }
+            // complete the window with the (at most 31, or W when W < 32) remaining positions
             for (int pbase = phi + 1; pbase < j0 + W; pbase += 32) {
                 const int p = pbase + lane;
                 const bool add = p < j0 + W && (int)rop[p < j0 + W ? p : 0] < m;
                 below += __popc(__ballot_sync(FULL, add));
             }
-        }
-        if (below > h) {                                 // down to the (below - h)-th window element under m
-            int need = below - h, base = m - 1;
-            for (;;) {
-                const int r = base - lane;
-                const bool in = r >= 0 && (unsigned)((int)spos[r >= 0 ? r : 0] - j0) < (unsigned)W;
-                const unsigned bal = __ballot_sync(FULL, in);
-                const int cn = __popc(bal);
-                if (need <= cn) { m = base - nth_set_bit(bal, need); break; }
-                need -= cn;
-                base -= 32;
-                if (base < 0) break;
+            if (below > h) {                                 // down to the (below - h)-th window element under m
+                int need = below - h;
+                WARP_SEEK(m, -1, need, j0, j0 + W - 1);
+            } else {                                         // up to the (h - below + 1)-th window element at or above m
+                int need = h - below + 1;
+                m -= 1;
+                WARP_SEEK(m, 1, need, j0, j0 + W - 1);
             }
-        } else {                                         // up to the (h - below + 1)-th window element at or above m
-            int need = h - below + 1, base = m;
-            for (;;) {
-                const int r = base + lane;
-                const bool in = r < LTe && (unsigned)((int)spos[r < LTe ? r : 0] - j0) < (unsigned)W;
-                const unsigned bal = __ballot_sync(FULL, in);
-                const int cn = __popc(bal);
-                if (need <= cn) { m = base + nth_set_bit(bal, need); break; }
-                need -= cn;
-                base += 32;
-                if (base >= LTe) break;
-            }
+            if (lane == 0) cm[c] = (uint16_t)m;
         }
-        if (lane == 0) cm[c] = (uint16_t)m;
+        const int c_last = (c_first + cpw < n_coarse) ? c_first + cpw : n_coarse;
+        for (int c = c_first + 1; c < c_last; ++c) {
+            const int j0 = c * MED_PB;                       // window [j0, j0 + W); the last one started 32 bins earlier
+            const int gone = rop[j0 - MED_PB + lane], come = rop[j0 - MED_PB + W + lane];
+            const int n_gone = __popc(__ballot_sync(FULL, gone < m)), n_come = __popc(__ballot_sync(FULL, come < m));
+            const bool m_left = __ballot_sync(FULL, gone == m) != 0u;
+            const int below = h + n_come - n_gone;
+            int dir, need;
+            if (below > h) { dir = -1; need = below - h; }
+            else { dir = 1; need = h - below + (m_left ? 1 : 0); }
+            if (need) { WARP_SEEK(m, dir, need, j0, j0 + W - 1); }
+            if (lane == 0) cm[c] = (uint16_t)m;
+        }
     }
     __syncthreads();
 
@@ -356,7 +365,7 @@ running_median_kernel(MedianArgs a)
     // when it is still in the window.  A thread steps along the sorted order on its own for at most
     // MED_STEP_CAP places; spectra with plateaus (wide chirps put the same power in consecutive bins)
     // and level-correlated neighbourhoods have stretches of hundreds of out-of-window elements, and
-    // those searches are finished by the whole warp, 32 places per step (warp_finish).
+    // those searches are finished by the whole warp, 32 places per step.
     {
         const int s = tid / n_coarse, c = tid - s * n_coarse;
         const int j_first = c * MED_PB + s * MED_FINE;
@@ -373,17 +382,7 @@ running_median_kernel(MedianArgs a)
             const int wdir = __shfl_sync(FULL, dir, src);                                          \
             int wneed = __shfl_sync(FULL, need, src);                                              \
             const int wplo = __shfl_sync(FULL, plo, src), wphi = __shfl_sync(FULL, phi, src);      \
-            for (;;) {                                                                             \
-                const int r = wm + wdir * (1 + lane);                                              \
-                const bool ok = (unsigned)r < (unsigned)LTe;                                       \
-                const bool in = ok && (unsigned)((int)spos[ok ? r : 0] - wplo) <= (unsigned)(wphi - wplo); \
-                const unsigned bal = __ballot_sync(FULL, in);                                      \
-                const int cn = __popc(bal);                                                        \
-                if (wneed <= cn) { wm += wdir * (1 + nth_set_bit(bal, wneed)); break; }            \
-                wneed -= cn;                                                                       \
-                wm += 32 * wdir;                                                                   \
-                if ((unsigned)wm >= (unsigned)LTe) break;      /* not reachable: the window holds the element */ \
-            }                                                                                      \
+            WARP_SEEK(wm, wdir, wneed, wplo, wphi);                                                \
             if (lane == src) { m = wm; need = 0; }                                                 \
         }
         if (alive) {
@@ -422,6 +421,7 @@ running_median_kernel(MedianArgs a)
             if (on) orank[j] = (uint16_t)m;
         }
 #undef WARP_FINISH
+#undef WARP_SEEK
 #undef IN_SET
     }
     __syncthreads();
