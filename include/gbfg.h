@@ -86,6 +86,8 @@ typedef struct gbfg_iter_result {
     int64_t n_resolved;         /* sources resolved by this call */
     int64_t n_near_threshold;   /* tests with |rho^2 / rho_th^2 - 1| <= 2e-9, summed over iterations */
     int64_t n_candidates;       /* sources that passed the pre-selection (= tested sources if disabled) */
+    int64_t n_median_outputs;   /* running-median outputs computed, summed over iterations (n_bins per full pass) */
+    int64_t n_snr_tests;        /* SNR tests evaluated, summed over iterations */
     int64_t n_new_per_iter[GBFG_MAX_ITER_TRACE];
 } gbfg_iter_result;
 
@@ -182,10 +184,14 @@ int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *of
 /* The same path with HOST buffers: the library allocates device memory, copies host_s_instr in,
  * runs gbfg_simulate on its own stream, and copies the PSD ([n_cat][n_bins] binary64) and the
  * resolved flags ([N] uint8, may be NULL) back.  Host pointers should be pinned for full speed.
- * Synchronous. */
+ * Synchronous.  The device memory it allocates is cached per host thread (gbfg_release_cached). */
 int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
                        uint64_t seed, const double *host_s_instr, const gbfg_iter_params *params,
                        double *host_psd, uint8_t *host_resolved, gbfg_iter_result *host_results);
+
+/* gbfg_simulate_host keeps its device arena and stream between calls of the same host thread, so that
+ * repeated calls do not pay cudaMalloc / cudaFree; this frees them (synchronises the stream first). */
+int gbfg_release_cached(void);
 
 /* Bytes of device workspace sufficient for any call above on this grid / batch. */
 size_t gbfg_workspace_bytes(const gbfg_grid *grid, int64_t n_src_total, int32_t n_cat);
@@ -208,7 +214,7 @@ enum {
     GBFG_K_PSD,             /* psd_kernel                         stage (iii) */
     GBFG_K_INV_BLOCKS,      /* block sums of 1/psd                stage (iv)  */
     GBFG_K_SNR,             /* SNR + select kernels               stage (iv)  */
-    GBFG_K_AUX,             /* small bookkeeping kernels                      */
+    GBFG_K_AUX,             /* plan_kernel: dirty blocks -> median work list  */
     GBFG_K_COUNT
 };
 typedef struct gbfg_kernel_time {

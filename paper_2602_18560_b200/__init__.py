@@ -23,7 +23,7 @@ EXPORTS = [
     "gbfg_version", "gbfg_strerror", "gbfg_last_cuda_error", "gbfg_grid_init", "gbfg_instrument_noise",
     "gbfg_sample_catalog", "gbfg_deposit", "gbfg_running_median", "gbfg_psd", "gbfg_snr_select",
     "gbfg_subtract_until_converged", "gbfg_simulate", "gbfg_simulate_host", "gbfg_workspace_bytes",
-    "gbfg_kernel_launch_count", "gbfg_profile_enable", "gbfg_profile_read",
+    "gbfg_kernel_launch_count", "gbfg_profile_enable", "gbfg_profile_read", "gbfg_release_cached",
 ]
 
 KERNEL_CLASSES = ["sample", "noise", "deposit", "scan", "median", "psd", "inv_blocks", "snr", "aux"]
@@ -54,6 +54,7 @@ class IterParams(C.Structure):
 class IterResult(C.Structure):
     _fields_ = [("n_iter", C.c_int32), ("converged", C.c_int32), ("n_resolved", C.c_int64),
                 ("n_near_threshold", C.c_int64), ("n_candidates", C.c_int64),
+                ("n_median_outputs", C.c_int64), ("n_snr_tests", C.c_int64),
                 ("n_new_per_iter", C.c_int64 * MAX_ITER_TRACE)]
 
 
@@ -148,6 +149,11 @@ def make_iter_params(window: int, median_norm: float, rho_th: float, max_iter: i
 
 def version() -> int:
     return load().gbfg_version()
+
+
+def release_cached():
+    """Frees the device arena gbfg_simulate_host keeps between calls."""
+    _check(load().gbfg_release_cached())
 
 
 def kernel_launch_count() -> int:

@@ -21,7 +21,7 @@ int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const 
                    const DepositMarks &mk, cudaStream_t st);
 int median_max_items(int64_t n_bins);
 int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins, int n_cat, int window,
-                const MedianPlan &pl, int64_t *zero_ptr, int zero_n, cudaStream_t st);
+                const MedianPlan &pl, int64_t *zero_ptr, int zero_n, int64_t *out_count, cudaStream_t st);
 int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *med,
                   const double *s_instr, double *psd, double norm, int scale_log2,
                   const MedianPlan *plan, int *neg_flag, cudaStream_t st);
@@ -36,16 +36,19 @@ int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, con
                       const SnrWork &sw, cudaStream_t st);
 int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th, uint8_t *resolved, double *rho2_out,
                     int64_t n_launch, int64_t *sel_idx, int64_t *sel_count, int64_t *near_count, int near_per_cat,
-                    const int *abort_flag, bool use_prefix, const SnrWork &sw, const DirtyView &dv, cudaStream_t st);
+                    const int *abort_flag, bool use_prefix, const SnrWork &sw, const DirtyView &dv, int64_t *test_count,
+                    cudaStream_t st);
 
 // ------------------------------------------------------------------------------- workspace
-constexpr int WS_COUNTERS = 4 * GBFG_MAX_CAT + 16;
+constexpr int WS_COUNTERS = 6 * GBFG_MAX_CAT + 16;
 
 // layout of `counters` (int64): what the host reads back each iteration comes first
 //   [0 .. n_cat]            sel_count: total, per catalog
 //   [1+n_cat .. 1+2 n_cat)  near-threshold counts per catalog
 //   [1+2 n_cat]             flags word: bit 0 = a median was negative
 //   [2+2 n_cat .. 3+3 n_cat) cand_count: total, per catalog
+//   [3+3 n_cat .. 3+4 n_cat) running-median outputs computed, per catalog (accumulated over the call)
+//   [3+4 n_cat .. 3+5 n_cat) SNR tests evaluated, per catalog (accumulated over the call)
 struct Workspace {
     int64_t *diff;        // [n_cat * n_bins]   difference array of the range-update deposit
     int64_t *tile_sums;   // [n_cat * scan_tiles]
@@ -139,6 +142,14 @@ static int64_t *host_scratch()
     return p;
 }
 
+// device arena and stream of gbfg_simulate_host, one per host thread
+struct HostCallCache { char *base; size_t bytes; int device; cudaStream_t stream; };
+static HostCallCache &host_call_cache()
+{
+    static thread_local HostCallCache c = {nullptr, 0, -1, nullptr};
+    return c;
+}
+
 static DepositMarks plain_marks(const Workspace &w, int64_t n_bins, int stamp)
 {
     DepositMarks mk;
@@ -217,7 +228,7 @@ extern "C" int gbfg_snr_select(const gbfg_grid *grid, const double *dev_A, const
     rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, nullptr, rho_th, dev_rho2_out, w.sw, st);
     if (rc) return rc;
     return launch_snr_cand(grid->n_bins, n_cat, dev_psd, rho_th, dev_resolved, dev_rho2_out, n, dev_sel_idx,
-                           dev_sel_count, dev_near_count, 0, nullptr, true, w.sw, all_dirty, st);
+                           dev_sel_count, dev_near_count, 0, nullptr, true, w.sw, all_dirty, nullptr, st);
 }
 
 extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double *dev_A, const double *dev_f,
@@ -256,7 +267,9 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     int64_t *near = w.counters + 1 + n_cat;             // [n_cat]
     int *neg_flag = (int *)(w.counters + 1 + 2 * n_cat);
     const size_t n_iter_counters = (size_t)(1 + 2 * n_cat);      // zeroed every iteration
-    const size_t n_read_all = (size_t)(3 + 3 * n_cat);           // ... + flags + cand_count
+    const size_t n_read_all = (size_t)(3 + 5 * n_cat);           // ... + flags + cand_count + work counters
+    int64_t *med_outputs = w.counters + 3 + 3 * n_cat, *snr_tests = w.counters + 3 + 4 * n_cat;
+    const int i_med = 3 + 3 * n_cat, i_tests = 3 + 4 * n_cat;
     const int i_flags = 1 + 2 * n_cat, i_cand = 2 + 2 * n_cat;
     bool preselect = (params->flags & GBFG_FLAG_NO_PRESELECT) == 0;
     const bool incremental = (params->flags & GBFG_FLAG_NO_INCREMENTAL) == 0;
@@ -289,7 +302,7 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     int n_done = 0;
     for (int it = 0; it < params->max_iter && n_done < n_cat; ++it) {
         // what the last subtraction made dirty (everything, the first time): work list + cum
-        rc = launch_plan(w.blk_stamp, it, it == 0 || !incremental, nb, n_cat, W, w.plan, w.counters, (int)n_iter_counters, st);
+        rc = launch_plan(w.blk_stamp, it, it == 0 || !incremental, nb, n_cat, W, w.plan, w.counters, (int)n_iter_counters, med_outputs, st);
         if (rc) return rc;
         rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
                            grid->scale_log2, &w.plan, neg_flag, st);
@@ -297,7 +310,7 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
         rc = launch_inv_prefix(dev_psd, nb, n_cat, w.sw, dirty, st);
         if (rc) return rc;
         rc = launch_snr_cand(nb, n_cat, dev_psd, params->rho_th, dev_resolved, nullptr, n_cand, w.sel_idx, sel_count,
-                             near, 1, preselect ? neg_flag : nullptr, true, w.sw, dirty, st);
+                             near, 1, preselect ? neg_flag : nullptr, true, w.sw, dirty, snr_tests, st);
         if (rc) return rc;
         GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
         GBFG_CUDA(cudaStreamSynchronize(st));
@@ -310,7 +323,7 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
             rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, nullptr, params->rho_th, nullptr, w.sw, st);
             if (rc) return rc;
             rc = launch_snr_cand(nb, n_cat, dev_psd, params->rho_th, dev_resolved, nullptr, n, w.sel_idx, sel_count,
-                                 near, 1, nullptr, true, w.sw, all_dirty, st);
+                                 near, 1, nullptr, true, w.sw, all_dirty, snr_tests, st);
             if (rc) return rc;
             GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
             GBFG_CUDA(cudaStreamSynchronize(st));
@@ -339,13 +352,18 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
         // cap hit: the PSD must match the returned residual (rows of converged catalogs are unchanged)
         for (int c = 0; c < n_cat; ++c)
             if (!done[c]) { host_results[c].n_iter = params->max_iter; host_results[c].converged = 0; }
-        rc = launch_plan(w.blk_stamp, params->max_iter, !incremental, nb, n_cat, W, w.plan, nullptr, 0, st);
+        rc = launch_plan(w.blk_stamp, params->max_iter, !incremental, nb, n_cat, W, w.plan, nullptr, 0, med_outputs, st);
         if (rc) return rc;
         rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
                            grid->scale_log2, &w.plan, nullptr, st);
         if (rc) return rc;
     }
+    GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
     GBFG_CUDA(cudaStreamSynchronize(st));
+    for (int c = 0; c < n_cat; ++c) {
+        host_results[c].n_median_outputs = host[i_med + c];
+        host_results[c].n_snr_tests = host[i_tests + c];
+    }
     return GBFG_OK;
 }
 
@@ -394,11 +412,22 @@ extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, c
     const size_t oA = take(8 * nn), oF = take(8 * nn), oD = take(8 * nn);
     const size_t oS = take(8 * rows), oM = take(8 * rows), oP = take(8 * rows), oI = take(8 * nb);
     const size_t oR = take(nn), oW = take(ws_bytes);
-    char *base = nullptr;
-    cudaStream_t st = nullptr;
-    GBFG_CUDA(cudaMalloc((void **)&base, off));
-    cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
-    if (e != cudaSuccess) { cudaFree(base); return set_cuda_error(e, "cudaStreamCreate"); }
+    // the device arena and the stream are kept between calls of the same host thread (gbfg_release_cached frees them)
+    HostCallCache &cc = host_call_cache();
+    int dev = 0;
+    GBFG_CUDA(cudaGetDevice(&dev));
+    if (cc.base && (cc.bytes < off || cc.device != dev)) { cudaFree(cc.base); cc.base = nullptr; cc.bytes = 0; }
+    if (!cc.base) {
+        GBFG_CUDA(cudaMalloc((void **)&cc.base, off));
+        cc.bytes = off; cc.device = dev;
+    }
+    if (!cc.stream) {
+        cudaError_t es = cudaStreamCreateWithFlags(&cc.stream, cudaStreamNonBlocking);
+        if (es != cudaSuccess) { cc.stream = nullptr; return set_cuda_error(es, "cudaStreamCreate"); }
+    }
+    char *base = cc.base;
+    cudaStream_t st = cc.stream;
+    cudaError_t e;
     rc = GBFG_OK;
     e = cudaMemcpyAsync(base + oI, host_s_instr, 8 * nb, cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) rc = set_cuda_error(e, "cudaMemcpyAsync(s_instr)");
@@ -415,7 +444,13 @@ extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, c
         if (e != cudaSuccess) rc = set_cuda_error(e, "copy back");
     }
     cudaStreamSynchronize(st);
-    cudaStreamDestroy(st);
-    cudaFree(base);
     return rc;
+}
+
+extern "C" int gbfg_release_cached(void)
+{
+    HostCallCache &cc = host_call_cache();
+    if (cc.stream) { cudaStreamSynchronize(cc.stream); cudaStreamDestroy(cc.stream); cc.stream = nullptr; }
+    if (cc.base) { cudaFree(cc.base); cc.base = nullptr; cc.bytes = 0; }
+    return GBFG_OK;
 }

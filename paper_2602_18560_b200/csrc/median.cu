@@ -480,6 +480,7 @@ struct PlanArgs {
     int max_items;
     int64_t *zero_ptr;      // per-iteration counters of the loop, cleared here (nullable)
     int zero_n;
+    int64_t *out_count;     // [n_cat] outputs planned, accumulated (nullable)
 };
 
 // len < 2^31 (n_bins is): 32-bit divisions, the 64-bit ones are long instruction sequences
@@ -586,6 +587,11 @@ plan_kernel(PlanArgs a)
     }
     __syncthreads();
     if (tid == 0) {
+        if (a.out_count) {                               // dirty outputs of the row = dirty blocks, the last one clipped
+            int64_t outs = (int64_t)s_cum[nb] << a.dblk_log2;
+            if (nb > 0 && s_cum[nb] != s_cum[nb - 1]) outs -= ((int64_t)nb << a.dblk_log2) - a.n_bins;
+            a.out_count[row] += outs;
+        }
         if (gridDim.x == 1) { row_base = 0; a.ctr[0] = row_pieces; a.ctr[1] = 0; }
         else row_base = atomicAdd(&a.ctr[0], row_pieces);
     }
@@ -624,10 +630,10 @@ int median_max_items(int64_t n_bins)
 
 // work list + cum from the stamps (blk_stamp NULL or all_dirty: everything)
 int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins, int n_cat, int window,
-                const MedianPlan &pl, int64_t *zero_ptr, int zero_n, cudaStream_t st)
+                const MedianPlan &pl, int64_t *zero_ptr, int zero_n, int64_t *out_count, cudaStream_t st)
 {
     PlanArgs a;
-    a.zero_ptr = zero_ptr; a.zero_n = zero_n;
+    a.zero_ptr = zero_ptr; a.zero_n = zero_n; a.out_count = out_count;
     a.blk_stamp = blk_stamp; a.stamp = stamp; a.all_dirty = (all_dirty || !blk_stamp) ? 1 : 0;
     a.n_dblk = pl.n_dblk; a.dblk_log2 = pl.dblk_log2; a.n_bins = n_bins;
     a.S = MED_LT - (window - 1);

@@ -422,6 +422,7 @@ struct SnrArgs {
     const int *bkt_reach;       // [n_cat][n_dblk] first bucket with a record that reaches block b
     int *any_near;
     int n_dblk;
+    int64_t *test_count;        // [n_cat] tests evaluated, accumulated (nullable)
     int64_t n_bins;
     int n_cat;
     double thr;                 // rho_th^2
@@ -457,9 +458,9 @@ snr_cand_kernel(SnrArgs a)
     // one global atomic per flush (tens of thousands of sources pass in the first iterations: one
     // atomic per warp on a single address is what the kernel then waits for).
     __shared__ int64_t s_sel[SNR_SEL_CAP + 256];
-    __shared__ int s_n, s_near;
+    __shared__ int s_n, s_near, s_tests;
     __shared__ long long s_base;
-    if (threadIdx.x == 0) { s_n = 0; s_near = 0; }
+    if (threadIdx.x == 0) { s_n = 0; s_near = 0; s_tests = 0; }
     __syncthreads();
     for (int64_t t0 = t_first + (int64_t)blockIdx.x * blockDim.x; t0 < n; t0 += stride) {
         const int64_t t = t0 + threadIdx.x;
@@ -491,6 +492,10 @@ snr_cand_kernel(SnrArgs a)
         }
         const unsigned sel_mask = __ballot_sync(0xffffffffu, sel);
         const unsigned near_mask = __ballot_sync(0xffffffffu, near);
+        if (a.test_count) {
+            const unsigned test_mask = __ballot_sync(0xffffffffu, w > 0);
+            if (test_mask && lane == 0) atomicAdd(&s_tests, __popc(test_mask));
+        }
         if (sel_mask) {
             int base = 0;
             if (lane == 0) base = atomicAdd(&s_n, __popc(sel_mask));
@@ -518,6 +523,7 @@ snr_cand_kernel(SnrArgs a)
             __syncthreads();
         }
     }
+    if (threadIdx.x == 0 && a.test_count && s_tests) atomicAdd((unsigned long long *)(a.test_count + rowc), (unsigned long long)s_tests);
     if (threadIdx.x == 0 && s_near && a.near_count)
         atomicAdd((unsigned long long *)(a.near_count + (a.near_per_cat ? rowc : 0)), (unsigned long long)s_near);
 }
@@ -608,10 +614,12 @@ int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, con
 // sel_count[0 .. n_cat] is accumulated into (zero it for a fresh selection).
 int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th, uint8_t *resolved, double *rho2_out,
                     int64_t n_launch, int64_t *sel_idx, int64_t *sel_count, int64_t *near_count, int near_per_cat,
-                    const int *abort_flag, bool use_prefix, const SnrWork &sw, const DirtyView &dv, cudaStream_t st)
+                    const int *abort_flag, bool use_prefix, const SnrWork &sw, const DirtyView &dv, int64_t *test_count,
+                    cudaStream_t st)
 {
     if (n_launch <= 0) return GBFG_OK;
     SnrArgs a;
+    a.test_count = test_count;
     a.dv = dv;
     a.psd = psd;
     a.pv = make_view(sw, n_bins);
