@@ -155,9 +155,9 @@ def algorithmic_bytes(w: wl.Workload, n_bins: int, res, prof) -> dict:
     }
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of one full-pass running_median_kernel launch, from the
-# committed `ncu --set full` capture (profiles/r01_ncu_full_v2.md)
-MEDIAN_FULL_PASS_DRAM_BYTES = None
+# dram__bytes_read.sum + dram__bytes_write.sum of running_median_kernel per output it recomputes, from the
+# committed `ncu --set full` capture (profiles/r01_ncu_full_v2.md: 71.5 MB for ~3.5e6 outputs)
+MEDIAN_DRAM_BYTES_PER_OUTPUT = 20.5
 
 
 def run_gpu(args, w: wl.Workload):
@@ -275,9 +275,9 @@ def run_gpu(args, w: wl.Workload):
     kd = kernels[dom]
     bytes_per_launch = kd["algorithmic_bytes_per_step"] / kd["launches_per_step"]
     traffic = args.traffic
-    if traffic is None and dom == "median" and MEDIAN_FULL_PASS_DRAM_BYTES is not None:
-        # per launch like `achieved`: the capture is of a full pass; an average launch recomputes a fraction
-        traffic = MEDIAN_FULL_PASS_DRAM_BYTES * bytes_per_launch / (32.0 * nb)
+    if traffic is None and dom == "median":
+        # per launch like `achieved`: an average launch recomputes bytes_per_launch / 32 outputs
+        traffic = MEDIAN_DRAM_BYTES_PER_OUTPUT * bytes_per_launch / 32.0
     roofline = {"kernel": dom, "bound": "hbm", "achieved": bytes_per_launch / (kd["avg_launch_ms"] * 1e-3) / 1e9,
                 "peak": peak, "peak_source": peak_src, "unit": "GB/s",
                 "frac": bytes_per_launch / (kd["avg_launch_ms"] * 1e-3) / 1e9 / peak,

@@ -366,3 +366,55 @@ def test_loop_batch_matches_per_catalog_oracle(gb, orc, torch):
         assert res[c].n_near_threshold == ref["n_near_threshold"]
         iters.add(ref["n_iter"])
     assert len(iters) > 1          # the catalogs really stop at different iterations
+
+
+@pytest.mark.slow
+def test_loop_config4_full(gb, orc, torch):
+    """configs[4] at full size (64 catalogs, 2.97e8 sources) in one batched launch sequence.  The oracle
+    checks three catalogs element by element (the two smallest and the largest); every catalog is checked
+    through properties that hold at any size: power conservation in fixed point (total - residual = the
+    deposit of exactly the resolved sources), residual and median >= 0, PSD >= S_instr, the iteration
+    trace adds up."""
+    w = wl.config(4)
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    n, nb, nc = w.n_src_total, g.n_bins, w.n_cat
+    s_instr_h = orc.instrument_noise(og)
+    s_instr = dev(torch, s_instr_h)
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    total, spec, med = (torch.empty((nc, nb), dtype=torch.int64, device="cuda") for _ in range(3))
+    psd = torch.empty((nc, nb), dtype=torch.float64, device="cuda")
+    resolved = torch.empty(n, dtype=torch.uint8, device="cuda")
+    ws = workspace(torch, gb, g, n, nc)
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter)
+    res = gb.simulate(g, w.pops, w.offsets(), w.seed, s_instr, params, A, f, fd, total, spec, med, psd, resolved, ws)
+    off = w.offsets()
+    # properties, every catalog
+    assert int(spec.min().item()) >= 0 and int(med.min().item()) >= 0
+    assert bool((psd >= s_instr.unsqueeze(0)).all().item())
+    sel = torch.nonzero(resolved, as_tuple=False).flatten().to(torch.int64)
+    cnt = torch.tensor([sel.numel()], dtype=torch.int64, device="cuda")
+    redep = torch.zeros((nc, nb), dtype=torch.int64, device="cuda")
+    gb.deposit(g, A, f, fd, off, redep, ws, sign=+1, dev_sel_idx=sel, dev_sel_count=cnt)
+    assert torch.equal(total - spec, redep)                       # power conservation, exactly
+    n_res_gpu = torch.zeros(nc, dtype=torch.int64)
+    for c in range(nc):
+        r = res[c]
+        k = min(r.n_iter, gb.MAX_ITER_TRACE)
+        assert 1 <= r.n_iter <= w.max_iter
+        assert sum(r.n_new_per_iter[:k]) == r.n_resolved
+        assert (r.n_new_per_iter[r.n_iter - 1] == 0) == bool(r.converged)
+        n_res_gpu[c] = int(resolved[int(off[c]):int(off[c + 1])].sum().item())
+        assert n_res_gpu[c] == r.n_resolved
+    # the oracle, element by element, on three catalogs
+    order = sorted(range(nc), key=lambda c: w.pops[c].n_src)
+    for c in (order[0], order[1], order[-1]):
+        ref = orc.simulate(w, cat=c)
+        s = slice(int(off[c]), int(off[c + 1]))
+        assert np.array_equal(bits(A[s].cpu().numpy()), bits(ref["A"]))
+        assert np.array_equal(total[c].cpu().numpy(), ref["total"])
+        assert np.array_equal(spec[c].cpu().numpy(), ref["residual"])
+        assert np.array_equal(med[c].cpu().numpy(), ref["median"])
+        assert np.array_equal(bits(psd[c].cpu().numpy()), bits(ref["psd"]))
+        assert np.array_equal(resolved[s].cpu().numpy(), ref["resolved"])
+        assert (res[c].n_iter, res[c].converged, res[c].n_resolved) == (ref["n_iter"], ref["converged"], ref["n_resolved"])
