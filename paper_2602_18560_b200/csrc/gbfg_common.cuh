@@ -111,6 +111,8 @@ struct DepositMarks {
 struct MedianPlan {
     int4 *items;
     int *ctr;           // [0] number of items, [1] next item to take (both zero before plan_kernel)
+    int4 *wide_items;   // [max_items] tiles left to the 64-bit-key kernel
+    int *wide_ctr;      // [0] their number, [1] next to take
     int *cum;           // [n_cat][n_dblk + 1]
     int *range;         // [n_cat][2] first and last dirty block
     int n_dblk;

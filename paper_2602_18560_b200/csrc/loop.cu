@@ -24,7 +24,7 @@ int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins,
                 const MedianPlan &pl, int64_t *zero_ptr, int zero_n, int64_t *out_count, cudaStream_t st);
 int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *med,
                   const double *s_instr, double *psd, double norm, int scale_log2,
-                  const MedianPlan *plan, int *neg_flag, cudaStream_t st);
+                  const MedianPlan *plan, int4 *wide_items, int *wide_ctr, int *neg_flag, cudaStream_t st);
 int pfx_tiles_per_row(int64_t n_bins);
 size_t snr_pref_bytes(int64_t n_bins, int n_cat);
 size_t snr_tile_off_bytes(int64_t n_bins, int n_cat);
@@ -84,6 +84,8 @@ static Workspace carve(void *base, int64_t n_bins, int64_t n_src_total, int n_ca
     w.plan.range = (int *)take(sizeof(int) * 2 * (size_t)n_cat);
     w.plan.items = (int4 *)take(sizeof(int4) * (size_t)w.plan.max_items);
     w.plan.ctr = (int *)take(sizeof(int) * 4);
+    w.plan.wide_items = (int4 *)take(sizeof(int4) * (size_t)w.plan.max_items);
+    w.plan.wide_ctr = (int *)take(sizeof(int) * 4);
     w.sel_idx = (int64_t *)take(sizeof(int64_t) * nsrc);
     w.counters = (int64_t *)take(sizeof(int64_t) * WS_COUNTERS);
     w.wide_flag = (int *)take(sizeof(int) * (size_t)(1 + n_cat));   // flag, then one scan ticket per row
@@ -305,7 +307,7 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
         rc = launch_plan(w.blk_stamp, it, it == 0 || !incremental, nb, n_cat, W, w.plan, w.counters, (int)n_iter_counters, med_outputs, st);
         if (rc) return rc;
         rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
-                           grid->scale_log2, &w.plan, neg_flag, st);
+                           grid->scale_log2, &w.plan, nullptr, nullptr, neg_flag, st);
         if (rc) return rc;
         rc = launch_inv_prefix(dev_psd, nb, n_cat, w.sw, dirty, st);
         if (rc) return rc;
@@ -355,7 +357,7 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
         rc = launch_plan(w.blk_stamp, params->max_iter, !incremental, nb, n_cat, W, w.plan, nullptr, 0, med_outputs, st);
         if (rc) return rc;
         rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
-                           grid->scale_log2, &w.plan, nullptr, st);
+                           grid->scale_log2, &w.plan, nullptr, nullptr, nullptr, st);
         if (rc) return rc;
     }
     GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));

@@ -21,425 +21,9 @@
 //     (on average LT/W steps).
 // The per-output rank is kept in shared memory and written out coalesced, fused with
 //     psd[k] = s_instr[k] + C * (med[k] * 2^scale_log2)        (eqs. 10, D2, D3).
-#include "gbfg_common.cuh"
+#include "median_kernel.cuh"
 
 namespace gbfg {
-
-constexpr int MED_LT = 8192;                  // positions per tile, halos included (power of two)
-constexpr int MED_THREADS = 1024;
-constexpr int MED_WARPS = MED_THREADS / 32;
-constexpr int MED_ITEMS = MED_LT / MED_THREADS;   // 8 keys per thread in the sort
-constexpr int MED_PB = 32;                    // position block = outputs per coarse chunk
-constexpr int MED_FINE = 8;                   // outputs per walking thread
-constexpr int MED_STEP_CAP = 12;               // places a thread steps alone before the warp takes over
-constexpr int MED_RB = 128;                   // sorted ranks per bucket
-constexpr int MED_NPB = MED_LT / MED_PB;      // 256
-constexpr int MED_NRB = MED_LT / MED_RB;      // 64
-constexpr int MED_TROW = MED_NPB + 2;         // table row stride in u16 (even: rows stay 4-byte aligned)
-constexpr int MED_CROW = 256 + 2;             // radix counter row stride in u16 (one row per warp)
-constexpr uint64_t SIGN64 = 0x8000000000000000ull;
-
-constexpr size_t MED_AUX_U16 = (MED_NRB * MED_TROW > MED_WARPS * MED_CROW) ? MED_NRB * MED_TROW : MED_WARPS * MED_CROW;
-constexpr size_t MED_SMEM = sizeof(uint64_t) * MED_LT      // skey
-                          + sizeof(uint16_t) * MED_LT      // spos
-                          + sizeof(uint16_t) * MED_LT      // rop
-                          + sizeof(uint16_t) * MED_LT      // orank
-                          + sizeof(uint16_t) * MED_AUX_U16 // radix counters, then the count table
-                          + sizeof(uint16_t) * MED_NPB     // coarse medians
-                          + sizeof(uint32_t) * 40;         // scan partials, varying-bit mask
-
-struct MedianArgs {
-    const int64_t *x;        // [n_cat][n]
-    int64_t *med;            // [n_cat][n]
-    const double *s_instr;   // [n] or NULL (no PSD)
-    double *psd;             // [n_cat][n] or NULL
-    const int4 *items;       // work list (row, first output, outputs, -) or NULL: static tiling of every row
-    int *ctr;                // [0] number of items, [1] next item
-    int n_cat;
-    int *neg_flag;           // nullable: set to 1 when a median is negative
-    int64_t n;
-    int h;
-    int S;                   // outputs per tile = MED_LT - 2h
-    int tiles;
-    double norm, scale;      // C and 2^scale_log2
-};
-
-// n-th (1-based) set bit of a non-zero mask that has at least n bits set
-__device__ __forceinline__ int nth_set_bit(unsigned m, int n)
-{
-    int pos = 0, c;
-    c = __popc(m & 0xffffu); if (n > c) { n -= c; m >>= 16; pos += 16; }
-    c = __popc(m & 0xffu);   if (n > c) { n -= c; m >>= 8;  pos += 8; }
-    c = __popc(m & 0xfu);    if (n > c) { n -= c; m >>= 4;  pos += 4; }
-    c = __popc(m & 0x3u);    if (n > c) { n -= c; m >>= 2;  pos += 2; }
-    if (n > (int)(m & 1u)) pos += 1;
-    return pos;
-}
-
-// lanes of the warp whose 8-bit digit equals this lane's (what match.any computes, from 8 ballots)
-__device__ __forceinline__ unsigned same_digit_lanes(unsigned d)
-{
-    unsigned peers = 0xffffffffu;
-#pragma unroll
-    for (int b = 0; b < 8; ++b) {
-        const bool bit = (d >> b) & 1u;
-        const unsigned bal = __ballot_sync(0xffffffffu, bit);
-        peers &= bit ? bal : ~bal;
-    }
-    return peers;
-}
-
-__global__ void __launch_bounds__(MED_THREADS, 1)
-running_median_kernel(MedianArgs a)
-{
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    uint64_t *skey = reinterpret_cast<uint64_t *>(smem_raw);
-    uint16_t *spos = reinterpret_cast<uint16_t *>(skey + MED_LT);
-    uint16_t *rop = spos + MED_LT;
-    uint16_t *orank = rop + MED_LT;
-    uint16_t *aux = orank + MED_LT;                       // radix counters, later the count table
-    uint16_t *cm = aux + MED_AUX_U16;                     // coarse medians
-    uint32_t *misc = reinterpret_cast<uint32_t *>(cm + MED_NPB);
-    uint16_t *tab = aux;
-    uint32_t *aux32 = reinterpret_cast<uint32_t *>(aux);
-
-    const int tid = threadIdx.x;
-    const int warp = tid >> 5, lane = tid & 31;
-    const unsigned FULL = 0xffffffffu;
-    const unsigned lt_mask = (1u << lane) - 1u;
-    const int h = a.h, W = 2 * a.h + 1;
-    __shared__ int s_item;
-    bool neg = false;
-
-  for (int64_t turn = blockIdx.x;; turn += gridDim.x) {
-    int64_t row, o0;
-    int n_out;
-    __syncthreads();                                     // the previous tile's epilogue is done with shared memory
-    if (a.items) {
-        if (tid == 0) s_item = atomicAdd(&a.ctr[1], 1);
-        __syncthreads();
-        const int item = s_item;
-        if (item >= a.ctr[0]) break;
-        const int4 v = a.items[item];
-        row = (int64_t)v.x * a.n;
-        o0 = v.y;
-        n_out = v.z;
-    } else {
-        if (turn >= (int64_t)a.tiles * a.n_cat) break;
-        const int64_t r = turn / a.tiles, tile = turn - r * a.tiles;
-        row = r * a.n;
-        o0 = tile * a.S;
-        n_out = (int)((a.n - o0 < a.S) ? (a.n - o0) : a.S);
-    }
-    const int Lt = n_out + 2 * h;                        // positions really used
-    const int rounds = (Lt + MED_THREADS - 1) / MED_THREADS;   // keys per thread in the sort (<= MED_ITEMS)
-    const int LTe = rounds * MED_THREADS;                // positions sorted
-
-    // ---- stage the tile: position p <-> global bin o0 - h + p, reflected at both ends.
-    // Unused positions (Lt <= p < LTe) repeat position 0: they are never inside a window.
-    if (tid < 2) misc[32 + tid] = 0u;
-    __syncthreads();
-    {
-        int64_t g0 = o0 - h;
-        if (g0 < 0) g0 = -g0 - 1;
-        if (g0 >= a.n) g0 = 2 * a.n - 1 - g0;
-        const uint64_t key_ref = (uint64_t)a.x[row + g0] ^ SIGN64;
-        uint64_t vary = 0;
-        for (int p = tid; p < LTe; p += MED_THREADS) {
-            uint64_t key = key_ref;
-            if (p < Lt) {
-                int64_t g = o0 - h + p;
-                if (g < 0) g = -g - 1;
-                if (g >= a.n) g = 2 * a.n - 1 - g;
-                key = (uint64_t)a.x[row + g] ^ SIGN64;
-            }
-            vary |= key ^ key_ref;
-            skey[p] = key;
-            spos[p] = (uint16_t)p;
-        }
-        const unsigned vlo = __reduce_or_sync(FULL, (unsigned)vary);
-        const unsigned vhi = __reduce_or_sync(FULL, (unsigned)(vary >> 32));
-        if (lane == 0) {
-            if (vlo) atomicOr(&misc[32], vlo);
-            if (vhi) atomicOr(&misc[33], vhi);
-        }
-    }
-    __syncthreads();
-    const uint64_t vary_all = ((uint64_t)misc[33] << 32) | misc[32];
-    const int n_pass = vary_all ? (64 - __clzll((long long)vary_all) + 7) / 8 : 0;
-
-    // ---- LSD radix sort by key, stable, so that equal keys stay in position order.
-    // Warp w owns elements [32 rounds w, 32 rounds (w + 1)) of the current order, 32 consecutive ones per round.
-    for (int pass = 0; pass < n_pass; ++pass) {
-        const int shift = 8 * pass;
-        for (int e = tid; e < MED_WARPS * MED_CROW / 2; e += MED_THREADS) aux32[e] = 0u;
-        __syncthreads();
-        uint16_t *cw = aux + warp * MED_CROW;
-        uint64_t k[MED_ITEMS];
-        uint32_t pp[MED_ITEMS], off[MED_ITEMS], peers[MED_ITEMS];
-#pragma unroll
-        for (int r = 0; r < MED_ITEMS; ++r) {            // the matches are independent: issue them together
-            if (r < rounds) {
-                const int e = warp * (32 * rounds) + r * 32 + lane;
-                k[r] = skey[e];
-                pp[r] = spos[e];
-                off[r] = (unsigned)(k[r] >> shift) & 255u;
-                peers[r] = same_digit_lanes(off[r]);
-            }
-        }
-#pragma unroll
-        for (int r = 0; r < MED_ITEMS; ++r) {            // counter updates, round after round
-            if (r < rounds) {
-                const unsigned d = off[r];
-                const unsigned base = cw[d];
-                __syncwarp();
-                const unsigned rank = __popc(peers[r] & lt_mask);
-                if (rank == 0) cw[d] = (uint16_t)(base + __popc(peers[r]));
-                __syncwarp();
-                off[r] = (d << 16) | (base + rank);
-            }
-        }
-        __syncthreads();
-        {   // exclusive scan of the counters in (digit, warp) order: thread t owns digit t/4, warps 8(t%4)..+8
-            const int d = tid >> 2, wg = (tid & 3) * 8;
-            unsigned v[8], s = 0;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) { v[i] = aux[(wg + i) * MED_CROW + d]; s += v[i]; }
-            unsigned incl = s;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                unsigned up = __shfl_up_sync(FULL, incl, o);
-                if (lane >= o) incl += up;
-            }
-            if (lane == 31) misc[warp] = incl;
-            __syncthreads();
-            unsigned wt = misc[lane], wincl = wt;
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                unsigned up = __shfl_up_sync(FULL, wincl, o);
-                if (lane >= o) wincl += up;
-            }
-            const unsigned wprev = __shfl_sync(FULL, wincl - wt, warp);
-            unsigned run = wprev + incl - s;
-#pragma unroll
-            for (int i = 0; i < 8; ++i) { aux[(wg + i) * MED_CROW + d] = (uint16_t)run; run += v[i]; }
-        }
-        __syncthreads();
-#pragma unroll
-        for (int r = 0; r < MED_ITEMS; ++r) {
-            if (r < rounds) {
-                const unsigned dst = (unsigned)cw[off[r] >> 16] + (off[r] & 0xffffu);
-                skey[dst] = k[r];
-                spos[dst] = (uint16_t)pp[r];
-            }
-        }
-        __syncthreads();
-    }
-
-    // ---- inverse permutation and the count table
-    for (int e = tid; e < MED_NRB * MED_TROW / 2; e += MED_THREADS) aux32[e] = 0u;
-    __syncthreads();
-    for (int r = tid; r < LTe; r += MED_THREADS) {
-        int p = spos[r];
-        rop[p] = (uint16_t)r;
-        int e = (r / MED_RB) * MED_TROW + (p / MED_PB) + 1;
-        atomicAdd(&aux32[e >> 1], (e & 1) ? 0x10000u : 1u);
-    }
-    __syncthreads();
-    // prefix along the position blocks: tab[rb][pb] = #{r in bucket rb : pos < pb*PB}
-    {
-        constexpr int PER = (MED_NPB + 1 + 31) / 32;     // 9 entries per lane
-        for (int rb = warp; rb < MED_NRB; rb += MED_WARPS) {
-            uint16_t *rowp = tab + rb * MED_TROW;
-            int v[PER], s = 0;
-#pragma unroll
-            for (int q = 0; q < PER; ++q) {
-                int idx = lane * PER + q;
-                v[q] = idx <= MED_NPB ? rowp[idx] : 0;
-                s += v[q];
-            }
-            int incl = s;
-            for (int o = 1; o < 32; o <<= 1) {
-                int up = __shfl_up_sync(FULL, incl, o);
-                if (lane >= o) incl += up;
-            }
-            int run = incl - s;
-#pragma unroll
-            for (int q = 0; q < PER; ++q) {
-                int idx = lane * PER + q;
-                run += v[q];
-                if (idx <= MED_NPB) rowp[idx] = (uint16_t)run;
-            }
-        }
-    }
-    __syncthreads();
-    // exclusive prefix along the rank buckets: tab[rb][pb] = #{r < rb*RB : pos < pb*PB}
-    for (int pb = tid; pb <= MED_NPB; pb += MED_THREADS) {
-        int run = 0;
-        for (int rb = 0; rb < MED_NRB; ++rb) {
-            int v = tab[rb * MED_TROW + pb];
-            tab[rb * MED_TROW + pb] = (uint16_t)run;
-            run += v;
-        }
-    }
-    __syncthreads();
-
-    // ---- coarse states.  Warp w owns the chunks [w cpw, (w+1) cpw) of 32 outputs.  The median rank of
-    // the window of its first chunk comes from the count table; the following ones by sliding the
-    // window 32 bins at a time: two ballots count the ranks under m that left and entered, and the
-    // warp moves m by that many window elements, 32 places of the sorted order per step.
-    const int n_coarse = (n_out + MED_PB - 1) / MED_PB;
-    const int cpw = (n_coarse + MED_WARPS - 1) / MED_WARPS;
-    const int c_first = warp * cpw;
-    // warp-cooperative search: from rank wm (exclusive) in direction wdir to the wneed-th element whose
-    // position lies in [wplo, wphi]; all arguments warp-uniform; wm is updated
-#define WARP_SEEK(wm, wdir, wneed, wplo, wphi)                                                     \
-        for (;;) {                                                                                 \
-            const int r_ = (wm) + (wdir) * (1 + lane);                                             \
-            const bool ok_ = (unsigned)r_ < (unsigned)LTe;                                         \
-            const bool in_ = ok_ && (unsigned)((int)spos[ok_ ? r_ : 0] - (wplo)) <= (unsigned)((wphi) - (wplo)); \
-            const unsigned bal_ = __ballot_sync(FULL, in_);                                        \
-            const int cn_ = __popc(bal_);                                                          \
-            if ((wneed) <= cn_) { (wm) += (wdir) * (1 + nth_set_bit(bal_, (wneed))); break; }      \
-            (wneed) -= cn_;                                                                        \
-            (wm) += 32 * (wdir);                                                                   \
-            if ((unsigned)(wm) >= (unsigned)LTe) break;    /* not reachable: the window holds the element */ \
-        }
-    if (c_first < n_coarse) {
-        int m = LTe;
-        {
-            const int c = c_first;
-            const int j0 = c * MED_PB;
-            const int b0 = c, b1 = (j0 + W) / MED_PB;
-            const int na = b1 * MED_PB - j0;                 // block-aligned part of the window
-            int below = 0, phi = j0 - 1;
-            if (na > 0) {
-                const int t = (h < na - 1) ? h : na - 1;
-                // largest bucket lo with #{rank < 128 lo, position in the aligned part} <= t
-                const int c0 = (int)tab[lane * MED_TROW + b1] - (int)tab[lane * MED_TROW + b0];
-                const int c1 = (int)tab[(lane + 32) * MED_TROW + b1] - (int)tab[(lane + 32) * MED_TROW + b0];
-                const unsigned m0 = __ballot_sync(FULL, c0 <= t), m1 = __ballot_sync(FULL, c1 <= t);
-                const int lo = m1 ? 63 - __clz(m1) : 31 - __clz(m0);
-                const int cl = lo < 32 ? __shfl_sync(FULL, c0, lo & 31) : __shfl_sync(FULL, c1, lo & 31);
-                int need = t - cl + 1;                       // the (t - cl + 1)-th aligned element from rank 128 lo on
-                m = lo * MED_RB - 1;
-                WARP_SEEK(m, 1, need, j0, j0 + na - 1);
-                below = t;
-                phi = b1 * MED_PB - 1;
-            }
-            // complete the window with the (at most 31, or W when W < 32) remaining positions
-            for (int pbase = phi + 1; pbase < j0 + W; pbase += 32) {
-                const int p = pbase + lane;
-                const bool add = p < j0 + W && (int)rop[p < j0 + W ? p : 0] < m;
-                below += __popc(__ballot_sync(FULL, add));
-            }
-            if (below > h) {                                 // down to the (below - h)-th window element under m
-                int need = below - h;
-                WARP_SEEK(m, -1, need, j0, j0 + W - 1);
-            } else {                                         // up to the (h - below + 1)-th window element at or above m
-                int need = h - below + 1;
-                m -= 1;
-                WARP_SEEK(m, 1, need, j0, j0 + W - 1);
-            }
-            if (lane == 0) cm[c] = (uint16_t)m;
-        }
-        const int c_last = (c_first + cpw < n_coarse) ? c_first + cpw : n_coarse;
-        for (int c = c_first + 1; c < c_last; ++c) {
-            const int j0 = c * MED_PB;                       // window [j0, j0 + W); the last one started 32 bins earlier
-            const int gone = rop[j0 - MED_PB + lane], come = rop[j0 - MED_PB + W + lane];
-            const int n_gone = __popc(__ballot_sync(FULL, gone < m)), n_come = __popc(__ballot_sync(FULL, come < m));
-            const bool m_left = __ballot_sync(FULL, gone == m) != 0u;
-            const int below = h + n_come - n_gone;
-            int dir, need;
-            if (below > h) { dir = -1; need = below - h; }
-            else { dir = 1; need = h - below + (m_left ? 1 : 0); }
-            if (need) { WARP_SEEK(m, dir, need, j0, j0 + W - 1); }
-            if (lane == 0) cm[c] = (uint16_t)m;
-        }
-    }
-    __syncthreads();
-
-    // ---- every thread walks MED_FINE outputs, starting from the coarse state of its chunk.
-    // `below` = #{window elements of rank < m}.  One rule for every move: the median is the
-    // (below - h)-th window element under m, or the (h - below)-th above it, counting m itself first
-    // when it is still in the window.  A thread steps along the sorted order on its own for at most
-    // MED_STEP_CAP places; spectra with plateaus (wide chirps put the same power in consecutive bins)
-    // and level-correlated neighbourhoods have stretches of hundreds of out-of-window elements, and
-    // those searches are finished by the whole warp, 32 places per step.
-    {
-        const int s = tid / n_coarse, c = tid - s * n_coarse;
-        const int j_first = c * MED_PB + s * MED_FINE;
-        const bool alive = s < MED_PB / MED_FINE && j_first < n_out;
-        const int j_end = alive ? ((j_first + MED_FINE < n_out) ? j_first + MED_FINE : n_out) : j_first;
-        int m = 0, plo = 0, phi = -1, dir = 1, need = 0;
-#define IN_SET(r) ((unsigned)((int)spos[r] - plo) <= (unsigned)(phi - plo))
-        // the warp completes the searches its lanes left unfinished: lane `src` still needs `need`
-        // window elements from rank m (exclusive) in direction dir
-#define WARP_FINISH()                                                                              \
-        for (unsigned pend = __ballot_sync(FULL, need > 0); pend; pend &= pend - 1) {              \
-            const int src = __ffs(pend) - 1;                                                       \
-            int wm = __shfl_sync(FULL, m, src);                                                    \
-            const int wdir = __shfl_sync(FULL, dir, src);                                          \
-            int wneed = __shfl_sync(FULL, need, src);                                              \
-            const int wplo = __shfl_sync(FULL, plo, src), wphi = __shfl_sync(FULL, phi, src);      \
-            WARP_SEEK(wm, wdir, wneed, wplo, wphi);                                                \
-            if (lane == src) { m = wm; need = 0; }                                                 \
-        }
-        if (alive) {
-            int below = h;
-            m = cm[c];
-            plo = c * MED_PB;
-            phi = plo + W - 1;
-            // jump: count the ranks under m that left and entered
-            const int jump = s * MED_FINE;
-            for (int i = 0; i < jump; ++i) {
-                below += ((int)rop[phi + 1 + i] < m) - ((int)rop[plo + i] < m);
-            }
-            plo += jump;
-            phi += jump;
-            if (below > h) { dir = -1; need = below - h; }
-            else { dir = 1; need = h - below + (IN_SET(m) ? 0 : 1); }
-            for (int t = 0; need && t < 3 * MED_STEP_CAP; ++t) { m += dir; if (IN_SET(m)) --need; }
-        }
-        WARP_FINISH();
-        if (alive) orank[j_first] = (uint16_t)m;
-#pragma unroll 1
-        for (int jj = 1; jj < MED_FINE; ++jj) {
-            const int j = j_first + jj;
-            const bool on = j < j_end;
-            if (on) {
-                const int gone = rop[plo];                    // position j-1 leaves
-                ++plo;
-                const int come = rop[phi + 1];                // position j+2h enters
-                ++phi;
-                const int b = h + (come < m) - (gone < m);    // h-1, h or h+1
-                dir = b > h ? -1 : 1;
-                need = (b != h || gone == m) ? 1 : 0;
-                for (int t = 0; need && t < MED_STEP_CAP; ++t) { m += dir; if (IN_SET(m)) need = 0; }
-            }
-            WARP_FINISH();
-            if (on) orank[j] = (uint16_t)m;
-        }
-#undef WARP_FINISH
-#undef WARP_SEEK
-#undef IN_SET
-    }
-    __syncthreads();
-
-    // ---- coalesced epilogue: median and PSD
-    for (int j = tid; j < n_out; j += MED_THREADS) {
-        int64_t v = (int64_t)(skey[orank[j]] ^ SIGN64);
-        int64_t g = o0 + j;
-        a.med[row + g] = v;
-        neg |= v < 0;
-        if (a.psd) {
-            double e = (double)v * a.scale;
-            a.psd[row + g] = a.s_instr[g] + a.norm * e;
-        }
-    }
-  }   // tiles
-    if (a.neg_flag && neg) *a.neg_flag = 1;
-}
 
 __global__ void __launch_bounds__(256)
 psd_kernel(const int64_t *__restrict__ med, const double *__restrict__ s_instr, int64_t n, double norm,
@@ -481,6 +65,7 @@ struct PlanArgs {
     int64_t *zero_ptr;      // per-iteration counters of the loop, cleared here (nullable)
     int zero_n;
     int64_t *out_count;     // [n_cat] outputs planned, accumulated (nullable)
+    int *wide_ctr;          // [2] counter words of the wide list, cleared here
 };
 
 // len < 2^31 (n_bins is): 32-bit divisions, the 64-bit ones are long instruction sequences
@@ -511,6 +96,7 @@ plan_kernel(PlanArgs a)
     const int b_lo = min(tid * per, nb), b_hi = min(b_lo + per, nb);
     int *s_run = s_cum + nb + 1;
     if (tid == 0) { n_runs = 0; row_pieces = 0; }
+    if (row == 0 && tid < 2) a.wide_ctr[tid] = 0;
     if (row == 0 && a.zero_ptr) for (int i = tid; i < a.zero_n; i += PLAN_THREADS) a.zero_ptr[i] = 0;
     for (int b0 = tid; b0 < nb; b0 += 8 * PLAN_THREADS) {   // coalesced, eight loads in flight per thread
         int v[8];
@@ -637,7 +223,8 @@ int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins,
     a.blk_stamp = blk_stamp; a.stamp = stamp; a.all_dirty = (all_dirty || !blk_stamp) ? 1 : 0;
     a.n_dblk = pl.n_dblk; a.dblk_log2 = pl.dblk_log2; a.n_bins = n_bins;
     a.S = MED_LT - (window - 1);
-    a.wave = sm_count();
+    a.wave = 2 * sm_count();                             // two CTAs of the 32-bit-key kernel per SM
+    a.wide_ctr = pl.wide_ctr;
     a.cum = pl.cum; a.range = pl.range; a.items = pl.items; a.ctr = pl.ctr; a.max_items = pl.max_items;
     const size_t smem = plan_smem_bytes(pl.n_dblk);
     static thread_local int attr_dev = -1;
@@ -658,38 +245,54 @@ int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins,
 }
 
 // internal entry: median (+ PSD when psd != NULL).  plan != NULL: the tiles of its work list (made by
-// launch_plan on the same stream); NULL: every row, statically tiled.  neg_flag nullable: raised when
-// a median is negative.
+// launch_plan on the same stream); NULL: every row, statically tiled, and wide_items / wide_ctr give the
+// room for the wide list ([tiles of the call] int4, 2 ints zeroed here).  neg_flag nullable: raised when
+// a median is negative.  Two launches: the 32-bit-key kernel, two CTAs per SM, then the 64-bit-key kernel
+// on the tiles the first one could not order (none for spectra in units of 2^-140 strain^2).
+int median_static_tiles(int64_t n_bins, int n_cat, int window, int *S_out)
+{
+    const int s_max = MED_LT - (window - 1);
+    const int slots = 2 * sm_count();
+    int64_t tiles = (n_bins + s_max - 1) / s_max;
+    if (tiles * n_cat > slots && n_cat == 1) tiles = (tiles + slots - 1) / slots * slots;   // whole waves of CTAs
+    const int S = (int)((n_bins + tiles - 1) / tiles);
+    if (S_out) *S_out = S;
+    return (int)((n_bins + S - 1) / S);
+}
+
 int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *med,
                   const double *s_instr, double *psd, double norm, int scale_log2,
-                  const MedianPlan *plan, int *neg_flag, cudaStream_t st)
+                  const MedianPlan *plan, int4 *wide_items, int *wide_ctr, int *neg_flag, cudaStream_t st)
 {
     MedianArgs a;
     a.x = x; a.med = med; a.s_instr = s_instr; a.psd = psd; a.neg_flag = neg_flag;
     a.items = plan ? plan->items : nullptr; a.ctr = plan ? plan->ctr : nullptr; a.n_cat = n_cat;
+    a.wide_items = plan ? plan->wide_items : wide_items;
+    a.wide_ctr = plan ? plan->wide_ctr : wide_ctr;
     a.n = n_bins; a.h = window / 2;
-    const int s_max = MED_LT - 2 * a.h;
-    const int sms = sm_count();
-    // static tiling: whole waves of CTAs when a row needs more than one
-    int64_t tiles = (n_bins + s_max - 1) / s_max;
-    if (tiles * n_cat > sms && n_cat == 1) tiles = (tiles + sms - 1) / sms * sms;
-    a.S = (int)((n_bins + tiles - 1) / tiles);
-    a.tiles = (int)((n_bins + a.S - 1) / a.S);
+    a.tiles = median_static_tiles(n_bins, n_cat, window, &a.S);
     a.norm = norm; a.scale = ldexp(1.0, scale_log2);
+    constexpr size_t smem32 = median_smem_bytes<uint32_t>(), smem64 = median_smem_bytes<uint64_t>();
     static thread_local int attr_dev = -1;
     int dev = 0;
     GBFG_CUDA(cudaGetDevice(&dev));
     if (attr_dev != dev) {
-        GBFG_CUDA(cudaFuncSetAttribute(running_median_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)MED_SMEM));
+        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint32_t, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem32));
+        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint64_t, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem64));
         attr_dev = dev;
     }
-    int64_t grid = plan ? sms : (int64_t)a.tiles * n_cat;
+    const int sms = sm_count();
+    if (!plan) GBFG_CUDA(cudaMemsetAsync(a.wide_ctr, 0, 2 * sizeof(int), st));     // plan_kernel clears them otherwise
+    int64_t grid = plan ? 2 * sms : (int64_t)a.tiles * n_cat;
+    if (grid > 2 * sms) grid = 2 * sms;
+    LaunchTimer lt(K_MEDIAN, st);
+    running_median_tile_kernel<uint32_t, 512><<<(int)grid, 512, smem32, st>>>(a);
+    GBFG_LAUNCH_CHECK("running_median_tile_kernel<u32>");
+    a.items = a.wide_items; a.ctr = a.wide_ctr;
+    a.wide_items = nullptr; a.wide_ctr = nullptr;
     if (grid > sms) grid = sms;
-    {
-        LaunchTimer lt(K_MEDIAN, st);
-        running_median_kernel<<<(int)grid, MED_THREADS, MED_SMEM, st>>>(a);
-    }
-    GBFG_LAUNCH_CHECK("running_median_kernel");
+    running_median_tile_kernel<uint64_t, 1024><<<(int)grid, 1024, smem64, st>>>(a);
+    GBFG_LAUNCH_CHECK("running_median_tile_kernel<u64>");
     return GBFG_OK;
 }
 
@@ -706,8 +309,16 @@ extern "C" int gbfg_running_median(const int64_t *dev_spectrum, int64_t n_bins, 
     if (n_bins < window / 2 + 1) return GBFG_ERR_INVALID_ARG;
     int rc = check_device();
     if (rc) return rc;
-    return launch_median(dev_spectrum, n_bins, n_cat, window, dev_median_out, nullptr, nullptr, 1.0, 0, nullptr, nullptr,
-                         (cudaStream_t)stream);
+    // room for the wide list (tiles whose values differ in their high 32 bits), stream ordered
+    cudaStream_t st = (cudaStream_t)stream;
+    const int tiles = median_static_tiles(n_bins, n_cat, window, nullptr);
+    char *tmp = nullptr;
+    GBFG_CUDA(cudaMallocAsync((void **)&tmp, 16 + sizeof(int4) * (size_t)tiles * (size_t)n_cat, st));
+    rc = launch_median(dev_spectrum, n_bins, n_cat, window, dev_median_out, nullptr, nullptr, 1.0, 0, nullptr,
+                       (int4 *)(tmp + 16), (int *)tmp, nullptr, st);
+    cudaError_t e = cudaFreeAsync(tmp, st);
+    if (!rc && e != cudaSuccess) rc = set_cuda_error(e, "cudaFreeAsync");
+    return rc;
 }
 
 extern "C" int gbfg_psd(const int64_t *dev_median, const double *dev_s_instr, int64_t n_bins, int32_t n_cat,
