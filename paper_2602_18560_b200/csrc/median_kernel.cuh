@@ -186,7 +186,7 @@ running_median_tile_kernel(MedianArgs a)
             if (r < rounds) {
                 const int e = warp * (32 * rounds) + r * 32 + lane;
                 k[r] = skey[e];
-                pk[r] = same_digit_lanes((unsigned)(k[r] >> shift) & 255u);
+                pk[r] = __match_any_sync(FULL, (unsigned)(k[r] >> shift) & 255u);
             }
         }
 #pragma unroll
