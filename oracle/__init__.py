@@ -80,6 +80,12 @@ def lib():
         L.orc_subtract_until_converged.argtypes = [
             C.POINTER(Grid), dp, dp, dp, C.c_int64, dp, C.c_int32, C.c_double, C.c_double, C.c_int32,
             ip, ip, dp, up, C.POINTER(IterResult), ip]
+        L.orc_subtract_until_converged_est.argtypes = [
+            C.POINTER(Grid), dp, dp, dp, C.c_int64, dp, C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_int32,
+            ip, ip, dp, up, C.POINTER(IterResult), ip]
+        L.orc_running_sum_def.argtypes = [ip, C.c_int64, C.c_int32, C.c_int64, C.c_int64, ip]
+        L.orc_running_sum.argtypes = [ip, C.c_int64, C.c_int32, ip]
+        L.orc_psd_mean.argtypes = [ip, dp, C.c_int64, C.c_int32, C.c_int32, dp]
     return _lib
 
 
@@ -199,6 +205,33 @@ def running_median(x: np.ndarray, window: int) -> np.ndarray:
     return out
 
 
+def running_sum_def(x: np.ndarray, window: int, k_begin: int = 0, k_end: int | None = None) -> np.ndarray:
+    """Window sums of the running-mean estimator (eq. D1), the definition: one loop per output."""
+    x = np.ascontiguousarray(x, dtype=np.int64)
+    if k_end is None:
+        k_end = x.size
+    out = np.empty(k_end - k_begin, dtype=np.int64)
+    if lib().orc_running_sum_def(_i(x), x.size, window, k_begin, k_end, _i(out)):
+        raise ValueError("invalid window / size")
+    return out
+
+
+def running_sum(x: np.ndarray, window: int) -> np.ndarray:
+    x = np.ascontiguousarray(x, dtype=np.int64)
+    out = np.empty_like(x)
+    if lib().orc_running_sum(_i(x), x.size, window, _i(out)):
+        raise ValueError("invalid window / size")
+    return out
+
+
+def psd_from_sum(wsum: np.ndarray, s_instr: np.ndarray, window: int, scale_log2: int) -> np.ndarray:
+    wsum = np.ascontiguousarray(wsum, dtype=np.int64)
+    s_instr = _f64(s_instr)
+    out = np.empty(wsum.size, dtype=np.float64)
+    lib().orc_psd_mean(_i(wsum), _d(s_instr), wsum.size, window, scale_log2, _d(out))
+    return out
+
+
 def psd_from_median(med: np.ndarray, s_instr: np.ndarray, median_norm: float, scale_log2: int) -> np.ndarray:
     med = np.ascontiguousarray(med, dtype=np.int64)
     s_instr = _f64(s_instr)
@@ -228,7 +261,7 @@ def snr_select(grid: Grid, A, f, fdot, psd, rho_th: float, resolved: np.ndarray)
 
 def subtract_until_converged(grid: Grid, A, f, fdot, s_instr, window: int, median_norm: float,
                              rho_th: float, max_iter: int, spectrum: np.ndarray,
-                             resolved: np.ndarray | None = None):
+                             resolved: np.ndarray | None = None, estimator: int = 0):
     """Runs the loop in place on `spectrum` (total -> residual).
     -> dict(median, psd, resolved, n_iter, converged, n_resolved, n_near_threshold, n_new_per_iter)"""
     A, f, fdot, s_instr = _f64(A), _f64(f), _f64(fdot), _f64(s_instr)
@@ -240,9 +273,9 @@ def subtract_until_converged(grid: Grid, A, f, fdot, s_instr, window: int, media
     psd = np.empty(grid.n_bins, dtype=np.float64)
     res = IterResult()
     trace = np.zeros(max(max_iter, 1), dtype=np.int64)
-    rc = lib().orc_subtract_until_converged(C.byref(grid), _d(A), _d(f), _d(fdot), n, _d(s_instr), window,
-                                            median_norm, rho_th, max_iter, _i(spectrum), _i(med), _d(psd),
-                                            _u(resolved), C.byref(res), _i(trace))
+    rc = lib().orc_subtract_until_converged_est(C.byref(grid), _d(A), _d(f), _d(fdot), n, _d(s_instr), window,
+                                                median_norm, rho_th, max_iter, estimator, _i(spectrum), _i(med),
+                                                _d(psd), _u(resolved), C.byref(res), _i(trace))
     if rc:
         raise ValueError("invalid window / size")
     return dict(median=med, psd=psd, resolved=resolved, n_iter=res.n_iter, converged=res.converged,
@@ -250,7 +283,7 @@ def subtract_until_converged(grid: Grid, A, f, fdot, s_instr, window: int, media
                 n_new_per_iter=trace[:max_iter])
 
 
-def simulate(w, cat: int = 0, n_src: int | None = None):
+def simulate(w, cat: int = 0, n_src: int | None = None, estimator: int = 0):
     """Whole path for catalog `cat` of a gbfg_workloads.Workload: sample -> deposit -> loop."""
     grid = make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
     pop = make_pop(w.pops[cat])
@@ -261,6 +294,7 @@ def simulate(w, cat: int = 0, n_src: int | None = None):
     spec = np.zeros(grid.n_bins, dtype=np.int64)
     rejected = deposit(grid, A, f, fd, spec)
     total = spec.copy()
-    out = subtract_until_converged(grid, A, f, fd, s_instr, w.window, w.median_norm, w.rho_th, w.max_iter, spec)
+    out = subtract_until_converged(grid, A, f, fd, s_instr, w.window, w.median_norm, w.rho_th, w.max_iter, spec,
+                                   estimator=estimator)
     out.update(A=A, f=f, fdot=fd, s_instr=s_instr, total=total, residual=spec, rejected=rejected, grid=grid)
     return out

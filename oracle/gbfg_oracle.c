@@ -446,6 +446,56 @@ void orc_psd(const int64_t *med, const double *s_instr, int64_t n, double median
 }
 
 /* ------------------------------------------------------------------------------------ */
+/* Running-mean estimator, eq. (D1) PAPER.md:538 (the paper's production choice, :176, :552);  */
+/* DESIGN.md R8.  Same window as the median: W = 2h+1 bins centred on k, ends reflected.        */
+/* The exact object is the int64 window SUM; the mean enters the PSD as one division by W.      */
+/* ------------------------------------------------------------------------------------ */
+
+/* The definition written out: add up every window.  Outputs k in [k_begin, k_end). */
+int orc_running_sum_def(const int64_t *x, int64_t n, int32_t window,
+                        int64_t k_begin, int64_t k_end, int64_t *out)
+{
+    if (window < 1 || (window & 1) == 0) return -1;
+    int64_t h = window / 2;
+    if (n < h + 1) return -1;
+    for (int64_t k = k_begin; k < k_end; ++k) {
+        int64_t acc = 0;
+        for (int64_t j = -h; j <= h; ++j) acc += x[orc_reflect(k + j, n)];
+        out[k - k_begin] = acc;
+    }
+    return 0;
+}
+
+/* Same result, sliding: subtract the value that leaves, add the value that enters (integers:
+ * no rounding, so this is the definition regrouped).  Checked against the definition above. */
+int orc_running_sum(const int64_t *x, int64_t n, int32_t window, int64_t *out)
+{
+    if (window < 1 || (window & 1) == 0) return -1;
+    int64_t h = window / 2;
+    if (n < h + 1) return -1;
+    int64_t acc = 0;
+    for (int64_t j = -h; j <= h; ++j) acc += x[orc_reflect(j, n)];
+    out[0] = acc;
+    for (int64_t k = 1; k < n; ++k) {
+        acc -= x[orc_reflect(k - 1 - h, n)];
+        acc += x[orc_reflect(k + h, n)];
+        out[k] = acc;
+    }
+    return 0;
+}
+
+/* psd[k] = s_instr[k] + (sum[k] * 2^scale_log2) / W, eqs. (10), (D1) */
+void orc_psd_mean(const int64_t *sum, const double *s_instr, int64_t n, int32_t window,
+                  int32_t scale_log2, double *psd)
+{
+    for (int64_t k = 0; k < n; ++k) {
+        double e = ldexp((double)sum[k], scale_log2);
+        double m = e / (double)window;
+        psd[k] = s_instr[k] + m;
+    }
+}
+
+/* ------------------------------------------------------------------------------------ */
 /* Stage (iv) — SNR and selection, eqs. (11)-(12) in the power domain, R4.     */
 /* ------------------------------------------------------------------------------------ */
 
@@ -512,9 +562,26 @@ typedef struct {
 /* spectrum: in = total deposited spectrum, out = residual.  resolved: in/out flags.
  * n_new_per_iter (nullable, length max_iter) receives the newly-resolved count of each
  * iteration.  median / psd always correspond to the returned residual. */
-int orc_subtract_until_converged(const orc_grid *g, const double *A, const double *f,
+static int orc_estimate(int estimator, const int64_t *spectrum, const double *s_instr, int64_t n_bins,
+                        int32_t window, double median_norm, int32_t scale_log2, int64_t *stat, double *psd)
+{
+    int rc;
+    if (estimator == 1) {                      /* running mean, eq. (D1): stat = window sums */
+        rc = orc_running_sum(spectrum, n_bins, window, stat);
+        if (rc == 0) orc_psd_mean(stat, s_instr, n_bins, window, scale_log2, psd);
+    } else {                                   /* running median, eq. (D2)-(D3) */
+        rc = orc_running_median(spectrum, n_bins, window, stat);
+        if (rc == 0) orc_psd(stat, s_instr, n_bins, median_norm, scale_log2, psd);
+    }
+    return rc;
+}
+
+/* estimator: 0 = running median (eqs. D2-D3), 1 = running mean (eq. D1; `median` receives the
+ * window sums, median_norm is not used). */
+int orc_subtract_until_converged_est(const orc_grid *g, const double *A, const double *f,
                                  const double *fdot, int64_t n, const double *s_instr,
                                  int32_t window, double median_norm, double rho_th, int32_t max_iter,
+                                 int32_t estimator,
                                  int64_t *spectrum, int64_t *median, double *psd, uint8_t *resolved,
                                  orc_iter_result *res, int64_t *n_new_per_iter)
 {
@@ -523,9 +590,8 @@ int orc_subtract_until_converged(const orc_grid *g, const double *A, const doubl
     int rc = 0;
     int32_t it;
     for (it = 0; it < max_iter; ++it) {
-        rc = orc_running_median(spectrum, g->n_bins, window, median);
+        rc = orc_estimate(estimator, spectrum, s_instr, g->n_bins, window, median_norm, g->scale_log2, median, psd);
         if (rc) break;
-        orc_psd(median, s_instr, g->n_bins, median_norm, g->scale_log2, psd);
         int64_t near = 0;
         int64_t n_new = orc_snr_select(g, A, f, fdot, n, psd, rho_th, resolved, NULL, sel, &near);
         res->n_near_threshold += near;
@@ -536,9 +602,18 @@ int orc_subtract_until_converged(const orc_grid *g, const double *A, const doubl
     }
     if (rc == 0 && !res->converged) {          /* cap hit: PSD must match the returned residual */
         res->n_iter = max_iter;
-        rc = orc_running_median(spectrum, g->n_bins, window, median);
-        if (rc == 0) orc_psd(median, s_instr, g->n_bins, median_norm, g->scale_log2, psd);
+        rc = orc_estimate(estimator, spectrum, s_instr, g->n_bins, window, median_norm, g->scale_log2, median, psd);
     }
     free(sel);
     return rc;
+}
+
+int orc_subtract_until_converged(const orc_grid *g, const double *A, const double *f,
+                                 const double *fdot, int64_t n, const double *s_instr,
+                                 int32_t window, double median_norm, double rho_th, int32_t max_iter,
+                                 int64_t *spectrum, int64_t *median, double *psd, uint8_t *resolved,
+                                 orc_iter_result *res, int64_t *n_new_per_iter)
+{
+    return orc_subtract_until_converged_est(g, A, f, fdot, n, s_instr, window, median_norm, rho_th, max_iter, 0,
+                                            spectrum, median, psd, resolved, res, n_new_per_iter);
 }
