@@ -78,6 +78,8 @@ typedef struct gbfg_iter_params {
 
 #define GBFG_FLAG_NO_PRESELECT 1u   /* test every unresolved source every iteration (no R5 candidate cut) */
 #define GBFG_FLAG_NO_INCREMENTAL 2u /* recompute every median tile every iteration (no dirty-tile skipping) */
+#define GBFG_FLAG_ESTIMATOR_MEAN 4u /* running mean, eq. (D1), instead of the running median (R8):
+                                       dev_median receives the window sums, median_norm is not used */
 
 /* Per-catalog outcome of the loop (HOST). */
 typedef struct gbfg_iter_result {
@@ -134,6 +136,15 @@ int gbfg_deposit(const gbfg_grid *grid, const double *dev_A, const double *dev_f
  * dev_spectrum, dev_median_out: [n_cat][n_bins] int64 (must not alias). */
 int gbfg_running_median(const int64_t *dev_spectrum, int64_t n_bins, int32_t n_cat, int32_t window,
                         int64_t *dev_median_out, void *stream);
+
+/* Running-mean estimator of eq. (D1), PAPER.md:538 (the paper's production choice, :176, :552; R8):
+ * sum_out[c][k] = sum of x[c][k-h .. k+h], W = 2h+1 odd, ends reflected as for the median (the exact
+ * object is the int64 window sum; it must fit int64), and, when dev_psd != NULL,
+ * psd[c][k] = s_instr[k] + (sum_out[c][k] * 2^scale_log2) / W   (eq. 10).  dev_s_instr and dev_psd are both
+ * NULL or both given.  Same size limits as gbfg_running_median. */
+int gbfg_running_mean(const int64_t *dev_spectrum, int64_t n_bins, int32_t n_cat, int32_t window,
+                      int64_t *dev_sum_out, const double *dev_s_instr, int32_t scale_log2,
+                      double *dev_psd, void *stream);
 
 /* psd[c][k] = s_instr[k] + median_norm * (median[c][k] * 2^scale_log2): eqs. (10), (D2), (D3)
  * (PAPER.md:142-145, 542-549).  dev_s_instr: [n_bins], shared by the batch. */

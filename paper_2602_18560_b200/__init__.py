@@ -18,12 +18,14 @@ MAX_WINDOW = 4097
 MAX_ITER_TRACE = 64
 FLAG_NO_PRESELECT = 1
 FLAG_NO_INCREMENTAL = 2
+FLAG_ESTIMATOR_MEAN = 4
 
 EXPORTS = [
     "gbfg_version", "gbfg_strerror", "gbfg_last_cuda_error", "gbfg_grid_init", "gbfg_instrument_noise",
     "gbfg_sample_catalog", "gbfg_deposit", "gbfg_running_median", "gbfg_psd", "gbfg_snr_select",
     "gbfg_subtract_until_converged", "gbfg_simulate", "gbfg_simulate_host", "gbfg_workspace_bytes",
     "gbfg_kernel_launch_count", "gbfg_profile_enable", "gbfg_profile_read", "gbfg_release_cached",
+    "gbfg_running_mean",
 ]
 
 KERNEL_CLASSES = ["sample", "noise", "deposit", "scan", "median", "psd", "inv_blocks", "snr", "aux"]
@@ -88,6 +90,7 @@ def load():
     L.gbfg_deposit.argtypes = [gp, vp, vp, vp, op, i32, vp, vp, i32, vp, vp, vp, sz, vp]
     L.gbfg_running_median.argtypes = [vp, i64, i32, i32, vp, vp]
     L.gbfg_psd.argtypes = [vp, vp, i64, i32, dbl, i32, vp, vp]
+    L.gbfg_running_mean.argtypes = [vp, i64, i32, i32, vp, vp, i32, vp, vp]
     L.gbfg_snr_select.argtypes = [gp, vp, vp, vp, op, i32, vp, dbl, vp, vp, vp, vp, vp, vp, sz, vp]
     L.gbfg_subtract_until_converged.argtypes = [gp, vp, vp, vp, op, i32, vp, ip, vp, vp, vp, vp, rp, vp, sz, vp]
     L.gbfg_simulate.argtypes = [gp, pp, op, i32, u64, vp, ip, vp, vp, vp, vp, vp, vp, vp, vp, vp, rp, vp, sz, vp]
@@ -200,6 +203,12 @@ def deposit(grid: Grid, dev_A, dev_f, dev_fdot, offsets, dev_spectrum, workspace
 
 def running_median(dev_spectrum, n_bins: int, n_cat: int, window: int, dev_median_out, stream=None):
     _check(load().gbfg_running_median(_ptr(dev_spectrum), n_bins, n_cat, window, _ptr(dev_median_out), _stream(stream)))
+
+
+def running_mean(dev_spectrum, n_bins: int, n_cat: int, window: int, dev_sum_out, dev_s_instr=None,
+                 scale_log2: int = -140, dev_psd=None, stream=None):
+    _check(load().gbfg_running_mean(_ptr(dev_spectrum), n_bins, n_cat, window, _ptr(dev_sum_out), _ptr(dev_s_instr),
+                                    scale_log2, _ptr(dev_psd), _stream(stream)))
 
 
 def psd(dev_median, dev_s_instr, n_bins: int, n_cat: int, median_norm: float, scale_log2: int, dev_psd, stream=None):

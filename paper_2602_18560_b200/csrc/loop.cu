@@ -25,6 +25,8 @@ int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins,
 int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *med,
                   const double *s_instr, double *psd, double norm, int scale_log2,
                   const MedianPlan *plan, int4 *wide_items, int *wide_ctr, int *neg_flag, cudaStream_t st);
+int launch_mean(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *sum,
+                const double *s_instr, double *psd, int scale_log2, int *neg_flag, cudaStream_t st);
 int pfx_tiles_per_row(int64_t n_bins);
 size_t snr_pref_bytes(int64_t n_bins, int n_cat);
 size_t snr_tile_off_bytes(int64_t n_bins, int n_cat);
@@ -243,7 +245,8 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     if (!valid_grid(grid) || !params || params->struct_size != sizeof(gbfg_iter_params)) return GBFG_ERR_INVALID_ARG;
     if (!dev_s_instr || !dev_spectrum || !dev_median || !dev_psd || !dev_resolved || !host_results) return GBFG_ERR_INVALID_ARG;
     const int W = params->window;
-    if (W < 1 || (W & 1) == 0 || params->max_iter < 1 || !(params->rho_th >= 0.0) || !(params->median_norm > 0.0))
+    const bool use_mean = (params->flags & GBFG_FLAG_ESTIMATOR_MEAN) != 0;
+    if (W < 1 || (W & 1) == 0 || params->max_iter < 1 || !(params->rho_th >= 0.0) || (!use_mean && !(params->median_norm > 0.0)))
         return GBFG_ERR_INVALID_ARG;
     if (W > GBFG_MAX_WINDOW) return GBFG_ERR_UNSUPPORTED;
     if (grid->n_bins < W / 2 + 1) return GBFG_ERR_INVALID_ARG;
@@ -295,6 +298,7 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
                            params->rho_th, nullptr, w.sw, st);
     if (rc) return rc;
 
+    int64_t mean_passes = 0;
     bool done[GBFG_MAX_CAT];
     for (int c = 0; c < n_cat; ++c) {
         memset(&host_results[c], 0, sizeof(gbfg_iter_result));
@@ -304,10 +308,16 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     int n_done = 0;
     for (int it = 0; it < params->max_iter && n_done < n_cat; ++it) {
         // what the last subtraction made dirty (everything, the first time): work list + cum
-        rc = launch_plan(w.blk_stamp, it, it == 0 || !incremental, nb, n_cat, W, w.plan, w.counters, (int)n_iter_counters, med_outputs, st);
+        rc = launch_plan(w.blk_stamp, it, it == 0 || !incremental, nb, n_cat, W, w.plan, w.counters, (int)n_iter_counters,
+                         use_mean ? nullptr : med_outputs, st);
         if (rc) return rc;
-        rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
-                           grid->scale_log2, &w.plan, nullptr, nullptr, neg_flag, st);
+        if (use_mean) {      // eq. (D1): HBM bound, every bin every iteration
+            rc = launch_mean(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, grid->scale_log2, neg_flag, st);
+            ++mean_passes;
+        } else {
+            rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
+                               grid->scale_log2, &w.plan, nullptr, nullptr, neg_flag, st);
+        }
         if (rc) return rc;
         rc = launch_inv_prefix(dev_psd, nb, n_cat, w.sw, dirty, st);
         if (rc) return rc;
@@ -354,16 +364,21 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
         // cap hit: the PSD must match the returned residual (rows of converged catalogs are unchanged)
         for (int c = 0; c < n_cat; ++c)
             if (!done[c]) { host_results[c].n_iter = params->max_iter; host_results[c].converged = 0; }
-        rc = launch_plan(w.blk_stamp, params->max_iter, !incremental, nb, n_cat, W, w.plan, nullptr, 0, med_outputs, st);
-        if (rc) return rc;
-        rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
-                           grid->scale_log2, &w.plan, nullptr, nullptr, nullptr, st);
+        if (use_mean) {
+            rc = launch_mean(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, grid->scale_log2, nullptr, st);
+            ++mean_passes;
+        } else {
+            rc = launch_plan(w.blk_stamp, params->max_iter, !incremental, nb, n_cat, W, w.plan, nullptr, 0, med_outputs, st);
+            if (rc) return rc;
+            rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
+                               grid->scale_log2, &w.plan, nullptr, nullptr, nullptr, st);
+        }
         if (rc) return rc;
     }
     GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
     GBFG_CUDA(cudaStreamSynchronize(st));
     for (int c = 0; c < n_cat; ++c) {
-        host_results[c].n_median_outputs = host[i_med + c];
+        host_results[c].n_median_outputs = use_mean ? mean_passes * nb : host[i_med + c];
         host_results[c].n_snr_tests = host[i_tests + c];
     }
     return GBFG_OK;

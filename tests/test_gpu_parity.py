@@ -418,3 +418,64 @@ def test_loop_config4_full(gb, orc, torch):
         assert np.array_equal(bits(psd[c].cpu().numpy()), bits(ref["psd"]))
         assert np.array_equal(resolved[s].cpu().numpy(), ref["resolved"])
         assert (res[c].n_iter, res[c].converged, res[c].n_resolved) == (ref["n_iter"], ref["converged"], ref["n_resolved"])
+
+
+# ------------------------------------------------- running-mean estimator, eq. (D1) (R8)
+@pytest.mark.parametrize("kind", ["lognormal", "dupes", "zeros", "ramp", "const"])
+@pytest.mark.parametrize("n,window", [(20011, 1001), (30000, 2001), (9000, 4097), (7000, 3), (6193, 2001),
+                                      (1001, 2001), (40000, 1)])
+def test_running_mean_bit_exact(gb, orc, torch, kind, n, window):
+    x = wl.random_spectrum(n, seed=3 * n + window, kind=kind)
+    ref = orc.running_sum(x, window)
+    s_instr = 10.0 ** np.random.default_rng(n).uniform(-41, -33, n)
+    out = torch.empty(n, dtype=torch.int64, device="cuda")
+    psd = torch.empty(n, dtype=torch.float64, device="cuda")
+    gb.running_mean(dev(torch, x), n, 1, window, out, dev(torch, s_instr), -140, psd)
+    assert np.array_equal(out.cpu().numpy(), ref)
+    assert np.array_equal(bits(psd.cpu().numpy()), bits(orc.psd_from_sum(ref, s_instr, window, -140)))
+    out2 = torch.empty(n, dtype=torch.int64, device="cuda")
+    gb.running_mean(dev(torch, x), n, 1, window, out2)            # sums only
+    assert np.array_equal(out2.cpu().numpy(), ref)
+
+
+def test_running_mean_batch_rows_and_large_grid(gb, orc, torch):
+    n, window = 3_774_349, 2001                                   # the 4-yr grid, three rows
+    rows = np.stack([wl.random_spectrum(n, seed=70 + r, kind="lognormal") for r in range(3)])
+    out = torch.empty((3, n), dtype=torch.int64, device="cuda")
+    gb.running_mean(dev(torch, rows), n, 3, window, out)
+    got = out.cpu().numpy()
+    for r in range(3):
+        assert np.array_equal(got[r], orc.running_sum(rows[r], window))
+
+
+def _loop_case_mean(gb, orc, torch, w, flags=0):
+    ref = orc.simulate(w, estimator=1)
+    g = gpu_grid(gb, w)
+    n, nb = w.n_src_total, g.n_bins
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    total, spec, stat = (torch.empty(nb, dtype=torch.int64, device="cuda") for _ in range(3))
+    psd = torch.empty(nb, dtype=torch.float64, device="cuda")
+    resolved = torch.empty(n, dtype=torch.uint8, device="cuda")
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter, gb.FLAG_ESTIMATOR_MEAN | flags)
+    res = gb.simulate(g, w.pops, w.offsets(), w.seed, dev(torch, ref["s_instr"]), params, A, f, fd, total, spec, stat,
+                      psd, resolved, workspace(torch, gb, g, n))[0]
+    assert np.array_equal(total.cpu().numpy(), ref["total"])
+    assert np.array_equal(spec.cpu().numpy(), ref["residual"])
+    assert np.array_equal(stat.cpu().numpy(), ref["median"])              # window sums: bit-exact
+    assert np.array_equal(bits(psd.cpu().numpy()), bits(ref["psd"]))
+    assert np.array_equal(resolved.cpu().numpy(), ref["resolved"])
+    assert (res.n_iter, res.converged, res.n_resolved) == (ref["n_iter"], ref["converged"], ref["n_resolved"])
+    assert res.n_near_threshold == ref["n_near_threshold"]
+    return ref
+
+
+def test_loop_mean_estimator(gb, orc, torch):
+    _loop_case_mean(gb, orc, torch, wl.config(0))
+    ref = _loop_case_mean(gb, orc, torch, wl.dense_case("short"))
+    assert ref["n_iter"] >= 3
+    _loop_case_mean(gb, orc, torch, wl.dense_case("short"), flags=gb.FLAG_NO_PRESELECT)
+
+
+@pytest.mark.slow
+def test_loop_mean_estimator_config2_full(gb, orc, torch):
+    _loop_case_mean(gb, orc, torch, wl.config(2))
