@@ -154,6 +154,14 @@ static HostCallCache &host_call_cache()
     return c;
 }
 
+// event that marks the per-iteration readback (one per host thread)
+static cudaEvent_t readback_event()
+{
+    static thread_local cudaEvent_t ev = nullptr;
+    if (!ev && cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) { (void)cudaGetLastError(); ev = nullptr; }
+    return ev;
+}
+
 static DepositMarks plain_marks(const Workspace &w, int64_t n_bins, int stamp)
 {
     DepositMarks mk;
@@ -305,6 +313,9 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
         done[c] = false;
     }
     int64_t n_cand = n;                                 // upper bound until the first readback
+    int64_t last_total = 0;
+    cudaEvent_t ev_read = readback_event();
+    if (!ev_read) return set_cuda_error(cudaErrorMemoryAllocation, "cudaEventCreate");
     int n_done = 0;
     for (int it = 0; it < params->max_iter && n_done < n_cat; ++it) {
         // what the last subtraction made dirty (everything, the first time): work list + cum
@@ -325,11 +336,22 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
                              near, 1, preselect ? neg_flag : nullptr, true, w.sw, dirty, snr_tests, st);
         if (rc) return rc;
         GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
-        GBFG_CUDA(cudaStreamSynchronize(st));
+        GBFG_CUDA(cudaEventRecord(ev_read, st));
+        // The subtraction takes its list and count from device memory: it is queued before the host
+        // has seen the counters (a count of zero makes it a no-op), so the GPU does not idle while the
+        // host waits for the 8-byte scalar that decides whether the loop goes on.
+        DepositMarks mk = plain_marks(w, nb, it + 1);
+        mk.blk_stamp = w.blk_stamp; mk.n_dblk = w.plan.n_dblk; mk.dblk_log2 = w.plan.dblk_log2; mk.med_h = W / 2;
+        const int64_t sub_bound = it == 0 ? n : 2 * last_total + 4096;     // grid sizing only
+        rc = launch_deposit(g, ct, dev_A, dev_f, dev_fdot, w.sel_idx, sel_count, sub_bound, -1, dev_spectrum, nullptr,
+                            w.diff, w.tile_sums, w.wide_flag, mk, st);
+        if (rc) return rc;
+        GBFG_CUDA(cudaEventSynchronize(ev_read));
         if (preselect && host[i_flags] != 0) {
             // A negative median: S_n >= S_instr no longer holds, so the pre-selection is not valid
             // (the caller's spectrum does not contain the catalog).  Every unresolved source becomes
-            // a candidate, and this iteration's test, which did nothing, is run on them.
+            // a candidate, and this iteration's test, which did nothing (as did the subtraction queued
+            // behind it), is run on them.
             preselect = false;
             GBFG_CUDA(cudaMemsetAsync(w.sw.cand_count, 0, sizeof(int64_t) * (size_t)(1 + n_cat), st));
             rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, nullptr, params->rho_th, nullptr, w.sw, st);
@@ -338,11 +360,15 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
                                  near, 1, nullptr, true, w.sw, all_dirty, snr_tests, st);
             if (rc) return rc;
             GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
+            rc = launch_deposit(g, ct, dev_A, dev_f, dev_fdot, w.sel_idx, sel_count, n, -1, dev_spectrum, nullptr,
+                                w.diff, w.tile_sums, w.wide_flag, mk, st);
+            if (rc) return rc;
             GBFG_CUDA(cudaStreamSynchronize(st));
             for (int c = 0; c < n_cat; ++c) host_results[c].n_candidates = 0;
         }
         n_cand = host[i_cand];
         const int64_t total = host[0];
+        last_total = total;
         for (int c = 0; c < n_cat; ++c) {
             gbfg_iter_result &r = host_results[c];
             if (r.n_candidates == 0) r.n_candidates = n_cat == 1 ? host[i_cand] : host[i_cand + 1 + c];
@@ -354,11 +380,6 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
             if (n_new == 0) { done[c] = true; ++n_done; r.n_iter = it + 1; r.converged = 1; }
         }
         if (total == 0) break;
-        DepositMarks mk = plain_marks(w, nb, it + 1);
-        mk.blk_stamp = w.blk_stamp; mk.n_dblk = w.plan.n_dblk; mk.dblk_log2 = w.plan.dblk_log2; mk.med_h = W / 2;
-        rc = launch_deposit(g, ct, dev_A, dev_f, dev_fdot, w.sel_idx, sel_count, total, -1, dev_spectrum, nullptr,
-                            w.diff, w.tile_sums, w.wide_flag, mk, st);
-        if (rc) return rc;
     }
     if (n_done < n_cat) {
         // cap hit: the PSD must match the returned residual (rows of converged catalogs are unchanged)
