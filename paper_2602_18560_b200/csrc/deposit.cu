@@ -6,9 +6,10 @@
 //   * wide sources use the range-update form: +q at k0 and -q at k0+w_eff in a difference array,
 //     followed by one inclusive scan that is added into the spectrum (2 updates per source instead
 //     of w; chirps reach 7e4 bins at 4 yr).  sum_k spectrum[k] is identical bit for bit.
-// The scan is the three-phase tile scan (tile sums -> scan of tile sums -> rescan + add); the
-// difference array is zeroed again on the way so the workspace is reusable.  Scan tiles that hold
-// no update and start from a zero running value are skipped (stamps written by the deposit kernel).
+// The scan is a two-launch tile scan (sums of the tiles that hold updates -> every tile adds up the
+// sums before it, rescans and adds); the difference array is zeroed again on the way so the
+// workspace is reusable.  Scan tiles that hold no update and start from a zero running value are
+// skipped (stamps written by the deposit kernel).
 // A subtraction also stamps the dirty blocks (gbfg_common.cuh) whose running-median outputs see a
 // changed bin, so that stages (iii) and (iv) redo only those (DepositMarks).
 #include "gbfg_common.cuh"
@@ -67,27 +68,25 @@ deposit_kernel(GridDev g, CatTable ct, const double *__restrict__ A, const doubl
     }
 }
 
-// phase 1: tile sums of the difference array, grid = (tiles_per_row, n_cat); the last CTA of a row
-// to finish (ticket) turns the row's tile sums into exclusive offsets (phase 2).
+// phase 1: sums of the tiles of the difference array that hold an update (the others are not touched:
+// their sum is zero by definition, whatever tile_sums holds from an earlier call).
+// grid = (tiles_per_row, n_cat)
 __global__ void __launch_bounds__(SCAN_THREADS)
 scan_tile_sums_kernel(const int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
                       int64_t *__restrict__ tile_sums, const int *__restrict__ wide_flag,
-                      const int *__restrict__ scan_stamp, int stamp, unsigned *__restrict__ ticket)
+                      const int *__restrict__ scan_stamp, int stamp)
 {
     if (*wide_flag != stamp) return;
-    __shared__ int64_t warp_sum[SCAN_THREADS / 32];
-    __shared__ int64_t carry_s;
-    __shared__ int is_last;
     const int64_t ti = (int64_t)blockIdx.y * tiles_per_row + blockIdx.x;
+    if (scan_stamp[ti] != stamp) return;
+    __shared__ int64_t warp_sum[SCAN_THREADS / 32];
+    const int64_t row = (int64_t)blockIdx.y * n_bins;
+    const int64_t base = (int64_t)blockIdx.x * SCAN_TILE;
     int64_t acc = 0;
-    if (scan_stamp[ti] == stamp) {                      // untouched tile: sum 0
-        const int64_t row = (int64_t)blockIdx.y * n_bins;
-        const int64_t base = (int64_t)blockIdx.x * SCAN_TILE;
 #pragma unroll
-        for (int j = 0; j < SCAN_ITEMS; ++j) {
-            int64_t k = base + (int64_t)j * SCAN_THREADS + threadIdx.x;
-            if (k < n_bins) acc += diff[row + k];
-        }
+    for (int j = 0; j < SCAN_ITEMS; ++j) {
+        int64_t k = base + (int64_t)j * SCAN_THREADS + threadIdx.x;
+        if (k < n_bins) acc += diff[row + k];
     }
     for (int o = 16; o; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
     if ((threadIdx.x & 31) == 0) warp_sum[threadIdx.x >> 5] = acc;
@@ -96,48 +95,37 @@ scan_tile_sums_kernel(const int64_t *__restrict__ diff, int64_t n_bins, int tile
         int64_t t = 0;
         for (int w = 0; w < SCAN_THREADS / 32; ++w) t += warp_sum[w];
         tile_sums[ti] = t;
-        __threadfence();
-        is_last = atomicAdd(ticket + blockIdx.y, 1u) == (unsigned)tiles_per_row - 1u;
-        carry_s = 0;
-    }
-    __syncthreads();
-    if (!is_last) return;
-    __threadfence();
-    if (threadIdx.x == 0) ticket[blockIdx.y] = 0u;      // ready for the next call
-    // phase 2: exclusive scan of the row's tile sums
-    volatile int64_t *rowp = tile_sums + (int64_t)blockIdx.y * tiles_per_row;
-    for (int base = 0; base < tiles_per_row; base += SCAN_THREADS) {
-        const int idx = base + threadIdx.x;
-        const int64_t v = idx < tiles_per_row ? rowp[idx] : 0;
-        int64_t incl = v;
-        for (int o = 1; o < 32; o <<= 1) {
-            int64_t up = __shfl_up_sync(0xffffffffu, incl, o);
-            if ((threadIdx.x & 31) >= o) incl += up;
-        }
-        __syncthreads();
-        if ((threadIdx.x & 31) == 31) warp_sum[threadIdx.x >> 5] = incl;
-        __syncthreads();
-        int64_t before = carry_s;
-        for (int w = 0; w < (threadIdx.x >> 5); ++w) before += warp_sum[w];
-        if (idx < tiles_per_row) rowp[idx] = before + incl - v;
-        __syncthreads();
-        if (threadIdx.x == SCAN_THREADS - 1) carry_s = before + incl;
-        __syncthreads();
     }
 }
 
-// phase 3: rescan each tile, add the running value into the spectrum, zero the difference array
+// phase 2: every CTA adds up the sums of the stamped tiles before its own (a few thousand L2 reads:
+// cheaper than a separate scan launch or a ticket per tile), rescans its tile, adds the running value
+// into the spectrum and zeroes the difference array.
 __global__ void __launch_bounds__(SCAN_THREADS)
 scan_add_kernel(int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
-                const int64_t *__restrict__ tile_offsets, int64_t *__restrict__ spectrum,
+                const int64_t *__restrict__ tile_sums, int64_t *__restrict__ spectrum,
                 const int *__restrict__ wide_flag, const int *__restrict__ scan_stamp, int stamp)
 {
     if (*wide_flag != stamp) return;
     __shared__ int64_t warp_tot[SCAN_THREADS / 32];
-    {   // nothing to add in a tile without updates that starts from a zero running value
-        const int64_t ti = (int64_t)blockIdx.y * tiles_per_row + blockIdx.x;
-        if (scan_stamp[ti] != stamp && tile_offsets[ti] == 0) return;
+    __shared__ int64_t tile_offset;
+    const int64_t t0 = (int64_t)blockIdx.y * tiles_per_row;
+    {
+        int64_t acc = 0;
+        for (int t = threadIdx.x; t < (int)blockIdx.x; t += SCAN_THREADS)
+            if (scan_stamp[t0 + t] == stamp) acc += tile_sums[t0 + t];
+        for (int o = 16; o; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
+        if ((threadIdx.x & 31) == 0) warp_tot[threadIdx.x >> 5] = acc;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int64_t s = 0;
+            for (int w = 0; w < SCAN_THREADS / 32; ++w) s += warp_tot[w];
+            tile_offset = s;
+        }
+        __syncthreads();
     }
+    // nothing to add in a tile without updates that starts from a zero running value
+    if (scan_stamp[t0 + blockIdx.x] != stamp && tile_offset == 0) return;
     const int64_t row = (int64_t)blockIdx.y * n_bins;
     const int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
     int64_t v[SCAN_ITEMS];
@@ -153,9 +141,10 @@ scan_add_kernel(int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
         int64_t up = __shfl_up_sync(0xffffffffu, incl, o);
         if ((threadIdx.x & 31) >= o) incl += up;
     }
+    __syncthreads();
     if ((threadIdx.x & 31) == 31) warp_tot[threadIdx.x >> 5] = incl;
     __syncthreads();
-    int64_t run = tile_offsets[(int64_t)blockIdx.y * tiles_per_row + blockIdx.x] + incl - tsum;
+    int64_t run = tile_offset + incl - tsum;
     for (int w = 0; w < (threadIdx.x >> 5); ++w) run += warp_tot[w];
 #pragma unroll
     for (int j = 0; j < SCAN_ITEMS; ++j) {
@@ -170,9 +159,8 @@ scan_add_kernel(int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
 
 // ---------------------------------------------------------------------------------------------
 // internal entry used by the stage call and by the loop.  diff: [n_cat*n_bins] zero on entry and
-// on exit; tile_sums: [n_cat*tiles_per_row]; wide_flag: one int followed by n_cat ticket words: the
-// flag must differ from mk.stamp on entry (it is left equal to it when a wide source was seen), the
-// tickets are zero on entry and on exit.
+// on exit; tile_sums: [n_cat*tiles_per_row]; wide_flag: one int that must differ from mk.stamp on
+// entry (it is left equal to it when a wide source was seen).
 // mk.scan_stamp: [n_cat*tiles_per_row] ints, none equal to mk.stamp on entry.
 // ---------------------------------------------------------------------------------------------
 int scan_tiles_per_row(int64_t n_bins) { return (int)((n_bins + SCAN_TILE - 1) / SCAN_TILE); }
@@ -195,8 +183,7 @@ int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const 
     const int tiles = scan_tiles_per_row(g.n_bins);
     dim3 grid(tiles, ct.n_cat);
     LaunchTimer lt_scan(K_SCAN, st);     // the two scan kernels, as one
-    scan_tile_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, wide_flag, mk.scan_stamp, mk.stamp,
-                                                         (unsigned *)(wide_flag + 1));
+    scan_tile_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, wide_flag, mk.scan_stamp, mk.stamp);
     GBFG_LAUNCH_CHECK("scan_tile_sums_kernel");
     scan_add_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, spectrum, wide_flag, mk.scan_stamp, mk.stamp);
     GBFG_LAUNCH_CHECK("scan_add_kernel");
