@@ -168,9 +168,12 @@ int scan_tiles_per_row(int64_t n_bins) { return (int)((n_bins + SCAN_TILE - 1) /
 int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
                    const int64_t *sel_idx, const int64_t *sel_count, int64_t n_launch, int32_t sign,
                    int64_t *spectrum, int64_t *err_count, int64_t *diff, int64_t *tile_sums, int *wide_flag,
-                   const DepositMarks &mk, cudaStream_t st)
+                   const DepositMarks &mk, cudaStream_t st, cudaEvent_t after_deposit)
 {
-    if (n_launch <= 0) return GBFG_OK;
+    if (n_launch <= 0) {
+        if (after_deposit) GBFG_CUDA(cudaEventRecord(after_deposit, st));
+        return GBFG_OK;
+    }
     int64_t blocks = (n_launch + 255) / 256;
     int64_t cap = (int64_t)sm_count() * 16;
     if (blocks > cap) blocks = cap;
@@ -180,6 +183,7 @@ int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const 
                                                     spectrum, diff, err_count, wide_flag, mk);
     }
     GBFG_LAUNCH_CHECK("deposit_kernel");
+    if (after_deposit) GBFG_CUDA(cudaEventRecord(after_deposit, st));   // the stamps are written: the plan may start
     const int tiles = scan_tiles_per_row(g.n_bins);
     dim3 grid(tiles, ct.n_cat);
     LaunchTimer lt_scan(K_SCAN, st);     // the two scan kernels, as one

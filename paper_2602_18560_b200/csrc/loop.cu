@@ -18,7 +18,7 @@ int scan_tiles_per_row(int64_t n_bins);
 int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
                    const int64_t *sel_idx, const int64_t *sel_count, int64_t n_launch, int32_t sign,
                    int64_t *spectrum, int64_t *err_count, int64_t *diff, int64_t *tile_sums, int *wide_flag,
-                   const DepositMarks &mk, cudaStream_t st);
+                   const DepositMarks &mk, cudaStream_t st, cudaEvent_t after_deposit = nullptr);
 int median_max_items(int64_t n_bins);
 int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins, int n_cat, int window,
                 const MedianPlan &pl, int64_t *zero_ptr, int zero_n, int64_t *out_count, cudaStream_t st);
@@ -160,6 +160,23 @@ static cudaEvent_t readback_event()
     static thread_local cudaEvent_t ev = nullptr;
     if (!ev && cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) { (void)cudaGetLastError(); ev = nullptr; }
     return ev;
+}
+
+// side stream on which the plan of the next pass runs next to the scan of the subtraction (one per host thread)
+struct SideStream { cudaStream_t s; cudaEvent_t ev_dep, ev_plan; };
+static SideStream *side_stream()
+{
+    static thread_local SideStream ss = {nullptr, nullptr, nullptr};
+    if (!ss.s) {
+        if (cudaStreamCreateWithFlags(&ss.s, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&ss.ev_dep, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&ss.ev_plan, cudaEventDisableTiming) != cudaSuccess) {
+            (void)cudaGetLastError();
+            ss.s = nullptr;
+            return nullptr;
+        }
+    }
+    return &ss;
 }
 
 static DepositMarks plain_marks(const Workspace &w, int64_t n_bins, int stamp)
@@ -314,14 +331,22 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     }
     int64_t n_cand = n;                                 // upper bound until the first readback
     int64_t last_total = 0;
+    bool plan_queued = false;
+    SideStream *side = side_stream();
+    if (!side) return set_cuda_error(cudaErrorMemoryAllocation, "side stream");
     cudaEvent_t ev_read = readback_event();
     if (!ev_read) return set_cuda_error(cudaErrorMemoryAllocation, "cudaEventCreate");
     int n_done = 0;
     for (int it = 0; it < params->max_iter && n_done < n_cat; ++it) {
         // what the last subtraction made dirty (everything, the first time): work list + cum
-        rc = launch_plan(w.blk_stamp, it, it == 0 || !incremental, nb, n_cat, W, w.plan, w.counters, (int)n_iter_counters,
-                         use_mean ? nullptr : med_outputs, st);
-        if (rc) return rc;
+        if (plan_queued) {
+            GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_plan, 0));
+        } else {
+            rc = launch_plan(w.blk_stamp, it, it == 0 || !incremental, nb, n_cat, W, w.plan, w.counters, (int)n_iter_counters,
+                             use_mean ? nullptr : med_outputs, st);
+            if (rc) return rc;
+        }
+        plan_queued = false;
         if (use_mean) {      // eq. (D1): HBM bound, every bin every iteration
             rc = launch_mean(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, grid->scale_log2, neg_flag, st);
             ++mean_passes;
@@ -344,10 +369,23 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
         mk.blk_stamp = w.blk_stamp; mk.n_dblk = w.plan.n_dblk; mk.dblk_log2 = w.plan.dblk_log2; mk.med_h = W / 2;
         const int64_t sub_bound = it == 0 ? n : 2 * last_total + 4096;     // grid sizing only
         rc = launch_deposit(g, ct, dev_A, dev_f, dev_fdot, w.sel_idx, sel_count, sub_bound, -1, dev_spectrum, nullptr,
-                            w.diff, w.tile_sums, w.wide_flag, mk, st);
+                            w.diff, w.tile_sums, w.wide_flag, mk, st, side->ev_dep);
         if (rc) return rc;
+        // ... and the plan of the next pass runs on the side stream next to the scan of this subtraction: it
+        // reads the stamps the deposit kernel wrote and clears the counters the copy above has taken.  After
+        // the last iteration it is the plan of the closing median pass.
+        if (!(use_mean && it + 1 == params->max_iter)) {
+            const bool closing = it + 1 == params->max_iter;
+            GBFG_CUDA(cudaStreamWaitEvent(side->s, side->ev_dep, 0));
+            rc = launch_plan(w.blk_stamp, it + 1, !incremental, nb, n_cat, W, w.plan, closing ? nullptr : w.counters,
+                             closing ? 0 : (int)n_iter_counters, use_mean ? nullptr : med_outputs, side->s);
+            if (rc) return rc;
+            GBFG_CUDA(cudaEventRecord(side->ev_plan, side->s));
+            plan_queued = true;
+        }
         GBFG_CUDA(cudaEventSynchronize(ev_read));
         if (preselect && host[i_flags] != 0) {
+            if (plan_queued) { GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_plan, 0)); plan_queued = false; }   // it saw no stamps: made again
             // A negative median: S_n >= S_instr no longer holds, so the pre-selection is not valid
             // (the caller's spectrum does not contain the catalog).  Every unresolved source becomes
             // a candidate, and this iteration's test, which did nothing (as did the subtraction queued
@@ -389,13 +427,19 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
             rc = launch_mean(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, grid->scale_log2, nullptr, st);
             ++mean_passes;
         } else {
-            rc = launch_plan(w.blk_stamp, params->max_iter, !incremental, nb, n_cat, W, w.plan, nullptr, 0, med_outputs, st);
-            if (rc) return rc;
+            if (plan_queued) {
+                GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_plan, 0));
+            } else {
+                rc = launch_plan(w.blk_stamp, params->max_iter, !incremental, nb, n_cat, W, w.plan, nullptr, 0, med_outputs, st);
+                if (rc) return rc;
+            }
+            plan_queued = false;
             rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
                                grid->scale_log2, &w.plan, nullptr, nullptr, nullptr, st);
         }
         if (rc) return rc;
     }
+    if (plan_queued) GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_plan, 0));     // nothing of this call runs after it returns
     GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
     GBFG_CUDA(cudaStreamSynchronize(st));
     for (int c = 0; c < n_cat; ++c) {
