@@ -241,8 +241,9 @@ running_median_tile_kernel(MedianArgs a)
         __syncthreads();
     }
 
-    // ---- inverse permutation and the count table
-    for (int e = tid; e < MED_NRB * MED_TROW / 2; e += THREADS) aux32[e] = 0u;
+    // ---- inverse permutation and the count table (only the rank buckets and position blocks the tile has)
+    const int nrb = LTe / MED_RB, npb = LTe / MED_PB;     // LTe is a multiple of 256
+    for (int e = tid; e < nrb * MED_TROW / 2; e += THREADS) aux32[e] = 0u;
     __syncthreads();
     for (int r = tid; r < LTe; r += THREADS) {
         int p = spos[r];
@@ -254,13 +255,13 @@ running_median_tile_kernel(MedianArgs a)
     // prefix along the position blocks: tab[rb][pb] = #{r in bucket rb : pos < pb*PB}
     {
         constexpr int PER = (MED_NPB + 1 + 31) / 32;     // 9 entries per lane
-        for (int rb = warp; rb < MED_NRB; rb += WARPS) {
+        for (int rb = warp; rb < nrb; rb += WARPS) {
             uint16_t *rowp = tab + rb * MED_TROW;
             int v[PER], s = 0;
 #pragma unroll
             for (int q = 0; q < PER; ++q) {
                 int idx = lane * PER + q;
-                v[q] = idx <= MED_NPB ? rowp[idx] : 0;
+                v[q] = idx <= npb ? rowp[idx] : 0;
                 s += v[q];
             }
             int incl = s;
@@ -273,15 +274,15 @@ running_median_tile_kernel(MedianArgs a)
             for (int q = 0; q < PER; ++q) {
                 int idx = lane * PER + q;
                 run += v[q];
-                if (idx <= MED_NPB) rowp[idx] = (uint16_t)run;
+                if (idx <= npb) rowp[idx] = (uint16_t)run;
             }
         }
     }
     __syncthreads();
     // exclusive prefix along the rank buckets: tab[rb][pb] = #{r < rb*RB : pos < pb*PB}
-    for (int pb = tid; pb <= MED_NPB; pb += THREADS) {
+    for (int pb = tid; pb <= npb; pb += THREADS) {
         int run = 0;
-        for (int rb = 0; rb < MED_NRB; ++rb) {
+        for (int rb = 0; rb < nrb; ++rb) {
             int v = tab[rb * MED_TROW + pb];
             tab[rb * MED_TROW + pb] = (uint16_t)run;
             run += v;
@@ -321,8 +322,9 @@ running_median_tile_kernel(MedianArgs a)
             if (na > 0) {
                 const int t = (h < na - 1) ? h : na - 1;
                 // largest bucket lo with #{rank < 128 lo, position in the aligned part} <= t
-                const int c0 = (int)tab[lane * MED_TROW + b1] - (int)tab[lane * MED_TROW + b0];
-                const int c1 = (int)tab[(lane + 32) * MED_TROW + b1] - (int)tab[(lane + 32) * MED_TROW + b0];
+                // (a bucket past the tile's last one counts everything: never chosen)
+                const int c0 = lane < nrb ? (int)tab[lane * MED_TROW + b1] - (int)tab[lane * MED_TROW + b0] : 0x7fffffff;
+                const int c1 = lane + 32 < nrb ? (int)tab[(lane + 32) * MED_TROW + b1] - (int)tab[(lane + 32) * MED_TROW + b0] : 0x7fffffff;
                 const unsigned m0 = __ballot_sync(FULL, c0 <= t), m1 = __ballot_sync(FULL, c1 <= t);
                 const int lo = m1 ? 63 - __clz(m1) : 31 - __clz(m0);
                 const int cl = lo < 32 ? __shfl_sync(FULL, c0, lo & 31) : __shfl_sync(FULL, c1, lo & 31);
