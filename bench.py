@@ -144,7 +144,7 @@ def algorithmic_bytes(w: wl.Workload, n_bins: int, res, prof) -> dict:
     n_scan = prof["scan"][0]
     return {
         "sample": 24 * n,                                   # 24 B written per source
-        "deposit": 24 * n + 32 * n_sub,                     # catalog read once; 8 B index + 24 B per subtracted source
+        "deposit": 24 * n,                                  # catalog read once (the loop subtracts inside the SNR test)
         "scan": 16 * n_bins * n_scan,                       # spectrum read + written per range-update pass (upper bound: untouched tiles are skipped)
         "median": 32 * int(res.n_median_outputs),           # per output: spectrum in, median out, s_instr in, PSD out
         "inv_blocks": 8 * int(res.n_median_outputs) + 8 * n_bins,   # PSD read where it changed (+ s_instr once)

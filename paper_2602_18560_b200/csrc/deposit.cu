@@ -16,10 +16,11 @@
 
 namespace gbfg {
 
-constexpr int NARROW = 4;            // <= NARROW bins: direct atomics
+constexpr int NARROW = DEP_NARROW;   // <= NARROW bins: direct atomics
 constexpr int SCAN_THREADS = 256;
 constexpr int SCAN_ITEMS = 8;        // int64 per thread
 constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
+static_assert(SCAN_TILE == DEP_SCAN_TILE, "snr.cu stamps scan tiles of this size");
 
 // One thread per addressed source.  `wide_flag` is set if any source used the difference array.
 __global__ void __launch_bounds__(256)
@@ -165,6 +166,9 @@ scan_add_kernel(int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
 // ---------------------------------------------------------------------------------------------
 int scan_tiles_per_row(int64_t n_bins) { return (int)((n_bins + SCAN_TILE - 1) / SCAN_TILE); }
 
+int launch_scan(int64_t n_bins, int n_cat, int64_t *spectrum, int64_t *diff, int64_t *tile_sums, int *wide_flag,
+                const DepositMarks &mk, cudaStream_t st);
+
 int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
                    const int64_t *sel_idx, const int64_t *sel_count, int64_t n_launch, int32_t sign,
                    int64_t *spectrum, int64_t *err_count, int64_t *diff, int64_t *tile_sums, int *wide_flag,
@@ -184,12 +188,19 @@ int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const 
     }
     GBFG_LAUNCH_CHECK("deposit_kernel");
     if (after_deposit) GBFG_CUDA(cudaEventRecord(after_deposit, st));   // the stamps are written: the plan may start
-    const int tiles = scan_tiles_per_row(g.n_bins);
-    dim3 grid(tiles, ct.n_cat);
+    return launch_scan(g.n_bins, ct.n_cat, spectrum, diff, tile_sums, wide_flag, mk, st);
+}
+
+// the scan of the difference array into the spectrum (no-op unless wide_flag holds mk.stamp)
+int launch_scan(int64_t n_bins, int n_cat, int64_t *spectrum, int64_t *diff, int64_t *tile_sums, int *wide_flag,
+                const DepositMarks &mk, cudaStream_t st)
+{
+    const int tiles = scan_tiles_per_row(n_bins);
+    dim3 grid(tiles, n_cat);
     LaunchTimer lt_scan(K_SCAN, st);     // the two scan kernels, as one
-    scan_tile_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, wide_flag, mk.scan_stamp, mk.stamp);
+    scan_tile_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, n_bins, tiles, tile_sums, wide_flag, mk.scan_stamp, mk.stamp);
     GBFG_LAUNCH_CHECK("scan_tile_sums_kernel");
-    scan_add_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, g.n_bins, tiles, tile_sums, spectrum, wide_flag, mk.scan_stamp, mk.stamp);
+    scan_add_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, n_bins, tiles, tile_sums, spectrum, wide_flag, mk.scan_stamp, mk.stamp);
     GBFG_LAUNCH_CHECK("scan_add_kernel");
     return GBFG_OK;
 }

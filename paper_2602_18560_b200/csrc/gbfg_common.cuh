@@ -107,6 +107,20 @@ struct DepositMarks {
     int stamp;          // value written
 };
 
+// Range-update deposit (deposit.cu): sources of at most DEP_NARROW bins add q with L2 atomics, wider
+// ones write +q / -q into the difference array, scanned in tiles of DEP_SCAN_TILE bins.
+constexpr int DEP_NARROW = 4;
+constexpr int DEP_SCAN_TILE = 2048;
+
+// What stage (iv) needs to subtract the sources it selects on the spot (snr.cu; spectrum NULL: it only selects)
+struct SubtractView {
+    int64_t *spectrum;      // [n_cat][n_bins]
+    int64_t *diff;          // [n_cat][n_bins]
+    int *wide_flag;
+    DepositMarks mk;
+    int scale_log2;
+};
+
 // Work list of the running median (median.cu): items[i] = (row, first output, outputs, 0).
 struct MedianPlan {
     int4 *items;

@@ -19,6 +19,8 @@ int launch_deposit(const GridDev &g, const CatTable &ct, const double *A, const 
                    const int64_t *sel_idx, const int64_t *sel_count, int64_t n_launch, int32_t sign,
                    int64_t *spectrum, int64_t *err_count, int64_t *diff, int64_t *tile_sums, int *wide_flag,
                    const DepositMarks &mk, cudaStream_t st, cudaEvent_t after_deposit = nullptr);
+int launch_scan(int64_t n_bins, int n_cat, int64_t *spectrum, int64_t *diff, int64_t *tile_sums, int *wide_flag,
+                const DepositMarks &mk, cudaStream_t st);
 int median_max_items(int64_t n_bins);
 int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins, int n_cat, int window,
                 const MedianPlan &pl, int64_t *zero_ptr, int zero_n, int64_t *out_count, cudaStream_t st);
@@ -39,7 +41,7 @@ int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, con
 int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th, uint8_t *resolved, double *rho2_out,
                     int64_t n_launch, int64_t *sel_idx, int64_t *sel_count, int64_t *near_count, int near_per_cat,
                     const int *abort_flag, bool use_prefix, const SnrWork &sw, const DirtyView &dv, int64_t *test_count,
-                    cudaStream_t st);
+                    const SubtractView *sub, cudaStream_t st);
 
 // ------------------------------------------------------------------------------- workspace
 constexpr int WS_COUNTERS = 6 * GBFG_MAX_CAT + 16;
@@ -163,13 +165,12 @@ static cudaEvent_t readback_event()
 }
 
 // side stream on which the plan of the next pass runs next to the scan of the subtraction (one per host thread)
-struct SideStream { cudaStream_t s; cudaEvent_t ev_dep, ev_plan; };
+struct SideStream { cudaStream_t s; cudaEvent_t ev_plan; };
 static SideStream *side_stream()
 {
-    static thread_local SideStream ss = {nullptr, nullptr, nullptr};
+    static thread_local SideStream ss = {nullptr, nullptr};
     if (!ss.s) {
         if (cudaStreamCreateWithFlags(&ss.s, cudaStreamNonBlocking) != cudaSuccess ||
-            cudaEventCreateWithFlags(&ss.ev_dep, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&ss.ev_plan, cudaEventDisableTiming) != cudaSuccess) {
             (void)cudaGetLastError();
             ss.s = nullptr;
@@ -257,7 +258,7 @@ extern "C" int gbfg_snr_select(const gbfg_grid *grid, const double *dev_A, const
     rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, nullptr, rho_th, dev_rho2_out, w.sw, st);
     if (rc) return rc;
     return launch_snr_cand(grid->n_bins, n_cat, dev_psd, rho_th, dev_resolved, dev_rho2_out, n, dev_sel_idx,
-                           dev_sel_count, dev_near_count, 0, nullptr, true, w.sw, all_dirty, nullptr, st);
+                           dev_sel_count, dev_near_count, 0, nullptr, true, w.sw, all_dirty, nullptr, nullptr, st);
 }
 
 extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double *dev_A, const double *dev_f,
@@ -330,7 +331,6 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
         done[c] = false;
     }
     int64_t n_cand = n;                                 // upper bound until the first readback
-    int64_t last_total = 0;
     bool plan_queued = false;
     SideStream *side = side_stream();
     if (!side) return set_cuda_error(cudaErrorMemoryAllocation, "side stream");
@@ -357,26 +357,26 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
         if (rc) return rc;
         rc = launch_inv_prefix(dev_psd, nb, n_cat, w.sw, dirty, st);
         if (rc) return rc;
+        // The test subtracts what it selects on the spot (stage v, eq. D4) and stamps the blocks that become dirty.
+        DepositMarks mk = plain_marks(w, nb, it + 1);
+        mk.blk_stamp = w.blk_stamp; mk.n_dblk = w.plan.n_dblk; mk.dblk_log2 = w.plan.dblk_log2; mk.med_h = W / 2;
+        const SubtractView sub = {dev_spectrum, w.diff, w.wide_flag, mk, grid->scale_log2};
         rc = launch_snr_cand(nb, n_cat, dev_psd, params->rho_th, dev_resolved, nullptr, n_cand, w.sel_idx, sel_count,
-                             near, 1, preselect ? neg_flag : nullptr, true, w.sw, dirty, snr_tests, st);
+                             near, 1, preselect ? neg_flag : nullptr, true, w.sw, dirty, snr_tests, &sub, st);
         if (rc) return rc;
         GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
         GBFG_CUDA(cudaEventRecord(ev_read, st));
-        // The subtraction takes its list and count from device memory: it is queued before the host
-        // has seen the counters (a count of zero makes it a no-op), so the GPU does not idle while the
-        // host waits for the 8-byte scalar that decides whether the loop goes on.
-        DepositMarks mk = plain_marks(w, nb, it + 1);
-        mk.blk_stamp = w.blk_stamp; mk.n_dblk = w.plan.n_dblk; mk.dblk_log2 = w.plan.dblk_log2; mk.med_h = W / 2;
-        const int64_t sub_bound = it == 0 ? n : 2 * last_total + 4096;     // grid sizing only
-        rc = launch_deposit(g, ct, dev_A, dev_f, dev_fdot, w.sel_idx, sel_count, sub_bound, -1, dev_spectrum, nullptr,
-                            w.diff, w.tile_sums, w.wide_flag, mk, st, side->ev_dep);
+        // Everything below is queued before the host has seen the counters (a pass that selected nothing makes
+        // it a no-op), so the GPU does not idle while the host waits for the scalar that decides whether the
+        // loop goes on: the scan of the wide sources' range updates into the spectrum ...
+        rc = launch_scan(nb, n_cat, dev_spectrum, w.diff, w.tile_sums, w.wide_flag, mk, st);
         if (rc) return rc;
-        // ... and the plan of the next pass runs on the side stream next to the scan of this subtraction: it
-        // reads the stamps the deposit kernel wrote and clears the counters the copy above has taken.  After
-        // the last iteration it is the plan of the closing median pass.
+        // ... and, on the side stream next to it, the plan of the next pass: it reads the stamps the test wrote
+        // and clears the counters the copy above has taken.  After the last iteration it is the plan of the
+        // closing median pass.
         if (!(use_mean && it + 1 == params->max_iter)) {
             const bool closing = it + 1 == params->max_iter;
-            GBFG_CUDA(cudaStreamWaitEvent(side->s, side->ev_dep, 0));
+            GBFG_CUDA(cudaStreamWaitEvent(side->s, ev_read, 0));
             rc = launch_plan(w.blk_stamp, it + 1, !incremental, nb, n_cat, W, w.plan, closing ? nullptr : w.counters,
                              closing ? 0 : (int)n_iter_counters, use_mean ? nullptr : med_outputs, side->s);
             if (rc) return rc;
@@ -388,25 +388,23 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
             if (plan_queued) { GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_plan, 0)); plan_queued = false; }   // it saw no stamps: made again
             // A negative median: S_n >= S_instr no longer holds, so the pre-selection is not valid
             // (the caller's spectrum does not contain the catalog).  Every unresolved source becomes
-            // a candidate, and this iteration's test, which did nothing (as did the subtraction queued
-            // behind it), is run on them.
+            // a candidate, and this iteration's test, which did nothing (as did the scan queued behind it),
+            // is run on them.
             preselect = false;
             GBFG_CUDA(cudaMemsetAsync(w.sw.cand_count, 0, sizeof(int64_t) * (size_t)(1 + n_cat), st));
             rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, nullptr, params->rho_th, nullptr, w.sw, st);
             if (rc) return rc;
             rc = launch_snr_cand(nb, n_cat, dev_psd, params->rho_th, dev_resolved, nullptr, n, w.sel_idx, sel_count,
-                                 near, 1, nullptr, true, w.sw, all_dirty, snr_tests, st);
+                                 near, 1, nullptr, true, w.sw, all_dirty, snr_tests, &sub, st);
             if (rc) return rc;
             GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
-            rc = launch_deposit(g, ct, dev_A, dev_f, dev_fdot, w.sel_idx, sel_count, n, -1, dev_spectrum, nullptr,
-                                w.diff, w.tile_sums, w.wide_flag, mk, st);
+            rc = launch_scan(nb, n_cat, dev_spectrum, w.diff, w.tile_sums, w.wide_flag, mk, st);
             if (rc) return rc;
             GBFG_CUDA(cudaStreamSynchronize(st));
             for (int c = 0; c < n_cat; ++c) host_results[c].n_candidates = 0;
         }
         n_cand = host[i_cand];
         const int64_t total = host[0];
-        last_total = total;
         for (int c = 0; c < n_cat; ++c) {
             gbfg_iter_result &r = host_results[c];
             if (r.n_candidates == 0) r.n_candidates = n_cat == 1 ? host[i_cand] : host[i_cand + 1 + c];

@@ -423,6 +423,7 @@ struct SnrArgs {
     int *any_near;
     int n_dblk;
     int64_t *test_count;        // [n_cat] tests evaluated, accumulated (nullable)
+    SubtractView sub;           // spectrum != NULL: a selected source is subtracted on the spot (eq. D4)
     int64_t n_bins;
     int n_cat;
     double thr;                 // rho_th^2
@@ -504,6 +505,33 @@ snr_cand_kernel(SnrArgs a)
                 s_sel[base + __popc(sel_mask & ((1u << lane) - 1u))] = src;
                 a.resolved[src] = 1;
                 a.cand.w[t] = 0;
+            }
+        }
+        if (sel && a.sub.spectrum) {
+            // stage (v), eq. (D4): spectrum[k] -= q over the source's bins, in the range-update form of deposit.cu
+            // (q from p = four_p / 4, exactly the deposit's), and the blocks whose median can change are stamped
+            const int64_t q = __double2ll_rn(ldexp(0.25 * a.cand.four_p[t], -a.sub.scale_log2));
+            if (q != 0) {
+                const int64_t k0 = gk0 - (int64_t)cat * a.n_bins;
+                const DepositMarks &mk = a.sub.mk;
+                if (w <= DEP_NARROW) {
+                    for (int k = 0; k < w; ++k) atomic_add_i64(a.sub.spectrum + gk0 + k, -q);
+                } else {
+                    atomic_add_i64(a.sub.diff + gk0, -q);
+                    mk.scan_stamp[(int64_t)cat * mk.scan_tiles + k0 / DEP_SCAN_TILE] = mk.stamp;
+                    if (k0 + w < a.n_bins) {
+                        atomic_add_i64(a.sub.diff + gk0 + w, q);
+                        mk.scan_stamp[(int64_t)cat * mk.scan_tiles + (k0 + w) / DEP_SCAN_TILE] = mk.stamp;
+                    }
+                    *a.sub.wide_flag = mk.stamp;
+                }
+                if (mk.blk_stamp) {
+                    int64_t lo = k0 - mk.med_h, hi = k0 + w - 1 + mk.med_h;
+                    if (lo < 0) lo = 0;
+                    if (hi > a.n_bins - 1) hi = a.n_bins - 1;
+                    int *bs = mk.blk_stamp + (int64_t)cat * mk.n_dblk;
+                    for (int64_t b = lo >> mk.dblk_log2; b <= (hi >> mk.dblk_log2); ++b) bs[b] = mk.stamp;
+                }
             }
         }
         if (near && !sel && !always) { a.cand.w[t] = -w; *a.any_near = 1; }
@@ -615,11 +643,12 @@ int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, con
 int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th, uint8_t *resolved, double *rho2_out,
                     int64_t n_launch, int64_t *sel_idx, int64_t *sel_count, int64_t *near_count, int near_per_cat,
                     const int *abort_flag, bool use_prefix, const SnrWork &sw, const DirtyView &dv, int64_t *test_count,
-                    cudaStream_t st)
+                    const SubtractView *sub, cudaStream_t st)
 {
     if (n_launch <= 0) return GBFG_OK;
     SnrArgs a;
     a.test_count = test_count;
+    if (sub) a.sub = *sub; else a.sub.spectrum = nullptr;
     a.dv = dv;
     a.psd = psd;
     a.pv = make_view(sw, n_bins);
