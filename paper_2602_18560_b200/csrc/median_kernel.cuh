@@ -145,17 +145,28 @@ running_median_tile_kernel(MedianArgs a)
         if (g0 >= a.n) g0 = 2 * a.n - 1 - g0;
         key_ref = (uint64_t)a.x[row + g0] ^ SIGN64;
         uint64_t vary = 0;
-        for (int p = tid; p < LTe; p += THREADS) {
-            uint64_t key = key_ref;
-            if (p < Lt) {
-                int64_t g = o0 - h + p;
-                if (g < 0) g = -g - 1;
-                if (g >= a.n) g = 2 * a.n - 1 - g;
-                key = (uint64_t)a.x[row + g] ^ SIGN64;
+        for (int p0 = tid; p0 < LTe; p0 += 4 * THREADS) {    // four independent loads in flight per thread
+            uint64_t key[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int p = p0 + u * THREADS;
+                key[u] = key_ref;
+                if (p < Lt) {
+                    int64_t g = o0 - h + p;
+                    if (g < 0) g = -g - 1;
+                    if (g >= a.n) g = 2 * a.n - 1 - g;
+                    key[u] = (uint64_t)__ldg(a.x + row + g) ^ SIGN64;
+                }
             }
-            vary |= key ^ key_ref;
-            skey[p] = (KeyT)key;
-            spos[p] = (uint16_t)p;
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int p = p0 + u * THREADS;
+                if (p < LTe) {
+                    vary |= key[u] ^ key_ref;
+                    skey[p] = (KeyT)key[u];
+                    spos[p] = (uint16_t)p;
+                }
+            }
         }
         const unsigned vlo = __reduce_or_sync(FULL, (unsigned)vary);
         const unsigned vhi = __reduce_or_sync(FULL, (unsigned)(vary >> 32));
@@ -436,16 +447,30 @@ running_median_tile_kernel(MedianArgs a)
     __syncthreads();
 
     // ---- coalesced epilogue: median and PSD
-    for (int j = tid; j < n_out; j += THREADS) {
-        int64_t v;
-        if (NARROW) v = (int64_t)(((key_ref & 0xffffffff00000000ull) | (uint64_t)skey[orank[j]]) ^ SIGN64);
-        else v = (int64_t)((uint64_t)skey[orank[j]] ^ SIGN64);
-        int64_t g = o0 + j;
-        a.med[row + g] = v;
-        neg |= v < 0;
+    for (int j0 = tid; j0 < n_out; j0 += 4 * THREADS) {
+        double si[4];
         if (a.psd) {
-            double e = (double)v * a.scale;
-            a.psd[row + g] = a.s_instr[g] + a.norm * e;
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const int j = j0 + u * THREADS;
+                si[u] = j < n_out ? __ldg(a.s_instr + o0 + j) : 0.0;
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int j = j0 + u * THREADS;
+            if (j < n_out) {
+                int64_t v;
+                if (NARROW) v = (int64_t)(((key_ref & 0xffffffff00000000ull) | (uint64_t)skey[orank[j]]) ^ SIGN64);
+                else v = (int64_t)((uint64_t)skey[orank[j]] ^ SIGN64);
+                const int64_t g = o0 + j;
+                a.med[row + g] = v;
+                neg |= v < 0;
+                if (a.psd) {
+                    const double e = (double)v * a.scale;
+                    a.psd[row + g] = si[u] + a.norm * e;
+                }
+            }
         }
     }
   }   // tiles
