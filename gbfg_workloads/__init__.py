@@ -186,3 +186,15 @@ def random_spectrum(n: int, seed: int, kind: str = "lognormal") -> np.ndarray:
     if kind == "const":
         return np.full(n, 42, dtype=np.int64)
     raise ValueError(kind)
+
+
+def log_bin_edges(w: Workload, n_coarse: int = 100, f_lo: float | None = None, f_hi: float | None = None) -> np.ndarray:
+    """Fine-bin index edges of n_coarse logarithmically spaced coarse bins over [f_lo, f_hi] (100 bins
+    over 0.1-10 mHz; default: the workload's band).  Harness-side, handed to both the oracle and the library:
+    coarse bin k holds the fine bins whose centre f_min + (i + 1/2)/T lies in [e_k, e_{k+1})."""
+    f_lo = w.f_min if f_lo is None else f_lo
+    f_hi = w.f_max if f_hi is None else f_hi
+    n_bins = int(np.ceil((w.f_max - w.f_min) * w.t_obs))
+    e = np.geomspace(f_lo, f_hi, n_coarse + 1)
+    idx = np.ceil((e - w.f_min) * w.t_obs - 0.5).astype(np.int64)      # first bin whose centre is >= e_k
+    return np.clip(idx, 0, n_bins)

@@ -298,3 +298,29 @@ def simulate(w, cat: int = 0, n_src: int | None = None, estimator: int = 0):
                                    estimator=estimator)
     out.update(A=A, f=f, fdot=fd, s_instr=s_instr, total=total, residual=spec, rejected=rejected, grid=grid)
     return out
+
+
+# ---------------------------------------------------------------------------------------------
+# Coarse-graining of the PSD, eqs. (13)-(14) PAPER.md:186-199, and the characteristic strain, eq. (B1)
+# PAPER.md:465 (R10).  Plain Python / numpy: math.fsum is the exactly rounded sum.
+# ---------------------------------------------------------------------------------------------
+def coarse_grain(psd: np.ndarray, edges, f_min: float, t_obs: float):
+    """edges: n_coarse+1 non-decreasing fine-bin indices; coarse bin k holds the fine bins
+    edges[k] <= i < edges[k+1], whose frequencies are the bin centres f_i = f_min + (i + 1/2)/T.
+    -> (S[k] = (1/N_k) sum S_n(f_i)  (eq. 13),  f[k] = (1/N_k) sum f_i  (eq. 14),  hc[k] = sqrt(f[k] S[k])  (eq. B1));
+    an empty coarse bin gives NaN in all three."""
+    import math
+    psd = _f64(psd)
+    n_coarse = len(edges) - 1
+    S = np.full(n_coarse, np.nan)
+    fk = np.full(n_coarse, np.nan)
+    hc = np.full(n_coarse, np.nan)
+    for k in range(n_coarse):
+        i0, i1 = int(edges[k]), int(edges[k + 1])
+        nk = i1 - i0
+        if nk <= 0:
+            continue
+        S[k] = math.fsum(psd[i0:i1].tolist()) / nk
+        fk[k] = math.fsum(f_min + (i + 0.5) / t_obs for i in range(i0, i1)) / nk
+        hc[k] = math.sqrt(fk[k] * S[k])
+    return S, fk, hc
