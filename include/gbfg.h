@@ -151,6 +151,16 @@ int gbfg_running_mean(const int64_t *dev_spectrum, int64_t n_bins, int32_t n_cat
 int gbfg_psd(const int64_t *dev_median, const double *dev_s_instr, int64_t n_bins, int32_t n_cat,
              double median_norm, int32_t scale_log2, double *dev_psd, void *stream);
 
+/* Coarse-graining of the PSD, eqs. (13)-(14), and the characteristic strain of eq. (B1)
+ * (PAPER.md:465); R10.  dev_edges: DEVICE [n_coarse + 1] non-decreasing fine-bin indices; coarse bin k
+ * holds the fine bins edges[k] <= i < edges[k+1] (clipped to [0, n_bins]), whose frequencies are the bin centres
+ * f_min + (i + 1/2)/t_obs.  Written: dev_S [n_cat][n_coarse] = mean PSD of the bin (eq. 13), dev_f [n_coarse] =
+ * mean frequency (eq. 14; may be NULL), dev_hc [n_cat][n_coarse] = sqrt(f S) (eq. B1; may be NULL).  An empty
+ * coarse bin gives NaN.  The mean is within a few ulp of the exactly rounded one (compensated summation). */
+int gbfg_coarse_grain(const double *dev_psd, int64_t n_bins, int32_t n_cat, const int64_t *dev_edges,
+                      int32_t n_coarse, double f_min, double t_obs, double *dev_S, double *dev_f,
+                      double *dev_hc, void *stream);
+
 /* Stage (iv) — SNR of every unresolved source against the current PSD and selection
  * (eqs. 11-12; R4): rho2_i = sum_{k in bins(i)} 4 p_i / psd[c][k];
  * newly resolved iff rho2_i > rho_th^2 (strict).  For those, dev_resolved[i] is set to 1 and i is

@@ -25,7 +25,7 @@ EXPORTS = [
     "gbfg_sample_catalog", "gbfg_deposit", "gbfg_running_median", "gbfg_psd", "gbfg_snr_select",
     "gbfg_subtract_until_converged", "gbfg_simulate", "gbfg_simulate_host", "gbfg_workspace_bytes",
     "gbfg_kernel_launch_count", "gbfg_profile_enable", "gbfg_profile_read", "gbfg_release_cached",
-    "gbfg_running_mean",
+    "gbfg_running_mean", "gbfg_coarse_grain",
 ]
 
 KERNEL_CLASSES = ["sample", "noise", "deposit", "scan", "median", "psd", "inv_blocks", "snr", "aux"]
@@ -91,6 +91,7 @@ def load():
     L.gbfg_running_median.argtypes = [vp, i64, i32, i32, vp, vp]
     L.gbfg_psd.argtypes = [vp, vp, i64, i32, dbl, i32, vp, vp]
     L.gbfg_running_mean.argtypes = [vp, i64, i32, i32, vp, vp, i32, vp, vp]
+    L.gbfg_coarse_grain.argtypes = [vp, i64, i32, vp, i32, dbl, dbl, vp, vp, vp, vp]
     L.gbfg_snr_select.argtypes = [gp, vp, vp, vp, op, i32, vp, dbl, vp, vp, vp, vp, vp, vp, sz, vp]
     L.gbfg_subtract_until_converged.argtypes = [gp, vp, vp, vp, op, i32, vp, ip, vp, vp, vp, vp, rp, vp, sz, vp]
     L.gbfg_simulate.argtypes = [gp, pp, op, i32, u64, vp, ip, vp, vp, vp, vp, vp, vp, vp, vp, vp, rp, vp, sz, vp]
@@ -209,6 +210,12 @@ def running_mean(dev_spectrum, n_bins: int, n_cat: int, window: int, dev_sum_out
                  scale_log2: int = -140, dev_psd=None, stream=None):
     _check(load().gbfg_running_mean(_ptr(dev_spectrum), n_bins, n_cat, window, _ptr(dev_sum_out), _ptr(dev_s_instr),
                                     scale_log2, _ptr(dev_psd), _stream(stream)))
+
+
+def coarse_grain(dev_psd, n_bins: int, n_cat: int, dev_edges, n_coarse: int, f_min: float, t_obs: float, dev_S,
+                 dev_f=None, dev_hc=None, stream=None):
+    _check(load().gbfg_coarse_grain(_ptr(dev_psd), n_bins, n_cat, _ptr(dev_edges), n_coarse, f_min, t_obs, _ptr(dev_S),
+                                    _ptr(dev_f), _ptr(dev_hc), _stream(stream)))
 
 
 def psd(dev_median, dev_s_instr, n_bins: int, n_cat: int, median_norm: float, scale_log2: int, dev_psd, stream=None):

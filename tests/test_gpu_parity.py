@@ -479,3 +479,38 @@ def test_loop_mean_estimator(gb, orc, torch):
 @pytest.mark.slow
 def test_loop_mean_estimator_config2_full(gb, orc, torch):
     _loop_case_mean(gb, orc, torch, wl.config(2))
+
+
+# ------------------------------------------- coarse-graining, eqs. (13)-(14), (B1) (R10)
+COARSE_RTOL = 1e-14        # compensated sums + a 256-leaf tree against the oracle's exactly rounded sum (R10)
+
+
+@pytest.mark.parametrize("cfg,n_coarse,band", [(0, 100, (1e-4, 1e-2)), (2, 100, (1e-4, 1e-2)), (2, 37, None), (2, 1, None)])
+def test_coarse_grain_matches_oracle(gb, orc, torch, cfg, n_coarse, band):
+    w = wl.config(cfg)
+    g = gpu_grid(gb, w)
+    nb = g.n_bins
+    rng = np.random.default_rng(cfg + n_coarse)
+    psd = np.stack([10.0 ** rng.uniform(-41, -34, nb), 10.0 ** (-38 + 0.5 * np.sin(np.arange(nb) / 3e4))])
+    e = wl.log_bin_edges(w, n_coarse, *(band or (None, None)))
+    S = torch.empty((2, n_coarse), dtype=torch.float64, device="cuda")
+    hc = torch.empty((2, n_coarse), dtype=torch.float64, device="cuda")
+    fk = torch.empty(n_coarse, dtype=torch.float64, device="cuda")
+    gb.coarse_grain(dev(torch, psd), nb, 2, dev(torch, e), n_coarse, w.f_min, w.t_obs, S, fk, hc)
+    for r in range(2):
+        S_ref, f_ref, hc_ref = orc.coarse_grain(psd[r], e, w.f_min, w.t_obs)
+        assert np.allclose(S[r].cpu().numpy(), S_ref, rtol=COARSE_RTOL, atol=0, equal_nan=True)
+        assert np.allclose(hc[r].cpu().numpy(), hc_ref, rtol=COARSE_RTOL, atol=0, equal_nan=True)
+        assert np.allclose(fk.cpu().numpy(), f_ref, rtol=1e-15, atol=0, equal_nan=True)
+
+
+def test_coarse_grain_empty_bins_and_clipping(gb, orc, torch):
+    w = wl.config(0)
+    g = gpu_grid(gb, w)
+    nb = g.n_bins
+    psd = np.full(nb, 2.0 ** -131)
+    e = np.array([0, 7, 7, 100, nb, nb + 50], dtype=np.int64)           # an empty bin, one past the end
+    S = torch.empty((1, 5), dtype=torch.float64, device="cuda")
+    gb.coarse_grain(dev(torch, psd), nb, 1, dev(torch, e), 5, w.f_min, w.t_obs, S)
+    got = S.cpu().numpy()[0]
+    assert got[0] == 2.0 ** -131 and np.isnan(got[1]) and got[2] == 2.0 ** -131 and got[3] == 2.0 ** -131 and np.isnan(got[4])
