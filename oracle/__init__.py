@@ -83,6 +83,8 @@ def lib():
         L.orc_subtract_until_converged_est.argtypes = [
             C.POINTER(Grid), dp, dp, dp, C.c_int64, dp, C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_int32,
             ip, ip, dp, up, C.POINTER(IterResult), ip]
+        L.orc_aet_noise.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, dp]
+        L.orc_instrument_noise_aet.argtypes = [C.POINTER(Grid), C.c_double, C.c_double, C.c_double, C.c_int, dp, dp, dp, dp]
         L.orc_running_sum_def.argtypes = [ip, C.c_int64, C.c_int32, C.c_int64, C.c_int64, ip]
         L.orc_running_sum.argtypes = [ip, C.c_int64, C.c_int32, ip]
         L.orc_psd_mean.argtypes = [ip, dp, C.c_int64, C.c_int32, C.c_int32, dp]
@@ -203,6 +205,19 @@ def running_median(x: np.ndarray, window: int) -> np.ndarray:
     if rc:
         raise ValueError("invalid window / size")
     return out
+
+
+def aet_noise(f: float, P: float = 15.0, A: float = 3.0, L: float = 2.5e9, tdi2: bool = True):
+    """(S_AA, S_TT, S_AA / R_AA, S_TT / R_TT) at frequency f: eqs. (C1)-(C5), (B2)-(B5)."""
+    out = (C.c_double * 4)()
+    lib().orc_aet_noise(f, P, A, L, 1 if tdi2 else 0, out)
+    return tuple(out)
+
+
+def instrument_noise_aet(grid: Grid, P: float = 15.0, A: float = 3.0, L: float = 2.5e9, tdi2: bool = True):
+    outs = [np.empty(grid.n_bins, dtype=np.float64) for _ in range(4)]
+    lib().orc_instrument_noise_aet(C.byref(grid), P, A, L, 1 if tdi2 else 0, *[_d(o) for o in outs])
+    return tuple(outs)
 
 
 def running_sum_def(x: np.ndarray, window: int, k_begin: int = 0, k_end: int | None = None) -> np.ndarray:

@@ -311,6 +311,66 @@ double orc_robson_sn(double fq)
     return (10.0 / (3.0 * L * L)) * (p_oms + acc) * (1.0 + 0.6 * (x * x));
 }
 
+/* SciRDv1 noise in the TDI A/E/T channels, eqs. (C1)-(C5) PAPER.md:494-509, and its rescaling by the
+ * TDI response, eqs. (B2)-(B5) PAPER.md:475-487 (R11).  P in pm, A in fm s^-2, L in m.
+ * out[0] = S^AA = S^EE (C3), out[1] = S^TT (C4) (both times 4 sin^2(2 f/f*) when tdi2, C5),
+ * out[2] = S^AA / R_AA, out[3] = S^TT / R_TT (B2; the TDI generation cancels in the ratio).
+ * (C2) is garbled in PAPER.md:496: "(f / 8 mHz^4)" is read as (f / 8 mHz)^4.
+ * 1 - cos x is taken as 2 sin^2(x/2): no cancellation at the low end of the band. */
+void orc_aet_noise(double fq, double P, double A, double L, int tdi2, double out[4])
+{
+    const double c = 299792458.0;
+    double fstar = c / (ORC_TWO_PI * L);
+    double x = fq / fstar;
+    double sn, cs, sh, ch;
+    orc_sincos(x, &sn, &cs);
+    orc_sincos(0.5 * x, &sh, &ch);
+    double omc = 2.0 * (sh * sh);                               /* 1 - cos x */
+    double k2 = ORC_TWO_PI * fq / c;  k2 = k2 * k2;             /* (2 pi f / c)^2 */
+    double r2 = 2.0e-3 / fq;  r2 = r2 * r2;
+    double a_oms = P * 1.0e-12;
+    double p_oms = (a_oms * a_oms) * (1.0 + r2 * r2) * k2;     /* (C1) */
+    double r4 = 0.4e-3 / fq;
+    double r8 = fq / 8.0e-3;  r8 = r8 * r8;
+    double a_tm = A * 1.0e-15;
+    double y = ORC_TWO_PI * fq;  y = y * y;  y = y * y;         /* (2 pi f)^4 */
+    double p_tm = (a_tm * a_tm) * (1.0 + r4 * r4) * (1.0 + r8 * r8) / y * k2;   /* (C2) */
+    double s2 = sn * sn;
+    double s_aa = 8.0 * s2 * (4.0 * (1.0 + cs + cs * cs) * p_tm + (2.0 + cs) * p_oms);   /* (C3) */
+    double s_tt = 16.0 * s2 * (2.0 * (omc * omc) * p_tm + omc * p_oms);                  /* (C4) */
+    double x2 = x * x;
+    double pre = 16.0 * s2 * x2;                                /* (B3) */
+    double r_aa = pre * (0.45 / (1.0 + 0.7 * x2));              /* (B4), 9/20 */
+    double x4 = x2 * x2;
+    double r_tt = pre * (0.45 * (x4 * x2) / (1.8e3 + 0.7 * (x4 * x4)));   /* (B5) */
+    out[2] = s_aa / r_aa;
+    out[3] = s_tt / r_tt;
+    if (tdi2) {
+        double s2x, c2x;
+        orc_sincos(2.0 * x, &s2x, &c2x);
+        double fac = 4.0 * (s2x * s2x);                         /* (C5) */
+        s_aa = fac * s_aa;
+        s_tt = fac * s_tt;
+    }
+    out[0] = s_aa;
+    out[1] = s_tt;
+}
+
+/* the four curves at the bin centres f_min + (k + 1/2)/T; any output may be NULL */
+void orc_instrument_noise_aet(const orc_grid *g, double P, double A, double L, int tdi2,
+                              double *s_aa, double *s_tt, double *sh_aa, double *sh_tt)
+{
+    for (int64_t k = 0; k < g->n_bins; ++k) {
+        double fk = g->f_min + ((double)k + 0.5) / g->t_obs;
+        double o[4];
+        orc_aet_noise(fk, P, A, L, tdi2, o);
+        if (s_aa) s_aa[k] = o[0];
+        if (s_tt) s_tt[k] = o[1];
+        if (sh_aa) sh_aa[k] = o[2];
+        if (sh_tt) sh_tt[k] = o[3];
+    }
+}
+
 void orc_instrument_noise(const orc_grid *g, double *s_instr)
 {
     for (int64_t k = 0; k < g->n_bins; ++k) {
