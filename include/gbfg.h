@@ -106,6 +106,15 @@ int gbfg_grid_init(double f_min, double f_max, double t_obs, int32_t scale_log2,
  * dev_s_instr: [n_bins] binary64, written. */
 int gbfg_instrument_noise(const gbfg_grid *grid, double *dev_s_instr, void *stream);
 
+/* Helper: SciRDv1 noise of the TDI channels, eqs. (C1)-(C5), and its rescaling by the TDI
+ * response, eqs. (B2)-(B5), at the bin centres (R11).  P_pm, A_fm: the OMS and
+ * test-mass amplitudes in pm and fm s^-2 (SciRDv1: 15 and 3); L_m: arm length in metres; tdi2 != 0: TDI 2.0,
+ * eq. (C5).  Written (each [n_bins] binary64, any may be NULL but not all): dev_S_AA = S^AA = S^EE (C3),
+ * dev_S_TT (C4), dev_Sh_AA = S^AA / R_AA, dev_Sh_TT = S^TT / R_TT (B2: strain-equivalent noise, usable as the
+ * s_instr of the stage calls). */
+int gbfg_instrument_noise_aet(const gbfg_grid *grid, double P_pm, double A_fm, double L_m, int32_t tdi2,
+                              double *dev_S_AA, double *dev_S_TT, double *dev_Sh_AA, double *dev_Sh_TT, void *stream);
+
 /* Stage (i) — step 1 of the algorithm: draw every catalog of the batch from its
  * population with Philox4x32-10 (R1, §4).  pops: HOST [n_cat]; offsets: HOST [n_cat+1]
  * with offsets[c+1]-offsets[c] = pops[c].n_src.  Catalog c uses Philox counter word 3 =

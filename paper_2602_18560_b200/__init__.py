@@ -25,7 +25,7 @@ EXPORTS = [
     "gbfg_sample_catalog", "gbfg_deposit", "gbfg_running_median", "gbfg_psd", "gbfg_snr_select",
     "gbfg_subtract_until_converged", "gbfg_simulate", "gbfg_simulate_host", "gbfg_workspace_bytes",
     "gbfg_kernel_launch_count", "gbfg_profile_enable", "gbfg_profile_read", "gbfg_release_cached",
-    "gbfg_running_mean", "gbfg_coarse_grain",
+    "gbfg_running_mean", "gbfg_coarse_grain", "gbfg_instrument_noise_aet",
 ]
 
 KERNEL_CLASSES = ["sample", "noise", "deposit", "scan", "median", "psd", "inv_blocks", "snr", "aux"]
@@ -86,6 +86,7 @@ def load():
     L.gbfg_kernel_launch_count.restype = i64
     L.gbfg_grid_init.argtypes = [dbl, dbl, dbl, i32, gp]
     L.gbfg_instrument_noise.argtypes = [gp, vp, vp]
+    L.gbfg_instrument_noise_aet.argtypes = [gp, dbl, dbl, dbl, i32, vp, vp, vp, vp, vp]
     L.gbfg_sample_catalog.argtypes = [gp, pp, op, i32, u32, u64, vp, vp, vp, vp]
     L.gbfg_deposit.argtypes = [gp, vp, vp, vp, op, i32, vp, vp, i32, vp, vp, vp, sz, vp]
     L.gbfg_running_median.argtypes = [vp, i64, i32, i32, vp, vp]
@@ -187,6 +188,12 @@ def workspace_bytes(grid: Grid, n_src_total: int, n_cat: int = 1) -> int:
 
 def instrument_noise(grid: Grid, dev_s_instr, stream=None):
     _check(load().gbfg_instrument_noise(C.byref(grid), _ptr(dev_s_instr), _stream(stream)))
+
+
+def instrument_noise_aet(grid: Grid, dev_S_AA=None, dev_S_TT=None, dev_Sh_AA=None, dev_Sh_TT=None, P_pm: float = 15.0,
+                         A_fm: float = 3.0, L_m: float = 2.5e9, tdi2: bool = True, stream=None):
+    _check(load().gbfg_instrument_noise_aet(C.byref(grid), P_pm, A_fm, L_m, 1 if tdi2 else 0, _ptr(dev_S_AA), _ptr(dev_S_TT),
+                                            _ptr(dev_Sh_AA), _ptr(dev_Sh_TT), _stream(stream)))
 
 
 def sample_catalog(grid: Grid, pops, offsets, seed: int, dev_A, dev_f, dev_fdot, first_cat_id: int = 0, stream=None):

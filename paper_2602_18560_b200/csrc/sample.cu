@@ -257,6 +257,68 @@ instrument_noise_kernel(double f_min, double T, int64_t n_bins, double *__restri
     }
 }
 
+// SciRDv1 noise of the TDI channels and its rescaling by the response (R11; eqs. C1-C5
+// PAPER.md:494-509, B2-B5 PAPER.md:475-487), operation by operation as R11 lists them.
+struct AetOut { double s_aa, s_tt, sh_aa, sh_tt; };
+
+__device__ __forceinline__ AetOut aet_noise(double fq, double P, double A, double L, int tdi2)
+{
+    const double c = 299792458.0;
+    const double fstar = c / (GB_TWO_PI * L);
+    const double x = fq / fstar;
+    double sn, cs, sh, ch;
+    det_sincos(x, sn, cs);
+    det_sincos(0.5 * x, sh, ch);
+    const double omc = 2.0 * (sh * sh);                       // 1 - cos x
+    double k2 = GB_TWO_PI * fq / c;  k2 = k2 * k2;
+    double r2 = 2.0e-3 / fq;  r2 = r2 * r2;
+    const double a_oms = P * 1.0e-12;
+    const double p_oms = (a_oms * a_oms) * (1.0 + r2 * r2) * k2;
+    const double r4 = 0.4e-3 / fq;
+    double r8 = fq / 8.0e-3;  r8 = r8 * r8;
+    const double a_tm = A * 1.0e-15;
+    double y = GB_TWO_PI * fq;  y = y * y;  y = y * y;
+    const double p_tm = (a_tm * a_tm) * (1.0 + r4 * r4) * (1.0 + r8 * r8) / y * k2;
+    const double s2 = sn * sn;
+    double s_aa = 8.0 * s2 * (4.0 * (1.0 + cs + cs * cs) * p_tm + (2.0 + cs) * p_oms);
+    double s_tt = 16.0 * s2 * (2.0 * (omc * omc) * p_tm + omc * p_oms);
+    const double x2 = x * x;
+    const double pre = 16.0 * s2 * x2;
+    const double r_aa = pre * (0.45 / (1.0 + 0.7 * x2));
+    const double x4 = x2 * x2;
+    const double r_tt = pre * (0.45 * (x4 * x2) / (1.8e3 + 0.7 * (x4 * x4)));
+    AetOut o;
+    o.sh_aa = s_aa / r_aa;
+    o.sh_tt = s_tt / r_tt;
+    if (tdi2) {
+        double s2x, c2x;
+        det_sincos(2.0 * x, s2x, c2x);
+        const double fac = 4.0 * (s2x * s2x);
+        s_aa = fac * s_aa;
+        s_tt = fac * s_tt;
+    }
+    o.s_aa = s_aa;
+    o.s_tt = s_tt;
+    return o;
+}
+
+__global__ void __launch_bounds__(256)
+instrument_noise_aet_kernel(double f_min, double T, int64_t n_bins, double P, double A, double L, int tdi2,
+                            double *__restrict__ s_aa, double *__restrict__ s_tt,
+                            double *__restrict__ sh_aa, double *__restrict__ sh_tt)
+{
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (; k < n_bins; k += stride) {
+        const double fk = f_min + ((double)k + 0.5) / T;
+        const AetOut o = aet_noise(fk, P, A, L, tdi2);
+        if (s_aa) s_aa[k] = o.s_aa;
+        if (s_tt) s_tt[k] = o.s_tt;
+        if (sh_aa) sh_aa[k] = o.sh_aa;
+        if (sh_tt) sh_tt[k] = o.sh_tt;
+    }
+}
+
 }  // namespace gbfg
 
 using namespace gbfg;
@@ -274,6 +336,27 @@ extern "C" int gbfg_instrument_noise(const gbfg_grid *grid, double *dev_s_instr,
         instrument_noise_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(grid->f_min, grid->t_obs, grid->n_bins, dev_s_instr);
     }
     GBFG_LAUNCH_CHECK("instrument_noise_kernel");
+    return GBFG_OK;
+}
+
+extern "C" int gbfg_instrument_noise_aet(const gbfg_grid *grid, double P_pm, double A_fm, double L_m, int32_t tdi2,
+                                         double *dev_S_AA, double *dev_S_TT, double *dev_Sh_AA, double *dev_Sh_TT,
+                                         void *stream)
+{
+    if (!grid || grid->struct_size != sizeof(gbfg_grid)) return GBFG_ERR_INVALID_ARG;
+    if (!(P_pm > 0.0) || !(A_fm > 0.0) || !(L_m > 0.0)) return GBFG_ERR_INVALID_ARG;
+    if (!dev_S_AA && !dev_S_TT && !dev_Sh_AA && !dev_Sh_TT) return GBFG_ERR_INVALID_ARG;
+    int rc = check_device();
+    if (rc) return rc;
+    int blocks = (int)((grid->n_bins + 255) / 256);
+    int cap = sm_count() * 8;
+    if (blocks > cap) blocks = cap;
+    {
+        LaunchTimer lt(K_NOISE, (cudaStream_t)stream);
+        instrument_noise_aet_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(grid->f_min, grid->t_obs, grid->n_bins, P_pm, A_fm,
+                                                                              L_m, tdi2 ? 1 : 0, dev_S_AA, dev_S_TT, dev_Sh_AA, dev_Sh_TT);
+    }
+    GBFG_LAUNCH_CHECK("instrument_noise_aet_kernel");
     return GBFG_OK;
 }
 

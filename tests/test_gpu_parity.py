@@ -514,3 +514,44 @@ def test_coarse_grain_empty_bins_and_clipping(gb, orc, torch):
     gb.coarse_grain(dev(torch, psd), nb, 1, dev(torch, e), 5, w.f_min, w.t_obs, S)
     got = S.cpu().numpy()[0]
     assert got[0] == 2.0 ** -131 and np.isnan(got[1]) and got[2] == 2.0 ** -131 and got[3] == 2.0 ** -131 and np.isnan(got[4])
+
+
+# ----------------------------------------------- SciRDv1 A/E/T noise, eqs. (C1)-(C5), (B2)-(B5) (R11)
+@pytest.mark.parametrize("cfg,tdi2", [(0, True), (0, False), (2, True)])
+def test_instrument_noise_aet_bit_exact(gb, orc, torch, cfg, tdi2):
+    w = wl.config(cfg)
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    ref = orc.instrument_noise_aet(og, tdi2=tdi2)
+    outs = [torch.empty(g.n_bins, dtype=torch.float64, device="cuda") for _ in range(4)]
+    gb.instrument_noise_aet(g, *outs, tdi2=tdi2)
+    for o, r in zip(outs, ref):
+        assert np.array_equal(bits(o.cpu().numpy()), bits(r))
+    only = torch.empty(g.n_bins, dtype=torch.float64, device="cuda")
+    gb.instrument_noise_aet(g, dev_Sh_AA=only, tdi2=tdi2)
+    assert np.array_equal(bits(only.cpu().numpy()), bits(ref[2]))
+
+
+def test_loop_with_the_aet_strain_noise(gb, orc, torch):
+    """The loop takes any s_instr: here S^AA / R_AA of eqs. (C3), (B2)-(B4) in place of the Robson curve."""
+    w = wl.dense_case("short")
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    sh_aa = orc.instrument_noise_aet(og)[2]
+    A, f, fd = orc.sample_catalog(og, w.pops[0], 0, w.seed)
+    spec = np.zeros(og.n_bins, dtype=np.int64)
+    orc.deposit(og, A, f, fd, spec)
+    ref_spec = spec.copy()
+    ref = orc.subtract_until_converged(og, A, f, fd, sh_aa, w.window, w.median_norm, w.rho_th, w.max_iter, ref_spec)
+    n, nb = A.size, g.n_bins
+    d_spec = dev(torch, spec)
+    med = torch.empty(nb, dtype=torch.int64, device="cuda")
+    psd = torch.empty(nb, dtype=torch.float64, device="cuda")
+    resolved = torch.zeros(n, dtype=torch.uint8, device="cuda")
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter)
+    res = gb.subtract_until_converged(g, dev(torch, A), dev(torch, f), dev(torch, fd), [0, n], dev(torch, sh_aa), params,
+                                      d_spec, med, psd, resolved, workspace(torch, gb, g, n))[0]
+    assert np.array_equal(d_spec.cpu().numpy(), ref_spec)
+    assert np.array_equal(bits(psd.cpu().numpy()), bits(ref["psd"]))
+    assert np.array_equal(resolved.cpu().numpy(), ref["resolved"])
+    assert (res.n_iter, res.n_resolved) == (ref["n_iter"], ref["n_resolved"])
