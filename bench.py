@@ -156,8 +156,8 @@ def algorithmic_bytes(w: wl.Workload, n_bins: int, res, prof) -> dict:
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of running_median_kernel per output it recomputes, from the
-# committed `ncu --set full` capture (profiles/r01_ncu_full_v2.md: 71.5 MB for ~3.5e6 outputs)
-MEDIAN_DRAM_BYTES_PER_OUTPUT = 20.5
+# committed `ncu --set full` capture (profiles/r01_ncu_full_v3.md: 67.1 MB for ~3.4e6 outputs)
+MEDIAN_DRAM_BYTES_PER_OUTPUT = 20.0
 
 
 def run_gpu(args, w: wl.Workload):
