@@ -165,13 +165,14 @@ static cudaEvent_t readback_event()
 }
 
 // side stream on which the plan of the next pass runs next to the scan of the subtraction (one per host thread)
-struct SideStream { cudaStream_t s; cudaEvent_t ev_plan; };
+struct SideStream { cudaStream_t s; cudaEvent_t ev_plan, ev_aux; };
 static SideStream *side_stream()
 {
-    static thread_local SideStream ss = {nullptr, nullptr};
+    static thread_local SideStream ss = {nullptr, nullptr, nullptr};
     if (!ss.s) {
         if (cudaStreamCreateWithFlags(&ss.s, cudaStreamNonBlocking) != cudaSuccess ||
-            cudaEventCreateWithFlags(&ss.ev_plan, cudaEventDisableTiming) != cudaSuccess) {
+            cudaEventCreateWithFlags(&ss.ev_plan, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&ss.ev_aux, cudaEventDisableTiming) != cudaSuccess) {
             (void)cudaGetLastError();
             ss.s = nullptr;
             return nullptr;
@@ -261,23 +262,62 @@ extern "C" int gbfg_snr_select(const gbfg_grid *grid, const double *dev_A, const
                            dev_sel_count, dev_near_count, 0, nullptr, true, w.sw, all_dirty, nullptr, nullptr, st);
 }
 
-extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double *dev_A, const double *dev_f,
-                                             const double *dev_fdot, const int64_t *offsets, int32_t n_cat,
-                                             const double *dev_s_instr, const gbfg_iter_params *params,
-                                             int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
-                                             uint8_t *dev_resolved, gbfg_iter_result *host_results,
-                                             void *workspace, size_t workspace_bytes, void *stream)
+// workspace state the loop starts from (also what a deposit needs: zero difference array and stamps)
+static int loop_init_workspace(const Workspace &w, int64_t nb, int n_cat, cudaStream_t st)
+{
+    const size_t row_bytes = sizeof(int64_t) * (size_t)n_cat * (size_t)nb;
+    GBFG_CUDA(cudaMemsetAsync(w.diff, 0, row_bytes, st));
+    GBFG_CUDA(cudaMemsetAsync(w.wide_flag, 0, sizeof(int) * (size_t)(1 + n_cat), st));
+    GBFG_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(int64_t) * WS_COUNTERS, st));
+    GBFG_CUDA(cudaMemsetAsync(w.scan_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)scan_tiles_per_row(nb), st));
+    GBFG_CUDA(cudaMemsetAsync(w.blk_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)w.plan.n_dblk, st));
+    return GBFG_OK;
+}
+
+// candidate records: with pre-selection, only sources whose rho^2 against S_instr reaches the threshold
+static int loop_build_candidates(const GridDev &g, const CatTable &ct, const double *dev_A, const double *dev_f,
+                                 const double *dev_fdot, const uint8_t *dev_resolved, const double *dev_s_instr,
+                                 double rho_th, bool preselect, const Workspace &w, cudaStream_t st)
+{
+    const DirtyView all_dirty = {nullptr, nullptr, 0, 0};
+    int rc = launch_prefix_header(dev_s_instr, g.n_bins, g.n_bins, w.sw, st);
+    if (rc) return rc;
+    if (preselect) {
+        rc = launch_inv_prefix(dev_s_instr, g.n_bins, 1, w.sw, all_dirty, st);
+        if (rc) return rc;
+    }
+    return launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, preselect ? dev_s_instr : nullptr, rho_th, nullptr,
+                             w.sw, st);
+}
+
+static int loop_validate(const gbfg_grid *grid, const gbfg_iter_params *params)
 {
     if (!valid_grid(grid) || !params || params->struct_size != sizeof(gbfg_iter_params)) return GBFG_ERR_INVALID_ARG;
-    if (!dev_s_instr || !dev_spectrum || !dev_median || !dev_psd || !dev_resolved || !host_results) return GBFG_ERR_INVALID_ARG;
     const int W = params->window;
     const bool use_mean = (params->flags & GBFG_FLAG_ESTIMATOR_MEAN) != 0;
     if (W < 1 || (W & 1) == 0 || params->max_iter < 1 || !(params->rho_th >= 0.0) || (!use_mean && !(params->median_norm > 0.0)))
         return GBFG_ERR_INVALID_ARG;
     if (W > GBFG_MAX_WINDOW) return GBFG_ERR_UNSUPPORTED;
     if (grid->n_bins < W / 2 + 1) return GBFG_ERR_INVALID_ARG;
+    return GBFG_OK;
+}
+
+// the loop proper.  prepared: the caller has initialised the workspace and built the candidate records (gbfg_simulate
+// does both next to the deposit).
+static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *dev_f,
+                     const double *dev_fdot, const int64_t *offsets, int32_t n_cat,
+                     const double *dev_s_instr, const gbfg_iter_params *params,
+                     int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
+                     uint8_t *dev_resolved, gbfg_iter_result *host_results,
+                     void *workspace, size_t workspace_bytes, void *stream, bool prepared)
+{
+    int rc = loop_validate(grid, params);
+    if (rc) return rc;
+    if (!dev_s_instr || !dev_spectrum || !dev_median || !dev_psd || !dev_resolved || !host_results) return GBFG_ERR_INVALID_ARG;
+    const int W = params->window;
+    const bool use_mean = (params->flags & GBFG_FLAG_ESTIMATOR_MEAN) != 0;
     CatTable ct;
-    int rc = make_cat_table(offsets, n_cat, &ct);
+    rc = make_cat_table(offsets, n_cat, &ct);
     if (rc) return rc;
     const int64_t n = ct.offsets[n_cat];
     if (n > 0 && (!dev_A || !dev_f || !dev_fdot)) return GBFG_ERR_INVALID_ARG;
@@ -291,8 +331,6 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     cudaStream_t st = (cudaStream_t)stream;
     const GridDev g = make_grid_dev(grid);
     const int64_t nb = grid->n_bins;
-    const size_t row_bytes = sizeof(int64_t) * (size_t)n_cat * (size_t)nb;
-    const int scan_tiles = scan_tiles_per_row(nb);
 
     int64_t *sel_count = w.counters;                    // [1 + n_cat]
     int64_t *near = w.counters + 1 + n_cat;             // [n_cat]
@@ -305,24 +343,14 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     bool preselect = (params->flags & GBFG_FLAG_NO_PRESELECT) == 0;
     const bool incremental = (params->flags & GBFG_FLAG_NO_INCREMENTAL) == 0;
 
-    GBFG_CUDA(cudaMemsetAsync(w.diff, 0, row_bytes, st));
-    GBFG_CUDA(cudaMemsetAsync(w.wide_flag, 0, sizeof(int) * (size_t)(1 + n_cat), st));
-    GBFG_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(int64_t) * WS_COUNTERS, st));
-    GBFG_CUDA(cudaMemsetAsync(w.scan_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)scan_tiles, st));
-    GBFG_CUDA(cudaMemsetAsync(w.blk_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)w.plan.n_dblk, st));
     const DirtyView all_dirty = {nullptr, nullptr, 0, 0};
     const DirtyView dirty = {w.plan.cum, w.plan.range, w.plan.n_dblk, w.plan.dblk_log2};
-
-    // candidate records: with pre-selection, only sources whose rho^2 against S_instr reaches the threshold
-    rc = launch_prefix_header(dev_s_instr, nb, nb, w.sw, st);
-    if (rc) return rc;
-    if (preselect) {
-        rc = launch_inv_prefix(dev_s_instr, nb, 1, w.sw, all_dirty, st);
+    if (!prepared) {
+        rc = loop_init_workspace(w, nb, n_cat, st);
+        if (rc) return rc;
+        rc = loop_build_candidates(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, dev_s_instr, params->rho_th, preselect, w, st);
         if (rc) return rc;
     }
-    rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, preselect ? dev_s_instr : nullptr,
-                           params->rho_th, nullptr, w.sw, st);
-    if (rc) return rc;
 
     int64_t mean_passes = 0;
     bool done[GBFG_MAX_CAT];
@@ -447,6 +475,19 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
     return GBFG_OK;
 }
 
+extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double *dev_A, const double *dev_f,
+                                             const double *dev_fdot, const int64_t *offsets, int32_t n_cat,
+                                             const double *dev_s_instr, const gbfg_iter_params *params,
+                                             int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
+                                             uint8_t *dev_resolved, gbfg_iter_result *host_results,
+                                             void *workspace, size_t workspace_bytes, void *stream)
+{
+    return loop_impl(grid, dev_A, dev_f, dev_fdot, offsets, n_cat, dev_s_instr, params, dev_spectrum, dev_median, dev_psd,
+                     dev_resolved, host_results, workspace, workspace_bytes, stream, false);
+}
+
+// sample -> deposit -> loop.  The candidate records of the loop (a pass over the catalog against S_instr alone) are
+// built on the side stream while the deposit runs: both only read the catalog.
 extern "C" int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
                              uint64_t seed, const double *dev_s_instr, const gbfg_iter_params *params,
                              double *dev_A, double *dev_f, double *dev_fdot,
@@ -454,22 +495,44 @@ extern "C" int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const 
                              uint8_t *dev_resolved, int64_t *dev_err_count, gbfg_iter_result *host_results,
                              void *workspace, size_t workspace_bytes, void *stream)
 {
-    if (!valid_grid(grid) || !offsets || n_cat < 1 || !dev_spectrum || !dev_resolved) return GBFG_ERR_INVALID_ARG;
-    if (n_cat > GBFG_MAX_CAT) return GBFG_ERR_UNSUPPORTED;
-    cudaStream_t st = (cudaStream_t)stream;
-    int rc = gbfg_sample_catalog(grid, pops, offsets, n_cat, 0u, seed, dev_A, dev_f, dev_fdot, stream);
+    int rc = loop_validate(grid, params);
     if (rc) return rc;
-    const int64_t n = offsets[n_cat];
-    const size_t row_bytes = sizeof(int64_t) * (size_t)n_cat * (size_t)grid->n_bins;
+    if (!offsets || n_cat < 1 || !dev_s_instr || !dev_spectrum || !dev_median || !dev_psd || !dev_resolved || !host_results)
+        return GBFG_ERR_INVALID_ARG;
+    CatTable ct;
+    rc = make_cat_table(offsets, n_cat, &ct);
+    if (rc) return rc;
+    const int64_t n = ct.offsets[n_cat];
+    if (!workspace) return GBFG_ERR_WORKSPACE;
+    Workspace w = carve(workspace, grid->n_bins, n, n_cat);
+    if (workspace_bytes < w.bytes) return GBFG_ERR_WORKSPACE;
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = gbfg_sample_catalog(grid, pops, offsets, n_cat, 0u, seed, dev_A, dev_f, dev_fdot, stream);
+    if (rc) return rc;
+    SideStream *side = side_stream();
+    if (!side) return set_cuda_error(cudaErrorMemoryAllocation, "side stream");
+    const GridDev g = make_grid_dev(grid);
+    const int64_t nb = grid->n_bins;
+    const size_t row_bytes = sizeof(int64_t) * (size_t)n_cat * (size_t)nb;
     GBFG_CUDA(cudaMemsetAsync(dev_spectrum, 0, row_bytes, st));
     if (n > 0) GBFG_CUDA(cudaMemsetAsync(dev_resolved, 0, (size_t)n, st));
-    rc = gbfg_deposit(grid, dev_A, dev_f, dev_fdot, offsets, n_cat, nullptr, nullptr, +1, dev_spectrum, dev_err_count,
-                      workspace, workspace_bytes, stream);
+    rc = loop_init_workspace(w, nb, n_cat, st);
+    if (rc) return rc;
+    GBFG_CUDA(cudaEventRecord(side->ev_aux, st));
+    // side stream: the candidate records
+    GBFG_CUDA(cudaStreamWaitEvent(side->s, side->ev_aux, 0));
+    const bool preselect = (params->flags & GBFG_FLAG_NO_PRESELECT) == 0;
+    rc = loop_build_candidates(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, dev_s_instr, params->rho_th, preselect, w, side->s);
+    if (rc) return rc;
+    GBFG_CUDA(cudaEventRecord(side->ev_aux, side->s));
+    // this stream: the deposit.  Its stamps (-1) never equal those of the loop's subtractions (1 .. max_iter).
+    rc = launch_deposit(g, ct, dev_A, dev_f, dev_fdot, nullptr, nullptr, n, +1, dev_spectrum, dev_err_count,
+                        w.diff, w.tile_sums, w.wide_flag, plain_marks(w, nb, -1), st);
     if (rc) return rc;
     if (dev_total) GBFG_CUDA(cudaMemcpyAsync(dev_total, dev_spectrum, row_bytes, cudaMemcpyDeviceToDevice, st));
-    return gbfg_subtract_until_converged(grid, dev_A, dev_f, dev_fdot, offsets, n_cat, dev_s_instr, params,
-                                         dev_spectrum, dev_median, dev_psd, dev_resolved, host_results,
-                                         workspace, workspace_bytes, stream);
+    GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_aux, 0));
+    return loop_impl(grid, dev_A, dev_f, dev_fdot, offsets, n_cat, dev_s_instr, params, dev_spectrum, dev_median, dev_psd,
+                     dev_resolved, host_results, workspace, workspace_bytes, stream, true);
 }
 
 extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
