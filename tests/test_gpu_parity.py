@@ -259,7 +259,7 @@ def test_snr_threshold_decisions_on_the_definition(gb, orc, torch):
 
 
 # ------------------------------------------------------------------------------- the whole loop
-def _loop_case(gb, orc, torch, w, max_iter=None, rho_th=None, check_host=False):
+def _loop_case(gb, orc, torch, w, max_iter=None, rho_th=None, check_host=False, flags=0):
     max_iter = w.max_iter if max_iter is None else max_iter
     rho_th = w.rho_th if rho_th is None else rho_th
     w = wl.replace(w, max_iter=max_iter, rho_th=rho_th)
@@ -272,7 +272,7 @@ def _loop_case(gb, orc, torch, w, max_iter=None, rho_th=None, check_host=False):
     psd = torch.empty(nb, dtype=torch.float64, device="cuda")
     resolved = torch.empty(n, dtype=torch.uint8, device="cuda")
     err = torch.zeros(1, dtype=torch.int64, device="cuda")
-    params = gb.make_iter_params(w.window, w.median_norm, rho_th, max_iter)
+    params = gb.make_iter_params(w.window, w.median_norm, rho_th, max_iter, flags)
     res = gb.simulate(g, w.pops, w.offsets(), w.seed, s_instr, params, A, f, fd, total, spec, med, psd, resolved,
                       workspace(torch, gb, g, n), dev_err_count=err)[0]
     assert np.array_equal(bits(A.cpu().numpy()), bits(ref["A"]))
@@ -323,6 +323,14 @@ def test_loop_degenerate_thresholds_and_cap(gb, orc, torch):
     assert ref["converged"] == 0
     ref = _loop_case(gb, orc, torch, wl.dense_case("short"), max_iter=3)
     assert ref["converged"] == 0 and ref["n_iter"] == 3
+
+
+@pytest.mark.parametrize("flags", [1, 2, 3])
+def test_loop_without_the_result_preserving_optimisations(gb, orc, torch, flags):
+    """GBFG_FLAG_NO_PRESELECT (1) and GBFG_FLAG_NO_INCREMENTAL (2): pre-selection (R5) and dirty blocks
+    (R7) never change a result, so the loop without them matches the oracle exactly as the default loop does."""
+    _loop_case(gb, orc, torch, wl.dense_case("short"), flags=flags)
+    _loop_case(gb, orc, torch, wl.config(1), flags=flags)
 
 
 @pytest.mark.slow
