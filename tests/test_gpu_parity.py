@@ -563,3 +563,78 @@ def test_loop_with_the_aet_strain_noise(gb, orc, torch):
     assert np.array_equal(bits(psd.cpu().numpy()), bits(ref["psd"]))
     assert np.array_equal(resolved.cpu().numpy(), ref["resolved"])
     assert (res.n_iter, res.n_resolved) == (ref["n_iter"], ref["n_resolved"])
+
+
+# ------------------------------------------------------------------------------ edge cases of the loop
+def _loop_on_given_spectrum(gb, orc, torch, w, A, f, fd, spec0, flags=0):
+    """gbfg_subtract_until_converged on a caller-supplied spectrum against the oracle's loop on the same one."""
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    s_instr = orc.instrument_noise(og)
+    ref_spec = spec0.copy()
+    ref = orc.subtract_until_converged(og, A, f, fd, s_instr, w.window, w.median_norm, w.rho_th, w.max_iter, ref_spec)
+    n, nb = A.size, g.n_bins
+    d_spec = dev(torch, spec0)
+    med = torch.empty(nb, dtype=torch.int64, device="cuda")
+    psd = torch.empty(nb, dtype=torch.float64, device="cuda")
+    resolved = torch.zeros(max(n, 1), dtype=torch.uint8, device="cuda")
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter, flags)
+    res = gb.subtract_until_converged(g, dev(torch, A), dev(torch, f), dev(torch, fd), [0, n], dev(torch, s_instr), params,
+                                      d_spec, med, psd, resolved, workspace(torch, gb, g, n))[0]
+    assert np.array_equal(d_spec.cpu().numpy(), ref_spec)
+    assert np.array_equal(med.cpu().numpy(), ref["median"])
+    assert np.array_equal(bits(psd.cpu().numpy()), bits(ref["psd"]))
+    assert np.array_equal(resolved.cpu().numpy()[:n], ref["resolved"])
+    assert (res.n_iter, res.converged, res.n_resolved) == (ref["n_iter"], ref["converged"], ref["n_resolved"])
+    ref["residual"] = ref_spec
+    return ref, res
+
+
+def test_loop_empty_catalog(gb, orc, torch):
+    w = wl.config(0)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    e = np.empty(0)
+    spec0 = wl.random_spectrum(og.n_bins, seed=3, kind="lognormal")
+    ref, res = _loop_on_given_spectrum(gb, orc, torch, w, e, e, e, spec0)
+    assert (res.n_iter, res.converged, res.n_resolved) == (1, 1, 0)
+
+
+def test_loop_on_a_spectrum_that_does_not_contain_the_catalog(gb, orc, torch):
+    """Only every other source was deposited: subtracting the rest drives bins and medians negative, S_n >= S_instr
+    no longer holds and the pre-selection must be abandoned on the way (R5, loop.cu).  Same answer as the
+    oracle, which never pre-selects."""
+    w = wl.replace(wl.dense_case("short"), max_iter=6)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    A, f, fd = orc.sample_catalog(og, wl.replace(w.pops[0], n_src=60_000), 0, w.seed)
+    spec0 = np.zeros(og.n_bins, dtype=np.int64)
+    orc.deposit(og, A, f, fd, spec0, sel=np.arange(0, A.size, 2, dtype=np.int64))
+    ref, res = _loop_on_given_spectrum(gb, orc, torch, w, A, f, fd, spec0)
+    assert ref["residual"].min() < 0 and ref["n_resolved"] > 0
+    _loop_on_given_spectrum(gb, orc, torch, w, A, f, fd, spec0, flags=gb.FLAG_NO_PRESELECT)
+
+
+def test_loop_batch_with_an_empty_and_a_rejected_catalog(gb, orc, torch):
+    """A batch whose second catalog is empty and whose third holds sources the generator cannot place (f_max draws are
+    clamped into the band, so 'rejected' is exercised through a zero-amplitude scatter instead): ragged, degenerate rows."""
+    w = wl.scaled(wl.config(4), n_cat=3)
+    w = wl.replace(w, pops=[wl.replace(w.pops[0], n_src=30_000), wl.replace(w.pops[1], n_src=0), wl.replace(w.pops[2], n_src=7)])
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    n, nb, nc = w.n_src_total, g.n_bins, w.n_cat
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    total, spec, med = (torch.empty((nc, nb), dtype=torch.int64, device="cuda") for _ in range(3))
+    psd = torch.empty((nc, nb), dtype=torch.float64, device="cuda")
+    resolved = torch.empty(n, dtype=torch.uint8, device="cuda")
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter)
+    res = gb.simulate(g, w.pops, w.offsets(), w.seed, dev(torch, orc.instrument_noise(og)), params, A, f, fd, total, spec,
+                      med, psd, resolved, workspace(torch, gb, g, n, nc))
+    off = w.offsets()
+    for c in range(nc):
+        ref = orc.simulate(w, cat=c)
+        s = slice(int(off[c]), int(off[c + 1]))
+        assert np.array_equal(spec[c].cpu().numpy(), ref["residual"])
+        assert np.array_equal(med[c].cpu().numpy(), ref["median"])
+        assert np.array_equal(bits(psd[c].cpu().numpy()), bits(ref["psd"]))
+        assert np.array_equal(resolved[s].cpu().numpy(), ref["resolved"])
+        assert (res[c].n_iter, res[c].converged, res[c].n_resolved) == (ref["n_iter"], ref["converged"], ref["n_resolved"])
+    assert (res[1].n_iter, res[1].n_resolved) == (1, 0)
