@@ -198,3 +198,27 @@ def log_bin_edges(w: Workload, n_coarse: int = 100, f_lo: float | None = None, f
     e = np.geomspace(f_lo, f_hi, n_coarse + 1)
     idx = np.ceil((e - w.f_min) * w.t_obs - 0.5).astype(np.int64)      # first bin whose centre is >= e_k
     return np.clip(idx, 0, n_bins)
+
+
+@dataclass(frozen=True)
+class PaperPopulation:
+    """Lambda of the paper's own population model, eq. (9) PAPER.md:126 (Table I).  Defaults: the
+    parameters of Fig. 1."""
+    alpha_pl: float = -2.9
+    alpha_gamma: float = 1.96
+    beta_gamma: float = 1.8
+    mu_gamma: float = -21.0
+    mu: float = -22.0
+    sigma: float = 0.18
+    rho: float = 0.99
+    n_src: int = 0
+
+
+def paper_prior_draw(seed: int, n_src: int | None = None) -> PaperPopulation:
+    """One draw of Lambda from the priors of Table I (harness-side, numpy default_rng)."""
+    rng = np.random.default_rng(seed)
+    return PaperPopulation(alpha_pl=float(rng.uniform(-4, -2)), alpha_gamma=float(rng.uniform(1, 3)),
+                           beta_gamma=float(rng.uniform(1, 3)), mu_gamma=float(rng.uniform(-22, -20)),
+                           mu=float(rng.uniform(-23, -21)), sigma=float(rng.uniform(0.1, 0.3)),
+                           rho=float(rng.uniform(0, 1)),
+                           n_src=int(rng.uniform(5e6, 30e6)) if n_src is None else int(n_src))

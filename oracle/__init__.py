@@ -37,6 +37,12 @@ class Pop(C.Structure):
                 ("logMc_mean", C.c_double), ("logMc_sigma", C.c_double), ("n_src", C.c_int64)]
 
 
+class PopPaper(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("reserved", C.c_uint32), ("alpha_pl", C.c_double),
+                ("alpha_gamma", C.c_double), ("beta_gamma", C.c_double), ("mu_gamma", C.c_double),
+                ("mu", C.c_double), ("sigma", C.c_double), ("rho", C.c_double), ("n_src", C.c_int64)]
+
+
 class IterResult(C.Structure):
     _fields_ = [("n_iter", C.c_int32), ("converged", C.c_int32), ("n_resolved", C.c_int64),
                 ("n_near_threshold", C.c_int64)]
@@ -83,6 +89,15 @@ def lib():
         L.orc_subtract_until_converged_est.argtypes = [
             C.POINTER(Grid), dp, dp, dp, C.c_int64, dp, C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_int32,
             ip, ip, dp, up, C.POINTER(IterResult), ip]
+        L.orc_erfc_pos.restype = C.c_double
+        L.orc_erfc_pos.argtypes = [C.c_double]
+        L.orc_norm_tail.restype = C.c_double
+        L.orc_norm_tail.argtypes = [C.c_double]
+        L.orc_gamma_pq.argtypes = [C.c_double, C.c_double, C.c_double, dp, dp, dp]
+        L.orc_gamma_quantile.restype = C.c_double
+        L.orc_gamma_quantile.argtypes = [C.c_double] * 4
+        L.orc_sample_catalog_paper.argtypes = [C.POINTER(Grid), C.POINTER(PopPaper), C.c_uint32, C.c_uint64,
+                                               C.c_int64, C.c_int64, dp, dp, dp]
         L.orc_aet_noise.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, dp]
         L.orc_instrument_noise_aet.argtypes = [C.POINTER(Grid), C.c_double, C.c_double, C.c_double, C.c_int, dp, dp, dp, dp]
         L.orc_running_sum_def.argtypes = [ip, C.c_int64, C.c_int32, C.c_int64, C.c_int64, ip]
@@ -205,6 +220,44 @@ def running_median(x: np.ndarray, window: int) -> np.ndarray:
     if rc:
         raise ValueError("invalid window / size")
     return out
+
+
+def erfc_pos(t: float) -> float:
+    return lib().orc_erfc_pos(t)
+
+
+def norm_tail(z: float) -> float:
+    """Phi(z) for z <= 0, 1 - Phi(z) for z > 0."""
+    return lib().orc_norm_tail(z)
+
+
+def gamma_pq(a: float, x: float):
+    """(P(a,x), Q(a,x)) regularized incomplete gamma functions."""
+    import math
+    P, Q, pref = C.c_double(), C.c_double(), C.c_double()
+    lib().orc_gamma_pq(a, x, math.lgamma(a), C.byref(P), C.byref(Q), C.byref(pref))
+    return P.value, Q.value
+
+
+def gamma_quantile(a: float, z: float) -> float:
+    """x with P(a, x) = Phi(z)."""
+    import math
+    return lib().orc_gamma_quantile(a, math.lgamma(a), math.lgamma(a + 1.0), z)
+
+
+def make_pop_paper(p) -> PopPaper:
+    return PopPaper(C.sizeof(PopPaper), 0, p.alpha_pl, p.alpha_gamma, p.beta_gamma, p.mu_gamma, p.mu, p.sigma, p.rho, p.n_src)
+
+
+def sample_catalog_paper(grid: Grid, pop, cat_id: int, seed: int, i_begin: int = 0, i_end: int | None = None):
+    """The paper's population sampler (Table I, eqs. 7-9, Gaussian copula): -> (A, f, fdot)."""
+    pp = pop if isinstance(pop, PopPaper) else make_pop_paper(pop)
+    if i_end is None:
+        i_end = pp.n_src
+    n = i_end - i_begin
+    A, f, fd = (np.empty(n, dtype=np.float64) for _ in range(3))
+    lib().orc_sample_catalog_paper(C.byref(grid), C.byref(pp), cat_id, seed, i_begin, i_end, _d(A), _d(f), _d(fd))
+    return A, f, fd
 
 
 def aet_noise(f: float, P: float = 15.0, A: float = 3.0, L: float = 2.5e9, tdi2: bool = True):

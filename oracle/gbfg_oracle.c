@@ -291,6 +291,157 @@ void orc_sample_catalog(const orc_grid *g, const orc_pop *pop, uint32_t cat_id, 
 }
 
 /* ------------------------------------------------------------------------------------ */
+/* The paper's own population sampler (R12): Table I            */
+/* (PAPER.md:81-87), eqs. (7)-(9), Gaussian copula of Appendix A steps     */
+/* (iii)-(iv).  Elementary functions as DESIGN.md R12 lists them.          */
+/* ------------------------------------------------------------------------------------ */
+static double orc_expn(double y) { return orc_exp10(y * ORC_LOG10_E); }   /* e^y */
+
+/* erfc(t), t >= 0: for t < 2 the all-positive series erf t = (2/sqrt pi) e^{-t^2} sum 2^n t^{2n+1} / (2n+1)!!
+ * (80 terms), else the continued fraction e^{-t^2} / (sqrt pi (t + (1/2)/(t + 1/(t + (3/2)/(t + ...))))), depth 40,
+ * evaluated from the bottom */
+double orc_erfc_pos(double t)
+{
+    const double SQRT_PI = 1.7724538509055159;
+    double t2 = t * t;
+    if (t < 2.0) {
+        double term = t, sum = t;
+        for (int n = 1; n < 80; ++n) {
+            term = term * (2.0 * t2) / (double)(2 * n + 1);
+            sum = sum + term;
+        }
+        return 1.0 - (2.0 / SQRT_PI) * orc_expn(-t2) * sum;
+    }
+    double r = t;
+    for (int k = 40; k >= 1; --k) r = t + (0.5 * (double)k) / r;
+    return orc_expn(-t2) / (SQRT_PI * r);
+}
+
+/* tail probability of a standard normal beyond z on z's own side: Phi(z) for z <= 0, 1 - Phi(z) for z > 0 */
+double orc_norm_tail(double z)
+{
+    return 0.5 * orc_erfc_pos(fabs(z) * 0.7071067811865476);
+}
+
+/* regularized incomplete gamma functions P(a,x), Q(a,x) and the prefactor x^a e^-x / Gamma(a); lg = ln Gamma(a).
+ * x < a + 3: series P = pref * sum_{n>=0} x^n / (a (a+1) ... (a+n)), 100 terms, Q = 1 - P;
+ * else Legendre's continued fraction Q = pref / (x+1-a - 1(1-a)/(x+3-a - 2(2-a)/(x+5-a - ...))), depth 120, P = 1 - Q */
+void orc_gamma_pq(double a, double x, double lg, double *P, double *Q, double *pref_out)
+{
+    double pref = orc_expn((a * orc_log(x) - x) - lg);
+    if (x < a + 3.0) {
+        double term = 1.0 / a, sum = term;
+        for (int n = 1; n <= 100; ++n) {
+            term = term * x / (a + (double)n);
+            sum = sum + term;
+        }
+        *P = sum * pref;
+        *Q = 1.0 - *P;
+    } else {
+        double r = (x + 241.0) - a;
+        for (int k = 120; k >= 1; --k) r = ((x + (double)(2 * k - 1)) - a) - ((double)k * ((double)k - a)) / r;
+        *Q = pref / r;
+        *P = 1.0 - *Q;
+    }
+    *pref_out = pref;
+}
+
+/* x with P(a,x) = Phi(z): Wilson-Hilferty start from z, then 14 Newton steps on the logarithm of the tail
+ * probability on z's side (P for z <= 0, Q for z > 0), each step kept within [x/10, 2x + 4].
+ * lg = ln Gamma(a), lg1 = ln Gamma(a + 1). */
+double orc_gamma_quantile(double a, double lg, double lg1, double z)
+{
+    double tail = orc_norm_tail(z);
+    double c = 1.0 / (9.0 * a);
+    double w = (1.0 - c) + z * sqrt(c);
+    double x = a * ((w * w) * w);
+    if (!(w > 0.0) || x < 1e-6 * a) x = orc_expn((orc_log(tail) + lg1) / a);   /* far lower tail: P ~ x^a / Gamma(a+1) */
+    for (int it = 0; it < 14; ++it) {
+        double P, Q, pref;
+        orc_gamma_pq(a, x, lg, &P, &Q, &pref);
+        double pdf = pref / x;
+        double g = (z <= 0.0) ? P * orc_log(P / tail) : -(Q * orc_log(Q / tail));
+        double xn = x - g / pdf;
+        if (xn < 0.1 * x) xn = 0.1 * x;
+        if (xn > 2.0 * x + 4.0) xn = 2.0 * x + 4.0;
+        x = xn;
+    }
+    return x;
+}
+
+typedef struct {
+    uint32_t struct_size, reserved;
+    double alpha_pl;       /* p(f) ∝ f^alpha_pl on the grid's band (Table I) */
+    double alpha_gamma, beta_gamma, mu_gamma;   /* log10(fdot) - mu_gamma ~ Gamma(alpha, rate beta), eq. (7) */
+    double mu, sigma;      /* log10[(f/Hz)^(-2/3) A] - mu ~ LogNormal(0, sigma), eq. (8) */
+    double rho;            /* Gaussian-copula correlation of f and fdot, eqs. (A4)-(A5) */
+    int64_t n_src;
+} orc_pop_paper;
+
+void orc_sample_catalog_paper(const orc_grid *g, const orc_pop_paper *pop, uint32_t cat_id, uint64_t seed,
+                              int64_t i_begin, int64_t i_end, double *A, double *f, double *fdot)
+{
+    const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+    const double lfmin = orc_log(g->f_min) * ORC_LOG10_E;
+    const double lfmax = orc_log(g->f_max) * ORC_LOG10_E;
+    const double f_top = nextafter(g->f_max, 0.0);
+    const double oms = 1.0 + pop->alpha_pl;              /* exponent of the CDF: f^(1 + alpha) */
+    const int flat_in_log = fabs(oms) < 1e-12;
+    double c0, c1, c2;
+    if (flat_in_log) {
+        c0 = lfmin; c1 = lfmax - lfmin; c2 = 1.0;
+    } else {
+        double a = orc_exp10(oms * lfmin);
+        double b = orc_exp10(oms * lfmax);
+        c0 = a; c1 = b - a; c2 = 1.0 / oms;
+    }
+    const double lg = lgamma(pop->alpha_gamma), lg1 = lgamma(pop->alpha_gamma + 1.0);
+    const double rho_c = sqrt(1.0 - pop->rho * pop->rho);
+    for (int64_t i = i_begin; i < i_end; ++i) {
+        uint32_t ctr[4] = {(uint32_t)i, (uint32_t)((uint64_t)i >> 32), 2u, cat_id};   /* blocks 2 and 3 */
+        uint32_t w0[4], w1[4];
+        orc_philox4x32_10(ctr, key, w0);
+        ctr[2] = 3u;
+        orc_philox4x32_10(ctr, key, w1);
+        double u_1 = orc_u01(w0[0], w0[1]), u_2 = orc_u01(w0[2], w0[3]);
+        double u_3 = orc_u01(w1[0], w1[1]), u_4 = orc_u01(w1[2], w1[3]);
+        double r = sqrt(-2.0 * orc_log(u_1));
+        double sn, cs;
+        orc_sincos2pi(u_2, &sn, &cs);
+        double n1 = r * cs, n2 = r * sn;
+        double r3 = sqrt(-2.0 * orc_log(u_3));
+        double s3, c3;
+        orc_sincos2pi(u_4, &s3, &c3);
+        double z3 = r3 * c3;
+        /* step (iii): (z1, z2) ~ N(0, Sigma) */
+        double z1 = n1;
+        double z2 = pop->rho * n1 + rho_c * n2;
+        /* step (iv), frequency: u' = Phi(z1) through the inverse CDF of the truncated power law */
+        double t1 = orc_norm_tail(z1);
+        double uf = (z1 <= 0.0) ? t1 : 1.0 - t1;
+        double lf;
+        if (flat_in_log) {
+            lf = c0 + uf * c1;
+        } else {
+            double x = c0 + uf * c1;
+            lf = (orc_log(x) * ORC_LOG10_E) * c2;
+        }
+        double fi = orc_exp10(lf);
+        if (fi < g->f_min) fi = g->f_min;
+        if (fi >= g->f_max) fi = f_top;
+        /* step (iv), chirp: v' = Phi(z2) through the inverse Gamma CDF, eq. (7) */
+        double xg = orc_gamma_quantile(pop->alpha_gamma, lg, lg1, z2);
+        double fd = orc_exp10(pop->mu_gamma + xg / pop->beta_gamma);
+        /* amplitude, eq. (8): A~ = exp(sigma z3) (log-normal), log10 A = mu + A~ + (2/3) log10(f / Hz) */
+        double at = orc_expn(pop->sigma * z3);
+        double Ai = orc_exp10((pop->mu + at) + (2.0 / 3.0) * lf);
+        A[i - i_begin] = Ai;
+        f[i - i_begin] = fi;
+        fdot[i - i_begin] = fd;
+    }
+}
+
+/* ------------------------------------------------------------------------------------ */
 /* Instrument noise: Robson, Cornish & Liu 2019 sky-averaged curve (PAPER.md:670 ref [70]) */
 /* with BASELINE.json:configs[0]'s constants, at bin centres.  DESIGN.md R3.              */
 /* ------------------------------------------------------------------------------------ */
