@@ -66,6 +66,16 @@ typedef struct gbfg_pop {
     int64_t n_src;
 } gbfg_pop;
 
+/* Population parameters Lambda of the paper's own model, eq. (9) PAPER.md:126 (Table I; R12):
+ *   p(f) ∝ f^alpha_pl on the grid's band;  log10(fdot / Hz s^-1) - mu_gamma ~ Gamma(alpha_gamma, rate beta_gamma) (eq. 7);
+ *   log10[(f/Hz)^(-2/3) A] - mu ~ LogNormal(0, sigma) (eq. 8);  (f, fdot) tied by a Gaussian copula of correlation rho. */
+typedef struct gbfg_pop_paper {
+    uint32_t struct_size;   /* = sizeof(gbfg_pop_paper) */
+    uint32_t reserved;
+    double alpha_pl, alpha_gamma, beta_gamma, mu_gamma, mu, sigma, rho;
+    int64_t n_src;
+} gbfg_pop_paper;
+
 /* Parameters of the subtraction loop (R3, R4, R6). */
 typedef struct gbfg_iter_params {
     uint32_t struct_size;   /* = sizeof(gbfg_iter_params) */
@@ -123,6 +133,13 @@ int gbfg_instrument_noise_aet(const gbfg_grid *grid, double P_pm, double A_fm, d
 int gbfg_sample_catalog(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets,
                         int32_t n_cat, uint32_t first_cat_id, uint64_t seed,
                         double *dev_A, double *dev_f, double *dev_fdot, void *stream);
+
+/* Stage (i) with the paper's own population model (Table I, eqs. 7-9, Gaussian copula of Appendix A steps iii-iv,
+ * PAPER.md:454-457; R12).  Same conventions as gbfg_sample_catalog (Philox counter blocks 2 and 3, so the two
+ * samplers never share a random number); alpha_gamma, beta_gamma > 0, sigma >= 0, 0 <= rho < 1 (INVALID_ARG otherwise). */
+int gbfg_sample_catalog_paper(const gbfg_grid *grid, const gbfg_pop_paper *pops, const int64_t *offsets,
+                              int32_t n_cat, uint32_t first_cat_id, uint64_t seed,
+                              double *dev_A, double *dev_f, double *dev_fdot, void *stream);
 
 /* Stage (ii)/(v) — deposit (sign = +1) or subtract (sign = -1) source power (R2;
  * subtraction is eq. (D4)): for every addressed source

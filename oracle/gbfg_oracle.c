@@ -324,29 +324,29 @@ double orc_norm_tail(double z)
 }
 
 /* regularized incomplete gamma functions P(a,x), Q(a,x) and the prefactor x^a e^-x / Gamma(a); lg = ln Gamma(a).
- * x < a + 3: series P = pref * sum_{n>=0} x^n / (a (a+1) ... (a+n)), 100 terms, Q = 1 - P;
- * else Legendre's continued fraction Q = pref / (x+1-a - 1(1-a)/(x+3-a - 2(2-a)/(x+5-a - ...))), depth 120, P = 1 - Q */
+ * x < a + 3: series P = pref * sum_{n>=0} x^n / (a (a+1) ... (a+n)), 48 terms, Q = 1 - P;
+ * else Legendre's continued fraction Q = pref / (x+1-a - 1(1-a)/(x+3-a - 2(2-a)/(x+5-a - ...))), depth 40, P = 1 - Q */
 void orc_gamma_pq(double a, double x, double lg, double *P, double *Q, double *pref_out)
 {
     double pref = orc_expn((a * orc_log(x) - x) - lg);
     if (x < a + 3.0) {
         double term = 1.0 / a, sum = term;
-        for (int n = 1; n <= 100; ++n) {
+        for (int n = 1; n <= 48; ++n) {
             term = term * x / (a + (double)n);
             sum = sum + term;
         }
         *P = sum * pref;
         *Q = 1.0 - *P;
     } else {
-        double r = (x + 241.0) - a;
-        for (int k = 120; k >= 1; --k) r = ((x + (double)(2 * k - 1)) - a) - ((double)k * ((double)k - a)) / r;
+        double r = (x + 81.0) - a;
+        for (int k = 40; k >= 1; --k) r = ((x + (double)(2 * k - 1)) - a) - ((double)k * ((double)k - a)) / r;
         *Q = pref / r;
         *P = 1.0 - *Q;
     }
     *pref_out = pref;
 }
 
-/* x with P(a,x) = Phi(z): Wilson-Hilferty start from z, then 14 Newton steps on the logarithm of the tail
+/* x with P(a,x) = Phi(z): Wilson-Hilferty start from z, then 10 Newton steps on the logarithm of the tail
  * probability on z's side (P for z <= 0, Q for z > 0), each step kept within [x/10, 2x + 4].
  * lg = ln Gamma(a), lg1 = ln Gamma(a + 1). */
 double orc_gamma_quantile(double a, double lg, double lg1, double z)
@@ -356,7 +356,7 @@ double orc_gamma_quantile(double a, double lg, double lg1, double z)
     double w = (1.0 - c) + z * sqrt(c);
     double x = a * ((w * w) * w);
     if (!(w > 0.0) || x < 1e-6 * a) x = orc_expn((orc_log(tail) + lg1) / a);   /* far lower tail: P ~ x^a / Gamma(a+1) */
-    for (int it = 0; it < 14; ++it) {
+    for (int it = 0; it < 10; ++it) {
         double P, Q, pref;
         orc_gamma_pq(a, x, lg, &P, &Q, &pref);
         double pdf = pref / x;

@@ -26,6 +26,7 @@ EXPORTS = [
     "gbfg_subtract_until_converged", "gbfg_simulate", "gbfg_simulate_host", "gbfg_workspace_bytes",
     "gbfg_kernel_launch_count", "gbfg_profile_enable", "gbfg_profile_read", "gbfg_release_cached",
     "gbfg_running_mean", "gbfg_coarse_grain", "gbfg_instrument_noise_aet",
+    "gbfg_sample_catalog_paper",
 ]
 
 KERNEL_CLASSES = ["sample", "noise", "deposit", "scan", "median", "psd", "inv_blocks", "snr", "aux"]
@@ -46,6 +47,12 @@ class Pop(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("reserved", C.c_uint32), ("slope", C.c_double),
                 ("logA_offset", C.c_double), ("logA_sigma", C.c_double), ("logMc_mean", C.c_double),
                 ("logMc_sigma", C.c_double), ("n_src", C.c_int64)]
+
+
+class PopPaper(C.Structure):
+    _fields_ = [("struct_size", C.c_uint32), ("reserved", C.c_uint32), ("alpha_pl", C.c_double),
+                ("alpha_gamma", C.c_double), ("beta_gamma", C.c_double), ("mu_gamma", C.c_double),
+                ("mu", C.c_double), ("sigma", C.c_double), ("rho", C.c_double), ("n_src", C.c_int64)]
 
 
 class IterParams(C.Structure):
@@ -88,6 +95,7 @@ def load():
     L.gbfg_instrument_noise.argtypes = [gp, vp, vp]
     L.gbfg_instrument_noise_aet.argtypes = [gp, dbl, dbl, dbl, i32, vp, vp, vp, vp, vp]
     L.gbfg_sample_catalog.argtypes = [gp, pp, op, i32, u32, u64, vp, vp, vp, vp]
+    L.gbfg_sample_catalog_paper.argtypes = [gp, C.POINTER(PopPaper), op, i32, u32, u64, vp, vp, vp, vp]
     L.gbfg_deposit.argtypes = [gp, vp, vp, vp, op, i32, vp, vp, i32, vp, vp, vp, sz, vp]
     L.gbfg_running_median.argtypes = [vp, i64, i32, i32, vp, vp]
     L.gbfg_psd.argtypes = [vp, vp, i64, i32, dbl, i32, vp, vp]
@@ -188,6 +196,19 @@ def workspace_bytes(grid: Grid, n_src_total: int, n_cat: int = 1) -> int:
 
 def instrument_noise(grid: Grid, dev_s_instr, stream=None):
     _check(load().gbfg_instrument_noise(C.byref(grid), _ptr(dev_s_instr), _stream(stream)))
+
+
+def make_pop_paper(p) -> PopPaper:
+    """From any object with the fields of gbfg_pop_paper (e.g. gbfg_workloads.PaperPopulation)."""
+    return PopPaper(C.sizeof(PopPaper), 0, p.alpha_pl, p.alpha_gamma, p.beta_gamma, p.mu_gamma, p.mu, p.sigma, p.rho, p.n_src)
+
+
+def sample_catalog_paper(grid: Grid, pops, offsets, seed: int, dev_A, dev_f, dev_fdot, first_cat_id: int = 0, stream=None):
+    arr = (PopPaper * len(pops))()
+    for i, p in enumerate(pops):
+        arr[i] = p if isinstance(p, PopPaper) else make_pop_paper(p)
+    _check(load().gbfg_sample_catalog_paper(C.byref(grid), arr, _offsets(offsets), len(pops), first_cat_id, seed,
+                                            _ptr(dev_A), _ptr(dev_f), _ptr(dev_fdot), _stream(stream)))
 
 
 def instrument_noise_aet(grid: Grid, dev_S_AA=None, dev_S_TT=None, dev_Sh_AA=None, dev_Sh_TT=None, P_pm: float = 15.0,

@@ -257,6 +257,137 @@ instrument_noise_kernel(double f_min, double T, int64_t n_bins, double *__restri
     }
 }
 
+// ------------------------------------------------------------------------------ DESIGN.md R12
+// The paper's own population sampler: Table I, eqs. (7)-(9), Gaussian copula (App. A).
+#define GB_SQRT_PI 1.7724538509055159
+#define GB_INV_SQRT2 0.7071067811865476
+
+__host__ __device__ inline double det_expn(double y) { return det_exp10(y * GB_LOG10_E); }
+
+// erfc(t), t >= 0: all-positive series below 2, continued fraction of depth 40 from the bottom above
+__host__ __device__ inline double det_erfc_pos(double t)
+{
+    const double t2 = t * t;
+    if (t < 2.0) {
+        double term = t, sum = t;
+        for (int n = 1; n < 80; ++n) {
+            term = term * (2.0 * t2) / (double)(2 * n + 1);
+            sum = sum + term;
+        }
+        return 1.0 - (2.0 / GB_SQRT_PI) * det_expn(-t2) * sum;
+    }
+    double r = t;
+    for (int k = 40; k >= 1; --k) r = t + (0.5 * (double)k) / r;
+    return det_expn(-t2) / (GB_SQRT_PI * r);
+}
+
+// Phi(z) for z <= 0, 1 - Phi(z) for z > 0
+__host__ __device__ inline double det_norm_tail(double z)
+{
+    return 0.5 * det_erfc_pos(fabs(z) * GB_INV_SQRT2);
+}
+
+// P(a,x), Q(a,x), x^a e^-x / Gamma(a): series (48 terms) below a + 3, Legendre's continued fraction (depth 40) above
+__host__ __device__ inline void det_gamma_pq(double a, double x, double lg, double &P, double &Q, double &pref)
+{
+    pref = det_expn((a * det_log(x) - x) - lg);
+    if (x < a + 3.0) {
+        double term = 1.0 / a, sum = term;
+        for (int n = 1; n <= 48; ++n) {
+            term = term * x / (a + (double)n);
+            sum = sum + term;
+        }
+        P = sum * pref;
+        Q = 1.0 - P;
+    } else {
+        double r = (x + 81.0) - a;
+        for (int k = 40; k >= 1; --k) r = ((x + (double)(2 * k - 1)) - a) - ((double)k * ((double)k - a)) / r;
+        Q = pref / r;
+        P = 1.0 - Q;
+    }
+}
+
+// x with P(a,x) = Phi(z): Wilson-Hilferty start, 10 Newton steps on the log of the tail probability on z's side
+__host__ __device__ inline double det_gamma_quantile(double a, double lg, double lg1, double z)
+{
+    const double tail = det_norm_tail(z);
+    const double c = 1.0 / (9.0 * a);
+    const double w = (1.0 - c) + z * sqrt(c);
+    double x = a * ((w * w) * w);
+    if (!(w > 0.0) || x < 1e-6 * a) x = det_expn((det_log(tail) + lg1) / a);
+    for (int it = 0; it < 10; ++it) {
+        double P, Q, pref;
+        det_gamma_pq(a, x, lg, P, Q, pref);
+        const double pdf = pref / x;
+        const double g = (z <= 0.0) ? P * det_log(P / tail) : -(Q * det_log(Q / tail));
+        double xn = x - g / pdf;
+        if (xn < 0.1 * x) xn = 0.1 * x;
+        if (xn > 2.0 * x + 4.0) xn = 2.0 * x + 4.0;
+        x = xn;
+    }
+    return x;
+}
+
+struct PopPaperDev {
+    double c0, c1, c2;          // frequency draw
+    int flat_in_log;
+    double alpha_gamma, beta_gamma, mu_gamma, lg, lg1;
+    double mu, sigma, rho, rho_c;
+    double f_min, f_max, f_top;
+    int64_t n_src;
+    uint32_t cat_id, key0, key1;
+};
+
+__device__ __forceinline__ void draw_source_paper(const PopPaperDev &P, int64_t i, double &A, double &f, double &fdot)
+{
+    U4 ctr;
+    ctr.x = (uint32_t)i; ctr.y = (uint32_t)((uint64_t)i >> 32); ctr.z = 2u; ctr.w = P.cat_id;
+    const U4 b0 = philox4x32_10(ctr, P.key0, P.key1);
+    ctr.z = 3u;
+    const U4 b1 = philox4x32_10(ctr, P.key0, P.key1);
+    const double u_1 = u01(b0.x, b0.y), u_2 = u01(b0.z, b0.w);
+    const double u_3 = u01(b1.x, b1.y), u_4 = u01(b1.z, b1.w);
+    const double r = sqrt(-2.0 * det_log(u_1));
+    double sn, cs;
+    det_sincos2pi(u_2, sn, cs);
+    const double n1 = r * cs, n2 = r * sn;
+    const double r3 = sqrt(-2.0 * det_log(u_3));
+    double s3, c3;
+    det_sincos2pi(u_4, s3, c3);
+    const double z3 = r3 * c3;
+    const double z1 = n1;
+    const double z2 = P.rho * n1 + P.rho_c * n2;
+    const double t1 = det_norm_tail(z1);
+    const double uf = (z1 <= 0.0) ? t1 : 1.0 - t1;
+    double lf;
+    if (P.flat_in_log) {
+        lf = P.c0 + uf * P.c1;
+    } else {
+        const double x = P.c0 + uf * P.c1;
+        lf = (det_log(x) * GB_LOG10_E) * P.c2;
+    }
+    double fi = det_exp10(lf);
+    if (fi < P.f_min) fi = P.f_min;
+    if (fi >= P.f_max) fi = P.f_top;
+    const double xg = det_gamma_quantile(P.alpha_gamma, P.lg, P.lg1, z2);
+    fdot = det_exp10(P.mu_gamma + xg / P.beta_gamma);
+    const double at = det_expn(P.sigma * z3);
+    A = det_exp10((P.mu + at) + (2.0 / 3.0) * lf);
+    f = fi;
+}
+
+__global__ void __launch_bounds__(128)
+sample_paper_kernel(PopPaperDev P, double *__restrict__ A, double *__restrict__ f, double *__restrict__ fdot)
+{
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (; i < P.n_src; i += stride) {
+        double a, fr, fd;
+        draw_source_paper(P, i, a, fr, fd);
+        A[i] = a; f[i] = fr; fdot[i] = fd;
+    }
+}
+
 // SciRDv1 noise of the TDI channels and its rescaling by the response (R11; eqs. C1-C5
 // PAPER.md:494-509, B2-B5 PAPER.md:475-487), operation by operation as R11 lists them.
 struct AetOut { double s_aa, s_tt, sh_aa, sh_tt; };
@@ -357,6 +488,59 @@ extern "C" int gbfg_instrument_noise_aet(const gbfg_grid *grid, double P_pm, dou
                                                                               L_m, tdi2 ? 1 : 0, dev_S_AA, dev_S_TT, dev_Sh_AA, dev_Sh_TT);
     }
     GBFG_LAUNCH_CHECK("instrument_noise_aet_kernel");
+    return GBFG_OK;
+}
+
+extern "C" int gbfg_sample_catalog_paper(const gbfg_grid *grid, const gbfg_pop_paper *pops, const int64_t *offsets,
+                                         int32_t n_cat, uint32_t first_cat_id, uint64_t seed,
+                                         double *dev_A, double *dev_f, double *dev_fdot, void *stream)
+{
+    if (!grid || grid->struct_size != sizeof(gbfg_grid) || !pops || !offsets) return GBFG_ERR_INVALID_ARG;
+    if (n_cat < 1) return GBFG_ERR_INVALID_ARG;
+    if (n_cat > GBFG_MAX_CAT) return GBFG_ERR_UNSUPPORTED;
+    if (offsets[0] != 0) return GBFG_ERR_INVALID_ARG;
+    for (int c = 0; c < n_cat; ++c) {
+        const gbfg_pop_paper &p = pops[c];
+        if (p.struct_size != sizeof(gbfg_pop_paper) || p.n_src < 0) return GBFG_ERR_INVALID_ARG;
+        if (offsets[c + 1] - offsets[c] != p.n_src) return GBFG_ERR_INVALID_ARG;
+        if (!(p.alpha_gamma > 0.0) || !(p.beta_gamma > 0.0) || !(p.sigma >= 0.0) || !(p.rho >= 0.0) || !(p.rho < 1.0))
+            return GBFG_ERR_INVALID_ARG;
+    }
+    if (offsets[n_cat] > 0 && (!dev_A || !dev_f || !dev_fdot)) return GBFG_ERR_INVALID_ARG;
+    int rc = check_device();
+    if (rc) return rc;
+    const double lfmin = det_log(grid->f_min) * GB_LOG10_E;
+    const double lfmax = det_log(grid->f_max) * GB_LOG10_E;
+    for (int c = 0; c < n_cat; ++c) {
+        const gbfg_pop_paper &p = pops[c];
+        if (p.n_src == 0) continue;
+        PopPaperDev P;
+        const double oms = 1.0 + p.alpha_pl;
+        P.flat_in_log = fabs(oms) < 1e-12;
+        if (P.flat_in_log) {
+            P.c0 = lfmin; P.c1 = lfmax - lfmin; P.c2 = 1.0;
+        } else {
+            const double a = det_exp10(oms * lfmin);
+            const double b = det_exp10(oms * lfmax);
+            P.c0 = a; P.c1 = b - a; P.c2 = 1.0 / oms;
+        }
+        P.alpha_gamma = p.alpha_gamma; P.beta_gamma = p.beta_gamma; P.mu_gamma = p.mu_gamma;
+        P.lg = lgamma(p.alpha_gamma); P.lg1 = lgamma(p.alpha_gamma + 1.0);
+        P.mu = p.mu; P.sigma = p.sigma; P.rho = p.rho; P.rho_c = sqrt(1.0 - p.rho * p.rho);
+        P.f_min = grid->f_min; P.f_max = grid->f_max; P.f_top = nextafter(grid->f_max, 0.0);
+        P.n_src = p.n_src;
+        P.cat_id = first_cat_id + (uint32_t)c;
+        P.key0 = (uint32_t)seed; P.key1 = (uint32_t)(seed >> 32);
+        int64_t blocks = (p.n_src + 127) / 128;
+        const int64_t cap = (int64_t)sm_count() * 16;
+        if (blocks > cap) blocks = cap;
+        {
+            LaunchTimer lt(K_SAMPLE, (cudaStream_t)stream);
+            sample_paper_kernel<<<(int)blocks, 128, 0, (cudaStream_t)stream>>>(P, dev_A + offsets[c], dev_f + offsets[c],
+                                                                              dev_fdot + offsets[c]);
+        }
+        GBFG_LAUNCH_CHECK("sample_paper_kernel");
+    }
     return GBFG_OK;
 }
 

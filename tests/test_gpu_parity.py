@@ -638,3 +638,48 @@ def test_loop_batch_with_an_empty_and_a_rejected_catalog(gb, orc, torch):
         assert np.array_equal(resolved[s].cpu().numpy(), ref["resolved"])
         assert (res[c].n_iter, res[c].converged, res[c].n_resolved) == (ref["n_iter"], ref["converged"], ref["n_resolved"])
     assert (res[1].n_iter, res[1].n_resolved) == (1, 0)
+
+
+# ------------------------------------------------ the paper's population sampler (R12)
+@pytest.mark.parametrize("case", ["fig1", "priors", "flat_in_log", "batch"])
+def test_sample_catalog_paper_bit_exact(gb, orc, torch, case):
+    w = wl.config(1)                                          # 0.1-10 mHz: the band of Table I
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    if case == "fig1":
+        pops = [wl.PaperPopulation(n_src=150_001)]
+    elif case == "priors":
+        pops = [wl.paper_prior_draw(s, n_src=40_000) for s in (1, 2, 3)]
+    elif case == "flat_in_log":
+        pops = [wl.replace(wl.PaperPopulation(n_src=30_000), alpha_pl=-1.0, rho=0.0, sigma=0.0)]
+    else:
+        pops = [wl.PaperPopulation(n_src=777), wl.replace(wl.PaperPopulation(n_src=0), rho=0.5),
+                wl.replace(wl.PaperPopulation(n_src=12_345), alpha_gamma=1.0, beta_gamma=3.0, rho=0.3)]
+    off = np.concatenate([[0], np.cumsum([p.n_src for p in pops])]).astype(np.int64)
+    n = int(off[-1])
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    gb.sample_catalog_paper(g, pops, off, 5, A, f, fd, first_cat_id=4)
+    for c, p in enumerate(pops):
+        rA, rf, rfd = orc.sample_catalog_paper(og, p, 4 + c, 5)
+        s = slice(int(off[c]), int(off[c + 1]))
+        assert np.array_equal(bits(A[s].cpu().numpy()), bits(rA))
+        assert np.array_equal(bits(f[s].cpu().numpy()), bits(rf))
+        assert np.array_equal(bits(fd[s].cpu().numpy()), bits(rfd))
+
+
+def test_paper_catalog_through_the_loop(gb, orc, torch):
+    """A catalog drawn from the paper's model (Fig. 1 parameters) goes through deposit and loop like any other."""
+    w = wl.replace(wl.config(1), max_iter=8)
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    pop = wl.PaperPopulation(n_src=200_000)
+    n = pop.n_src
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    gb.sample_catalog_paper(g, [pop], [0, n], 9, A, f, fd)
+    hA, hf, hfd = A.cpu().numpy(), f.cpu().numpy(), fd.cpu().numpy()
+    spec0 = np.zeros(og.n_bins, dtype=np.int64)
+    orc.deposit(og, hA, hf, hfd, spec0)
+    d_spec = torch.zeros(g.n_bins, dtype=torch.int64, device="cuda")
+    gb.deposit(g, A, f, fd, [0, n], d_spec, workspace(torch, gb, g, n))
+    assert np.array_equal(d_spec.cpu().numpy(), spec0)
+    _loop_on_given_spectrum(gb, orc, torch, w, hA, hf, hfd, spec0)
