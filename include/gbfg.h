@@ -237,7 +237,8 @@ int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, const int64_
                        double *host_psd, uint8_t *host_resolved, gbfg_iter_result *host_results);
 
 /* gbfg_simulate_host keeps its device arena and stream between calls of the same host thread, so that
- * repeated calls do not pay cudaMalloc / cudaFree; this frees them (synchronises the stream first). */
+ * repeated calls do not pay cudaMalloc / cudaFree; this frees them (synchronises the stream first), together with
+ * the side stream and events the loop keeps per host thread. */
 int gbfg_release_cached(void);
 
 /* Bytes of device workspace sufficient for any call above on this grid / batch. */

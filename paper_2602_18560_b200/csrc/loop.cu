@@ -166,9 +166,15 @@ static cudaEvent_t readback_event()
 
 // side stream on which the plan of the next pass runs next to the scan of the subtraction (one per host thread)
 struct SideStream { cudaStream_t s; cudaEvent_t ev_plan, ev_aux; };
-static SideStream *side_stream()
+static SideStream &side_stream_slot()
 {
     static thread_local SideStream ss = {nullptr, nullptr, nullptr};
+    return ss;
+}
+static SideStream *side_stream_if_any() { return side_stream_slot().s ? &side_stream_slot() : nullptr; }
+static SideStream *side_stream()
+{
+    SideStream &ss = side_stream_slot();
     if (!ss.s) {
         if (cudaStreamCreateWithFlags(&ss.s, cudaStreamNonBlocking) != cudaSuccess ||
             cudaEventCreateWithFlags(&ss.ev_plan, cudaEventDisableTiming) != cudaSuccess ||
@@ -595,5 +601,13 @@ extern "C" int gbfg_release_cached(void)
     HostCallCache &cc = host_call_cache();
     if (cc.stream) { cudaStreamSynchronize(cc.stream); cudaStreamDestroy(cc.stream); cc.stream = nullptr; }
     if (cc.base) { cudaFree(cc.base); cc.base = nullptr; cc.bytes = 0; }
+    SideStream *side = side_stream_if_any();
+    if (side) {                                          // the loop's side stream and its events
+        cudaStreamSynchronize(side->s);
+        cudaEventDestroy(side->ev_plan);
+        cudaEventDestroy(side->ev_aux);
+        cudaStreamDestroy(side->s);
+        side->s = nullptr;
+    }
     return GBFG_OK;
 }

@@ -683,3 +683,19 @@ def test_paper_catalog_through_the_loop(gb, orc, torch):
     gb.deposit(g, A, f, fd, [0, n], d_spec, workspace(torch, gb, g, n))
     assert np.array_equal(d_spec.cpu().numpy(), spec0)
     _loop_on_given_spectrum(gb, orc, torch, w, hA, hf, hfd, spec0)
+
+
+def test_release_cached_and_reuse(gb, orc, torch):
+    """gbfg_release_cached frees the host-call arena and the loop's side stream; the next calls rebuild them."""
+    w = wl.config(0)
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    s_instr = orc.instrument_noise(og)
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter)
+    hp1, hp2 = (np.empty(g.n_bins, dtype=np.float64) for _ in range(2))
+    gb.simulate_host(g, w.pops, w.offsets(), w.seed, s_instr, params, hp1)
+    gb.release_cached()
+    gb.release_cached()                                    # idempotent
+    gb.simulate_host(g, w.pops, w.offsets(), w.seed, s_instr, params, hp2)
+    assert np.array_equal(bits(hp1), bits(hp2))
+    _loop_case(gb, orc, torch, w)
