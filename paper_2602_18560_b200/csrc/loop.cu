@@ -578,7 +578,11 @@ extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, c
     cudaStream_t st = cc.stream;
     cudaError_t e;
     rc = GBFG_OK;
-    e = cudaMemcpyAsync(base + oI, host_s_instr, 8 * nb, cudaMemcpyHostToDevice, st);
+    // S_instr goes up on the loop's side stream, ahead of the candidate build gbfg_simulate queues there: the copy
+    // runs while this stream samples and deposits, and gbfg_simulate joins the two streams before the loop reads it
+    SideStream *side = side_stream();
+    if (!side) return set_cuda_error(cudaErrorMemoryAllocation, "side stream");
+    e = cudaMemcpyAsync(base + oI, host_s_instr, 8 * nb, cudaMemcpyHostToDevice, side->s);
     if (e != cudaSuccess) rc = set_cuda_error(e, "cudaMemcpyAsync(s_instr)");
     if (!rc)
         rc = gbfg_simulate(grid, pops, offsets, n_cat, seed, (const double *)(base + oI), params,
