@@ -3,22 +3,21 @@
 // DESIGN.md R3: odd window W = 2h+1 centred on k, ends reflected, statistic = the h-th smallest
 // of the 2h+1 int64 values.  Only integer comparisons decide the result, so it is exact.
 //
-// Persistent CTAs, one per SM, take tiles of at most S = LT - 2h consecutive outputs — from the work
-// list plan_kernel derives from the blocks the last subtraction made dirty, or (stage call) from a
-// static tiling of every row.  The tile and its two h-bin halos (Lt = outputs + 2h <= LT positions,
-// rounded up to a multiple of 1024) are
-// staged in shared memory and sorted ONCE by (value, position): an LSD radix sort, 8 bits per pass,
-// that skips the passes whose digit is the same for the whole tile (spectrum values rarely need
-// more than four).  With the sorted order in hand a window is a position interval, and its median
-// is found without ever sorting a window:
-//   * a (rank-bucket x position-block) table of counts locates the h-th smallest element of a
-//     block-aligned position interval; one warp does this for the start of every chunk of 32
-//     outputs (coarse states);
-//   * every thread then takes 8 outputs: it jumps from the coarse state to its first output by
-//     counting the ranks that left and entered, and walks: sliding the window by one bin removes
-//     one position and adds one, which moves the median by at most one place in the sorted order;
-//     the neighbouring in-window element is found by stepping through the sorted positions
-//     (on average LT/W steps).
+// Persistent CTAs (two of 512 threads per SM for the 32-bit-key kernel, median_kernel.cuh) take tiles of at
+// most S = LT - 2h consecutive outputs — from the work list plan_kernel (below) derives from the blocks the
+// last subtraction made dirty, or (stage call) from a static tiling of every row.  The tile and its two h-bin
+// halos (Lt = outputs + 2h <= LT positions, rounded up to a multiple of the CTA width) are staged in shared
+// memory and sorted ONCE by (value, position): an LSD radix sort, 8 bits per pass, that skips the passes whose
+// digit is the same for the whole tile (spectrum values rarely need more than four).  With the sorted order in
+// hand a window is a position interval, and its median is found without ever sorting a window:
+//   * a (rank-bucket x position-block) table of counts locates the h-th smallest element of a block-aligned
+//     position interval: the coarse state (median rank of the window) of the first 32-output chunk of every
+//     warp; the warp's next chunks follow by sliding the window 32 bins at a time;
+//   * every thread then takes 8 outputs: it jumps from the coarse state to its first output by counting the
+//     ranks that left and entered, and walks: sliding the window by one bin removes one position and adds
+//     one, which moves the median by at most one place in the sorted order; the neighbouring in-window
+//     element is found by stepping through the sorted positions (on average LT/W steps; long stretches of
+//     out-of-window elements — plateaus left by wide chirps — are crossed by the whole warp, 32 ranks a step).
 // The per-output rank is kept in shared memory and written out coalesced, fused with
 //     psd[k] = s_instr[k] + C * (med[k] * 2^scale_log2)        (eqs. 10, D2, D3).
 #include "median_kernel.cuh"
