@@ -100,6 +100,9 @@ def lib():
                                                C.c_int64, C.c_int64, dp, dp, dp]
         L.orc_aet_noise.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double, C.c_int, dp]
         L.orc_instrument_noise_aet.argtypes = [C.POINTER(Grid), C.c_double, C.c_double, C.c_double, C.c_int, dp, dp, dp, dp]
+        L.orc_subtract_until_converged_tol.argtypes = [
+            C.POINTER(Grid), dp, dp, dp, C.c_int64, dp, C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_int32, C.c_double,
+            ip, ip, dp, up, C.POINTER(IterResult), ip]
         L.orc_running_sum_def.argtypes = [ip, C.c_int64, C.c_int32, C.c_int64, C.c_int64, ip]
         L.orc_running_sum.argtypes = [ip, C.c_int64, C.c_int32, ip]
         L.orc_psd_mean.argtypes = [ip, dp, C.c_int64, C.c_int32, C.c_int32, dp]
@@ -329,7 +332,7 @@ def snr_select(grid: Grid, A, f, fdot, psd, rho_th: float, resolved: np.ndarray)
 
 def subtract_until_converged(grid: Grid, A, f, fdot, s_instr, window: int, median_norm: float,
                              rho_th: float, max_iter: int, spectrum: np.ndarray,
-                             resolved: np.ndarray | None = None, estimator: int = 0):
+                             resolved: np.ndarray | None = None, estimator: int = 0, psd_rtol: float = 0.0):
     """Runs the loop in place on `spectrum` (total -> residual).
     -> dict(median, psd, resolved, n_iter, converged, n_resolved, n_near_threshold, n_new_per_iter)"""
     A, f, fdot, s_instr = _f64(A), _f64(f), _f64(fdot), _f64(s_instr)
@@ -341,9 +344,9 @@ def subtract_until_converged(grid: Grid, A, f, fdot, s_instr, window: int, media
     psd = np.empty(grid.n_bins, dtype=np.float64)
     res = IterResult()
     trace = np.zeros(max(max_iter, 1), dtype=np.int64)
-    rc = lib().orc_subtract_until_converged_est(C.byref(grid), _d(A), _d(f), _d(fdot), n, _d(s_instr), window,
-                                                median_norm, rho_th, max_iter, estimator, _i(spectrum), _i(med),
-                                                _d(psd), _u(resolved), C.byref(res), _i(trace))
+    rc = lib().orc_subtract_until_converged_tol(C.byref(grid), _d(A), _d(f), _d(fdot), n, _d(s_instr), window,
+                                                median_norm, rho_th, max_iter, estimator, psd_rtol, _i(spectrum),
+                                                _i(med), _d(psd), _u(resolved), C.byref(res), _i(trace))
     if rc:
         raise ValueError("invalid window / size")
     return dict(median=med, psd=psd, resolved=resolved, n_iter=res.n_iter, converged=res.converged,
@@ -351,7 +354,7 @@ def subtract_until_converged(grid: Grid, A, f, fdot, s_instr, window: int, media
                 n_new_per_iter=trace[:max_iter])
 
 
-def simulate(w, cat: int = 0, n_src: int | None = None, estimator: int = 0):
+def simulate(w, cat: int = 0, n_src: int | None = None, estimator: int = 0, psd_rtol: float = 0.0):
     """Whole path for catalog `cat` of a gbfg_workloads.Workload: sample -> deposit -> loop."""
     grid = make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
     pop = make_pop(w.pops[cat])
@@ -363,7 +366,7 @@ def simulate(w, cat: int = 0, n_src: int | None = None, estimator: int = 0):
     rejected = deposit(grid, A, f, fd, spec)
     total = spec.copy()
     out = subtract_until_converged(grid, A, f, fd, s_instr, w.window, w.median_norm, w.rho_th, w.max_iter, spec,
-                                   estimator=estimator)
+                                   estimator=estimator, psd_rtol=psd_rtol)
     out.update(A=A, f=f, fdot=fd, s_instr=s_instr, total=total, residual=spec, rejected=rejected, grid=grid)
     return out
 

@@ -789,20 +789,37 @@ static int orc_estimate(int estimator, const int64_t *spectrum, const double *s_
 
 /* estimator: 0 = running median (eqs. D2-D3), 1 = running mean (eq. D1; `median` receives the
  * window sums, median_norm is not used). */
-int orc_subtract_until_converged_est(const orc_grid *g, const double *A, const double *f,
+/* psd_rtol > 0: the second stop rule of PAPER.md:530, 552, "convergence in S_n is reached" (R13): from the
+ * second iteration on, delta = max_k |S_n^(i)[k] - S_n^(i-1)[k]| / S_n^(i-1)[k]; delta <= psd_rtol ends the loop
+ * before that iteration's SNR test (converged = 2).  psd_rtol <= 0: the rule is off. */
+int orc_subtract_until_converged_tol(const orc_grid *g, const double *A, const double *f,
                                  const double *fdot, int64_t n, const double *s_instr,
                                  int32_t window, double median_norm, double rho_th, int32_t max_iter,
-                                 int32_t estimator,
+                                 int32_t estimator, double psd_rtol,
                                  int64_t *spectrum, int64_t *median, double *psd, uint8_t *resolved,
                                  orc_iter_result *res, int64_t *n_new_per_iter)
 {
     int64_t *sel = (int64_t *)malloc(sizeof(int64_t) * (size_t)(n > 0 ? n : 1));
+    double *prev = (double *)malloc(sizeof(double) * (size_t)g->n_bins);
     res->n_iter = 0; res->converged = 0; res->n_resolved = 0; res->n_near_threshold = 0;
     int rc = 0;
     int32_t it;
     for (it = 0; it < max_iter; ++it) {
         rc = orc_estimate(estimator, spectrum, s_instr, g->n_bins, window, median_norm, g->scale_log2, median, psd);
         if (rc) break;
+        if (psd_rtol > 0.0 && it > 0) {
+            double delta = 0.0;
+            for (int64_t k = 0; k < g->n_bins; ++k) {
+                double d = fabs(psd[k] - prev[k]) / prev[k];
+                if (d > delta) delta = d;
+            }
+            if (delta <= psd_rtol) {
+                if (n_new_per_iter) n_new_per_iter[it] = 0;
+                res->n_iter = it + 1; res->converged = 2;
+                break;
+            }
+        }
+        if (psd_rtol > 0.0) memcpy(prev, psd, sizeof(double) * (size_t)g->n_bins);
         int64_t near = 0;
         int64_t n_new = orc_snr_select(g, A, f, fdot, n, psd, rho_th, resolved, NULL, sel, &near);
         res->n_near_threshold += near;
@@ -816,7 +833,19 @@ int orc_subtract_until_converged_est(const orc_grid *g, const double *A, const d
         rc = orc_estimate(estimator, spectrum, s_instr, g->n_bins, window, median_norm, g->scale_log2, median, psd);
     }
     free(sel);
+    free(prev);
     return rc;
+}
+
+int orc_subtract_until_converged_est(const orc_grid *g, const double *A, const double *f,
+                                 const double *fdot, int64_t n, const double *s_instr,
+                                 int32_t window, double median_norm, double rho_th, int32_t max_iter,
+                                 int32_t estimator,
+                                 int64_t *spectrum, int64_t *median, double *psd, uint8_t *resolved,
+                                 orc_iter_result *res, int64_t *n_new_per_iter)
+{
+    return orc_subtract_until_converged_tol(g, A, f, fdot, n, s_instr, window, median_norm, rho_th, max_iter, estimator, 0.0,
+                                            spectrum, median, psd, resolved, res, n_new_per_iter);
 }
 
 int orc_subtract_until_converged(const orc_grid *g, const double *A, const double *f,
