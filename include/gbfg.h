@@ -84,6 +84,9 @@ typedef struct gbfg_iter_params {
     double rho_th;          /* SNR threshold, 7 in the paper */
     int32_t max_iter;       /* iteration cap (BASELINE: 30) */
     uint32_t flags;         /* GBFG_FLAG_* */
+    double psd_rtol;        /* > 0: also stop when the PSD has converged (R13): from the second
+                               iteration on, max_k |S_n^(i)[k] - S_n^(i-1)[k]| / S_n^(i-1)[k] <= psd_rtol ends a catalog's
+                               loop before that iteration's SNR test.  <= 0: off (the paper gives no tolerance) */
 } gbfg_iter_params;
 
 #define GBFG_FLAG_NO_PRESELECT 1u   /* test every unresolved source every iteration (no R5 candidate cut) */
@@ -94,7 +97,7 @@ typedef struct gbfg_iter_params {
 /* Per-catalog outcome of the loop (HOST). */
 typedef struct gbfg_iter_result {
     int32_t n_iter;             /* iterations run; = max_iter when the cap was hit */
-    int32_t converged;          /* 1: an iteration resolved no new source; 0: cap hit */
+    int32_t converged;          /* 1: an iteration resolved no new source; 2: the PSD converged (psd_rtol); 0: cap hit */
     int64_t n_resolved;         /* sources resolved by this call */
     int64_t n_near_threshold;   /* tests with |rho^2 / rho_th^2 - 1| <= 2e-9, summed over iterations */
     int64_t n_candidates;       /* sources that passed the pre-selection (= tested sources if disabled) */

@@ -57,7 +57,7 @@ class PopPaper(C.Structure):
 
 class IterParams(C.Structure):
     _fields_ = [("struct_size", C.c_uint32), ("window", C.c_int32), ("median_norm", C.c_double),
-                ("rho_th", C.c_double), ("max_iter", C.c_int32), ("flags", C.c_uint32)]
+                ("rho_th", C.c_double), ("max_iter", C.c_int32), ("flags", C.c_uint32), ("psd_rtol", C.c_double)]
 
 
 class IterResult(C.Structure):
@@ -156,8 +156,9 @@ def make_pop(p) -> Pop:
     return Pop(C.sizeof(Pop), 0, p.slope, p.logA_offset, p.logA_sigma, p.logMc_mean, p.logMc_sigma, p.n_src)
 
 
-def make_iter_params(window: int, median_norm: float, rho_th: float, max_iter: int, flags: int = 0) -> IterParams:
-    return IterParams(C.sizeof(IterParams), window, median_norm, rho_th, max_iter, flags)
+def make_iter_params(window: int, median_norm: float, rho_th: float, max_iter: int, flags: int = 0,
+                     psd_rtol: float = 0.0) -> IterParams:
+    return IterParams(C.sizeof(IterParams), window, median_norm, rho_th, max_iter, flags, psd_rtol)
 
 
 def version() -> int:

@@ -23,12 +23,15 @@ int launch_scan(int64_t n_bins, int n_cat, int64_t *spectrum, int64_t *diff, int
                 const DepositMarks &mk, cudaStream_t st);
 int median_max_items(int64_t n_bins);
 int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins, int n_cat, int window,
-                const MedianPlan &pl, int64_t *zero_ptr, int zero_n, int64_t *out_count, cudaStream_t st);
+                const MedianPlan &pl, int64_t *zero_ptr, int zero_n, int64_t *out_count, unsigned long long *zero2_ptr,
+                cudaStream_t st);
 int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *med,
                   const double *s_instr, double *psd, double norm, int scale_log2,
-                  const MedianPlan *plan, int4 *wide_items, int *wide_ctr, int *neg_flag, cudaStream_t st);
+                  const MedianPlan *plan, int4 *wide_items, int *wide_ctr, int *neg_flag,
+                  unsigned long long *delta_bits, cudaStream_t st);
 int launch_mean(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *sum,
-                const double *s_instr, double *psd, int scale_log2, int *neg_flag, cudaStream_t st);
+                const double *s_instr, double *psd, int scale_log2, int *neg_flag, unsigned long long *delta_bits,
+                cudaStream_t st);
 int pfx_tiles_per_row(int64_t n_bins);
 size_t snr_pref_bytes(int64_t n_bins, int n_cat);
 size_t snr_tile_off_bytes(int64_t n_bins, int n_cat);
@@ -41,10 +44,10 @@ int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, con
 int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th, uint8_t *resolved, double *rho2_out,
                     int64_t n_launch, int64_t *sel_idx, int64_t *sel_count, int64_t *near_count, int near_per_cat,
                     const int *abort_flag, bool use_prefix, const SnrWork &sw, const DirtyView &dv, int64_t *test_count,
-                    const SubtractView *sub, cudaStream_t st);
+                    const SubtractView *sub, const unsigned long long *delta_bits, double psd_rtol, cudaStream_t st);
 
 // ------------------------------------------------------------------------------- workspace
-constexpr int WS_COUNTERS = 6 * GBFG_MAX_CAT + 16;
+constexpr int WS_COUNTERS = 7 * GBFG_MAX_CAT + 16;
 
 // layout of `counters` (int64): what the host reads back each iteration comes first
 //   [0 .. n_cat]            sel_count: total, per catalog
@@ -53,6 +56,7 @@ constexpr int WS_COUNTERS = 6 * GBFG_MAX_CAT + 16;
 //   [2+2 n_cat .. 3+3 n_cat) cand_count: total, per catalog
 //   [3+3 n_cat .. 3+4 n_cat) running-median outputs computed, per catalog (accumulated over the call)
 //   [3+4 n_cat .. 3+5 n_cat) SNR tests evaluated, per catalog (accumulated over the call)
+//   [3+5 n_cat .. 3+6 n_cat) largest relative PSD change of this pass, per catalog, as binary64 bits (R13)
 struct Workspace {
     int64_t *diff;        // [n_cat * n_bins]   difference array of the range-update deposit
     int64_t *tile_sums;   // [n_cat * scan_tiles]
@@ -265,7 +269,7 @@ extern "C" int gbfg_snr_select(const gbfg_grid *grid, const double *dev_A, const
     rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, nullptr, rho_th, dev_rho2_out, w.sw, st);
     if (rc) return rc;
     return launch_snr_cand(grid->n_bins, n_cat, dev_psd, rho_th, dev_resolved, dev_rho2_out, n, dev_sel_idx,
-                           dev_sel_count, dev_near_count, 0, nullptr, true, w.sw, all_dirty, nullptr, nullptr, st);
+                           dev_sel_count, dev_near_count, 0, nullptr, true, w.sw, all_dirty, nullptr, nullptr, nullptr, 0.0, st);
 }
 
 // workspace state the loop starts from (also what a deposit needs: zero difference array and stamps)
@@ -342,7 +346,10 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
     int64_t *near = w.counters + 1 + n_cat;             // [n_cat]
     int *neg_flag = (int *)(w.counters + 1 + 2 * n_cat);
     const size_t n_iter_counters = (size_t)(1 + 2 * n_cat);      // zeroed every iteration
-    const size_t n_read_all = (size_t)(3 + 5 * n_cat);           // ... + flags + cand_count + work counters
+    const size_t n_read_all = (size_t)(3 + 6 * n_cat);           // ... + flags + cand_count + work counters + PSD change
+    const double psd_rtol = params->psd_rtol > 0.0 ? params->psd_rtol : 0.0;
+    unsigned long long *delta_all = (unsigned long long *)(w.counters + 3 + 5 * n_cat);
+    const int i_delta = 3 + 5 * n_cat;
     int64_t *med_outputs = w.counters + 3 + 3 * n_cat, *snr_tests = w.counters + 3 + 4 * n_cat;
     const int i_med = 3 + 3 * n_cat, i_tests = 3 + 4 * n_cat;
     const int i_flags = 1 + 2 * n_cat, i_cand = 2 + 2 * n_cat;
@@ -377,16 +384,18 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
             GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_plan, 0));
         } else {
             rc = launch_plan(w.blk_stamp, it, it == 0 || !incremental, nb, n_cat, W, w.plan, w.counters, (int)n_iter_counters,
-                             use_mean ? nullptr : med_outputs, st);
+                             use_mean ? nullptr : med_outputs, delta_all, st);
             if (rc) return rc;
         }
         plan_queued = false;
+        // second stop rule (R13): from the second pass on the estimator also records the largest relative PSD change
+        unsigned long long *delta = (psd_rtol > 0.0 && it > 0) ? delta_all : nullptr;
         if (use_mean) {      // eq. (D1): HBM bound, every bin every iteration
-            rc = launch_mean(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, grid->scale_log2, neg_flag, st);
+            rc = launch_mean(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, grid->scale_log2, neg_flag, delta, st);
             ++mean_passes;
         } else {
             rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
-                               grid->scale_log2, &w.plan, nullptr, nullptr, neg_flag, st);
+                               grid->scale_log2, &w.plan, nullptr, nullptr, neg_flag, delta, st);
         }
         if (rc) return rc;
         rc = launch_inv_prefix(dev_psd, nb, n_cat, w.sw, dirty, st);
@@ -396,7 +405,7 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
         mk.blk_stamp = w.blk_stamp; mk.n_dblk = w.plan.n_dblk; mk.dblk_log2 = w.plan.dblk_log2; mk.med_h = W / 2;
         const SubtractView sub = {dev_spectrum, w.diff, w.wide_flag, mk, grid->scale_log2};
         rc = launch_snr_cand(nb, n_cat, dev_psd, params->rho_th, dev_resolved, nullptr, n_cand, w.sel_idx, sel_count,
-                             near, 1, preselect ? neg_flag : nullptr, true, w.sw, dirty, snr_tests, &sub, st);
+                             near, 1, preselect ? neg_flag : nullptr, true, w.sw, dirty, snr_tests, &sub, delta, psd_rtol, st);
         if (rc) return rc;
         GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
         GBFG_CUDA(cudaEventRecord(ev_read, st));
@@ -412,7 +421,8 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
             const bool closing = it + 1 == params->max_iter;
             GBFG_CUDA(cudaStreamWaitEvent(side->s, ev_read, 0));
             rc = launch_plan(w.blk_stamp, it + 1, !incremental, nb, n_cat, W, w.plan, closing ? nullptr : w.counters,
-                             closing ? 0 : (int)n_iter_counters, use_mean ? nullptr : med_outputs, side->s);
+                             closing ? 0 : (int)n_iter_counters, use_mean ? nullptr : med_outputs,
+                             closing ? nullptr : delta_all, side->s);
             if (rc) return rc;
             GBFG_CUDA(cudaEventRecord(side->ev_plan, side->s));
             plan_queued = true;
@@ -429,7 +439,7 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
             rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, nullptr, params->rho_th, nullptr, w.sw, st);
             if (rc) return rc;
             rc = launch_snr_cand(nb, n_cat, dev_psd, params->rho_th, dev_resolved, nullptr, n, w.sel_idx, sel_count,
-                                 near, 1, nullptr, true, w.sw, all_dirty, snr_tests, &sub, st);
+                                 near, 1, nullptr, true, w.sw, all_dirty, snr_tests, &sub, delta, psd_rtol, st);
             if (rc) return rc;
             GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
             rc = launch_scan(nb, n_cat, dev_spectrum, w.diff, w.tile_sums, w.wide_flag, mk, st);
@@ -443,6 +453,15 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
             gbfg_iter_result &r = host_results[c];
             if (r.n_candidates == 0) r.n_candidates = n_cat == 1 ? host[i_cand] : host[i_cand + 1 + c];
             if (done[c]) continue;
+            if (delta) {                                 // S_n converged: the test of this pass did not run for this catalog
+                double d;
+                memcpy(&d, &host[i_delta + c], sizeof(double));
+                if (d <= psd_rtol) {
+                    if (it < GBFG_MAX_ITER_TRACE) r.n_new_per_iter[it] = 0;
+                    done[c] = true; ++n_done; r.n_iter = it + 1; r.converged = 2;
+                    continue;
+                }
+            }
             const int64_t n_new = host[1 + c];
             if (it < GBFG_MAX_ITER_TRACE) r.n_new_per_iter[it] = n_new;
             r.n_resolved += n_new;
@@ -456,18 +475,18 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
         for (int c = 0; c < n_cat; ++c)
             if (!done[c]) { host_results[c].n_iter = params->max_iter; host_results[c].converged = 0; }
         if (use_mean) {
-            rc = launch_mean(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, grid->scale_log2, nullptr, st);
+            rc = launch_mean(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, grid->scale_log2, nullptr, nullptr, st);
             ++mean_passes;
         } else {
             if (plan_queued) {
                 GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_plan, 0));
             } else {
-                rc = launch_plan(w.blk_stamp, params->max_iter, !incremental, nb, n_cat, W, w.plan, nullptr, 0, med_outputs, st);
+                rc = launch_plan(w.blk_stamp, params->max_iter, !incremental, nb, n_cat, W, w.plan, nullptr, 0, med_outputs, nullptr, st);
                 if (rc) return rc;
             }
             plan_queued = false;
             rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
-                               grid->scale_log2, &w.plan, nullptr, nullptr, nullptr, st);
+                               grid->scale_log2, &w.plan, nullptr, nullptr, nullptr, nullptr, st);
         }
         if (rc) return rc;
     }

@@ -31,6 +31,7 @@ struct MeanArgs {
     const double *s_instr;   // [n] or NULL (no PSD)
     double *psd;             // [n_cat][n] or NULL
     int *neg_flag;           // nullable: set to 1 when a window sum is negative
+    unsigned long long *delta_bits;   // nullable: [n_cat] largest relative PSD change of the row, as binary64 bits (R13)
     int64_t n;
     int h;
     int S;                   // outputs per tile
@@ -99,6 +100,7 @@ running_mean_kernel(MeanArgs a)
     }
     __syncthreads();
     bool neg = false;
+    double dmax = 0.0;
     for (int j0 = tid; j0 < n_out; j0 += MEAN_OUT_UNROLL * MEAN_THREADS) {
         double si[MEAN_OUT_UNROLL];
         if (a.psd) {
@@ -121,19 +123,31 @@ running_mean_kernel(MeanArgs a)
                 if (a.psd) {
                     const double e = (double)sv * a.scale;
                     const double m = e / a.w;
-                    a.psd[row + g] = si[u] + m;
+                    const double pnew = si[u] + m;
+                    if (a.delta_bits) {
+                        const double pold = a.psd[row + g];
+                        const double d = fabs(pnew - pold) / pold;
+                        if (d > dmax) dmax = d;
+                    }
+                    a.psd[row + g] = pnew;
                 }
             }
         }
+    }
+    if (a.delta_bits) {
+        for (int o = 16; o; o >>= 1) dmax = fmax(dmax, __shfl_xor_sync(0xffffffffu, dmax, o));
+        if (lane == 0 && dmax > 0.0) atomicMax(a.delta_bits + blockIdx.y, (unsigned long long)__double_as_longlong(dmax));
     }
     if (a.neg_flag && neg) *a.neg_flag = 1;
 }
 
 // internal entry: window sums (+ PSD when psd != NULL) of every row
 int launch_mean(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *sum,
-                const double *s_instr, double *psd, int scale_log2, int *neg_flag, cudaStream_t st)
+                const double *s_instr, double *psd, int scale_log2, int *neg_flag, unsigned long long *delta_bits,
+                cudaStream_t st)
 {
     MeanArgs a;
+    a.delta_bits = delta_bits;
     a.x = x; a.sum = sum; a.s_instr = s_instr; a.psd = psd; a.neg_flag = neg_flag;
     a.n = n_bins; a.h = window / 2;
     const int s_max = MEAN_LT - (window - 1);
@@ -175,6 +189,6 @@ extern "C" int gbfg_running_mean(const int64_t *dev_spectrum, int64_t n_bins, in
     if (n_bins < window / 2 + 1) return GBFG_ERR_INVALID_ARG;
     int rc = check_device();
     if (rc) return rc;
-    return launch_mean(dev_spectrum, n_bins, n_cat, window, dev_sum_out, dev_s_instr, dev_psd, scale_log2, nullptr,
+    return launch_mean(dev_spectrum, n_bins, n_cat, window, dev_sum_out, dev_s_instr, dev_psd, scale_log2, nullptr, nullptr,
                        (cudaStream_t)stream);
 }

@@ -65,6 +65,7 @@ struct PlanArgs {
     int zero_n;
     int64_t *out_count;     // [n_cat] outputs planned, accumulated (nullable)
     int *wide_ctr;          // [2] counter words of the wide list, cleared here
+    unsigned long long *zero2_ptr;   // [n_cat] PSD-change words of the loop, cleared here (nullable)
 };
 
 // len < 2^31 (n_bins is): 32-bit divisions, the 64-bit ones are long instruction sequences
@@ -97,6 +98,7 @@ plan_kernel(PlanArgs a)
     if (tid == 0) { n_runs = 0; row_pieces = 0; }
     if (row == 0 && tid < 2) a.wide_ctr[tid] = 0;
     if (row == 0 && a.zero_ptr) for (int i = tid; i < a.zero_n; i += PLAN_THREADS) a.zero_ptr[i] = 0;
+    if (tid == 0 && a.zero2_ptr) a.zero2_ptr[row] = 0ull;
     for (int b0 = tid; b0 < nb; b0 += 8 * PLAN_THREADS) {   // coalesced, eight loads in flight per thread
         int v[8];
 #pragma unroll
@@ -215,9 +217,11 @@ int median_max_items(int64_t n_bins)
 
 // work list + cum from the stamps (blk_stamp NULL or all_dirty: everything)
 int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins, int n_cat, int window,
-                const MedianPlan &pl, int64_t *zero_ptr, int zero_n, int64_t *out_count, cudaStream_t st)
+                const MedianPlan &pl, int64_t *zero_ptr, int zero_n, int64_t *out_count, unsigned long long *zero2_ptr,
+                cudaStream_t st)
 {
     PlanArgs a;
+    a.zero2_ptr = zero2_ptr;
     a.zero_ptr = zero_ptr; a.zero_n = zero_n; a.out_count = out_count;
     a.blk_stamp = blk_stamp; a.stamp = stamp; a.all_dirty = (all_dirty || !blk_stamp) ? 1 : 0;
     a.n_dblk = pl.n_dblk; a.dblk_log2 = pl.dblk_log2; a.n_bins = n_bins;
@@ -261,9 +265,11 @@ int median_static_tiles(int64_t n_bins, int n_cat, int window, int *S_out)
 
 int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *med,
                   const double *s_instr, double *psd, double norm, int scale_log2,
-                  const MedianPlan *plan, int4 *wide_items, int *wide_ctr, int *neg_flag, cudaStream_t st)
+                  const MedianPlan *plan, int4 *wide_items, int *wide_ctr, int *neg_flag,
+                  unsigned long long *delta_bits, cudaStream_t st)
 {
     MedianArgs a;
+    a.delta_bits = delta_bits;
     a.x = x; a.med = med; a.s_instr = s_instr; a.psd = psd; a.neg_flag = neg_flag;
     a.items = plan ? plan->items : nullptr; a.ctr = plan ? plan->ctr : nullptr; a.n_cat = n_cat;
     a.wide_items = plan ? plan->wide_items : wide_items;
@@ -314,7 +320,7 @@ extern "C" int gbfg_running_median(const int64_t *dev_spectrum, int64_t n_bins, 
     char *tmp = nullptr;
     GBFG_CUDA(cudaMallocAsync((void **)&tmp, 16 + sizeof(int4) * (size_t)tiles * (size_t)n_cat, st));
     rc = launch_median(dev_spectrum, n_bins, n_cat, window, dev_median_out, nullptr, nullptr, 1.0, 0, nullptr,
-                       (int4 *)(tmp + 16), (int *)tmp, nullptr, st);
+                       (int4 *)(tmp + 16), (int *)tmp, nullptr, nullptr, st);
     cudaError_t e = cudaFreeAsync(tmp, st);
     if (!rc && e != cudaSuccess) rc = set_cuda_error(e, "cudaFreeAsync");
     return rc;

@@ -48,6 +48,7 @@ struct MedianArgs {
     int *wide_ctr;           // [0] number of wide items (appended with atomics)
     int n_cat;
     int *neg_flag;           // nullable: set to 1 when a median is negative
+    unsigned long long *delta_bits;   // nullable: [n_cat] largest relative PSD change of the row, as binary64 bits (R13)
     int64_t n;
     int h;
     int S;                   // outputs per tile of the static tiling
@@ -447,6 +448,7 @@ running_median_tile_kernel(MedianArgs a)
     __syncthreads();
 
     // ---- coalesced epilogue: median and PSD
+    double dmax = 0.0;
     for (int j0 = tid; j0 < n_out; j0 += 4 * THREADS) {
         double si[4];
         if (a.psd) {
@@ -468,10 +470,20 @@ running_median_tile_kernel(MedianArgs a)
                 neg |= v < 0;
                 if (a.psd) {
                     const double e = (double)v * a.scale;
-                    a.psd[row + g] = si[u] + a.norm * e;
+                    const double pnew = si[u] + a.norm * e;
+                    if (a.delta_bits) {                      // convergence in S_n: change against the last pass
+                        const double pold = a.psd[row + g];
+                        const double d = fabs(pnew - pold) / pold;
+                        if (d > dmax) dmax = d;
+                    }
+                    a.psd[row + g] = pnew;
                 }
             }
         }
+    }
+    if (a.delta_bits) {                                  // non-negative binary64 values order like their bits
+        for (int o = 16; o; o >>= 1) dmax = fmax(dmax, __shfl_xor_sync(FULL, dmax, o));
+        if (lane == 0 && dmax > 0.0) atomicMax(a.delta_bits + row_i, (unsigned long long)__double_as_longlong(dmax));
     }
   }   // tiles
     if (a.neg_flag && neg) *a.neg_flag = 1;

@@ -424,6 +424,8 @@ struct SnrArgs {
     int n_dblk;
     int64_t *test_count;        // [n_cat] tests evaluated, accumulated (nullable)
     SubtractView sub;           // spectrum != NULL: a selected source is subtracted on the spot (eq. D4)
+    const unsigned long long *delta_bits;   // nullable: [n_cat] PSD change of this pass; a row at or under psd_rtol is frozen (R13)
+    double psd_rtol;
     int64_t n_bins;
     int n_cat;
     double thr;                 // rho_th^2
@@ -439,6 +441,7 @@ __global__ void __launch_bounds__(256)
 snr_cand_kernel(SnrArgs a)
 {
     if (a.abort_flag && *a.abort_flag) return;
+    if (a.delta_bits && __longlong_as_double((long long)a.delta_bits[blockIdx.y]) <= a.psd_rtol) return;   // S_n has converged
     const int lane = threadIdx.x & 31;
     // records of row blockIdx.y, narrowed to the buckets that can reach a dirty block
     const int rowc = blockIdx.y;
@@ -643,10 +646,11 @@ int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, con
 int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th, uint8_t *resolved, double *rho2_out,
                     int64_t n_launch, int64_t *sel_idx, int64_t *sel_count, int64_t *near_count, int near_per_cat,
                     const int *abort_flag, bool use_prefix, const SnrWork &sw, const DirtyView &dv, int64_t *test_count,
-                    const SubtractView *sub, cudaStream_t st)
+                    const SubtractView *sub, const unsigned long long *delta_bits, double psd_rtol, cudaStream_t st)
 {
     if (n_launch <= 0) return GBFG_OK;
     SnrArgs a;
+    a.delta_bits = delta_bits; a.psd_rtol = psd_rtol;
     a.test_count = test_count;
     if (sub) a.sub = *sub; else a.sub.spectrum = nullptr;
     a.dv = dv;

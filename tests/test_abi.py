@@ -43,8 +43,8 @@ def test_library_exports_every_declared_function(gbcpu):
 
 
 def test_struct_sizes_match_the_header(gbcpu):
-    # gbfg_grid: 2 x 4 + 3 x 8 + 8; gbfg_pop: 2 x 4 + 5 x 8 + 8; gbfg_iter_params: 4+4+8+8+4+4
-    assert C.sizeof(gbcpu.Grid) == 40 and C.sizeof(gbcpu.Pop) == 56 and C.sizeof(gbcpu.IterParams) == 32
+    # gbfg_grid: 2 x 4 + 3 x 8 + 8; gbfg_pop: 2 x 4 + 5 x 8 + 8; gbfg_iter_params: 4+4+8+8+4+4+8
+    assert C.sizeof(gbcpu.Grid) == 40 and C.sizeof(gbcpu.Pop) == 56 and C.sizeof(gbcpu.IterParams) == 40
     # gbfg_iter_result: 2 x 4 + 5 x 8 + 64 x 8
     assert C.sizeof(gbcpu.IterResult) == 8 + 5 * 8 + 8 * gbcpu.MAX_ITER_TRACE
 

@@ -699,3 +699,58 @@ def test_release_cached_and_reuse(gb, orc, torch):
     gb.simulate_host(g, w.pops, w.offsets(), w.seed, s_instr, params, hp2)
     assert np.array_equal(bits(hp1), bits(hp2))
     _loop_case(gb, orc, torch, w)
+
+
+# ------------------------------------------------- second stop rule: convergence in S_n (R13)
+@pytest.mark.parametrize("tol", [1e300, 3e-2, 1e-3, 1e-6, 1e-300])
+@pytest.mark.parametrize("estimator", [0, 1])
+def test_loop_psd_stop_rule(gb, orc, torch, tol, estimator):
+    w = wl.dense_case("short")
+    ref = orc.simulate(w, estimator=estimator, psd_rtol=tol)
+    g = gpu_grid(gb, w)
+    n, nb = w.n_src_total, g.n_bins
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    total, spec, stat = (torch.empty(nb, dtype=torch.int64, device="cuda") for _ in range(3))
+    psd = torch.empty(nb, dtype=torch.float64, device="cuda")
+    resolved = torch.empty(n, dtype=torch.uint8, device="cuda")
+    flags = gb.FLAG_ESTIMATOR_MEAN if estimator else 0
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter, flags, psd_rtol=tol)
+    res = gb.simulate(g, w.pops, w.offsets(), w.seed, dev(torch, ref["s_instr"]), params, A, f, fd, total, spec, stat,
+                      psd, resolved, workspace(torch, gb, g, n))[0]
+    assert (res.n_iter, res.converged, res.n_resolved) == (ref["n_iter"], ref["converged"], ref["n_resolved"])
+    assert np.array_equal(spec.cpu().numpy(), ref["residual"])
+    assert np.array_equal(stat.cpu().numpy(), ref["median"])
+    assert np.array_equal(bits(psd.cpu().numpy()), bits(ref["psd"]))
+    assert np.array_equal(resolved.cpu().numpy(), ref["resolved"])
+    k = min(ref["n_iter"], gb.MAX_ITER_TRACE)
+    assert list(res.n_new_per_iter[:k]) == list(ref["n_new_per_iter"][:k])
+    if tol == 1e300:
+        assert (res.n_iter, res.converged) == (2, 2)
+
+
+def test_loop_psd_stop_rule_batch(gb, orc, torch):
+    """Catalogs of a batch stop on their own: some by the PSD rule, at different iterations."""
+    w = wl.scaled(wl.config(4), n_cat=3)
+    w = wl.replace(w, pops=[wl.replace(p, n_src=n) for p, n in zip(w.pops, (80_000, 30_001, 120_000))])
+    tol = 2e-3
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    n, nb, nc = w.n_src_total, g.n_bins, w.n_cat
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    total, spec, med = (torch.empty((nc, nb), dtype=torch.int64, device="cuda") for _ in range(3))
+    psd = torch.empty((nc, nb), dtype=torch.float64, device="cuda")
+    resolved = torch.empty(n, dtype=torch.uint8, device="cuda")
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter, psd_rtol=tol)
+    res = gb.simulate(g, w.pops, w.offsets(), w.seed, dev(torch, orc.instrument_noise(og)), params, A, f, fd, total, spec,
+                      med, psd, resolved, workspace(torch, gb, g, n, nc))
+    off = w.offsets()
+    outcomes = set()
+    for c in range(nc):
+        ref = orc.simulate(w, cat=c, psd_rtol=tol)
+        s = slice(int(off[c]), int(off[c + 1]))
+        assert (res[c].n_iter, res[c].converged, res[c].n_resolved) == (ref["n_iter"], ref["converged"], ref["n_resolved"])
+        assert np.array_equal(spec[c].cpu().numpy(), ref["residual"])
+        assert np.array_equal(bits(psd[c].cpu().numpy()), bits(ref["psd"]))
+        assert np.array_equal(resolved[s].cpu().numpy(), ref["resolved"])
+        outcomes.add((ref["n_iter"], ref["converged"]))
+    assert len(outcomes) > 1
