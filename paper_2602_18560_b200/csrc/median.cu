@@ -282,8 +282,10 @@ int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64
     int dev = 0;
     GBFG_CUDA(cudaGetDevice(&dev));
     if (attr_dev != dev) {
-        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint32_t, 512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem32));
-        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint64_t, 1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem64));
+        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint32_t, 512, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem32));
+        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint64_t, 1024, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem64));
+        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint32_t, 512, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem32));
+        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint64_t, 1024, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem64));
         attr_dev = dev;
     }
     const int sms = sm_count();
@@ -291,12 +293,14 @@ int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64
     int64_t grid = plan ? 2 * sms : (int64_t)a.tiles * n_cat;
     if (grid > 2 * sms) grid = 2 * sms;
     LaunchTimer lt(K_MEDIAN, st);
-    running_median_tile_kernel<uint32_t, 512><<<(int)grid, 512, smem32, st>>>(a);
+    if (delta_bits) running_median_tile_kernel<uint32_t, 512, true><<<(int)grid, 512, smem32, st>>>(a);
+    else running_median_tile_kernel<uint32_t, 512, false><<<(int)grid, 512, smem32, st>>>(a);
     GBFG_LAUNCH_CHECK("running_median_tile_kernel<u32>");
     a.items = a.wide_items; a.ctr = a.wide_ctr;
     a.wide_items = nullptr; a.wide_ctr = nullptr;
     if (grid > sms) grid = sms;
-    running_median_tile_kernel<uint64_t, 1024><<<(int)grid, 1024, smem64, st>>>(a);
+    if (delta_bits) running_median_tile_kernel<uint64_t, 1024, true><<<(int)grid, 1024, smem64, st>>>(a);
+    else running_median_tile_kernel<uint64_t, 1024, false><<<(int)grid, 1024, smem64, st>>>(a);
     GBFG_LAUNCH_CHECK("running_median_tile_kernel<u64>");
     return GBFG_OK;
 }

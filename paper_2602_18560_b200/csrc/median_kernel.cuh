@@ -81,7 +81,9 @@ __device__ __forceinline__ unsigned same_digit_lanes(unsigned d)
     return peers;
 }
 
-template <typename KeyT, int THREADS>
+// DELTA: also record the largest relative PSD change (the second stop rule, R13); a template parameter so
+// that the default kernel carries none of it
+template <typename KeyT, int THREADS, bool DELTA>
 __global__ void __launch_bounds__(THREADS, THREADS <= 512 ? 2 : 1)
 running_median_tile_kernel(MedianArgs a)
 {
@@ -471,7 +473,7 @@ running_median_tile_kernel(MedianArgs a)
                 if (a.psd) {
                     const double e = (double)v * a.scale;
                     const double pnew = si[u] + a.norm * e;
-                    if (a.delta_bits) {                      // convergence in S_n: change against the last pass
+                    if (DELTA) {                             // convergence in S_n: change against the last pass
                         const double pold = a.psd[row + g];
                         const double d = fabs(pnew - pold) / pold;
                         if (d > dmax) dmax = d;
@@ -481,7 +483,7 @@ running_median_tile_kernel(MedianArgs a)
             }
         }
     }
-    if (a.delta_bits) {                                  // non-negative binary64 values order like their bits
+    if (DELTA) {                                         // non-negative binary64 values order like their bits
         for (int o = 16; o; o >>= 1) dmax = fmax(dmax, __shfl_xor_sync(FULL, dmax, o));
         if (lane == 0 && dmax > 0.0) atomicMax(a.delta_bits + row_i, (unsigned long long)__double_as_longlong(dmax));
     }
