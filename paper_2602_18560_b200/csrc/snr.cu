@@ -26,8 +26,8 @@ namespace gbfg {
 constexpr int SNR_NARROW = 8;
 constexpr int SNR_SEL_CAP = 1024;              // selected indices a CTA holds before it appends them to the list
 constexpr int PFX_THREADS = 512;
-constexpr int PFX_ITEMS = 8;
-constexpr int PFX_TILE = PFX_THREADS * PFX_ITEMS;     // 4096 bins per prefix tile
+constexpr int PFX_ITEMS = 4;
+constexpr int PFX_TILE = PFX_THREADS * PFX_ITEMS;     // 2048 bins per prefix tile
 
 size_t snr_hdr_bytes();
 
@@ -141,7 +141,7 @@ prefix_header_kernel(const double *__restrict__ arr, int64_t n, int64_t n_bins_r
 
 // phase A: local inclusive prefix of every tile of PFX_TILE bins + the tile totals (skipped for
 // tiles without a dirty block: their prefix stands)
-__global__ void __launch_bounds__(PFX_THREADS)
+__global__ void __launch_bounds__(PFX_THREADS, 3)
 inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tiles_per_row,
                         U128 *__restrict__ pref, U128 *__restrict__ tile_tot, U128 *__restrict__ tile_off,
                         PrefixHeader *hdr, DirtyView dv, unsigned *__restrict__ ticket)
