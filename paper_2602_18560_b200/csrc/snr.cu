@@ -461,7 +461,7 @@ snr_cand_kernel(SnrArgs a)
     // The selected indices of the CTA are collected in shared memory and appended to the list with
     // one global atomic per flush (tens of thousands of sources pass in the first iterations: one
     // atomic per warp on a single address is what the kernel then waits for).
-    __shared__ int64_t s_sel[SNR_SEL_CAP + 256];
+    __shared__ int64_t s_sel[SNR_SEL_CAP];
     __shared__ int s_n, s_near, s_tests;
     __shared__ long long s_base;
     if (threadIdx.x == 0) { s_n = 0; s_near = 0; s_tests = 0; }
@@ -501,11 +501,22 @@ snr_cand_kernel(SnrArgs a)
             if (test_mask && lane == 0) atomicAdd(&s_tests, __popc(test_mask));
         }
         if (sel_mask) {
+            // a place in the CTA's buffer; once that is full (rare: > SNR_SEL_CAP selected by one CTA) straight into the list
             int base = 0;
             if (lane == 0) base = atomicAdd(&s_n, __popc(sel_mask));
             base = __shfl_sync(0xffffffffu, base, 0);
+            const int mine = base + __popc(sel_mask & ((1u << lane) - 1u));
+            long long gbase = 0;
+            const int n_over = base + __popc(sel_mask) - SNR_SEL_CAP;     // > 0: that many of this warp's do not fit
+            if (n_over > 0 && lane == 0) {
+                const int cnt = n_over < __popc(sel_mask) ? n_over : __popc(sel_mask);
+                gbase = (long long)atomicAdd((unsigned long long *)a.sel_count, (unsigned long long)cnt);
+                atomicAdd((unsigned long long *)(a.sel_count + 1 + rowc), (unsigned long long)cnt);
+            }
+            gbase = __shfl_sync(0xffffffffu, gbase, 0);
             if (sel) {
-                s_sel[base + __popc(sel_mask & ((1u << lane) - 1u))] = src;
+                if (mine < SNR_SEL_CAP) s_sel[mine] = src;
+                else a.sel_idx[gbase + (mine - (base > SNR_SEL_CAP ? base : SNR_SEL_CAP))] = src;
                 a.resolved[src] = 1;
                 a.cand.w[t] = 0;
             }
@@ -539,19 +550,18 @@ snr_cand_kernel(SnrArgs a)
         }
         if (near && !sel && !always) { a.cand.w[t] = -w; *a.any_near = 1; }
         if (near_mask && lane == 0) atomicAdd(&s_near, __popc(near_mask));
-        __syncthreads();
-        const bool last = t0 + stride >= n;
-        if (s_n > SNR_SEL_CAP || (last && s_n > 0)) {       // uniform over the CTA
-            const int cnt = s_n;
+    }
+    // one append per CTA for what its buffer holds
+    __syncthreads();
+    {
+        const int cnt = s_n < SNR_SEL_CAP ? s_n : SNR_SEL_CAP;
+        if (cnt > 0) {
             if (threadIdx.x == 0) {
                 s_base = (long long)atomicAdd((unsigned long long *)a.sel_count, (unsigned long long)cnt);
                 atomicAdd((unsigned long long *)(a.sel_count + 1 + rowc), (unsigned long long)cnt);
             }
             __syncthreads();
             for (int i = threadIdx.x; i < cnt; i += blockDim.x) a.sel_idx[s_base + i] = s_sel[i];
-            __syncthreads();
-            if (threadIdx.x == 0) s_n = 0;
-            __syncthreads();
         }
     }
     if (threadIdx.x == 0 && a.test_count && s_tests) atomicAdd((unsigned long long *)(a.test_count + rowc), (unsigned long long)s_tests);
