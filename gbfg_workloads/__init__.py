@@ -185,6 +185,14 @@ def random_spectrum(n: int, seed: int, kind: str = "lognormal") -> np.ndarray:
         return np.arange(n, dtype=np.int64) * 3 - n
     if kind == "const":
         return np.full(n, 42, dtype=np.int64)
+    if kind == "plateaus":          # what wide chirps leave: runs of equal values on a slowly drifting level
+        runs = rng.integers(1, 60, n)
+        vals = np.cumsum(rng.integers(-50, 51, n)) + 10_000
+        return np.repeat(vals, runs)[:n].astype(np.int64)
+    if kind == "straddle32":        # values on both sides of 2^32: the 32-bit-key path must hand the tile over
+        return ((1 << 32) + rng.integers(-5000, 5000, n)).astype(np.int64)
+    if kind == "negative":
+        return rng.integers(-(1 << 20), 1 << 20, n).astype(np.int64)
     raise ValueError(kind)
 
 

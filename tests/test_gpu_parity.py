@@ -754,3 +754,25 @@ def test_loop_psd_stop_rule_batch(gb, orc, torch):
         assert np.array_equal(resolved[s].cpu().numpy(), ref["resolved"])
         outcomes.add((ref["n_iter"], ref["converged"]))
     assert len(outcomes) > 1
+
+
+def test_running_median_random_sweep(gb, orc, torch):
+    """Seeded sweep over sizes, windows and value structures (plateaus, values straddling 2^32, negatives, ties),
+    sizes just above the minimum n = h + 1 and around the tile boundaries."""
+    rng = np.random.default_rng(2024)
+    kinds = ["lognormal", "dupes", "zeros", "full64", "plateaus", "straddle32", "negative"]
+    cases = []
+    for _ in range(36):
+        window = int(rng.choice([1, 3, 31, 33, 255, 1001, 2001, 3001, 4097]))
+        h = window // 2
+        n = int(rng.choice([h + 1, h + 2, 2 * h + 1, 6192, 6193, 8192, 8193, 12384, int(rng.integers(h + 1, 40000))]))
+        n = max(n, h + 1)
+        cases.append((n, window, str(rng.choice(kinds)), int(rng.integers(1 << 30))))
+    for n, window, kind, seed in cases:
+        x = wl.random_spectrum(n, seed=seed, kind=kind)
+        out = torch.empty(n, dtype=torch.int64, device="cuda")
+        gb.running_median(dev(torch, x), n, 1, window, out)
+        assert np.array_equal(out.cpu().numpy(), orc.running_median(x, window)), (n, window, kind, seed)
+        s = torch.empty(n, dtype=torch.int64, device="cuda")
+        gb.running_mean(dev(torch, x), n, 1, window, s)
+        assert np.array_equal(s.cpu().numpy(), orc.running_sum(x, window)), (n, window, kind, seed)
