@@ -77,6 +77,7 @@ scan_tile_sums_kernel(const int64_t *__restrict__ diff, int64_t n_bins, int tile
                       int64_t *__restrict__ tile_sums, const int *__restrict__ wide_flag,
                       const int *__restrict__ scan_stamp, int stamp)
 {
+    gbfg_let_next_kernel_start();
     if (*wide_flag != stamp) return;
     const int64_t ti = (int64_t)blockIdx.y * tiles_per_row + blockIdx.x;
     if (scan_stamp[ti] != stamp) return;
@@ -107,6 +108,7 @@ scan_add_kernel(int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
                 const int64_t *__restrict__ tile_sums, int64_t *__restrict__ spectrum,
                 const int *__restrict__ wide_flag, const int *__restrict__ scan_stamp, int stamp)
 {
+    gbfg_wait_prior_kernel();                           // the tile sums
     if (*wide_flag != stamp) return;
     __shared__ int64_t warp_tot[SCAN_THREADS / 32];
     __shared__ int64_t tile_offset;
@@ -200,7 +202,9 @@ int launch_scan(int64_t n_bins, int n_cat, int64_t *spectrum, int64_t *diff, int
     LaunchTimer lt_scan(K_SCAN, st);     // the two scan kernels, as one
     scan_tile_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, n_bins, tiles, tile_sums, wide_flag, mk.scan_stamp, mk.stamp);
     GBFG_LAUNCH_CHECK("scan_tile_sums_kernel");
-    scan_add_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, n_bins, tiles, tile_sums, spectrum, wide_flag, mk.scan_stamp, mk.stamp);
+    cudaError_t e = launch_dependent(scan_add_kernel, grid, dim3(SCAN_THREADS), 0, st, diff, n_bins, tiles,
+                                     (const int64_t *)tile_sums, spectrum, (const int *)wide_flag, (const int *)mk.scan_stamp, mk.stamp);
+    if (e != cudaSuccess) return set_cuda_error(e, "scan_add_kernel");
     GBFG_LAUNCH_CHECK("scan_add_kernel");
     return GBFG_OK;
 }

@@ -46,6 +46,26 @@ struct LaunchTimer {
         if (e__ != cudaSuccess) return gbfg::set_cuda_error(e__, name);        \
     } while (0)
 
+// Programmatic dependent launch (sm_90+): the kernel is queued so that its CTAs may start while the kernel before
+// it on the stream is still draining; it must call gbfg_wait_prior_kernel() before it touches anything that kernel
+// wrote.  A kernel that lets its successor start early calls gbfg_let_next_kernel_start() (all its CTAs are
+// resident by then, so the early CTAs of the successor can only take slots that are free).
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_dependent(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+#ifdef __CUDACC__
+__device__ __forceinline__ void gbfg_wait_prior_kernel() { cudaGridDependencySynchronize(); }
+__device__ __forceinline__ void gbfg_let_next_kernel_start() { cudaTriggerProgrammaticLaunchCompletion(); }
+#endif
+
 // Per-batch catalog table passed by value to kernels (<= GBFG_MAX_CAT catalogs).
 struct CatTable {
     int32_t n_cat;

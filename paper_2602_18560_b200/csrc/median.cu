@@ -299,8 +299,10 @@ int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64
     a.items = a.wide_items; a.ctr = a.wide_ctr;
     a.wide_items = nullptr; a.wide_ctr = nullptr;
     if (grid > sms) grid = sms;
-    if (delta_bits) running_median_tile_kernel<uint64_t, 1024, true><<<(int)grid, 1024, smem64, st>>>(a);
-    else running_median_tile_kernel<uint64_t, 1024, false><<<(int)grid, 1024, smem64, st>>>(a);
+    cudaError_t e = delta_bits
+        ? launch_dependent(running_median_tile_kernel<uint64_t, 1024, true>, dim3((unsigned)grid), dim3(1024), smem64, st, a)
+        : launch_dependent(running_median_tile_kernel<uint64_t, 1024, false>, dim3((unsigned)grid), dim3(1024), smem64, st, a);
+    if (e != cudaSuccess) return set_cuda_error(e, "running_median_tile_kernel<u64>");
     GBFG_LAUNCH_CHECK("running_median_tile_kernel<u64>");
     return GBFG_OK;
 }

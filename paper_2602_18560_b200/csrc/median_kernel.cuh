@@ -111,6 +111,8 @@ running_median_tile_kernel(MedianArgs a)
     const int h = a.h, W = 2 * a.h + 1;
     __shared__ int s_item;
     bool neg = false;
+    gbfg_let_next_kernel_start();                        // the wide-tile kernel / the prefix may queue up behind this one
+    gbfg_wait_prior_kernel();                            // (launched as a dependent: the 32-bit kernel's wide list)
 
   for (int64_t turn = blockIdx.x;; turn += gridDim.x) {
     int64_t row, o0;

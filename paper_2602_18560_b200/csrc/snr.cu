@@ -150,6 +150,8 @@ inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tile
     __shared__ U128 carry_s;
     __shared__ int is_last;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    gbfg_let_next_kernel_start();
+    gbfg_wait_prior_kernel();                               // the PSD of this pass
     bool clean = false;
     if (dv.cum) {                                           // psd of this tile unchanged: its prefix stands
         const int64_t k_first = (int64_t)blockIdx.x * PFX_TILE;
@@ -440,6 +442,7 @@ struct SnrArgs {
 __global__ void __launch_bounds__(256)
 snr_cand_kernel(SnrArgs a)
 {
+    gbfg_wait_prior_kernel();                               // the prefix of this pass
     if (a.abort_flag && *a.abort_flag) return;
     if (a.delta_bits && __longlong_as_double((long long)a.delta_bits[blockIdx.y]) <= a.psd_rtol) return;   // S_n has converged
     const int lane = threadIdx.x & 31;
@@ -605,8 +608,9 @@ int launch_inv_prefix(const double *psd, int64_t n_bins, int n_cat, const SnrWor
     const int tiles = pfx_tiles_per_row(n_bins);
     LaunchTimer lt(K_INV_BLOCKS, st);
     unsigned *ticket = reinterpret_cast<unsigned *>((char *)sw.hdr + sizeof(PrefixHeader) + sizeof(PrefixScratch));
-    inv_prefix_local_kernel<<<dim3(tiles, n_cat), PFX_THREADS, 0, st>>>(psd, n_bins, tiles, (U128 *)sw.pref, (U128 *)sw.tile_tot,
-                                                                        (U128 *)sw.tile_off, (PrefixHeader *)sw.hdr, dv, ticket);
+    cudaError_t e = launch_dependent(inv_prefix_local_kernel, dim3(tiles, n_cat), dim3(PFX_THREADS), 0, st, psd, n_bins, tiles,
+                                     (U128 *)sw.pref, (U128 *)sw.tile_tot, (U128 *)sw.tile_off, (PrefixHeader *)sw.hdr, dv, ticket);
+    if (e != cudaSuccess) return set_cuda_error(e, "inv_prefix_local_kernel");
     GBFG_LAUNCH_CHECK("inv_prefix_local_kernel");
     return GBFG_OK;
 }
@@ -680,7 +684,8 @@ int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th,
     if (cap < 4) cap = 4;
     if (blocks > cap) blocks = cap;
     LaunchTimer lt(K_SNR, st);
-    snr_cand_kernel<<<dim3((unsigned)blocks, (unsigned)n_cat), 256, 0, st>>>(a);
+    cudaError_t e = launch_dependent(snr_cand_kernel, dim3((unsigned)blocks, (unsigned)n_cat), dim3(256), 0, st, a);
+    if (e != cudaSuccess) return set_cuda_error(e, "snr_cand_kernel");
     GBFG_LAUNCH_CHECK("snr_cand_kernel");
     return GBFG_OK;
 }
