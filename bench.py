@@ -330,6 +330,7 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index (default 3: the headline 1e7-source run)")
     ap.add_argument("--n-src", type=int, default=None, help="override the number of sources (parity/debug only)")
     ap.add_argument("--flags", type=int, default=0, help="gbfg_iter_params.flags")
+    ap.add_argument("--max-iter", type=int, default=None, help="override the iteration cap (debug only: cost per iteration)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--traffic", type=float, default=None,
@@ -338,6 +339,8 @@ def main():
     w = wl.config(args.config)
     if args.n_src is not None:
         w = wl.scaled(w, n_src=args.n_src, name=f"{w.name}_n{args.n_src}")
+    if args.max_iter is not None:
+        w = wl.replace(w, max_iter=args.max_iter, name=f"{w.name}_cap{args.max_iter}")
     if args.impl == "reference":
         return run_reference(args, w)
     return run_gpu(args, w)
