@@ -114,15 +114,20 @@ running_median_tile_kernel(MedianArgs a)
     gbfg_let_next_kernel_start();                        // the wide-tile kernel / the prefix may queue up behind this one
     gbfg_wait_prior_kernel();                            // (launched as a dependent: the 32-bit kernel's wide list)
 
+    // work list: the first item of a CTA is its own index, the following ones come from the ticket counter,
+    // drawn just before the epilogue so that the atomic's round trip is hidden behind it (earlier would
+    // hand the last items to CTAs that are still busy)
+    const int n_items = a.items ? a.ctr[0] : 0;
+    int next_item = blockIdx.x;
   for (int64_t turn = blockIdx.x;; turn += gridDim.x) {
     int64_t row, o0;
     int n_out, row_i;
     __syncthreads();                                     // the previous tile's epilogue is done with shared memory
     if (a.items) {
-        if (tid == 0) s_item = atomicAdd(&a.ctr[1], 1);
+        if (tid == 0) s_item = next_item;
         __syncthreads();
         const int item = s_item;
-        if (item >= a.ctr[0]) break;
+        if (item >= n_items) break;
         const int4 v = a.items[item];
         row_i = v.x;
         o0 = v.y;
@@ -183,7 +188,10 @@ running_median_tile_kernel(MedianArgs a)
     __syncthreads();
     const uint64_t vary_all = ((uint64_t)misc[33] << 32) | misc[32];
     if (NARROW && (vary_all >> 32) != 0) {               // 32 bits do not order this tile: leave it to the wide kernel
-        if (tid == 0) a.wide_items[atomicAdd(&a.wide_ctr[0], 1)] = make_int4(row_i, (int)o0, n_out, 0);
+        if (tid == 0) {
+            a.wide_items[atomicAdd(&a.wide_ctr[0], 1)] = make_int4(row_i, (int)o0, n_out, 0);
+            if (a.items) next_item = (int)gridDim.x + atomicAdd(&a.ctr[1], 1);
+        }
         continue;
     }
     const int n_pass = vary_all ? (64 - __clzll((long long)vary_all) + 7) / 8 : 0;
@@ -452,6 +460,7 @@ running_median_tile_kernel(MedianArgs a)
     __syncthreads();
 
     // ---- coalesced epilogue: median and PSD
+    if (a.items && tid == 0) next_item = (int)gridDim.x + atomicAdd(&a.ctr[1], 1);
     double dmax = 0.0;
     for (int j0 = tid; j0 < n_out; j0 += 4 * THREADS) {
         double si[4];

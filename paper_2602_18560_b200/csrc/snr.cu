@@ -140,7 +140,9 @@ prefix_header_kernel(const double *__restrict__ arr, int64_t n, int64_t n_bins_r
 }
 
 // phase A: local inclusive prefix of every tile of PFX_TILE bins + the tile totals (skipped for
-// tiles without a dirty block: their prefix stands)
+// tiles without a dirty block: their prefix stands).  gridDim.x CTAs per row, resident together; CTA b
+// takes the tiles b, b + gridDim.x, ...: 32 of them are looked up at once (lane l the l-th), so a pass
+// with a handful of dirty tiles costs one look-up per CTA, not one CTA per tile.
 __global__ void __launch_bounds__(PFX_THREADS, 3)
 inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tiles_per_row,
                         U128 *__restrict__ pref, U128 *__restrict__ tile_tot, U128 *__restrict__ tile_off,
@@ -152,67 +154,82 @@ inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tile
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     gbfg_let_next_kernel_start();
     gbfg_wait_prior_kernel();                               // the PSD of this pass
-    bool clean = false;
-    if (dv.cum) {                                           // psd of this tile unchanged: its prefix stands
-        const int64_t k_first = (int64_t)blockIdx.x * PFX_TILE;
-        int64_t k_last = k_first + PFX_TILE - 1;
-        if (k_last > n_bins - 1) k_last = n_bins - 1;
-        const int *cum = dv.cum + (int64_t)blockIdx.y * (dv.n_dblk + 1);
-        clean = cum[(k_last >> dv.dblk_log2) + 1] == cum[k_first >> dv.dblk_log2];
+    const int *cum = dv.cum ? dv.cum + (int64_t)blockIdx.y * (dv.n_dblk + 1) : nullptr;
+    const int64_t row = (int64_t)blockIdx.y * n_bins;
+    int ok = 1;
+    int U = 0, e_top = 0;
+    bool have_hdr = false;
+    for (int t0 = blockIdx.x; t0 < tiles_per_row; t0 += 32 * gridDim.x) {
+        const int t_mine = t0 + lane * gridDim.x;
+        bool dirty = t_mine < tiles_per_row;
+        if (dirty && cum) {                                 // psd of this tile unchanged: its prefix stands
+            const int64_t k_first = (int64_t)t_mine * PFX_TILE;
+            int64_t k_last = k_first + PFX_TILE - 1;
+            if (k_last > n_bins - 1) k_last = n_bins - 1;
+            dirty = cum[(k_last >> dv.dblk_log2) + 1] != cum[k_first >> dv.dblk_log2];
+        }
+        for (unsigned todo = __ballot_sync(0xffffffffu, dirty); todo; todo &= todo - 1) {
+            const int tile = t0 + (__ffs(todo) - 1) * gridDim.x;
+            if (!have_hdr) { U = hdr->unit_exp; e_top = hdr->e_top; have_hdr = true; }
+            const int64_t base = (int64_t)tile * PFX_TILE + (int64_t)threadIdx.x * PFX_ITEMS;
+            U128 v[PFX_ITEMS];
+            U128 run; run.lo = 0; run.hi = 0;
+#pragma unroll
+            for (int j = 0; j < PFX_ITEMS; ++j) {
+                const int64_t k = base + j;
+                U128 t; t.lo = 0; t.hi = 0;
+                if (k < n_bins) t = inv_to_fixed(psd[row + k], U, e_top, &ok);
+                run = u128_add(run, t);
+                v[j] = run;
+            }
+            U128 incl = run;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                U128 up = u128_shfl_up(incl, o);
+                if (lane >= o) incl = u128_add(incl, up);
+            }
+            __syncthreads();                                // the last tile's readers of wtot are done
+            if (lane == 31) wtot[warp] = incl;
+            __syncthreads();
+            U128 before = u128_sub(incl, run);
+            for (int w = 0; w < warp; ++w) before = u128_add(before, wtot[w]);
+#pragma unroll
+            for (int j = 0; j < PFX_ITEMS; ++j) {
+                const int64_t k = base + j;
+                if (k < n_bins) pref[row + k] = u128_add(before, v[j]);
+            }
+            if (threadIdx.x == PFX_THREADS - 1) {
+                tile_tot[(int64_t)blockIdx.y * tiles_per_row + tile] = u128_add(before, run);
+                __threadfence();
+            }
+        }
     }
-    if (!clean) {
-        const int U = hdr->unit_exp, e_top = hdr->e_top;
-        const int64_t row = (int64_t)blockIdx.y * n_bins;
-        const int64_t base = (int64_t)blockIdx.x * PFX_TILE + (int64_t)threadIdx.x * PFX_ITEMS;
-        U128 v[PFX_ITEMS];
-        U128 run; run.lo = 0; run.hi = 0;
-        int ok = 1;
-#pragma unroll
-        for (int j = 0; j < PFX_ITEMS; ++j) {
-            const int64_t k = base + j;
-            U128 t; t.lo = 0; t.hi = 0;
-            if (k < n_bins) t = inv_to_fixed(psd[row + k], U, e_top, &ok);
-            run = u128_add(run, t);
-            v[j] = run;
-        }
-        U128 incl = run;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            U128 up = u128_shfl_up(incl, o);
-            if (lane >= o) incl = u128_add(incl, up);
-        }
-        if (lane == 31) wtot[warp] = incl;
-        __syncthreads();
-        U128 before = u128_sub(incl, run);
-        for (int w = 0; w < warp; ++w) before = u128_add(before, wtot[w]);
-#pragma unroll
-        for (int j = 0; j < PFX_ITEMS; ++j) {
-            const int64_t k = base + j;
-            if (k < n_bins) pref[row + k] = u128_add(before, v[j]);
-        }
-        if (threadIdx.x == PFX_THREADS - 1) {
-            tile_tot[(int64_t)blockIdx.y * tiles_per_row + blockIdx.x] = u128_add(before, run);
-            __threadfence();
-        }
-        if (!ok) hdr->bad = 1;
-    }
+    if (!ok) hdr->bad = 1;
     // phase B by the last CTA of the row to finish: exclusive scan of the row's tile totals
     __syncthreads();
     if (threadIdx.x == 0) {
-        is_last = atomicAdd(ticket + blockIdx.y, 1u) == (unsigned)tiles_per_row - 1u;
+        is_last = atomicAdd(ticket + blockIdx.y, 1u) == gridDim.x - 1u;
         carry_s.lo = 0; carry_s.hi = 0;
     }
     __syncthreads();
     if (!is_last) return;
     __threadfence();
     if (threadIdx.x == 0) ticket[blockIdx.y] = 0u;
+    // PFX_ITEMS consecutive tiles per thread: one round of loads, one block scan per PFX_TILE tiles
     const volatile uint64_t *totp = reinterpret_cast<const volatile uint64_t *>(tile_tot + (int64_t)blockIdx.y * tiles_per_row);
     U128 *outp = tile_off + (int64_t)blockIdx.y * tiles_per_row;
-    for (int b = 0; b < tiles_per_row; b += PFX_THREADS) {
-        const int idx = b + threadIdx.x;
-        U128 v; v.lo = 0; v.hi = 0;
-        if (idx < tiles_per_row) { v.lo = totp[2 * idx]; v.hi = totp[2 * idx + 1]; }
-        U128 incl = v;
+    for (int b = 0; b < tiles_per_row; b += PFX_TILE) {
+        const int i0 = b + threadIdx.x * PFX_ITEMS;
+        U128 v[PFX_ITEMS];
+#pragma unroll
+        for (int j = 0; j < PFX_ITEMS; ++j) {
+            v[j].lo = 0; v[j].hi = 0;
+            if (i0 + j < tiles_per_row) { v[j].lo = totp[2 * (i0 + j)]; v[j].hi = totp[2 * (i0 + j) + 1]; }
+        }
+        U128 run = v[0];
+#pragma unroll
+        for (int j = 1; j < PFX_ITEMS; ++j) run = u128_add(run, v[j]);
+        U128 incl = run;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
             U128 up = u128_shfl_up(incl, o);
@@ -221,11 +238,15 @@ inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tile
         __syncthreads();
         if (lane == 31) wtot[warp] = incl;
         __syncthreads();
-        U128 before = carry_s;
+        U128 before = u128_add(carry_s, u128_sub(incl, run));
         for (int w = 0; w < warp; ++w) before = u128_add(before, wtot[w]);
-        if (idx < tiles_per_row) outp[idx] = u128_add(before, u128_sub(incl, v));
+#pragma unroll
+        for (int j = 0; j < PFX_ITEMS; ++j) {
+            if (i0 + j < tiles_per_row) outp[i0 + j] = before;
+            before = u128_add(before, v[j]);
+        }
         __syncthreads();
-        if (threadIdx.x == PFX_THREADS - 1) carry_s = u128_add(before, incl);
+        if (threadIdx.x == PFX_THREADS - 1) carry_s = before;
         __syncthreads();
     }
 }
@@ -606,9 +627,11 @@ int launch_prefix_header(const double *arr, int64_t n, int64_t n_bins_row, const
 int launch_inv_prefix(const double *psd, int64_t n_bins, int n_cat, const SnrWork &sw, const DirtyView &dv, cudaStream_t st)
 {
     const int tiles = pfx_tiles_per_row(n_bins);
+    int per_row = (3 * sm_count() + n_cat - 1) / n_cat;        // three CTAs per SM over all rows
+    if (per_row > tiles) per_row = tiles;
     LaunchTimer lt(K_INV_BLOCKS, st);
     unsigned *ticket = reinterpret_cast<unsigned *>((char *)sw.hdr + sizeof(PrefixHeader) + sizeof(PrefixScratch));
-    cudaError_t e = launch_dependent(inv_prefix_local_kernel, dim3(tiles, n_cat), dim3(PFX_THREADS), 0, st, psd, n_bins, tiles,
+    cudaError_t e = launch_dependent(inv_prefix_local_kernel, dim3(per_row, n_cat), dim3(PFX_THREADS), 0, st, psd, n_bins, tiles,
                                      (U128 *)sw.pref, (U128 *)sw.tile_tot, (U128 *)sw.tile_off, (PrefixHeader *)sw.hdr, dv, ticket);
     if (e != cudaSuccess) return set_cuda_error(e, "inv_prefix_local_kernel");
     GBFG_LAUNCH_CHECK("inv_prefix_local_kernel");
