@@ -157,8 +157,7 @@ inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tile
     const int *cum = dv.cum ? dv.cum + (int64_t)blockIdx.y * (dv.n_dblk + 1) : nullptr;
     const int64_t row = (int64_t)blockIdx.y * n_bins;
     int ok = 1;
-    int U = 0, e_top = 0;
-    bool have_hdr = false;
+    const int U = hdr->unit_exp, e_top = hdr->e_top;        // in flight together with the first dirty look-up
     for (int t0 = blockIdx.x; t0 < tiles_per_row; t0 += 32 * gridDim.x) {
         const int t_mine = t0 + lane * gridDim.x;
         bool dirty = t_mine < tiles_per_row;
@@ -170,7 +169,6 @@ inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tile
         }
         for (unsigned todo = __ballot_sync(0xffffffffu, dirty); todo; todo &= todo - 1) {
             const int tile = t0 + (__ffs(todo) - 1) * gridDim.x;
-            if (!have_hdr) { U = hdr->unit_exp; e_top = hdr->e_top; have_hdr = true; }
             const int64_t base = (int64_t)tile * PFX_TILE + (int64_t)threadIdx.x * PFX_ITEMS;
             U128 v[PFX_ITEMS];
             U128 run; run.lo = 0; run.hi = 0;
@@ -464,24 +462,31 @@ __global__ void __launch_bounds__(256)
 snr_cand_kernel(SnrArgs a)
 {
     gbfg_wait_prior_kernel();                               // the prefix of this pass
-    if (a.abort_flag && *a.abort_flag) return;
-    if (a.delta_bits && __longlong_as_double((long long)a.delta_bits[blockIdx.y]) <= a.psd_rtol) return;   // S_n has converged
-    const int lane = threadIdx.x & 31;
-    // records of row blockIdx.y, narrowed to the buckets that can reach a dirty block
+    // every look-up that does not depend on another one is issued before the first is used (a late pass is a
+    // chain of L2 round trips, not work)
     const int rowc = blockIdx.y;
     const int64_t *off = a.bkt_off + (int64_t)rowc * (a.n_dblk + 1);
+    const int abort_v = a.abort_flag ? *a.abort_flag : 0;
+    const unsigned long long dbits = a.delta_bits ? a.delta_bits[rowc] : 0ull;
+    const int near_v = a.dv.cum ? *a.any_near : 1;
+    const int b_min = a.dv.cum ? a.dv.range[2 * rowc] : 0, b_max = a.dv.cum ? a.dv.range[2 * rowc + 1] : 0;
+    const int hdr_bad = a.pv.pref ? a.pv.hdr->bad : 1;
+    const int unit_exp = a.pv.pref ? a.pv.hdr->unit_exp : 0;
     int64_t t_first = off[0], n = off[a.n_dblk];
-    if (a.dv.cum && *a.any_near == 0) {
-        const int b_min = a.dv.range[2 * rowc], b_max = a.dv.range[2 * rowc + 1];
+    if (abort_v) return;
+    if (a.delta_bits && __longlong_as_double((long long)dbits) <= a.psd_rtol) return;   // S_n has converged
+    const int lane = threadIdx.x & 31;
+    // records of row blockIdx.y, narrowed to the buckets that can reach a dirty block
+    if (a.dv.cum && near_v == 0) {
         if (b_min > b_max) return;                          // nothing dirty in this row
+        const int64_t n_hi = off[b_max + 1];
         const int first_bucket = a.bkt_reach[(int64_t)rowc * a.n_dblk + b_min];
         if (first_bucket >= a.n_dblk) return;
         t_first = off[first_bucket];
-        n = off[b_max + 1];
+        n = n_hi;
     }
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    const bool pref_ok = a.pv.pref && a.pv.hdr->bad == 0;
-    const int unit_exp = a.pv.pref ? a.pv.hdr->unit_exp : 0;
+    const bool pref_ok = hdr_bad == 0;
     // The selected indices of the CTA are collected in shared memory and appended to the list with
     // one global atomic per flush (tens of thousands of sources pass in the first iterations: one
     // atomic per warp on a single address is what the kernel then waits for).
@@ -493,14 +498,13 @@ snr_cand_kernel(SnrArgs a)
     for (int64_t t0 = t_first + (int64_t)blockIdx.x * blockDim.x; t0 < n; t0 += stride) {
         const int64_t t = t0 + threadIdx.x;
         int32_t w = 0;
-        if (t < n) w = a.cand.w[t];
+        int64_t src = -1, gk0 = 0;
+        if (t < n) { w = a.cand.w[t]; gk0 = a.cand.gk0[t]; }
         bool sel = false, near = false;
         const int cat = rowc;
-        int64_t src = -1, gk0 = 0;
         const bool always = w < 0;                          // was near the threshold: counted every iteration
         if (always) w = -w;
         if (w > 0) {
-            gk0 = a.cand.gk0[t];
             if (a.dv.cum && !always) {
                 // the PSD under this source is what it was at its last test: same rho2, same answer
                 const int64_t k0 = gk0 - (int64_t)cat * a.n_bins;
