@@ -631,7 +631,8 @@ int launch_prefix_header(const double *arr, int64_t n, int64_t n_bins_row, const
 int launch_inv_prefix(const double *psd, int64_t n_bins, int n_cat, const SnrWork &sw, const DirtyView &dv, cudaStream_t st)
 {
     const int tiles = pfx_tiles_per_row(n_bins);
-    int per_row = (3 * sm_count() + n_cat - 1) / n_cat;        // three CTAs per SM over all rows
+    int per_row = (3 * sm_count() + n_cat - 1) / n_cat;        // three CTAs per SM over all rows;
+    if (per_row < 64) per_row = 64;                            // a batch: more, shorter CTAs (rows differ in how dirty they are)
     if (per_row > tiles) per_row = tiles;
     LaunchTimer lt(K_INV_BLOCKS, st);
     unsigned *ticket = reinterpret_cast<unsigned *>((char *)sw.hdr + sizeof(PrefixHeader) + sizeof(PrefixScratch));
