@@ -342,13 +342,15 @@ cand_build_kernel(GridDev g, CatTable ct, BuildArgs a)
             int64_t base = 0;
             if (lane == 0) base = (int64_t)atomicAdd((unsigned long long *)a.cand_count, (unsigned long long)__popc(mask));
             base = __shfl_sync(0xffffffffu, base, 0);
+            const unsigned same = ct.n_cat > 1 ? __match_any_sync(0xffffffffu, keep ? cat : -1) : 0u;   // kept lanes of my catalog
             if (keep) {
                 const int64_t t = base + __popc(mask & ((1u << lane) - 1u));
                 a.cand.gk0[t] = (int64_t)cat * g.n_bins + s.k0;
                 a.cand.w[t] = (int32_t)s.w_eff;
                 a.cand.four_p[t] = 4.0 * s.p;
                 a.cand.src[t] = i;
-                if (ct.n_cat > 1) atomicAdd((unsigned long long *)(a.cand_count + 1 + cat), 1ull);
+                if (ct.n_cat > 1 && lane == __ffs(same) - 1)   // one add per warp and catalog (a warp rarely straddles two)
+                    atomicAdd((unsigned long long *)(a.cand_count + 1 + cat), (unsigned long long)__popc(same));
                 const int64_t gb = (int64_t)cat * a.n_dblk + (s.k0 >> a.dblk_log2);
                 atomicAdd(a.bkt_count + gb, 1);
                 atomicMax(a.bkt_ext + gb, (int)((s.k0 + s.w_eff - 1) >> a.dblk_log2));
