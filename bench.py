@@ -158,6 +158,9 @@ def algorithmic_bytes(w: wl.Workload, n_bins: int, res, prof) -> dict:
 # dram__bytes_read.sum + dram__bytes_write.sum of running_median_kernel per output it recomputes, from the
 # committed `ncu --set full` capture (profiles/r01_ncu_full_v3.md: 67.1 MB for ~3.4e6 outputs)
 MEDIAN_DRAM_BYTES_PER_OUTPUT = 20.0
+# smsp__inst_executed.sum of the same kernel per output it recomputes (profiles/r01_ncu_full_v3.md: 1.14e8 warp
+# instructions for a full pass of 3 774 349 outputs; r01_ncu_full_v5.md: 9.97e7 for ~3.4e6)
+MEDIAN_WARP_INSTR_PER_OUTPUT = 30.0
 
 
 def run_gpu(args, w: wl.Workload):
@@ -286,6 +289,19 @@ def run_gpu(args, w: wl.Workload):
                 "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_ms": kd["avg_launch_ms"],
                 "traffic": traffic}
 
+    # What actually bounds the running median is instruction issue, not HBM: the same launches
+    # against the issue rate of the part, 4 warp instructions per SM and clock (B200_PROFILING.md: 148 SMs x 4 schedulers)
+    roofline_issue = None
+    if dom == "median":
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        mhz = (clk or {}).get("sm_mhz") or (clk or {}).get("sm_max_mhz") or 1965.0
+        peak_issue = sms * 4 * mhz * 1e6 / 1e9                      # G warp-instructions / s
+        ach = MEDIAN_WARP_INSTR_PER_OUTPUT * (bytes_per_launch / 32.0) / (kd["avg_launch_ms"] * 1e-3) / 1e9
+        roofline_issue = {"kernel": dom, "bound": "alu", "achieved": ach, "peak": peak_issue,
+                          "unit": "G warp-instr/s", "frac": ach / peak_issue,
+                          "peak_source": f"{sms} SMs x 4 schedulers x {mhz:.0f} MHz (sm clock under load)",
+                          "instr_per_output": MEDIAN_WARP_INSTR_PER_OUTPUT}
+
     # ---- the oracle on the host cores, bounded sample
     cpu = None
     if not args.no_cpu_baseline:
@@ -312,6 +328,7 @@ def run_gpu(args, w: wl.Workload):
         "gpu_launches": int(launches),
         "clocks": clk,
         "roofline": roofline,
+        "roofline_issue": roofline_issue,
         "kernels": kernels,
         "cpu_baseline": cpu,
     }
