@@ -29,7 +29,7 @@ int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64
                   const double *s_instr, double *psd, double norm, int scale_log2,
                   const MedianPlan *plan, int4 *wide_items, int *wide_ctr, int *neg_flag,
                   unsigned long long *delta_bits, cudaStream_t st);
-int launch_mean(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *sum,
+int launch_mean(const DirtyView *dv, const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *sum,
                 const double *s_instr, double *psd, int scale_log2, int *neg_flag, unsigned long long *delta_bits,
                 cudaStream_t st);
 int pfx_tiles_per_row(int64_t n_bins);
@@ -365,7 +365,6 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
         if (rc) return rc;
     }
 
-    int64_t mean_passes = 0;
     bool done[GBFG_MAX_CAT];
     for (int c = 0; c < n_cat; ++c) {
         memset(&host_results[c], 0, sizeof(gbfg_iter_result));
@@ -384,15 +383,14 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
             GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_plan, 0));
         } else {
             rc = launch_plan(w.blk_stamp, it, it == 0 || !incremental, nb, n_cat, W, w.plan, w.counters, (int)n_iter_counters,
-                             use_mean ? nullptr : med_outputs, delta_all, st);
+                             med_outputs, delta_all, st);
             if (rc) return rc;
         }
         plan_queued = false;
         // second stop rule (R13): from the second pass on the estimator also records the largest relative PSD change
         unsigned long long *delta = (psd_rtol > 0.0 && it > 0) ? delta_all : nullptr;
-        if (use_mean) {      // eq. (D1): HBM bound, every bin every iteration
-            rc = launch_mean(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, grid->scale_log2, neg_flag, delta, st);
-            ++mean_passes;
+        if (use_mean) {      // eq. (D1): HBM bound; tiles without a dirty block keep their sums and PSD
+            rc = launch_mean(&dirty, dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, grid->scale_log2, neg_flag, delta, st);
         } else {
             rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
                                grid->scale_log2, &w.plan, nullptr, nullptr, neg_flag, delta, st);
@@ -417,11 +415,11 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
         // ... and, on the side stream next to it, the plan of the next pass: it reads the stamps the test wrote
         // and clears the counters the copy above has taken.  After the last iteration it is the plan of the
         // closing median pass.
-        if (!(use_mean && it + 1 == params->max_iter)) {
+        {
             const bool closing = it + 1 == params->max_iter;
             GBFG_CUDA(cudaStreamWaitEvent(side->s, ev_read, 0));
             rc = launch_plan(w.blk_stamp, it + 1, !incremental, nb, n_cat, W, w.plan, closing ? nullptr : w.counters,
-                             closing ? 0 : (int)n_iter_counters, use_mean ? nullptr : med_outputs,
+                             closing ? 0 : (int)n_iter_counters, med_outputs,
                              closing ? nullptr : delta_all, side->s);
             if (rc) return rc;
             GBFG_CUDA(cudaEventRecord(side->ev_plan, side->s));
@@ -474,17 +472,16 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
         // cap hit: the PSD must match the returned residual (rows of converged catalogs are unchanged)
         for (int c = 0; c < n_cat; ++c)
             if (!done[c]) { host_results[c].n_iter = params->max_iter; host_results[c].converged = 0; }
-        if (use_mean) {
-            rc = launch_mean(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, grid->scale_log2, nullptr, nullptr, st);
-            ++mean_passes;
+        if (plan_queued) {
+            GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_plan, 0));
         } else {
-            if (plan_queued) {
-                GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_plan, 0));
-            } else {
-                rc = launch_plan(w.blk_stamp, params->max_iter, !incremental, nb, n_cat, W, w.plan, nullptr, 0, med_outputs, nullptr, st);
-                if (rc) return rc;
-            }
-            plan_queued = false;
+            rc = launch_plan(w.blk_stamp, params->max_iter, !incremental, nb, n_cat, W, w.plan, nullptr, 0, med_outputs, nullptr, st);
+            if (rc) return rc;
+        }
+        plan_queued = false;
+        if (use_mean) {
+            rc = launch_mean(&dirty, dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, grid->scale_log2, nullptr, nullptr, st);
+        } else {
             rc = launch_median(dev_spectrum, nb, n_cat, W, dev_median, dev_s_instr, dev_psd, params->median_norm,
                                grid->scale_log2, &w.plan, nullptr, nullptr, nullptr, nullptr, st);
         }
@@ -494,7 +491,7 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
     GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
     GBFG_CUDA(cudaStreamSynchronize(st));
     for (int c = 0; c < n_cat; ++c) {
-        host_results[c].n_median_outputs = use_mean ? mean_passes * nb : host[i_med + c];
+        host_results[c].n_median_outputs = host[i_med + c];
         host_results[c].n_snr_tests = host[i_tests + c];
     }
     return GBFG_OK;

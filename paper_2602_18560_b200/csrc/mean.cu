@@ -32,6 +32,8 @@ struct MeanArgs {
     double *psd;             // [n_cat][n] or NULL
     int *neg_flag;           // nullable: set to 1 when a window sum is negative
     unsigned long long *delta_bits;   // nullable: [n_cat] largest relative PSD change of the row, as binary64 bits (R13)
+    const int *cum;          // nullable: [n_cat][n_dblk + 1] dirty blocks before each block (DirtyView); a tile without one is skipped
+    int n_dblk, dblk_log2;
     int64_t n;
     int h;
     int S;                   // outputs per tile
@@ -48,6 +50,10 @@ running_mean_kernel(MeanArgs a)
     const int64_t row = (int64_t)blockIdx.y * a.n;
     const int64_t o0 = (int64_t)blockIdx.x * a.S;
     const int n_out = (int)((a.n - o0 < a.S) ? (a.n - o0) : a.S);
+    if (a.cum) {                                           // no output of the tile saw a changed bin: sums and PSD stand
+        const int *cum = a.cum + (int64_t)blockIdx.y * (a.n_dblk + 1);
+        if (cum[((o0 + n_out - 1) >> a.dblk_log2) + 1] == cum[o0 >> a.dblk_log2]) return;
+    }
     const int h = a.h;
     const int Lt = n_out + 2 * h;                          // position p <-> bin o0 - h + p, reflected
 
@@ -142,11 +148,14 @@ running_mean_kernel(MeanArgs a)
 }
 
 // internal entry: window sums (+ PSD when psd != NULL) of every row
-int launch_mean(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *sum,
+int launch_mean(const DirtyView *dv, const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *sum,
                 const double *s_instr, double *psd, int scale_log2, int *neg_flag, unsigned long long *delta_bits,
                 cudaStream_t st)
 {
     MeanArgs a;
+    a.cum = dv ? dv->cum : nullptr;
+    a.n_dblk = dv ? dv->n_dblk : 0;
+    a.dblk_log2 = dv ? dv->dblk_log2 : 0;
     a.delta_bits = delta_bits;
     a.x = x; a.sum = sum; a.s_instr = s_instr; a.psd = psd; a.neg_flag = neg_flag;
     a.n = n_bins; a.h = window / 2;
@@ -189,6 +198,6 @@ extern "C" int gbfg_running_mean(const int64_t *dev_spectrum, int64_t n_bins, in
     if (n_bins < window / 2 + 1) return GBFG_ERR_INVALID_ARG;
     int rc = check_device();
     if (rc) return rc;
-    return launch_mean(dev_spectrum, n_bins, n_cat, window, dev_sum_out, dev_s_instr, dev_psd, scale_log2, nullptr, nullptr,
+    return launch_mean(nullptr, dev_spectrum, n_bins, n_cat, window, dev_sum_out, dev_s_instr, dev_psd, scale_log2, nullptr, nullptr,
                        (cudaStream_t)stream);
 }
