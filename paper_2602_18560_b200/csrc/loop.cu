@@ -284,18 +284,21 @@ static int loop_init_workspace(const Workspace &w, int64_t nb, int n_cat, cudaSt
     return GBFG_OK;
 }
 
-// candidate records: with pre-selection, only sources whose rho^2 against S_instr reaches the threshold
-static int loop_build_candidates(const GridDev &g, const CatTable &ct, const double *dev_A, const double *dev_f,
-                                 const double *dev_fdot, const uint8_t *dev_resolved, const double *dev_s_instr,
-                                 double rho_th, bool preselect, const Workspace &w, cudaStream_t st)
+// candidate records: with pre-selection, only sources whose rho^2 against S_instr reaches the threshold.
+// First half: the header and (for the pre-selection) the prefix of 1/S_instr, which need nothing of the catalog.
+static int loop_prefix_s_instr(const GridDev &g, const double *dev_s_instr, bool preselect, const Workspace &w, cudaStream_t st)
 {
     const DirtyView all_dirty = {nullptr, nullptr, 0, 0};
     int rc = launch_prefix_header(dev_s_instr, g.n_bins, g.n_bins, w.sw, st);
     if (rc) return rc;
-    if (preselect) {
-        rc = launch_inv_prefix(dev_s_instr, g.n_bins, 1, w.sw, all_dirty, st);
-        if (rc) return rc;
-    }
+    if (preselect) rc = launch_inv_prefix(dev_s_instr, g.n_bins, 1, w.sw, all_dirty, st);
+    return rc;
+}
+
+static int loop_build_candidates(const GridDev &g, const CatTable &ct, const double *dev_A, const double *dev_f,
+                                 const double *dev_fdot, const uint8_t *dev_resolved, const double *dev_s_instr,
+                                 double rho_th, bool preselect, const Workspace &w, cudaStream_t st)
+{
     return launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, preselect ? dev_s_instr : nullptr, rho_th, nullptr,
                              w.sw, st);
 }
@@ -360,6 +363,8 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
     const DirtyView dirty = {w.plan.cum, w.plan.range, w.plan.n_dblk, w.plan.dblk_log2};
     if (!prepared) {
         rc = loop_init_workspace(w, nb, n_cat, st);
+        if (rc) return rc;
+        rc = loop_prefix_s_instr(g, dev_s_instr, preselect, w, st);
         if (rc) return rc;
         rc = loop_build_candidates(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, dev_s_instr, params->rho_th, preselect, w, st);
         if (rc) return rc;
@@ -529,12 +534,18 @@ extern "C" int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const 
     Workspace w = carve(workspace, grid->n_bins, n, n_cat);
     if (workspace_bytes < w.bytes) return GBFG_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;
-    rc = gbfg_sample_catalog(grid, pops, offsets, n_cat, 0u, seed, dev_A, dev_f, dev_fdot, stream);
-    if (rc) return rc;
     SideStream *side = side_stream();
     if (!side) return set_cuda_error(cudaErrorMemoryAllocation, "side stream");
     const GridDev g = make_grid_dev(grid);
     const int64_t nb = grid->n_bins;
+    const bool preselect = (params->flags & GBFG_FLAG_NO_PRESELECT) == 0;
+    // side stream, next to the sampling: the prefix of 1/S_instr (after whatever the caller queued to produce S_instr)
+    GBFG_CUDA(cudaEventRecord(side->ev_aux, st));
+    GBFG_CUDA(cudaStreamWaitEvent(side->s, side->ev_aux, 0));
+    rc = loop_prefix_s_instr(g, dev_s_instr, preselect, w, side->s);
+    if (rc) return rc;
+    rc = gbfg_sample_catalog(grid, pops, offsets, n_cat, 0u, seed, dev_A, dev_f, dev_fdot, stream);
+    if (rc) return rc;
     const size_t row_bytes = sizeof(int64_t) * (size_t)n_cat * (size_t)nb;
     GBFG_CUDA(cudaMemsetAsync(dev_spectrum, 0, row_bytes, st));
     if (n > 0) GBFG_CUDA(cudaMemsetAsync(dev_resolved, 0, (size_t)n, st));
@@ -543,7 +554,6 @@ extern "C" int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const 
     GBFG_CUDA(cudaEventRecord(side->ev_aux, st));
     // side stream: the candidate records
     GBFG_CUDA(cudaStreamWaitEvent(side->s, side->ev_aux, 0));
-    const bool preselect = (params->flags & GBFG_FLAG_NO_PRESELECT) == 0;
     rc = loop_build_candidates(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, dev_s_instr, params->rho_th, preselect, w, side->s);
     if (rc) return rc;
     GBFG_CUDA(cudaEventRecord(side->ev_aux, side->s));
