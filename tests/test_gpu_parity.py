@@ -776,3 +776,62 @@ def test_running_median_random_sweep(gb, orc, torch):
         s = torch.empty(n, dtype=torch.int64, device="cuda")
         gb.running_mean(dev(torch, x), n, 1, window, s)
         assert np.array_equal(s.cpu().numpy(), orc.running_sum(x, window)), (n, window, kind, seed)
+
+
+def test_loop_batch_mean_estimator(gb, orc, torch):
+    """Ragged batch with the estimator of eq. (D1): rows skip the tiles without a dirty block independently."""
+    w = wl.scaled(wl.config(4), n_cat=3)
+    w = wl.replace(w, pops=[wl.replace(p, n_src=n) for p, n in zip(w.pops, (50_000, 20_003, 70_000))])
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    n, nb, nc = w.n_src_total, g.n_bins, w.n_cat
+    s_instr_h = orc.instrument_noise(og)
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    total, spec, stat = (torch.empty((nc, nb), dtype=torch.int64, device="cuda") for _ in range(3))
+    psd = torch.empty((nc, nb), dtype=torch.float64, device="cuda")
+    resolved = torch.empty(n, dtype=torch.uint8, device="cuda")
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter, gb.FLAG_ESTIMATOR_MEAN)
+    res = gb.simulate(g, w.pops, w.offsets(), w.seed, dev(torch, s_instr_h), params, A, f, fd, total, spec, stat, psd,
+                      resolved, workspace(torch, gb, g, n, nc))
+    off = w.offsets()
+    for c in range(nc):
+        ref = orc.simulate(w, cat=c, estimator=1)
+        s = slice(int(off[c]), int(off[c + 1]))
+        assert np.array_equal(spec[c].cpu().numpy(), ref["residual"])
+        assert np.array_equal(stat[c].cpu().numpy(), ref["median"])
+        assert np.array_equal(bits(psd[c].cpu().numpy()), bits(ref["psd"]))
+        assert np.array_equal(resolved[s].cpu().numpy(), ref["resolved"])
+        assert (res[c].n_iter, res[c].converged, res[c].n_resolved) == (ref["n_iter"], ref["converged"], ref["n_resolved"])
+        # what the estimator recomputed: everything in the first pass, never more than everything later
+        assert nb <= res[c].n_median_outputs <= (ref["n_iter"] + 1) * nb
+
+
+def test_simulate_back_to_back_on_a_stream(gb, orc, torch):
+    """Two calls queued on one non-default stream right behind the kernel that writes S_instr, sharing the workspace:
+    the library's side stream must order itself behind the caller's stream, and a call leaves nothing in flight."""
+    w = wl.config(0)
+    g = gpu_grid(gb, w)
+    n, nb = w.n_src_total, g.n_bins
+    refs = [orc.simulate(wl.replace(w, seed=s)) for s in (w.seed, w.seed + 1)]
+    st = torch.cuda.Stream()
+    ws = workspace(torch, gb, g, n)
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter)
+    outs = []
+    with torch.cuda.stream(st):
+        s_instr = torch.full((nb,), float("nan"), dtype=torch.float64, device="cuda")
+        gb.instrument_noise(g, s_instr, stream=st)                          # not synchronised before the calls below
+        for k, s in enumerate((w.seed, w.seed + 1)):
+            A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+            total, spec, med = (torch.empty(nb, dtype=torch.int64, device="cuda") for _ in range(3))
+            psd = torch.empty(nb, dtype=torch.float64, device="cuda")
+            resolved = torch.empty(n, dtype=torch.uint8, device="cuda")
+            res = gb.simulate(g, w.pops, w.offsets(), s, s_instr, params, A, f, fd, total, spec, med, psd, resolved, ws,
+                              stream=st)[0]
+            outs.append((res, spec, med, psd, resolved))
+    st.synchronize()
+    for ref, (res, spec, med, psd, resolved) in zip(refs, outs):
+        assert np.array_equal(spec.cpu().numpy(), ref["residual"])
+        assert np.array_equal(med.cpu().numpy(), ref["median"])
+        assert np.array_equal(bits(psd.cpu().numpy()), bits(ref["psd"]))
+        assert np.array_equal(resolved.cpu().numpy(), ref["resolved"])
+        assert (res.n_iter, res.n_resolved) == (ref["n_iter"], ref["n_resolved"])
