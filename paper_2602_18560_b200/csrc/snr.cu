@@ -310,12 +310,18 @@ struct BuildArgs {
     int n_dblk, dblk_log2;
 };
 
+// CTA_APPEND: one append to the candidate counter per CTA and trip instead of one per warp (batches of 1e8 sources)
+template <bool CTA_APPEND>
 __global__ void __launch_bounds__(256)
 cand_build_kernel(GridDev g, CatTable ct, BuildArgs a)
 {
-    const int lane = threadIdx.x & 31;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    const int64_t n_round = (a.n_all + 31) & ~(int64_t)31;
+    const int64_t n_round = (a.n_all + 255) & ~(int64_t)255;   // the same number of trips for every thread of a CTA
+    // CTA_APPEND: a batch of 3e8 sources would otherwise put 1e7 atomics on one counter
+    __shared__ int s_wcnt[2][8];
+    __shared__ long long s_base[2];
+    int trip = 0;
     bool pref_ok = false;
     int unit_exp = 0;
     if (a.s_instr && a.pv.pref) { pref_ok = a.pv.hdr->bad == 0; unit_exp = a.pv.hdr->unit_exp; }
@@ -338,10 +344,27 @@ cand_build_kernel(GridDev g, CatTable ct, BuildArgs a)
             }
         }
         const unsigned mask = __ballot_sync(0xffffffffu, keep);
+        const int buf = trip & 1;
+        ++trip;
+        if (CTA_APPEND) {
+            if (lane == 0) s_wcnt[buf][warp] = __popc(mask);
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                int tot = 0;
+                for (int w = 0; w < 8; ++w) tot += s_wcnt[buf][w];
+                s_base[buf] = tot ? (long long)atomicAdd((unsigned long long *)a.cand_count, (unsigned long long)tot) : 0ll;
+            }
+            __syncthreads();
+        }
         if (mask) {
             int64_t base = 0;
-            if (lane == 0) base = (int64_t)atomicAdd((unsigned long long *)a.cand_count, (unsigned long long)__popc(mask));
-            base = __shfl_sync(0xffffffffu, base, 0);
+            if (CTA_APPEND) {
+                base = s_base[buf];
+                for (int w = 0; w < warp; ++w) base += s_wcnt[buf][w];
+            } else {
+                if (lane == 0) base = (int64_t)atomicAdd((unsigned long long *)a.cand_count, (unsigned long long)__popc(mask));
+                base = __shfl_sync(0xffffffffu, base, 0);
+            }
             const unsigned same = ct.n_cat > 1 ? __match_any_sync(0xffffffffu, keep ? cat : -1) : 0u;   // kept lanes of my catalog
             if (keep) {
                 const int64_t t = base + __popc(mask & ((1u << lane) - 1u));
@@ -671,7 +694,8 @@ int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, con
     const int64_t cap = (int64_t)sm_count() * 16;
     if (blocks > cap) blocks = cap;
     LaunchTimer lt(K_SNR, st);
-    cand_build_kernel<<<(int)blocks, 256, 0, st>>>(g, ct, a);
+    if (ct.n_cat > 1 || n >= 30000000) cand_build_kernel<true><<<(int)blocks, 256, 0, st>>>(g, ct, a);
+    else cand_build_kernel<false><<<(int)blocks, 256, 0, st>>>(g, ct, a);
     GBFG_LAUNCH_CHECK("cand_build_kernel");
     // order the records by (row, dirty block of the first bin)
     cand_bucket_scan_kernel<<<ct.n_cat, BKT_THREADS, 0, st>>>(sw.bkt_count, sw.bkt_ext, sw.bkt_off, sw.cand_count, n_dblk);
