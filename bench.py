@@ -156,7 +156,7 @@ def algorithmic_bytes(w: wl.Workload, n_bins: int, res, prof) -> dict:
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of running_median_kernel per output it recomputes, from the
-# committed `ncu --set full` capture (profiles/r01_ncu_full_v3.md: 67.1 MB for ~3.4e6 outputs)
+# committed `ncu --set full` captures (profiles/r01_profiles_v6.md: 76.3 MB for a full pass of 3 774 349 outputs)
 MEDIAN_DRAM_BYTES_PER_OUTPUT = 20.0
 # smsp__inst_executed.sum of the same kernel per output it recomputes (profiles/r01_ncu_full_v3.md: 1.14e8 warp
 # instructions for a full pass of 3 774 349 outputs; r01_ncu_full_v5.md: 9.97e7 for ~3.4e6)
