@@ -17,7 +17,7 @@ namespace gbfg {
 constexpr int MED_LT = 8192;                  // positions per tile, halos included
 constexpr int MED_PB = 32;                    // position block = outputs per coarse chunk
 constexpr int MED_FINE = 8;                   // outputs per walking thread
-constexpr int MED_STEP_CAP = 12;              // places a thread steps alone before the warp takes over
+constexpr int MED_STEP_CAP = 20;              // places a thread steps alone before the warp takes over
 constexpr int MED_RB = 128;                   // sorted ranks per bucket
 constexpr int MED_NPB = MED_LT / MED_PB;      // 256
 constexpr int MED_NRB = MED_LT / MED_RB;      // 64
