@@ -46,15 +46,58 @@ def measured_peaks():
 
 # ------------------------------------------------------------------------------------ clocks
 class ClockSampler:
+    """SM clock, power and throttle reasons while the GPU is under the benchmark's load: an NVML polling thread
+    (one sample every 2 ms, so that a 30 ms timed region is seen a dozen times); `nvidia-smi -lms` when the
+    NVML binding is missing."""
     QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
              "clocks_event_reasons.sw_power_cap")
+    PERIOD_S = 0.002
 
-    def __init__(self, index: int):
+    def __init__(self, index: int, uuid=None):
         self.index = index
+        self.uuid = uuid
         self.proc = None
+        self.thread = None
+        self.stop_flag = False
+        self.sm, self.pw, self.reasons, self.mx = [], [], set(), None
+
+    def _nvml_loop(self, nv, h):
+        masks = {"hw_slowdown": nv.nvmlClocksThrottleReasonHwSlowdown,
+                 "hw_thermal_slowdown": nv.nvmlClocksThrottleReasonHwThermalSlowdown,
+                 "sw_thermal_slowdown": nv.nvmlClocksThrottleReasonSwThermalSlowdown,
+                 "sw_power_cap": nv.nvmlClocksThrottleReasonSwPowerCap}
+        while not self.stop_flag:
+            try:
+                self.sm.append(float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                self.pw.append(nv.nvmlDeviceGetPowerUsage(h) / 1000.0)
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                for name, m in masks.items():
+                    if r & m:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.PERIOD_S)
 
     def start(self):
+        try:
+            import threading
+            import pynvml as nv
+            nv.nvmlInit()
+            h = None
+            if self.uuid:
+                try:
+                    h = nv.nvmlDeviceGetHandleByUUID(self.uuid if str(self.uuid).startswith("GPU-") else "GPU-" + str(self.uuid))
+                except Exception:
+                    h = None
+            if h is None:
+                h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.mx = float(nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM))
+            self.thread = threading.Thread(target=self._nvml_loop, args=(nv, h), daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.thread = None
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits",
@@ -62,7 +105,20 @@ class ClockSampler:
         except OSError:
             self.proc = None
 
+    def mark(self):
+        """Forget what was sampled so far (called where the timed region starts)."""
+        if self.thread is not None:
+            self.sm, self.pw = [], []
+
     def stop(self) -> dict:
+        if self.thread is not None:
+            self.stop_flag = True
+            self.thread.join(timeout=2)
+            if not self.sm:
+                return {"sm_mhz": None, "sm_max_mhz": self.mx, "reasons": ["no samples"]}
+            return {"sm_mhz": float(np.median(self.sm)), "sm_min_mhz": float(min(self.sm)), "sm_max_mhz": self.mx,
+                    "power_w_max": float(max(self.pw)), "samples": len(self.sm), "source": "nvml, 2 ms period",
+                    "reasons": sorted(self.reasons)}
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
@@ -87,7 +143,7 @@ class ClockSampler:
         if not sm:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
         return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
-                "samples": len(sm), "reasons": sorted(reasons)}
+                "samples": len(sm), "source": "nvidia-smi -lms 20", "reasons": sorted(reasons)}
 
 
 # ------------------------------------------------------------------------------- reference arm
@@ -201,7 +257,8 @@ def run_gpu(args, w: wl.Workload):
             dist.barrier()
         torch.cuda.synchronize()
 
-    clocks = ClockSampler(local)        # sampled from the warm-up steps on: the GPU is under this load throughout
+    uuid = getattr(torch.cuda.get_device_properties(dev), "uuid", None)
+    clocks = ClockSampler(local, uuid)  # runs from the warm-up on; the samples kept are those of the two timed regions
     clocks.start()
     for _ in range(max(args.warmup, 0)):
         step()
@@ -211,6 +268,7 @@ def run_gpu(args, w: wl.Workload):
     launches0 = gb.kernel_launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
+    clocks.mark()
     e0.record()
     for _ in range(args.steps):
         res = step()
