@@ -322,7 +322,8 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
                      const double *dev_s_instr, const gbfg_iter_params *params,
                      int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
                      uint8_t *dev_resolved, gbfg_iter_result *host_results,
-                     void *workspace, size_t workspace_bytes, void *stream, bool prepared)
+                     void *workspace, size_t workspace_bytes, void *stream, bool prepared,
+                     cudaEvent_t records_ready = nullptr)
 {
     int rc = loop_validate(grid, params);
     if (rc) return rc;
@@ -401,6 +402,9 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
                                grid->scale_log2, &w.plan, nullptr, nullptr, neg_flag, delta, st);
         }
         if (rc) return rc;
+        // gbfg_simulate builds the candidate records on the side stream; the first estimator pass above does not need
+        // them, the prefix below reuses the buffers their pre-selection reads (the prefix of 1/S_instr)
+        if (it == 0 && records_ready) GBFG_CUDA(cudaStreamWaitEvent(st, records_ready, 0));
         rc = launch_inv_prefix(dev_psd, nb, n_cat, w.sw, dirty, st);
         if (rc) return rc;
         // The test subtracts what it selects on the spot (stage v, eq. D4) and stamps the blocks that become dirty.
@@ -562,9 +566,9 @@ extern "C" int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const 
                         w.diff, w.tile_sums, w.wide_flag, plain_marks(w, nb, -1), st);
     if (rc) return rc;
     if (dev_total) GBFG_CUDA(cudaMemcpyAsync(dev_total, dev_spectrum, row_bytes, cudaMemcpyDeviceToDevice, st));
-    GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_aux, 0));
+    // the loop waits for the records (side->ev_aux) after its first estimator pass, which overlaps their build
     return loop_impl(grid, dev_A, dev_f, dev_fdot, offsets, n_cat, dev_s_instr, params, dev_spectrum, dev_median, dev_psd,
-                     dev_resolved, host_results, workspace, workspace_bytes, stream, true);
+                     dev_resolved, host_results, workspace, workspace_bytes, stream, true, side->ev_aux);
 }
 
 extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
