@@ -169,10 +169,10 @@ static cudaEvent_t readback_event()
 }
 
 // side stream on which the plan of the next pass runs next to the scan of the subtraction (one per host thread)
-struct SideStream { cudaStream_t s; cudaEvent_t ev_plan, ev_aux; };
+struct SideStream { cudaStream_t s; cudaEvent_t ev_plan, ev_aux, ev_noise; };
 static SideStream &side_stream_slot()
 {
-    static thread_local SideStream ss = {nullptr, nullptr, nullptr};
+    static thread_local SideStream ss = {nullptr, nullptr, nullptr, nullptr};
     return ss;
 }
 static SideStream *side_stream_if_any() { return side_stream_slot().s ? &side_stream_slot() : nullptr; }
@@ -182,7 +182,8 @@ static SideStream *side_stream()
     if (!ss.s) {
         if (cudaStreamCreateWithFlags(&ss.s, cudaStreamNonBlocking) != cudaSuccess ||
             cudaEventCreateWithFlags(&ss.ev_plan, cudaEventDisableTiming) != cudaSuccess ||
-            cudaEventCreateWithFlags(&ss.ev_aux, cudaEventDisableTiming) != cudaSuccess) {
+            cudaEventCreateWithFlags(&ss.ev_aux, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&ss.ev_noise, cudaEventDisableTiming) != cudaSuccess) {
             (void)cudaGetLastError();
             ss.s = nullptr;
             return nullptr;
@@ -548,6 +549,7 @@ extern "C" int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const 
     GBFG_CUDA(cudaStreamWaitEvent(side->s, side->ev_aux, 0));
     rc = loop_prefix_s_instr(g, dev_s_instr, preselect, w, side->s);
     if (rc) return rc;
+    GBFG_CUDA(cudaEventRecord(side->ev_noise, side->s));    // S_instr is on the device by now (gbfg_simulate_host copies it on this stream)
     rc = gbfg_sample_catalog(grid, pops, offsets, n_cat, 0u, seed, dev_A, dev_f, dev_fdot, stream);
     if (rc) return rc;
     const size_t row_bytes = sizeof(int64_t) * (size_t)n_cat * (size_t)nb;
@@ -566,6 +568,7 @@ extern "C" int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const 
                         w.diff, w.tile_sums, w.wide_flag, plain_marks(w, nb, -1), st);
     if (rc) return rc;
     if (dev_total) GBFG_CUDA(cudaMemcpyAsync(dev_total, dev_spectrum, row_bytes, cudaMemcpyDeviceToDevice, st));
+    GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_noise, 0));  // the first estimator pass reads S_instr
     // the loop waits for the records (side->ev_aux) after its first estimator pass, which overlaps their build
     return loop_impl(grid, dev_A, dev_f, dev_fdot, offsets, n_cat, dev_s_instr, params, dev_spectrum, dev_median, dev_psd,
                      dev_resolved, host_results, workspace, workspace_bytes, stream, true, side->ev_aux);
@@ -640,6 +643,7 @@ extern "C" int gbfg_release_cached(void)
         cudaStreamSynchronize(side->s);
         cudaEventDestroy(side->ev_plan);
         cudaEventDestroy(side->ev_aux);
+        cudaEventDestroy(side->ev_noise);
         cudaStreamDestroy(side->s);
         side->s = nullptr;
     }
