@@ -861,3 +861,26 @@ def test_loop_repeated_runs_are_bit_identical(gb, orc, torch):
         assert np.array_equal(bits(psd.cpu().numpy()), bits(ref["psd"])), rep
         assert np.array_equal(med.cpu().numpy(), ref["median"]), rep
         assert np.array_equal(resolved.cpu().numpy(), ref["resolved"]), rep
+
+
+def test_simulate_host_never_reads_a_stale_s_instr(gb, orc, torch):
+    """gbfg_simulate_host uploads S_instr on the library's side stream while the catalog is sampled; the first
+    estimator pass must wait for it.  The cached device arena still holds the previous call's S_instr (here 4x
+    larger), so a pass that ran early would give another PSD.  A small catalog on the 4-yr grid: sampling and deposit
+    take microseconds, the 30 MB upload half a millisecond (without the wait 7.7e5 bins of the PSD come out wrong)."""
+    w = wl.config(2)
+    w = wl.scaled(w, n_src=20_000, name="cfg2_20k")
+    ref = orc.simulate(w)
+    g = gpu_grid(gb, w)
+    nb, n = g.n_bins, w.n_src_total
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter)
+    h_noise = torch.from_numpy(ref["s_instr"]).pin_memory()
+    h_wrong = (h_noise * 4.0).pin_memory()
+    h_psd = torch.empty(nb, dtype=torch.float64).pin_memory()
+    h_res = torch.empty(n, dtype=torch.uint8).pin_memory()
+    for rep in range(4):
+        gb.simulate_host(g, w.pops, w.offsets(), w.seed, h_wrong.numpy(), params, h_psd.numpy(), h_res.numpy())
+        res = gb.simulate_host(g, w.pops, w.offsets(), w.seed, h_noise.numpy(), params, h_psd.numpy(), h_res.numpy())[0]
+        assert np.array_equal(bits(h_psd.numpy()), bits(ref["psd"])), rep
+        assert np.array_equal(h_res.numpy(), ref["resolved"]), rep
+        assert (res.n_iter, res.n_resolved) == (ref["n_iter"], ref["n_resolved"])
