@@ -154,6 +154,15 @@ struct MedianPlan {
     int max_items;
 };
 
+// What plan_kernel hands to the host before it clears the iteration's counters (loop.cu): n words of src copied to
+// dst (mapped pinned host memory), then seq written at dst[flag_at].
+struct PlanPublish {
+    const int64_t *src;
+    int64_t *dst;
+    int n, flag_at;
+    int64_t seq;
+};
+
 // Workspace of stage (iv) (snr.cu): the 128-bit fixed-point prefix of 1/psd and the candidate records.
 struct SnrWork {
     void *pref;         // [n_cat][n_bins] 16-byte local prefixes

@@ -10,6 +10,7 @@
 #include <string.h>
 
 #include "gbfg_common.cuh"
+#include <atomic>
 
 namespace gbfg {
 
@@ -24,7 +25,7 @@ int launch_scan(int64_t n_bins, int n_cat, int64_t *spectrum, int64_t *diff, int
 int median_max_items(int64_t n_bins);
 int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins, int n_cat, int window,
                 const MedianPlan &pl, int64_t *zero_ptr, int zero_n, int64_t *out_count, unsigned long long *zero2_ptr,
-                cudaStream_t st);
+                cudaStream_t st, const PlanPublish *pub = nullptr);
 int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *med,
                   const double *s_instr, double *psd, double norm, int scale_log2,
                   const MedianPlan *plan, int4 *wide_items, int *wide_ctr, int *neg_flag,
@@ -139,17 +140,41 @@ static int valid_grid(const gbfg_grid *g)
            g->f_min > 0.0 && g->f_max > g->f_min && g->t_obs > 0.0 && g->scale_log2 >= -1000 && g->scale_log2 <= 0;
 }
 
-// pinned host scratch for the per-iteration readback (one per host thread)
+// pinned host scratch for the per-iteration readback (one per host thread), mapped: the plan kernel stores the
+// iteration's counters into it, then a sequence number in its last word
+constexpr int HOST_SEQ_AT = WS_COUNTERS - 1;
 static int64_t *host_scratch()
 {
     static thread_local int64_t *p = nullptr;
     if (!p) {
-        if (cudaHostAlloc((void **)&p, sizeof(int64_t) * WS_COUNTERS, cudaHostAllocDefault) != cudaSuccess) {
+        if (cudaHostAlloc((void **)&p, sizeof(int64_t) * WS_COUNTERS, cudaHostAllocPortable | cudaHostAllocMapped) != cudaSuccess) {
             (void)cudaGetLastError();
             p = nullptr;
+        } else {
+            memset(p, 0, sizeof(int64_t) * WS_COUNTERS);
         }
     }
     return p;
+}
+
+// the host's wait for the counters of one iteration: the sequence number the plan kernel writes behind them.
+// ev_plan (recorded behind that kernel) is looked at now and then, so that a failed launch ends the wait.
+static int wait_published(const int64_t *host, int64_t seq, cudaEvent_t ev_plan)
+{
+    const volatile int64_t *flag = host + HOST_SEQ_AT;
+    for (unsigned spins = 1;; ++spins) {
+        if (*flag == seq) break;
+        if ((spins & 2047u) == 0u) {
+            const cudaError_t e = cudaEventQuery(ev_plan);
+            if (e == cudaSuccess) {
+                if (*flag == seq) break;
+                return set_cuda_error(cudaErrorUnknown, "plan_kernel did not publish the counters");
+            }
+            if (e != cudaErrorNotReady) return set_cuda_error(e, "plan_kernel");
+        }
+    }
+    std::atomic_thread_fence(std::memory_order_acquire);
+    return GBFG_OK;
 }
 
 // device arena and stream of gbfg_simulate_host, one per host thread
@@ -415,27 +440,29 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
         rc = launch_snr_cand(nb, n_cat, dev_psd, params->rho_th, dev_resolved, nullptr, n_cand, w.sel_idx, sel_count,
                              near, 1, preselect ? neg_flag : nullptr, true, w.sw, dirty, snr_tests, &sub, delta, psd_rtol, st);
         if (rc) return rc;
-        GBFG_CUDA(cudaMemcpyAsync(host, w.counters, sizeof(int64_t) * n_read_all, cudaMemcpyDeviceToHost, st));
-        GBFG_CUDA(cudaEventRecord(ev_read, st));
+        GBFG_CUDA(cudaEventRecord(ev_read, st));            // the test is queued; its counters reach the host through the plan below
         // Everything below is queued before the host has seen the counters (a pass that selected nothing makes
         // it a no-op), so the GPU does not idle while the host waits for the scalar that decides whether the
         // loop goes on: the scan of the wide sources' range updates into the spectrum ...
         rc = launch_scan(nb, n_cat, dev_spectrum, w.diff, w.tile_sums, w.wide_flag, mk, st);
         if (rc) return rc;
-        // ... and, on the side stream next to it, the plan of the next pass: it reads the stamps the test wrote
-        // and clears the counters the copy above has taken.  After the last iteration it is the plan of the
-        // closing median pass.
+        // ... and, on the side stream next to it, the plan of the next pass: it stores the test's counters into the
+        // host's mapped scratch (no copy engine between the test and the scan), clears them and reads the stamps
+        // the test wrote.  After the last iteration it is the plan of the closing median pass.
         {
             const bool closing = it + 1 == params->max_iter;
+            static thread_local int64_t seq_counter = 0;
+            const PlanPublish pub = {w.counters, host, (int)n_read_all, HOST_SEQ_AT, ++seq_counter};
             GBFG_CUDA(cudaStreamWaitEvent(side->s, ev_read, 0));
             rc = launch_plan(w.blk_stamp, it + 1, !incremental, nb, n_cat, W, w.plan, closing ? nullptr : w.counters,
                              closing ? 0 : (int)n_iter_counters, med_outputs,
-                             closing ? nullptr : delta_all, side->s);
+                             closing ? nullptr : delta_all, side->s, &pub);
             if (rc) return rc;
             GBFG_CUDA(cudaEventRecord(side->ev_plan, side->s));
             plan_queued = true;
+            rc = wait_published(host, pub.seq, side->ev_plan);
+            if (rc) return rc;
         }
-        GBFG_CUDA(cudaEventSynchronize(ev_read));
         if (preselect && host[i_flags] != 0) {
             if (plan_queued) { GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_plan, 0)); plan_queued = false; }   // it saw no stamps: made again
             // A negative median: S_n >= S_instr no longer holds, so the pre-selection is not valid

@@ -66,6 +66,12 @@ struct PlanArgs {
     int64_t *out_count;     // [n_cat] outputs planned, accumulated (nullable)
     int *wide_ctr;          // [2] counter words of the wide list, cleared here
     unsigned long long *zero2_ptr;   // [n_cat] PSD-change words of the loop, cleared here (nullable)
+    // the iteration's counters, handed to the host before they are cleared (nullable): pub_n words copied to
+    // mapped pinned host memory, then the sequence number written behind them (the host polls it)
+    const int64_t *pub_src;
+    int64_t *pub_dst;
+    int pub_n, pub_flag_at;
+    int64_t pub_seq;
 };
 
 // len < 2^31 (n_bins is): 32-bit divisions, the 64-bit ones are long instruction sequences
@@ -97,8 +103,19 @@ plan_kernel(PlanArgs a)
     int *s_run = s_cum + nb + 1;
     if (tid == 0) { n_runs = 0; row_pieces = 0; }
     if (row == 0 && tid < 2) a.wide_ctr[tid] = 0;
+    if (row == 0 && a.pub_dst) {
+        // what the pass before wrote (this kernel runs behind the SNR test) goes to the host by plain stores over
+        // PCIe: no copy engine on the path, and the counters can be cleared by the same CTA right behind
+        for (int i = tid; i < a.pub_n; i += PLAN_THREADS) a.pub_dst[i] = a.pub_src[i];
+        __threadfence_system();
+        __syncthreads();
+        if (tid == 0) {
+            __threadfence_system();
+            *(volatile int64_t *)(a.pub_dst + a.pub_flag_at) = a.pub_seq;
+        }
+    }
     if (row == 0 && a.zero_ptr) for (int i = tid; i < a.zero_n; i += PLAN_THREADS) a.zero_ptr[i] = 0;
-    if (tid == 0 && a.zero2_ptr) a.zero2_ptr[row] = 0ull;
+    if (row == 0 && a.zero2_ptr) for (int i = tid; i < (int)gridDim.x; i += PLAN_THREADS) a.zero2_ptr[i] = 0ull;
     for (int b0 = tid; b0 < nb; b0 += 8 * PLAN_THREADS) {   // coalesced, eight loads in flight per thread
         int v[8];
 #pragma unroll
@@ -218,9 +235,11 @@ int median_max_items(int64_t n_bins)
 // work list + cum from the stamps (blk_stamp NULL or all_dirty: everything)
 int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins, int n_cat, int window,
                 const MedianPlan &pl, int64_t *zero_ptr, int zero_n, int64_t *out_count, unsigned long long *zero2_ptr,
-                cudaStream_t st)
+                cudaStream_t st, const PlanPublish *pub)
 {
     PlanArgs a;
+    if (pub) { a.pub_src = pub->src; a.pub_dst = pub->dst; a.pub_n = pub->n; a.pub_flag_at = pub->flag_at; a.pub_seq = pub->seq; }
+    else { a.pub_src = nullptr; a.pub_dst = nullptr; a.pub_n = 0; a.pub_flag_at = 0; a.pub_seq = 0; }
     a.zero2_ptr = zero2_ptr;
     a.zero_ptr = zero_ptr; a.zero_n = zero_n; a.out_count = out_count;
     a.blk_stamp = blk_stamp; a.stamp = stamp; a.all_dirty = (all_dirty || !blk_stamp) ? 1 : 0;
