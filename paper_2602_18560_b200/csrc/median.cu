@@ -75,7 +75,9 @@ struct PlanArgs {
 };
 
 // len < 2^31 (n_bins is): 32-bit divisions, the 64-bit ones are long instruction sequences
-static size_t plan_smem_bytes(int n_dblk) { return sizeof(int) * (size_t)((n_dblk + 1) + 3 * (n_dblk / 2 + 1)); }
+// shared memory: [n_dblk + 9] ints for the dirty words and their two prefixes (3 * ceil(n_dblk / 32) used), then the
+// runs, 3 ints each, [n_dblk / 2 + 1]
+static size_t plan_smem_bytes(int n_dblk) { return sizeof(int) * (size_t)((n_dblk + 9) + 3 * (n_dblk / 2 + 1)); }
 
 __device__ __forceinline__ void plan_pieces(int64_t len64, int S, int wave, int *pieces, int *piece_len)
 {
@@ -87,21 +89,26 @@ __device__ __forceinline__ void plan_pieces(int64_t len64, int S, int wave, int 
     *pieces = (int)((len + pl - 1u) / pl);
 }
 
+// The dirty flags of a row are kept as bits, 32 blocks per word (at most 512 words): cum comes from a scan of
+// the words' popcounts, the runs from the words' rising and falling edges (the k-th start belongs to the k-th
+// end), so that a late pass (a few hundred short runs) is a few thousand warp instructions on the one SM it runs on.
 __global__ void __launch_bounds__(PLAN_THREADS)
 plan_kernel(PlanArgs a)
 {
-    extern __shared__ int s_cum[];                      // [n_dblk + 1], then the runs: 3 ints each, [n_dblk / 2 + 1]
+    extern __shared__ int s_mem[];
     __shared__ int wtot[32];
-    __shared__ int n_runs, row_pieces, row_base;
+    __shared__ int row_pieces, row_base, s_total;
+    const unsigned FULL = 0xffffffffu;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int row = blockIdx.x;
-    const int nb = a.n_dblk;
+    const int nb = a.n_dblk, nw = (nb + 31) >> 5;
     const int *st = a.blk_stamp ? a.blk_stamp + (int64_t)row * nb : nullptr;
     int *cum = a.cum + (int64_t)row * (nb + 1);
-    const int per = (nb + PLAN_THREADS - 1) / PLAN_THREADS;
-    const int b_lo = min(tid * per, nb), b_hi = min(b_lo + per, nb);
-    int *s_run = s_cum + nb + 1;
-    if (tid == 0) { n_runs = 0; row_pieces = 0; }
+    unsigned *s_word = reinterpret_cast<unsigned *>(s_mem);   // [nw] dirty flags
+    int *s_wpre = s_mem + nw;                                  // [nw] dirty blocks before the word
+    int *s_rpre = s_mem + 2 * nw;                              // [nw] runs that start before the word
+    int *s_run = s_mem + nb + 9;                               // (first block, end block, first piece) per run
+    if (tid == 0) row_pieces = 0;
     if (row == 0 && tid < 2) a.wide_ctr[tid] = 0;
     if (row == 0 && a.pub_dst) {
         // what the pass before wrote (this kernel runs behind the SNR test) goes to the host by plain stores over
@@ -116,91 +123,98 @@ plan_kernel(PlanArgs a)
     }
     if (row == 0 && a.zero_ptr) for (int i = tid; i < a.zero_n; i += PLAN_THREADS) a.zero_ptr[i] = 0;
     if (row == 0 && a.zero2_ptr) for (int i = tid; i < (int)gridDim.x; i += PLAN_THREADS) a.zero2_ptr[i] = 0ull;
-    for (int b0 = tid; b0 < nb; b0 += 8 * PLAN_THREADS) {   // coalesced, eight loads in flight per thread
+    // stamps -> one bit per block (coalesced, eight loads in flight per thread)
+    for (int base = 0; base < nb; base += 8 * PLAN_THREADS) {
         int v[8];
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-            const int b = b0 + u * PLAN_THREADS;
+            const int b = base + u * PLAN_THREADS + tid;
             v[u] = (!a.all_dirty && b < nb) ? st[b] : a.stamp;
         }
 #pragma unroll
         for (int u = 0; u < 8; ++u) {
-            const int b = b0 + u * PLAN_THREADS;
-            if (b < nb) s_cum[b + 1] = (v[u] == a.stamp) ? 1 : 0;
+            const int b = base + u * PLAN_THREADS + tid;
+            const unsigned wd = __ballot_sync(FULL, b < nb && v[u] == a.stamp);
+            if (lane == 0 && b < nb) s_word[b >> 5] = wd;
         }
     }
     __syncthreads();
-    int cnt = 0;
-    for (int b = b_lo; b < b_hi; ++b) cnt += s_cum[b + 1];
-    int incl = cnt;
-    for (int o = 1; o < 32; o <<= 1) {
-        const int up = __shfl_up_sync(0xffffffffu, incl, o);
-        if (lane >= o) incl += up;
+    // per word: dirty blocks, run starts (a dirty block behind a clean one), run ends; one scan for both counts
+    unsigned w = 0, starts = 0, ends = 0, open_in = 0;
+    if (tid < nw) {
+        w = s_word[tid];
+        const unsigned prev = tid > 0 ? s_word[tid - 1] >> 31 : 0u;
+        const unsigned next = tid + 1 < nw ? s_word[tid + 1] & 1u : 0u;
+        starts = w & ~((w << 1) | prev);
+        ends = w & ~((w >> 1) | (next << 31));
+        open_in = prev & w & 1u;                              // a run crosses into this word
     }
-    if (lane == 31) wtot[warp] = incl;
-    __syncthreads();
-    int run = incl - cnt;
-    for (int w = 0; w < warp; ++w) run += wtot[w];
-    if (tid == 0) s_cum[0] = 0;
-    for (int b = b_lo; b < b_hi; ++b) {                 // s_cum[b + 1] = flag of block b -> inclusive count
-        run += s_cum[b + 1];
-        s_cum[b + 1] = run;
+    const int c = __popc(w);
+    {
+        const int packed = c | (__popc(starts) << 16);        // both totals stay under 2^16 (n_dblk <= 16384)
+        int incl = packed;
+        for (int o = 1; o < 32; o <<= 1) {
+            const int up = __shfl_up_sync(FULL, incl, o);
+            if (lane >= o) incl += up;
+        }
+        if (lane == 31) wtot[warp] = incl;
+        __syncthreads();
+        int excl = incl - packed;
+        for (int k = 0; k < warp; ++k) excl += wtot[k];
+        if (tid < nw) { s_wpre[tid] = excl & 0xffff; s_rpre[tid] = excl >> 16; }
+        if (tid == PLAN_THREADS - 1) s_total = excl + packed;
     }
     __syncthreads();
+    const int n_dirty = s_total & 0xffff, nr = s_total >> 16;
     for (int b = tid; b <= nb; b += PLAN_THREADS) {
-        cum[b] = s_cum[b];
-        if (b < nb && s_cum[b + 1] != s_cum[b]) {          // first / last dirty block of the row
-            if (s_cum[b] == 0) a.range[2 * row] = b;
-            if (s_cum[b + 1] == s_cum[nb]) a.range[2 * row + 1] = b;
-        }
+        const int wi = b >> 5;
+        cum[b] = wi < nw ? s_wpre[wi] + __popc(s_word[wi] & ((1u << (b & 31)) - 1u)) : n_dirty;
     }
-    if (tid == 0 && s_cum[nb] == 0) { a.range[2 * row] = 1; a.range[2 * row + 1] = 0; }
-    __syncthreads();
+    if (w) {                                                 // first / last dirty block of the row
+        const int before = s_wpre[tid];
+        if (before == 0) a.range[2 * row] = tid * 32 + __ffs(w) - 1;
+        if (before + c == n_dirty) a.range[2 * row + 1] = tid * 32 + 31 - __clz(w);
+    }
+    if (tid == 0 && n_dirty == 0) { a.range[2 * row] = 1; a.range[2 * row + 1] = 0; }
+    if (tid < nw) {
+        int k = s_rpre[tid];
+        for (unsigned m = starts; m; m &= m - 1u) s_run[3 * k++] = tid * 32 + __ffs(m) - 1;
+        k = s_rpre[tid] - (int)open_in;                      // runs that ended before this word
+        for (unsigned m = ends; m; m &= m - 1u) s_run[3 * k++ + 1] = tid * 32 + __ffs(m);
+    }
     // Tile size of this row: S outputs at most, less when the dirty part of the row would not fill
     // the row's share of one wave of CTAs (the latency of a short tile is what the tail iterations pay).
     int S = a.S;
     {
-        const unsigned dirty_out = (unsigned)s_cum[nb] << a.dblk_log2;      // <= n_bins + one block
+        const unsigned dirty_out = (unsigned)n_dirty << a.dblk_log2;        // <= n_bins + one block
         int share = a.wave / (int)gridDim.x;
         if (share < 1) share = 1;
         unsigned s_fit = (dirty_out + (unsigned)share - 1u) / (unsigned)share;
         if (s_fit < (unsigned)PLAN_MIN_OUT) s_fit = PLAN_MIN_OUT;
         if (s_fit < (unsigned)S) S = (int)s_fit;
     }
-    // runs: a dirty block whose predecessor is clean starts one; its end by bisection on cum.
-    // Every run is recorded in shared memory with the place of its pieces in the row's part of the
-    // list; then the warps write the items, one run per warp at a time.
-    for (int b = b_lo; b < b_hi; ++b) {
-        const bool dirty = s_cum[b + 1] != s_cum[b];
-        if (!dirty || (b > 0 && s_cum[b] != s_cum[b - 1])) continue;
-        int lo = b + 1, hi = nb;                        // largest e in [b+1, nb] with cum[e] - cum[b] == e - b
-        while (lo < hi) {
-            const int mid = (lo + hi + 1) >> 1;
-            if (s_cum[mid] - s_cum[b] == mid - b) lo = mid; else hi = mid - 1;
-        }
-        const int e = lo;
-        const int64_t first = (int64_t)b << a.dblk_log2;
-        int64_t last = (int64_t)e << a.dblk_log2;
+    __syncthreads();
+    // the place of every run's pieces in the row's part of the list
+    for (int r = tid; r < nr; r += PLAN_THREADS) {
+        const int64_t first = (int64_t)s_run[3 * r] << a.dblk_log2;
+        int64_t last = (int64_t)s_run[3 * r + 1] << a.dblk_log2;
         if (last > a.n_bins) last = a.n_bins;
         int pieces, piece_len;
         plan_pieces(last - first, S, a.wave, &pieces, &piece_len);
-        const int slot = atomicAdd(&n_runs, 1);
-        s_run[3 * slot] = b;
-        s_run[3 * slot + 1] = e;
-        s_run[3 * slot + 2] = atomicAdd(&row_pieces, pieces);
+        s_run[3 * r + 2] = atomicAdd(&row_pieces, pieces);
     }
     __syncthreads();
     if (tid == 0) {
         if (a.out_count) {                               // dirty outputs of the row = dirty blocks, the last one clipped
-            int64_t outs = (int64_t)s_cum[nb] << a.dblk_log2;
-            if (nb > 0 && s_cum[nb] != s_cum[nb - 1]) outs -= ((int64_t)nb << a.dblk_log2) - a.n_bins;
+            int64_t outs = (int64_t)n_dirty << a.dblk_log2;
+            if (nb > 0 && ((s_word[nw - 1] >> ((nb - 1) & 31)) & 1u)) outs -= ((int64_t)nb << a.dblk_log2) - a.n_bins;
             a.out_count[row] += outs;
         }
         if (gridDim.x == 1) { row_base = 0; a.ctr[0] = row_pieces; a.ctr[1] = 0; }
         else row_base = atomicAdd(&a.ctr[0], row_pieces);
     }
     __syncthreads();
-    const int nr = n_runs, rb0 = row_base;
+    const int rb0 = row_base;
     for (int r = warp; r < nr; r += PLAN_THREADS / 32) {
         const int64_t first = (int64_t)s_run[3 * r] << a.dblk_log2;
         int64_t last = (int64_t)s_run[3 * r + 1] << a.dblk_log2;
