@@ -884,3 +884,47 @@ def test_simulate_host_never_reads_a_stale_s_instr(gb, orc, torch):
         assert np.array_equal(bits(h_psd.numpy()), bits(ref["psd"])), rep
         assert np.array_equal(h_res.numpy(), ref["resolved"]), rep
         assert (res.n_iter, res.n_resolved) == (ref["n_iter"], ref["n_resolved"])
+
+
+def test_simulate_from_two_host_threads(gb, orc, torch):
+    """The loop's host-side state is per host thread (side stream, events, the mapped scratch the plan kernel writes the
+    iteration's counters into, the sequence number the host polls): two threads running different catalogs at the same
+    time, each on its own stream and buffers, must both get the oracle's bits, run after run."""
+    import threading
+    w = wl.config(0)
+    g = gpu_grid(gb, w)
+    n, nb = w.n_src_total, g.n_bins
+    seeds = (w.seed, w.seed + 3)
+    refs = [orc.simulate(wl.replace(w, seed=s)) for s in seeds]
+    s_instr = dev(torch, refs[0]["s_instr"])
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter)
+    torch.cuda.synchronize()
+    errors = []
+
+    def run(k):
+        try:
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+                total, spec, med = (torch.empty(nb, dtype=torch.int64, device="cuda") for _ in range(3))
+                psd = torch.empty(nb, dtype=torch.float64, device="cuda")
+                resolved = torch.empty(n, dtype=torch.uint8, device="cuda")
+                ws = workspace(torch, gb, g, n)
+                for rep in range(8):
+                    res = gb.simulate(g, w.pops, w.offsets(), seeds[k], s_instr, params, A, f, fd, total, spec, med, psd,
+                                      resolved, ws, stream=st)[0]
+                    st.synchronize()
+                    ref = refs[k]
+                    assert (res.n_iter, res.n_resolved) == (ref["n_iter"], ref["n_resolved"]), (k, rep)
+                    assert np.array_equal(bits(psd.cpu().numpy()), bits(ref["psd"])), (k, rep)
+                    assert np.array_equal(spec.cpu().numpy(), ref["residual"]), (k, rep)
+                    assert np.array_equal(resolved.cpu().numpy(), ref["resolved"]), (k, rep)
+        except BaseException as e:          # noqa: BLE001 — reported by the main thread
+            errors.append((k, repr(e)))
+
+    threads = [threading.Thread(target=run, args=(k,)) for k in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
