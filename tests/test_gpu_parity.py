@@ -928,3 +928,41 @@ def test_simulate_from_two_host_threads(gb, orc, torch):
     for t in threads:
         t.join()
     assert not errors, errors
+
+
+@pytest.mark.parametrize("pattern", ["alternating", "random", "word_edges", "pairs"])
+def test_loop_dirty_block_patterns(gb, orc, torch, pattern):
+    """plan_kernel keeps a row's dirty blocks as bits (32 per word) and finds the runs from the words' edges.  A window
+    of 3 bins and one loud narrow source in the middle of chosen 256-bin blocks make the second pass's dirty set exactly
+    those blocks: every other block (the largest possible number of runs), a random half, blocks around the word
+    boundaries with the first and the (partial, 1221 = 38 * 32 + 5) last block, and pairs that straddle words.  The
+    background is a spectrum the catalog is not part of, so a block the plan missed keeps a stale median."""
+    w = wl.replace(wl.config(0), window=3, max_iter=5)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    nb = og.n_bins
+    n_blk = (nb + 255) // 256
+    assert n_blk % 32 != 0
+    rng = np.random.default_rng(11)
+    if pattern == "alternating":
+        blocks = np.arange(0, n_blk, 2)
+    elif pattern == "random":
+        blocks = np.flatnonzero(rng.random(n_blk) < 0.5)
+    elif pattern == "word_edges":
+        edges = np.arange(32, n_blk, 32)
+        blocks = np.unique(np.concatenate([[0, n_blk - 1], edges - 1, edges[::2], edges[1::3] + 1]))
+    else:
+        starts = np.arange(31, n_blk - 1, 7)
+        blocks = np.unique(np.concatenate([starts, starts + 1]))
+    last_len = nb - (n_blk - 1) * 256
+    off = np.where(blocks == n_blk - 1, min(128, last_len - 2), 128)          # away from the block's ends: h = 1
+    k = blocks * 256 + off
+    f = w.f_min + (k + 0.5) / w.t_obs
+    A = np.full(k.size, 1e-20) * (1.0 + 0.5 * rng.random(k.size))
+    fd = np.zeros(k.size)
+    spec0 = wl.random_spectrum(nb, seed=5, kind="lognormal")
+    assert orc.deposit(og, A, f, fd, spec0) == 0
+    ref, res = _loop_on_given_spectrum(gb, orc, torch, w, A, f, fd, spec0)
+    assert ref["n_resolved"] >= 0.95 * k.size and ref["n_iter"] == 2     # (a few at 0.1 mHz stay under the threshold)
+    hit = blocks[ref["resolved"] == 1]
+    assert res.n_median_outputs == nb + sum(min(256, nb - b * 256) for b in hit)      # second pass: exactly those blocks
+    _loop_on_given_spectrum(gb, orc, torch, w, A, f, fd, spec0, flags=gb.FLAG_NO_INCREMENTAL)
