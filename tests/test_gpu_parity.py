@@ -998,3 +998,56 @@ def test_loop_random_sweep(gb, orc, torch):
                 _loop_case(gb, orc, torch, w, flags=flags, check_host=bool(rng.integers(2)))
         except AssertionError as e:
             raise AssertionError(f"case {i}: {w} flags={flags}") from e
+
+
+def _batch_case(gb, orc, torch, w, estimator=0, flags=0):
+    """One batched launch sequence over w's catalogs against the oracle run catalog by catalog."""
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    n, nb, nc = w.n_src_total, g.n_bins, w.n_cat
+    A, f, fd = (torch.empty(max(n, 1), dtype=torch.float64, device="cuda") for _ in range(3))
+    total, spec, stat = (torch.empty((nc, nb), dtype=torch.int64, device="cuda") for _ in range(3))
+    psd = torch.empty((nc, nb), dtype=torch.float64, device="cuda")
+    resolved = torch.empty(max(n, 1), dtype=torch.uint8, device="cuda")
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter,
+                                 flags | (gb.FLAG_ESTIMATOR_MEAN if estimator else 0))
+    res = gb.simulate(g, w.pops, w.offsets(), w.seed, dev(torch, orc.instrument_noise(og)), params, A, f, fd, total,
+                      spec, stat, psd, resolved, workspace(torch, gb, g, n, nc))
+    off = w.offsets()
+    for c in range(nc):
+        ref = orc.simulate(w, cat=c, estimator=estimator)
+        s = slice(int(off[c]), int(off[c + 1]))
+        assert np.array_equal(total[c].cpu().numpy(), ref["total"]), c
+        assert np.array_equal(spec[c].cpu().numpy(), ref["residual"]), c
+        assert np.array_equal(stat[c].cpu().numpy(), ref["median"]), c
+        assert np.array_equal(bits(psd[c].cpu().numpy()), bits(ref["psd"])), c
+        assert np.array_equal(resolved[s].cpu().numpy(), ref["resolved"]), c
+        assert (res[c].n_iter, res[c].converged, res[c].n_resolved) == (ref["n_iter"], ref["converged"], ref["n_resolved"]), c
+        assert res[c].n_near_threshold == ref["n_near_threshold"], c
+
+
+def test_loop_batch_random_sweep(gb, orc, torch):
+    """Seeded sweep of ragged batches in the manner of configs[4]: 2-6 catalogs per launch sequence, each with its own
+    Lambda from the prior box and its own size (empty catalogs and single sources included), both estimators, the flags.
+    GBFG_SWEEP_SECONDS extends it as in test_loop_random_sweep."""
+    import os
+    import time
+    rng = np.random.default_rng(4242)
+    budget = float(os.environ.get("GBFG_SWEEP_SECONDS", "0"))
+    t0, i = time.time(), 0
+    while i < 12 or time.time() - t0 < budget:
+        i += 1
+        nc = int(rng.integers(2, 7))
+        pops = [wl.Population(slope=float(rng.uniform(1.0, 2.0)), logA_offset=float(rng.uniform(-23.0, -22.0)),
+                              logA_sigma=float(rng.uniform(0.2, 0.6)), logMc_mean=float(rng.uniform(-0.8, -0.2)),
+                              n_src=int(rng.choice([0, 1, 4_099, 30_000, 120_001])))
+                for _ in range(nc)]
+        w = wl.Workload(name=f"batch_sweep{i}", t_obs=float(rng.choice([0.5, 1.0])) * wl.YEAR_S, f_min=1e-4,
+                        f_max=float(rng.choice([2e-3, 3e-3, 1e-2])), window=int(rng.choice([501, 1001, 2001])),
+                        rho_th=float(rng.choice([5.0, 7.0])), max_iter=int(rng.choice([4, 30])),
+                        seed=int(rng.integers(1 << 31)), pops=pops)
+        estimator, flags = int(rng.integers(2)), int(rng.choice([0, 0, 1, 2, 3]))
+        try:
+            _batch_case(gb, orc, torch, w, estimator=estimator, flags=flags)
+        except AssertionError as e:
+            raise AssertionError(f"case {i}: {w} estimator={estimator} flags={flags}") from e
