@@ -1051,3 +1051,30 @@ def test_loop_batch_random_sweep(gb, orc, torch):
             _batch_case(gb, orc, torch, w, estimator=estimator, flags=flags)
         except AssertionError as e:
             raise AssertionError(f"case {i}: {w} estimator={estimator} flags={flags}") from e
+
+
+def test_sample_catalog_paper_prior_sweep(gb, orc, torch):
+    """48 draws of Lambda from the priors of Table I in one batched call, each catalog bit-exact:
+    the inverse Gamma CDF, Phi and its inverse and the copula (App. A) over the whole prior box.
+    GBFG_SWEEP_SECONDS repeats it with further draws."""
+    import os
+    import time
+    w = wl.config(1)
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    budget = float(os.environ.get("GBFG_SWEEP_SECONDS", "0"))
+    t0, rnd = time.time(), 0
+    while rnd < 1 or time.time() - t0 < budget:
+        pops = [wl.paper_prior_draw(1000 + 48 * rnd + s, n_src=10_007 + 64 * (s % 5)) for s in range(48)]
+        off = np.concatenate([[0], np.cumsum([p.n_src for p in pops])]).astype(np.int64)
+        n = int(off[-1])
+        A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+        gb.sample_catalog_paper(g, pops, off, 77 + rnd, A, f, fd, first_cat_id=0)
+        hA, hf, hfd = A.cpu().numpy(), f.cpu().numpy(), fd.cpu().numpy()
+        for c, p in enumerate(pops):
+            rA, rf, rfd = orc.sample_catalog_paper(og, p, c, 77 + rnd)
+            s = slice(int(off[c]), int(off[c + 1]))
+            assert np.array_equal(bits(hA[s]), bits(rA)), (rnd, c, p)
+            assert np.array_equal(bits(hf[s]), bits(rf)), (rnd, c, p)
+            assert np.array_equal(bits(hfd[s]), bits(rfd)), (rnd, c, p)
+        rnd += 1
