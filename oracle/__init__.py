@@ -103,6 +103,7 @@ def lib():
         L.orc_subtract_until_converged_tol.argtypes = [
             C.POINTER(Grid), dp, dp, dp, C.c_int64, dp, C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_int32, C.c_double,
             ip, ip, dp, up, C.POINTER(IterResult), ip]
+        L.orc_stage_seconds.argtypes = [C.POINTER(C.c_double), C.c_int]
         L.orc_running_sum_def.argtypes = [ip, C.c_int64, C.c_int32, C.c_int64, C.c_int64, ip]
         L.orc_running_sum.argtypes = [ip, C.c_int64, C.c_int32, ip]
         L.orc_psd_mean.argtypes = [ip, dp, C.c_int64, C.c_int32, C.c_int32, dp]
@@ -354,20 +355,37 @@ def subtract_until_converged(grid: Grid, A, f, fdot, s_instr, window: int, media
                 n_new_per_iter=trace[:max_iter])
 
 
-def simulate(w, cat: int = 0, n_src: int | None = None, estimator: int = 0, psd_rtol: float = 0.0):
-    """Whole path for catalog `cat` of a gbfg_workloads.Workload: sample -> deposit -> loop."""
+def stage_seconds(reset: bool = True):
+    """Seconds the calling thread's loop calls spent in (estimator passes, SNR passes, subtractions) since the last reset."""
+    out = (C.c_double * 3)()
+    lib().orc_stage_seconds(out, 1 if reset else 0)
+    return tuple(out)
+
+
+def simulate(w, cat: int = 0, n_src: int | None = None, estimator: int = 0, psd_rtol: float = 0.0, cat_id: int | None = None):
+    """Whole path for catalog `cat` of a gbfg_workloads.Workload: sample -> deposit -> loop.  `stage_s` of the result:
+    wall-clock seconds per stage (measurement only).  cat_id: Philox catalog id (default: cat)."""
+    import time
     grid = make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
     pop = make_pop(w.pops[cat])
     if n_src is not None:
         pop.n_src = n_src
-    A, f, fd = sample_catalog(grid, pop, cat, w.seed)
+    t0 = time.perf_counter()
+    A, f, fd = sample_catalog(grid, pop, cat if cat_id is None else cat_id, w.seed)
+    t1 = time.perf_counter()
     s_instr = instrument_noise(grid)
+    t2 = time.perf_counter()
     spec = np.zeros(grid.n_bins, dtype=np.int64)
     rejected = deposit(grid, A, f, fd, spec)
+    t3 = time.perf_counter()
     total = spec.copy()
+    stage_seconds(reset=True)
     out = subtract_until_converged(grid, A, f, fd, s_instr, w.window, w.median_norm, w.rho_th, w.max_iter, spec,
                                    estimator=estimator, psd_rtol=psd_rtol)
-    out.update(A=A, f=f, fdot=fd, s_instr=s_instr, total=total, residual=spec, rejected=rejected, grid=grid)
+    est_s, snr_s, sub_s = stage_seconds(reset=True)
+    out.update(A=A, f=f, fdot=fd, s_instr=s_instr, total=total, residual=spec, rejected=rejected, grid=grid,
+               stage_s={"sample": t1 - t0, "noise": t2 - t1, "deposit": t3 - t2, "estimator_passes": est_s,
+                        "snr_passes": snr_s, "subtract": sub_s})
     return out
 
 

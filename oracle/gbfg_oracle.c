@@ -35,10 +35,12 @@
  * and the catalog distribution against the paper's population (different data model,
  * DESIGN.md §3 R0).
  */
+#define _POSIX_C_SOURCE 199309L
 #include <math.h>
 #include <stdint.h>
 #include <stdlib.h>
 #include <string.h>
+#include <time.h>
 
 /* ------------------------------------------------------------------------------------ */
 /* Stage (i) — Philox4x32-10 (Salmon et al. 2011), R1                          */
@@ -297,6 +299,25 @@ void orc_sample_catalog(const orc_grid *g, const orc_pop *pop, uint32_t cat_id, 
 /* ------------------------------------------------------------------------------------ */
 static double orc_expn(double y) { return orc_exp10(y * ORC_LOG10_E); }   /* e^y */
 
+/* Lengths of the fixed recurrences below (R12 derives them and states the domain they cover:
+ * 0.25 <= alpha_Gamma <= 16, |z| <= 8.6).  Macros only so that tests/test_oracle_paper_sampler.py can build this
+ * file "one notch shorter" and show that the pins catch it; the product of this file uses the defaults. */
+#ifndef ORC_ERFC_SERIES_TERMS
+#define ORC_ERFC_SERIES_TERMS 80
+#endif
+#ifndef ORC_ERFC_CF_DEPTH
+#define ORC_ERFC_CF_DEPTH 40
+#endif
+#ifndef ORC_GAMMA_SERIES_TERMS
+#define ORC_GAMMA_SERIES_TERMS 48
+#endif
+#ifndef ORC_GAMMA_CF_DEPTH
+#define ORC_GAMMA_CF_DEPTH 40
+#endif
+#ifndef ORC_QUANTILE_NEWTON_STEPS
+#define ORC_QUANTILE_NEWTON_STEPS 10
+#endif
+
 /* erfc(t), t >= 0: for t < 2 the all-positive series erf t = (2/sqrt pi) e^{-t^2} sum 2^n t^{2n+1} / (2n+1)!!
  * (80 terms), else the continued fraction e^{-t^2} / (sqrt pi (t + (1/2)/(t + 1/(t + (3/2)/(t + ...))))), depth 40,
  * evaluated from the bottom */
@@ -306,14 +327,14 @@ double orc_erfc_pos(double t)
     double t2 = t * t;
     if (t < 2.0) {
         double term = t, sum = t;
-        for (int n = 1; n < 80; ++n) {
+        for (int n = 1; n < ORC_ERFC_SERIES_TERMS; ++n) {
             term = term * (2.0 * t2) / (double)(2 * n + 1);
             sum = sum + term;
         }
         return 1.0 - (2.0 / SQRT_PI) * orc_expn(-t2) * sum;
     }
     double r = t;
-    for (int k = 40; k >= 1; --k) r = t + (0.5 * (double)k) / r;
+    for (int k = ORC_ERFC_CF_DEPTH; k >= 1; --k) r = t + (0.5 * (double)k) / r;
     return orc_expn(-t2) / (SQRT_PI * r);
 }
 
@@ -331,15 +352,15 @@ void orc_gamma_pq(double a, double x, double lg, double *P, double *Q, double *p
     double pref = orc_expn((a * orc_log(x) - x) - lg);
     if (x < a + 3.0) {
         double term = 1.0 / a, sum = term;
-        for (int n = 1; n <= 48; ++n) {
+        for (int n = 1; n <= ORC_GAMMA_SERIES_TERMS; ++n) {
             term = term * x / (a + (double)n);
             sum = sum + term;
         }
         *P = sum * pref;
         *Q = 1.0 - *P;
     } else {
-        double r = (x + 81.0) - a;
-        for (int k = 40; k >= 1; --k) r = ((x + (double)(2 * k - 1)) - a) - ((double)k * ((double)k - a)) / r;
+        double r = (x + (double)(2 * ORC_GAMMA_CF_DEPTH + 1)) - a;        /* depth 40: x + 81 - a */
+        for (int k = ORC_GAMMA_CF_DEPTH; k >= 1; --k) r = ((x + (double)(2 * k - 1)) - a) - ((double)k * ((double)k - a)) / r;
         *Q = pref / r;
         *P = 1.0 - *Q;
     }
@@ -356,7 +377,7 @@ double orc_gamma_quantile(double a, double lg, double lg1, double z)
     double w = (1.0 - c) + z * sqrt(c);
     double x = a * ((w * w) * w);
     if (!(w > 0.0) || x < 1e-6 * a) x = orc_expn((orc_log(tail) + lg1) / a);   /* far lower tail: P ~ x^a / Gamma(a+1) */
-    for (int it = 0; it < 10; ++it) {
+    for (int it = 0; it < ORC_QUANTILE_NEWTON_STEPS; ++it) {
         double P, Q, pref;
         orc_gamma_pq(a, x, lg, &P, &Q, &pref);
         double pdf = pref / x;
@@ -770,6 +791,21 @@ typedef struct {
     int64_t n_near_threshold;
 } orc_iter_result;
 
+/* Stopwatch around the three stage calls of the loop below (bench.py's cpu_baseline reports where the oracle's
+ * time goes).  Measurement only: nothing here feeds back into a result.
+ * [0] estimator passes (median or mean, + PSD), [1] SNR passes, [2] subtractions; seconds, accumulated per thread. */
+static __thread double orc_stage_s[3];
+static double orc_now(void)
+{
+    struct timespec ts;
+    clock_gettime(CLOCK_MONOTONIC, &ts);
+    return (double)ts.tv_sec + 1e-9 * (double)ts.tv_nsec;
+}
+void orc_stage_seconds(double out[3], int reset)
+{
+    for (int i = 0; i < 3; ++i) { out[i] = orc_stage_s[i]; if (reset) orc_stage_s[i] = 0.0; }
+}
+
 /* spectrum: in = total deposited spectrum, out = residual.  resolved: in/out flags.
  * n_new_per_iter (nullable, length max_iter) receives the newly-resolved count of each
  * iteration.  median / psd always correspond to the returned residual. */
@@ -805,7 +841,9 @@ int orc_subtract_until_converged_tol(const orc_grid *g, const double *A, const d
     int rc = 0;
     int32_t it;
     for (it = 0; it < max_iter; ++it) {
+        double t0 = orc_now();
         rc = orc_estimate(estimator, spectrum, s_instr, g->n_bins, window, median_norm, g->scale_log2, median, psd);
+        orc_stage_s[0] += orc_now() - t0;
         if (rc) break;
         if (psd_rtol > 0.0 && it > 0) {
             double delta = 0.0;
@@ -821,16 +859,22 @@ int orc_subtract_until_converged_tol(const orc_grid *g, const double *A, const d
         }
         if (psd_rtol > 0.0) memcpy(prev, psd, sizeof(double) * (size_t)g->n_bins);
         int64_t near = 0;
+        t0 = orc_now();
         int64_t n_new = orc_snr_select(g, A, f, fdot, n, psd, rho_th, resolved, NULL, sel, &near);
+        orc_stage_s[1] += orc_now() - t0;
         res->n_near_threshold += near;
         if (n_new_per_iter) n_new_per_iter[it] = n_new;
         if (n_new == 0) { res->n_iter = it + 1; res->converged = 1; break; }
+        t0 = orc_now();
         orc_deposit(g, A, f, fdot, n, sel, n_new, -1, spectrum);
+        orc_stage_s[2] += orc_now() - t0;
         res->n_resolved += n_new;
     }
     if (rc == 0 && !res->converged) {          /* cap hit: PSD must match the returned residual */
         res->n_iter = max_iter;
+        double t0 = orc_now();
         rc = orc_estimate(estimator, spectrum, s_instr, g->n_bins, window, median_norm, g->scale_log2, median, psd);
+        orc_stage_s[0] += orc_now() - t0;
     }
     free(sel);
     free(prev);

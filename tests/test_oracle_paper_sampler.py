@@ -104,3 +104,83 @@ def test_counter_layout_and_pieces(orc):
     B = orc.sample_catalog_paper(g, pop, 3, 11)[1]
     assert not np.array_equal(f, B)                                        # another catalog id, another stream
     assert np.all((f >= w.f_min) & (f < w.f_max)) and np.all(fd > 0) and np.all(A > 0)
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# DESIGN.md R12: the lengths of the fixed recurrences (erfc: 80 terms / depth 40; P, Q: 48 terms / depth 40; quantile:
+# 10 Newton steps) and the domain they are stated for (0.25 <= alpha_Gamma <= 16, |z| <= 8.6: every z a binary64
+# uniform in [2^-53, 1 - 2^-53] can give through Box-Muller).  The pins below sit on the corners of that domain, on both
+# sides of the series / continued-fraction switches, and the SAME oracle source built one notch shorter fails them.
+# ---------------------------------------------------------------------------------------------------------------
+A_DOMAIN = [0.25, 1.0, 3.0, 8.0, 16.0]
+Z_DOMAIN = [-8.6, -8.0, -5.0, -2.0, -0.3, 0.0, 0.3, 2.0, 5.0, 8.0, 8.6]
+
+
+def _pins_of_the_recurrences(L):
+    """Worst relative errors against mpmath of erfc, (P, Q) and the quantile, through the C functions of library L."""
+    import ctypes as C
+    import math
+    mp.mp.dps = 40
+    L.orc_erfc_pos.restype = C.c_double
+    L.orc_erfc_pos.argtypes = [C.c_double]
+    L.orc_gamma_pq.argtypes = [C.c_double] * 3 + [C.POINTER(C.c_double)] * 3
+    L.orc_gamma_quantile.restype = C.c_double
+    L.orc_gamma_quantile.argtypes = [C.c_double] * 4
+    w_erfc = 0
+    for t in [0.0, 0.5, 1.0, 1.5, np.nextafter(2.0, 0.0), 2.0, 2.05, 2.5, 4.0, 8.6 / np.sqrt(2.0)]:
+        w_erfc = max(w_erfc, abs(mp.mpf(L.orc_erfc_pos(float(t))) / mp.erfc(mp.mpf(float(t))) - 1))
+    w_pq = 0
+    for a in A_DOMAIN:
+        sw = a + 3.0
+        for x in [1e-9, 0.1 * a, a, np.nextafter(sw, 0.0), sw, sw + 0.5, 2 * sw, sw + 40.0, sw + 80.0]:
+            P, Q, pref = C.c_double(), C.c_double(), C.c_double()
+            L.orc_gamma_pq(a, float(x), math.lgamma(a), C.byref(P), C.byref(Q), C.byref(pref))
+            if x < sw:
+                w_pq = max(w_pq, abs(mp.mpf(P.value) / mp.gammainc(a, 0, float(x), regularized=True) - 1))
+            else:
+                w_pq = max(w_pq, abs(mp.mpf(Q.value) / mp.gammainc(a, float(x), mp.inf, regularized=True) - 1))
+    w_q = 0
+    for a in A_DOMAIN:
+        # the Wilson-Hilferty start hands over to the far-tail start where w = (1 - c) + z sqrt(c) reaches 0, c = 1 / (9 a):
+        # both starts are at their worst next to that point, which is where the number of Newton steps is decided
+        c = 1.0 / (9.0 * a)
+        z_sw = -(1.0 - c) / np.sqrt(c)
+        for z in Z_DOMAIN + [float(z_sw + d) for d in (-0.2, -0.05, 0.0, 0.05, 0.2, 0.5) if abs(z_sw + d) <= 8.6]:
+            x = L.orc_gamma_quantile(a, math.lgamma(a), math.lgamma(a + 1.0), z)
+            tail = mp.ncdf(-abs(mp.mpf(z)))
+            back = mp.gammainc(a, 0, x, regularized=True) if z <= 0 else mp.gammainc(a, x, mp.inf, regularized=True)
+            w_q = max(w_q, abs(back / tail - 1))
+    return float(w_erfc), float(w_pq), float(w_q)
+
+
+def _build_variant(tmp_path, name, **macros):
+    import ctypes as C
+    import os
+    import subprocess
+    import oracle
+    so = os.path.join(tmp_path, f"liboracle_{name}.so")
+    defs = [f"-D{k}={v}" for k, v in macros.items()]
+    subprocess.check_call(["gcc", *oracle.GCC_FLAGS, *defs, "-o", so, oracle._SRC, "-lm"])
+    return C.CDLL(so)
+
+
+def test_recurrence_lengths_cover_the_stated_domain_and_a_notch_shorter_fails(orc, tmp_path):
+    TOL_ERFC, TOL_PQ, TOL_Q = 3e-13, 3e-13, 1e-12
+    e, pq, q = _pins_of_the_recurrences(_build_variant(tmp_path, "default"))
+    assert e < TOL_ERFC and pq < TOL_PQ and q < TOL_Q, (e, pq, q)
+    # one notch shorter, one recurrence at a time: the pin of that recurrence fails, so a cut that is too deep is seen
+    e, _, _ = _pins_of_the_recurrences(_build_variant(tmp_path, "erfc_cf32", ORC_ERFC_CF_DEPTH=32))
+    assert e > TOL_ERFC, e
+    e, _, _ = _pins_of_the_recurrences(_build_variant(tmp_path, "erfc_s20", ORC_ERFC_SERIES_TERMS=20))
+    assert e > TOL_ERFC, e
+    _, pq, _ = _pins_of_the_recurrences(_build_variant(tmp_path, "gamma_cf16", ORC_GAMMA_CF_DEPTH=16))
+    assert pq > TOL_PQ, pq
+    _, pq, _ = _pins_of_the_recurrences(_build_variant(tmp_path, "gamma_s24", ORC_GAMMA_SERIES_TERMS=24))
+    assert pq > TOL_PQ, pq
+    _, _, q = _pins_of_the_recurrences(_build_variant(tmp_path, "newton8", ORC_QUANTILE_NEWTON_STEPS=8))
+    assert q > TOL_Q, q
+    # and the lengths the oracle had before commit 60b0425 (100 terms, depth 120, 14 steps) change nothing the pins see:
+    # the shorter recurrences lose no accuracy on the domain
+    e2, pq2, q2 = _pins_of_the_recurrences(_build_variant(tmp_path, "long", ORC_GAMMA_SERIES_TERMS=100, ORC_GAMMA_CF_DEPTH=120,
+                                                          ORC_QUANTILE_NEWTON_STEPS=14, ORC_ERFC_CF_DEPTH=120))
+    assert pq2 < TOL_PQ and q2 < TOL_Q and e2 < TOL_ERFC
