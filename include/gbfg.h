@@ -17,8 +17,12 @@
  *  - The spectrum is int64 fixed point: one unit = 2^scale_log2 strain^2 (configs: -140).
  *  - Every function returns GBFG_OK (0) or a negative gbfg_status.  Nothing throws, aborts or
  *    prints.  The four stage calls and the helpers are asynchronous on `stream`;
- *    gbfg_subtract_until_converged and gbfg_simulate* synchronise `stream` (one 8-byte scalar per
- *    iteration) and fill HOST results.
+ *    gbfg_subtract_until_converged and gbfg_simulate* wait, once per iteration, for that iteration's block of
+ *    counters (selected and near-threshold sources per catalog, flags: a few dozen int64 the device stores into
+ *    mapped pinned host memory, R9), synchronise `stream` before they return and fill HOST results.
+ *  - What the library keeps between calls is per host thread and belongs to the device that was current when it
+ *    was made (a side stream, a few events, gbfg_simulate_host's device arena); a thread that calls again with
+ *    another current device gets fresh ones.  An error return leaves no work of the call in flight.
  *  - The library runs on compute capability 10.x devices only (GBFG_ERR_ARCH otherwise).  There is
  *    no CPU fallback and no other backend.
  */
@@ -38,12 +42,14 @@ typedef enum gbfg_status {
     GBFG_ERR_WORKSPACE = -2,   /* workspace NULL or smaller than gbfg_workspace_bytes() */
     GBFG_ERR_CUDA = -3,        /* a CUDA runtime call failed: see gbfg_last_cuda_error() */
     GBFG_ERR_ARCH = -4,        /* current device is not compute capability 10.x */
-    GBFG_ERR_UNSUPPORTED = -5  /* window wider than GBFG_MAX_WINDOW, or n_cat > GBFG_MAX_CAT */
+    GBFG_ERR_UNSUPPORTED = -5  /* window wider than GBFG_MAX_WINDOW, n_cat > GBFG_MAX_CAT, alpha_gamma outside its stated range */
 } gbfg_status;
 
 #define GBFG_MAX_CAT 256        /* catalogs per batched call */
 #define GBFG_MAX_WINDOW 4097    /* widest running-median window of this build (odd) */
 #define GBFG_MAX_ITER_TRACE 64  /* per-iteration counts kept in gbfg_iter_result */
+#define GBFG_PAPER_ALPHA_MIN 0.25   /* range of gbfg_pop_paper.alpha_gamma the special functions of DESIGN.md R12 are */
+#define GBFG_PAPER_ALPHA_MAX 16.0   /* stated and pinned for (Table I, draws it from [1, 3]) */
 
 /* Frequency grid: bins of width 1/t_obs covering [f_min, f_max); bin k = [f_min + k/T, f_min + (k+1)/T).
  * n_bins = ceil((f_max - f_min) * t_obs)  (R2).  Fill with gbfg_grid_init. */
@@ -139,7 +145,8 @@ int gbfg_sample_catalog(const gbfg_grid *grid, const gbfg_pop *pops, const int64
 
 /* Stage (i) with the paper's own population model (Table I, eqs. 7-9, Gaussian copula of Appendix A steps iii-iv,
  * PAPER.md:454-457; R12).  Same conventions as gbfg_sample_catalog (Philox counter blocks 2 and 3, so the two
- * samplers never share a random number); alpha_gamma, beta_gamma > 0, sigma >= 0, 0 <= rho < 1 (INVALID_ARG otherwise). */
+ * samplers never share a random number); alpha_gamma, beta_gamma > 0, sigma >= 0, 0 <= rho < 1 (INVALID_ARG otherwise);
+ * alpha_gamma outside [GBFG_PAPER_ALPHA_MIN, GBFG_PAPER_ALPHA_MAX]: GBFG_ERR_UNSUPPORTED. */
 int gbfg_sample_catalog_paper(const gbfg_grid *grid, const gbfg_pop_paper *pops, const int64_t *offsets,
                               int32_t n_cat, uint32_t first_cat_id, uint64_t seed,
                               double *dev_A, double *dev_f, double *dev_fdot, void *stream);
@@ -207,8 +214,8 @@ int gbfg_snr_select(const gbfg_grid *grid, const double *dev_A, const double *de
                     int64_t *dev_sel_idx, int64_t *dev_sel_count, int64_t *dev_near_count,
                     void *workspace, size_t workspace_bytes, void *stream);
 
-/* Stage (v) — the loop, steps 4-10 (R6), device resident with one
- * 8-byte scalar read back per iteration.  Catalogs of a batch iterate independently; a catalog
+/* Stage (v) — the loop, steps 4-10 (R6), device resident; the host reads one small
+ * block of counters per iteration (see Conventions).  Catalogs of a batch iterate independently; a catalog
  * that resolved nothing is frozen.
  *  dev_spectrum: [n_cat][n_bins] in: total deposited spectrum, out: residual.
  *  dev_median, dev_psd: [n_cat][n_bins] out, always those of the returned residual.
@@ -223,9 +230,12 @@ int gbfg_subtract_until_converged(const gbfg_grid *grid, const double *dev_A, co
 
 /* The whole hot path on device buffers: sample (i) -> deposit (ii) -> loop (iii)-(v).
  * Outputs as above plus the catalog itself and the total spectrum (dev_total may be NULL).
- * dev_err_count: one int64 or NULL. */
+ * dev_err_count: one int64 or NULL.
+ * cat_ids: HOST [n_cat] or NULL.  Philox counter word 3 of catalog c (R1) is cat_ids[c], or c when NULL:
+ * a rank that runs a share {c_0, c_1, ...} of a batch (any subset, any order) passes those ids and
+ * gets, row by row, the bits the whole batch gives for those catalogs. */
 int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
-                  uint64_t seed, const double *dev_s_instr, const gbfg_iter_params *params,
+                  uint64_t seed, const uint32_t *cat_ids, const double *dev_s_instr, const gbfg_iter_params *params,
                   double *dev_A, double *dev_f, double *dev_fdot,
                   int64_t *dev_total, int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
                   uint8_t *dev_resolved, int64_t *dev_err_count, gbfg_iter_result *host_results,
@@ -236,7 +246,7 @@ int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *of
  * resolved flags ([N] uint8, may be NULL) back.  Host pointers should be pinned for full speed.
  * Synchronous.  The device memory it allocates is cached per host thread (gbfg_release_cached). */
 int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
-                       uint64_t seed, const double *host_s_instr, const gbfg_iter_params *params,
+                       uint64_t seed, const uint32_t *cat_ids, const double *host_s_instr, const gbfg_iter_params *params,
                        double *host_psd, uint8_t *host_resolved, gbfg_iter_result *host_results);
 
 /* gbfg_simulate_host keeps its device arena and stream between calls of the same host thread, so that

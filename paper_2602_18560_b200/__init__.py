@@ -103,8 +103,8 @@ def load():
     L.gbfg_coarse_grain.argtypes = [vp, i64, i32, vp, i32, dbl, dbl, vp, vp, vp, vp]
     L.gbfg_snr_select.argtypes = [gp, vp, vp, vp, op, i32, vp, dbl, vp, vp, vp, vp, vp, vp, sz, vp]
     L.gbfg_subtract_until_converged.argtypes = [gp, vp, vp, vp, op, i32, vp, ip, vp, vp, vp, vp, rp, vp, sz, vp]
-    L.gbfg_simulate.argtypes = [gp, pp, op, i32, u64, vp, ip, vp, vp, vp, vp, vp, vp, vp, vp, vp, rp, vp, sz, vp]
-    L.gbfg_simulate_host.argtypes = [gp, pp, op, i32, u64, vp, ip, vp, vp, rp]
+    L.gbfg_simulate.argtypes = [gp, pp, op, i32, u64, C.POINTER(u32), vp, ip, vp, vp, vp, vp, vp, vp, vp, vp, vp, rp, vp, sz, vp]
+    L.gbfg_simulate_host.argtypes = [gp, pp, op, i32, u64, C.POINTER(u32), vp, ip, vp, vp, rp]
     L.gbfg_profile_enable.argtypes = [C.c_int]
     L.gbfg_profile_read.argtypes = [C.POINTER(KernelTime), i32]
     L.gbfg_workspace_bytes.restype = sz
@@ -271,12 +271,21 @@ def subtract_until_converged(grid: Grid, dev_A, dev_f, dev_fdot, offsets, dev_s_
     return list(res)
 
 
+def _cat_ids(cat_ids, n_cat: int):
+    if cat_ids is None:
+        return None
+    if len(cat_ids) != n_cat:
+        raise ValueError("cat_ids must name every catalog of the call")
+    return (C.c_uint32 * n_cat)(*[int(c) for c in cat_ids])
+
+
 def simulate(grid: Grid, pops, offsets, seed: int, dev_s_instr, params: IterParams, dev_A, dev_f, dev_fdot,
-             dev_total, dev_spectrum, dev_median, dev_psd, dev_resolved, workspace, dev_err_count=None, stream=None):
+             dev_total, dev_spectrum, dev_median, dev_psd, dev_resolved, workspace, dev_err_count=None, stream=None,
+             cat_ids=None):
     n_cat = len(offsets) - 1
     res = (IterResult * n_cat)()
     _check(load().gbfg_simulate(
-        C.byref(grid), _pops(pops), _offsets(offsets), n_cat, seed, _ptr(dev_s_instr), C.byref(params),
+        C.byref(grid), _pops(pops), _offsets(offsets), n_cat, seed, _cat_ids(cat_ids, n_cat), _ptr(dev_s_instr), C.byref(params),
         _ptr(dev_A), _ptr(dev_f), _ptr(dev_fdot), _ptr(dev_total), _ptr(dev_spectrum), _ptr(dev_median),
         _ptr(dev_psd), _ptr(dev_resolved), _ptr(dev_err_count), res, _ptr(workspace),
         workspace.numel() * workspace.element_size(), _stream(stream)))
@@ -284,9 +293,10 @@ def simulate(grid: Grid, pops, offsets, seed: int, dev_s_instr, params: IterPara
 
 
 def simulate_host(grid: Grid, pops, offsets, seed: int, host_s_instr, params: IterParams, host_psd,
-                  host_resolved=None):
+                  host_resolved=None, cat_ids=None):
     n_cat = len(offsets) - 1
     res = (IterResult * n_cat)()
-    _check(load().gbfg_simulate_host(C.byref(grid), _pops(pops), _offsets(offsets), n_cat, seed, _ptr(host_s_instr),
+    _check(load().gbfg_simulate_host(C.byref(grid), _pops(pops), _offsets(offsets), n_cat, seed, _cat_ids(cat_ids, n_cat),
+                                     _ptr(host_s_instr),
                                      C.byref(params), _ptr(host_psd), _ptr(host_resolved), res))
     return list(res)

@@ -91,7 +91,7 @@ extern "C" const char *gbfg_strerror(int status)
     case GBFG_ERR_WORKSPACE: return "workspace missing or too small";
     case GBFG_ERR_CUDA: return "CUDA runtime error (see gbfg_last_cuda_error)";
     case GBFG_ERR_ARCH: return "device is not compute capability 10.x (sm_100)";
-    case GBFG_ERR_UNSUPPORTED: return "unsupported size (window > GBFG_MAX_WINDOW or n_cat > GBFG_MAX_CAT)";
+    case GBFG_ERR_UNSUPPORTED: return "unsupported size or parameter (window > GBFG_MAX_WINDOW, n_cat > GBFG_MAX_CAT, alpha_gamma outside its stated range)";
     default: return "unknown status";
     }
 }

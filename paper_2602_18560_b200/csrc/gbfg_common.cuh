@@ -20,6 +20,10 @@ int set_cuda_error(cudaError_t e, const char *where);   // records text, returns
 int check_device();                                     // GBFG_OK or GBFG_ERR_ARCH / GBFG_ERR_CUDA
 void count_launch(int n = 1);
 int sm_count();
+// stage (i) with explicit catalog ids (sample.cu): cat_ids HOST [n_cat] or NULL (first_cat_id + c)
+int sample_catalog_ids(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
+                       uint32_t first_cat_id, const uint32_t *cat_ids, uint64_t seed,
+                       double *dev_A, double *dev_f, double *dev_fdot, void *stream);
 
 // Kernel classes of the per-kernel timing helper (gbfg_profile_*; order = GBFG_K_* in gbfg.h).
 enum KernelId { K_SAMPLE = 0, K_NOISE, K_DEPOSIT, K_SCAN, K_MEDIAN, K_PSD, K_INV_BLOCKS, K_SNR, K_AUX, K_COUNT };
@@ -152,6 +156,7 @@ struct MedianPlan {
     int n_dblk;
     int dblk_log2;
     int max_items;
+    int *near_fold;     // SnrWork::any_near (nullable): plan_kernel folds word 1 into word 0
 };
 
 // What plan_kernel hands to the host before it clears the iteration's counters (loop.cu): n words of src copied to
@@ -185,7 +190,9 @@ struct SnrWork {
     int *bkt_ext;       // [n_cat][n_dblk]      last block any record of the bucket reaches, then its prefix maximum
     int *bkt_reach;     // [n_cat][n_dblk]      first bucket with a record that reaches block b (n_dblk: none)
     int64_t *bkt_off;   // [n_cat][n_dblk + 1]  first record of each bucket (global record index)
-    int *any_near;      // one int: a record was flagged near-threshold (the whole list is tested from then on)
+    int *any_near;      // two ints.  [0]: a record was flagged near-threshold in an EARLIER pass (the whole list is tested
+                        // from then on); read-only for the test, so that every CTA of one launch takes the same record
+                        // range.  [1]: raised by the test of this pass; plan_kernel folds it into [0] between two passes
 };
 
 // ---------------------------------------------------------------------------------------------

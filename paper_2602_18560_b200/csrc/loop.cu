@@ -115,7 +115,8 @@ static Workspace carve(void *base, int64_t n_bins, int64_t n_src_total, int n_ca
     w.sw.bkt_ext = (int *)take(sizeof(int) * (size_t)n_cat * (size_t)n_dblk);
     w.sw.bkt_reach = (int *)take(sizeof(int) * (size_t)n_cat * (size_t)n_dblk);
     w.sw.bkt_off = (int64_t *)take(sizeof(int64_t) * (size_t)n_cat * (size_t)(n_dblk + 1));
-    w.sw.any_near = (int *)take(sizeof(int));
+    w.sw.any_near = (int *)take(2 * sizeof(int));
+    w.plan.near_fold = w.sw.any_near;
     w.bytes = off;
     return w;
 }
@@ -186,9 +187,10 @@ static HostCallCache &host_call_cache()
 }
 
 // event that marks the per-iteration readback (one per host thread)
+static thread_local cudaEvent_t g_ev_read = nullptr;
 static cudaEvent_t readback_event()
 {
-    static thread_local cudaEvent_t ev = nullptr;
+    cudaEvent_t &ev = g_ev_read;
     if (!ev && cudaEventCreateWithFlags(&ev, cudaEventDisableTiming) != cudaSuccess) { (void)cudaGetLastError(); ev = nullptr; }
     return ev;
 }
@@ -215,6 +217,56 @@ static SideStream *side_stream()
         }
     }
     return &ss;
+}
+
+// Everything above that is kept per host thread (stream, events, device arena) belongs to the device that was current
+// when it was made.  A thread that comes back with another current device gets fresh ones (a stream or an event of one
+// device is an invalid handle under another; the mapped host scratch is portable and stays).
+static void release_thread_resources()
+{
+    HostCallCache &cc = host_call_cache();
+    if (cc.stream) { cudaStreamSynchronize(cc.stream); cudaStreamDestroy(cc.stream); cc.stream = nullptr; }
+    if (cc.base) { cudaFree(cc.base); cc.base = nullptr; cc.bytes = 0; }
+    SideStream *side = side_stream_if_any();
+    if (side) {                                          // the loop's side stream and its events
+        cudaStreamSynchronize(side->s);
+        cudaEventDestroy(side->ev_plan);
+        cudaEventDestroy(side->ev_aux);
+        cudaEventDestroy(side->ev_noise);
+        cudaStreamDestroy(side->s);
+        side->s = nullptr;
+    }
+    if (g_ev_read) { cudaEventDestroy(g_ev_read); g_ev_read = nullptr; }
+    (void)cudaGetLastError();
+}
+
+static int bind_thread_to_current_device()
+{
+    static thread_local int tl_dev = -1;
+    int dev = 0;
+    GBFG_CUDA(cudaGetDevice(&dev));
+    if (tl_dev != dev) {
+        if (tl_dev >= 0) {
+            // the old resources are destroyed with their own device current
+            if (cudaSetDevice(tl_dev) == cudaSuccess) release_thread_resources();
+            (void)cudaGetLastError();
+            GBFG_CUDA(cudaSetDevice(dev));
+        }
+        tl_dev = dev;
+    }
+    return GBFG_OK;
+}
+
+// an error return leaves nothing of the call in flight: kernels queued on the side stream still use the caller's buffers
+static int drain_on_error(int rc, cudaStream_t st)
+{
+    if (rc != GBFG_OK) {
+        SideStream *side = side_stream_if_any();
+        if (side) (void)cudaStreamSynchronize(side->s);
+        (void)cudaStreamSynchronize(st);
+        (void)cudaGetLastError();
+    }
+    return rc;
 }
 
 static DepositMarks plain_marks(const Workspace &w, int64_t n_bins, int stamp)
@@ -343,13 +395,13 @@ static int loop_validate(const gbfg_grid *grid, const gbfg_iter_params *params)
 
 // the loop proper.  prepared: the caller has initialised the workspace and built the candidate records (gbfg_simulate
 // does both next to the deposit).
-static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *dev_f,
+static int loop_body(const gbfg_grid *grid, const double *dev_A, const double *dev_f,
                      const double *dev_fdot, const int64_t *offsets, int32_t n_cat,
                      const double *dev_s_instr, const gbfg_iter_params *params,
                      int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
                      uint8_t *dev_resolved, gbfg_iter_result *host_results,
                      void *workspace, size_t workspace_bytes, void *stream, bool prepared,
-                     cudaEvent_t records_ready = nullptr)
+                     cudaEvent_t records_ready)
 {
     int rc = loop_validate(grid, params);
     if (rc) return rc;
@@ -534,6 +586,23 @@ static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *d
     return GBFG_OK;
 }
 
+static int loop_impl(const gbfg_grid *grid, const double *dev_A, const double *dev_f,
+                     const double *dev_fdot, const int64_t *offsets, int32_t n_cat,
+                     const double *dev_s_instr, const gbfg_iter_params *params,
+                     int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
+                     uint8_t *dev_resolved, gbfg_iter_result *host_results,
+                     void *workspace, size_t workspace_bytes, void *stream, bool prepared,
+                     cudaEvent_t records_ready = nullptr)
+{
+    int rc = loop_validate(grid, params);                  // argument errors are reported before any CUDA call
+    if (rc) return rc;
+    rc = bind_thread_to_current_device();
+    if (rc) return rc;
+    return drain_on_error(loop_body(grid, dev_A, dev_f, dev_fdot, offsets, n_cat, dev_s_instr, params, dev_spectrum, dev_median,
+                                    dev_psd, dev_resolved, host_results, workspace, workspace_bytes, stream, prepared,
+                                    records_ready), (cudaStream_t)stream);
+}
+
 extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double *dev_A, const double *dev_f,
                                              const double *dev_fdot, const int64_t *offsets, int32_t n_cat,
                                              const double *dev_s_instr, const gbfg_iter_params *params,
@@ -547,12 +616,12 @@ extern "C" int gbfg_subtract_until_converged(const gbfg_grid *grid, const double
 
 // sample -> deposit -> loop.  The candidate records of the loop (a pass over the catalog against S_instr alone) are
 // built on the side stream while the deposit runs: both only read the catalog.
-extern "C" int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
-                             uint64_t seed, const double *dev_s_instr, const gbfg_iter_params *params,
-                             double *dev_A, double *dev_f, double *dev_fdot,
-                             int64_t *dev_total, int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
-                             uint8_t *dev_resolved, int64_t *dev_err_count, gbfg_iter_result *host_results,
-                             void *workspace, size_t workspace_bytes, void *stream)
+static int simulate_body(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
+                         uint64_t seed, const uint32_t *cat_ids, const double *dev_s_instr, const gbfg_iter_params *params,
+                         double *dev_A, double *dev_f, double *dev_fdot,
+                         int64_t *dev_total, int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
+                         uint8_t *dev_resolved, int64_t *dev_err_count, gbfg_iter_result *host_results,
+                         void *workspace, size_t workspace_bytes, void *stream)
 {
     int rc = loop_validate(grid, params);
     if (rc) return rc;
@@ -577,7 +646,7 @@ extern "C" int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const 
     rc = loop_prefix_s_instr(g, dev_s_instr, preselect, w, side->s);
     if (rc) return rc;
     GBFG_CUDA(cudaEventRecord(side->ev_noise, side->s));    // S_instr is on the device by now (gbfg_simulate_host copies it on this stream)
-    rc = gbfg_sample_catalog(grid, pops, offsets, n_cat, 0u, seed, dev_A, dev_f, dev_fdot, stream);
+    rc = sample_catalog_ids(grid, pops, offsets, n_cat, 0u, cat_ids, seed, dev_A, dev_f, dev_fdot, stream);
     if (rc) return rc;
     const size_t row_bytes = sizeof(int64_t) * (size_t)n_cat * (size_t)nb;
     GBFG_CUDA(cudaMemsetAsync(dev_spectrum, 0, row_bytes, st));
@@ -597,18 +666,36 @@ extern "C" int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const 
     if (dev_total) GBFG_CUDA(cudaMemcpyAsync(dev_total, dev_spectrum, row_bytes, cudaMemcpyDeviceToDevice, st));
     GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_noise, 0));  // the first estimator pass reads S_instr
     // the loop waits for the records (side->ev_aux) after its first estimator pass, which overlaps their build
-    return loop_impl(grid, dev_A, dev_f, dev_fdot, offsets, n_cat, dev_s_instr, params, dev_spectrum, dev_median, dev_psd,
+    return loop_body(grid, dev_A, dev_f, dev_fdot, offsets, n_cat, dev_s_instr, params, dev_spectrum, dev_median, dev_psd,
                      dev_resolved, host_results, workspace, workspace_bytes, stream, true, side->ev_aux);
 }
 
+extern "C" int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
+                             uint64_t seed, const uint32_t *cat_ids, const double *dev_s_instr, const gbfg_iter_params *params,
+                             double *dev_A, double *dev_f, double *dev_fdot,
+                             int64_t *dev_total, int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
+                             uint8_t *dev_resolved, int64_t *dev_err_count, gbfg_iter_result *host_results,
+                             void *workspace, size_t workspace_bytes, void *stream)
+{
+    int rc = loop_validate(grid, params);
+    if (rc) return rc;
+    rc = bind_thread_to_current_device();
+    if (rc) return rc;
+    return drain_on_error(simulate_body(grid, pops, offsets, n_cat, seed, cat_ids, dev_s_instr, params, dev_A, dev_f, dev_fdot,
+                                        dev_total, dev_spectrum, dev_median, dev_psd, dev_resolved, dev_err_count, host_results,
+                                        workspace, workspace_bytes, stream), (cudaStream_t)stream);
+}
+
 extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
-                                  uint64_t seed, const double *host_s_instr, const gbfg_iter_params *params,
+                                  uint64_t seed, const uint32_t *cat_ids, const double *host_s_instr, const gbfg_iter_params *params,
                                   double *host_psd, uint8_t *host_resolved, gbfg_iter_result *host_results)
 {
     if (!valid_grid(grid) || !pops || !offsets || n_cat < 1 || !host_s_instr || !host_psd || !host_results)
         return GBFG_ERR_INVALID_ARG;
     if (n_cat > GBFG_MAX_CAT) return GBFG_ERR_UNSUPPORTED;
     int rc = check_device();
+    if (rc) return rc;
+    rc = bind_thread_to_current_device();
     if (rc) return rc;
     const int64_t n = offsets[n_cat];
     const size_t nb = (size_t)grid->n_bins, rows = (size_t)n_cat * nb;
@@ -645,7 +732,7 @@ extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, c
     e = cudaMemcpyAsync(base + oI, host_s_instr, 8 * nb, cudaMemcpyHostToDevice, side->s);
     if (e != cudaSuccess) rc = set_cuda_error(e, "cudaMemcpyAsync(s_instr)");
     if (!rc)
-        rc = gbfg_simulate(grid, pops, offsets, n_cat, seed, (const double *)(base + oI), params,
+        rc = gbfg_simulate(grid, pops, offsets, n_cat, seed, cat_ids, (const double *)(base + oI), params,
                            (double *)(base + oA), (double *)(base + oF), (double *)(base + oD), nullptr,
                            (int64_t *)(base + oS), (int64_t *)(base + oM), (double *)(base + oP),
                            (uint8_t *)(base + oR), nullptr, host_results, base + oW, ws_bytes, st);
@@ -662,17 +749,6 @@ extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, c
 
 extern "C" int gbfg_release_cached(void)
 {
-    HostCallCache &cc = host_call_cache();
-    if (cc.stream) { cudaStreamSynchronize(cc.stream); cudaStreamDestroy(cc.stream); cc.stream = nullptr; }
-    if (cc.base) { cudaFree(cc.base); cc.base = nullptr; cc.bytes = 0; }
-    SideStream *side = side_stream_if_any();
-    if (side) {                                          // the loop's side stream and its events
-        cudaStreamSynchronize(side->s);
-        cudaEventDestroy(side->ev_plan);
-        cudaEventDestroy(side->ev_aux);
-        cudaEventDestroy(side->ev_noise);
-        cudaStreamDestroy(side->s);
-        side->s = nullptr;
-    }
+    release_thread_resources();
     return GBFG_OK;
 }

@@ -72,6 +72,8 @@ struct PlanArgs {
     int64_t *pub_dst;
     int pub_n, pub_flag_at;
     int64_t pub_seq;
+    int *near_fold;         // SnrWork::any_near (nullable): a near-threshold flag raised by the last test (word 1) becomes
+                            // visible to the next one (word 0) here, between the two launches
 };
 
 // len < 2^31 (n_bins is): 32-bit divisions, the 64-bit ones are long instruction sequences
@@ -110,6 +112,7 @@ plan_kernel(PlanArgs a)
     int *s_run = s_mem + nb + 9;                               // (first block, end block, first piece) per run
     if (tid == 0) row_pieces = 0;
     if (row == 0 && tid < 2) a.wide_ctr[tid] = 0;
+    if (row == 0 && tid == 0 && a.near_fold && a.near_fold[1]) a.near_fold[0] = 1;
     if (row == 0 && a.pub_dst) {
         // what the pass before wrote (this kernel runs behind the SNR test) goes to the host by plain stores over
         // PCIe: no copy engine on the path, and the counters can be cleared by the same CTA right behind
@@ -255,6 +258,7 @@ int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins,
     if (pub) { a.pub_src = pub->src; a.pub_dst = pub->dst; a.pub_n = pub->n; a.pub_flag_at = pub->flag_at; a.pub_seq = pub->seq; }
     else { a.pub_src = nullptr; a.pub_dst = nullptr; a.pub_n = 0; a.pub_flag_at = 0; a.pub_seq = 0; }
     a.zero2_ptr = zero2_ptr;
+    a.near_fold = pl.near_fold;
     a.zero_ptr = zero_ptr; a.zero_n = zero_n; a.out_count = out_count;
     a.blk_stamp = blk_stamp; a.stamp = stamp; a.all_dirty = (all_dirty || !blk_stamp) ? 1 : 0;
     a.n_dblk = pl.n_dblk; a.dblk_log2 = pl.dblk_log2; a.n_bins = n_bins;

@@ -505,6 +505,8 @@ extern "C" int gbfg_sample_catalog_paper(const gbfg_grid *grid, const gbfg_pop_p
         if (offsets[c + 1] - offsets[c] != p.n_src) return GBFG_ERR_INVALID_ARG;
         if (!(p.alpha_gamma > 0.0) || !(p.beta_gamma > 0.0) || !(p.sigma >= 0.0) || !(p.rho >= 0.0) || !(p.rho < 1.0))
             return GBFG_ERR_INVALID_ARG;
+        // the fixed-length recurrences of DESIGN.md R12 are stated (and pinned) for this range; Table I draws alpha from [1, 3]
+        if (p.alpha_gamma < GBFG_PAPER_ALPHA_MIN || p.alpha_gamma > GBFG_PAPER_ALPHA_MAX) return GBFG_ERR_UNSUPPORTED;
     }
     if (offsets[n_cat] > 0 && (!dev_A || !dev_f || !dev_fdot)) return GBFG_ERR_INVALID_ARG;
     int rc = check_device();
@@ -544,9 +546,10 @@ extern "C" int gbfg_sample_catalog_paper(const gbfg_grid *grid, const gbfg_pop_p
     return GBFG_OK;
 }
 
-extern "C" int gbfg_sample_catalog(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets,
-                                   int32_t n_cat, uint32_t first_cat_id, uint64_t seed,
-                                   double *dev_A, double *dev_f, double *dev_fdot, void *stream)
+// cat_ids (HOST [n_cat], nullable): Philox counter word 3 of catalog c; NULL: first_cat_id + c
+int gbfg::sample_catalog_ids(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets,
+                             int32_t n_cat, uint32_t first_cat_id, const uint32_t *cat_ids, uint64_t seed,
+                             double *dev_A, double *dev_f, double *dev_fdot, void *stream)
 {
     if (!grid || grid->struct_size != sizeof(gbfg_grid) || !pops || !offsets) return GBFG_ERR_INVALID_ARG;
     if (n_cat < 1) return GBFG_ERR_INVALID_ARG;
@@ -579,7 +582,7 @@ extern "C" int gbfg_sample_catalog(const gbfg_grid *grid, const gbfg_pop *pops, 
         P.logMc_mean = p.logMc_mean; P.logMc_sigma = p.logMc_sigma;
         P.f_min = grid->f_min; P.f_max = grid->f_max; P.f_top = nextafter(grid->f_max, 0.0);
         P.n_src = p.n_src;
-        P.cat_id = first_cat_id + (uint32_t)c;
+        P.cat_id = cat_ids ? cat_ids[c] : first_cat_id + (uint32_t)c;
         P.key0 = (uint32_t)seed; P.key1 = (uint32_t)(seed >> 32);
         int head = (int)(offsets[c] & 1);                 // keep the pairs 16-byte aligned
         if (head > p.n_src) head = (int)p.n_src;
@@ -596,4 +599,11 @@ extern "C" int gbfg_sample_catalog(const gbfg_grid *grid, const gbfg_pop *pops, 
         GBFG_LAUNCH_CHECK("sample_kernel");
     }
     return GBFG_OK;
+}
+
+extern "C" int gbfg_sample_catalog(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets,
+                                   int32_t n_cat, uint32_t first_cat_id, uint64_t seed,
+                                   double *dev_A, double *dev_f, double *dev_fdot, void *stream)
+{
+    return sample_catalog_ids(grid, pops, offsets, n_cat, first_cat_id, nullptr, seed, dev_A, dev_f, dev_fdot, stream);
 }

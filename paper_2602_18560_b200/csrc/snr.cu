@@ -493,7 +493,7 @@ snr_cand_kernel(SnrArgs a)
     const int64_t *off = a.bkt_off + (int64_t)rowc * (a.n_dblk + 1);
     const int abort_v = a.abort_flag ? *a.abort_flag : 0;
     const unsigned long long dbits = a.delta_bits ? a.delta_bits[rowc] : 0ull;
-    const int near_v = a.dv.cum ? *a.any_near : 1;
+    const int near_v = a.dv.cum ? a.any_near[0] : 1;     // launch-invariant: raised flags go to word 1
     const int b_min = a.dv.cum ? a.dv.range[2 * rowc] : 0, b_max = a.dv.cum ? a.dv.range[2 * rowc + 1] : 0;
     const int hdr_bad = a.pv.pref ? a.pv.hdr->bad : 1;
     const int unit_exp = a.pv.pref ? a.pv.hdr->unit_exp : 0;
@@ -601,7 +601,7 @@ snr_cand_kernel(SnrArgs a)
                 }
             }
         }
-        if (near && !sel && !always) { a.cand.w[t] = -w; *a.any_near = 1; }
+        if (near && !sel && !always) { a.cand.w[t] = -w; a.any_near[1] = 1; }
         if (near_mask && lane == 0) atomicAdd(&s_near, __popc(near_mask));
     }
     // one append per CTA for what its buffer holds
@@ -689,7 +689,7 @@ int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, con
     a.bkt_count = sw.bkt_count; a.bkt_ext = sw.bkt_ext; a.n_dblk = n_dblk; a.dblk_log2 = dblk_log2;
     GBFG_CUDA(cudaMemsetAsync(sw.bkt_count, 0, sizeof(int) * (size_t)ct.n_cat * (size_t)n_dblk, st));
     GBFG_CUDA(cudaMemsetAsync(sw.bkt_ext, 0, sizeof(int) * (size_t)ct.n_cat * (size_t)n_dblk, st));
-    GBFG_CUDA(cudaMemsetAsync(sw.any_near, 0, sizeof(int), st));
+    GBFG_CUDA(cudaMemsetAsync(sw.any_near, 0, 2 * sizeof(int), st));
     int64_t blocks = (n + 255) / 256;
     const int64_t cap = (int64_t)sm_count() * 16;
     if (blocks > cap) blocks = cap;

@@ -107,6 +107,27 @@ def test_invalid_arguments_are_rejected_before_any_cuda_call(gbcpu):
     assert L.gbfg_subtract_until_converged(C.byref(g), 8, 8, 8, off, 1, 8, C.byref(p2), 8, 8, 8, 8, res, 8, 1 << 40, None) == -1
 
 
+def test_paper_sampler_rejects_parameters_outside_the_stated_domain(gbcpu):
+    """DESIGN.md R12: the special functions of the paper's sampler are stated and pinned for 0.25 <= alpha_Gamma <= 16."""
+    L = gbcpu.load()
+    g = gbcpu.grid_init(1e-4, 1e-2, 3.15581e7, -140)
+    off = (C.c_int64 * 2)(0, 10)
+
+    class P:
+        alpha_pl, alpha_gamma, beta_gamma, mu_gamma, mu, sigma, rho, n_src = -2.9, 1.96, 1.8, -21.0, -22.0, 0.18, 0.5, 10
+
+    def call(**kw):
+        p = P()
+        for k, v in kw.items():
+            setattr(p, k, v)
+        arr = (gbcpu.PopPaper * 1)(gbcpu.make_pop_paper(p))
+        return L.gbfg_sample_catalog_paper(C.byref(g), arr, off, 1, 0, 1, 16, 16, 16, None)
+
+    assert call(alpha_gamma=0.2) == -5 and call(alpha_gamma=16.5) == -5
+    assert call(alpha_gamma=-1.0) == -1 and call(beta_gamma=0.0) == -1 and call(rho=1.0) == -1 and call(sigma=-0.1) == -1
+    assert call(alpha_gamma=1.0) in (0, -3, -4)            # accepted: reaches the device check (no GPU here: -3 / -4)
+
+
 def test_workspace_bytes_grows_with_the_problem(gbcpu):
     g = gbcpu.grid_init(1e-4, 3e-2, 4 * 3.15581e7, -140)
     a = gbcpu.workspace_bytes(g, 10**6, 1)
