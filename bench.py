@@ -8,9 +8,12 @@ through the C ABI (gbfg_simulate).  Prints ONE JSON line (see the task contract)
   e2e        the same through gbfg_simulate_host: host buffers, H2D/D2H inside the timed region
   roofline   the dominant kernel's algorithmic bytes / CUDA-event time against MEASURED_PEAKS.json
   kernels    the same for every kernel class (events recorded on the launching stream, live)
-  cpu_baseline  the oracle, as it stands, on the host cores, on a bounded sample
+  cpu_baseline  the oracle, as it stands, on one host core, on the SAME workload in full (config 3: about half a
+                minute), with the seconds it spends per stage; `--cpu-config4` adds the 64 catalogs of configs[4]
+                over all host cores (one oracle process per catalog)
 
-`--impl reference` times the oracle alone (rank 0 only) and prints its own line.
+`--impl reference` times the oracle alone (rank 0 only) on the same full workload and prints its own line; it
+honours --steps up to a time budget (REFERENCE_BUDGET_S), with a floor of one step, and says how many it ran.
 N > 1 (torchrun): every rank runs its own independent catalog (seed + rank); no data-path
 collective; value = all ranks' sources / max-over-ranks time; scaling "weak".
 """
@@ -33,7 +36,7 @@ import gbfg_workloads as wl
 
 METRIC = "catalog_to_foreground_throughput"
 UNIT = "sources/s"
-CPU_SAMPLE_SOURCES = 1_000_000      # bounded oracle sample: the first 1e6 sources of the config-3 catalog
+REFERENCE_BUDGET_S = 150.0          # the reference arm stops taking further steps once this much oracle time is spent
 
 
 def measured_peaks():
@@ -147,44 +150,66 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------- reference arm
-def oracle_sample_run(w: wl.Workload, n_src: int):
-    """The oracle, as it stands, on the first n_src sources of workload w's catalog, whole path."""
+def oracle_full_run(w: wl.Workload):
+    """The oracle, as it stands, on workload w's catalog 0 in full, whole path, one thread."""
     import oracle
     oracle.build()
     oracle.lib()
     t0 = time.perf_counter()
-    out = oracle.simulate(w, cat=0, n_src=n_src)
+    out = oracle.simulate(w, cat=0)
     dt = time.perf_counter() - t0
     return dt, out
+
+
+def oracle_sample_text(w: wl.Workload, out) -> str:
+    return (f"{w.name} in full: all {w.n_src_total} sources of the seeded catalog on the full grid (window {w.window}, "
+            f"cap {w.max_iter}), whole path sample->deposit->loop, {int(out['n_iter'])} iterations, "
+            f"{int(out['n_resolved'])} resolved, 1 thread")
 
 
 def run_reference(args, w: wl.Workload):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return 0
-    n_s = min(CPU_SAMPLE_SOURCES, w.n_src_total)
-    sample = (f"{w.name}: first {n_s} of {w.n_src_total} sources of the seeded catalog on the full grid "
-              f"(window {w.window}, cap {w.max_iter}), whole path sample->deposit->loop, 1 thread")
-    for _ in range(args.warmup):
-        pass        # the oracle has no warm-up state; warm-up steps are not run (minutes each)
-    times, iters = [], None
-    for _ in range(args.steps):
-        dt, out = oracle_sample_run(w, n_s)
+    # the oracle has no warm-up state: warm-up steps are not run (half a minute each)
+    times, out = [], None
+    spent = 0.0
+    for _ in range(max(1, args.steps)):
+        dt, out = oracle_full_run(w)
         times.append(dt)
-        iters = int(out["n_iter"])
+        spent += dt
+        if spent + dt > REFERENCE_BUDGET_S:
+            break
     t = float(np.mean(times))
-    val = n_s / t
+    n = w.n_src_total
+    val = n / t
+    sample = oracle_sample_text(w, out) + f"; {len(times)} of the {args.steps} requested steps run (time budget {REFERENCE_BUDGET_S:.0f} s)"
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
-        "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True, "scaling": "weak",
+        "steps_run": len(times), "warmup": args.warmup, "ms_per_step": 1e3 * t, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64+i64", "data": "synthetic",
-        "config": {"workload": w.name, "sample": sample, "n_iter": iters},
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "config": {"workload": w.name, "n_src": n, "n_cat": w.n_cat, "window": w.window, "rho_th": w.rho_th,
+                   "max_iter": w.max_iter, "t_obs_s": w.t_obs, "band_hz": [w.f_min, w.f_max], "seed": w.seed,
+                   "n_iter": int(out["n_iter"]), "converged": int(out["converged"]), "n_resolved": int(out["n_resolved"])},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample,
+                         "seconds": t, "stage_seconds": out["stage_s"]},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
     return 0
+
+
+def oracle_config4_leg():
+    """configs[4] through the oracle: 64 independent single-threaded runs over the host cores."""
+    from oracle import pool
+    w4 = wl.config(4)
+    out = pool.simulate_many(w4, range(w4.n_cat))
+    core_s = sum(r["seconds"] for r in out["results"].values())
+    return {"workload": w4.name, "n_src": w4.n_src_total, "n_cat": w4.n_cat, "cores": out["n_proc"],
+            "host_cores": pool.host_cores(), "wall_seconds": out["wall_seconds"], "core_seconds": core_s,
+            "value": w4.n_src_total / out["wall_seconds"], "unit": UNIT, "kind": "oracle",
+            "sample": "all 64 catalogs in full, one oracle process per catalog"}
 
 
 # ------------------------------------------------------------------------------------ GPU arm
@@ -360,15 +385,16 @@ def run_gpu(args, w: wl.Workload):
                           "peak_source": f"{sms} SMs x 4 schedulers x {mhz:.0f} MHz (sm clock under load)",
                           "instr_per_output": MEDIAN_WARP_INSTR_PER_OUTPUT}
 
-    # ---- the oracle on the host cores, bounded sample
+    # ---- the oracle on one host core, the same workload in full (a reported baseline, not the target)
     cpu = None
     if not args.no_cpu_baseline:
-        n_s = min(CPU_SAMPLE_SOURCES, n)
-        dt, out = oracle_sample_run(wl.replace(w, seed=w.seed), n_s)
-        cpu = {"value": n_s / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
-               "sample": f"first {n_s} of {n} sources of the same seeded catalog on the full grid, whole path "
-                         f"(sample->deposit->loop, {int(out['n_iter'])} iterations), 1 thread of "
-                         f"{os.cpu_count()} host cores"}
+        dt, out = oracle_full_run(wl.replace(w, seed=w.seed))
+        same = (int(out["n_iter"]), int(out["n_resolved"])) == (int(r0.n_iter), int(r0.n_resolved))
+        cpu = {"value": n / dt, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt,
+               "stage_seconds": out["stage_s"], "host_cores": os.cpu_count(),
+               "same_outcome_as_gpu": same, "sample": oracle_sample_text(w, out)}
+        if args.cpu_config4:
+            cpu["config4"] = oracle_config4_leg()
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -408,6 +434,8 @@ def main():
     ap.add_argument("--max-iter", type=int, default=None, help="override the iteration cap (debug only: cost per iteration)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-config4", action="store_true",
+                    help="also time the oracle on configs[4] (64 catalogs) over all host cores: minutes")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel from the committed ncu --set full capture")
     args = ap.parse_args()
