@@ -8,16 +8,18 @@
 // last subtraction made dirty, or (stage call) from a static tiling of every row.  The tile and its two h-bin
 // halos (Lt = outputs + 2h <= LT positions, rounded up to a multiple of the CTA width) are staged in shared
 // memory and sorted ONCE by (value, position): an LSD radix sort, 8 bits per pass, that skips the passes whose
-// digit is the same for the whole tile (spectrum values rarely need more than four).  With the sorted order in
-// hand a window is a position interval, and its median is found without ever sorting a window:
-//   * a (rank-bucket x position-block) table of counts locates the h-th smallest element of a block-aligned
-//     position interval: the coarse state (median rank of the window) of the first 32-output chunk of every
-//     warp; the warp's next chunks follow by sliding the window 32 bins at a time;
-//   * every thread then takes 8 outputs: it jumps from the coarse state to its first output by counting the
-//     ranks that left and entered, and walks: sliding the window by one bin removes one position and adds
-//     one, which moves the median by at most one place in the sorted order; the neighbouring in-window
-//     element is found by stepping through the sorted positions (on average LT/W steps; long stretches of
-//     out-of-window elements — plateaus left by wide chirps — are crossed by the whole warp, 32 ranks a step).
+// digit is the same for the whole tile (spectrum values rarely need more than four).  The lanes of a warp that
+// hold the same digit are found with eight warp reductions (a ballot each), not with match.any: the SM retires
+// one MATCH every ~50 clocks, which made it the single slowest thing in the kernel.  With the sorted order in
+// hand a window is a set of ranks, kept as a bitmap (one bit per rank), and its median is the (h+1)-th set bit:
+//   * the bitmaps of 16 windows per tile (one per warp, evenly spaced) are built by ballots over the sorted
+//     positions, and the (h+1)-th set bit of each is found by counting words;
+//   * every warp then slides its window 32 outputs at a time.  Inside such a chunk lane i takes output j0 + i:
+//     two popcounts of ballots (how many of the ranks that left / entered lie under the chunk's first median)
+//     say how many window elements it must move, and in which direction; it moves word by word — 32 ranks and
+//     typically 8 window elements per step, one popcount — testing positions only for the 64 "special" ranks
+//     that enter or leave inside the chunk (a second bitmap marks them), and picks the bit in the last word.
+//     Plateaus left by wide chirps (long stretches of out-of-window ranks) cost one step per 32 ranks.
 // The per-output rank is kept in shared memory and written out coalesced, fused with
 //     psd[k] = s_instr[k] + C * (med[k] * 2^scale_log2)        (eqs. 10, D2, D3).
 #include "median_kernel.cuh"
@@ -314,7 +316,7 @@ int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64
     a.n = n_bins; a.h = window / 2;
     a.tiles = median_static_tiles(n_bins, n_cat, window, &a.S);
     a.norm = norm; a.scale = ldexp(1.0, scale_log2);
-    constexpr size_t smem32 = median_smem_bytes<uint32_t>(), smem64 = median_smem_bytes<uint64_t>();
+    constexpr size_t smem32 = median_smem_bytes<uint32_t, 512>(), smem64 = median_smem_bytes<uint64_t, 1024>();
     static thread_local int attr_dev = -1;
     int dev = 0;
     GBFG_CUDA(cudaGetDevice(&dev));

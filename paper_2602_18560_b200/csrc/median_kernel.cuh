@@ -7,7 +7,7 @@
 //                     order a tile whenever its values agree in their high 32 bits — spectra in units of
 //                     2^-140 strain^2 always do.  A tile that does not is appended to the wide list.
 //   <uint64_t, 1024>  full 64-bit keys, one CTA per SM: the tiles of the wide list.
-// See median.cu for the algorithm (sort once per tile, count table, coarse states, walk).
+// See median.cu for the algorithm (sort once per tile, window bitmaps over the sorted order, word-wise walk).
 #pragma once
 
 #include "gbfg_common.cuh"
@@ -15,26 +15,28 @@
 namespace gbfg {
 
 constexpr int MED_LT = 8192;                  // positions per tile, halos included
-constexpr int MED_PB = 32;                    // position block = outputs per coarse chunk
-constexpr int MED_FINE = 8;                   // outputs per walking thread
-constexpr int MED_STEP_CAP = 20;              // places a thread steps alone before the warp takes over
-constexpr int MED_RB = 128;                   // sorted ranks per bucket
-constexpr int MED_NPB = MED_LT / MED_PB;      // 256
-constexpr int MED_NRB = MED_LT / MED_RB;      // 64
-constexpr int MED_TROW = MED_NPB + 2;         // table row stride in u16 (even: rows stay 4-byte aligned)
+constexpr int MED_PB = 32;                    // outputs per chunk (one per lane)
 constexpr int MED_CROW = 256 + 2;             // radix counter row stride in u16 (one row per warp)
 constexpr uint64_t SIGN64 = 0x8000000000000000ull;
-constexpr int MED_AUX_U16 = MED_NRB * MED_TROW;   // count table (>= 32 rows of radix counters, >= LT output ranks)
 
-template <typename KeyT>
+// aux: the radix counters (one row per warp) during the sort; afterwards one window bitmap per warp (LT bits) and,
+// behind them, the output ranks
+__host__ __device__ constexpr int median_aux_u16(int threads)
+{
+    const int warps = threads / 32;
+    const int sort_u16 = warps * MED_CROW;
+    const int walk_u16 = 2 * warps * (MED_LT / 32) * 2 + MED_LT;      // window and specials bitmaps, output ranks
+    return sort_u16 > walk_u16 ? sort_u16 : walk_u16;
+}
+
+template <typename KeyT, int THREADS>
 constexpr size_t median_smem_bytes()
 {
-    return sizeof(KeyT) * MED_LT             // skey
-         + sizeof(uint16_t) * MED_LT         // spos
-         + sizeof(uint16_t) * MED_LT         // rop
-         + sizeof(uint16_t) * MED_AUX_U16    // radix counters, then the count table, then the output ranks
-         + sizeof(uint16_t) * MED_NPB        // coarse medians
-         + sizeof(uint32_t) * 40;            // scan partials, varying-bit mask
+    return sizeof(KeyT) * MED_LT                          // skey
+         + sizeof(uint16_t) * MED_LT                      // spos
+         + sizeof(uint16_t) * MED_LT                      // rop
+         + sizeof(uint16_t) * median_aux_u16(THREADS)     // radix counters, then the window bitmaps and the output ranks
+         + sizeof(uint32_t) * 40;                         // scan partials, varying-bit mask
 }
 
 struct MedianArgs {
@@ -54,7 +56,17 @@ struct MedianArgs {
     int S;                   // outputs per tile of the static tiling
     int tiles;
     double norm, scale;      // C and 2^scale_log2
+#ifdef MED_TIMING
+    long long *dbg;          // probe builds only (-DMED_TIMING): [gridDim.x][16] cycles per phase, summed over a CTA's tiles
+#endif
 };
+
+#ifdef MED_TIMING
+// phase i = the time between tick i and the tick before it, summed over the CTA's tiles, per CTA
+#define MED_TICK(i) do { if (tid == 0) { const long long now_ = clock64(); if (i) a.dbg[blockIdx.x * 16 + (i)] += now_ - med_t_prev; med_t_prev = now_; } } while (0)
+#else
+#define MED_TICK(i) do { } while (0)
+#endif
 
 // n-th (1-based) set bit of a non-zero mask that has at least n bits set
 __device__ __forceinline__ int nth_set_bit(unsigned m, int n)
@@ -68,14 +80,28 @@ __device__ __forceinline__ int nth_set_bit(unsigned m, int n)
     return pos;
 }
 
-// lanes of the warp whose 8-bit digit equals this lane's (what match.any computes, from 8 ballots)
+// bit updates of the window bitmaps: shared-memory reductions on a 32-bit shared address (the generic-address form
+// costs a dozen instructions of address arithmetic per update)
+__device__ __forceinline__ void smem_or(uint32_t addr, unsigned v)
+{
+    asm volatile("red.shared.or.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ void smem_and(uint32_t addr, unsigned v)
+{
+    asm volatile("red.shared.and.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+
+// lanes of the warp whose 8-bit digit equals this lane's: what match.any computes, from 8 ballots.  MATCH.ANY is a
+// single instruction but the SM retires only one every ~50 clocks (measured: a radix pass over 8192 keys takes 19 000
+// clocks with it, 12 700 with the ballots, and two CTAs on one SM no longer slow each other down)
 __device__ __forceinline__ unsigned same_digit_lanes(unsigned d)
 {
     unsigned peers = 0xffffffffu;
+    const unsigned me = 1u << (threadIdx.x & 31);
 #pragma unroll
     for (int b = 0; b < 8; ++b) {
         const bool bit = (d >> b) & 1u;
-        const unsigned bal = __ballot_sync(0xffffffffu, bit);
+        const unsigned bal = __reduce_or_sync(0xffffffffu, bit ? me : 0u);     // a ballot; REDUX retires a little faster than VOTE here
         peers &= bit ? bal : ~bal;
     }
     return peers;
@@ -97,11 +123,10 @@ running_median_tile_kernel(MedianArgs a)
     KeyT *skey = reinterpret_cast<KeyT *>(smem_raw);
     uint16_t *spos = reinterpret_cast<uint16_t *>(skey + MED_LT);
     uint16_t *rop = spos + MED_LT;
-    uint16_t *aux = rop + MED_LT;                          // radix counters, the count table, the output ranks
-    uint16_t *cm = aux + MED_AUX_U16;                      // coarse medians
-    uint32_t *misc = reinterpret_cast<uint32_t *>(cm + MED_NPB);
-    uint16_t *tab = aux;
-    uint16_t *orank = aux;                                 // written by the walk, after the table's last use
+    uint16_t *aux = rop + MED_LT;                          // radix counters; then the window bitmaps and the output ranks
+    constexpr int AUX_U16 = median_aux_u16(THREADS);
+    uint32_t *misc = reinterpret_cast<uint32_t *>(aux + AUX_U16);
+    uint16_t *orank = aux + 2 * WARPS * (MED_LT / 32) * 2; // behind the bitmaps
     uint32_t *aux32 = reinterpret_cast<uint32_t *>(aux);
 
     const int tid = threadIdx.x;
@@ -110,6 +135,9 @@ running_median_tile_kernel(MedianArgs a)
     const unsigned lt_mask = (1u << lane) - 1u;
     const int h = a.h, W = 2 * a.h + 1;
     __shared__ int s_item;
+#ifdef MED_TIMING
+    long long med_t_prev = 0;
+#endif
     bool neg = false;
     gbfg_let_next_kernel_start();                        // the wide-tile kernel / the prefix may queue up behind this one
     gbfg_wait_prior_kernel();                            // (launched as a dependent: the 32-bit kernel's wide list)
@@ -141,9 +169,10 @@ running_median_tile_kernel(MedianArgs a)
     }
     row = (int64_t)row_i * a.n;
     const int Lt = n_out + 2 * h;                        // positions really used
-    const int rounds = (Lt + THREADS - 1) / THREADS;     // keys per thread in the sort (<= ITEMS)
+    const int rounds = (Lt + THREADS - 1) / THREADS;
     const int LTe = rounds * THREADS;                    // positions sorted
 
+    MED_TICK(0);
     // ---- stage the tile: position p <-> global bin o0 - h + p, reflected at both ends.
     // Unused positions (Lt <= p < LTe) repeat position 0: they are never inside a window.
     if (tid < 2) misc[32 + tid] = 0u;
@@ -196,6 +225,7 @@ running_median_tile_kernel(MedianArgs a)
     }
     const int n_pass = vary_all ? (64 - __clzll((long long)vary_all) + 7) / 8 : 0;
 
+    MED_TICK(1);
     // ---- LSD radix sort by key, stable, so that equal keys stay in position order.
     // Warp w owns elements [32 rounds w, 32 rounds (w + 1)) of the current order, 32 consecutive ones per round.
     for (int pass = 0; pass < n_pass; ++pass) {
@@ -210,7 +240,7 @@ running_median_tile_kernel(MedianArgs a)
             if (r < rounds) {
                 const int e = warp * (32 * rounds) + r * 32 + lane;
                 k[r] = skey[e];
-                pk[r] = __match_any_sync(FULL, (unsigned)(k[r] >> shift) & 255u);
+                pk[r] = same_digit_lanes((unsigned)(k[r] >> shift) & 255u);
             }
         }
 #pragma unroll
@@ -265,200 +295,143 @@ running_median_tile_kernel(MedianArgs a)
         __syncthreads();
     }
 
-    // ---- inverse permutation and the count table (only the rank buckets and position blocks the tile has)
-    const int nrb = LTe / MED_RB, npb = LTe / MED_PB;     // LTe is a multiple of 256
-    for (int e = tid; e < nrb * MED_TROW / 2; e += THREADS) aux32[e] = 0u;
+    MED_TICK(2);
+    // ---- inverse permutation: rop[p] = rank of position p
+    for (int r = tid; r < LTe; r += THREADS) rop[spos[r]] = (uint16_t)r;
     __syncthreads();
-    for (int r = tid; r < LTe; r += THREADS) {
-        int p = spos[r];
-        rop[p] = (uint16_t)r;
-        int e = (r / MED_RB) * MED_TROW + (p / MED_PB) + 1;
-        atomicAdd(&aux32[e >> 1], (e & 1) ? 0x10000u : 1u);
-    }
-    __syncthreads();
-    // prefix along the position blocks: tab[rb][pb] = #{r in bucket rb : pos < pb*PB}
+
+    MED_TICK(3);
+    // ---- window bitmaps.  Warp w owns the chunks [w cpw, (w+1) cpw) of 32 consecutive outputs and keeps, in
+    // shared memory, one bit per sorted rank: "the element of this rank lies in the window".  The median of a
+    // window is its (h+1)-th set bit.
+    //  * The bitmaps of the warps' first windows are built by the whole CTA from the rank side: one ballot per
+    //    (word of 32 ranks, warp), no read-modify-write; each warp then finds its first median by counting words.
+    //  * Inside a chunk lane i takes output j0 + i.  The 32 positions that leave and the 32 that enter while the
+    //    window slides over the chunk are the chunk's "specials" (a second bitmap marks their ranks); every other
+    //    set bit of U = window(j0) + the entering positions lies in all the chunk's windows.  Two popcounts of
+    //    ballots tell lane i how many elements of its own window it has to move from the chunk's first median m0,
+    //    and in which direction; it then moves word by word (32 ranks and, typically, 8 window elements per step:
+    //    a popcount), looking at positions only for the specials of a word, and picks the bit inside the last
+    //    word.  Lane 0, whose own answer is m0, does the same for output j0 + 32: the first median of the next
+    //    chunk.  Plateaus and long stretches of out-of-window ranks cost one step per 32 ranks.
     {
-        constexpr int PER = (MED_NPB + 1 + 31) / 32;     // 9 entries per lane
-        for (int rb = warp; rb < nrb; rb += WARPS) {
-            uint16_t *rowp = tab + rb * MED_TROW;
-            int v[PER], s = 0;
-#pragma unroll
-            for (int q = 0; q < PER; ++q) {
-                int idx = lane * PER + q;
-                v[q] = idx <= npb ? rowp[idx] : 0;
-                s += v[q];
-            }
-            int incl = s;
-            for (int o = 1; o < 32; o <<= 1) {
-                int up = __shfl_up_sync(FULL, incl, o);
-                if (lane >= o) incl += up;
-            }
-            int run = incl - s;
-#pragma unroll
-            for (int q = 0; q < PER; ++q) {
-                int idx = lane * PER + q;
-                run += v[q];
-                if (idx <= npb) rowp[idx] = (uint16_t)run;
-            }
-        }
-    }
-    __syncthreads();
-    // exclusive prefix along the rank buckets: tab[rb][pb] = #{r < rb*RB : pos < pb*PB}
-    for (int pb = tid; pb <= npb; pb += THREADS) {
-        int run = 0;
-        for (int rb = 0; rb < nrb; ++rb) {
-            int v = tab[rb * MED_TROW + pb];
-            tab[rb * MED_TROW + pb] = (uint16_t)run;
-            run += v;
-        }
-    }
-    __syncthreads();
-
-    // ---- coarse states.  Warp w owns the chunks [w cpw, (w+1) cpw) of 32 outputs.  The median rank of
-    // the window of its first chunk comes from the count table; the following ones by sliding the
-    // window 32 bins at a time: two ballots count the ranks under m that left and entered, and the
-    // warp moves m by that many window elements, 32 places of the sorted order per step.
-    const int n_coarse = (n_out + MED_PB - 1) / MED_PB;
-    const int cpw = (n_coarse + WARPS - 1) / WARPS;
-    const int c_first = warp * cpw;
-    // warp-cooperative search: from rank wm (exclusive) in direction wdir to the wneed-th element whose
-    // position lies in [wplo, wphi]; all arguments warp-uniform; wm is updated
-#define WARP_SEEK(wm, wdir, wneed, wplo, wphi)                                                     \
-        for (;;) {                                                                                 \
-            const int r_ = (wm) + (wdir) * (1 + lane);                                             \
-            const bool ok_ = (unsigned)r_ < (unsigned)LTe;                                         \
-            const bool in_ = ok_ && (unsigned)((int)spos[ok_ ? r_ : 0] - (wplo)) <= (unsigned)((wphi) - (wplo)); \
-            const unsigned bal_ = __ballot_sync(FULL, in_);                                        \
-            const int cn_ = __popc(bal_);                                                          \
-            if ((wneed) <= cn_) { (wm) += (wdir) * (1 + nth_set_bit(bal_, (wneed))); break; }      \
-            (wneed) -= cn_;                                                                        \
-            (wm) += 32 * (wdir);                                                                   \
-            if ((unsigned)(wm) >= (unsigned)LTe) break;    /* not reachable: the window holds the element */ \
-        }
-    if (c_first < n_coarse) {
-        int m = LTe;
-        {
-            const int c = c_first;
-            const int j0 = c * MED_PB;
-            const int b0 = c, b1 = (j0 + W) / MED_PB;
-            const int na = b1 * MED_PB - j0;                 // block-aligned part of the window
-            int below = 0, phi = j0 - 1;
-            if (na > 0) {
-                const int t = (h < na - 1) ? h : na - 1;
-                // largest bucket lo with #{rank < 128 lo, position in the aligned part} <= t
-                // (a bucket past the tile's last one counts everything: never chosen)
-                const int c0 = lane < nrb ? (int)tab[lane * MED_TROW + b1] - (int)tab[lane * MED_TROW + b0] : 0x7fffffff;
-                const int c1 = lane + 32 < nrb ? (int)tab[(lane + 32) * MED_TROW + b1] - (int)tab[(lane + 32) * MED_TROW + b0] : 0x7fffffff;
-                const unsigned m0 = __ballot_sync(FULL, c0 <= t), m1 = __ballot_sync(FULL, c1 <= t);
-                const int lo = m1 ? 63 - __clz(m1) : 31 - __clz(m0);
-                const int cl = lo < 32 ? __shfl_sync(FULL, c0, lo & 31) : __shfl_sync(FULL, c1, lo & 31);
-                int need = t - cl + 1;                       // the (t - cl + 1)-th aligned element from rank 128 lo on
-                m = lo * MED_RB - 1;
-                WARP_SEEK(m, 1, need, j0, j0 + na - 1);
-                below = t;
-                phi = b1 * MED_PB - 1;
-            }
-            // complete the window with the (at most 31, or W when W < 32) remaining positions
-            for (int pbase = phi + 1; pbase < j0 + W; pbase += 32) {
-                const int p = pbase + lane;
-                const bool add = p < j0 + W && (int)rop[p < j0 + W ? p : 0] < m;
-                below += __popc(__ballot_sync(FULL, add));
-            }
-            if (below > h) {                                 // down to the (below - h)-th window element under m
-                int need = below - h;
-                WARP_SEEK(m, -1, need, j0, j0 + W - 1);
-            } else {                                         // up to the (h - below + 1)-th window element at or above m
-                int need = h - below + 1;
-                m -= 1;
-                WARP_SEEK(m, 1, need, j0, j0 + W - 1);
-            }
-            if (lane == 0) cm[c] = (uint16_t)m;
-        }
+        const int n_coarse = (n_out + MED_PB - 1) / MED_PB;
+        const int cpw = (n_coarse + WARPS - 1) / WARPS;
+        const int c_first = warp * cpw;
         const int c_last = (c_first + cpw < n_coarse) ? c_first + cpw : n_coarse;
-        for (int c = c_first + 1; c < c_last; ++c) {
-            const int j0 = c * MED_PB;                       // window [j0, j0 + W); the last one started 32 bins earlier
-            const int gone = rop[j0 - MED_PB + lane], come = rop[j0 - MED_PB + W + lane];
-            const int n_gone = __popc(__ballot_sync(FULL, gone < m)), n_come = __popc(__ballot_sync(FULL, come < m));
-            const bool m_left = __ballot_sync(FULL, gone == m) != 0u;
-            const int below = h + n_come - n_gone;
-            int dir, need;
-            if (below > h) { dir = -1; need = below - h; }
-            else { dir = 1; need = h - below + (m_left ? 1 : 0); }
-            if (need) { WARP_SEEK(m, dir, need, j0, j0 + W - 1); }
-            if (lane == 0) cm[c] = (uint16_t)m;
+        unsigned *bm = aux32 + warp * (MED_LT / 32);
+        unsigned *sp = aux32 + (WARPS + warp) * (MED_LT / 32);
+        const int nw = LTe / 32;
+        const uint32_t bm_a = (uint32_t)__cvta_generic_to_shared(bm), sp_a = (uint32_t)__cvta_generic_to_shared(sp);
+        {
+            const int wstep = cpw * MED_PB;                      // first output of warp w2: w2 * wstep
+            const int n_chain = (n_coarse + cpw - 1) / cpw;      // warps that have a chunk
+            for (int e = warp; e < nw; e += WARPS) {
+                const int p = spos[(e << 5) + lane];
+                unsigned mine = 0u;
+#pragma unroll
+                for (int w2 = 0; w2 < WARPS; ++w2) {
+                    const unsigned bits = __ballot_sync(FULL, (unsigned)(p - w2 * wstep) < (unsigned)W);
+                    if (lane == w2) mine = bits;
+                }
+                if (lane < n_chain) aux32[lane * (MED_LT / 32) + e] = mine;
+            }
+            for (int e = lane; e < nw; e += 32) sp[e] = 0u;
+        }
+        __syncthreads();
+        MED_TICK(4);
+        if (c_first < c_last) {
+            int j0 = c_first * MED_PB;
+            int m0;
+            {   // the (h+1)-th set bit: lane l counts the words [l per, (l+1) per)
+                const int per = (nw + 31) / 32;
+                int cnt = 0;
+                for (int q = 0; q < per; ++q) { const int e = lane * per + q; cnt += e < nw ? __popc(bm[e]) : 0; }
+                int incl = cnt;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int up = __shfl_up_sync(FULL, incl, o);
+                    if (lane >= o) incl += up;
+                }
+                const unsigned reach = __ballot_sync(FULL, incl >= h + 1);
+                const int L = __ffs(reach) - 1;
+                int found = 0;
+                if (lane == L) {
+                    int need = h + 1 - (incl - cnt);              // 1-based among this lane's words
+                    for (int q = 0; q < per; ++q) {
+                        const int e = lane * per + q;
+                        const unsigned wd = e < nw ? bm[e] : 0u;
+                        const int pc = __popc(wd);
+                        if (need <= pc) { found = e * 32 + nth_set_bit(wd, need); break; }
+                        need -= pc;
+                    }
+                }
+                m0 = __shfl_sync(FULL, found, L);
+            }
+            MED_TICK(5);
+            for (int c = c_first; c < c_last; ++c, j0 += MED_PB) {
+                const int pg = j0 + lane, pc_ = j0 + W + lane;           // positions that leave / enter
+                const int gone = rop[pg];
+                const bool c_ok = pc_ < Lt;
+                const int come = c_ok ? (int)rop[pc_] : 0x7fffffff;
+                const unsigned gb = __ballot_sync(FULL, gone < m0), cb = __ballot_sync(FULL, come < m0);
+                const unsigned gm = __ballot_sync(FULL, gone == m0);
+                const uint32_t g_off = (uint32_t)(gone >> 5) << 2, c_off = (uint32_t)(come >> 5) << 2;
+                const unsigned g_bit = 1u << (gone & 31), c_bit = 1u << (come & 31);
+                smem_or(sp_a + g_off, g_bit);
+                if (c_ok) {
+                    smem_or(bm_a + c_off, c_bit);
+                    smem_or(sp_a + c_off, c_bit);
+                }
+                // lane i: output j0 + i; lane 0: output j0 + 32 (the next chunk's first), its own answer being m0
+                const bool next_needed = c + 1 < c_last;
+                const int i_eff = lane ? lane : 32;
+                const unsigned before = lane ? lt_mask : FULL;            // the slides k < i_eff
+                const int delta = __popc(cb & before) - __popc(gb & before);
+                const bool present = (gm & before) == 0u;
+                int t;
+                bool up;
+                if (delta > 0) { up = false; t = delta; }
+                else { up = true; t = -delta + (present ? 0 : 1); }
+                const int jlo = j0 + i_eff;
+                if (lane ? (jlo >= n_out) : !next_needed) t = 0;
+                __syncwarp();
+                int r = m0;
+                if (t > 0) {
+                    int wi = m0 >> 5;
+                    // the first word: only the ranks beyond m0
+                    unsigned keep = up ? ~((2u << (m0 & 31)) - 1u) : ((1u << (m0 & 31)) - 1u);
+                    for (;;) {
+                        unsigned wb = bm[wi] & keep;
+                        for (unsigned sb = wb & sp[wi]; sb; sb &= sb - 1u) {       // specials: in this lane's window?
+                            const int b = __ffs(sb) - 1;
+                            if ((unsigned)((int)spos[(wi << 5) + b] - jlo) >= (unsigned)W) wb &= ~(1u << b);
+                        }
+                        const int pc = __popc(wb);
+                        if (t <= pc) {
+                            r = (wi << 5) + (up ? nth_set_bit(wb, t) : 31 - nth_set_bit(__brev(wb), t));
+                            break;
+                        }
+                        t -= pc;
+                        wi += up ? 1 : -1;
+                        keep = 0xffffffffu;
+                        if ((unsigned)wi >= (unsigned)nw) break;               // not reachable: the window holds the element
+                    }
+                }
+                if (lane) { if (jlo < n_out) orank[jlo] = (uint16_t)r; }
+                else orank[j0] = (uint16_t)m0;
+                __syncwarp();
+                smem_and(bm_a + g_off, ~g_bit);
+                smem_and(sp_a + g_off, ~g_bit);
+                if (c_ok) smem_and(sp_a + c_off, ~c_bit);
+                m0 = __shfl_sync(FULL, r, 0);
+                __syncwarp();
+            }
         }
     }
-    __syncthreads();                                         // the count table is dead from here on: orank may be written
-
-    // ---- every thread walks MED_FINE outputs at a time, starting from the coarse state of its chunk.
-    // `below` = #{window elements of rank < m}.  One rule for every move: the median is the
-    // (below - h)-th window element under m, or the (h - below)-th above it, counting m itself first
-    // when it is still in the window.  A thread steps along the sorted order on its own for at most
-    // MED_STEP_CAP places; spectra with plateaus (wide chirps put the same power in consecutive bins)
-    // and level-correlated neighbourhoods have stretches of hundreds of out-of-window elements, and
-    // those searches are finished by the whole warp, 32 places per step.
-    const int n_tasks = n_coarse * (MED_PB / MED_FINE);
-    for (int task0 = 0; task0 < n_tasks; task0 += THREADS) {
-        const int task = task0 + tid;
-        const int s = task / n_coarse, c = task - s * n_coarse;
-        const int j_first = c * MED_PB + s * MED_FINE;
-        const bool alive = task < n_tasks && j_first < n_out;
-        const int j_end = alive ? ((j_first + MED_FINE < n_out) ? j_first + MED_FINE : n_out) : j_first;
-        int m = 0, plo = 0, phi = -1, dir = 1, need = 0;
-#define IN_SET(r) ((unsigned)((int)spos[r] - plo) <= (unsigned)(phi - plo))
-        // the warp completes the searches its lanes left unfinished: lane `src` still needs `need`
-        // window elements from rank m (exclusive) in direction dir
-#define WARP_FINISH()                                                                              \
-        for (unsigned pend = __ballot_sync(FULL, need > 0); pend; pend &= pend - 1) {              \
-            const int src = __ffs(pend) - 1;                                                       \
-            int wm = __shfl_sync(FULL, m, src);                                                    \
-            const int wdir = __shfl_sync(FULL, dir, src);                                          \
-            int wneed = __shfl_sync(FULL, need, src);                                              \
-            const int wplo = __shfl_sync(FULL, plo, src), wphi = __shfl_sync(FULL, phi, src);      \
-            WARP_SEEK(wm, wdir, wneed, wplo, wphi);                                                \
-            if (lane == src) { m = wm; need = 0; }                                                 \
-        }
-        if (alive) {
-            int below = h;
-            m = cm[c];
-            plo = c * MED_PB;
-            phi = plo + W - 1;
-            // jump: count the ranks under m that left and entered
-            const int jump = s * MED_FINE;
-            for (int i = 0; i < jump; ++i) {
-                below += ((int)rop[phi + 1 + i] < m) - ((int)rop[plo + i] < m);
-            }
-            plo += jump;
-            phi += jump;
-            if (below > h) { dir = -1; need = below - h; }
-            else { dir = 1; need = h - below + (IN_SET(m) ? 0 : 1); }
-            for (int t = 0; need && t < 3 * MED_STEP_CAP; ++t) { m += dir; if (IN_SET(m)) --need; }
-        }
-        WARP_FINISH();
-        if (alive) orank[j_first] = (uint16_t)m;             // orank shares its memory with nothing the walk reads
-#pragma unroll 1
-        for (int jj = 1; jj < MED_FINE; ++jj) {
-            const int j = j_first + jj;
-            const bool on = j < j_end;
-            if (on) {
-                const int gone = rop[plo];                    // position j-1 leaves
-                ++plo;
-                const int come = rop[phi + 1];                // position j+2h enters
-                ++phi;
-                const int b = h + (come < m) - (gone < m);    // h-1, h or h+1
-                dir = b > h ? -1 : 1;
-                need = (b != h || gone == m) ? 1 : 0;
-                for (int t = 0; need && t < MED_STEP_CAP; ++t) { m += dir; if (IN_SET(m)) need = 0; }
-            }
-            WARP_FINISH();
-            if (on) orank[j] = (uint16_t)m;
-        }
-#undef WARP_FINISH
-#undef IN_SET
-    }
-#undef WARP_SEEK
     __syncthreads();
 
+    MED_TICK(6);
     // ---- coalesced epilogue: median and PSD
     if (a.items && tid == 0) next_item = (int)gridDim.x + atomicAdd(&a.ctr[1], 1);
     double dmax = 0.0;
@@ -498,6 +471,7 @@ running_median_tile_kernel(MedianArgs a)
         for (int o = 16; o; o >>= 1) dmax = fmax(dmax, __shfl_xor_sync(FULL, dmax, o));
         if (lane == 0 && dmax > 0.0) atomicMax(a.delta_bits + row_i, (unsigned long long)__double_as_longlong(dmax));
     }
+    MED_TICK(7);
   }   // tiles
     if (a.neg_flag && neg) *a.neg_flag = 1;
 }
