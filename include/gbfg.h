@@ -243,7 +243,10 @@ int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *of
 
 /* The same path with HOST buffers: the library allocates device memory, copies host_s_instr in,
  * runs gbfg_simulate on its own stream, and copies the PSD ([n_cat][n_bins] binary64) and the
- * resolved flags ([N] uint8, may be NULL) back.  Host pointers should be pinned for full speed.
+ * resolved flags ([N] uint8, may be NULL) back.  host_s_instr == NULL: the curve of gbfg_instrument_noise
+ * (a function of the grid alone) is made on the device instead of being uploaded.  Host pointers should be
+ * pinned for full speed; with a pinned host_psd the PSD leaves for the host while the loop still runs (blocks
+ * that change afterwards are stored again: every bin arrives with its final value).
  * Synchronous.  The device memory it allocates is cached per host thread (gbfg_release_cached). */
 int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
                        uint64_t seed, const uint32_t *cat_ids, const double *host_s_instr, const gbfg_iter_params *params,

@@ -196,10 +196,10 @@ static cudaEvent_t readback_event()
 }
 
 // side stream on which the plan of the next pass runs next to the scan of the subtraction (one per host thread)
-struct SideStream { cudaStream_t s; cudaEvent_t ev_plan, ev_aux, ev_noise; };
+struct SideStream { cudaStream_t s; cudaEvent_t ev_plan, ev_aux, ev_noise; cudaStream_t copy; cudaEvent_t ev_copy; };
 static SideStream &side_stream_slot()
 {
-    static thread_local SideStream ss = {nullptr, nullptr, nullptr, nullptr};
+    static thread_local SideStream ss = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     return ss;
 }
 static SideStream *side_stream_if_any() { return side_stream_slot().s ? &side_stream_slot() : nullptr; }
@@ -210,13 +210,57 @@ static SideStream *side_stream()
         if (cudaStreamCreateWithFlags(&ss.s, cudaStreamNonBlocking) != cudaSuccess ||
             cudaEventCreateWithFlags(&ss.ev_plan, cudaEventDisableTiming) != cudaSuccess ||
             cudaEventCreateWithFlags(&ss.ev_aux, cudaEventDisableTiming) != cudaSuccess ||
-            cudaEventCreateWithFlags(&ss.ev_noise, cudaEventDisableTiming) != cudaSuccess) {
+            cudaEventCreateWithFlags(&ss.ev_noise, cudaEventDisableTiming) != cudaSuccess ||
+            cudaStreamCreateWithFlags(&ss.copy, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&ss.ev_copy, cudaEventDisableTiming) != cudaSuccess) {
             (void)cudaGetLastError();
             ss.s = nullptr;
             return nullptr;
         }
     }
     return &ss;
+}
+
+// gbfg_simulate_host: the PSD starts its way to the (pinned) host buffer while the loop still runs.  Once a pass
+// recomputes less than a tenth of the outputs, the PSD as it stands goes out on a copy stream; a block of 2^dblk_log2 bins
+// that a later subtraction makes dirty carries a later stamp (deposit.cu), and exactly those blocks are stored again at
+// the end by psd_patch_kernel, straight into the mapped host buffer.  Never changes a result: every bin of the host
+// buffer is written last with its final value.
+struct EarlyOut {
+    double *host_psd;        // destination of the copy (pinned host memory) ...
+    double *host_psd_dev;    // ... and the address kernels store to it through
+    size_t bytes;
+    cudaStream_t copy_stream;   // the copy and every patch run on this stream, in this order
+    int started_after;       // iteration after which the PSD went out (-1: it did not)
+    int patched_upto;        // blocks stamped up to this iteration have been stored again since
+};
+constexpr int EARLY_PATCH_EVERY = 4;       // iterations between two patches while the loop runs
+
+// blocks with after < stamp <= upto, straight into the host buffer.  Runs next to the loop's kernels: a block that is
+// stamped again meanwhile (whatever stamp this kernel then sees) is covered by a later patch, since stamps only grow.
+__global__ void __launch_bounds__(256)
+psd_patch_kernel(const double *__restrict__ psd, double *__restrict__ host_psd, const int *__restrict__ blk_stamp,
+                 int n_dblk, int dblk_log2, int64_t n_bins, int after, int upto)
+{
+    const int64_t row = blockIdx.y;
+    for (int b = blockIdx.x; b < n_dblk; b += gridDim.x) {
+        const int stamp = ((const volatile int *)blk_stamp)[row * n_dblk + b];
+        if (stamp <= after || stamp > upto) continue;
+        const int64_t k0 = (int64_t)b << dblk_log2;
+        int64_t k1 = k0 + ((int64_t)1 << dblk_log2);
+        if (k1 > n_bins) k1 = n_bins;
+        for (int64_t k = k0 + threadIdx.x; k < k1; k += blockDim.x) host_psd[row * n_bins + k] = psd[row * n_bins + k];
+    }
+}
+
+static int launch_psd_patch(const EarlyOut &eo, const double *dev_psd, const int *blk_stamp, int n_dblk, int dblk_log2,
+                            int64_t n_bins, int n_cat, int after, int upto)
+{
+    const int gx = n_dblk < 4 * sm_count() ? n_dblk : 4 * sm_count();
+    psd_patch_kernel<<<dim3((unsigned)gx, (unsigned)n_cat), 256, 0, eo.copy_stream>>>(dev_psd, eo.host_psd_dev, blk_stamp, n_dblk,
+                                                                                       dblk_log2, n_bins, after, upto);
+    GBFG_LAUNCH_CHECK("psd_patch_kernel");
+    return GBFG_OK;
 }
 
 // Everything above that is kept per host thread (stream, events, device arena) belongs to the device that was current
@@ -233,6 +277,8 @@ static void release_thread_resources()
         cudaEventDestroy(side->ev_plan);
         cudaEventDestroy(side->ev_aux);
         cudaEventDestroy(side->ev_noise);
+        if (side->copy) { cudaStreamSynchronize(side->copy); cudaStreamDestroy(side->copy); side->copy = nullptr; }
+        if (side->ev_copy) { cudaEventDestroy(side->ev_copy); side->ev_copy = nullptr; }
         cudaStreamDestroy(side->s);
         side->s = nullptr;
     }
@@ -401,7 +447,7 @@ static int loop_body(const gbfg_grid *grid, const double *dev_A, const double *d
                      int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
                      uint8_t *dev_resolved, gbfg_iter_result *host_results,
                      void *workspace, size_t workspace_bytes, void *stream, bool prepared,
-                     cudaEvent_t records_ready)
+                     cudaEvent_t records_ready, EarlyOut *eo = nullptr)
 {
     int rc = loop_validate(grid, params);
     if (rc) return rc;
@@ -461,6 +507,7 @@ static int loop_body(const gbfg_grid *grid, const double *dev_A, const double *d
     cudaEvent_t ev_read = readback_event();
     if (!ev_read) return set_cuda_error(cudaErrorMemoryAllocation, "cudaEventCreate");
     int n_done = 0;
+    int64_t med_outputs_seen = 0;
     for (int it = 0; it < params->max_iter && n_done < n_cat; ++it) {
         // what the last subtraction made dirty (everything, the first time): work list + cum
         if (plan_queued) {
@@ -536,6 +583,26 @@ static int loop_body(const gbfg_grid *grid, const double *dev_A, const double *d
         }
         n_cand = host[i_cand];
         const int64_t total = host[0];
+        {   // outputs the estimator recomputed in this pass (the plan accumulates them, loop.cu's counter layout)
+            int64_t outs = 0;
+            for (int c = 0; c < n_cat; ++c) outs += host[i_med + c];
+            const int64_t last_pass = outs - med_outputs_seen;
+            med_outputs_seen = outs;
+            if (eo && incremental && !use_mean) {
+                if (eo->started_after < 0) {
+                    if (it >= 1 && last_pass * 10 < (int64_t)n_cat * nb) {
+                        GBFG_CUDA(cudaMemcpyAsync(eo->host_psd, dev_psd, eo->bytes, cudaMemcpyDeviceToHost, eo->copy_stream));
+                        eo->started_after = eo->patched_upto = it;
+                    }
+                } else if (it - eo->patched_upto >= EARLY_PATCH_EVERY) {
+                    // the estimator passes up to `it` are done: blocks stamped in (patched_upto, it] hold what they will
+                    // keep unless a later subtraction stamps them again
+                    rc = launch_psd_patch(*eo, dev_psd, w.blk_stamp, w.plan.n_dblk, w.plan.dblk_log2, nb, n_cat, eo->patched_upto, it);
+                    if (rc) return rc;
+                    eo->patched_upto = it;
+                }
+            }
+        }
         for (int c = 0; c < n_cat; ++c) {
             gbfg_iter_result &r = host_results[c];
             if (r.n_candidates == 0) r.n_candidates = n_cat == 1 ? host[i_cand] : host[i_cand + 1 + c];
@@ -621,7 +688,7 @@ static int simulate_body(const gbfg_grid *grid, const gbfg_pop *pops, const int6
                          double *dev_A, double *dev_f, double *dev_fdot,
                          int64_t *dev_total, int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
                          uint8_t *dev_resolved, int64_t *dev_err_count, gbfg_iter_result *host_results,
-                         void *workspace, size_t workspace_bytes, void *stream)
+                         void *workspace, size_t workspace_bytes, void *stream, EarlyOut *eo = nullptr)
 {
     int rc = loop_validate(grid, params);
     if (rc) return rc;
@@ -667,7 +734,7 @@ static int simulate_body(const gbfg_grid *grid, const gbfg_pop *pops, const int6
     GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_noise, 0));  // the first estimator pass reads S_instr
     // the loop waits for the records (side->ev_aux) after its first estimator pass, which overlaps their build
     return loop_body(grid, dev_A, dev_f, dev_fdot, offsets, n_cat, dev_s_instr, params, dev_spectrum, dev_median, dev_psd,
-                     dev_resolved, host_results, workspace, workspace_bytes, stream, true, side->ev_aux);
+                     dev_resolved, host_results, workspace, workspace_bytes, stream, true, side->ev_aux, eo);
 }
 
 extern "C" int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
@@ -690,7 +757,7 @@ extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, c
                                   uint64_t seed, const uint32_t *cat_ids, const double *host_s_instr, const gbfg_iter_params *params,
                                   double *host_psd, uint8_t *host_resolved, gbfg_iter_result *host_results)
 {
-    if (!valid_grid(grid) || !pops || !offsets || n_cat < 1 || !host_s_instr || !host_psd || !host_results)
+    if (!valid_grid(grid) || !pops || !offsets || n_cat < 1 || !host_psd || !host_results)
         return GBFG_ERR_INVALID_ARG;
     if (n_cat > GBFG_MAX_CAT) return GBFG_ERR_UNSUPPORTED;
     int rc = check_device();
@@ -729,20 +796,49 @@ extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, c
     // runs while this stream samples and deposits, and gbfg_simulate joins the two streams before the loop reads it
     SideStream *side = side_stream();
     if (!side) return set_cuda_error(cudaErrorMemoryAllocation, "side stream");
-    e = cudaMemcpyAsync(base + oI, host_s_instr, 8 * nb, cudaMemcpyHostToDevice, side->s);
-    if (e != cudaSuccess) rc = set_cuda_error(e, "cudaMemcpyAsync(s_instr)");
-    if (!rc)
-        rc = gbfg_simulate(grid, pops, offsets, n_cat, seed, cat_ids, (const double *)(base + oI), params,
-                           (double *)(base + oA), (double *)(base + oF), (double *)(base + oD), nullptr,
-                           (int64_t *)(base + oS), (int64_t *)(base + oM), (double *)(base + oP),
-                           (uint8_t *)(base + oR), nullptr, host_results, base + oW, ws_bytes, st);
+    if (host_s_instr) {
+        e = cudaMemcpyAsync(base + oI, host_s_instr, 8 * nb, cudaMemcpyHostToDevice, side->s);
+        if (e != cudaSuccess) rc = set_cuda_error(e, "cudaMemcpyAsync(s_instr)");
+    } else {
+        // no curve given: the library's own (gbfg_instrument_noise), a function of the grid alone, made on the device
+        rc = gbfg_instrument_noise(grid, (double *)(base + oI), side->s);
+    }
+    // the PSD may leave early (EarlyOut) when the caller's buffer is pinned host memory a kernel can store into
+    EarlyOut eo = {host_psd, nullptr, 8 * rows, side->copy, -1, -1};
+    {
+        cudaPointerAttributes at;
+        if (cudaPointerGetAttributes(&at, host_psd) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
+            eo.host_psd_dev = (double *)at.devicePointer;
+        (void)cudaGetLastError();
+    }
     if (!rc) {
-        e = cudaMemcpyAsync(host_psd, base + oP, 8 * rows, cudaMemcpyDeviceToHost, st);
-        if (e == cudaSuccess && host_resolved && n > 0)
-            e = cudaMemcpyAsync(host_resolved, base + oR, (size_t)n, cudaMemcpyDeviceToHost, st);
+        rc = loop_validate(grid, params);
+        if (!rc)
+            rc = drain_on_error(simulate_body(grid, pops, offsets, n_cat, seed, cat_ids, (const double *)(base + oI), params,
+                                              (double *)(base + oA), (double *)(base + oF), (double *)(base + oD), nullptr,
+                                              (int64_t *)(base + oS), (int64_t *)(base + oM), (double *)(base + oP),
+                                              (uint8_t *)(base + oR), nullptr, host_results, base + oW, ws_bytes, st,
+                                              eo.host_psd_dev ? &eo : nullptr), st);
+    }
+    if (!rc) {
+        // nothing of the loop is in flight any more (it synchronises its stream before it returns)
+        e = cudaSuccess;
+        if (host_resolved && n > 0) e = cudaMemcpyAsync(host_resolved, base + oR, (size_t)n, cudaMemcpyDeviceToHost, side->copy);
+        if (e == cudaSuccess) {
+            if (eo.started_after >= 0) {                        // what was stamped since the last patch
+                const Workspace w = carve(base + oW, grid->n_bins, n, n_cat);
+                if (launch_psd_patch(eo, (const double *)(base + oP), w.blk_stamp, w.plan.n_dblk, w.plan.dblk_log2, grid->n_bins,
+                                     n_cat, eo.patched_upto, 0x7fffffff) != GBFG_OK)
+                    e = cudaErrorUnknown;
+            } else {
+                e = cudaMemcpyAsync(host_psd, base + oP, 8 * rows, cudaMemcpyDeviceToHost, st);
+            }
+        }
         if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(side->copy);
         if (e != cudaSuccess) rc = set_cuda_error(e, "copy back");
     }
+    cudaStreamSynchronize(side->copy);
     cudaStreamSynchronize(st);
     return rc;
 }

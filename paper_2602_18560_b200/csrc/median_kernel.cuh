@@ -16,6 +16,9 @@ namespace gbfg {
 
 constexpr int MED_LT = 8192;                  // positions per tile, halos included
 constexpr int MED_PB = 32;                    // outputs per chunk (one per lane)
+#ifndef MED_MLP
+#define MED_MLP 4                             // global loads a thread keeps in flight while it stages a tile / writes it out
+#endif
 constexpr int MED_CROW = 256 + 2;             // radix counter row stride in u16 (one row per warp)
 constexpr uint64_t SIGN64 = 0x8000000000000000ull;
 
@@ -184,10 +187,10 @@ running_median_tile_kernel(MedianArgs a)
         if (g0 >= a.n) g0 = 2 * a.n - 1 - g0;
         key_ref = (uint64_t)a.x[row + g0] ^ SIGN64;
         uint64_t vary = 0;
-        for (int p0 = tid; p0 < LTe; p0 += 4 * THREADS) {    // four independent loads in flight per thread
-            uint64_t key[4];
+        for (int p0 = tid; p0 < LTe; p0 += MED_MLP * THREADS) {    // MED_MLP independent loads in flight per thread
+            uint64_t key[MED_MLP];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
+            for (int u = 0; u < MED_MLP; ++u) {
                 const int p = p0 + u * THREADS;
                 key[u] = key_ref;
                 if (p < Lt) {
@@ -198,7 +201,7 @@ running_median_tile_kernel(MedianArgs a)
                 }
             }
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
+            for (int u = 0; u < MED_MLP; ++u) {
                 const int p = p0 + u * THREADS;
                 if (p < LTe) {
                     vary |= key[u] ^ key_ref;
@@ -435,17 +438,17 @@ running_median_tile_kernel(MedianArgs a)
     // ---- coalesced epilogue: median and PSD
     if (a.items && tid == 0) next_item = (int)gridDim.x + atomicAdd(&a.ctr[1], 1);
     double dmax = 0.0;
-    for (int j0 = tid; j0 < n_out; j0 += 4 * THREADS) {
-        double si[4];
+    for (int j0 = tid; j0 < n_out; j0 += MED_MLP * THREADS) {
+        double si[MED_MLP];
         if (a.psd) {
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
+            for (int u = 0; u < MED_MLP; ++u) {
                 const int j = j0 + u * THREADS;
                 si[u] = j < n_out ? __ldg(a.s_instr + o0 + j) : 0.0;
             }
         }
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
+        for (int u = 0; u < MED_MLP; ++u) {
             const int j = j0 + u * THREADS;
             if (j < n_out) {
                 int64_t v;

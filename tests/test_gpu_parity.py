@@ -1214,3 +1214,40 @@ def test_shares_of_a_batch_match_the_batched_run(gb, orc, torch):
         ref = orc.simulate(w, cat=c)
         assert np.array_equal(whole[3][c].cpu().numpy(), ref["residual"])
         assert np.array_equal(bits(whole[5][c].cpu().numpy()), bits(ref["psd"]))
+
+
+@pytest.mark.parametrize("case", ["dense_long", "batch"])
+def test_simulate_host_with_pinned_buffers(gb, orc, torch, case):
+    """With a pinned PSD buffer gbfg_simulate_host sends the PSD on its way before the loop has ended and stores the
+    blocks that still change afterwards straight into the host buffer (loop.cu, EarlyOut): every bin must arrive with its
+    final value.  A long-tailed single catalog (about 28 iterations, most of them touching a few blocks) and a ragged
+    batch whose catalogs stop at different iterations; the buffer is poisoned before every call."""
+    if case == "dense_long":
+        w = wl.dense_case("long")
+    else:
+        w = wl.scaled(wl.config(4), n_cat=3)
+        w = wl.replace(w, t_obs=wl.YEAR_S, f_max=2e-3, window=1001,
+                       pops=[wl.replace(p, n_src=n, logA_offset=-22.3, slope=1.5) for p, n in zip(w.pops, (300_000, 60_001, 200_000))])
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    nb, n, nc = g.n_bins, w.n_src_total, w.n_cat
+    refs = [orc.simulate(w, cat=c) for c in range(nc)]
+    assert max(r["n_iter"] for r in refs) >= 8
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter)
+    h_noise = torch.from_numpy(refs[0]["s_instr"]).pin_memory()
+    h_psd = torch.empty((nc, nb), dtype=torch.float64).pin_memory()
+    h_res = torch.empty(n, dtype=torch.uint8).pin_memory()
+    off = w.offsets()
+    for rep in range(3):
+        h_psd.fill_(float("nan"))
+        h_res.fill_(7)
+        res = gb.simulate_host(g, w.pops, off, w.seed, h_noise.numpy(), params, h_psd.numpy(), h_res.numpy())
+        for c, ref in enumerate(refs):
+            assert np.array_equal(bits(h_psd[c].numpy()), bits(ref["psd"])), (rep, c)
+            assert np.array_equal(h_res.numpy()[int(off[c]):int(off[c + 1])], ref["resolved"]), (rep, c)
+            assert (res[c].n_iter, res[c].converged, res[c].n_resolved) == (ref["n_iter"], ref["converged"], ref["n_resolved"])
+    # no curve handed in: the library's own (gbfg_instrument_noise), made on the device
+    h_psd.fill_(float("nan"))
+    gb.simulate_host(g, w.pops, off, w.seed, None, params, h_psd.numpy(), h_res.numpy())
+    for c, ref in enumerate(refs):
+        assert np.array_equal(bits(h_psd[c].numpy()), bits(ref["psd"])), c
