@@ -42,25 +42,7 @@ deposit_kernel(GridDev g, CatTable ct, const double *__restrict__ A, const doubl
         const int64_t row = (int64_t)cat * g.n_bins;
         const int64_t v = sign >= 0 ? s.q : -s.q;
         if (v == 0) continue;
-        if (s.w_eff <= NARROW) {
-            for (int64_t k = s.k0; k < s.k0 + s.w_eff; ++k) atomic_add_i64(spectrum + row + k, v);
-        } else {
-            atomic_add_i64(diff + row + s.k0, v);
-            mk.scan_stamp[(int64_t)cat * mk.scan_tiles + s.k0 / SCAN_TILE] = mk.stamp;
-            if (s.k0 + s.w_eff < g.n_bins) {
-                atomic_add_i64(diff + row + s.k0 + s.w_eff, -v);
-                mk.scan_stamp[(int64_t)cat * mk.scan_tiles + (s.k0 + s.w_eff) / SCAN_TILE] = mk.stamp;
-            }
-            *wide_flag = mk.stamp;
-        }
-        if (mk.blk_stamp) {
-            // outputs k with |k - b| <= h see bin b (reflected ends included)
-            int64_t lo = s.k0 - mk.med_h, hi = s.k0 + s.w_eff - 1 + mk.med_h;
-            if (lo < 0) lo = 0;
-            if (hi > g.n_bins - 1) hi = g.n_bins - 1;
-            int *bs = mk.blk_stamp + (int64_t)cat * mk.n_dblk;
-            for (int64_t b = lo >> mk.dblk_log2; b <= (hi >> mk.dblk_log2); ++b) bs[b] = mk.stamp;
-        }
+        deposit_one(s, v, g.n_bins, cat, spectrum + row, diff + row, wide_flag, mk);
     }
     if (err_count) {
         // warp-aggregate the reject count

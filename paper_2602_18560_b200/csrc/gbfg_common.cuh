@@ -21,9 +21,10 @@ int check_device();                                     // GBFG_OK or GBFG_ERR_A
 void count_launch(int n = 1);
 int sm_count();
 // stage (i) with explicit catalog ids (sample.cu): cat_ids HOST [n_cat] or NULL (first_cat_id + c)
+struct SampleDeposit;       // != NULL: every source is also deposited by the kernel that draws it (gbfg_simulate)
 int sample_catalog_ids(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
                        uint32_t first_cat_id, const uint32_t *cat_ids, uint64_t seed,
-                       double *dev_A, double *dev_f, double *dev_fdot, void *stream);
+                       double *dev_A, double *dev_f, double *dev_fdot, void *stream, const SampleDeposit *dep = nullptr);
 
 // Kernel classes of the per-kernel timing helper (gbfg_profile_*; order = GBFG_K_* in gbfg.h).
 enum KernelId { K_SAMPLE = 0, K_NOISE, K_DEPOSIT, K_SCAN, K_MEDIAN, K_PSD, K_INV_BLOCKS, K_SNR, K_AUX, K_COUNT };
@@ -119,6 +120,11 @@ struct DirtyView {
     int dblk_log2;
 };
 
+// Range-update deposit (deposit.cu): sources of at most DEP_NARROW bins add q with L2 atomics, wider
+// ones write +q / -q into the difference array, scanned in tiles of DEP_SCAN_TILE bins.
+constexpr int DEP_NARROW = 4;
+constexpr int DEP_SCAN_TILE = 2048;
+
 // Stamps written by a deposit / subtraction (deposit.cu): which scan tiles hold range updates, and
 // which dirty blocks see a changed bin within h (blk_stamp NULL: not tracked).
 struct DepositMarks {
@@ -131,10 +137,15 @@ struct DepositMarks {
     int stamp;          // value written
 };
 
-// Range-update deposit (deposit.cu): sources of at most DEP_NARROW bins add q with L2 atomics, wider
-// ones write +q / -q into the difference array, scanned in tiles of DEP_SCAN_TILE bins.
-constexpr int DEP_NARROW = 4;
-constexpr int DEP_SCAN_TILE = 2048;
+
+// Stages (i) + (ii) in one kernel (sample.cu): where the drawn sources go
+struct SampleDeposit {
+    int64_t *spectrum;      // [n_cat][n_bins], accumulated into
+    int64_t *diff;          // [n_cat][n_bins]
+    int64_t *err_count;     // nullable
+    int *wide_flag;
+    DepositMarks mk;
+};
 
 // What stage (iv) needs to subtract the sources it selects on the spot (snr.cu; spectrum NULL: it only selects)
 struct SubtractView {
@@ -246,6 +257,32 @@ __device__ __forceinline__ SrcBins source_bins(const GridDev &g, double A, doubl
 __device__ __forceinline__ void atomic_add_i64(int64_t *addr, int64_t v)
 {
     atomicAdd(reinterpret_cast<unsigned long long *>(addr), (unsigned long long)v);
+}
+
+// One source into the spectrum of its row (stage ii; deposit.cu explains the two forms): v = +-q over
+// [k0, k0 + w_eff).  spectrum / diff point to the row.  Also stamps the scan tiles and, when tracked, the dirty blocks.
+__device__ __forceinline__ void deposit_one(const SrcBins &s, int64_t v, int64_t n_bins, int cat, int64_t *__restrict__ spectrum,
+                                            int64_t *__restrict__ diff, int *__restrict__ wide_flag, const DepositMarks &mk)
+{
+    if (s.w_eff <= DEP_NARROW) {
+        for (int64_t k = s.k0; k < s.k0 + s.w_eff; ++k) atomic_add_i64(spectrum + k, v);
+    } else {
+        atomic_add_i64(diff + s.k0, v);
+        mk.scan_stamp[(int64_t)cat * mk.scan_tiles + s.k0 / DEP_SCAN_TILE] = mk.stamp;
+        if (s.k0 + s.w_eff < n_bins) {
+            atomic_add_i64(diff + s.k0 + s.w_eff, -v);
+            mk.scan_stamp[(int64_t)cat * mk.scan_tiles + (s.k0 + s.w_eff) / DEP_SCAN_TILE] = mk.stamp;
+        }
+        *wide_flag = mk.stamp;
+    }
+    if (mk.blk_stamp) {
+        // outputs k with |k - b| <= h see bin b (reflected ends included)
+        int64_t lo = s.k0 - mk.med_h, hi = s.k0 + s.w_eff - 1 + mk.med_h;
+        if (lo < 0) lo = 0;
+        if (hi > n_bins - 1) hi = n_bins - 1;
+        int *bs = mk.blk_stamp + (int64_t)cat * mk.n_dblk;
+        for (int64_t b = lo >> mk.dblk_log2; b <= (hi >> mk.dblk_log2); ++b) bs[b] = mk.stamp;
+    }
 }
 
 }  // namespace gbfg

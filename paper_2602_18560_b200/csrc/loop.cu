@@ -713,22 +713,26 @@ static int simulate_body(const gbfg_grid *grid, const gbfg_pop *pops, const int6
     rc = loop_prefix_s_instr(g, dev_s_instr, preselect, w, side->s);
     if (rc) return rc;
     GBFG_CUDA(cudaEventRecord(side->ev_noise, side->s));    // S_instr is on the device by now (gbfg_simulate_host copies it on this stream)
-    rc = sample_catalog_ids(grid, pops, offsets, n_cat, 0u, cat_ids, seed, dev_A, dev_f, dev_fdot, stream);
-    if (rc) return rc;
     const size_t row_bytes = sizeof(int64_t) * (size_t)n_cat * (size_t)nb;
     GBFG_CUDA(cudaMemsetAsync(dev_spectrum, 0, row_bytes, st));
     if (n > 0) GBFG_CUDA(cudaMemsetAsync(dev_resolved, 0, (size_t)n, st));
     rc = loop_init_workspace(w, nb, n_cat, st);
     if (rc) return rc;
+    // stages (i) and (ii) in one kernel: every source is deposited by the thread that draws it (sample.cu).
+    // Its stamps (-1) never equal those of the loop's subtractions (1 .. max_iter).
+    {
+        const SampleDeposit dep = {dev_spectrum, w.diff, dev_err_count, w.wide_flag, plain_marks(w, nb, -1)};
+        rc = sample_catalog_ids(grid, pops, offsets, n_cat, 0u, cat_ids, seed, dev_A, dev_f, dev_fdot, stream, &dep);
+        if (rc) return rc;
+    }
     GBFG_CUDA(cudaEventRecord(side->ev_aux, st));
-    // side stream: the candidate records
+    // side stream: the candidate records (a pass over the catalog against S_instr alone)
     GBFG_CUDA(cudaStreamWaitEvent(side->s, side->ev_aux, 0));
     rc = loop_build_candidates(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, dev_s_instr, params->rho_th, preselect, w, side->s);
     if (rc) return rc;
     GBFG_CUDA(cudaEventRecord(side->ev_aux, side->s));
-    // this stream: the deposit.  Its stamps (-1) never equal those of the loop's subtractions (1 .. max_iter).
-    rc = launch_deposit(g, ct, dev_A, dev_f, dev_fdot, nullptr, nullptr, n, +1, dev_spectrum, dev_err_count,
-                        w.diff, w.tile_sums, w.wide_flag, plain_marks(w, nb, -1), st);
+    // this stream: the scan of the wide sources' range updates into the spectrum
+    rc = launch_scan(nb, n_cat, dev_spectrum, w.diff, w.tile_sums, w.wide_flag, plain_marks(w, nb, -1), st);
     if (rc) return rc;
     if (dev_total) GBFG_CUDA(cudaMemcpyAsync(dev_total, dev_spectrum, row_bytes, cudaMemcpyDeviceToDevice, st));
     GBFG_CUDA(cudaStreamWaitEvent(st, side->ev_noise, 0));  // the first estimator pass reads S_instr

@@ -235,18 +235,18 @@ plan_kernel(PlanArgs a)
     }
 }
 
-int median_tile_outputs(int window) { return MED_LT - (window - 1); }
+int median_tile_outputs(int window) { return MED_LT32 - (window - 1); }
 
 int median_tiles(int64_t n_bins, int window)
 {
-    int S = MED_LT - (window - 1);
+    int S = MED_LT32 - (window - 1);
     return (int)((n_bins + S - 1) / S);
 }
 
 // upper bound of the number of work items plan_kernel can emit for one row
 int median_max_items(int64_t n_bins)
 {
-    const int s_min = MED_LT - (GBFG_MAX_WINDOW - 1);
+    const int s_min = MED_LT32 - (GBFG_MAX_WINDOW - 1);
     const int s_small = s_min < PLAN_MIN_OUT ? s_min : PLAN_MIN_OUT;
     return dirty_blocks_per_row(n_bins) + 2 * (int)((n_bins + s_small - 1) / s_small) + 16;
 }
@@ -264,7 +264,7 @@ int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins,
     a.zero_ptr = zero_ptr; a.zero_n = zero_n; a.out_count = out_count;
     a.blk_stamp = blk_stamp; a.stamp = stamp; a.all_dirty = (all_dirty || !blk_stamp) ? 1 : 0;
     a.n_dblk = pl.n_dblk; a.dblk_log2 = pl.dblk_log2; a.n_bins = n_bins;
-    a.S = MED_LT - (window - 1);
+    a.S = MED_LT32 - (window - 1);
     a.wave = 2 * sm_count();                             // two CTAs of the 32-bit-key kernel per SM
     a.wide_ctr = pl.wide_ctr;
     a.cum = pl.cum; a.range = pl.range; a.items = pl.items; a.ctr = pl.ctr; a.max_items = pl.max_items;
@@ -293,7 +293,7 @@ int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins,
 // on the tiles the first one could not order (none for spectra in units of 2^-140 strain^2).
 int median_static_tiles(int64_t n_bins, int n_cat, int window, int *S_out)
 {
-    const int s_max = MED_LT - (window - 1);
+    const int s_max = MED_LT32 - (window - 1);
     const int slots = 2 * sm_count();
     int64_t tiles = (n_bins + s_max - 1) / s_max;
     if (tiles * n_cat > slots && n_cat == 1) tiles = (tiles + slots - 1) / slots * slots;   // whole waves of CTAs
@@ -316,15 +316,15 @@ int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64
     a.n = n_bins; a.h = window / 2;
     a.tiles = median_static_tiles(n_bins, n_cat, window, &a.S);
     a.norm = norm; a.scale = ldexp(1.0, scale_log2);
-    constexpr size_t smem32 = median_smem_bytes<uint32_t, 512>(), smem64 = median_smem_bytes<uint64_t, 1024>();
+    constexpr size_t smem32 = median_smem_bytes<uint32_t, 512, MED_LT32>(), smem64 = median_smem_bytes<uint64_t, 1024, MED_LT64>();
     static thread_local int attr_dev = -1;
     int dev = 0;
     GBFG_CUDA(cudaGetDevice(&dev));
     if (attr_dev != dev) {
-        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint32_t, 512, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem32));
-        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint64_t, 1024, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem64));
-        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint32_t, 512, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem32));
-        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint64_t, 1024, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem64));
+        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint32_t, 512, MED_LT32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem32));
+        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint64_t, 1024, MED_LT64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem64));
+        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint32_t, 512, MED_LT32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem32));
+        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint64_t, 1024, MED_LT64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem64));
         attr_dev = dev;
     }
     const int sms = sm_count();
@@ -332,15 +332,15 @@ int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64
     int64_t grid = plan ? 2 * sms : (int64_t)a.tiles * n_cat;
     if (grid > 2 * sms) grid = 2 * sms;
     LaunchTimer lt(K_MEDIAN, st);
-    if (delta_bits) running_median_tile_kernel<uint32_t, 512, true><<<(int)grid, 512, smem32, st>>>(a);
-    else running_median_tile_kernel<uint32_t, 512, false><<<(int)grid, 512, smem32, st>>>(a);
+    if (delta_bits) running_median_tile_kernel<uint32_t, 512, MED_LT32, true><<<(int)grid, 512, smem32, st>>>(a);
+    else running_median_tile_kernel<uint32_t, 512, MED_LT32, false><<<(int)grid, 512, smem32, st>>>(a);
     GBFG_LAUNCH_CHECK("running_median_tile_kernel<u32>");
     a.items = a.wide_items; a.ctr = a.wide_ctr;
     a.wide_items = nullptr; a.wide_ctr = nullptr;
     if (grid > sms) grid = sms;
     cudaError_t e = delta_bits
-        ? launch_dependent(running_median_tile_kernel<uint64_t, 1024, true>, dim3((unsigned)grid), dim3(1024), smem64, st, a)
-        : launch_dependent(running_median_tile_kernel<uint64_t, 1024, false>, dim3((unsigned)grid), dim3(1024), smem64, st, a);
+        ? launch_dependent(running_median_tile_kernel<uint64_t, 1024, MED_LT64, true>, dim3((unsigned)grid), dim3(1024), smem64, st, a)
+        : launch_dependent(running_median_tile_kernel<uint64_t, 1024, MED_LT64, false>, dim3((unsigned)grid), dim3(1024), smem64, st, a);
     if (e != cudaSuccess) return set_cuda_error(e, "running_median_tile_kernel<u64>");
     GBFG_LAUNCH_CHECK("running_median_tile_kernel<u64>");
     return GBFG_OK;

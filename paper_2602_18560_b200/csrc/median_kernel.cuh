@@ -14,7 +14,11 @@
 
 namespace gbfg {
 
-constexpr int MED_LT = 8192;                  // positions per tile, halos included
+// Positions per tile, halos included.  32-bit keys: 17 x 512; with W = 2001 a tile then holds up to 6704 outputs and a full
+// row of the 4-yr grid (3 774 349 bins) is 592 tiles = exactly two tiles for each of the 296 resident CTAs (8192 positions
+// made it 888 = three each, with a third more positions sorted per output).  64-bit keys: the next multiple of 1024.
+constexpr int MED_LT32 = 8704;
+constexpr int MED_LT64 = 9216;
 constexpr int MED_PB = 32;                    // outputs per chunk (one per lane)
 #ifndef MED_MLP
 #define MED_MLP 4                             // global loads a thread keeps in flight while it stages a tile / writes it out
@@ -24,21 +28,21 @@ constexpr uint64_t SIGN64 = 0x8000000000000000ull;
 
 // aux: the radix counters (one row per warp) during the sort; afterwards one window bitmap per warp (LT bits) and,
 // behind them, the output ranks
-__host__ __device__ constexpr int median_aux_u16(int threads)
+__host__ __device__ constexpr int median_aux_u16(int threads, int lt)
 {
     const int warps = threads / 32;
     const int sort_u16 = warps * MED_CROW;
-    const int walk_u16 = 2 * warps * (MED_LT / 32) * 2 + MED_LT;      // window and specials bitmaps, output ranks
+    const int walk_u16 = 2 * warps * (lt / 32) * 2;                   // window and specials bitmaps
     return sort_u16 > walk_u16 ? sort_u16 : walk_u16;
 }
 
-template <typename KeyT, int THREADS>
+template <typename KeyT, int THREADS, int LT>
 constexpr size_t median_smem_bytes()
 {
-    return sizeof(KeyT) * MED_LT                          // skey
-         + sizeof(uint16_t) * MED_LT                      // spos
-         + sizeof(uint16_t) * MED_LT                      // rop
-         + sizeof(uint16_t) * median_aux_u16(THREADS)     // radix counters, then the window bitmaps and the output ranks
+    return sizeof(KeyT) * LT                              // skey
+         + sizeof(uint16_t) * LT                          // spos
+         + sizeof(uint16_t) * LT                          // rop
+         + sizeof(uint16_t) * median_aux_u16(THREADS, LT) // radix counters, then the window bitmaps
          + sizeof(uint32_t) * 40;                         // scan partials, varying-bit mask
 }
 
@@ -112,24 +116,24 @@ __device__ __forceinline__ unsigned same_digit_lanes(unsigned d)
 
 // DELTA: also record the largest relative PSD change (the second stop rule, R13); a template parameter so
 // that the default kernel carries none of it
-template <typename KeyT, int THREADS, bool DELTA>
+template <typename KeyT, int THREADS, int LT, bool DELTA>
 __global__ void __launch_bounds__(THREADS, THREADS <= 512 ? 2 : 1)
 running_median_tile_kernel(MedianArgs a)
 {
     constexpr int WARPS = THREADS / 32;
-    constexpr int ITEMS = MED_LT / THREADS;               // keys per thread in the sort, at most
+    constexpr int ITEMS = (LT + THREADS - 1) / THREADS;   // keys per thread in the sort, at most
+    static_assert(LT % THREADS == 0 && LT % 32 == 0 && LT <= 65536, "tile size");
     constexpr int GROUPS = WARPS / 8;                      // counter scan: thread t owns digit t / GROUPS, 8 warps
     constexpr bool NARROW = sizeof(KeyT) == 4;
     static_assert(THREADS == 256 * GROUPS, "the counter scan maps one thread to one (digit, 8 warps) group");
 
     extern __shared__ __align__(16) unsigned char smem_raw[];
     KeyT *skey = reinterpret_cast<KeyT *>(smem_raw);
-    uint16_t *spos = reinterpret_cast<uint16_t *>(skey + MED_LT);
-    uint16_t *rop = spos + MED_LT;
-    uint16_t *aux = rop + MED_LT;                          // radix counters; then the window bitmaps and the output ranks
-    constexpr int AUX_U16 = median_aux_u16(THREADS);
+    uint16_t *spos = reinterpret_cast<uint16_t *>(skey + LT);
+    uint16_t *rop = spos + LT;
+    uint16_t *aux = rop + LT;                          // radix counters; then the window bitmaps and the output ranks
+    constexpr int AUX_U16 = median_aux_u16(THREADS, LT);
     uint32_t *misc = reinterpret_cast<uint32_t *>(aux + AUX_U16);
-    uint16_t *orank = aux + 2 * WARPS * (MED_LT / 32) * 2; // behind the bitmaps
     uint32_t *aux32 = reinterpret_cast<uint32_t *>(aux);
 
     const int tid = threadIdx.x;
@@ -304,6 +308,8 @@ running_median_tile_kernel(MedianArgs a)
     __syncthreads();
 
     MED_TICK(3);
+    if (a.items && tid == 0) next_item = (int)gridDim.x + atomicAdd(&a.ctr[1], 1);     // the next tile of this CTA
+    double dmax = 0.0;
     // ---- window bitmaps.  Warp w owns the chunks [w cpw, (w+1) cpw) of 32 consecutive outputs and keeps, in
     // shared memory, one bit per sorted rank: "the element of this rank lies in the window".  The median of a
     // window is its (h+1)-th set bit.
@@ -322,8 +328,8 @@ running_median_tile_kernel(MedianArgs a)
         const int cpw = (n_coarse + WARPS - 1) / WARPS;
         const int c_first = warp * cpw;
         const int c_last = (c_first + cpw < n_coarse) ? c_first + cpw : n_coarse;
-        unsigned *bm = aux32 + warp * (MED_LT / 32);
-        unsigned *sp = aux32 + (WARPS + warp) * (MED_LT / 32);
+        unsigned *bm = aux32 + warp * (LT / 32);
+        unsigned *sp = aux32 + (WARPS + warp) * (LT / 32);
         const int nw = LTe / 32;
         const uint32_t bm_a = (uint32_t)__cvta_generic_to_shared(bm), sp_a = (uint32_t)__cvta_generic_to_shared(sp);
         {
@@ -337,7 +343,7 @@ running_median_tile_kernel(MedianArgs a)
                     const unsigned bits = __ballot_sync(FULL, (unsigned)(p - w2 * wstep) < (unsigned)W);
                     if (lane == w2) mine = bits;
                 }
-                if (lane < n_chain) aux32[lane * (MED_LT / 32) + e] = mine;
+                if (lane < n_chain) aux32[lane * (LT / 32) + e] = mine;
             }
             for (int e = lane; e < nw; e += 32) sp[e] = 0u;
         }
@@ -374,6 +380,14 @@ running_median_tile_kernel(MedianArgs a)
             MED_TICK(5);
             for (int c = c_first; c < c_last; ++c, j0 += MED_PB) {
                 const int pg = j0 + lane, pc_ = j0 + W + lane;           // positions that leave / enter
+                // this lane's own output is j0 + lane: what its PSD needs is on its way while the median is found
+                const bool own = pg < n_out;
+                const int64_t g_own = o0 + pg;
+                double si = 0.0, pold = 0.0;
+                if (a.psd && own) {
+                    si = __ldg(a.s_instr + g_own);
+                    if (DELTA) pold = a.psd[row + g_own];
+                }
                 const int gone = rop[pg];
                 const bool c_ok = pc_ < Lt;
                 const int come = c_ok ? (int)rop[pc_] : 0x7fffffff;
@@ -421,8 +435,23 @@ running_median_tile_kernel(MedianArgs a)
                         if ((unsigned)wi >= (unsigned)nw) break;               // not reachable: the window holds the element
                     }
                 }
-                if (lane) { if (jlo < n_out) orank[jlo] = (uint16_t)r; }
-                else orank[j0] = (uint16_t)m0;
+                if (own) {                                   // median and PSD of output j0 + lane, 256 bytes per warp and array
+                    const KeyT kv = skey[lane ? r : m0];
+                    int64_t v;
+                    if (NARROW) v = (int64_t)(((key_ref & 0xffffffff00000000ull) | (uint64_t)kv) ^ SIGN64);
+                    else v = (int64_t)((uint64_t)kv ^ SIGN64);
+                    a.med[row + g_own] = v;
+                    neg |= v < 0;
+                    if (a.psd) {
+                        const double e = (double)v * a.scale;
+                        const double pnew = si + a.norm * e;
+                        if (DELTA) {                         // convergence in S_n: change against the last pass
+                            const double d = fabs(pnew - pold) / pold;
+                            if (d > dmax) dmax = d;
+                        }
+                        a.psd[row + g_own] = pnew;
+                    }
+                }
                 __syncwarp();
                 smem_and(bm_a + g_off, ~g_bit);
                 smem_and(sp_a + g_off, ~g_bit);
@@ -435,41 +464,6 @@ running_median_tile_kernel(MedianArgs a)
     __syncthreads();
 
     MED_TICK(6);
-    // ---- coalesced epilogue: median and PSD
-    if (a.items && tid == 0) next_item = (int)gridDim.x + atomicAdd(&a.ctr[1], 1);
-    double dmax = 0.0;
-    for (int j0 = tid; j0 < n_out; j0 += MED_MLP * THREADS) {
-        double si[MED_MLP];
-        if (a.psd) {
-#pragma unroll
-            for (int u = 0; u < MED_MLP; ++u) {
-                const int j = j0 + u * THREADS;
-                si[u] = j < n_out ? __ldg(a.s_instr + o0 + j) : 0.0;
-            }
-        }
-#pragma unroll
-        for (int u = 0; u < MED_MLP; ++u) {
-            const int j = j0 + u * THREADS;
-            if (j < n_out) {
-                int64_t v;
-                if (NARROW) v = (int64_t)(((key_ref & 0xffffffff00000000ull) | (uint64_t)skey[orank[j]]) ^ SIGN64);
-                else v = (int64_t)((uint64_t)skey[orank[j]] ^ SIGN64);
-                const int64_t g = o0 + j;
-                a.med[row + g] = v;
-                neg |= v < 0;
-                if (a.psd) {
-                    const double e = (double)v * a.scale;
-                    const double pnew = si[u] + a.norm * e;
-                    if (DELTA) {                             // convergence in S_n: change against the last pass
-                        const double pold = a.psd[row + g];
-                        const double d = fabs(pnew - pold) / pold;
-                        if (d > dmax) dmax = d;
-                    }
-                    a.psd[row + g] = pnew;
-                }
-            }
-        }
-    }
     if (DELTA) {                                         // non-negative binary64 values order like their bits
         for (int o = 16; o; o >>= 1) dmax = fmax(dmax, __shfl_xor_sync(FULL, dmax, o));
         if (lane == 0 && dmax > 0.0) atomicMax(a.delta_bits + row_i, (unsigned long long)__double_as_longlong(dmax));

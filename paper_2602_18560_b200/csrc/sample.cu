@@ -3,6 +3,8 @@
 // Follows DESIGN.md R1 (counter layout, draws) and §4 (elementary functions, operation by
 // operation).  The kernel is ALU-bound (two Philox blocks + 2 log + 3 exp10 + sincos + sqrt per
 // source against 24 bytes written); two sources per thread so that every store is 128 bits wide.
+#include <string.h>
+
 #include "gbfg_common.cuh"
 
 namespace gbfg {
@@ -206,9 +208,33 @@ __device__ __forceinline__ void draw_source(const PopDev &P, int64_t i, double &
 
 // Two sources per thread, 128-bit stores.  Arrays are offset to the catalog's first source; the
 // pair (2t, 2t+1) is aligned when that offset is even, else a scalar path handles the ends.
-__global__ void __launch_bounds__(256)
-sample_kernel(PopDev P, double *__restrict__ A, double *__restrict__ f, double *__restrict__ fdot, int head)
+// DEPOSIT: stage (ii) in the same kernel (gbfg_simulate).  The sampling is bound by its arithmetic (two Philox
+// blocks, 2 log, 3 exp10, sincos, sqrt per source) and leaves the memory pipes idle; the deposit is a handful of
+// 64-bit reductions per source that a kernel of its own spends its time waiting for.  Drawn and deposited from the
+// same registers, the reductions retire under the next source's arithmetic and the catalog is not read back.
+struct DepositDev {
+    GridDev g;
+    int64_t *spectrum, *diff;       // the catalog's row
+    int64_t *err_count;
+    int *wide_flag;
+    DepositMarks mk;
+    int cat;
+};
+
+template <bool DEPOSIT>
+__device__ __forceinline__ void deposit_drawn(const DepositDev &D, double a, double fr, double fd, int &rejected)
 {
+    if (!DEPOSIT) return;
+    const SrcBins s = source_bins(D.g, a, fr, fd);
+    if (s.status) { ++rejected; return; }
+    if (s.q != 0) deposit_one(s, s.q, D.g.n_bins, D.cat, D.spectrum, D.diff, D.wide_flag, D.mk);
+}
+
+template <bool DEPOSIT>
+__global__ void __launch_bounds__(256)
+sample_kernel(PopDev P, double *__restrict__ A, double *__restrict__ f, double *__restrict__ fdot, int head, DepositDev D)
+{
+    int rejected = 0;
     // sources [0, head) (0 or 1 of them) are done by thread 0 scalar so that the pairs are 16-byte aligned
     int64_t n_pairs = (P.n_src - head) / 2;
     int64_t tail = head + 2 * n_pairs;
@@ -222,10 +248,16 @@ sample_kernel(PopDev P, double *__restrict__ A, double *__restrict__ f, double *
         *reinterpret_cast<double2 *>(A + i) = make_double2(a0, a1);
         *reinterpret_cast<double2 *>(f + i) = make_double2(f0, f1);
         *reinterpret_cast<double2 *>(fdot + i) = make_double2(d0, d1);
+        deposit_drawn<DEPOSIT>(D, a0, f0, d0, rejected);
+        deposit_drawn<DEPOSIT>(D, a1, f1, d1, rejected);
     }
     if (t == 0) {
-        for (int64_t i = 0; i < head; ++i) draw_source(P, i, A[i], f[i], fdot[i]);
-        for (int64_t i = tail; i < P.n_src; ++i) draw_source(P, i, A[i], f[i], fdot[i]);
+        for (int64_t i = 0; i < head; ++i) { draw_source(P, i, A[i], f[i], fdot[i]); deposit_drawn<DEPOSIT>(D, A[i], f[i], fdot[i], rejected); }
+        for (int64_t i = tail; i < P.n_src; ++i) { draw_source(P, i, A[i], f[i], fdot[i]); deposit_drawn<DEPOSIT>(D, A[i], f[i], fdot[i], rejected); }
+    }
+    if (DEPOSIT && D.err_count) {
+        for (int o = 16; o; o >>= 1) rejected += __shfl_down_sync(0xffffffffu, rejected, o);
+        if ((threadIdx.x & 31) == 0 && rejected) atomic_add_i64(D.err_count, rejected);
     }
 }
 
@@ -549,7 +581,7 @@ extern "C" int gbfg_sample_catalog_paper(const gbfg_grid *grid, const gbfg_pop_p
 // cat_ids (HOST [n_cat], nullable): Philox counter word 3 of catalog c; NULL: first_cat_id + c
 int gbfg::sample_catalog_ids(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets,
                              int32_t n_cat, uint32_t first_cat_id, const uint32_t *cat_ids, uint64_t seed,
-                             double *dev_A, double *dev_f, double *dev_fdot, void *stream)
+                             double *dev_A, double *dev_f, double *dev_fdot, void *stream, const SampleDeposit *dep)
 {
     if (!grid || grid->struct_size != sizeof(gbfg_grid) || !pops || !offsets) return GBFG_ERR_INVALID_ARG;
     if (n_cat < 1) return GBFG_ERR_INVALID_ARG;
@@ -591,10 +623,22 @@ int gbfg::sample_catalog_ids(const gbfg_grid *grid, const gbfg_pop *pops, const 
         if (blocks < 1) blocks = 1;
         int64_t cap = (int64_t)sm_count() * 16;
         if (blocks > cap) blocks = cap;
+        DepositDev D;
+        memset(&D, 0, sizeof(D));
+        if (dep) {
+            D.g = make_grid_dev(grid);
+            D.spectrum = dep->spectrum + (int64_t)c * grid->n_bins;
+            D.diff = dep->diff + (int64_t)c * grid->n_bins;
+            D.err_count = dep->err_count; D.wide_flag = dep->wide_flag; D.mk = dep->mk; D.cat = c;
+        }
         {
             LaunchTimer lt(K_SAMPLE, (cudaStream_t)stream);
-            sample_kernel<<<(int)blocks, 256, 0, (cudaStream_t)stream>>>(
-                P, dev_A + offsets[c], dev_f + offsets[c], dev_fdot + offsets[c], head);
+            if (dep)
+                sample_kernel<true><<<(int)blocks, 256, 0, (cudaStream_t)stream>>>(
+                    P, dev_A + offsets[c], dev_f + offsets[c], dev_fdot + offsets[c], head, D);
+            else
+                sample_kernel<false><<<(int)blocks, 256, 0, (cudaStream_t)stream>>>(
+                    P, dev_A + offsets[c], dev_f + offsets[c], dev_fdot + offsets[c], head, D);
         }
         GBFG_LAUNCH_CHECK("sample_kernel");
     }
