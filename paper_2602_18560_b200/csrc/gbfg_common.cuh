@@ -145,6 +145,9 @@ struct SampleDeposit {
     int64_t *err_count;     // nullable
     int *wide_flag;
     DepositMarks mk;
+    int64_t piece;          // > 0: catalogs are drawn in pieces of at most this many sources ...
+    int (*after_piece)(void *ctx, int64_t i_begin, int64_t i_end);   // ... and this is called (host) after each launch
+    void *ctx;
 };
 
 // What stage (iv) needs to subtract the sources it selects on the spot (snr.cu; spectrum NULL: it only selects)

@@ -42,6 +42,11 @@ int launch_inv_prefix(const double *psd, int64_t n_bins, int n_cat, const SnrWor
 int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
                       const uint8_t *resolved, const double *s_instr, double rho_th, double *rho2_out,
                       const SnrWork &sw, cudaStream_t st);
+int cand_build_begin(const CatTable &ct, int64_t n_bins, const SnrWork &sw, cudaStream_t st);
+int cand_build_range(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
+                     const uint8_t *resolved, const double *s_instr, double rho_th, double *rho2_out,
+                     const SnrWork &sw, int64_t i_begin, int64_t i_end, cudaStream_t st);
+int cand_build_finish(const GridDev &g, const CatTable &ct, const SnrWork &sw, cudaStream_t st);
 int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th, uint8_t *resolved, double *rho2_out,
                     int64_t n_launch, int64_t *sel_idx, int64_t *sel_count, int64_t *near_count, int near_per_cat,
                     const int *abort_flag, bool use_prefix, const SnrWork &sw, const DirtyView &dv, int64_t *test_count,
@@ -720,17 +725,38 @@ static int simulate_body(const gbfg_grid *grid, const gbfg_pop *pops, const int6
     if (rc) return rc;
     // stages (i) and (ii) in one kernel: every source is deposited by the thread that draws it (sample.cu).
     // Its stamps (-1) never equal those of the loop's subtractions (1 .. max_iter).
+    // The catalog is drawn in a few pieces; the candidate records of a piece (a pass over its sources against S_instr
+    // alone) are built on the side stream while the next piece is drawn: the drawing is bound by its arithmetic, the
+    // pre-selection by L2 round trips, so the two share the SMs well.
+    struct PieceCtx {
+        const GridDev *g; const CatTable *ct; const double *A, *f, *fdot; const uint8_t *resolved; const double *s_instr;
+        double rho_th; bool preselect; const Workspace *w; cudaStream_t st; SideStream *side;
+    } pc = {&g, &ct, dev_A, dev_f, dev_fdot, dev_resolved, dev_s_instr, params->rho_th, preselect, &w, st, side};
+    auto after_piece = [](void *ctx, int64_t i_begin, int64_t i_end) -> int {
+        PieceCtx &p = *(PieceCtx *)ctx;
+        GBFG_CUDA(cudaEventRecord(p.side->ev_aux, p.st));
+        GBFG_CUDA(cudaStreamWaitEvent(p.side->s, p.side->ev_aux, 0));
+        return cand_build_range(*p.g, *p.ct, p.A, p.f, p.fdot, p.resolved, p.preselect ? p.s_instr : nullptr, p.rho_th, nullptr,
+                                p.w->sw, i_begin, i_end, p.side->s);
+    };
+    if (n > 0) {
+        rc = cand_build_begin(ct, nb, w.sw, side->s);
+        if (rc) return rc;
+    }
     {
-        const SampleDeposit dep = {dev_spectrum, w.diff, dev_err_count, w.wide_flag, plain_marks(w, nb, -1)};
+        SampleDeposit dep = {dev_spectrum, w.diff, dev_err_count, w.wide_flag, plain_marks(w, nb, -1), 0, nullptr, nullptr};
+        dep.piece = n_cat == 1 ? (n + 3) / 4 : 0;               // a batch: catalog by catalog
+        if (dep.piece < 1000000) dep.piece = dep.piece ? 1000000 : 0;
+        dep.after_piece = after_piece;
+        dep.ctx = &pc;
         rc = sample_catalog_ids(grid, pops, offsets, n_cat, 0u, cat_ids, seed, dev_A, dev_f, dev_fdot, stream, &dep);
         if (rc) return rc;
     }
-    GBFG_CUDA(cudaEventRecord(side->ev_aux, st));
-    // side stream: the candidate records (a pass over the catalog against S_instr alone)
-    GBFG_CUDA(cudaStreamWaitEvent(side->s, side->ev_aux, 0));
-    rc = loop_build_candidates(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, dev_s_instr, params->rho_th, preselect, w, side->s);
-    if (rc) return rc;
-    GBFG_CUDA(cudaEventRecord(side->ev_aux, side->s));
+    if (n > 0) {
+        rc = cand_build_finish(g, ct, w.sw, side->s);
+        if (rc) return rc;
+    }
+    GBFG_CUDA(cudaEventRecord(side->ev_aux, side->s));      // the records are ready
     // this stream: the scan of the wide sources' range updates into the spectrum
     rc = launch_scan(nb, n_cat, dev_spectrum, w.diff, w.tile_sums, w.wide_flag, plain_marks(w, nb, -1), st);
     if (rc) return rc;

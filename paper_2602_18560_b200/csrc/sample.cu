@@ -165,12 +165,14 @@ struct PopDev {
     int flat_in_log;
     double logA_offset, logA_sigma, logMc_mean, logMc_sigma;
     double f_min, f_max, f_top; // clamp
-    int64_t n_src;
+    int64_t n_src;              // sources this launch draws ...
+    int64_t i_base;             // ... the first of which is source i_base of its catalog
     uint32_t cat_id, key0, key1;
 };
 
-__device__ __forceinline__ void draw_source(const PopDev &P, int64_t i, double &A, double &f, double &fdot)
+__device__ __forceinline__ void draw_source(const PopDev &P, int64_t i_rel, double &A, double &f, double &fdot)
 {
+    const int64_t i = P.i_base + i_rel;
     U4 ctr;
     ctr.x = (uint32_t)i; ctr.y = (uint32_t)((uint64_t)i >> 32); ctr.z = 0u; ctr.w = P.cat_id;
     U4 b0 = philox4x32_10(ctr, P.key0, P.key1);
@@ -616,13 +618,6 @@ int gbfg::sample_catalog_ids(const gbfg_grid *grid, const gbfg_pop *pops, const 
         P.n_src = p.n_src;
         P.cat_id = cat_ids ? cat_ids[c] : first_cat_id + (uint32_t)c;
         P.key0 = (uint32_t)seed; P.key1 = (uint32_t)(seed >> 32);
-        int head = (int)(offsets[c] & 1);                 // keep the pairs 16-byte aligned
-        if (head > p.n_src) head = (int)p.n_src;
-        int64_t n_pairs = (p.n_src - head) / 2;
-        int64_t blocks = (n_pairs + 255) / 256;
-        if (blocks < 1) blocks = 1;
-        int64_t cap = (int64_t)sm_count() * 16;
-        if (blocks > cap) blocks = cap;
         DepositDev D;
         memset(&D, 0, sizeof(D));
         if (dep) {
@@ -631,16 +626,34 @@ int gbfg::sample_catalog_ids(const gbfg_grid *grid, const gbfg_pop *pops, const 
             D.diff = dep->diff + (int64_t)c * grid->n_bins;
             D.err_count = dep->err_count; D.wide_flag = dep->wide_flag; D.mk = dep->mk; D.cat = c;
         }
-        {
-            LaunchTimer lt(K_SAMPLE, (cudaStream_t)stream);
-            if (dep)
-                sample_kernel<true><<<(int)blocks, 256, 0, (cudaStream_t)stream>>>(
-                    P, dev_A + offsets[c], dev_f + offsets[c], dev_fdot + offsets[c], head, D);
-            else
-                sample_kernel<false><<<(int)blocks, 256, 0, (cudaStream_t)stream>>>(
-                    P, dev_A + offsets[c], dev_f + offsets[c], dev_fdot + offsets[c], head, D);
+        // pieces of at most `piece` sources (even, so that the pairs of every piece stay 16-byte aligned); after each
+        // piece the caller is told which sources of the batch are now on their way (gbfg_simulate builds their
+        // candidate records next to the drawing of the following piece)
+        int64_t piece = p.n_src;
+        if (dep && dep->piece > 0 && dep->piece < piece) piece = dep->piece & ~(int64_t)1;
+        for (int64_t i0 = 0; i0 < p.n_src; i0 += piece) {
+            const int64_t cnt = p.n_src - i0 < piece ? p.n_src - i0 : piece;
+            P.n_src = cnt;
+            P.i_base = i0;
+            int head = (int)((offsets[c] + i0) & 1);          // keep the pairs 16-byte aligned
+            if (head > cnt) head = (int)cnt;
+            int64_t n_pairs = (cnt - head) / 2;
+            int64_t blocks = (n_pairs + 255) / 256;
+            if (blocks < 1) blocks = 1;
+            int64_t cap = (int64_t)sm_count() * 16;
+            if (blocks > cap) blocks = cap;
+            double *pA = dev_A + offsets[c] + i0, *pf = dev_f + offsets[c] + i0, *pd = dev_fdot + offsets[c] + i0;
+            {
+                LaunchTimer lt(K_SAMPLE, (cudaStream_t)stream);
+                if (dep) sample_kernel<true><<<(int)blocks, 256, 0, (cudaStream_t)stream>>>(P, pA, pf, pd, head, D);
+                else sample_kernel<false><<<(int)blocks, 256, 0, (cudaStream_t)stream>>>(P, pA, pf, pd, head, D);
+            }
+            GBFG_LAUNCH_CHECK("sample_kernel");
+            if (dep && dep->after_piece) {
+                const int rc2 = dep->after_piece(dep->ctx, offsets[c] + i0, offsets[c] + i0 + cnt);
+                if (rc2) return rc2;
+            }
         }
-        GBFG_LAUNCH_CHECK("sample_kernel");
     }
     return GBFG_OK;
 }

@@ -305,7 +305,7 @@ struct BuildArgs {
     double *rho2_out;           // nullable: NaN is written for rejected sources
     CandArrays cand;
     int64_t *cand_count;        // [1 + n_cat]: total, per catalog
-    int64_t n_all;
+    int64_t i_begin, n_all;     // sources [i_begin, n_all) of the batch
     int *bkt_count, *bkt_ext;   // [n_cat][n_dblk]: zero on entry
     int n_dblk, dblk_log2;
 };
@@ -317,7 +317,7 @@ cand_build_kernel(GridDev g, CatTable ct, BuildArgs a)
 {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
-    const int64_t n_round = (a.n_all + 255) & ~(int64_t)255;   // the same number of trips for every thread of a CTA
+    const int64_t n_round = a.i_begin + ((a.n_all - a.i_begin + 255) & ~(int64_t)255);   // the same number of trips for every thread of a CTA
     // CTA_APPEND: a batch of 3e8 sources would otherwise put 1e7 atomics on one counter
     __shared__ int s_wcnt[2][8];
     __shared__ long long s_base[2];
@@ -325,7 +325,7 @@ cand_build_kernel(GridDev g, CatTable ct, BuildArgs a)
     bool pref_ok = false;
     int unit_exp = 0;
     if (a.s_instr && a.pv.pref) { pref_ok = a.pv.hdr->bad == 0; unit_exp = a.pv.hdr->unit_exp; }
-    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += stride) {
+    for (int64_t i = a.i_begin + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_round; i += stride) {
         bool keep = false;
         SrcBins s; s.status = 1; s.k0 = 0; s.w_eff = 0; s.p = 0.0; s.q = 0;
         int cat = 0;
@@ -671,12 +671,22 @@ int launch_inv_prefix(const double *psd, int64_t n_bins, int n_cat, const SnrWor
 // candidate records of every unresolved valid source; s_instr != NULL: pre-selection against the
 // instrument noise (the prefix in sw must then be that of 1/s_instr, one row).
 // sw.cand_count[0 .. n_cat] must be zero on entry.
-int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
-                      const uint8_t *resolved, const double *s_instr, double rho_th, double *rho2_out,
-                      const SnrWork &sw, cudaStream_t st)
+// Three steps, so that the records of a catalog can be built piece by piece while it is still being drawn (loop.cu):
+// begin (clears the bucket counts), any number of ranges [i_begin, i_end) of the batch, finish (orders the records).
+int cand_build_begin(const CatTable &ct, int64_t n_bins, const SnrWork &sw, cudaStream_t st)
 {
-    const int64_t n = ct.offsets[ct.n_cat];
-    if (n <= 0) return GBFG_OK;
+    const int n_dblk = dirty_blocks_per_row(n_bins);
+    GBFG_CUDA(cudaMemsetAsync(sw.bkt_count, 0, sizeof(int) * (size_t)ct.n_cat * (size_t)n_dblk, st));
+    GBFG_CUDA(cudaMemsetAsync(sw.bkt_ext, 0, sizeof(int) * (size_t)ct.n_cat * (size_t)n_dblk, st));
+    GBFG_CUDA(cudaMemsetAsync(sw.any_near, 0, 2 * sizeof(int), st));
+    return GBFG_OK;
+}
+
+int cand_build_range(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
+                     const uint8_t *resolved, const double *s_instr, double rho_th, double *rho2_out,
+                     const SnrWork &sw, int64_t i_begin, int64_t i_end, cudaStream_t st)
+{
+    if (i_end <= i_begin) return GBFG_OK;
     BuildArgs a;
     a.A = A; a.f = f; a.fdot = fdot; a.resolved = resolved; a.s_instr = s_instr;
     a.pv = make_view(sw, g.n_bins);
@@ -684,19 +694,28 @@ int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, con
     a.rho2_out = rho2_out;
     a.cand.gk0 = sw.tmp_gk0; a.cand.w = sw.tmp_w; a.cand.four_p = sw.tmp_4p; a.cand.src = sw.tmp_src;
     a.cand_count = sw.cand_count;
-    a.n_all = n;
-    const int n_dblk = dirty_blocks_per_row(g.n_bins), dblk_log2 = dirty_block_log2(g.n_bins);
-    a.bkt_count = sw.bkt_count; a.bkt_ext = sw.bkt_ext; a.n_dblk = n_dblk; a.dblk_log2 = dblk_log2;
-    GBFG_CUDA(cudaMemsetAsync(sw.bkt_count, 0, sizeof(int) * (size_t)ct.n_cat * (size_t)n_dblk, st));
-    GBFG_CUDA(cudaMemsetAsync(sw.bkt_ext, 0, sizeof(int) * (size_t)ct.n_cat * (size_t)n_dblk, st));
-    GBFG_CUDA(cudaMemsetAsync(sw.any_near, 0, 2 * sizeof(int), st));
-    int64_t blocks = (n + 255) / 256;
+    a.i_begin = i_begin; a.n_all = i_end;
+    a.bkt_count = sw.bkt_count; a.bkt_ext = sw.bkt_ext;
+    a.n_dblk = dirty_blocks_per_row(g.n_bins); a.dblk_log2 = dirty_block_log2(g.n_bins);
+    int64_t blocks = (i_end - i_begin + 255) / 256;
     const int64_t cap = (int64_t)sm_count() * 16;
     if (blocks > cap) blocks = cap;
     LaunchTimer lt(K_SNR, st);
-    if (ct.n_cat > 1 || n >= 30000000) cand_build_kernel<true><<<(int)blocks, 256, 0, st>>>(g, ct, a);
+    if (ct.n_cat > 1 || ct.offsets[ct.n_cat] >= 30000000) cand_build_kernel<true><<<(int)blocks, 256, 0, st>>>(g, ct, a);
     else cand_build_kernel<false><<<(int)blocks, 256, 0, st>>>(g, ct, a);
     GBFG_LAUNCH_CHECK("cand_build_kernel");
+    return GBFG_OK;
+}
+
+int cand_build_finish(const GridDev &g, const CatTable &ct, const SnrWork &sw, cudaStream_t st)
+{
+    const int64_t n = ct.offsets[ct.n_cat];
+    const int n_dblk = dirty_blocks_per_row(g.n_bins), dblk_log2 = dirty_block_log2(g.n_bins);
+    int64_t blocks = (n + 255) / 256;
+    const int64_t cap = (int64_t)sm_count() * 16;
+    if (blocks > cap) blocks = cap;
+    if (blocks < 1) blocks = 1;
+    LaunchTimer lt(K_SNR, st);
     // order the records by (row, dirty block of the first bin)
     cand_bucket_scan_kernel<<<ct.n_cat, BKT_THREADS, 0, st>>>(sw.bkt_count, sw.bkt_ext, sw.bkt_off, sw.cand_count, n_dblk);
     GBFG_LAUNCH_CHECK("cand_bucket_scan_kernel");
@@ -707,6 +726,18 @@ int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, con
     cand_scatter_kernel<<<(int)blocks, 256, 0, st>>>(in, out, sw.cand_count, sw.bkt_count, sw.bkt_off, g.n_bins, n_dblk, dblk_log2);
     GBFG_LAUNCH_CHECK("cand_scatter_kernel");
     return GBFG_OK;
+}
+
+int launch_cand_build(const GridDev &g, const CatTable &ct, const double *A, const double *f, const double *fdot,
+                      const uint8_t *resolved, const double *s_instr, double rho_th, double *rho2_out,
+                      const SnrWork &sw, cudaStream_t st)
+{
+    const int64_t n = ct.offsets[ct.n_cat];
+    if (n <= 0) return GBFG_OK;
+    int rc = cand_build_begin(ct, g.n_bins, sw, st);
+    if (!rc) rc = cand_build_range(g, ct, A, f, fdot, resolved, s_instr, rho_th, rho2_out, sw, 0, n, st);
+    if (!rc) rc = cand_build_finish(g, ct, sw, st);
+    return rc;
 }
 
 // the test over the candidate records; n_launch = upper bound of the candidate count (grid sizing).
