@@ -236,12 +236,22 @@ def algorithmic_bytes(w: wl.Workload, n_bins: int, res, prof) -> dict:
     }
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of running_median_kernel per output it recomputes, from the
-# committed `ncu --set full` captures (profiles/r01_profiles_v6.md: 76.3 MB for a full pass of 3 774 349 outputs)
-MEDIAN_DRAM_BYTES_PER_OUTPUT = 20.0
-# smsp__inst_executed.sum of the same kernel per output it recomputes (profiles/r01_ncu_full_v3.md: 1.14e8 warp
-# instructions for a full pass of 3 774 349 outputs; r01_ncu_full_v5.md: 9.97e7 for ~3.4e6)
-MEDIAN_WARP_INSTR_PER_OUTPUT = 30.0
+def median_kernel_counters():
+    """dram bytes and warp instructions of the running-median kernel per output it recomputes, as the committed
+    `ncu --set full` summary states them (profiles/r02_ncu_full.md, lines `median_...: value`); nothing is hard-coded here,
+    so a stale figure can only come from a stale summary, whose commit is reported next to it."""
+    path = os.path.join(ROOT, "profiles", "r02_ncu_full.md")
+    out = {"source": "profiles/r02_ncu_full.md"}
+    try:
+        with open(path) as fh:
+            for line in fh:
+                for key in ("median_dram_bytes_per_output", "median_warp_instr_per_output", "median_capture_commit"):
+                    if line.startswith(key + ":"):
+                        v = line.split(":", 1)[1].strip()
+                        out[key] = v if key.endswith("commit") else float(v)
+    except OSError:
+        pass
+    return out
 
 
 def run_gpu(args, w: wl.Workload):
@@ -373,27 +383,29 @@ def run_gpu(args, w: wl.Workload):
     kd = kernels[dom]
     bytes_per_launch = kd["algorithmic_bytes_per_step"] / kd["launches_per_step"]
     traffic = args.traffic
-    if traffic is None and dom == "median":
+    mk = median_kernel_counters()
+    if traffic is None and dom == "median" and "median_dram_bytes_per_output" in mk:
         # per launch like `achieved`: an average launch recomputes bytes_per_launch / 32 outputs
-        traffic = MEDIAN_DRAM_BYTES_PER_OUTPUT * bytes_per_launch / 32.0
+        traffic = mk["median_dram_bytes_per_output"] * bytes_per_launch / 32.0
     roofline = {"kernel": dom, "bound": "hbm", "achieved": bytes_per_launch / (kd["avg_launch_ms"] * 1e-3) / 1e9,
                 "peak": peak, "peak_source": peak_src, "unit": "GB/s",
                 "frac": bytes_per_launch / (kd["avg_launch_ms"] * 1e-3) / 1e9 / peak,
                 "algorithmic_bytes_per_launch": bytes_per_launch, "avg_launch_ms": kd["avg_launch_ms"],
-                "traffic": traffic}
+                "traffic": traffic, "traffic_source": mk if dom == "median" else None}
 
     # What actually bounds the running median is instruction issue, not HBM: the same launches
     # against the issue rate of the part, 4 warp instructions per SM and clock (B200_PROFILING.md: 148 SMs x 4 schedulers)
     roofline_issue = None
-    if dom == "median":
+    if dom == "median" and "median_warp_instr_per_output" in mk:
+        ipo = mk["median_warp_instr_per_output"]
         sms = torch.cuda.get_device_properties(dev).multi_processor_count
         mhz = (clk or {}).get("sm_mhz") or (clk or {}).get("sm_max_mhz") or 1965.0
         peak_issue = sms * 4 * mhz * 1e6 / 1e9                      # G warp-instructions / s
-        ach = MEDIAN_WARP_INSTR_PER_OUTPUT * (bytes_per_launch / 32.0) / (kd["avg_launch_ms"] * 1e-3) / 1e9
+        ach = ipo * (bytes_per_launch / 32.0) / (kd["avg_launch_ms"] * 1e-3) / 1e9
         roofline_issue = {"kernel": dom, "bound": "alu", "achieved": ach, "peak": peak_issue,
                           "unit": "G warp-instr/s", "frac": ach / peak_issue,
                           "peak_source": f"{sms} SMs x 4 schedulers x {mhz:.0f} MHz (sm clock under load)",
-                          "instr_per_output": MEDIAN_WARP_INSTR_PER_OUTPUT}
+                          "instr_per_output": ipo}
 
     # ---- the oracle on one host core, the same workload in full (a reported baseline, not the target)
     cpu = None
@@ -436,6 +448,50 @@ def run_gpu(args, w: wl.Workload):
     return 0
 
 
+def run_stage_bench(args, w: wl.Workload):
+    """`--stage-bench`: the two PSD estimators alone, one full pass over the workload's grid per launch (stage calls
+    gbfg_running_median / gbfg_running_mean on the deposited spectrum of the workload's catalog), CUDA events on the
+    launching stream, 256 MB written between repetitions to flush the 126 MB L2.  Prints one JSON line."""
+    import torch
+    import paper_2602_18560_b200 as gb
+    torch.cuda.set_device(0)
+    gb.load()
+    dev = torch.device("cuda", 0)
+    g = gb.grid_init(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    n, nb = w.n_src_total, g.n_bins
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device=dev) for _ in range(3))
+    gb.sample_catalog(g, w.pops, w.offsets(), w.seed, A, f, fd)
+    spec = torch.zeros(nb, dtype=torch.int64, device=dev)
+    ws = torch.empty(gb.workspace_bytes(g, n, 1), dtype=torch.uint8, device=dev)
+    gb.deposit(g, A, f, fd, w.offsets(), spec, ws)
+    s_instr = torch.empty(nb, dtype=torch.float64, device=dev)
+    gb.instrument_noise(g, s_instr)
+    out = torch.empty(nb, dtype=torch.int64, device=dev)
+    psd = torch.empty(nb, dtype=torch.float64, device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    peak, peak_src = measured_peaks()
+    res = {}
+    calls = {"running_median": (lambda: gb.running_median(spec, nb, 1, w.window, out, ws), 16),
+             "running_mean": (lambda: gb.running_mean(spec, nb, 1, w.window, out, s_instr, w.scale_log2, psd), 32)}
+    for name, (fn, bytes_per_bin) in calls.items():
+        for _ in range(3):
+            fn()
+        ts = []
+        for _ in range(max(args.steps, 5)):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); fn(); e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        t = float(np.median(ts))
+        gbs = bytes_per_bin * nb / (t * 1e-3) / 1e9
+        res[name] = {"ms": t, "algorithmic_bytes": bytes_per_bin * nb, "achieved_gbs": gbs, "frac_of_hbm": gbs / peak}
+    print(json.dumps({"stage_bench": res, "workload": w.name, "n_bins": nb, "window": w.window, "peak_gbs": peak,
+                      "peak_source": peak_src, "l2": "flushed between repetitions (256 MB written)",
+                      "note": "running_median: stage call without the PSD epilogue (16 B per bin), two launches"}), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -447,6 +503,7 @@ def main():
     ap.add_argument("--flags", type=int, default=0, help="gbfg_iter_params.flags")
     ap.add_argument("--max-iter", type=int, default=None, help="override the iteration cap (debug only: cost per iteration)")
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--stage-bench", action="store_true", help="time the two PSD estimators alone (one full pass each) and exit")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-config4", action="store_true",
                     help="also time the oracle on configs[4] (64 catalogs) over all host cores: minutes")
@@ -460,6 +517,8 @@ def main():
         w = wl.replace(w, max_iter=args.max_iter, name=f"{w.name}_cap{args.max_iter}")
     if args.impl == "reference":
         return run_reference(args, w)
+    if args.stage_bench:
+        return run_stage_bench(args, w)
     return run_gpu(args, w)
 
 

@@ -169,9 +169,12 @@ int gbfg_deposit(const gbfg_grid *grid, const double *dev_A, const double *dev_f
 /* Stage (iii) — exact running median of eq. (D2), PAPER.md:542 (R3): for each row,
  * median_out[k] = the h-th smallest of x[k-h .. k+h], W = 2h+1 odd, ends reflected
  * (x[-j] = x[j-1], x[n-1+j] = x[n-j]).  Requires n_bins >= h+1 and W <= GBFG_MAX_WINDOW.
- * dev_spectrum, dev_median_out: [n_cat][n_bins] int64 (must not alias). */
+ * dev_spectrum, dev_median_out: [n_cat][n_bins] int64 (must not alias).
+ * workspace: DEVICE, 16-byte aligned, >= gbfg_running_median_workspace_bytes(n_bins, n_cat, window) bytes (a workspace of
+ * gbfg_workspace_bytes() for the same grid is large enough too); GBFG_ERR_WORKSPACE otherwise.  Nothing is allocated. */
 int gbfg_running_median(const int64_t *dev_spectrum, int64_t n_bins, int32_t n_cat, int32_t window,
-                        int64_t *dev_median_out, void *stream);
+                        int64_t *dev_median_out, void *workspace, size_t workspace_bytes, void *stream);
+size_t gbfg_running_median_workspace_bytes(int64_t n_bins, int32_t n_cat, int32_t window);   /* 0: invalid arguments */
 
 /* Running-mean estimator of eq. (D1), PAPER.md:538 (the paper's production choice, :176, :552; R8):
  * sum_out[c][k] = sum of x[c][k-h .. k+h], W = 2h+1 odd, ends reflected as for the median (the exact

@@ -26,7 +26,7 @@ EXPORTS = [
     "gbfg_subtract_until_converged", "gbfg_simulate", "gbfg_simulate_host", "gbfg_workspace_bytes",
     "gbfg_kernel_launch_count", "gbfg_profile_enable", "gbfg_profile_read", "gbfg_release_cached",
     "gbfg_running_mean", "gbfg_coarse_grain", "gbfg_instrument_noise_aet",
-    "gbfg_sample_catalog_paper",
+    "gbfg_sample_catalog_paper", "gbfg_running_median_workspace_bytes",
 ]
 
 KERNEL_CLASSES = ["sample", "noise", "deposit", "scan", "median", "psd", "inv_blocks", "snr", "aux"]
@@ -97,7 +97,9 @@ def load():
     L.gbfg_sample_catalog.argtypes = [gp, pp, op, i32, u32, u64, vp, vp, vp, vp]
     L.gbfg_sample_catalog_paper.argtypes = [gp, C.POINTER(PopPaper), op, i32, u32, u64, vp, vp, vp, vp]
     L.gbfg_deposit.argtypes = [gp, vp, vp, vp, op, i32, vp, vp, i32, vp, vp, vp, sz, vp]
-    L.gbfg_running_median.argtypes = [vp, i64, i32, i32, vp, vp]
+    L.gbfg_running_median.argtypes = [vp, i64, i32, i32, vp, vp, sz, vp]
+    L.gbfg_running_median_workspace_bytes.restype = sz
+    L.gbfg_running_median_workspace_bytes.argtypes = [i64, i32, i32]
     L.gbfg_psd.argtypes = [vp, vp, i64, i32, dbl, i32, vp, vp]
     L.gbfg_running_mean.argtypes = [vp, i64, i32, i32, vp, vp, i32, vp, vp]
     L.gbfg_coarse_grain.argtypes = [vp, i64, i32, vp, i32, dbl, dbl, vp, vp, vp, vp]
@@ -231,8 +233,18 @@ def deposit(grid: Grid, dev_A, dev_f, dev_fdot, offsets, dev_spectrum, workspace
                                _stream(stream)))
 
 
-def running_median(dev_spectrum, n_bins: int, n_cat: int, window: int, dev_median_out, stream=None):
-    _check(load().gbfg_running_median(_ptr(dev_spectrum), n_bins, n_cat, window, _ptr(dev_median_out), _stream(stream)))
+def running_median_workspace_bytes(n_bins: int, n_cat: int, window: int) -> int:
+    return load().gbfg_running_median_workspace_bytes(n_bins, n_cat, window)
+
+
+def running_median(dev_spectrum, n_bins: int, n_cat: int, window: int, dev_median_out, workspace=None, stream=None):
+    """workspace: a device tensor of >= running_median_workspace_bytes(...) bytes; None: one is taken from torch."""
+    if workspace is None:
+        import torch
+        workspace = torch.empty(max(running_median_workspace_bytes(n_bins, n_cat, window), 256), dtype=torch.uint8,
+                                device=dev_spectrum.device)
+    _check(load().gbfg_running_median(_ptr(dev_spectrum), n_bins, n_cat, window, _ptr(dev_median_out), _ptr(workspace),
+                                      workspace.numel() * workspace.element_size(), _stream(stream)))
 
 
 def running_mean(dev_spectrum, n_bins: int, n_cat: int, window: int, dev_sum_out, dev_s_instr=None,

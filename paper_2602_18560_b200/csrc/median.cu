@@ -350,25 +350,33 @@ int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64
 
 using namespace gbfg;
 
+// room for the list of tiles the 32-bit-key kernel leaves to the 64-bit-key one: 16 bytes of counters + one int4 per tile
+extern "C" size_t gbfg_running_median_workspace_bytes(int64_t n_bins, int32_t n_cat, int32_t window)
+{
+    if (window < 1 || (window & 1) == 0 || window > GBFG_MAX_WINDOW || n_cat < 1 || n_cat > GBFG_MAX_CAT || n_bins < 1 ||
+        n_bins >= 2147483648ll)
+        return 0;
+    const int s_max = MED_LT32 - (window - 1);
+    const size_t tiles = (size_t)((n_bins + s_max - 1) / s_max) + 2 * 148 * 4;     // whole waves of CTAs on any part
+    return 256 + sizeof(int4) * tiles * (size_t)n_cat;
+}
+
 extern "C" int gbfg_running_median(const int64_t *dev_spectrum, int64_t n_bins, int32_t n_cat, int32_t window,
-                                   int64_t *dev_median_out, void *stream)
+                                   int64_t *dev_median_out, void *workspace, size_t workspace_bytes, void *stream)
 {
     if (!dev_spectrum || !dev_median_out || dev_spectrum == dev_median_out) return GBFG_ERR_INVALID_ARG;
     if (window < 1 || (window & 1) == 0 || n_cat < 1 || n_bins < 1 || n_bins >= 2147483648ll) return GBFG_ERR_INVALID_ARG;
     if (window > GBFG_MAX_WINDOW || n_cat > GBFG_MAX_CAT) return GBFG_ERR_UNSUPPORTED;
     if (n_bins < window / 2 + 1) return GBFG_ERR_INVALID_ARG;
+    if (!workspace || ((uintptr_t)workspace & 15)) return GBFG_ERR_WORKSPACE;
+    const int tiles = median_static_tiles(n_bins, n_cat, window, nullptr);
+    if (workspace_bytes < 256 + sizeof(int4) * (size_t)tiles * (size_t)n_cat) return GBFG_ERR_WORKSPACE;
     int rc = check_device();
     if (rc) return rc;
-    // room for the wide list (tiles whose values differ in their high 32 bits), stream ordered
-    cudaStream_t st = (cudaStream_t)stream;
-    const int tiles = median_static_tiles(n_bins, n_cat, window, nullptr);
-    char *tmp = nullptr;
-    GBFG_CUDA(cudaMallocAsync((void **)&tmp, 16 + sizeof(int4) * (size_t)tiles * (size_t)n_cat, st));
-    rc = launch_median(dev_spectrum, n_bins, n_cat, window, dev_median_out, nullptr, nullptr, 1.0, 0, nullptr,
-                       (int4 *)(tmp + 16), (int *)tmp, nullptr, nullptr, st);
-    cudaError_t e = cudaFreeAsync(tmp, st);
-    if (!rc && e != cudaSuccess) rc = set_cuda_error(e, "cudaFreeAsync");
-    return rc;
+    // the caller's workspace holds the wide list (tiles whose values differ in their high 32 bits)
+    char *tmp = (char *)workspace;
+    return launch_median(dev_spectrum, n_bins, n_cat, window, dev_median_out, nullptr, nullptr, 1.0, 0, nullptr,
+                         (int4 *)(tmp + 256), (int *)tmp, nullptr, nullptr, (cudaStream_t)stream);
 }
 
 extern "C" int gbfg_psd(const int64_t *dev_median, const double *dev_s_instr, int64_t n_bins, int32_t n_cat,

@@ -289,6 +289,10 @@ __device__ __forceinline__ double rho2_of(const double *__restrict__ psd, const 
     return four_p * fixed_to_double(hi, unit_exp);
 }
 
+// source index (< 2^36) and place inside the bucket (< 2^28) of a record as first compacted
+constexpr int CAND_SLOT_SHIFT = 36;
+constexpr int64_t CAND_SRC_MASK = ((int64_t)1 << CAND_SLOT_SHIFT) - 1;
+
 struct CandArrays {
     int64_t *gk0;       // first bin, as index into the [n_cat][n_bins] arrays
     int32_t *w;         // w_eff; set to 0 once the source is resolved
@@ -371,11 +375,13 @@ cand_build_kernel(GridDev g, CatTable ct, BuildArgs a)
                 a.cand.gk0[t] = (int64_t)cat * g.n_bins + s.k0;
                 a.cand.w[t] = (int32_t)s.w_eff;
                 a.cand.four_p[t] = 4.0 * s.p;
-                a.cand.src[t] = i;
                 if (ct.n_cat > 1 && lane == __ffs(same) - 1)   // one add per warp and catalog (a warp rarely straddles two)
                     atomicAdd((unsigned long long *)(a.cand_count + 1 + cat), (unsigned long long)__popc(same));
                 const int64_t gb = (int64_t)cat * a.n_dblk + (s.k0 >> a.dblk_log2);
-                atomicAdd(a.bkt_count + gb, 1);
+                // the record's place inside its bucket is taken here, so that the ordering pass (cand_scatter_kernel)
+                // needs no atomics of its own: it rides in the upper bits of the source index
+                const int64_t slot = atomicAdd(a.bkt_count + gb, 1);
+                a.cand.src[t] = i | (slot << CAND_SLOT_SHIFT);
                 atomicMax(a.bkt_ext + gb, (int)((s.k0 + s.w_eff - 1) >> a.dblk_log2));
             }
         }
@@ -449,11 +455,12 @@ cand_scatter_kernel(CandArraysConst in, CandArrays out, const int64_t *__restric
         const int64_t gk0 = in.gk0[t];
         const int64_t row = gk0 / n_bins;
         const int64_t b = (gk0 - row * n_bins) >> dblk_log2;
-        const int64_t dst = bkt_off[row * (n_dblk + 1) + b] + atomicAdd(bkt_cur + row * n_dblk + b, 1);
+        const int64_t packed = in.src[t];
+        const int64_t dst = bkt_off[row * (n_dblk + 1) + b] + (packed >> CAND_SLOT_SHIFT);
         out.gk0[dst] = gk0;
         out.w[dst] = in.w[t];
         out.four_p[dst] = in.four_p[t];
-        out.src[dst] = in.src[t];
+        out.src[dst] = packed & CAND_SRC_MASK;
     }
 }
 

@@ -77,11 +77,17 @@ def test_invalid_arguments_are_rejected_before_any_cuda_call(gbcpu):
     g = gbcpu.grid_init(1e-4, 1e-2, 3.15581e7, -140)
     off = (C.c_int64 * 2)(0, 10)
     # running median: even window, window wider than the build supports, n_bins < h + 1, aliasing
-    assert L.gbfg_running_median(8, 1000, 1, 10, 16, None) == -1
-    assert L.gbfg_running_median(8, 100000, 1, 4099, 16, None) == -5
-    assert L.gbfg_running_median(8, 100, 1, 1001, 16, None) == -1
-    assert L.gbfg_running_median(8, 1000, 1, 11, 8, None) == -1
-    assert L.gbfg_running_median(None, 1000, 1, 11, 16, None) == -1
+    assert L.gbfg_running_median(8, 1000, 1, 10, 16, 32, 1 << 20, None) == -1
+    assert L.gbfg_running_median(8, 100000, 1, 4099, 16, 32, 1 << 20, None) == -5
+    assert L.gbfg_running_median(8, 100, 1, 1001, 16, 32, 1 << 20, None) == -1
+    assert L.gbfg_running_median(8, 1000, 1, 11, 8, 32, 1 << 20, None) == -1
+    assert L.gbfg_running_median(None, 1000, 1, 11, 16, 32, 1 << 20, None) == -1
+    # the caller's workspace: missing, misaligned, too small
+    assert L.gbfg_running_median(8, 1000, 1, 11, 16, None, 0, None) == -2
+    assert L.gbfg_running_median(8, 1000, 1, 11, 16, 36, 1 << 20, None) == -2
+    assert L.gbfg_running_median(8, 1000, 1, 11, 16, 32, 64, None) == -2
+    need = L.gbfg_running_median_workspace_bytes(3774349, 1, 2001)
+    assert 256 < need < (1 << 20) and L.gbfg_running_median_workspace_bytes(3774349, 1, 2000) == 0
     # deposit: sign, null spectrum, list without count, missing workspace
     assert L.gbfg_deposit(C.byref(g), 8, 8, 8, off, 1, None, None, 2, 8, None, 8, 1 << 30, None) == -1
     assert L.gbfg_deposit(C.byref(g), 8, 8, 8, off, 1, None, None, 1, None, None, 8, 1 << 30, None) == -1
