@@ -247,7 +247,10 @@ running_median_tile_kernel(MedianArgs a)
             if (r < rounds) {
                 const int e = warp * (32 * rounds) + r * 32 + lane;
                 k[r] = skey[e];
-                pk[r] = same_digit_lanes((unsigned)(k[r] >> shift) & 255u);
+                // every third round by MATCH.ANY, the others by eight reductions: the two run on different units of the
+                // SM (one MATCH per ~50 clocks, ~50 issue slots for the reductions), so the mix beats either alone
+                pk[r] = (r % 3 == 0) ? __match_any_sync(FULL, (unsigned)(k[r] >> shift) & 255u)
+                                     : same_digit_lanes((unsigned)(k[r] >> shift) & 255u);
             }
         }
 #pragma unroll

@@ -63,7 +63,7 @@ struct PrefixHeader { int unit_exp; int e_top; int bad; int pad; };
 // x = 1/psd as fixed point with unit 2^U, truncated.  ok = 0 when x is negative, not finite or >= 2^e_top.
 __device__ __forceinline__ U128 inv_to_fixed(double psd, int U, int e_top, int *ok)
 {
-    const double x = 1.0 / psd;
+    const double x = __drcp_rn(psd);                        // the correctly rounded 1 / psd, as the division gives
     const long long bits = __double_as_longlong(x);
     const int e = (int)((bits >> 52) & 0x7ff);
     U128 v; v.lo = 0; v.hi = 0;
@@ -105,7 +105,7 @@ prefix_header_kernel(const double *__restrict__ arr, int64_t n, int64_t n_bins_r
     int bad = 0;
     const int64_t stride = (int64_t)gridDim.x * blockDim.x;
     for (int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n; k += stride) {
-        const double x = 1.0 / arr[k];
+        const double x = __drcp_rn(arr[k]);
         const long long bits = __double_as_longlong(x);
         const int e = (int)((bits >> 52) & 0x7ff);
         if (bits < 0 || e == 0x7ff) bad = 1;
