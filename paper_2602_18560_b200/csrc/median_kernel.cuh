@@ -182,7 +182,7 @@ running_median_tile_kernel(MedianArgs a)
     MED_TICK(0);
     // ---- stage the tile: position p <-> global bin o0 - h + p, reflected at both ends.
     // Unused positions (Lt <= p < LTe) repeat position 0: they are never inside a window.
-    if (tid < 2) misc[32 + tid] = 0u;
+    if (tid < 4) misc[32 + tid] = tid == 2 ? 0xffffffffu : 0u;      // varying bits (lo, hi), smallest high word, varying bits again
     __syncthreads();
     uint64_t key_ref;
     {
@@ -222,13 +222,53 @@ running_median_tile_kernel(MedianArgs a)
         }
     }
     __syncthreads();
-    const uint64_t vary_all = ((uint64_t)misc[33] << 32) | misc[32];
-    if (NARROW && (vary_all >> 32) != 0) {               // 32 bits do not order this tile: leave it to the wide kernel
-        if (tid == 0) {
-            a.wide_items[atomicAdd(&a.wide_ctr[0], 1)] = make_int4(row_i, (int)o0, n_out, 0);
-            if (a.items) next_item = (int)gridDim.x + atomicAdd(&a.ctr[1], 1);
+    uint64_t vary_all = ((uint64_t)misc[33] << 32) | misc[32];
+    bool saturated = false;                              // keys above the tile's smallest high word share the key 0xffffffff
+    if (NARROW && (vary_all >> 32) != 0) {
+        // 32 bits do not order this tile.  Most often a handful of very loud bins stick out above 2^32 while the medians
+        // sit far below: every value whose high word exceeds the tile's smallest one then gets the key 0xffffffff (they
+        // are all larger than the rest, and their order among themselves does not matter as long as no median is one of
+        // them, which the walk checks).  Otherwise, or when that check fails, the tile goes to the 64-bit-key kernel.
+        // (Not with the PSD-change rule: a second attempt would compare against the first attempt's PSD.)
+        if (DELTA) {
+            if (tid == 0) {
+                a.wide_items[atomicAdd(&a.wide_ctr[0], 1)] = make_int4(row_i, (int)o0, n_out, 0);
+                if (a.items) next_item = (int)gridDim.x + atomicAdd(&a.ctr[1], 1);
+            }
+            continue;
         }
-        continue;
+        unsigned hmin = 0xffffffffu;
+        for (int p = tid; p < Lt; p += THREADS) {
+            int64_t g = o0 - h + p;
+            if (g < 0) g = -g - 1;
+            if (g >= a.n) g = 2 * a.n - 1 - g;
+            const unsigned hi = (unsigned)(((uint64_t)__ldg(a.x + row + g) ^ SIGN64) >> 32);
+            hmin = hi < hmin ? hi : hmin;
+        }
+        hmin = __reduce_min_sync(FULL, hmin);
+        if (lane == 0) atomicMin(&misc[34], hmin);
+        __syncthreads();
+        hmin = misc[34];
+        const unsigned k_first = (unsigned)(key_ref >> 32) == hmin ? (unsigned)key_ref : 0xffffffffu;
+        unsigned vary32 = 0u;
+        for (int p = tid; p < LTe; p += THREADS) {
+            unsigned k32 = k_first;
+            if (p < Lt) {
+                int64_t g = o0 - h + p;
+                if (g < 0) g = -g - 1;
+                if (g >= a.n) g = 2 * a.n - 1 - g;
+                const uint64_t key = (uint64_t)__ldg(a.x + row + g) ^ SIGN64;
+                k32 = (unsigned)(key >> 32) == hmin ? (unsigned)key : 0xffffffffu;
+            }
+            vary32 |= k32 ^ k_first;
+            skey[p] = (KeyT)k32;
+        }
+        vary32 = __reduce_or_sync(FULL, vary32);
+        if (lane == 0 && vary32) atomicOr(&misc[35], vary32);
+        __syncthreads();
+        vary_all = misc[35];
+        key_ref = ((uint64_t)hmin << 32) | k_first;      // the high word of every value that can be a median
+        saturated = true;
     }
     const int n_pass = vary_all ? (64 - __clzll((long long)vary_all) + 7) / 8 : 0;
 
@@ -313,6 +353,7 @@ running_median_tile_kernel(MedianArgs a)
     MED_TICK(3);
     if (a.items && tid == 0) next_item = (int)gridDim.x + atomicAdd(&a.ctr[1], 1);     // the next tile of this CTA
     double dmax = 0.0;
+    bool sat_hit = false;                                // a median of a saturated tile landed on the saturated key
     // ---- window bitmaps.  Warp w owns the chunks [w cpw, (w+1) cpw) of 32 consecutive outputs and keeps, in
     // shared memory, one bit per sorted rank: "the element of this rank lies in the window".  The median of a
     // window is its (h+1)-th set bit.
@@ -440,6 +481,7 @@ running_median_tile_kernel(MedianArgs a)
                 }
                 if (own) {                                   // median and PSD of output j0 + lane, 256 bytes per warp and array
                     const KeyT kv = skey[lane ? r : m0];
+                    if (NARROW && saturated && kv == (KeyT)0xffffffffu) sat_hit = true;
                     int64_t v;
                     if (NARROW) v = (int64_t)(((key_ref & 0xffffffff00000000ull) | (uint64_t)kv) ^ SIGN64);
                     else v = (int64_t)((uint64_t)kv ^ SIGN64);
@@ -464,7 +506,10 @@ running_median_tile_kernel(MedianArgs a)
             }
         }
     }
-    __syncthreads();
+    {
+        const int any_hit = __syncthreads_or(NARROW && saturated && sat_hit);      // (also the barrier of the walk's end)
+        if (NARROW && any_hit && tid == 0) a.wide_items[atomicAdd(&a.wide_ctr[0], 1)] = make_int4(row_i, (int)o0, n_out, 0);
+    }
 
     MED_TICK(6);
     if (DELTA) {                                         // non-negative binary64 values order like their bits
