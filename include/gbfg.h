@@ -134,6 +134,13 @@ int gbfg_instrument_noise(const gbfg_grid *grid, double *dev_s_instr, void *stre
 int gbfg_instrument_noise_aet(const gbfg_grid *grid, double P_pm, double A_fm, double L_m, int32_t tdi2,
                               double *dev_S_AA, double *dev_S_TT, double *dev_Sh_AA, double *dev_Sh_TT, void *stream);
 
+/* Helper: the noise curve of the SNR summed over the TDI channels A, E, T, eq. (11), in the power domain
+ * (R14): a source's strain power p enters channel X with the sky-averaged response R_XX, so the channel's term of
+ * eq. (11) is 4 p / S_h^XX with S_h^XX = S^XX / R_XX (the dev_Sh_* outputs of gbfg_instrument_noise_aet); A and E are equal,
+ * hence rho^2 = sum_bins 4 p / S_sum with  S_sum = 1 / ((2 / S_h^AA) + (1 / S_h^TT)).  Handing dev_Sh_sum to the stage calls as
+ * their s_instr makes every SNR of the loop the channel-summed one.  All arrays [n_bins] binary64, DEVICE. */
+int gbfg_channel_sum_noise(const double *dev_Sh_AA, const double *dev_Sh_TT, int64_t n_bins, double *dev_Sh_sum, void *stream);
+
 /* Stage (i) — step 1 of the algorithm: draw every catalog of the batch from its
  * population with Philox4x32-10 (R1, §4).  pops: HOST [n_cat]; offsets: HOST [n_cat+1]
  * with offsets[c+1]-offsets[c] = pops[c].n_src.  Catalog c uses Philox counter word 3 =

@@ -103,6 +103,7 @@ def lib():
         L.orc_subtract_until_converged_tol.argtypes = [
             C.POINTER(Grid), dp, dp, dp, C.c_int64, dp, C.c_int32, C.c_double, C.c_double, C.c_int32, C.c_int32, C.c_double,
             ip, ip, dp, up, C.POINTER(IterResult), ip]
+        L.orc_channel_sum_noise.argtypes = [dp, dp, C.c_int64, dp]
         L.orc_stage_seconds.argtypes = [C.POINTER(C.c_double), C.c_int]
         L.orc_running_sum_def.argtypes = [ip, C.c_int64, C.c_int32, C.c_int64, C.c_int64, ip]
         L.orc_running_sum.argtypes = [ip, C.c_int64, C.c_int32, ip]
@@ -275,6 +276,14 @@ def instrument_noise_aet(grid: Grid, P: float = 15.0, A: float = 3.0, L: float =
     outs = [np.empty(grid.n_bins, dtype=np.float64) for _ in range(4)]
     lib().orc_instrument_noise_aet(C.byref(grid), P, A, L, 1 if tdi2 else 0, *[_d(o) for o in outs])
     return tuple(outs)
+
+
+def channel_sum_noise(sh_aa, sh_tt) -> np.ndarray:
+    """S_sum = 1 / (2 / S_h^AA + 1 / S_h^TT): the noise curve of the SNR summed over A, E, T (eq. 11; R14)."""
+    sh_aa, sh_tt = _f64(sh_aa), _f64(sh_tt)
+    out = np.empty_like(sh_aa)
+    lib().orc_channel_sum_noise(_d(sh_aa), _d(sh_tt), sh_aa.size, _d(out))
+    return out
 
 
 def running_sum_def(x: np.ndarray, window: int, k_begin: int = 0, k_end: int | None = None) -> np.ndarray:

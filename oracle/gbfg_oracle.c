@@ -31,6 +31,7 @@
  *   running median     sort-per-output definition; scipy.ndimage.median_filter(mode='reflect')
  *   snr                closed form for an isolated source; long-double summation; scalings
  *   loop               power conservation; monotone foreground; idempotence; rho_th -> inf, 0+
+ *   channel-sum noise  exact rationals; eq. (11) for an isolated source at 40 digits (R14)
  * parity unpinned: iteration counts / N_res against the paper's Table III
  * and the catalog distribution against the paper's population (different data model,
  * DESIGN.md §3 R0).
@@ -540,6 +541,21 @@ void orc_instrument_noise_aet(const orc_grid *g, double P, double A, double L, i
         if (s_tt) s_tt[k] = o[1];
         if (sh_aa) sh_aa[k] = o[2];
         if (sh_tt) sh_tt[k] = o[3];
+    }
+}
+
+/* Noise curve of the SNR summed over the TDI channels, eq. (11) PAPER.md:159-166 (R14).  In the power domain a
+ * source's strain power p enters channel X with the sky-averaged response R_XX, so that channel's term of eq. (11) is
+ * 4 p R_XX / S^XX = 4 p / S_h^XX; A and E are equal (C3), hence  rho^2 = sum_bins 4 p (2 / S_h^AA + 1 / S_h^TT)
+ * = sum_bins 4 p / S_sum  with  S_sum = 1 / ((2 / S_h^AA) + (1 / S_h^TT)):  the loop run on S_sum as its s_instr is the
+ * channel-summed SNR.  Four IEEE operations per bin, in this order. */
+void orc_channel_sum_noise(const double *sh_aa, const double *sh_tt, int64_t n, double *out)
+{
+    for (int64_t k = 0; k < n; ++k) {
+        double ta = 2.0 / sh_aa[k];
+        double tt = 1.0 / sh_tt[k];
+        double s = ta + tt;
+        out[k] = 1.0 / s;
     }
 }
 

@@ -26,7 +26,7 @@ EXPORTS = [
     "gbfg_subtract_until_converged", "gbfg_simulate", "gbfg_simulate_host", "gbfg_workspace_bytes",
     "gbfg_kernel_launch_count", "gbfg_profile_enable", "gbfg_profile_read", "gbfg_release_cached",
     "gbfg_running_mean", "gbfg_coarse_grain", "gbfg_instrument_noise_aet",
-    "gbfg_sample_catalog_paper", "gbfg_running_median_workspace_bytes",
+    "gbfg_sample_catalog_paper", "gbfg_running_median_workspace_bytes", "gbfg_channel_sum_noise",
 ]
 
 KERNEL_CLASSES = ["sample", "noise", "deposit", "scan", "median", "psd", "inv_blocks", "snr", "aux"]
@@ -94,6 +94,7 @@ def load():
     L.gbfg_grid_init.argtypes = [dbl, dbl, dbl, i32, gp]
     L.gbfg_instrument_noise.argtypes = [gp, vp, vp]
     L.gbfg_instrument_noise_aet.argtypes = [gp, dbl, dbl, dbl, i32, vp, vp, vp, vp, vp]
+    L.gbfg_channel_sum_noise.argtypes = [vp, vp, i64, vp, vp]
     L.gbfg_sample_catalog.argtypes = [gp, pp, op, i32, u32, u64, vp, vp, vp, vp]
     L.gbfg_sample_catalog_paper.argtypes = [gp, C.POINTER(PopPaper), op, i32, u32, u64, vp, vp, vp, vp]
     L.gbfg_deposit.argtypes = [gp, vp, vp, vp, op, i32, vp, vp, i32, vp, vp, vp, sz, vp]
@@ -218,6 +219,10 @@ def instrument_noise_aet(grid: Grid, dev_S_AA=None, dev_S_TT=None, dev_Sh_AA=Non
                          A_fm: float = 3.0, L_m: float = 2.5e9, tdi2: bool = True, stream=None):
     _check(load().gbfg_instrument_noise_aet(C.byref(grid), P_pm, A_fm, L_m, 1 if tdi2 else 0, _ptr(dev_S_AA), _ptr(dev_S_TT),
                                             _ptr(dev_Sh_AA), _ptr(dev_Sh_TT), _stream(stream)))
+
+
+def channel_sum_noise(dev_Sh_AA, dev_Sh_TT, n_bins: int, dev_Sh_sum, stream=None):
+    _check(load().gbfg_channel_sum_noise(_ptr(dev_Sh_AA), _ptr(dev_Sh_TT), n_bins, _ptr(dev_Sh_sum), _stream(stream)))
 
 
 def sample_catalog(grid: Grid, pops, offsets, seed: int, dev_A, dev_f, dev_fdot, first_cat_id: int = 0, stream=None):

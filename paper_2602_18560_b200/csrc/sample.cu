@@ -484,9 +484,40 @@ instrument_noise_aet_kernel(double f_min, double T, int64_t n_bins, double P, do
     }
 }
 
+// S_sum = 1 / ((2 / S_h^AA) + (1 / S_h^TT)): eq. (11) summed over A, E, T in the power domain (R14)
+__global__ void __launch_bounds__(256)
+channel_sum_noise_kernel(const double *__restrict__ sh_aa, const double *__restrict__ sh_tt, int64_t n, double *__restrict__ out)
+{
+    int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int64_t stride = (int64_t)gridDim.x * blockDim.x;
+    for (; k < n; k += stride) {
+        const double ta = 2.0 / sh_aa[k];
+        const double tt = 1.0 / sh_tt[k];
+        const double s = ta + tt;
+        out[k] = 1.0 / s;
+    }
+}
+
 }  // namespace gbfg
 
 using namespace gbfg;
+
+extern "C" int gbfg_channel_sum_noise(const double *dev_Sh_AA, const double *dev_Sh_TT, int64_t n_bins, double *dev_Sh_sum,
+                                      void *stream)
+{
+    if (!dev_Sh_AA || !dev_Sh_TT || !dev_Sh_sum || n_bins < 1) return GBFG_ERR_INVALID_ARG;
+    int rc = check_device();
+    if (rc) return rc;
+    int blocks = (int)((n_bins + 255) / 256);
+    const int cap = sm_count() * 8;
+    if (blocks > cap) blocks = cap;
+    {
+        LaunchTimer lt(K_NOISE, (cudaStream_t)stream);
+        channel_sum_noise_kernel<<<blocks, 256, 0, (cudaStream_t)stream>>>(dev_Sh_AA, dev_Sh_TT, n_bins, dev_Sh_sum);
+    }
+    GBFG_LAUNCH_CHECK("channel_sum_noise_kernel");
+    return GBFG_OK;
+}
 
 extern "C" int gbfg_instrument_noise(const gbfg_grid *grid, double *dev_s_instr, void *stream)
 {

@@ -1251,3 +1251,40 @@ def test_simulate_host_with_pinned_buffers(gb, orc, torch, case):
     gb.simulate_host(g, w.pops, off, w.seed, None, params, h_psd.numpy(), h_res.numpy())
     for c, ref in enumerate(refs):
         assert np.array_equal(bits(h_psd[c].numpy()), bits(ref["psd"])), c
+
+
+# ------------------------------------------------- SNR summed over the TDI channels, eq. (11) (R14)
+def test_channel_summed_snr_loop(gb, orc, torch):
+    """gbfg_channel_sum_noise bit for bit, and the loop on S_sum as its s_instr: every SNR is then the sum over A, E, T of
+    eq. (11).  With three channels instead of the strain-equivalent A channel alone more sources are resolved."""
+    w = wl.dense_case("short")
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    _, _, sh_aa, sh_tt = orc.instrument_noise_aet(og)
+    ref_sum = orc.channel_sum_noise(sh_aa, sh_tt)
+    nb = g.n_bins
+    d = [torch.empty(nb, dtype=torch.float64, device="cuda") for _ in range(3)]
+    gb.instrument_noise_aet(g, dev_Sh_AA=d[0], dev_Sh_TT=d[1])
+    gb.channel_sum_noise(d[0], d[1], nb, d[2])
+    assert np.array_equal(bits(d[2].cpu().numpy()), bits(ref_sum))
+    A, f, fd = orc.sample_catalog(og, w.pops[0], 0, w.seed)
+    spec = np.zeros(nb, dtype=np.int64)
+    orc.deposit(og, A, f, fd, spec)
+    n = A.size
+    outs = {}
+    for name, curve in (("sum", ref_sum), ("aa", sh_aa)):
+        ref_spec = spec.copy()
+        ref = orc.subtract_until_converged(og, A, f, fd, curve, w.window, w.median_norm, w.rho_th, w.max_iter, ref_spec)
+        d_spec = dev(torch, spec)
+        med = torch.empty(nb, dtype=torch.int64, device="cuda")
+        psd = torch.empty(nb, dtype=torch.float64, device="cuda")
+        resolved = torch.zeros(n, dtype=torch.uint8, device="cuda")
+        params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter)
+        res = gb.subtract_until_converged(g, dev(torch, A), dev(torch, f), dev(torch, fd), [0, n], dev(torch, curve), params,
+                                          d_spec, med, psd, resolved, workspace(torch, gb, g, n))[0]
+        assert np.array_equal(d_spec.cpu().numpy(), ref_spec)
+        assert np.array_equal(bits(psd.cpu().numpy()), bits(ref["psd"]))
+        assert np.array_equal(resolved.cpu().numpy(), ref["resolved"])
+        assert (res.n_iter, res.n_resolved) == (ref["n_iter"], ref["n_resolved"])
+        outs[name] = ref["n_resolved"]
+    assert outs["sum"] > outs["aa"]

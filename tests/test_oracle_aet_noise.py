@@ -65,3 +65,40 @@ def test_instrument_noise_aet_array(orc):
         want = orc.aet_noise(w.f_min + (k + 0.5) / w.t_obs)
         assert tuple(a[k] for a in arrs) == want
     assert all(np.all(a > 0) and np.all(np.isfinite(a)) for a in arrs)
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# The SNR summed over the TDI channels, eq. (11), in the power domain (R14)
+# ------------------------------------------------------------------------------------------------------------------
+def test_channel_sum_noise_is_the_harmonic_sum_of_the_channels(orc):
+    """1 / S_sum = 1 / S_h^AA + 1 / S_h^EE + 1 / S_h^TT with E = A (C3), against exact rationals of the inputs."""
+    from fractions import Fraction
+    rng = np.random.default_rng(3)
+    a = 10.0 ** rng.uniform(-41, -36, 500)
+    t = 10.0 ** rng.uniform(-38, -20, 500)
+    s = orc.channel_sum_noise(a, t)
+    for ai, ti, si in zip(a, t, s):
+        exact = 1 / (2 / Fraction(ai) + 1 / Fraction(ti))
+        assert abs(Fraction(si) / exact - 1) < Fraction(4, 2 ** 52)          # four roundings
+    assert np.all(s < a / 2 * (1 + 1e-15))                                   # three channels never do worse than two
+
+
+def test_channel_summed_snr_of_an_isolated_source_is_eq_11(orc):
+    """An isolated one-bin source: rho^2 against S_sum equals the sum over A, E, T of 4 p R_XX / S^XX with the noises and
+    responses of eqs. (C3)-(C4), (B4)-(B5) evaluated at 40 digits as the paper prints them; and the T channel adds next to
+    nothing below a few mHz."""
+    import gbfg_workloads as wl
+    w = wl.config(0)
+    g = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    _, _, sh_aa, sh_tt = orc.instrument_noise_aet(g)
+    s_sum = orc.channel_sum_noise(sh_aa, sh_tt)
+    for f0, A0 in [(3.3e-4, 2e-21), (1.2e-3, 4e-22), (4.7e-3, 1e-22), (9.1e-3, 3e-22)]:
+        st, k0, wdt, we, p, q = orc.source_bins(g, A0, f0, 0.0)
+        assert st == 0 and we == 1
+        got = orc.rho2(g, A0, f0, 0.0, s_sum)
+        fk = mp.mpf(w.f_min) + (mp.mpf(k0) + mp.mpf(1) / 2) / mp.mpf(w.t_obs)
+        s_aa, s_tt, shaa, shtt = _mp_formulas(fk)                            # S^XX and S^XX / R_XX at 40 digits
+        want = 4 * mp.mpf(p) * (2 / shaa + 1 / shtt)                          # = sum_X 4 p R_XX / S^XX, A = E
+        assert abs(mp.mpf(got) / want - 1) < mp.mpf("5e-14"), (f0, got, want)
+        two = orc.rho2(g, A0, f0, 0.0, sh_aa / 2)                             # A and E alone
+        assert 0 <= got / two - 1 < (1e-3 if f0 < 5e-3 else 0.2)
