@@ -492,6 +492,52 @@ def run_stage_bench(args, w: wl.Workload):
     return 0
 
 
+def run_paper_path(args):
+    """`--paper-path`: the path as the paper runs it (Fig. 3) through gbfg_simulate_paper: Lambda of Fig. 1
+     with N_b = 1e7, T_obs = 4 yr, 0.1-10 mHz (Table I), running mean of eq. (D1) over 2001 bins, S_n stop rule
+    at 1e-3, 100 coarse bins (eqs. 13-14).  Prints one JSON line (not the headline metric: another population model)."""
+    import torch
+    import paper_2602_18560_b200 as gb
+    torch.cuda.set_device(0)
+    gb.load()
+    dev = torch.device("cuda", 0)
+    w = wl.Workload(name="paper_fig1_1e7_4yr", t_obs=4 * wl.YEAR_S, f_min=1e-4, f_max=1e-2, window=2001, rho_th=7.0, max_iter=30, seed=7)
+    pop = wl.PaperPopulation(n_src=10_000_000)
+    g = gb.grid_init(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    n, nb = pop.n_src, g.n_bins
+    s_instr = torch.empty(nb, dtype=torch.float64, device=dev)
+    gb.instrument_noise(g, s_instr)
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device=dev) for _ in range(3))
+    spec, stat = (torch.empty(nb, dtype=torch.int64, device=dev) for _ in range(2))
+    psd = torch.empty(nb, dtype=torch.float64, device=dev)
+    resolved = torch.empty(n, dtype=torch.uint8, device=dev)
+    ws = torch.empty(gb.workspace_bytes(g, n, 1), dtype=torch.uint8, device=dev)
+    edges = torch.from_numpy(wl.log_bin_edges(w, 100)).to(dev)
+    S, hc = (torch.empty(100, dtype=torch.float64, device=dev) for _ in range(2))
+    fk = torch.empty(100, dtype=torch.float64, device=dev)
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter, gb.FLAG_ESTIMATOR_MEAN, psd_rtol=1e-3)
+
+    def step():
+        return gb.simulate_paper(g, [pop], [0, n], w.seed, s_instr, params, A, f, fd, None, spec, stat, psd, resolved, ws,
+                                 dev_edges=edges, n_coarse=100, dev_S_coarse=S, dev_f_coarse=fk, dev_hc=hc)
+    for _ in range(max(args.warmup, 1)):
+        res = step()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        res = step()
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / args.steps
+    r = res[0]
+    print(json.dumps({"paper_path": {"ms_per_simulation": ms, "sources_per_s": n / (ms * 1e-3), "n_src": n, "n_bins": nb,
+                                     "estimator": "running mean (eq. D1), 2001 bins", "psd_rtol": 1e-3, "n_iter": r.n_iter,
+                                     "converged": r.converged, "n_resolved": r.n_resolved, "coarse_bins": 100,
+                                     "population": "Fig. 1 parameters of the paper's model (Table I)", "steps": args.steps}}), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -504,6 +550,7 @@ def main():
     ap.add_argument("--max-iter", type=int, default=None, help="override the iteration cap (debug only: cost per iteration)")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--stage-bench", action="store_true", help="time the two PSD estimators alone (one full pass each) and exit")
+    ap.add_argument("--paper-path", action="store_true", help="time gbfg_simulate_paper (the paper's population, mean estimator, S_n stop rule, coarse-grained output) and exit")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-config4", action="store_true",
                     help="also time the oracle on configs[4] (64 catalogs) over all host cores: minutes")
@@ -519,6 +566,8 @@ def main():
         return run_reference(args, w)
     if args.stage_bench:
         return run_stage_bench(args, w)
+    if args.paper_path:
+        return run_paper_path(args)
     return run_gpu(args, w)
 
 

@@ -251,6 +251,19 @@ int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *of
                   uint8_t *dev_resolved, int64_t *dev_err_count, gbfg_iter_result *host_results,
                   void *workspace, size_t workspace_bytes, void *stream);
 
+/* The path as the paper runs it (Fig. 3): the paper's own population model (gbfg_pop_paper, Table I)
+ * -> catalog -> deposit -> loop -> optionally the coarse-grained S_n, mean frequencies and h_c of eqs. (13)-(14), (B1)
+ * (dev_edges / n_coarse / dev_S_coarse / dev_f_coarse / dev_hc as for gbfg_coarse_grain; dev_edges = dev_S_coarse = NULL:
+ * no epilogue).  The paper's production settings are params->flags = GBFG_FLAG_ESTIMATOR_MEAN (eq. D1) and a psd_rtol > 0
+ * (PAPER.md:530, 552).  Everything else as gbfg_simulate. */
+int gbfg_simulate_paper(const gbfg_grid *grid, const gbfg_pop_paper *pops, const int64_t *offsets, int32_t n_cat,
+                        uint64_t seed, const uint32_t *cat_ids, const double *dev_s_instr, const gbfg_iter_params *params,
+                        double *dev_A, double *dev_f, double *dev_fdot,
+                        int64_t *dev_total, int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
+                        uint8_t *dev_resolved, int64_t *dev_err_count, gbfg_iter_result *host_results,
+                        const int64_t *dev_edges, int32_t n_coarse, double *dev_S_coarse, double *dev_f_coarse, double *dev_hc,
+                        void *workspace, size_t workspace_bytes, void *stream);
+
 /* The same path with HOST buffers: the library allocates device memory, copies host_s_instr in,
  * runs gbfg_simulate on its own stream, and copies the PSD ([n_cat][n_bins] binary64) and the
  * resolved flags ([N] uint8, may be NULL) back.  host_s_instr == NULL: the curve of gbfg_instrument_noise

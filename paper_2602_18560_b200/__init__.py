@@ -26,7 +26,7 @@ EXPORTS = [
     "gbfg_subtract_until_converged", "gbfg_simulate", "gbfg_simulate_host", "gbfg_workspace_bytes",
     "gbfg_kernel_launch_count", "gbfg_profile_enable", "gbfg_profile_read", "gbfg_release_cached",
     "gbfg_running_mean", "gbfg_coarse_grain", "gbfg_instrument_noise_aet",
-    "gbfg_sample_catalog_paper", "gbfg_running_median_workspace_bytes", "gbfg_channel_sum_noise",
+    "gbfg_sample_catalog_paper", "gbfg_running_median_workspace_bytes", "gbfg_channel_sum_noise", "gbfg_simulate_paper",
 ]
 
 KERNEL_CLASSES = ["sample", "noise", "deposit", "scan", "median", "psd", "inv_blocks", "snr", "aux"]
@@ -107,6 +107,8 @@ def load():
     L.gbfg_snr_select.argtypes = [gp, vp, vp, vp, op, i32, vp, dbl, vp, vp, vp, vp, vp, vp, sz, vp]
     L.gbfg_subtract_until_converged.argtypes = [gp, vp, vp, vp, op, i32, vp, ip, vp, vp, vp, vp, rp, vp, sz, vp]
     L.gbfg_simulate.argtypes = [gp, pp, op, i32, u64, C.POINTER(u32), vp, ip, vp, vp, vp, vp, vp, vp, vp, vp, vp, rp, vp, sz, vp]
+    L.gbfg_simulate_paper.argtypes = [gp, C.POINTER(PopPaper), op, i32, u64, C.POINTER(u32), vp, ip, vp, vp, vp, vp, vp, vp, vp, vp, vp,
+                                      rp, vp, i32, vp, vp, vp, vp, sz, vp]
     L.gbfg_simulate_host.argtypes = [gp, pp, op, i32, u64, C.POINTER(u32), vp, ip, vp, vp, rp]
     L.gbfg_profile_enable.argtypes = [C.c_int]
     L.gbfg_profile_read.argtypes = [C.POINTER(KernelTime), i32]
@@ -306,6 +308,22 @@ def simulate(grid: Grid, pops, offsets, seed: int, dev_s_instr, params: IterPara
         _ptr(dev_A), _ptr(dev_f), _ptr(dev_fdot), _ptr(dev_total), _ptr(dev_spectrum), _ptr(dev_median),
         _ptr(dev_psd), _ptr(dev_resolved), _ptr(dev_err_count), res, _ptr(workspace),
         workspace.numel() * workspace.element_size(), _stream(stream)))
+    return list(res)
+
+
+def simulate_paper(grid: Grid, pops, offsets, seed: int, dev_s_instr, params: IterParams, dev_A, dev_f, dev_fdot,
+                   dev_total, dev_spectrum, dev_median, dev_psd, dev_resolved, workspace, dev_edges=None, n_coarse: int = 0,
+                   dev_S_coarse=None, dev_f_coarse=None, dev_hc=None, dev_err_count=None, stream=None, cat_ids=None):
+    n_cat = len(offsets) - 1
+    res = (IterResult * n_cat)()
+    arr = (PopPaper * len(pops))()
+    for i, p in enumerate(pops):
+        arr[i] = p if isinstance(p, PopPaper) else make_pop_paper(p)
+    _check(load().gbfg_simulate_paper(
+        C.byref(grid), arr, _offsets(offsets), n_cat, seed, _cat_ids(cat_ids, n_cat), _ptr(dev_s_instr), C.byref(params),
+        _ptr(dev_A), _ptr(dev_f), _ptr(dev_fdot), _ptr(dev_total), _ptr(dev_spectrum), _ptr(dev_median), _ptr(dev_psd),
+        _ptr(dev_resolved), _ptr(dev_err_count), res, _ptr(dev_edges), n_coarse, _ptr(dev_S_coarse), _ptr(dev_f_coarse),
+        _ptr(dev_hc), _ptr(workspace), workspace.numel() * workspace.element_size(), _stream(stream)))
     return list(res)
 
 

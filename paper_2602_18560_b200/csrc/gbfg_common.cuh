@@ -21,6 +21,9 @@ int check_device();                                     // GBFG_OK or GBFG_ERR_A
 void count_launch(int n = 1);
 int sm_count();
 // stage (i) with explicit catalog ids (sample.cu): cat_ids HOST [n_cat] or NULL (first_cat_id + c)
+int sample_catalog_paper_ids(const gbfg_grid *grid, const gbfg_pop_paper *pops, const int64_t *offsets, int32_t n_cat,
+                             uint32_t first_cat_id, const uint32_t *cat_ids, uint64_t seed,
+                             double *dev_A, double *dev_f, double *dev_fdot, void *stream);
 struct SampleDeposit;       // != NULL: every source is also deposited by the kernel that draws it (gbfg_simulate)
 int sample_catalog_ids(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
                        uint32_t first_cat_id, const uint32_t *cat_ids, uint64_t seed,

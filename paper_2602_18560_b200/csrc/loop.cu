@@ -783,6 +783,44 @@ extern "C" int gbfg_simulate(const gbfg_grid *grid, const gbfg_pop *pops, const 
                                         workspace, workspace_bytes, stream), (cudaStream_t)stream);
 }
 
+// The path as the paper runs it (Fig. 3): Lambda of the paper's own population model -> catalog ->
+// deposit -> loop (typically with the running mean of eq. D1 and the S_n stop rule) -> coarse-grained S_n and h_c.
+extern "C" int gbfg_simulate_paper(const gbfg_grid *grid, const gbfg_pop_paper *pops, const int64_t *offsets, int32_t n_cat,
+                                   uint64_t seed, const uint32_t *cat_ids, const double *dev_s_instr,
+                                   const gbfg_iter_params *params, double *dev_A, double *dev_f, double *dev_fdot,
+                                   int64_t *dev_total, int64_t *dev_spectrum, int64_t *dev_median, double *dev_psd,
+                                   uint8_t *dev_resolved, int64_t *dev_err_count, gbfg_iter_result *host_results,
+                                   const int64_t *dev_edges, int32_t n_coarse, double *dev_S_coarse, double *dev_f_coarse,
+                                   double *dev_hc, void *workspace, size_t workspace_bytes, void *stream)
+{
+    int rc = loop_validate(grid, params);
+    if (rc) return rc;
+    if (!offsets || n_cat < 1 || !dev_s_instr || !dev_spectrum || !dev_median || !dev_psd || !dev_resolved || !host_results)
+        return GBFG_ERR_INVALID_ARG;
+    if ((dev_edges != nullptr) != (dev_S_coarse != nullptr) || (dev_edges && n_coarse < 1)) return GBFG_ERR_INVALID_ARG;
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = sample_catalog_paper_ids(grid, pops, offsets, n_cat, 0u, cat_ids, seed, dev_A, dev_f, dev_fdot, stream);
+    if (rc) return rc;
+    const int64_t n = offsets[n_cat];
+    const size_t row_bytes = sizeof(int64_t) * (size_t)n_cat * (size_t)grid->n_bins;
+    GBFG_CUDA(cudaMemsetAsync(dev_spectrum, 0, row_bytes, st));
+    if (n > 0) GBFG_CUDA(cudaMemsetAsync(dev_resolved, 0, (size_t)n, st));
+    rc = gbfg_deposit(grid, dev_A, dev_f, dev_fdot, offsets, n_cat, nullptr, nullptr, +1, dev_spectrum, dev_err_count,
+                      workspace, workspace_bytes, stream);
+    if (rc) return rc;
+    if (dev_total) GBFG_CUDA(cudaMemcpyAsync(dev_total, dev_spectrum, row_bytes, cudaMemcpyDeviceToDevice, st));
+    rc = loop_impl(grid, dev_A, dev_f, dev_fdot, offsets, n_cat, dev_s_instr, params, dev_spectrum, dev_median, dev_psd,
+                   dev_resolved, host_results, workspace, workspace_bytes, stream, false);
+    if (rc) return rc;
+    if (dev_edges) {                                        // eqs. (13)-(14), (B1): the datum the inference works with
+        rc = gbfg_coarse_grain(dev_psd, grid->n_bins, n_cat, dev_edges, n_coarse, grid->f_min, grid->t_obs, dev_S_coarse,
+                               dev_f_coarse, dev_hc, stream);
+        if (rc) return rc;
+        GBFG_CUDA(cudaStreamSynchronize(st));
+    }
+    return GBFG_OK;
+}
+
 extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, const int64_t *offsets, int32_t n_cat,
                                   uint64_t seed, const uint32_t *cat_ids, const double *host_s_instr, const gbfg_iter_params *params,
                                   double *host_psd, uint8_t *host_resolved, gbfg_iter_result *host_results)

@@ -556,9 +556,10 @@ extern "C" int gbfg_instrument_noise_aet(const gbfg_grid *grid, double P_pm, dou
     return GBFG_OK;
 }
 
-extern "C" int gbfg_sample_catalog_paper(const gbfg_grid *grid, const gbfg_pop_paper *pops, const int64_t *offsets,
-                                         int32_t n_cat, uint32_t first_cat_id, uint64_t seed,
-                                         double *dev_A, double *dev_f, double *dev_fdot, void *stream)
+// cat_ids (HOST [n_cat], nullable): Philox counter word 3 of catalog c; NULL: first_cat_id + c
+int gbfg::sample_catalog_paper_ids(const gbfg_grid *grid, const gbfg_pop_paper *pops, const int64_t *offsets,
+                                   int32_t n_cat, uint32_t first_cat_id, const uint32_t *cat_ids, uint64_t seed,
+                                   double *dev_A, double *dev_f, double *dev_fdot, void *stream)
 {
     if (!grid || grid->struct_size != sizeof(gbfg_grid) || !pops || !offsets) return GBFG_ERR_INVALID_ARG;
     if (n_cat < 1) return GBFG_ERR_INVALID_ARG;
@@ -596,7 +597,7 @@ extern "C" int gbfg_sample_catalog_paper(const gbfg_grid *grid, const gbfg_pop_p
         P.mu = p.mu; P.sigma = p.sigma; P.rho = p.rho; P.rho_c = sqrt(1.0 - p.rho * p.rho);
         P.f_min = grid->f_min; P.f_max = grid->f_max; P.f_top = nextafter(grid->f_max, 0.0);
         P.n_src = p.n_src;
-        P.cat_id = first_cat_id + (uint32_t)c;
+        P.cat_id = cat_ids ? cat_ids[c] : first_cat_id + (uint32_t)c;
         P.key0 = (uint32_t)seed; P.key1 = (uint32_t)(seed >> 32);
         int64_t blocks = (p.n_src + 127) / 128;
         const int64_t cap = (int64_t)sm_count() * 16;
@@ -609,6 +610,13 @@ extern "C" int gbfg_sample_catalog_paper(const gbfg_grid *grid, const gbfg_pop_p
         GBFG_LAUNCH_CHECK("sample_paper_kernel");
     }
     return GBFG_OK;
+}
+
+extern "C" int gbfg_sample_catalog_paper(const gbfg_grid *grid, const gbfg_pop_paper *pops, const int64_t *offsets,
+                                         int32_t n_cat, uint32_t first_cat_id, uint64_t seed,
+                                         double *dev_A, double *dev_f, double *dev_fdot, void *stream)
+{
+    return sample_catalog_paper_ids(grid, pops, offsets, n_cat, first_cat_id, nullptr, seed, dev_A, dev_f, dev_fdot, stream);
 }
 
 // cat_ids (HOST [n_cat], nullable): Philox counter word 3 of catalog c; NULL: first_cat_id + c

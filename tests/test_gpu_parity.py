@@ -1288,3 +1288,49 @@ def test_channel_summed_snr_loop(gb, orc, torch):
         assert (res.n_iter, res.n_resolved) == (ref["n_iter"], ref["n_resolved"])
         outs[name] = ref["n_resolved"]
     assert outs["sum"] > outs["aa"]
+
+
+# ------------------------------------------------- the path as the paper runs it
+@pytest.mark.parametrize("estimator,tol", [(1, 2e-3), (0, 0.0)])
+def test_simulate_paper_population_to_coarse_grained_psd(gb, orc, torch, estimator, tol):
+    """gbfg_simulate_paper: Lambda of Table I -> catalog -> deposit -> loop -> coarse-grained S_n, f and h_c (eqs. 13-14, B1),
+    two catalogs in one call, with the paper's production settings (running mean of eq. D1 + the S_n stop rule) and with
+    the running median; against the oracle's stages run catalog by catalog."""
+    w = wl.replace(wl.config(1), max_iter=10)
+    g = gpu_grid(gb, w)
+    og = orc.make_grid(w.f_min, w.f_max, w.t_obs, w.scale_log2)
+    pops = [wl.PaperPopulation(n_src=150_000), wl.replace(wl.paper_prior_draw(5, n_src=90_001), mu=-21.6)]
+    off = np.concatenate([[0], np.cumsum([p.n_src for p in pops])]).astype(np.int64)
+    n, nb, nc = int(off[-1]), g.n_bins, len(pops)
+    s_instr_h = orc.instrument_noise(og)
+    edges = wl.log_bin_edges(w, 100, 1e-4, 1e-2)
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    total, spec, stat = (torch.empty((nc, nb), dtype=torch.int64, device="cuda") for _ in range(3))
+    psd = torch.empty((nc, nb), dtype=torch.float64, device="cuda")
+    resolved = torch.empty(n, dtype=torch.uint8, device="cuda")
+    S = torch.empty((nc, 100), dtype=torch.float64, device="cuda")
+    hc = torch.empty((nc, 100), dtype=torch.float64, device="cuda")
+    fk = torch.empty(100, dtype=torch.float64, device="cuda")
+    flags = gb.FLAG_ESTIMATOR_MEAN if estimator else 0
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter, flags, psd_rtol=tol)
+    res = gb.simulate_paper(g, pops, off, 9, dev(torch, s_instr_h), params, A, f, fd, total, spec, stat, psd, resolved,
+                            workspace(torch, gb, g, n, nc), dev_edges=dev(torch, edges), n_coarse=100, dev_S_coarse=S,
+                            dev_f_coarse=fk, dev_hc=hc, cat_ids=[0, 1])
+    for c, p in enumerate(pops):
+        rA, rf, rfd = orc.sample_catalog_paper(og, p, c, 9)
+        s = slice(int(off[c]), int(off[c + 1]))
+        assert np.array_equal(bits(A[s].cpu().numpy()), bits(rA))
+        ref_spec = np.zeros(nb, dtype=np.int64)
+        orc.deposit(og, rA, rf, rfd, ref_spec)
+        assert np.array_equal(total[c].cpu().numpy(), ref_spec)
+        ref = orc.subtract_until_converged(og, rA, rf, rfd, s_instr_h, w.window, w.median_norm, w.rho_th, w.max_iter, ref_spec,
+                                           estimator=estimator, psd_rtol=tol)
+        assert np.array_equal(spec[c].cpu().numpy(), ref_spec)
+        assert np.array_equal(stat[c].cpu().numpy(), ref["median"])
+        assert np.array_equal(bits(psd[c].cpu().numpy()), bits(ref["psd"]))
+        assert np.array_equal(resolved[s].cpu().numpy(), ref["resolved"])
+        assert (res[c].n_iter, res[c].converged, res[c].n_resolved) == (ref["n_iter"], ref["converged"], ref["n_resolved"])
+        S_ref, f_ref, hc_ref = orc.coarse_grain(ref["psd"], edges, w.f_min, w.t_obs)
+        assert np.allclose(S[c].cpu().numpy(), S_ref, rtol=COARSE_RTOL, atol=0, equal_nan=True)
+        assert np.allclose(hc[c].cpu().numpy(), hc_ref, rtol=COARSE_RTOL, atol=0, equal_nan=True)
+        assert np.allclose(fk.cpu().numpy(), f_ref, rtol=1e-15, atol=0, equal_nan=True)
