@@ -23,7 +23,7 @@
 
 namespace gbfg {
 
-constexpr int SNR_NARROW = 8;
+constexpr int SNR_NARROW = 4;
 constexpr int SNR_SEL_CAP = 1024;              // selected indices a CTA holds before it appends them to the list
 constexpr int PFX_THREADS = 512;
 constexpr int PFX_ITEMS = 4;
