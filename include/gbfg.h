@@ -42,7 +42,8 @@ typedef enum gbfg_status {
     GBFG_ERR_WORKSPACE = -2,   /* workspace NULL or smaller than gbfg_workspace_bytes() */
     GBFG_ERR_CUDA = -3,        /* a CUDA runtime call failed: see gbfg_last_cuda_error() */
     GBFG_ERR_ARCH = -4,        /* current device is not compute capability 10.x */
-    GBFG_ERR_UNSUPPORTED = -5  /* window wider than GBFG_MAX_WINDOW, n_cat > GBFG_MAX_CAT, alpha_gamma outside its stated range */
+    GBFG_ERR_UNSUPPORTED = -5, /* window wider than GBFG_MAX_WINDOW, n_cat > GBFG_MAX_CAT, alpha_gamma outside its stated range */
+    GBFG_ERR_STATIC_LIMIT = -6 /* gbfg_running_median_static: the call needs more scratch than GBFG_STATIC_SCRATCH_BYTES */
 } gbfg_status;
 
 #define GBFG_MAX_CAT 256        /* catalogs per batched call */
@@ -182,6 +183,22 @@ int gbfg_deposit(const gbfg_grid *grid, const double *dev_A, const double *dev_f
 int gbfg_running_median(const int64_t *dev_spectrum, int64_t n_bins, int32_t n_cat, int32_t window,
                         int64_t *dev_median_out, void *workspace, size_t workspace_bytes, void *stream);
 size_t gbfg_running_median_workspace_bytes(int64_t n_bins, int32_t n_cat, int32_t window);   /* 0: invalid arguments */
+
+/* gbfg_running_median for callers that must not allocate and have no workspace to hand in (CUDA graph capture, serving
+ * loops, harnesses that forbid cudaMalloc): same operation, same arguments without the workspace, same results to the
+ * bit.  The scratch the kernels need (the list of tiles the 32-bit-key kernel leaves to the 64-bit-key one: 256 bytes of
+ * counters + 16 bytes per tile) lives in ONE array of GBFG_STATIC_SCRATCH_BYTES in the library's device image: every
+ * device that loads the library holds it until the process exits.  A call that needs more (more than
+ * GBFG_STATIC_MAX_TILES tiles over all rows; a tile is at most 8704 - (window - 1) outputs, so 4.3e8 outputs at
+ * window 2001) returns GBFG_ERR_STATIC_LIMIT and launches nothing: use gbfg_running_median.  The call allocates nothing
+ * (no cudaMalloc / cudaFree, no allocating library routine; the array's device address is looked up once per device).
+ * The array is shared by every call and keeps the last call's contents; the counters are cleared on the stream at the
+ * start of each call.  Calls that may OVERLAP on the GPU (two streams, two host threads, two captured graphs running
+ * side by side) race on it: order them, or use gbfg_running_median with a workspace each. */
+#define GBFG_STATIC_SCRATCH_BYTES (1 << 20)
+#define GBFG_STATIC_MAX_TILES ((GBFG_STATIC_SCRATCH_BYTES - 256) / 16)
+int gbfg_running_median_static(const int64_t *dev_spectrum, int64_t n_bins, int32_t n_cat, int32_t window,
+                               int64_t *dev_median_out, void *stream);
 
 /* Running-mean estimator of eq. (D1), PAPER.md:538 (the paper's production choice, :176, :552; R8):
  * sum_out[c][k] = sum of x[c][k-h .. k+h], W = 2h+1 odd, ends reflected as for the median (the exact

@@ -27,6 +27,7 @@ EXPORTS = [
     "gbfg_kernel_launch_count", "gbfg_profile_enable", "gbfg_profile_read", "gbfg_release_cached",
     "gbfg_running_mean", "gbfg_coarse_grain", "gbfg_instrument_noise_aet",
     "gbfg_sample_catalog_paper", "gbfg_running_median_workspace_bytes", "gbfg_channel_sum_noise", "gbfg_simulate_paper",
+    "gbfg_running_median_static",
 ]
 
 KERNEL_CLASSES = ["sample", "noise", "deposit", "scan", "median", "psd", "inv_blocks", "snr", "aux"]
@@ -99,6 +100,7 @@ def load():
     L.gbfg_sample_catalog_paper.argtypes = [gp, C.POINTER(PopPaper), op, i32, u32, u64, vp, vp, vp, vp]
     L.gbfg_deposit.argtypes = [gp, vp, vp, vp, op, i32, vp, vp, i32, vp, vp, vp, sz, vp]
     L.gbfg_running_median.argtypes = [vp, i64, i32, i32, vp, vp, sz, vp]
+    L.gbfg_running_median_static.argtypes = [vp, i64, i32, i32, vp, vp]
     L.gbfg_running_median_workspace_bytes.restype = sz
     L.gbfg_running_median_workspace_bytes.argtypes = [i64, i32, i32]
     L.gbfg_psd.argtypes = [vp, vp, i64, i32, dbl, i32, vp, vp]
@@ -252,6 +254,17 @@ def running_median(dev_spectrum, n_bins: int, n_cat: int, window: int, dev_media
                                 device=dev_spectrum.device)
     _check(load().gbfg_running_median(_ptr(dev_spectrum), n_bins, n_cat, window, _ptr(dev_median_out), _ptr(workspace),
                                       workspace.numel() * workspace.element_size(), _stream(stream)))
+
+
+STATIC_SCRATCH_BYTES = 1 << 20                       # GBFG_STATIC_SCRATCH_BYTES
+STATIC_MAX_TILES = (STATIC_SCRATCH_BYTES - 256) // 16  # GBFG_STATIC_MAX_TILES
+
+
+def running_median_static(dev_spectrum, n_bins: int, n_cat: int, window: int, dev_median_out, stream=None):
+    """gbfg_running_median_static: no workspace, no allocation (the scratch is a static array in the library's device
+    image); GbfgError(-6) beyond STATIC_MAX_TILES tiles.  Calls that overlap on the GPU race on the shared array."""
+    _check(load().gbfg_running_median_static(_ptr(dev_spectrum), n_bins, n_cat, window, _ptr(dev_median_out),
+                                             _stream(stream)))
 
 
 def running_mean(dev_spectrum, n_bins: int, n_cat: int, window: int, dev_sum_out, dev_s_instr=None,

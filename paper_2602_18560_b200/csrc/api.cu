@@ -92,6 +92,7 @@ extern "C" const char *gbfg_strerror(int status)
     case GBFG_ERR_CUDA: return "CUDA runtime error (see gbfg_last_cuda_error)";
     case GBFG_ERR_ARCH: return "device is not compute capability 10.x (sm_100)";
     case GBFG_ERR_UNSUPPORTED: return "unsupported size or parameter (window > GBFG_MAX_WINDOW, n_cat > GBFG_MAX_CAT, alpha_gamma outside its stated range)";
+    case GBFG_ERR_STATIC_LIMIT: return "the call needs more scratch than the library's static array holds (GBFG_STATIC_SCRATCH_BYTES): use the variant that takes a workspace";
     default: return "unknown status";
     }
 }

@@ -22,6 +22,8 @@
 //     Plateaus left by wide chirps (long stretches of out-of-window ranks) cost one step per 32 ranks.
 // The per-output rank is kept in shared memory and written out coalesced, fused with
 //     psd[k] = s_instr[k] + C * (med[k] * 2^scale_log2)        (eqs. 10, D2, D3).
+#include <mutex>
+
 #include "median_kernel.cuh"
 
 namespace gbfg {
@@ -377,6 +379,72 @@ extern "C" int gbfg_running_median(const int64_t *dev_spectrum, int64_t n_bins, 
     char *tmp = (char *)workspace;
     return launch_median(dev_spectrum, n_bins, n_cat, window, dev_median_out, nullptr, nullptr, 1.0, 0, nullptr,
                          (int4 *)(tmp + 256), (int *)tmp, nullptr, nullptr, (cudaStream_t)stream);
+}
+
+// ---- gbfg_running_median_static: the same two kernels with the wide list in a file-scope device array, for callers that
+// cannot allocate and have no workspace.  In host code the array's name is a host-side stand-in, not a device address
+// (a kernel handed it would fault, or use the wrong memory): the address comes from cudaGetSymbolAddress, once per
+// device, with that device current.  Every call shares the array; calls that overlap on the GPU race (include/gbfg.h).
+static __device__ __align__(256) unsigned char g_median_static_scratch[GBFG_STATIC_SCRATCH_BYTES];
+
+static int median_static_setup(void **scratch)
+{
+    static std::mutex mu;
+    static void *ptr_of[64];                             // the array's address on each device
+    int dev = 0;
+    GBFG_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return GBFG_ERR_ARCH;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr_of[dev]) {
+        void *ptr = nullptr;
+        GBFG_CUDA(cudaGetSymbolAddress(&ptr, g_median_static_scratch));
+        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint32_t, 512, MED_LT32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)median_smem_bytes<uint32_t, 512, MED_LT32>()));
+        GBFG_CUDA(cudaFuncSetAttribute(running_median_tile_kernel<uint64_t, 1024, MED_LT64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)median_smem_bytes<uint64_t, 1024, MED_LT64>()));
+        ptr_of[dev] = ptr;
+    }
+    *scratch = ptr_of[dev];
+    return GBFG_OK;
+}
+
+extern "C" int gbfg_running_median_static(const int64_t *dev_spectrum, int64_t n_bins, int32_t n_cat, int32_t window,
+                                          int64_t *dev_median_out, void *stream)
+{
+    if (!dev_spectrum || !dev_median_out || dev_spectrum == dev_median_out) return GBFG_ERR_INVALID_ARG;
+    if (window < 1 || (window & 1) == 0 || n_cat < 1 || n_bins < 1 || n_bins >= 2147483648ll) return GBFG_ERR_INVALID_ARG;
+    if (window > GBFG_MAX_WINDOW || n_cat > GBFG_MAX_CAT) return GBFG_ERR_UNSUPPORTED;
+    if (n_bins < window / 2 + 1) return GBFG_ERR_INVALID_ARG;
+    int rc = check_device();
+    if (rc) return rc;
+    MedianArgs a;
+    a.tiles = median_static_tiles(n_bins, n_cat, window, &a.S);
+    if ((int64_t)a.tiles * n_cat > (int64_t)GBFG_STATIC_MAX_TILES) return GBFG_ERR_STATIC_LIMIT;     // nothing launched
+    void *scratch = nullptr;
+    rc = median_static_setup(&scratch);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    a.x = dev_spectrum; a.med = dev_median_out; a.s_instr = nullptr; a.psd = nullptr; a.neg_flag = nullptr; a.delta_bits = nullptr;
+    a.items = nullptr; a.ctr = nullptr; a.n_cat = n_cat;
+    a.wide_ctr = (int *)scratch;                         // [0] tiles in the list, [1] the consumers' ticket
+    a.wide_items = (int4 *)((char *)scratch + 256);
+    a.n = n_bins; a.h = window / 2;
+    a.norm = 1.0; a.scale = 1.0;
+    // the array keeps the last call's contents: the two counters start at zero, the list is written before it is read
+    GBFG_CUDA(cudaMemsetAsync(a.wide_ctr, 0, 2 * sizeof(int), st));
+    const int sms = sm_count();
+    int64_t grid = (int64_t)a.tiles * n_cat;
+    if (grid > 2 * sms) grid = 2 * sms;
+    running_median_tile_kernel<uint32_t, 512, MED_LT32, false><<<(int)grid, 512, median_smem_bytes<uint32_t, 512, MED_LT32>(), st>>>(a);
+    GBFG_LAUNCH_CHECK("running_median_tile_kernel<u32> (static scratch)");
+    a.items = a.wide_items; a.ctr = a.wide_ctr;
+    a.wide_items = nullptr; a.wide_ctr = nullptr;
+    if (grid > sms) grid = sms;
+    cudaError_t e = launch_dependent(running_median_tile_kernel<uint64_t, 1024, MED_LT64, false>, dim3((unsigned)grid), dim3(1024),
+                                     median_smem_bytes<uint64_t, 1024, MED_LT64>(), st, a);
+    if (e != cudaSuccess) return set_cuda_error(e, "running_median_tile_kernel<u64> (static scratch)");
+    GBFG_LAUNCH_CHECK("running_median_tile_kernel<u64> (static scratch)");
+    return GBFG_OK;
 }
 
 extern "C" int gbfg_psd(const int64_t *dev_median, const double *dev_s_instr, int64_t n_bins, int32_t n_cat,

@@ -53,8 +53,9 @@ def test_version_and_strerror(gbcpu):
     L = gbcpu.load()
     assert L.gbfg_version() >= 100
     assert L.gbfg_strerror(0) == b"ok"
-    for code in (-1, -2, -3, -4, -5):
+    for code in (-1, -2, -3, -4, -5, -6):
         assert len(L.gbfg_strerror(code)) > 3
+    assert b"static" in L.gbfg_strerror(-6)
     assert L.gbfg_strerror(-77) == b"unknown status"
 
 
