@@ -304,12 +304,32 @@ int median_static_tiles(int64_t n_bins, int n_cat, int window, int *S_out)
     return (int)((n_bins + S - 1) / S);
 }
 
+#ifdef MED_TIMING
+// probe builds (-DMED_TIMING): clocks per phase of the tile loop, [CTA][16], summed over the CTA's tiles and over the
+// launches since the last read
+static long long *median_timing_words()
+{
+    static long long *p = nullptr;
+    if (!p) { cudaMalloc(&p, 1024 * 16 * sizeof(long long)); cudaMemset(p, 0, 1024 * 16 * sizeof(long long)); }
+    return p;
+}
+extern "C" void gbfg_debug_median_timing(long long *out, int n_cta)
+{
+    cudaDeviceSynchronize();
+    cudaMemcpy(out, median_timing_words(), (size_t)n_cta * 16 * sizeof(long long), cudaMemcpyDeviceToHost);
+    cudaMemset(median_timing_words(), 0, 1024 * 16 * sizeof(long long));
+}
+#endif
+
 int launch_median(const int64_t *x, int64_t n_bins, int n_cat, int window, int64_t *med,
                   const double *s_instr, double *psd, double norm, int scale_log2,
                   const MedianPlan *plan, int4 *wide_items, int *wide_ctr, int *neg_flag,
                   unsigned long long *delta_bits, cudaStream_t st)
 {
     MedianArgs a;
+#ifdef MED_TIMING
+    a.dbg = median_timing_words();
+#endif
     a.delta_bits = delta_bits;
     a.x = x; a.med = med; a.s_instr = s_instr; a.psd = psd; a.neg_flag = neg_flag;
     a.items = plan ? plan->items : nullptr; a.ctr = plan ? plan->ctr : nullptr; a.n_cat = n_cat;
@@ -418,6 +438,9 @@ extern "C" int gbfg_running_median_static(const int64_t *dev_spectrum, int64_t n
     int rc = check_device();
     if (rc) return rc;
     MedianArgs a;
+#ifdef MED_TIMING
+    a.dbg = median_timing_words();
+#endif
     a.tiles = median_static_tiles(n_bins, n_cat, window, &a.S);
     if ((int64_t)a.tiles * n_cat > (int64_t)GBFG_STATIC_MAX_TILES) return GBFG_ERR_STATIC_LIMIT;     // nothing launched
     void *scratch = nullptr;

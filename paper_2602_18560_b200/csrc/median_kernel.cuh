@@ -23,6 +23,9 @@ constexpr int MED_PB = 32;                    // outputs per chunk (one per lane
 #ifndef MED_MLP
 #define MED_MLP 4                             // global loads a thread keeps in flight while it stages a tile / writes it out
 #endif
+#ifndef MED_MATCH_EVERY
+#define MED_MATCH_EVERY 3                     // sort rounds whose peer masks come from MATCH.ANY: one in this many
+#endif
 constexpr int MED_CROW = 256 + 2;             // radix counter row stride in u16 (one row per warp)
 constexpr uint64_t SIGN64 = 0x8000000000000000ull;
 
@@ -32,7 +35,7 @@ __host__ __device__ constexpr int median_aux_u16(int threads, int lt)
 {
     const int warps = threads / 32;
     const int sort_u16 = warps * MED_CROW;
-    const int walk_u16 = 2 * warps * (lt / 32) * 2;                   // window and specials bitmaps
+    const int walk_u16 = 2 * warps * (lt / 32 + 1) * 2;               // window and specials bitmaps, rows of lt / 32 + 1 words
     return sort_u16 > walk_u16 ? sort_u16 : walk_u16;
 }
 
@@ -107,11 +110,33 @@ __device__ __forceinline__ unsigned same_digit_lanes(unsigned d)
     const unsigned me = 1u << (threadIdx.x & 31);
 #pragma unroll
     for (int b = 0; b < 8; ++b) {
-        const bool bit = (d >> b) & 1u;
-        const unsigned bal = __reduce_or_sync(0xffffffffu, bit ? me : 0u);     // a ballot; REDUX retires a little faster than VOTE here
-        peers &= bit ? bal : ~bal;
+        const unsigned sb = (unsigned)((int)(d << (31 - b)) >> 31);            // all ones when bit b of the digit is set
+        const unsigned bal = __reduce_or_sync(0xffffffffu, me & sb);           // a ballot; REDUX retires a little faster than VOTE here
+        peers &= ~(bal ^ sb);                                                  // bit set: & bal, clear: & ~bal
     }
     return peers;
+}
+
+// 32 x 32 bit matrix, row i in lane i -> column j in lane j (bit i of the result of lane j = bit j of the value of
+// lane i): five butterfly steps, each one shuffle
+template <int K, unsigned M>
+__device__ __forceinline__ unsigned transpose_bits_step(unsigned v, int lane)
+{
+    const unsigned x = __shfl_xor_sync(0xffffffffu, v, K);
+    const bool upper = lane & K;
+    const unsigned xs = upper ? (x >> K) : (x << K);
+    const unsigned take = upper ? M : ~M;                                      // the bits that come from the partner
+    return (v & ~take) | (xs & take);
+}
+__device__ __forceinline__ unsigned transpose_bits_32(unsigned v)
+{
+    const int lane = threadIdx.x & 31;
+    v = transpose_bits_step<16, 0x0000ffffu>(v, lane);
+    v = transpose_bits_step<8, 0x00ff00ffu>(v, lane);
+    v = transpose_bits_step<4, 0x0f0f0f0fu>(v, lane);
+    v = transpose_bits_step<2, 0x33333333u>(v, lane);
+    v = transpose_bits_step<1, 0x55555555u>(v, lane);
+    return v;
 }
 
 // DELTA: also record the largest relative PSD change (the second stop rule, R13); a template parameter so
@@ -289,7 +314,7 @@ running_median_tile_kernel(MedianArgs a)
                 k[r] = skey[e];
                 // every third round by MATCH.ANY, the others by eight reductions: the two run on different units of the
                 // SM (one MATCH per ~50 clocks, ~50 issue slots for the reductions), so the mix beats either alone
-                pk[r] = (r % 3 == 0) ? __match_any_sync(FULL, (unsigned)(k[r] >> shift) & 255u)
+                pk[r] = (r % MED_MATCH_EVERY == 0) ? __match_any_sync(FULL, (unsigned)(k[r] >> shift) & 255u)
                                      : same_digit_lanes((unsigned)(k[r] >> shift) & 255u);
             }
         }
@@ -372,22 +397,37 @@ running_median_tile_kernel(MedianArgs a)
         const int cpw = (n_coarse + WARPS - 1) / WARPS;
         const int c_first = warp * cpw;
         const int c_last = (c_first + cpw < n_coarse) ? c_first + cpw : n_coarse;
-        unsigned *bm = aux32 + warp * (LT / 32);
-        unsigned *sp = aux32 + (WARPS + warp) * (LT / 32);
+        constexpr int BMW = LT / 32 + 1;                         // words per bitmap row (odd: rows start on different banks)
+        unsigned *bm = aux32 + warp * BMW;
+        unsigned *sp = aux32 + (WARPS + warp) * BMW;
         const int nw = LTe / 32;
         const uint32_t bm_a = (uint32_t)__cvta_generic_to_shared(bm), sp_a = (uint32_t)__cvta_generic_to_shared(sp);
         {
-            const int wstep = cpw * MED_PB;                      // first output of warp w2: w2 * wstep
+            // Position p lies in the first window of warp w2 iff w2 wstep <= p < w2 wstep + W (wstep = the outputs of a
+            // warp): a range of w2, i.e. a mask of at most 32 bits per lane.  What warp w2 needs is the transposed thing,
+            // for every word of 32 ranks the lanes whose mask has bit w2: one 32 x 32 bit transpose per word (sixteen
+            // warps: per two words, their 16-bit masks side by side) instead of one ballot per (word, warp).
+            const int wstep = cpw * MED_PB;
             const int n_chain = (n_coarse + cpw - 1) / cpw;      // warps that have a chunk
-            for (int e = warp; e < nw; e += WARPS) {
-                const int p = spos[(e << 5) + lane];
-                unsigned mine = 0u;
-#pragma unroll
-                for (int w2 = 0; w2 < WARPS; ++w2) {
-                    const unsigned bits = __ballot_sync(FULL, (unsigned)(p - w2 * wstep) < (unsigned)W);
-                    if (lane == w2) mine = bits;
+            const unsigned magic = 0xffffffffu / (unsigned)wstep + 1u;     // p / wstep = umulhi(p, magic) for p wstep < 2^32
+            const int back = wstep - W;
+            auto first_windows = [&](int p) -> unsigned {
+                const unsigned hi = min(__umulhi((unsigned)p, magic), 31u);
+                const unsigned lo = __umulhi((unsigned)max(p + back, 0), magic);
+                return lo > hi ? 0u : (((2u << hi) - 1u) & ~((1u << lo) - 1u));
+            };
+            if (WARPS == 16) {
+                // nw is a multiple of 16: lanes 0-15 get word e2 for the warps 0-15, lanes 16-31 word e2 + 1
+                for (int e2 = 2 * warp; e2 < nw; e2 += 2 * WARPS) {
+                    const int pa = spos[(e2 << 5) + lane], pb = spos[((e2 + 1) << 5) + lane];
+                    const unsigned v = transpose_bits_32((first_windows(pa) & 0xffffu) | (first_windows(pb) << 16));
+                    if ((lane & 15) < n_chain) aux32[(lane & 15) * BMW + e2 + (lane >> 4)] = v;
                 }
-                if (lane < n_chain) aux32[lane * (LT / 32) + e] = mine;
+            } else {
+                for (int e = warp; e < nw; e += WARPS) {
+                    const unsigned v = transpose_bits_32(first_windows(spos[(e << 5) + lane]));
+                    if (lane < n_chain) aux32[lane * BMW + e] = v;
+                }
             }
             for (int e = lane; e < nw; e += 32) sp[e] = 0u;
         }
