@@ -101,6 +101,21 @@ __device__ __forceinline__ void smem_and(uint32_t addr, unsigned v)
     asm volatile("red.shared.and.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
 }
 
+// loads from a 32-bit shared address (the arrays of the tile sit at constant offsets from one base: no generic
+// pointers to keep, no 64-bit address arithmetic in the walk)
+__device__ __forceinline__ unsigned smem_ld32(uint32_t addr)
+{
+    unsigned v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned smem_ld16(uint32_t addr)
+{
+    unsigned short v;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(addr) : "memory");
+    return v;
+}
+
 // lanes of the warp whose 8-bit digit equals this lane's: what match.any computes, from 8 ballots.  MATCH.ANY is a
 // single instruction but the SM retires only one every ~50 clocks (measured: a radix pass over 8192 keys takes 19 000
 // clocks with it, 12 700 with the ballots, and two CTAs on one SM no longer slow each other down)
@@ -170,7 +185,7 @@ running_median_tile_kernel(MedianArgs a)
 #ifdef MED_TIMING
     long long med_t_prev = 0;
 #endif
-    bool neg = false;
+    int flags = 0;                                       // bit 0: a negative median (kernel-wide); bit 1: a median on a saturated key (this tile)
     gbfg_let_next_kernel_start();                        // the wide-tile kernel / the prefix may queue up behind this one
     gbfg_wait_prior_kernel();                            // (launched as a dependent: the 32-bit kernel's wide list)
 
@@ -378,7 +393,7 @@ running_median_tile_kernel(MedianArgs a)
     MED_TICK(3);
     if (a.items && tid == 0) next_item = (int)gridDim.x + atomicAdd(&a.ctr[1], 1);     // the next tile of this CTA
     double dmax = 0.0;
-    bool sat_hit = false;                                // a median of a saturated tile landed on the saturated key
+    flags &= 1;
     // ---- window bitmaps.  Warp w owns the chunks [w cpw, (w+1) cpw) of 32 consecutive outputs and keeps, in
     // shared memory, one bit per sorted rank: "the element of this rank lies in the window".  The median of a
     // window is its (h+1)-th set bit.
@@ -401,7 +416,7 @@ running_median_tile_kernel(MedianArgs a)
         unsigned *bm = aux32 + warp * BMW;
         unsigned *sp = aux32 + (WARPS + warp) * BMW;
         const int nw = LTe / 32;
-        const uint32_t bm_a = (uint32_t)__cvta_generic_to_shared(bm), sp_a = (uint32_t)__cvta_generic_to_shared(sp);
+        const uint32_t bm_a = (uint32_t)__cvta_generic_to_shared(bm);
         {
             // Position p lies in the first window of warp w2 iff w2 wstep <= p < w2 wstep + W (wstep = the outputs of a
             // warp): a range of w2, i.e. a mask of at most 32 bits per lane.  What warp w2 needs is the transposed thing,
@@ -462,27 +477,32 @@ running_median_tile_kernel(MedianArgs a)
                 m0 = __shfl_sync(FULL, found, L);
             }
             MED_TICK(5);
+            // the arrays as 32-bit shared addresses: skey at 0, spos, rop, then the bitmaps (sp of a warp SP_D behind its bm)
+            const uint32_t sm0 = (uint32_t)__cvta_generic_to_shared(smem_raw);
+            constexpr uint32_t SPOS_A = sizeof(KeyT) * LT, ROP_A = SPOS_A + 2u * LT, SP_D = 4u * WARPS * BMW;
+            int64_t *const med_row = a.med + row + o0;           // output j of the tile: med_row[j]
+            double *const psd_row = a.psd ? a.psd + row + o0 : nullptr;
+            const double *const si_row = a.s_instr ? a.s_instr + o0 : nullptr;
             for (int c = c_first; c < c_last; ++c, j0 += MED_PB) {
                 const int pg = j0 + lane, pc_ = j0 + W + lane;           // positions that leave / enter
                 // this lane's own output is j0 + lane: what its PSD needs is on its way while the median is found
                 const bool own = pg < n_out;
-                const int64_t g_own = o0 + pg;
                 double si = 0.0, pold = 0.0;
-                if (a.psd && own) {
-                    si = __ldg(a.s_instr + g_own);
-                    if (DELTA) pold = a.psd[row + g_own];
+                if (psd_row && own) {
+                    si = __ldg(si_row + pg);
+                    if (DELTA) pold = psd_row[pg];
                 }
-                const int gone = rop[pg];
+                const int gone = (int)smem_ld16(sm0 + ROP_A + 2u * (uint32_t)pg);
                 const bool c_ok = pc_ < Lt;
-                const int come = c_ok ? (int)rop[pc_] : 0x7fffffff;
+                const int come = c_ok ? (int)smem_ld16(sm0 + ROP_A + 2u * (uint32_t)pc_) : 0x7fffffff;
                 const unsigned gb = __ballot_sync(FULL, gone < m0), cb = __ballot_sync(FULL, come < m0);
                 const unsigned gm = __ballot_sync(FULL, gone == m0);
                 const uint32_t g_off = (uint32_t)(gone >> 5) << 2, c_off = (uint32_t)(come >> 5) << 2;
                 const unsigned g_bit = 1u << (gone & 31), c_bit = 1u << (come & 31);
-                smem_or(sp_a + g_off, g_bit);
+                smem_or(bm_a + SP_D + g_off, g_bit);
                 if (c_ok) {
                     smem_or(bm_a + c_off, c_bit);
-                    smem_or(sp_a + c_off, c_bit);
+                    smem_or(bm_a + SP_D + c_off, c_bit);
                 }
                 // lane i: output j0 + i; lane 0: output j0 + 32 (the next chunk's first), its own answer being m0
                 const bool next_needed = c + 1 < c_last;
@@ -500,54 +520,62 @@ running_median_tile_kernel(MedianArgs a)
                 int r = m0;
                 if (t > 0) {
                     int wi = m0 >> 5;
+                    const int step = up ? 1 : -1;
                     // the first word: only the ranks beyond m0
                     unsigned keep = up ? ~((2u << (m0 & 31)) - 1u) : ((1u << (m0 & 31)) - 1u);
                     for (;;) {
-                        unsigned wb = bm[wi] & keep;
-                        for (unsigned sb = wb & sp[wi]; sb; sb &= sb - 1u) {       // specials: in this lane's window?
+                        const uint32_t w_a = bm_a + 4u * (uint32_t)wi;
+                        unsigned wb = smem_ld32(w_a) & keep;
+                        for (unsigned sb = wb & smem_ld32(w_a + SP_D); sb; sb &= sb - 1u) {       // specials: in this lane's window?
                             const int b = __ffs(sb) - 1;
-                            if ((unsigned)((int)spos[(wi << 5) + b] - jlo) >= (unsigned)W) wb &= ~(1u << b);
+                            const int pos = (int)smem_ld16(sm0 + SPOS_A + 2u * (uint32_t)((wi << 5) + b));
+                            if ((unsigned)(pos - jlo) >= (unsigned)W) wb &= ~(1u << b);
                         }
                         const int pc = __popc(wb);
                         if (t <= pc) {
-                            r = (wi << 5) + (up ? nth_set_bit(wb, t) : 31 - nth_set_bit(__brev(wb), t));
+                            // the t-th set bit from below (up) or from above (down): one search, on the word or its mirror image
+                            const int at = nth_set_bit(up ? wb : __brev(wb), t);
+                            r = (wi << 5) + (up ? at : 31 - at);
                             break;
                         }
                         t -= pc;
-                        wi += up ? 1 : -1;
+                        wi += step;
                         keep = 0xffffffffu;
                         if ((unsigned)wi >= (unsigned)nw) break;               // not reachable: the window holds the element
                     }
                 }
                 if (own) {                                   // median and PSD of output j0 + lane, 256 bytes per warp and array
-                    const KeyT kv = skey[lane ? r : m0];
-                    if (NARROW && saturated && kv == (KeyT)0xffffffffu) sat_hit = true;
+                    const int at = lane ? r : m0;
+                    KeyT kv;
+                    if (NARROW) kv = (KeyT)smem_ld32(sm0 + 4u * (uint32_t)at);
+                    else kv = skey[at];
+                    if (NARROW && saturated && kv == (KeyT)0xffffffffu) flags |= 2;
                     int64_t v;
                     if (NARROW) v = (int64_t)(((key_ref & 0xffffffff00000000ull) | (uint64_t)kv) ^ SIGN64);
                     else v = (int64_t)((uint64_t)kv ^ SIGN64);
-                    a.med[row + g_own] = v;
-                    neg |= v < 0;
-                    if (a.psd) {
+                    med_row[pg] = v;
+                    flags |= (int)(v < 0);
+                    if (psd_row) {
                         const double e = (double)v * a.scale;
                         const double pnew = si + a.norm * e;
                         if (DELTA) {                         // convergence in S_n: change against the last pass
                             const double d = fabs(pnew - pold) / pold;
                             if (d > dmax) dmax = d;
                         }
-                        a.psd[row + g_own] = pnew;
+                        psd_row[pg] = pnew;
                     }
                 }
                 __syncwarp();
                 smem_and(bm_a + g_off, ~g_bit);
-                smem_and(sp_a + g_off, ~g_bit);
-                if (c_ok) smem_and(sp_a + c_off, ~c_bit);
+                smem_and(bm_a + SP_D + g_off, ~g_bit);
+                if (c_ok) smem_and(bm_a + SP_D + c_off, ~c_bit);
                 m0 = __shfl_sync(FULL, r, 0);
                 __syncwarp();
             }
         }
     }
     {
-        const int any_hit = __syncthreads_or(NARROW && saturated && sat_hit);      // (also the barrier of the walk's end)
+        const int any_hit = __syncthreads_or(NARROW && saturated && (flags & 2));      // (also the barrier of the walk's end)
         if (NARROW && any_hit && tid == 0) a.wide_items[atomicAdd(&a.wide_ctr[0], 1)] = make_int4(row_i, (int)o0, n_out, 0);
     }
 
@@ -558,7 +586,7 @@ running_median_tile_kernel(MedianArgs a)
     }
     MED_TICK(7);
   }   // tiles
-    if (a.neg_flag && neg) *a.neg_flag = 1;
+    if (a.neg_flag && (flags & 1)) *a.neg_flag = 1;
 }
 
 }  // namespace gbfg
