@@ -160,6 +160,32 @@ def test_running_median_bit_exact(gb, orc, torch, kind, n, window):
     assert np.array_equal(out.cpu().numpy(), ref)
 
 
+@pytest.mark.parametrize("n_big_minus_h", [-3, 0, 1, 40])
+@pytest.mark.parametrize("window", [101, 2001])
+def test_running_median_few_loud_bins(gb, orc, torch, window, n_big_minus_h):
+    """Tiles whose keys need a fourth radix pass only for a few loud bins: about h of them per tile (the count up to which
+    a sort that lumps them into its top digit would still be exact), with loud values on both sides of 2^24 and at the
+    edge 0x00ff0000 of that digit; then a loud plateau as wide as the window."""
+    n, h = 20000, window // 2
+    rng = np.random.default_rng(window + n_big_minus_h)
+    x = rng.integers(1000, 1 << 20, n).astype(np.int64)
+    for start in (0, 9000):                                  # first tile, and a stretch that straddles two tiles
+        n_big = h + n_big_minus_h
+        at = start + rng.choice(3000, n_big, replace=False)
+        loud = rng.choice(np.array([0x00ff0000, 0x00ff0001, 0x00ffffff, 1 << 24, (1 << 24) + 5, 0xfffffffe, 0xffffffff,
+                                    0x00feffff], dtype=np.int64), n_big)
+        x[at] = loud
+    ref = orc.running_median(x, window)
+    out = torch.empty(n, dtype=torch.int64, device="cuda")
+    gb.running_median(dev(torch, x), n, 1, window, out)
+    assert np.array_equal(out.cpu().numpy(), ref)
+    # the same with a plateau of loud bins as wide as the window: every median inside it is loud
+    x[4000:4000 + 3 * window] = (1 << 26) + rng.integers(0, 1000, 3 * window)
+    ref = orc.running_median(x, window)
+    gb.running_median(dev(torch, x), n, 1, window, out)
+    assert np.array_equal(out.cpu().numpy(), ref)
+
+
 def test_running_median_batch_rows(gb, orc, torch):
     n, window = 15000, 1001
     rows = [wl.random_spectrum(n, seed=100 + r, kind=k) for r, k in enumerate(["lognormal", "zeros", "full64"])]
