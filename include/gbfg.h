@@ -328,6 +328,15 @@ typedef struct gbfg_kernel_time {
 } gbfg_kernel_time;
 int gbfg_profile_enable(int on);
 int gbfg_profile_read(gbfg_kernel_time *out, int32_t n_out);
+/* The same record launch by launch, in the order the launches were issued: kernel class, start and end of each timed
+ * launch in milliseconds since the first one's start (launches on different streams overlap).  out: HOST, room for cap
+ * entries; *n_written = the number filled (at most cap; *n_total = the number recorded).  Does not clear the record:
+ * gbfg_profile_read or gbfg_profile_enable does. */
+typedef struct gbfg_launch_time {
+    int32_t kernel;         /* GBFG_K_* */
+    float start_ms, end_ms;
+} gbfg_launch_time;
+int gbfg_profile_timeline(gbfg_launch_time *out, int32_t cap, int32_t *n_written, int32_t *n_total);
 
 #ifdef __cplusplus
 }

@@ -27,7 +27,7 @@ EXPORTS = [
     "gbfg_kernel_launch_count", "gbfg_profile_enable", "gbfg_profile_read", "gbfg_release_cached",
     "gbfg_running_mean", "gbfg_coarse_grain", "gbfg_instrument_noise_aet",
     "gbfg_sample_catalog_paper", "gbfg_running_median_workspace_bytes", "gbfg_channel_sum_noise", "gbfg_simulate_paper",
-    "gbfg_running_median_static",
+    "gbfg_running_median_static", "gbfg_profile_timeline",
 ]
 
 KERNEL_CLASSES = ["sample", "noise", "deposit", "scan", "median", "psd", "inv_blocks", "snr", "aux"]
@@ -179,6 +179,21 @@ def release_cached():
 
 def kernel_launch_count() -> int:
     return load().gbfg_kernel_launch_count()
+
+
+class LaunchTime(C.Structure):
+    _fields_ = [("kernel", C.c_int32), ("start_ms", C.c_float), ("end_ms", C.c_float)]
+
+
+def profile_timeline(cap: int = 4096) -> list:
+    """[(kernel class, start_ms, end_ms)] of the launches timed since the last profile_read / profile_enable, in issue
+    order, times since the first launch's start."""
+    arr = (LaunchTime * cap)()
+    n_w, n_t = C.c_int32(0), C.c_int32(0)
+    L = load()
+    L.gbfg_profile_timeline.argtypes = [C.POINTER(LaunchTime), C.c_int32, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
+    _check(L.gbfg_profile_timeline(arr, cap, C.byref(n_w), C.byref(n_t)))
+    return [(KERNEL_CLASSES[arr[i].kernel], float(arr[i].start_ms), float(arr[i].end_ms)) for i in range(n_w.value)]
 
 
 def profile_enable(on: bool):

@@ -125,6 +125,25 @@ extern "C" int gbfg_profile_read(gbfg_kernel_time *out, int32_t n_out)
     return GBFG_OK;
 }
 
+extern "C" int gbfg_profile_timeline(gbfg_launch_time *out, int32_t cap, int32_t *n_written, int32_t *n_total)
+{
+    if (!out || cap < 0 || !n_written || !n_total) return GBFG_ERR_INVALID_ARG;
+    *n_total = (int32_t)g_prof_used;
+    *n_written = 0;
+    for (size_t i = 0; i < g_prof_used && (int32_t)i < cap; ++i) {
+        TimedLaunch &t = (*g_prof)[i];
+        GBFG_CUDA(cudaEventSynchronize(t.b));
+        float a_ms = 0.f, b_ms = 0.f;
+        if (i) GBFG_CUDA(cudaEventElapsedTime(&a_ms, (*g_prof)[0].a, t.a));
+        GBFG_CUDA(cudaEventElapsedTime(&b_ms, (*g_prof)[0].a, t.b));
+        out[i].kernel = t.kid;
+        out[i].start_ms = a_ms;
+        out[i].end_ms = b_ms;
+        *n_written = (int32_t)i + 1;
+    }
+    return GBFG_OK;
+}
+
 extern "C" int gbfg_grid_init(double f_min, double f_max, double t_obs, int32_t scale_log2, gbfg_grid *out)
 {
     if (!out) return GBFG_ERR_INVALID_ARG;

@@ -49,6 +49,11 @@ psd_kernel(const int64_t *__restrict__ med, const double *__restrict__ s_instr, 
 // all_dirty != 0: every block counts as dirty (first iteration, cap branch without tracking).
 // ctr[0] must be zero on entry; ctr[1] (the consumers' ticket) likewise.
 // ---------------------------------------------------------------------------------------------
+#ifdef PLAN_TIMING
+#define PLAN_TICK(i) do { __syncthreads(); if (tid == 0 && blockIdx.x == 0) { const long long now_ = clock64(); if (i) a.dbg[i] += now_ - plan_t_prev; plan_t_prev = now_; } } while (0)
+#else
+#define PLAN_TICK(i) do { } while (0)
+#endif
 constexpr int PLAN_THREADS = 1024;
 constexpr int PLAN_MIN_OUT = 512;              // outputs of the smallest tile the plan cuts
 
@@ -76,6 +81,9 @@ struct PlanArgs {
     int64_t *pub_dst;
     int pub_n, pub_flag_at;
     int64_t pub_seq;
+#ifdef PLAN_TIMING
+    long long *dbg;         // probe builds only: clocks per phase, summed over launches, [16]
+#endif
     int *near_fold;         // SnrWork::any_near (nullable): a near-threshold flag raised by the last test (word 1) becomes
                             // visible to the next one (word 0) here, between the two launches
 };
@@ -114,38 +122,45 @@ plan_kernel(PlanArgs a)
     int *s_wpre = s_mem + nw;                                  // [nw] dirty blocks before the word
     int *s_rpre = s_mem + 2 * nw;                              // [nw] runs that start before the word
     int *s_run = s_mem + nb + 9;                               // (first block, end block, first piece) per run
+#ifdef PLAN_TIMING
+    long long plan_t_prev = 0;
+#endif
+    PLAN_TICK(0);
     if (tid == 0) row_pieces = 0;
     if (row == 0 && tid < 2) a.wide_ctr[tid] = 0;
     if (row == 0 && tid == 0 && a.near_fold && a.near_fold[1]) a.near_fold[0] = 1;
-    if (row == 0 && a.pub_dst) {
-        // what the pass before wrote (this kernel runs behind the SNR test) goes to the host by plain stores over
-        // PCIe: no copy engine on the path, and the counters can be cleared by the same CTA right behind
-        for (int i = tid; i < a.pub_n; i += PLAN_THREADS) a.pub_dst[i] = a.pub_src[i];
-        __threadfence_system();
-        __syncthreads();
-        if (tid == 0) {
+    // the stamps first: all of a thread's loads in flight while warp 0 hands the last pass's counters to the host
+    constexpr int PLAN_LOADS = DIRTY_MAX_BLOCKS / PLAN_THREADS;
+    static_assert(PLAN_LOADS * PLAN_THREADS == DIRTY_MAX_BLOCKS && PLAN_LOADS <= 16, "one round of loads covers a row");
+    int v[PLAN_LOADS];
+#pragma unroll
+    for (int u = 0; u < PLAN_LOADS; ++u) {
+        const int b = u * PLAN_THREADS + tid;
+        v[u] = (!a.all_dirty && b < nb) ? st[b] : a.stamp;
+    }
+    if (row == 0 && warp == 0) {
+        // What the pass before wrote (this kernel runs behind the SNR test) goes to the host by plain stores over
+        // PCIe: no copy engine on the path.  One warp does it, and clears the counters behind its own loads, while
+        // the others go on; the CTA meets again at the barrier below.
+        if (a.pub_dst) for (int i = lane; i < a.pub_n; i += 32) a.pub_dst[i] = a.pub_src[i];
+        __syncwarp();                                        // every lane has its values: the words may be cleared
+        if (a.zero_ptr) for (int i = lane; i < a.zero_n; i += 32) a.zero_ptr[i] = 0;
+        if (a.zero2_ptr) for (int i = lane; i < (int)gridDim.x; i += 32) a.zero2_ptr[i] = 0ull;
+        if (a.pub_dst) {
             __threadfence_system();
-            *(volatile int64_t *)(a.pub_dst + a.pub_flag_at) = a.pub_seq;
+            __syncwarp();
+            if (lane == 0) *(volatile int64_t *)(a.pub_dst + a.pub_flag_at) = a.pub_seq;
         }
     }
-    if (row == 0 && a.zero_ptr) for (int i = tid; i < a.zero_n; i += PLAN_THREADS) a.zero_ptr[i] = 0;
-    if (row == 0 && a.zero2_ptr) for (int i = tid; i < (int)gridDim.x; i += PLAN_THREADS) a.zero2_ptr[i] = 0ull;
-    // stamps -> one bit per block (coalesced, eight loads in flight per thread)
-    for (int base = 0; base < nb; base += 8 * PLAN_THREADS) {
-        int v[8];
+    PLAN_TICK(1);
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            const int b = base + u * PLAN_THREADS + tid;
-            v[u] = (!a.all_dirty && b < nb) ? st[b] : a.stamp;
-        }
-#pragma unroll
-        for (int u = 0; u < 8; ++u) {
-            const int b = base + u * PLAN_THREADS + tid;
-            const unsigned wd = __ballot_sync(FULL, b < nb && v[u] == a.stamp);
-            if (lane == 0 && b < nb) s_word[b >> 5] = wd;
-        }
+    for (int u = 0; u < PLAN_LOADS; ++u) {
+        const int b = u * PLAN_THREADS + tid;
+        const unsigned wd = __ballot_sync(FULL, b < nb && v[u] == a.stamp);
+        if (lane == 0 && b < nb) s_word[b >> 5] = wd;
     }
     __syncthreads();
+    PLAN_TICK(2);
     // per word: dirty blocks, run starts (a dirty block behind a clean one), run ends; one scan for both counts
     unsigned w = 0, starts = 0, ends = 0, open_in = 0;
     if (tid < nw) {
@@ -173,10 +188,13 @@ plan_kernel(PlanArgs a)
     }
     __syncthreads();
     const int n_dirty = s_total & 0xffff, nr = s_total >> 16;
+    PLAN_TICK(3);
+#pragma unroll 4
     for (int b = tid; b <= nb; b += PLAN_THREADS) {
         const int wi = b >> 5;
         cum[b] = wi < nw ? s_wpre[wi] + __popc(s_word[wi] & ((1u << (b & 31)) - 1u)) : n_dirty;
     }
+    PLAN_TICK(4);
     if (w) {                                                 // first / last dirty block of the row
         const int before = s_wpre[tid];
         if (before == 0) a.range[2 * row] = tid * 32 + __ffs(w) - 1;
@@ -201,6 +219,7 @@ plan_kernel(PlanArgs a)
         if (s_fit < (unsigned)S) S = (int)s_fit;
     }
     __syncthreads();
+    PLAN_TICK(5);
     // the place of every run's pieces in the row's part of the list
     for (int r = tid; r < nr; r += PLAN_THREADS) {
         const int64_t first = (int64_t)s_run[3 * r] << a.dblk_log2;
@@ -221,6 +240,7 @@ plan_kernel(PlanArgs a)
         else row_base = atomicAdd(&a.ctr[0], row_pieces);
     }
     __syncthreads();
+    PLAN_TICK(6);
     const int rb0 = row_base;
     for (int r = warp; r < nr; r += PLAN_THREADS / 32) {
         const int64_t first = (int64_t)s_run[3 * r] << a.dblk_log2;
@@ -235,7 +255,23 @@ plan_kernel(PlanArgs a)
             if (base + i < a.max_items) a.items[base + i] = make_int4(row, (int)o, (int)n_out, 0);
         }
     }
+    PLAN_TICK(7);
 }
+
+#ifdef PLAN_TIMING
+static long long *plan_timing_words()
+{
+    static long long *p = nullptr;
+    if (!p) { cudaMalloc(&p, 16 * sizeof(long long)); cudaMemset(p, 0, 16 * sizeof(long long)); }
+    return p;
+}
+extern "C" void gbfg_debug_plan_timing(long long *out)
+{
+    cudaDeviceSynchronize();
+    cudaMemcpy(out, plan_timing_words(), 16 * sizeof(long long), cudaMemcpyDeviceToHost);
+    cudaMemset(plan_timing_words(), 0, 16 * sizeof(long long));
+}
+#endif
 
 int median_tile_outputs(int window) { return MED_LT32 - (window - 1); }
 
@@ -261,6 +297,9 @@ int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins,
     PlanArgs a;
     if (pub) { a.pub_src = pub->src; a.pub_dst = pub->dst; a.pub_n = pub->n; a.pub_flag_at = pub->flag_at; a.pub_seq = pub->seq; }
     else { a.pub_src = nullptr; a.pub_dst = nullptr; a.pub_n = 0; a.pub_flag_at = 0; a.pub_seq = 0; }
+#ifdef PLAN_TIMING
+    a.dbg = plan_timing_words();
+#endif
     a.zero2_ptr = zero2_ptr;
     a.near_fold = pl.near_fold;
     a.zero_ptr = zero_ptr; a.zero_n = zero_n; a.out_count = out_count;
