@@ -238,6 +238,12 @@ struct EarlyOut {
     cudaStream_t copy_stream;   // the copy and every patch run on this stream, in this order
     int started_after;       // iteration after which the PSD went out (-1: it did not)
     int patched_upto;        // blocks stamped up to this iteration have been stored again since
+    // the resolved flags: final once the last test of a loop that runs to its cap is done, so their copy can run next
+    // to the closing estimator pass
+    uint8_t *host_resolved;  // nullable
+    size_t resolved_bytes;
+    cudaEvent_t ev_last_test;
+    bool resolved_out;       // the copy of the final flags is queued on copy_stream
 };
 constexpr int EARLY_PATCH_EVERY = 4;       // iterations between two patches while the loop runs
 
@@ -544,6 +550,12 @@ static int loop_body(const gbfg_grid *grid, const double *dev_A, const double *d
         rc = launch_snr_cand(nb, n_cat, dev_psd, params->rho_th, dev_resolved, nullptr, n_cand, w.sel_idx, sel_count,
                              near, 1, preselect ? neg_flag : nullptr, true, w.sw, dirty, snr_tests, &sub, delta, psd_rtol, st);
         if (rc) return rc;
+        if (eo && eo->host_resolved && eo->resolved_bytes && it + 1 == params->max_iter) {
+            GBFG_CUDA(cudaEventRecord(eo->ev_last_test, st));
+            GBFG_CUDA(cudaStreamWaitEvent(eo->copy_stream, eo->ev_last_test, 0));
+            GBFG_CUDA(cudaMemcpyAsync(eo->host_resolved, dev_resolved, eo->resolved_bytes, cudaMemcpyDeviceToHost, eo->copy_stream));
+            eo->resolved_out = true;
+        }
         GBFG_CUDA(cudaEventRecord(ev_read, st));            // the test is queued; its counters reach the host through the plan below
         // Everything below is queued before the host has seen the counters (a pass that selected nothing makes
         // it a no-op), so the GPU does not idle while the host waits for the scalar that decides whether the
@@ -574,6 +586,7 @@ static int loop_body(const gbfg_grid *grid, const double *dev_A, const double *d
             // a candidate, and this iteration's test, which did nothing (as did the scan queued behind it),
             // is run on them.
             preselect = false;
+            if (eo) eo->resolved_out = false;            // the test runs again: the flags go out at the end
             GBFG_CUDA(cudaMemsetAsync(w.sw.cand_count, 0, sizeof(int64_t) * (size_t)(1 + n_cat), st));
             rc = launch_cand_build(g, ct, dev_A, dev_f, dev_fdot, dev_resolved, nullptr, params->rho_th, nullptr, w.sw, st);
             if (rc) return rc;
@@ -872,11 +885,15 @@ extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, c
         rc = gbfg_instrument_noise(grid, (double *)(base + oI), side->s);
     }
     // the PSD may leave early (EarlyOut) when the caller's buffer is pinned host memory a kernel can store into
-    EarlyOut eo = {host_psd, nullptr, 8 * rows, side->copy, -1, -1};
+    EarlyOut eo = {host_psd, nullptr, 8 * rows, side->copy, -1, -1, host_resolved, (size_t)n, side->ev_copy, false};
     {
         cudaPointerAttributes at;
         if (cudaPointerGetAttributes(&at, host_psd) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
             eo.host_psd_dev = (double *)at.devicePointer;
+        (void)cudaGetLastError();
+        // (a copy into pageable memory would hold the host up in the middle of the loop)
+        if (!host_resolved || cudaPointerGetAttributes(&at, host_resolved) != cudaSuccess || at.type != cudaMemoryTypeHost)
+            eo.host_resolved = nullptr;
         (void)cudaGetLastError();
     }
     if (!rc) {
@@ -891,7 +908,8 @@ extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, c
     if (!rc) {
         // nothing of the loop is in flight any more (it synchronises its stream before it returns)
         e = cudaSuccess;
-        if (host_resolved && n > 0) e = cudaMemcpyAsync(host_resolved, base + oR, (size_t)n, cudaMemcpyDeviceToHost, side->copy);
+        if (host_resolved && n > 0 && !eo.resolved_out)
+            e = cudaMemcpyAsync(host_resolved, base + oR, (size_t)n, cudaMemcpyDeviceToHost, side->copy);
         if (e == cudaSuccess) {
             if (eo.started_after >= 0) {                        // what was stamped since the last patch
                 const Workspace w = carve(base + oW, grid->n_bins, n, n_cat);
