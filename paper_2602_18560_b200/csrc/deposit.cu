@@ -51,6 +51,16 @@ deposit_kernel(GridDev g, CatTable ct, const double *__restrict__ A, const doubl
     }
 }
 
+// 256-bit global accesses (sm_100): one 32-byte sector per thread and instruction; p must be 32-byte aligned
+__device__ __forceinline__ void ld_global_256(const int64_t *p, int64_t *v)
+{
+    asm volatile("ld.global.v4.s64 {%0, %1, %2, %3}, [%4];" : "=l"(v[0]), "=l"(v[1]), "=l"(v[2]), "=l"(v[3]) : "l"(p) : "memory");
+}
+__device__ __forceinline__ void st_global_256(int64_t *p, const int64_t *v)
+{
+    asm volatile("st.global.v4.s64 [%0], {%1, %2, %3, %4};" ::"l"(p), "l"(v[0]), "l"(v[1]), "l"(v[2]), "l"(v[3]) : "memory");
+}
+
 // phase 1: sums of the tiles of the difference array that hold an update (the others are not touched:
 // their sum is zero by definition, whatever tile_sums holds from an earlier call).
 // grid = (tiles_per_row, n_cat)
@@ -96,9 +106,25 @@ scan_add_kernel(int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
     __shared__ int64_t tile_offset;
     const int64_t t0 = (int64_t)blockIdx.y * tiles_per_row;
     {
+        // (every look-up of a thread in flight at once: a CTA far into the row would otherwise wait for two dependent
+        // L2 round trips per 256 tiles before it)
         int64_t acc = 0;
-        for (int t = threadIdx.x; t < (int)blockIdx.x; t += SCAN_THREADS)
-            if (scan_stamp[t0 + t] == stamp) acc += tile_sums[t0 + t];
+        for (int tb = 0; tb < (int)blockIdx.x; tb += 8 * SCAN_THREADS) {
+            int stp[8];
+            int64_t sum[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int t = tb + u * SCAN_THREADS + threadIdx.x;
+                stp[u] = t < (int)blockIdx.x ? scan_stamp[t0 + t] : stamp - 1;
+            }
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int t = tb + u * SCAN_THREADS + threadIdx.x;
+                sum[u] = stp[u] == stamp ? tile_sums[t0 + t] : 0;
+            }
+#pragma unroll
+            for (int u = 0; u < 8; ++u) acc += sum[u];
+        }
         for (int o = 16; o; o >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, o);
         if ((threadIdx.x & 31) == 0) warp_tot[threadIdx.x >> 5] = acc;
         __syncthreads();
@@ -113,13 +139,25 @@ scan_add_kernel(int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
     if (scan_stamp[t0 + blockIdx.x] != stamp && tile_offset == 0) return;
     const int64_t row = (int64_t)blockIdx.y * n_bins;
     const int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+    // A thread's SCAN_ITEMS = 8 consecutive bins are two 32-byte sectors: moved as 256-bit vectors where the row
+    // starts on a 32-byte boundary, a sector is touched once (with 64-bit accesses every load instruction of the warp
+    // touches 32 sectors and every sector is touched four times: the kernel was bound by that).
+    static_assert(SCAN_ITEMS == 8, "two 256-bit vectors per thread");
+    const bool vec = ((((uintptr_t)(diff + row)) | ((uintptr_t)(spectrum + row))) & 31u) == 0 && base + SCAN_ITEMS <= n_bins;
     int64_t v[SCAN_ITEMS];
     int64_t tsum = 0;
+    if (vec) {
+        ld_global_256(diff + row + base, v);
+        ld_global_256(diff + row + base + 4, v + 4);
 #pragma unroll
-    for (int j = 0; j < SCAN_ITEMS; ++j) {
-        int64_t k = base + j;
-        v[j] = k < n_bins ? diff[row + k] : 0;
-        tsum += v[j];
+        for (int j = 0; j < SCAN_ITEMS; ++j) tsum += v[j];
+    } else {
+#pragma unroll
+        for (int j = 0; j < SCAN_ITEMS; ++j) {
+            int64_t k = base + j;
+            v[j] = k < n_bins ? diff[row + k] : 0;
+            tsum += v[j];
+        }
     }
     int64_t incl = tsum;
     for (int o = 1; o < 32; o <<= 1) {
@@ -131,6 +169,33 @@ scan_add_kernel(int64_t *__restrict__ diff, int64_t n_bins, int tiles_per_row,
     __syncthreads();
     int64_t run = tile_offset + incl - tsum;
     for (int w = 0; w < (threadIdx.x >> 5); ++w) run += warp_tot[w];
+    if (vec) {
+#pragma unroll
+        for (int half = 0; half < 2; ++half) {
+            int64_t r[4];
+            int64_t any_r = 0, any_v = 0;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                run += v[4 * half + j];
+                r[j] = run;
+                any_r |= run;
+                any_v |= v[4 * half + j];
+            }
+            int64_t *const sp = spectrum + row + base + 4 * half;
+            if (any_r != 0) {                               // (a bin whose running value is zero gets its own value back)
+                int64_t s4[4];
+                ld_global_256(sp, s4);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) s4[j] += r[j];
+                st_global_256(sp, s4);
+            }
+            if (any_v != 0) {
+                const int64_t z[4] = {0, 0, 0, 0};
+                st_global_256(diff + row + base + 4 * half, z);
+            }
+        }
+        return;
+    }
 #pragma unroll
     for (int j = 0; j < SCAN_ITEMS; ++j) {
         int64_t k = base + j;
