@@ -158,6 +158,8 @@ inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tile
     const int64_t row = (int64_t)blockIdx.y * n_bins;
     int ok = 1;
     const int U = hdr->unit_exp, e_top = hdr->e_top;        // in flight together with the first dirty look-up
+    static_assert(PFX_ITEMS == 4, "one 256-bit vector of psd per thread");
+    const bool vec_row = ((((uintptr_t)(psd + row)) | ((uintptr_t)(pref + row))) & 31u) == 0;
     for (int t0 = blockIdx.x; t0 < tiles_per_row; t0 += 32 * gridDim.x) {
         const int t_mine = t0 + lane * gridDim.x;
         bool dirty = t_mine < tiles_per_row;
@@ -170,13 +172,23 @@ inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tile
         for (unsigned todo = __ballot_sync(0xffffffffu, dirty); todo; todo &= todo - 1) {
             const int tile = t0 + (__ffs(todo) - 1) * gridDim.x;
             const int64_t base = (int64_t)tile * PFX_TILE + (int64_t)threadIdx.x * PFX_ITEMS;
+            // a thread's four bins are one 32-byte sector of psd and two of the prefix: moved as 256-bit vectors where
+            // the row allows it (with narrower accesses every sector is touched four times and the L1 is what limits)
+            const bool vec = vec_row && base + PFX_ITEMS <= n_bins;
+            double x[PFX_ITEMS];
+            if (vec) {
+                asm volatile("ld.global.v4.f64 {%0, %1, %2, %3}, [%4];" : "=d"(x[0]), "=d"(x[1]), "=d"(x[2]), "=d"(x[3]) : "l"(psd + row + base) : "memory");
+            } else {
+#pragma unroll
+                for (int j = 0; j < PFX_ITEMS; ++j) x[j] = base + j < n_bins ? psd[row + base + j] : 0.0;
+            }
             U128 v[PFX_ITEMS];
             U128 run; run.lo = 0; run.hi = 0;
 #pragma unroll
             for (int j = 0; j < PFX_ITEMS; ++j) {
                 const int64_t k = base + j;
                 U128 t; t.lo = 0; t.hi = 0;
-                if (k < n_bins) t = inv_to_fixed(psd[row + k], U, e_top, &ok);
+                if (k < n_bins) t = inv_to_fixed(x[j], U, e_top, &ok);
                 run = u128_add(run, t);
                 v[j] = run;
             }
@@ -191,10 +203,18 @@ inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tile
             __syncthreads();
             U128 before = u128_sub(incl, run);
             for (int w = 0; w < warp; ++w) before = u128_add(before, wtot[w]);
+            if (vec) {
 #pragma unroll
-            for (int j = 0; j < PFX_ITEMS; ++j) {
-                const int64_t k = base + j;
-                if (k < n_bins) pref[row + k] = u128_add(before, v[j]);
+                for (int j = 0; j < PFX_ITEMS; j += 2) {
+                    const U128 a0 = u128_add(before, v[j]), a1 = u128_add(before, v[j + 1]);
+                    asm volatile("st.global.v4.u64 [%0], {%1, %2, %3, %4};" ::"l"(pref + row + base + j), "l"(a0.lo), "l"(a0.hi), "l"(a1.lo), "l"(a1.hi) : "memory");
+                }
+            } else {
+#pragma unroll
+                for (int j = 0; j < PFX_ITEMS; ++j) {
+                    const int64_t k = base + j;
+                    if (k < n_bins) pref[row + k] = u128_add(before, v[j]);
+                }
             }
             if (threadIdx.x == PFX_THREADS - 1) {
                 tile_tot[(int64_t)blockIdx.y * tiles_per_row + tile] = u128_add(before, run);
