@@ -15,6 +15,8 @@
  *    the concatenation of its catalogs; `offsets` (HOST, n_cat+1 entries, offsets[0] = 0) gives the
  *    first source of each.  Per-bin arrays of a batch are [n_cat][n_bins], row-major.
  *  - The spectrum is int64 fixed point: one unit = 2^scale_log2 strain^2 (configs: -140).
+ *  - A `workspace` is DEVICE memory, 32-byte aligned (cudaMalloc gives 256), of at least gbfg_workspace_bytes();
+ *    GBFG_ERR_WORKSPACE otherwise.
  *  - Every function returns GBFG_OK (0) or a negative gbfg_status.  Nothing throws, aborts or
  *    prints.  The four stage calls and the helpers are asynchronous on `stream`;
  *    gbfg_subtract_until_converged and gbfg_simulate* wait, once per iteration, for that iteration's block of
@@ -39,7 +41,7 @@ extern "C" {
 typedef enum gbfg_status {
     GBFG_OK = 0,
     GBFG_ERR_INVALID_ARG = -1, /* null pointer, even / non-positive window, n_bins < h+1, f_min >= f_max, bad struct_size, n_cat out of range */
-    GBFG_ERR_WORKSPACE = -2,   /* workspace NULL or smaller than gbfg_workspace_bytes() */
+    GBFG_ERR_WORKSPACE = -2,   /* workspace NULL, not aligned or smaller than gbfg_workspace_bytes() */
     GBFG_ERR_CUDA = -3,        /* a CUDA runtime call failed: see gbfg_last_cuda_error() */
     GBFG_ERR_ARCH = -4,        /* current device is not compute capability 10.x */
     GBFG_ERR_UNSUPPORTED = -5, /* window wider than GBFG_MAX_WINDOW, n_cat > GBFG_MAX_CAT, alpha_gamma outside its stated range */

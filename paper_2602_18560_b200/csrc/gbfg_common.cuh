@@ -185,18 +185,25 @@ struct PlanPublish {
     int64_t seq;
 };
 
+// A candidate record as the test reads it: one 32-byte sector, moved by one 256-bit access (four arrays cost four
+// partly used sectors per record in the ordering pass, which scatters them)
+struct __align__(32) CandRec {
+    int64_t gk0;        // first bin (index into [n_cat][n_bins])
+    double four_p;
+    int64_t src;        // global source index
+    int32_t w;          // width; 0 once resolved; negated once a test was near the threshold
+    int32_t pad;
+};
+
 // Workspace of stage (iv) (snr.cu): the 128-bit fixed-point prefix of 1/psd and the candidate records.
 struct SnrWork {
     void *pref;         // [n_cat][n_bins] 16-byte local prefixes
     void *tile_off;     // [n_cat][pfx_tiles_per_row] 16-byte tile offsets (exclusive scan of tile_tot)
     void *tile_tot;     // [n_cat][pfx_tiles_per_row] 16-byte tile totals
     void *hdr;          // scale of the fixed point
-    int64_t *cand_gk0;  // [n_src_total] first bin (index into [n_cat][n_bins])
-    int32_t *cand_w;    // [n_src_total] width; 0 once resolved; negated once a test was near the threshold
-    double *cand_4p;    // [n_src_total]
-    int64_t *cand_src;  // [n_src_total] global source index
+    CandRec *cand_rec;  // [n_src_total] the records the test reads, one 32-byte sector each
     int64_t *cand_count;// [1 + n_cat]: number of records, per catalog
-    // the records as first compacted (any order); the arrays above hold them ordered by (row, dirty
+    // the records as first compacted (any order); cand_rec holds them ordered by (row, dirty
     // block of the first bin), which makes the gathers of the test coherent and lets it skip the
     // part of the list that lies outside the dirty range
     int64_t *tmp_gk0;   // [n_src_total]

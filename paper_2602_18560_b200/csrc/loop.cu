@@ -107,10 +107,7 @@ static Workspace carve(void *base, int64_t n_bins, int64_t n_src_total, int n_ca
     w.sw.tile_off = take(snr_tile_off_bytes(n_bins, n_cat));
     w.sw.tile_tot = take(snr_tile_off_bytes(n_bins, n_cat));
     w.sw.hdr = take(snr_hdr_bytes());
-    w.sw.cand_gk0 = (int64_t *)take(sizeof(int64_t) * nsrc);
-    w.sw.cand_w = (int32_t *)take(sizeof(int32_t) * nsrc);
-    w.sw.cand_4p = (double *)take(sizeof(double) * nsrc);
-    w.sw.cand_src = (int64_t *)take(sizeof(int64_t) * nsrc);
+    w.sw.cand_rec = (CandRec *)take(sizeof(CandRec) * nsrc);
     w.sw.cand_count = w.counters + 2 + 2 * n_cat;
     w.sw.tmp_gk0 = (int64_t *)take(sizeof(int64_t) * nsrc);
     w.sw.tmp_w = (int32_t *)take(sizeof(int32_t) * nsrc);
@@ -358,7 +355,7 @@ extern "C" int gbfg_deposit(const gbfg_grid *grid, const double *dev_A, const do
     if (rc) return rc;
     const int64_t n = ct.offsets[n_cat];
     if (n > 0 && (!dev_A || !dev_f || !dev_fdot)) return GBFG_ERR_INVALID_ARG;
-    if (!workspace) return GBFG_ERR_WORKSPACE;
+    if (!workspace || ((uintptr_t)workspace & 31u)) return GBFG_ERR_WORKSPACE;     // (256-bit accesses to its records)
     Workspace w = carve(workspace, grid->n_bins, n, n_cat);
     if (workspace_bytes < w.bytes) return GBFG_ERR_WORKSPACE;
     rc = check_device();
@@ -385,7 +382,7 @@ extern "C" int gbfg_snr_select(const gbfg_grid *grid, const double *dev_A, const
     if (rc) return rc;
     const int64_t n = ct.offsets[n_cat];
     if (n > 0 && (!dev_A || !dev_f || !dev_fdot)) return GBFG_ERR_INVALID_ARG;
-    if (!workspace) return GBFG_ERR_WORKSPACE;
+    if (!workspace || ((uintptr_t)workspace & 31u)) return GBFG_ERR_WORKSPACE;     // (256-bit accesses to its records)
     Workspace w = carve(workspace, grid->n_bins, n, n_cat);
     if (workspace_bytes < w.bytes) return GBFG_ERR_WORKSPACE;
     rc = check_device();
@@ -470,7 +467,7 @@ static int loop_body(const gbfg_grid *grid, const double *dev_A, const double *d
     if (rc) return rc;
     const int64_t n = ct.offsets[n_cat];
     if (n > 0 && (!dev_A || !dev_f || !dev_fdot)) return GBFG_ERR_INVALID_ARG;
-    if (!workspace) return GBFG_ERR_WORKSPACE;
+    if (!workspace || ((uintptr_t)workspace & 31u)) return GBFG_ERR_WORKSPACE;     // (256-bit accesses to its records)
     Workspace w = carve(workspace, grid->n_bins, n, n_cat);
     if (workspace_bytes < w.bytes) return GBFG_ERR_WORKSPACE;
     rc = check_device();
@@ -716,7 +713,7 @@ static int simulate_body(const gbfg_grid *grid, const gbfg_pop *pops, const int6
     rc = make_cat_table(offsets, n_cat, &ct);
     if (rc) return rc;
     const int64_t n = ct.offsets[n_cat];
-    if (!workspace) return GBFG_ERR_WORKSPACE;
+    if (!workspace || ((uintptr_t)workspace & 31u)) return GBFG_ERR_WORKSPACE;     // (256-bit accesses to its records)
     Workspace w = carve(workspace, grid->n_bins, n, n_cat);
     if (workspace_bytes < w.bytes) return GBFG_ERR_WORKSPACE;
     cudaStream_t st = (cudaStream_t)stream;

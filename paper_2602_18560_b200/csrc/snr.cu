@@ -465,8 +465,21 @@ cand_bucket_reach_kernel(const int *__restrict__ bkt_pm, int *__restrict__ bkt_r
 
 struct CandArraysConst { const int64_t *gk0; const int32_t *w; const double *four_p; const int64_t *src; };
 
+__device__ __forceinline__ void store_rec(CandRec *p, int64_t gk0, double four_p, int64_t src, int32_t w)
+{
+    asm volatile("st.global.v4.u64 [%0], {%1, %2, %3, %4};" ::"l"(p), "l"(gk0), "l"(__double_as_longlong(four_p)), "l"(src),
+                 "l"((int64_t)(uint32_t)w) : "memory");
+}
+__device__ __forceinline__ void load_rec(const CandRec *p, int64_t &gk0, double &four_p, int64_t &src, int32_t &w)
+{
+    int64_t fp, wp;
+    asm volatile("ld.global.v4.u64 {%0, %1, %2, %3}, [%4];" : "=l"(gk0), "=l"(fp), "=l"(src), "=l"(wp) : "l"(p) : "memory");
+    four_p = __longlong_as_double(fp);
+    w = (int32_t)(uint32_t)wp;
+}
+
 __global__ void __launch_bounds__(256)
-cand_scatter_kernel(CandArraysConst in, CandArrays out, const int64_t *__restrict__ cand_count, int *__restrict__ bkt_cur,
+cand_scatter_kernel(CandArraysConst in, CandRec *__restrict__ out, const int64_t *__restrict__ cand_count, int *__restrict__ bkt_cur,
                     const int64_t *__restrict__ bkt_off, int64_t n_bins, int n_dblk, int dblk_log2)
 {
     const int64_t n = *cand_count;
@@ -477,17 +490,14 @@ cand_scatter_kernel(CandArraysConst in, CandArrays out, const int64_t *__restric
         const int64_t b = (gk0 - row * n_bins) >> dblk_log2;
         const int64_t packed = in.src[t];
         const int64_t dst = bkt_off[row * (n_dblk + 1) + b] + (packed >> CAND_SLOT_SHIFT);
-        out.gk0[dst] = gk0;
-        out.w[dst] = in.w[t];
-        out.four_p[dst] = in.four_p[t];
-        out.src[dst] = packed & CAND_SRC_MASK;
+        store_rec(out + dst, gk0, in.four_p[t], packed & CAND_SRC_MASK, in.w[t]);
     }
 }
 
 struct SnrArgs {
     const double *psd;          // [n_cat][n_bins]
     PrefixView pv;              // prefix of 1/psd
-    CandArrays cand;
+    CandRec *rec;              // the ordered records
     const int64_t *cand_count;
     const int *abort_flag;      // nullable: when *abort_flag != 0 the kernel does nothing (loop.cu)
     DirtyView dv;               // cum != NULL: a candidate whose bins lie in clean blocks is not re-tested
@@ -550,8 +560,9 @@ snr_cand_kernel(SnrArgs a)
     for (int64_t t0 = t_first + (int64_t)blockIdx.x * blockDim.x; t0 < n; t0 += stride) {
         const int64_t t = t0 + threadIdx.x;
         int32_t w = 0;
-        int64_t src = -1, gk0 = 0;
-        if (t < n) { w = a.cand.w[t]; gk0 = a.cand.gk0[t]; }
+        int64_t src = -1, gk0 = 0, rec_src = -1;
+        double four_p = 0.0;
+        if (t < n) load_rec(a.rec + t, gk0, four_p, rec_src, w);
         bool sel = false, near = false;
         const int cat = rowc;
         const bool always = w < 0;                          // was near the threshold: counted every iteration
@@ -565,13 +576,12 @@ snr_cand_kernel(SnrArgs a)
             }
         }
         if (w > 0) {
-            const double four_p = a.cand.four_p[t];
             bool exact;
             double r2 = rho2_of(a.psd, a.pv, pref_ok, unit_exp, gk0, w, a.n_bins, cat, four_p, &exact);
             if (!exact && fabs(r2 / a.thr - 1.0) <= 4e-9) r2 = rho2_direct(a.psd, gk0, w, four_p);   // decide on the definition's sum
             near = fabs(r2 / a.thr - 1.0) <= 2e-9;
             sel = r2 > a.thr;
-            if (a.rho2_out || sel) src = a.cand.src[t];
+            if (a.rho2_out || sel) src = rec_src;
             if (a.rho2_out) a.rho2_out[src] = r2;
         }
         const unsigned sel_mask = __ballot_sync(0xffffffffu, sel);
@@ -598,13 +608,13 @@ snr_cand_kernel(SnrArgs a)
                 if (mine < SNR_SEL_CAP) s_sel[mine] = src;
                 else a.sel_idx[gbase + (mine - (base > SNR_SEL_CAP ? base : SNR_SEL_CAP))] = src;
                 a.resolved[src] = 1;
-                a.cand.w[t] = 0;
+                a.rec[t].w = 0;
             }
         }
         if (sel && a.sub.spectrum) {
             // stage (v), eq. (D4): spectrum[k] -= q over the source's bins, in the range-update form of deposit.cu
             // (q from p = four_p / 4, exactly the deposit's), and the blocks whose median can change are stamped
-            const int64_t q = __double2ll_rn(ldexp(0.25 * a.cand.four_p[t], -a.sub.scale_log2));
+            const int64_t q = __double2ll_rn(ldexp(0.25 * four_p, -a.sub.scale_log2));
             if (q != 0) {
                 const int64_t k0 = gk0 - (int64_t)cat * a.n_bins;
                 const DepositMarks &mk = a.sub.mk;
@@ -628,7 +638,7 @@ snr_cand_kernel(SnrArgs a)
                 }
             }
         }
-        if (near && !sel && !always) { a.cand.w[t] = -w; a.any_near[1] = 1; }
+        if (near && !sel && !always) { a.rec[t].w = -w; a.any_near[1] = 1; }
         if (near_mask && lane == 0) atomicAdd(&s_near, __popc(near_mask));
     }
     // one append per CTA for what its buffer holds
@@ -749,8 +759,7 @@ int cand_build_finish(const GridDev &g, const CatTable &ct, const SnrWork &sw, c
     cand_bucket_reach_kernel<<<dim3((n_dblk + 255) / 256, ct.n_cat), 256, 0, st>>>(sw.bkt_ext, sw.bkt_reach, n_dblk);
     GBFG_LAUNCH_CHECK("cand_bucket_reach_kernel");
     CandArraysConst in = {sw.tmp_gk0, sw.tmp_w, sw.tmp_4p, sw.tmp_src};
-    CandArrays out = {sw.cand_gk0, sw.cand_w, sw.cand_4p, sw.cand_src};
-    cand_scatter_kernel<<<(int)blocks, 256, 0, st>>>(in, out, sw.cand_count, sw.bkt_count, sw.bkt_off, g.n_bins, n_dblk, dblk_log2);
+    cand_scatter_kernel<<<(int)blocks, 256, 0, st>>>(in, sw.cand_rec, sw.cand_count, sw.bkt_count, sw.bkt_off, g.n_bins, n_dblk, dblk_log2);
     GBFG_LAUNCH_CHECK("cand_scatter_kernel");
     return GBFG_OK;
 }
@@ -783,7 +792,7 @@ int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th,
     a.psd = psd;
     a.pv = make_view(sw, n_bins);
     if (!use_prefix) { a.pv.pref = nullptr; a.pv.tile_off = nullptr; }
-    a.cand.gk0 = sw.cand_gk0; a.cand.w = sw.cand_w; a.cand.four_p = sw.cand_4p; a.cand.src = sw.cand_src;
+    a.rec = sw.cand_rec;
     a.cand_count = sw.cand_count;
     a.abort_flag = abort_flag;
     a.n_bins = n_bins; a.n_cat = n_cat;
