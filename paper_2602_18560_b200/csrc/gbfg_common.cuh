@@ -198,7 +198,6 @@ struct __align__(32) CandRec {
 // Workspace of stage (iv) (snr.cu): the 128-bit fixed-point prefix of 1/psd and the candidate records.
 struct SnrWork {
     void *pref;         // [n_cat][n_bins] 16-byte local prefixes
-    void *tile_off;     // [n_cat][pfx_tiles_per_row] 16-byte tile offsets (exclusive scan of tile_tot)
     void *tile_tot;     // [n_cat][pfx_tiles_per_row] 16-byte tile totals
     void *hdr;          // scale of the fixed point
     CandRec *cand_rec;  // [n_src_total] the records the test reads, one 32-byte sector each

@@ -104,7 +104,6 @@ static Workspace carve(void *base, int64_t n_bins, int64_t n_src_total, int n_ca
     w.counters = (int64_t *)take(sizeof(int64_t) * WS_COUNTERS);
     w.wide_flag = (int *)take(sizeof(int) * (size_t)(1 + n_cat));   // flag, then one scan ticket per row
     w.sw.pref = take(snr_pref_bytes(n_bins, n_cat));
-    w.sw.tile_off = take(snr_tile_off_bytes(n_bins, n_cat));
     w.sw.tile_tot = take(snr_tile_off_bytes(n_bins, n_cat));
     w.sw.hdr = take(snr_hdr_bytes());
     w.sw.cand_rec = (CandRec *)take(sizeof(CandRec) * nsrc);

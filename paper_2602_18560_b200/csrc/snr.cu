@@ -139,18 +139,16 @@ prefix_header_kernel(const double *__restrict__ arr, int64_t n, int64_t n_bins_r
     }
 }
 
-// phase A: local inclusive prefix of every tile of PFX_TILE bins + the tile totals (skipped for
+// Local inclusive prefix of every tile of PFX_TILE bins + the tile totals (no prefix across tiles: a sum over a
+// stretch of bins is a difference of two local prefixes plus the totals of the tiles it crosses, rho2_of); skipped for
 // tiles without a dirty block: their prefix stands).  gridDim.x CTAs per row, resident together; CTA b
 // takes the tiles b, b + gridDim.x, ...: 32 of them are looked up at once (lane l the l-th), so a pass
 // with a handful of dirty tiles costs one look-up per CTA, not one CTA per tile.
 __global__ void __launch_bounds__(PFX_THREADS, 3)
 inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tiles_per_row,
-                        U128 *__restrict__ pref, U128 *__restrict__ tile_tot, U128 *__restrict__ tile_off,
-                        PrefixHeader *hdr, DirtyView dv, unsigned *__restrict__ ticket)
+                        U128 *__restrict__ pref, U128 *__restrict__ tile_tot, PrefixHeader *hdr, DirtyView dv)
 {
     __shared__ U128 wtot[PFX_THREADS / 32];
-    __shared__ U128 carry_s;
-    __shared__ int is_last;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     gbfg_let_next_kernel_start();
     gbfg_wait_prior_kernel();                               // the PSD of this pass
@@ -216,72 +214,32 @@ inv_prefix_local_kernel(const double *__restrict__ psd, int64_t n_bins, int tile
                     if (k < n_bins) pref[row + k] = u128_add(before, v[j]);
                 }
             }
-            if (threadIdx.x == PFX_THREADS - 1) {
-                tile_tot[(int64_t)blockIdx.y * tiles_per_row + tile] = u128_add(before, run);
-                __threadfence();
-            }
+            if (threadIdx.x == PFX_THREADS - 1) tile_tot[(int64_t)blockIdx.y * tiles_per_row + tile] = u128_add(before, run);
         }
     }
     if (!ok) hdr->bad = 1;
-    // phase B by the last CTA of the row to finish: exclusive scan of the row's tile totals
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        is_last = atomicAdd(ticket + blockIdx.y, 1u) == gridDim.x - 1u;
-        carry_s.lo = 0; carry_s.hi = 0;
-    }
-    __syncthreads();
-    if (!is_last) return;
-    __threadfence();
-    if (threadIdx.x == 0) ticket[blockIdx.y] = 0u;
-    // PFX_ITEMS consecutive tiles per thread: one round of loads, one block scan per PFX_TILE tiles
-    const volatile uint64_t *totp = reinterpret_cast<const volatile uint64_t *>(tile_tot + (int64_t)blockIdx.y * tiles_per_row);
-    U128 *outp = tile_off + (int64_t)blockIdx.y * tiles_per_row;
-    for (int b = 0; b < tiles_per_row; b += PFX_TILE) {
-        const int i0 = b + threadIdx.x * PFX_ITEMS;
-        U128 v[PFX_ITEMS];
-#pragma unroll
-        for (int j = 0; j < PFX_ITEMS; ++j) {
-            v[j].lo = 0; v[j].hi = 0;
-            if (i0 + j < tiles_per_row) { v[j].lo = totp[2 * (i0 + j)]; v[j].hi = totp[2 * (i0 + j) + 1]; }
-        }
-        U128 run = v[0];
-#pragma unroll
-        for (int j = 1; j < PFX_ITEMS; ++j) run = u128_add(run, v[j]);
-        U128 incl = run;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            U128 up = u128_shfl_up(incl, o);
-            if (lane >= o) incl = u128_add(incl, up);
-        }
-        __syncthreads();
-        if (lane == 31) wtot[warp] = incl;
-        __syncthreads();
-        U128 before = u128_add(carry_s, u128_sub(incl, run));
-        for (int w = 0; w < warp; ++w) before = u128_add(before, wtot[w]);
-#pragma unroll
-        for (int j = 0; j < PFX_ITEMS; ++j) {
-            if (i0 + j < tiles_per_row) outp[i0 + j] = before;
-            before = u128_add(before, v[j]);
-        }
-        __syncthreads();
-        if (threadIdx.x == PFX_THREADS - 1) carry_s = before;
-        __syncthreads();
-    }
 }
 
-// inclusive prefix through bin k of row `row_tile0` (k >= 0)
-__device__ __forceinline__ U128 prefix_at(const U128 *__restrict__ pref, const U128 *__restrict__ tile_off,
-                                          int64_t row_bin0, int64_t row_tile0, int64_t k)
+// sum of the fixed-point terms of the bins [k0, k0 + w) of a row: local prefixes at both ends + the totals of the tiles
+// in between (integers: the same bits in whatever order they are added)
+__device__ __forceinline__ U128 prefix_range(const U128 *__restrict__ pref, const U128 *__restrict__ tile_tot,
+                                             int64_t row_bin0, int64_t row_tile0, int64_t k0, int64_t w)
 {
-    const U128 a = pref[row_bin0 + k];
-    const U128 b = tile_off[row_tile0 + k / PFX_TILE];
-    return u128_add(a, b);
+    const int64_t k1 = k0 + w - 1;
+    U128 sum = pref[row_bin0 + k1];
+    int64_t t = 0;
+    if (k0 > 0) {
+        sum = u128_sub(sum, pref[row_bin0 + k0 - 1]);
+        t = (k0 - 1) / PFX_TILE;
+    }
+    for (const int64_t t1 = k1 / PFX_TILE; t < t1; ++t) sum = u128_add(sum, tile_tot[row_tile0 + t]);
+    return sum;
 }
 
 // What the test needs of the prefix (all NULL / 0: direct sums only)
 struct PrefixView {
     const U128 *pref;           // [rows][n_bins] local inclusive prefixes
-    const U128 *tile_off;       // [rows][tiles_per_row] exclusive tile offsets
+    const U128 *tile_tot;       // [rows][tiles_per_row] tile totals
     const PrefixHeader *hdr;
     int tiles_per_row;
 };
@@ -301,8 +259,7 @@ __device__ __forceinline__ double rho2_of(const double *__restrict__ psd, const 
     if (w <= SNR_NARROW || !pref_ok) return rho2_direct(psd, gk0, w, four_p);
     const int64_t row_bin0 = (int64_t)row * n_bins, row_tile0 = (int64_t)row * pv.tiles_per_row;
     const int64_t k0 = gk0 - row_bin0;
-    U128 hi = prefix_at(pv.pref, pv.tile_off, row_bin0, row_tile0, k0 + w - 1);
-    if (k0 > 0) hi = u128_sub(hi, prefix_at(pv.pref, pv.tile_off, row_bin0, row_tile0, k0 - 1));
+    const U128 hi = prefix_range(pv.pref, pv.tile_tot, row_bin0, row_tile0, k0, w);
     // every term was truncated by less than one unit: keep the relative error under 2^-46
     if (hi.hi == 0 && hi.lo < ((uint64_t)w << 46)) return rho2_direct(psd, gk0, w, four_p);
     *exact = false;
@@ -668,7 +625,7 @@ static PrefixView make_view(const SnrWork &sw, int64_t n_bins)
 {
     PrefixView pv;
     pv.pref = (const U128 *)sw.pref;
-    pv.tile_off = (const U128 *)sw.tile_off;
+    pv.tile_tot = (const U128 *)sw.tile_tot;
     pv.hdr = (const PrefixHeader *)sw.hdr;
     pv.tiles_per_row = pfx_tiles_per_row(n_bins);
     return pv;
@@ -697,9 +654,8 @@ int launch_inv_prefix(const double *psd, int64_t n_bins, int n_cat, const SnrWor
     if (per_row < 64) per_row = 64;                            // a batch: more, shorter CTAs (rows differ in how dirty they are)
     if (per_row > tiles) per_row = tiles;
     LaunchTimer lt(K_INV_BLOCKS, st);
-    unsigned *ticket = reinterpret_cast<unsigned *>((char *)sw.hdr + sizeof(PrefixHeader) + sizeof(PrefixScratch));
     cudaError_t e = launch_dependent(inv_prefix_local_kernel, dim3(per_row, n_cat), dim3(PFX_THREADS), 0, st, psd, n_bins, tiles,
-                                     (U128 *)sw.pref, (U128 *)sw.tile_tot, (U128 *)sw.tile_off, (PrefixHeader *)sw.hdr, dv, ticket);
+                                     (U128 *)sw.pref, (U128 *)sw.tile_tot, (PrefixHeader *)sw.hdr, dv);
     if (e != cudaSuccess) return set_cuda_error(e, "inv_prefix_local_kernel");
     GBFG_LAUNCH_CHECK("inv_prefix_local_kernel");
     return GBFG_OK;
@@ -791,7 +747,7 @@ int launch_snr_cand(int64_t n_bins, int n_cat, const double *psd, double rho_th,
     a.dv = dv;
     a.psd = psd;
     a.pv = make_view(sw, n_bins);
-    if (!use_prefix) { a.pv.pref = nullptr; a.pv.tile_off = nullptr; }
+    if (!use_prefix) { a.pv.pref = nullptr; a.pv.tile_tot = nullptr; }
     a.rec = sw.cand_rec;
     a.cand_count = sw.cand_count;
     a.abort_flag = abort_flag;
