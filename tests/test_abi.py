@@ -112,6 +112,9 @@ def test_invalid_arguments_are_rejected_before_any_cuda_call(gbcpu):
     p2.window = 1001
     p2.max_iter = 0
     assert L.gbfg_subtract_until_converged(C.byref(g), 8, 8, 8, off, 1, 8, C.byref(p2), 8, 8, 8, 8, res, 8, 1 << 40, None) == -1
+    # a workspace must be 32-byte aligned (the candidate records and the scan move 256-bit vectors): checked before any CUDA call
+    assert L.gbfg_deposit(C.byref(g), 8, 8, 8, off, 1, None, None, 1, 8, None, 48, 1 << 40, None) == -2
+    assert L.gbfg_deposit(C.byref(g), 8, 8, 8, off, 1, None, None, 1, 8, None, 64, 1 << 40, None) != -2
 
 
 def test_paper_sampler_rejects_parameters_outside_the_stated_domain(gbcpu):
