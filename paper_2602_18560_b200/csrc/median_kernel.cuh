@@ -74,8 +74,11 @@ struct MedianArgs {
 #ifdef MED_TIMING
 // phase i = the time between tick i and the tick before it, summed over the CTA's tiles, per CTA
 #define MED_TICK(i) do { if (tid == 0) { const long long now_ = clock64(); if (i) a.dbg[blockIdx.x * 16 + (i)] += now_ - med_t_prev; med_t_prev = now_; } } while (0)
+// inside the sort: the time since the last sub-tick, summed over the passes
+#define MED_SUBTICK(i) do { if (tid == 0) { const long long now_ = clock64(); a.dbg[blockIdx.x * 16 + (i)] += now_ - med_t_sub; med_t_sub = now_; } } while (0)
 #else
 #define MED_TICK(i) do { } while (0)
+#define MED_SUBTICK(i) do { } while (0)
 #endif
 
 // n-th (1-based) set bit of a non-zero mask that has at least n bits set
@@ -183,7 +186,7 @@ running_median_tile_kernel(MedianArgs a)
     const int h = a.h, W = 2 * a.h + 1;
     __shared__ int s_item;
 #ifdef MED_TIMING
-    long long med_t_prev = 0;
+    long long med_t_prev = 0, med_t_sub = 0;
 #endif
     int flags = 0;                                       // bit 0: a negative median (kernel-wide); bit 1: a median on a saturated key (this tile)
     gbfg_let_next_kernel_start();                        // the wide-tile kernel / the prefix may queue up behind this one
@@ -317,8 +320,12 @@ running_median_tile_kernel(MedianArgs a)
     // Warp w owns elements [32 rounds w, 32 rounds (w + 1)) of the current order, 32 consecutive ones per round.
     for (int pass = 0; pass < n_pass; ++pass) {
         const int shift = 8 * pass;
+#ifdef MED_TIMING
+        if (tid == 0) med_t_sub = clock64();
+#endif
         for (int e = tid; e < WARPS * MED_CROW / 2; e += THREADS) aux32[e] = 0u;
         __syncthreads();
+        MED_SUBTICK(8);
         uint16_t *cw = aux + warp * MED_CROW;
         KeyT k[ITEMS];
         uint32_t pk[ITEMS];                              // position << 16 | place among the warp's keys of the same digit
@@ -333,6 +340,7 @@ running_median_tile_kernel(MedianArgs a)
                                      : same_digit_lanes((unsigned)(k[r] >> shift) & 255u);
             }
         }
+        MED_SUBTICK(9);
 #pragma unroll
         for (int r = 0; r < ITEMS; ++r) {                // counter updates, round after round
             if (r < rounds) {
@@ -348,6 +356,7 @@ running_median_tile_kernel(MedianArgs a)
             }
         }
         __syncthreads();
+        MED_SUBTICK(10);
         {   // exclusive scan of the counters in (digit, warp) order: thread t owns digit t / GROUPS, 8 warps
             const int d = tid / GROUPS, wg = (tid % GROUPS) * 8;
             unsigned v[8], s = 0;
@@ -373,6 +382,7 @@ running_median_tile_kernel(MedianArgs a)
             for (int i = 0; i < 8; ++i) { aux[(wg + i) * MED_CROW + d] = (uint16_t)run; run += v[i]; }
         }
         __syncthreads();
+        MED_SUBTICK(11);
 #pragma unroll
         for (int r = 0; r < ITEMS; ++r) {
             if (r < rounds) {
@@ -383,6 +393,7 @@ running_median_tile_kernel(MedianArgs a)
             }
         }
         __syncthreads();
+        MED_SUBTICK(12);
     }
 
     MED_TICK(2);
