@@ -11,6 +11,7 @@
 
 #include "gbfg_common.cuh"
 #include <atomic>
+#include <chrono>
 
 namespace gbfg {
 
@@ -232,8 +233,10 @@ struct EarlyOut {
     double *host_psd_dev;    // ... and the address kernels store to it through
     size_t bytes;
     cudaStream_t copy_stream;   // the copy and every patch run on this stream, in this order
-    int started_after;       // iteration after which the PSD went out (-1: it did not)
+    int started_after;       // iteration after which the PSD began to go out (-1: it did not)
     int patched_upto;        // blocks stamped up to this iteration have been stored again since
+    size_t psd_sent;         // bytes of the PSD copied so far: it leaves in pieces, one per iteration (loop_body)
+    double t_last;           // host clock [s] when the last iteration's counters were seen (0: not yet)
     // the resolved flags: final once the last test of a loop that runs to its cap is done, so their copy can run next
     // to the closing estimator pass
     uint8_t *host_resolved;  // nullable
@@ -603,12 +606,30 @@ static int loop_body(const gbfg_grid *grid, const double *dev_A, const double *d
             const int64_t last_pass = outs - med_outputs_seen;
             med_outputs_seen = outs;
             if (eo && incremental && !use_mean) {
+                const double t_now = std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count();
                 if (eo->started_after < 0) {
                     if (it >= 1 && last_pass * 10 < (int64_t)n_cat * nb) {
-                        GBFG_CUDA(cudaMemcpyAsync(eo->host_psd, dev_psd, eo->bytes, cudaMemcpyDeviceToHost, eo->copy_stream));
                         eo->started_after = eo->patched_upto = it;
+                        eo->psd_sent = 0;
                     }
-                } else if (it - eo->patched_upto >= EARLY_PATCH_EVERY) {
+                }
+                if (eo->started_after >= 0 && eo->psd_sent < eo->bytes) {
+                    // The PSD leaves in pieces, one per iteration, each sized to be through the link before the next plan
+                    // kernel hands over its counters: 30 MB in one copy kept the link busy for half a millisecond, and
+                    // the few stores and the system fence of every plan in that time queued up behind it while the host
+                    // (and with it the next pass) waited for them: the loop took 0.45 ms longer than without the copy.
+                    const double dt = eo->t_last > 0.0 ? t_now - eo->t_last : 50e-6;
+                    double want = 0.7 * dt * 50e9;                       // bytes at 50 GB/s in 70 % of the last iteration's time
+                    if (want < 1048576.0) want = 1048576.0;
+                    if (want > 8388608.0) want = 8388608.0;
+                    size_t sz = (size_t)want & ~(size_t)4095;
+                    if (sz > eo->bytes - eo->psd_sent) sz = eo->bytes - eo->psd_sent;
+                    GBFG_CUDA(cudaMemcpyAsync((char *)eo->host_psd + eo->psd_sent, (const char *)dev_psd + eo->psd_sent, sz,
+                                              cudaMemcpyDeviceToHost, eo->copy_stream));
+                    eo->psd_sent += sz;
+                }
+                eo->t_last = t_now;
+                if (eo->started_after >= 0 && it - eo->patched_upto >= EARLY_PATCH_EVERY) {
                     // the estimator passes up to `it` are done: blocks stamped in (patched_upto, it] hold what they will
                     // keep unless a later subtraction stamps them again
                     rc = launch_psd_patch(*eo, dev_psd, w.blk_stamp, w.plan.n_dblk, w.plan.dblk_log2, nb, n_cat, eo->patched_upto, it);
@@ -881,7 +902,7 @@ extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, c
         rc = gbfg_instrument_noise(grid, (double *)(base + oI), side->s);
     }
     // the PSD may leave early (EarlyOut) when the caller's buffer is pinned host memory a kernel can store into
-    EarlyOut eo = {host_psd, nullptr, 8 * rows, side->copy, -1, -1, host_resolved, (size_t)n, side->ev_copy, false};
+    EarlyOut eo = {host_psd, nullptr, 8 * rows, side->copy, -1, -1, 0, 0.0, host_resolved, (size_t)n, side->ev_copy, false};
     {
         cudaPointerAttributes at;
         if (cudaPointerGetAttributes(&at, host_psd) == cudaSuccess && at.type == cudaMemoryTypeHost && at.devicePointer)
@@ -907,7 +928,10 @@ extern "C" int gbfg_simulate_host(const gbfg_grid *grid, const gbfg_pop *pops, c
         if (host_resolved && n > 0 && !eo.resolved_out)
             e = cudaMemcpyAsync(host_resolved, base + oR, (size_t)n, cudaMemcpyDeviceToHost, side->copy);
         if (e == cudaSuccess) {
-            if (eo.started_after >= 0) {                        // what was stamped since the last patch
+            if (eo.started_after >= 0) {                        // the rest of the PSD, then what was stamped since the last patch
+                if (eo.psd_sent < eo.bytes)
+                    e = cudaMemcpyAsync((char *)host_psd + eo.psd_sent, base + oP + eo.psd_sent, eo.bytes - eo.psd_sent,
+                                        cudaMemcpyDeviceToHost, side->copy);
                 const Workspace w = carve(base + oW, grid->n_bins, n, n_cat);
                 if (launch_psd_patch(eo, (const double *)(base + oP), w.blk_stamp, w.plan.n_dblk, w.plan.dblk_log2, grid->n_bins,
                                      n_cat, eo.patched_upto, 0x7fffffff) != GBFG_OK)
