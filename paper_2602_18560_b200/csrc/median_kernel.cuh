@@ -225,7 +225,7 @@ running_median_tile_kernel(MedianArgs a)
     MED_TICK(0);
     // ---- stage the tile: position p <-> global bin o0 - h + p, reflected at both ends.
     // Unused positions (Lt <= p < LTe) repeat position 0: they are never inside a window.
-    if (tid < 4) misc[32 + tid] = tid == 2 ? 0xffffffffu : 0u;      // varying bits (lo, hi), smallest high word, varying bits again
+    if (tid < 5) misc[32 + tid] = tid == 2 ? 0xffffffffu : 0u;      // varying bits (lo, hi), smallest high word, varying bits again, keys >= 2^24
     __syncthreads();
     uint64_t key_ref;
     {
@@ -313,7 +313,23 @@ running_median_tile_kernel(MedianArgs a)
         key_ref = ((uint64_t)hmin << 32) | k_first;      // the high word of every value that can be a median
         saturated = true;
     }
-    const int n_pass = vary_all ? (64 - __clzll((long long)vary_all) + 7) / 8 : 0;
+    int n_pass = vary_all ? (64 - __clzll((long long)vary_all) + 7) / 8 : 0;
+    if (NARROW && n_pass == 4) {
+        // A fourth pass only for a few loud bins: with no more than h keys at or above 2^24 in the tile no window can have
+        // one of them as its median (a window of 2h+1 then holds at least h+1 smaller ones), so they may all become the
+        // largest 24-bit key: the ranks below them stay exact, and three passes sort the tile.
+        int big = 0;
+        for (int p = tid; p < LTe; p += THREADS) big += (unsigned)skey[p] >= 0x01000000u;
+        big = __reduce_add_sync(FULL, big);
+        if (lane == 0 && big) atomicAdd(&misc[36], (unsigned)big);
+        __syncthreads();
+        if (misc[36] <= (unsigned)h) {
+            for (int p = tid; p < LTe; p += THREADS)
+                if ((unsigned)skey[p] >= 0x01000000u) skey[p] = (KeyT)0x00ffffffu;
+            __syncthreads();
+            n_pass = 3;
+        }
+    }
 
     MED_TICK(1);
     // ---- LSD radix sort by key, stable, so that equal keys stay in position order.
