@@ -12,15 +12,17 @@
 // hold the same digit are found with eight warp reductions (a ballot each), not with match.any: the SM retires
 // one MATCH every ~50 clocks, which made it the single slowest thing in the kernel.  With the sorted order in
 // hand a window is a set of ranks, kept as a bitmap (one bit per rank), and its median is the (h+1)-th set bit:
-//   * the bitmaps of 16 windows per tile (one per warp, evenly spaced) are built by ballots over the sorted
-//     positions, and the (h+1)-th set bit of each is found by counting words;
+//   * the bitmaps of 16 windows per tile (one per warp, evenly spaced) are built from the sorted positions: the
+//     windows a position lies in are a range of warps (a 16-bit mask per lane), and a 32 x 32 bit transpose turns
+//     the masks of two words of ranks into the bitmap words of all warps; the (h+1)-th set bit of each bitmap is
+//     found by counting words;
 //   * every warp then slides its window 32 outputs at a time.  Inside such a chunk lane i takes output j0 + i:
 //     two popcounts of ballots (how many of the ranks that left / entered lie under the chunk's first median)
 //     say how many window elements it must move, and in which direction; it moves word by word — 32 ranks and
 //     typically 8 window elements per step, one popcount — testing positions only for the 64 "special" ranks
 //     that enter or leave inside the chunk (a second bitmap marks them), and picks the bit in the last word.
 //     Plateaus left by wide chirps (long stretches of out-of-window ranks) cost one step per 32 ranks.
-// The per-output rank is kept in shared memory and written out coalesced, fused with
+// Every lane writes the median of its own output from inside that loop, fused with
 //     psd[k] = s_instr[k] + C * (med[k] * 2^scale_log2)        (eqs. 10, D2, D3).
 #include <mutex>
 

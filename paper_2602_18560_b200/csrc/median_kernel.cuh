@@ -424,8 +424,8 @@ running_median_tile_kernel(MedianArgs a)
     // ---- window bitmaps.  Warp w owns the chunks [w cpw, (w+1) cpw) of 32 consecutive outputs and keeps, in
     // shared memory, one bit per sorted rank: "the element of this rank lies in the window".  The median of a
     // window is its (h+1)-th set bit.
-    //  * The bitmaps of the warps' first windows are built by the whole CTA from the rank side: one ballot per
-    //    (word of 32 ranks, warp), no read-modify-write; each warp then finds its first median by counting words.
+    //  * The bitmaps of the warps' first windows are built by the whole CTA from the rank side (a bit transpose per
+    //    two words of ranks, below), no read-modify-write; each warp then finds its first median by counting words.
     //  * Inside a chunk lane i takes output j0 + i.  The 32 positions that leave and the 32 that enter while the
     //    window slides over the chunk are the chunk's "specials" (a second bitmap marks their ranks); every other
     //    set bit of U = window(j0) + the entering positions lies in all the chunk's windows.  Two popcounts of
