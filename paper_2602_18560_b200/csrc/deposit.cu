@@ -247,8 +247,17 @@ int launch_scan(int64_t n_bins, int n_cat, int64_t *spectrum, int64_t *diff, int
     const int tiles = scan_tiles_per_row(n_bins);
     dim3 grid(tiles, n_cat);
     LaunchTimer lt_scan(K_SCAN, st);     // the two scan kernels, as one
-    scan_tile_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, n_bins, tiles, tile_sums, wide_flag, mk.scan_stamp, mk.stamp);
-    GBFG_LAUNCH_CHECK("scan_tile_sums_kernel");
+    if (mk.live_sums) {
+        // whoever wrote the range updates kept the tile sums as well (the loop's test): the second kernel alone, and not as
+        // a programmatic dependent of that test (its 1843 CTAs would sit on the SMs waiting while the test still runs)
+        scan_add_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, n_bins, tiles, (const int64_t *)mk.live_sums, spectrum, (const int *)wide_flag,
+                                                       (const int *)mk.scan_stamp, mk.stamp);
+        GBFG_LAUNCH_CHECK("scan_add_kernel");
+        return GBFG_OK;
+    } else {
+        scan_tile_sums_kernel<<<grid, SCAN_THREADS, 0, st>>>(diff, n_bins, tiles, tile_sums, wide_flag, mk.scan_stamp, mk.stamp);
+        GBFG_LAUNCH_CHECK("scan_tile_sums_kernel");
+    }
     cudaError_t e = launch_dependent(scan_add_kernel, grid, dim3(SCAN_THREADS), 0, st, diff, n_bins, tiles,
                                      (const int64_t *)tile_sums, spectrum, (const int *)wide_flag, (const int *)mk.scan_stamp, mk.stamp);
     if (e != cudaSuccess) return set_cuda_error(e, "scan_add_kernel");

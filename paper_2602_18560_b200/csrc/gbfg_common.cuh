@@ -138,6 +138,8 @@ struct DepositMarks {
     int dblk_log2;
     int med_h;          // half window
     int stamp;          // value written
+    int64_t *live_sums; // nullable: [n_cat][scan_tiles], zero on entry: the sums of the difference array's tiles, kept by
+                        // whoever writes a range update (the loop's test), so that the scan needs no pass of its own for them
 };
 
 
@@ -183,6 +185,8 @@ struct PlanPublish {
     int64_t *dst;
     int n, flag_at;
     int64_t seq;
+    int64_t *zero_sums;     // nullable: tile sums of the range updates after next (the other of two buffers), cleared here
+    int zero_sums_n;
 };
 
 // A candidate record as the test reads it: one 32-byte sector, moved by one 256-bit access (four arrays cost four

@@ -67,6 +67,7 @@ constexpr int WS_COUNTERS = 7 * GBFG_MAX_CAT + 16;
 struct Workspace {
     int64_t *diff;        // [n_cat * n_bins]   difference array of the range-update deposit
     int64_t *tile_sums;   // [n_cat * scan_tiles]
+    int64_t *live_sums[2]; // the same, kept by the loop's test itself: one buffer per parity of the iteration
     int *scan_stamp;      // [n_cat * scan_tiles]
     int *blk_stamp;       // [n_cat * n_dblk]        dirty-block stamps
     MedianPlan plan;      // work list of the running median, cum of the dirty blocks
@@ -119,6 +120,8 @@ static Workspace carve(void *base, int64_t n_bins, int64_t n_src_total, int n_ca
     w.sw.bkt_off = (int64_t *)take(sizeof(int64_t) * (size_t)n_cat * (size_t)(n_dblk + 1));
     w.sw.any_near = (int *)take(2 * sizeof(int));
     w.plan.near_fold = w.sw.any_near;
+    w.live_sums[0] = (int64_t *)take(sizeof(int64_t) * (size_t)n_cat * (size_t)scan_tiles_per_row(n_bins));
+    w.live_sums[1] = (int64_t *)take(sizeof(int64_t) * (size_t)n_cat * (size_t)scan_tiles_per_row(n_bins));
     w.bytes = off;
     return w;
 }
@@ -331,6 +334,7 @@ static DepositMarks plain_marks(const Workspace &w, int64_t n_bins, int stamp)
     mk.scan_stamp = w.scan_stamp; mk.scan_tiles = scan_tiles_per_row(n_bins);
     mk.blk_stamp = nullptr; mk.n_dblk = 0; mk.dblk_log2 = 0; mk.med_h = 0;
     mk.stamp = stamp;
+    mk.live_sums = nullptr;
     return mk;
 }
 
@@ -414,6 +418,7 @@ static int loop_init_workspace(const Workspace &w, int64_t nb, int n_cat, cudaSt
     GBFG_CUDA(cudaMemsetAsync(w.wide_flag, 0, sizeof(int) * (size_t)(1 + n_cat), st));
     GBFG_CUDA(cudaMemsetAsync(w.counters, 0, sizeof(int64_t) * WS_COUNTERS, st));
     GBFG_CUDA(cudaMemsetAsync(w.scan_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)scan_tiles_per_row(nb), st));
+    GBFG_CUDA(cudaMemsetAsync(w.live_sums[0], 0, 2 * align_up(sizeof(int64_t) * (size_t)n_cat * (size_t)scan_tiles_per_row(nb)), st));
     GBFG_CUDA(cudaMemsetAsync(w.blk_stamp, 0, sizeof(int) * (size_t)n_cat * (size_t)w.plan.n_dblk, st));
     return GBFG_OK;
 }
@@ -545,6 +550,9 @@ static int loop_body(const gbfg_grid *grid, const double *dev_A, const double *d
         // The test subtracts what it selects on the spot (stage v, eq. D4) and stamps the blocks that become dirty.
         DepositMarks mk = plain_marks(w, nb, it + 1);
         mk.blk_stamp = w.blk_stamp; mk.n_dblk = w.plan.n_dblk; mk.dblk_log2 = w.plan.dblk_log2; mk.med_h = W / 2;
+        // the test keeps the sums of the range updates' tiles itself (two buffers: the plan behind this iteration's test
+        // clears the one the next test will add into, which the scan before last was the last to read)
+        mk.live_sums = w.live_sums[it & 1];
         const SubtractView sub = {dev_spectrum, w.diff, w.wide_flag, mk, grid->scale_log2};
         rc = launch_snr_cand(nb, n_cat, dev_psd, params->rho_th, dev_resolved, nullptr, n_cand, w.sel_idx, sel_count,
                              near, 1, preselect ? neg_flag : nullptr, true, w.sw, dirty, snr_tests, &sub, delta, psd_rtol, st);
@@ -567,7 +575,8 @@ static int loop_body(const gbfg_grid *grid, const double *dev_A, const double *d
         {
             const bool closing = it + 1 == params->max_iter;
             static thread_local int64_t seq_counter = 0;
-            const PlanPublish pub = {w.counters, host, (int)n_read_all, HOST_SEQ_AT, ++seq_counter};
+            const PlanPublish pub = {w.counters, host, (int)n_read_all, HOST_SEQ_AT, ++seq_counter, w.live_sums[(it + 1) & 1],
+                                     n_cat * scan_tiles_per_row(nb)};
             GBFG_CUDA(cudaStreamWaitEvent(side->s, ev_read, 0));
             rc = launch_plan(w.blk_stamp, it + 1, !incremental, nb, n_cat, W, w.plan, closing ? nullptr : w.counters,
                              closing ? 0 : (int)n_iter_counters, med_outputs,

@@ -86,6 +86,8 @@ struct PlanArgs {
 #ifdef PLAN_TIMING
     long long *dbg;         // probe builds only: clocks per phase, summed over launches, [16]
 #endif
+    int64_t *zero_sums;     // nullable: cleared here (PlanPublish)
+    int zero_sums_n;
     int *near_fold;         // SnrWork::any_near (nullable): a near-threshold flag raised by the last test (word 1) becomes
                             // visible to the next one (word 0) here, between the two launches
 };
@@ -155,6 +157,7 @@ plan_kernel(PlanArgs a)
         }
     }
     PLAN_TICK(1);
+    if (row == 0 && a.zero_sums) for (int i = tid; i < a.zero_sums_n; i += PLAN_THREADS) a.zero_sums[i] = 0;
 #pragma unroll
     for (int u = 0; u < PLAN_LOADS; ++u) {
         const int b = u * PLAN_THREADS + tid;
@@ -299,6 +302,7 @@ int launch_plan(const int *blk_stamp, int stamp, bool all_dirty, int64_t n_bins,
     PlanArgs a;
     if (pub) { a.pub_src = pub->src; a.pub_dst = pub->dst; a.pub_n = pub->n; a.pub_flag_at = pub->flag_at; a.pub_seq = pub->seq; }
     else { a.pub_src = nullptr; a.pub_dst = nullptr; a.pub_n = 0; a.pub_flag_at = 0; a.pub_seq = 0; }
+    a.zero_sums = pub ? pub->zero_sums : nullptr; a.zero_sums_n = pub ? pub->zero_sums_n : 0;
 #ifdef PLAN_TIMING
     a.dbg = plan_timing_words();
 #endif

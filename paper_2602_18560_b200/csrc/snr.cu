@@ -578,11 +578,15 @@ snr_cand_kernel(SnrArgs a)
                 if (w <= DEP_NARROW) {
                     for (int k = 0; k < w; ++k) atomic_add_i64(a.sub.spectrum + gk0 + k, -q);
                 } else {
+                    const int64_t t_lo = (int64_t)cat * mk.scan_tiles + k0 / DEP_SCAN_TILE;
                     atomic_add_i64(a.sub.diff + gk0, -q);
-                    mk.scan_stamp[(int64_t)cat * mk.scan_tiles + k0 / DEP_SCAN_TILE] = mk.stamp;
+                    mk.scan_stamp[t_lo] = mk.stamp;
+                    if (mk.live_sums) atomic_add_i64(mk.live_sums + t_lo, -q);
                     if (k0 + w < a.n_bins) {
+                        const int64_t t_hi = (int64_t)cat * mk.scan_tiles + (k0 + w) / DEP_SCAN_TILE;
                         atomic_add_i64(a.sub.diff + gk0 + w, q);
-                        mk.scan_stamp[(int64_t)cat * mk.scan_tiles + (k0 + w) / DEP_SCAN_TILE] = mk.stamp;
+                        mk.scan_stamp[t_hi] = mk.stamp;
+                        if (mk.live_sums) atomic_add_i64(mk.live_sums + t_hi, q);
                     }
                     *a.sub.wide_flag = mk.stamp;
                 }
