@@ -545,8 +545,13 @@ running_median_tile_kernel(MedianArgs a)
                 if (lane ? (jlo >= n_out) : !next_needed) t = 0;
                 __syncwarp();
                 int r = m0;
+                // the word the lane's answer lies in, and which of its bits (from below or from above) it is; the bit itself
+                // is picked once for the whole warp behind the loop (inside it, lanes that end in different rounds would
+                // each run the search on their own)
+                unsigned w_fin = 1u;
+                int t_fin = 1, wi = m0 >> 5;
+                bool moved = false;
                 if (t > 0) {
-                    int wi = m0 >> 5;
                     const int step = up ? 1 : -1;
                     // the first word: only the ranks beyond m0
                     unsigned keep = up ? ~((2u << (m0 & 31)) - 1u) : ((1u << (m0 & 31)) - 1u);
@@ -559,17 +564,17 @@ running_median_tile_kernel(MedianArgs a)
                             if ((unsigned)(pos - jlo) >= (unsigned)W) wb &= ~(1u << b);
                         }
                         const int pc = __popc(wb);
-                        if (t <= pc) {
-                            // the t-th set bit from below (up) or from above (down): one search, on the word or its mirror image
-                            const int at = nth_set_bit(up ? wb : __brev(wb), t);
-                            r = (wi << 5) + (up ? at : 31 - at);
-                            break;
-                        }
+                        if (t <= pc) { w_fin = wb; t_fin = t; moved = true; break; }
                         t -= pc;
                         wi += step;
                         keep = 0xffffffffu;
                         if ((unsigned)wi >= (unsigned)nw) break;               // not reachable: the window holds the element
                     }
+                }
+                {
+                    // the t-th set bit from below (up) or from above (down): one search, on the word or its mirror image
+                    const int at = nth_set_bit(up ? w_fin : __brev(w_fin), t_fin);
+                    if (moved) r = (wi << 5) + (up ? at : 31 - at);
                 }
                 if (own) {                                   // median and PSD of output j0 + lane, 256 bytes per warp and array
                     const int at = lane ? r : m0;
