@@ -443,7 +443,10 @@ running_median_tile_kernel(MedianArgs a)
         unsigned *bm = aux32 + warp * BMW;
         unsigned *sp = aux32 + (WARPS + warp) * BMW;
         const int nw = LTe / 32;
-        const uint32_t bm_a = (uint32_t)__cvta_generic_to_shared(bm);
+        // (kept opaque to the compiler: it would otherwise work the address out again from the CTA's shared window and the
+        // warp index in every round of the walk, nine instructions, rather than hold it in a register)
+        uint32_t bm_a = (uint32_t)__cvta_generic_to_shared(bm);
+        asm volatile("" : "+r"(bm_a));
         {
             // Position p lies in the first window of warp w2 iff w2 wstep <= p < w2 wstep + W (wstep = the outputs of a
             // warp): a range of w2, i.e. a mask of at most 32 bits per lane.  What warp w2 needs is the transposed thing,
@@ -505,7 +508,8 @@ running_median_tile_kernel(MedianArgs a)
             }
             MED_TICK(5);
             // the arrays as 32-bit shared addresses: skey at 0, spos, rop, then the bitmaps (sp of a warp SP_D behind its bm)
-            const uint32_t sm0 = (uint32_t)__cvta_generic_to_shared(smem_raw);
+            uint32_t sm0 = (uint32_t)__cvta_generic_to_shared(smem_raw);
+            asm volatile("" : "+r"(sm0));
             constexpr uint32_t SPOS_A = sizeof(KeyT) * LT, ROP_A = SPOS_A + 2u * LT, SP_D = 4u * WARPS * BMW;
             int64_t *const med_row = a.med + row + o0;           // output j of the tile: med_row[j]
             double *const psd_row = a.psd ? a.psd + row + o0 : nullptr;
