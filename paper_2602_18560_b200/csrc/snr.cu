@@ -382,10 +382,21 @@ cand_bucket_scan_kernel(int *__restrict__ bkt_count, int *__restrict__ bkt_ext, 
     int *cnt = bkt_count + (int64_t)row * n_dblk;
     int *ext = bkt_ext + (int64_t)row * n_dblk;
     int64_t *off = bkt_off + (int64_t)row * (n_dblk + 1);
+    // a thread's buckets (at most 16: n_dblk <= DIRTY_MAX_BLOCKS) are read once, all loads in flight together; the two
+    // loops over them used to be chains of 15 dependent round trips each
+    constexpr int PER_MAX = DIRTY_MAX_BLOCKS / BKT_THREADS;
     const int per = (n_dblk + BKT_THREADS - 1) / BKT_THREADS;
     const int b_lo = min(tid * per, n_dblk), b_hi = min(b_lo + per, n_dblk);
+    int c_[PER_MAX], e_[PER_MAX];
+#pragma unroll
+    for (int u = 0; u < PER_MAX; ++u) {
+        const int b = b_lo + u;
+        c_[u] = b < b_hi ? cnt[b] : 0;
+        e_[u] = b < b_hi ? ext[b] : -1;
+    }
     int s = 0, m = -1;
-    for (int b = b_lo; b < b_hi; ++b) { s += cnt[b]; m = max(m, cnt[b] ? ext[b] : -1); }
+#pragma unroll
+    for (int u = 0; u < PER_MAX; ++u) { s += c_[u]; if (c_[u]) m = max(m, e_[u]); }
     int incl = s, imax = m;
     for (int o = 1; o < 32; o <<= 1) {
         const int us = __shfl_up_sync(0xffffffffu, incl, o), um = __shfl_up_sync(0xffffffffu, imax, o);
@@ -397,13 +408,16 @@ cand_bucket_scan_kernel(int *__restrict__ bkt_count, int *__restrict__ bkt_ext, 
     int pm = __shfl_up_sync(0xffffffffu, imax, 1);
     if (lane == 0) pm = -1;
     for (int w = 0; w < warp; ++w) { run += wsum[w]; pm = max(pm, wmax[w]); }
-    for (int b = b_lo; b < b_hi; ++b) {
-        const int c = cnt[b];
-        off[b] = base + run;
-        cnt[b] = 0;                                    // becomes the scatter cursor (relative to off[b])
-        if (c) pm = max(pm, ext[b]);
-        ext[b] = pm;
-        run += c;
+#pragma unroll
+    for (int u = 0; u < PER_MAX; ++u) {
+        const int b = b_lo + u;
+        if (b < b_hi) {
+            off[b] = base + run;
+            cnt[b] = 0;                                // becomes the scatter cursor (relative to off[b])
+            if (c_[u]) pm = max(pm, e_[u]);
+            ext[b] = pm;
+            run += c_[u];
+        }
     }
     if (tid == BKT_THREADS - 1) off[n_dblk] = base + run;
 }
