@@ -117,6 +117,15 @@ def test_invalid_arguments_are_rejected_before_any_cuda_call(gbcpu):
     assert L.gbfg_deposit(C.byref(g), 8, 8, 8, off, 1, None, None, 1, 8, None, 64, 1 << 40, None) != -2
 
 
+def test_profile_timeline_rejects_bad_arguments(gbcpu):
+    L = gbcpu.load()
+    n = C.c_int32(0)
+    assert L.gbfg_profile_timeline(None, 4, C.byref(n), C.byref(n)) == -1
+    buf = (gbcpu.LaunchTime * 4)()
+    assert L.gbfg_profile_timeline(buf, -1, C.byref(n), C.byref(n)) == -1
+    assert L.gbfg_profile_timeline(buf, 4, None, C.byref(n)) == -1
+
+
 def test_paper_sampler_rejects_parameters_outside_the_stated_domain(gbcpu):
     """DESIGN.md R12: the special functions of the paper's sampler are stated and pinned for 0.25 <= alpha_Gamma <= 16."""
     L = gbcpu.load()

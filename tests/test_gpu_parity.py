@@ -1360,3 +1360,47 @@ def test_simulate_paper_population_to_coarse_grained_psd(gb, orc, torch, estimat
         assert np.allclose(S[c].cpu().numpy(), S_ref, rtol=COARSE_RTOL, atol=0, equal_nan=True)
         assert np.allclose(hc[c].cpu().numpy(), hc_ref, rtol=COARSE_RTOL, atol=0, equal_nan=True)
         assert np.allclose(fk.cpu().numpy(), f_ref, rtol=1e-15, atol=0, equal_nan=True)
+
+
+# ------------------------------------------------------------------------- measurement helpers
+def test_profile_read_and_timeline_agree(gb, torch):
+    """gbfg_profile_read (time per kernel class) and gbfg_profile_timeline (launch by launch) describe the same record:
+    the same launches per class, the same summed time, starts and ends in order; and a call made with the helper off
+    leaves no record."""
+    w = wl.config(0)
+    g = gpu_grid(gb, w)
+    n, nb = w.n_src_total, g.n_bins
+    s_instr = torch.empty(nb, dtype=torch.float64, device="cuda")
+    gb.instrument_noise(g, s_instr)
+    A, f, fd = (torch.empty(n, dtype=torch.float64, device="cuda") for _ in range(3))
+    total, spec, med = (torch.empty(nb, dtype=torch.int64, device="cuda") for _ in range(3))
+    psd = torch.empty(nb, dtype=torch.float64, device="cuda")
+    resolved = torch.empty(n, dtype=torch.uint8, device="cuda")
+    ws = workspace(torch, gb, g, n)
+    params = gb.make_iter_params(w.window, w.median_norm, w.rho_th, w.max_iter)
+
+    def run():
+        gb.simulate(g, w.pops, w.offsets(), w.seed, s_instr, params, A, f, fd, total, spec, med, psd, resolved, ws)
+        torch.cuda.synchronize()
+
+    run()
+    gb.profile_enable(True)
+    before = gb.kernel_launch_count()
+    run()
+    launched = gb.kernel_launch_count() - before
+    tl = gb.profile_timeline()
+    per_class = gb.profile_read()                        # clears the record
+    gb.profile_enable(False)
+    assert len(tl) > 0 and tl[0][1] == 0.0
+    assert all(b >= a >= 0.0 for _, a, b in tl)
+    assert sum(v[0] for v in per_class.values()) == len(tl) <= launched      # (a timer may bracket several launches)
+    for k, (cnt, total_ms, max_ms) in per_class.items():
+        mine = [b - a for kk, a, b in tl if kk == k]
+        assert len(mine) == cnt
+        if cnt:
+            assert abs(sum(mine) - total_ms) <= 1e-3 * max(total_ms, 1e-3) + 1e-3 and abs(max(mine) - max_ms) <= 1e-3
+    run()                                                # helper off: nothing recorded
+    gb.profile_enable(True)
+    assert gb.profile_timeline() == []
+    gb.profile_enable(False)
+
